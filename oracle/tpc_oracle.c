@@ -1,0 +1,673 @@
+/*
+ * oracle/tpc_oracle.c -- CPU ORACLE of the TPC sector tracker.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * build, load or call this file.  It shares no code, header, table or helper with the CUDA
+ * path (paper_1709_00618_b200/csrc, include/); neither side includes the other.
+ *
+ * What it computes: the sector tracker of /root/reference/PAPER.md:25 (section 2, "Online
+ * Tracking in ALICE"), stage by stage, in the paper's order:
+ *   S1 grid (acceleration only)           -- not in the paper; BASELINE.json north_star
+ *   S2 neighbour finding ("forming links of adjacent hits arranged close to a straight line")
+ *   S3 neighbour cleaning (mutual links)  -- north_star
+ *   S4 start hits + concatenation ("concatenating links", candidates "of usually 4 to 10 hits")
+ *   S5 track following ("fits track parameters to the track candidate and extrapolates the
+ *      trajectory through the TPC sector volume to pick up additional clusters and refine the
+ *      fit using a simplified Kalman filter"); pure Bz
+ *   S6 selection ("selection of good tracks and final assignment of clusters to tracks
+ *      dissolving ambiguities")
+ * The paper gives no formula for any stage; every formula below is the reading fixed in
+ * SURVEY.md section 8(c) and restated in DESIGN.md ("Readings").  The method is a heuristic
+ * pipeline, so the oracle is the algorithm written out step by step, in plain loops.
+ *
+ * Arithmetic: S2 and the S5 pick-up test are fp32 with every operation individually rounded
+ * (compile with -ffp-contract=off, no -ffast-math); the Kalman filter is fp64.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): grid search == brute force; noise-free straight
+ * and helical tracks link to their own neighbours and are recovered with all hits; cleaning and
+ * chain invariants; Jacobian == central finite differences; forward+backward transport is the
+ * identity; Bz->0 limit is the straight line; zero-smear fits reproduce the generating helix to
+ * 1e-6; pulls ~ N(0,1) and chi2/ndf ~ 1; a one-shot weighted least-squares fit (numpy) equals
+ * the filter result.  Parity unpinned: the absolute values of the tuning constants (window sizes,
+ * D2 cut, gate, gap, selector threshold) -- the paper gives none (readings A3,A4,A9,A11).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct {
+    int32_t n_rows;
+    const float *row_x;          /* [n_rows] */
+    int32_t sectors_per_event;   /* 36: instance i is sector i % 36; sector >= 18 is the z<0 side */
+    float half_angle_rad;
+    float z_lo, z_hi;            /* z range of the z>=0 side; mirrored for the z<0 side */
+    float sigma_y, sigma_z;
+    float nf_win_y, nf_win_z, nf_d2_max;
+    int32_t cand_min_hits, cand_max_hits;
+    double kf_p0[5];
+    double kf_gate_sigma, kf_win_max;
+    int32_t kf_max_gap;
+    double kf_max_sinphi, kf_edge_margin;
+    int32_t sel_min_hits;
+    float grid_cell_y, grid_cell_z;
+    double bz;
+} orc_config;
+
+typedef struct {               /* one tracklet (S5 output) */
+    int32_t ok;                /* 0: candidate produced no tracklet */
+    int32_t nhits, first_row, last_row, ref_row;
+    double p[5];
+    double cov[15];            /* lower triangle, row-major: (0,0),(1,0),(1,1),(2,0),... */
+    double chi2;
+} orc_tracklet;
+
+#define KAPPA_PER_TESLA 0.00299792458
+
+static double curv_const(const orc_config *c) { return -KAPPA_PER_TESLA * c->bz; }
+
+/* ------------------------------------------------------------------ S1: grid (acceleration) */
+
+typedef struct {
+    int ny, nz;
+    float y0, z0, inv_cy, inv_cz;
+    int32_t *bin_start;  /* [ny*nz+1] */
+    int32_t *perm;       /* [n] local indices sorted by bin, stable */
+    int n;
+} orc_rowgrid;
+
+static int grid_bin1(float v, float origin, float inv, int n) {
+    int b = (int)floorf((v - origin) * inv);
+    if (b < 0) b = 0;
+    if (b > n - 1) b = n - 1;
+    return b;
+}
+
+/* origin y0 = -y_max(r) - 1 cm, z0 = z_lo (mirrored for z<0 sectors), bin id = bz*ny + by. */
+static void grid_build(orc_rowgrid *g, const orc_config *c, int inst, int row, const float *cl, int n) {
+    double ymax = (double)c->row_x[row] * tan((double)c->half_angle_rad);
+    int side_c = (inst % c->sectors_per_event) >= c->sectors_per_event / 2;
+    float zlo = side_c ? -c->z_hi : c->z_lo, zhi = side_c ? -c->z_lo : c->z_hi;
+    g->y0 = (float)(-ymax - 1.0);
+    g->z0 = zlo;
+    g->inv_cy = 1.0f / c->grid_cell_y;
+    g->inv_cz = 1.0f / c->grid_cell_z;
+    g->ny = (int)ceil((2.0 * ymax + 2.0) / c->grid_cell_y);
+    g->nz = (int)ceil(((double)zhi - (double)zlo) / c->grid_cell_z);
+    if (g->ny < 1) g->ny = 1;
+    if (g->nz < 1) g->nz = 1;
+    g->n = n;
+    int nb = g->ny * g->nz;
+    g->bin_start = (int32_t *)calloc((size_t)nb + 1, sizeof(int32_t));
+    g->perm = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    int32_t *bins = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    for (int i = 0; i < n; i++) {
+        int by = grid_bin1(cl[4 * i + 1], g->y0, g->inv_cy, g->ny);
+        int bz = grid_bin1(cl[4 * i + 2], g->z0, g->inv_cz, g->nz);
+        bins[i] = bz * g->ny + by;
+        g->bin_start[bins[i] + 1]++;
+    }
+    for (int b = 0; b < nb; b++) g->bin_start[b + 1] += g->bin_start[b];
+    int32_t *fill = (int32_t *)malloc(sizeof(int32_t) * (size_t)nb);
+    memcpy(fill, g->bin_start, sizeof(int32_t) * (size_t)nb);
+    for (int i = 0; i < n; i++) g->perm[fill[bins[i]]++] = i;
+    free(fill);
+    free(bins);
+}
+
+static void grid_free(orc_rowgrid *g) {
+    free(g->bin_start);
+    free(g->perm);
+    g->bin_start = NULL;
+    g->perm = NULL;
+}
+
+/* ------------------------------------------------------------------ S2: neighbour finder */
+
+/* SURVEY 8(c) S2.  cl_* point at the first cluster (x,y,z,w) of rows r-1, r, r+1; indices written are
+ * LOCAL to the rows (position within the row segment of the input array), -1 if none.
+ * use_grid = 0: brute force over all (u,d); 1: visit only bins overlapping the window.  Both apply the
+ * identical exact tests, so they must agree bit for bit (pin: tests/test_oracle_ca.py). */
+static void neighbours_row(const orc_config *c, const float *cl_dn, int n_dn, const float *cl_r, int n_r,
+                           const float *cl_up, int n_up, const orc_rowgrid *g_dn, const orc_rowgrid *g_up,
+                           int use_grid, int32_t *up_loc, int32_t *dn_loc) {
+    const float WY = c->nf_win_y, WZ = c->nf_win_z, D2MAX = c->nf_d2_max;
+    int32_t *ulist = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_up + 1));
+    int32_t *dlist = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_dn + 1));
+    for (int h = 0; h < n_r; h++) {
+        const float y = cl_r[4 * h + 1], z = cl_r[4 * h + 2];
+        const float ylo = y - WY, yhi = y + WY, zlo = z - WZ, zhi = z + WZ;
+        int nu = 0, nd = 0;
+        for (int pass = 0; pass < 2; pass++) {
+            const float *cl = pass ? cl_dn : cl_up;
+            int n = pass ? n_dn : n_up;
+            const orc_rowgrid *g = pass ? g_dn : g_up;
+            int32_t *list = pass ? dlist : ulist;
+            int cnt = 0;
+            if (!use_grid) {
+                for (int j = 0; j < n; j++) {
+                    float yj = cl[4 * j + 1], zj = cl[4 * j + 2];
+                    if (ylo <= yj && yj <= yhi && zlo <= zj && zj <= zhi) list[cnt++] = j;
+                }
+            } else if (n > 0) {
+                int by0 = grid_bin1(ylo, g->y0, g->inv_cy, g->ny), by1 = grid_bin1(yhi, g->y0, g->inv_cy, g->ny);
+                int bz0 = grid_bin1(zlo, g->z0, g->inv_cz, g->nz), bz1 = grid_bin1(zhi, g->z0, g->inv_cz, g->nz);
+                for (int bz = bz0; bz <= bz1; bz++)
+                    for (int k = g->bin_start[bz * g->ny + by0]; k < g->bin_start[bz * g->ny + by1 + 1]; k++) {
+                        int j = g->perm[k];
+                        float yj = cl[4 * j + 1], zj = cl[4 * j + 2];
+                        if (ylo <= yj && yj <= yhi && zlo <= zj && zj <= zhi) list[cnt++] = j;
+                    }
+            }
+            if (pass) nd = cnt; else nu = cnt;
+        }
+        /* minimum over (D, u, d) lexicographically: independent of the visiting order */
+        int bu = -1, bd = -1;
+        float bD = 0.0f;
+        for (int a = 0; a < nu; a++)
+            for (int b = 0; b < nd; b++) {
+                int u = ulist[a], d = dlist[b];
+                float t1 = cl_up[4 * u + 1] - y, t2 = y - cl_dn[4 * d + 1], ey = t1 - t2;
+                float t3 = cl_up[4 * u + 2] - z, t4 = z - cl_dn[4 * d + 2], ez = t3 - t4;
+                float pyy = ey * ey, pzz = ez * ez;
+                float D = pyy + pzz;
+                if (!(D <= D2MAX)) continue;
+                if (bu < 0 || D < bD || (D == bD && (u < bu || (u == bu && d < bd)))) {
+                    bD = D; bu = u; bd = d;
+                }
+            }
+        up_loc[h] = bu;
+        dn_loc[h] = bd;
+    }
+    free(ulist);
+    free(dlist);
+}
+
+/* Raw links for all instances.  link_up/link_dn: [n_clusters] GLOBAL cluster indices or -1. */
+int orc_neighbours(const orc_config *c, const float *clusters, const int32_t *row_offsets, int32_t n_inst,
+                   int32_t use_grid, int32_t *link_up, int32_t *link_dn) {
+    const int R = c->n_rows;
+    for (int inst = 0; inst < n_inst; inst++) {
+        const int32_t *ro = row_offsets + (size_t)inst * R;
+        orc_rowgrid *grids = (orc_rowgrid *)calloc((size_t)R, sizeof(orc_rowgrid));
+        if (use_grid)
+            for (int r = 0; r < R; r++) grid_build(&grids[r], c, inst, r, clusters + 4 * (size_t)ro[r], ro[r + 1] - ro[r]);
+        for (int r = 0; r < R; r++) {
+            int n_r = ro[r + 1] - ro[r];
+            if (r == 0 || r == R - 1) {
+                for (int h = 0; h < n_r; h++) link_up[ro[r] + h] = link_dn[ro[r] + h] = -1;
+                continue;
+            }
+            int n_dn = ro[r] - ro[r - 1], n_up = ro[r + 2] - ro[r + 1];
+            int32_t *ul = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_r + 1));
+            int32_t *dl = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_r + 1));
+            neighbours_row(c, clusters + 4 * (size_t)ro[r - 1], n_dn, clusters + 4 * (size_t)ro[r], n_r,
+                           clusters + 4 * (size_t)ro[r + 1], n_up, &grids[r - 1], &grids[r + 1], use_grid, ul, dl);
+            for (int h = 0; h < n_r; h++) {
+                link_up[ro[r] + h] = ul[h] < 0 ? -1 : ro[r + 1] + ul[h];
+                link_dn[ro[r] + h] = dl[h] < 0 ? -1 : ro[r - 1] + dl[h];
+            }
+            free(ul);
+            free(dl);
+        }
+        if (use_grid)
+            for (int r = 0; r < R; r++) grid_free(&grids[r]);
+        free(grids);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ S3: cleaning */
+
+/* keep up[h]=u iff dn[u]==h; keep dn[h]=d iff up[d]==h; from the raw arrays into new ones. */
+void orc_clean(int64_t n, const int32_t *up, const int32_t *dn, int32_t *cu, int32_t *cd) {
+    for (int64_t h = 0; h < n; h++) {
+        cu[h] = (up[h] >= 0 && dn[up[h]] == h) ? up[h] : -1;
+        cd[h] = (dn[h] >= 0 && up[dn[h]] == h) ? dn[h] : -1;
+    }
+}
+
+/* ------------------------------------------------------------------ S4: start hits, candidates */
+
+/* SURVEY 8(c) S4.  start hit: cu>=0 and cd<0; chain follows cu; candidate iff length >= cand_min; it keeps the
+ * first min(L,cand_max) hits.  Order = ascending global index of the start hit.  Returns the REQUIRED counts in
+ * n_out[0]=n_start, n_out[1]=n_cand even if the capacities are smaller (nothing is written beyond them). */
+void orc_candidates(const orc_config *c, int64_t n, const int32_t *cu, const int32_t *cd, int32_t *start_hits,
+                    int64_t start_cap, int32_t *cand_hits /*[cap][cand_max]*/, int32_t *cand_n, int64_t cand_cap,
+                    int64_t *n_out) {
+    int64_t ns = 0, nc = 0;
+    const int M = c->cand_max_hits;
+    for (int64_t h = 0; h < n; h++) {
+        if (!(cu[h] >= 0 && cd[h] < 0)) continue;
+        if (ns < start_cap) start_hits[ns] = (int32_t)h;
+        ns++;
+        int len = 0;
+        for (int32_t x = (int32_t)h; x >= 0; x = cu[x]) len++;
+        if (len < c->cand_min_hits) continue;
+        if (nc < cand_cap) {
+            int k = 0;
+            for (int32_t x = (int32_t)h; x >= 0 && k < M; x = cu[x]) cand_hits[nc * M + k++] = x;
+            cand_n[nc] = k;
+            for (; k < M; k++) cand_hits[nc * M + k] = -1;
+        }
+        nc++;
+    }
+    n_out[0] = ns;
+    n_out[1] = nc;
+}
+
+/* ------------------------------------------------------------------ S5: Kalman track following */
+
+/* arc length over chord ratio asin(a)/a */
+static double asin_over(double a) { return fabs(a) < 1e-8 ? 1.0 + a * a / 6.0 : asin(a) / a; }
+
+/* SURVEY 8(c) S5 "Transport by dx": exact helix for constant Bz (only Bz is respected).
+ * p = (y, z, sinphi, dz/ds, q/pt).  P is a full symmetric 5x5 (row-major).  F (row-major 5x5) may be NULL.
+ * Returns 0 on success, 1 if |sinphi| would exceed max_sinphi (outputs untouched). */
+int orc_transport(const double p[5], const double P[25], double dx, double cB, double max_sinphi, double p1[5],
+                  double P1[25], double F_out[25]) {
+    const double y = p[0], z = p[1], s = p[2], t = p[3], k = p[4];
+    const double kap = cB * k;
+    const double s1 = s + kap * dx;
+    if (fabs(s) > max_sinphi || fabs(s1) > max_sinphi) return 1;
+    const double c0 = sqrt(1.0 - s * s), c1 = sqrt(1.0 - s1 * s1);
+    const double tg = (s + s1) / (c0 + c1);
+    const double sec2 = 1.0 + tg * tg;
+    const double chord = dx * sqrt(sec2);
+    const double a = 0.5 * kap * chord;
+    const double dS = chord * asin_over(a);
+    double F[25];
+    for (int i = 0; i < 25; i++) F[i] = (i % 6 == 0) ? 1.0 : 0.0;
+    F[0 * 5 + 2] = dx * sec2 * 0.5 * (1.0 / c0 + 1.0 / c1);
+    F[0 * 5 + 4] = cB * dx * dx * sec2 / (2.0 * c1);
+    F[1 * 5 + 2] = t * dx * tg / (c0 * c1);
+    F[1 * 5 + 3] = dS;
+    /* d(dS)/d(kappa) = (dx/c1 - dS)/kappa exactly (dS = (asin s1 - asin s)/kappa).  For |kappa dx| < 1e-4 the
+     * difference cancels; there use its Taylor series 1/2 dx^2 g(s) + 1/3 kappa dx^3 g'(s) + ..., g = s/c^3, which to
+     * second order is 1/2 dx^2 g(s + 2/3 kappa dx) (relative error O((kappa dx)^2) < 1e-8). */
+    if (fabs(kap * dx) > 1e-4) {
+        F[1 * 5 + 4] = cB * t * (dx / c1 - dS) / kap;
+    } else {
+        const double se = s + (2.0 / 3.0) * kap * dx, ce = sqrt(1.0 - se * se);
+        F[1 * 5 + 4] = cB * t * 0.5 * dx * dx * se / (ce * ce * ce);
+    }
+    F[2 * 5 + 4] = cB * dx;
+    double FP[25], Pn[25];
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j < 5; j++) {
+            double acc = 0.0;
+            for (int m = 0; m < 5; m++) acc += F[i * 5 + m] * P[m * 5 + j];
+            FP[i * 5 + j] = acc;
+        }
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j < 5; j++) {
+            double acc = 0.0;
+            for (int m = 0; m < 5; m++) acc += FP[i * 5 + m] * F[j * 5 + m];
+            Pn[i * 5 + j] = acc;
+        }
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j < 5; j++) P1[i * 5 + j] = 0.5 * (Pn[i * 5 + j] + Pn[j * 5 + i]);
+    p1[0] = y + dx * tg;
+    p1[1] = z + t * dS;
+    p1[2] = s1;
+    p1[3] = t;
+    p1[4] = k;
+    if (F_out) memcpy(F_out, F, sizeof(F));
+    return 0;
+}
+
+/* SURVEY 8(c) S5 "Update": two sequential scalar updates (y with sigma_y^2, then z with sigma_z^2). In place.
+ * Returns the chi2 increment. */
+double orc_update(double p[5], double P[25], double ym, double zm, double sy2, double sz2) {
+    double chi2 = 0.0;
+    for (int i = 0; i < 2; i++) {
+        const double m = i ? zm : ym, r = i ? sz2 : sy2;
+        const double S = P[i * 5 + i] + r;
+        const double res = m - p[i];
+        double K[5], Pi[5];
+        for (int a = 0; a < 5; a++) { K[a] = P[a * 5 + i] / S; Pi[a] = P[i * 5 + a]; }
+        chi2 += res * res / S;
+        for (int a = 0; a < 5; a++) p[a] += K[a] * res;
+        for (int a = 0; a < 5; a++)
+            for (int b = 0; b < 5; b++) P[a * 5 + b] -= K[a] * Pi[b];
+        for (int a = 0; a < 5; a++)
+            for (int b = a + 1; b < 5; b++) {
+                double v = 0.5 * (P[a * 5 + b] + P[b * 5 + a]);
+                P[a * 5 + b] = P[b * 5 + a] = v;
+            }
+    }
+    return chi2;
+}
+
+/* SURVEY 8(c) S5 "Seed": circle through three points in (x,y), dz/ds from the end points. */
+void orc_seed(const double x[3], const double y[3], const double z[3], double cB, double p[5]) {
+    const double ax = x[1] - x[0], ay = y[1] - y[0], bx = x[2] - x[0], by = y[2] - y[0];
+    const double cross = ax * by - ay * bx;
+    const double d01 = sqrt(ax * ax + ay * ay), d02 = sqrt(bx * bx + by * by);
+    const double ex = x[2] - x[1], ey = y[2] - y[1];
+    const double d12 = sqrt(ex * ex + ey * ey);
+    const double kap = 2.0 * cross / (d01 * d02 * d12);
+    const double phi0 = atan2(ay, ax) - asin(0.5 * kap * d01);
+    const double S02 = d02 * asin_over(0.5 * kap * d02);
+    p[0] = y[0];
+    p[1] = z[0];
+    p[2] = sin(phi0);
+    p[3] = (z[2] - z[0]) / S02;
+    p[4] = cB != 0.0 ? kap / cB : 0.0;
+}
+
+static int row_of(const int32_t *ro, int R, int32_t h) { /* ro: this instance's row offsets [R+1] */
+    int lo = 0, hi = R; /* find r with ro[r] <= h < ro[r+1] */
+    while (hi - lo > 1) {
+        int mid = (lo + hi) / 2;
+        if (ro[mid] <= h) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+/* SURVEY 8(c) S5 pick-up: nearest cluster of the row inside the window; fp32 test on the fp32-rounded prediction;
+ * tie -> lowest local index.  Returns the local index or -1. */
+static int pickup(const float *cl, int n, const orc_rowgrid *g, double y_pred, double z_pred, double wy_d,
+                  double wz_d) {
+    const float yp = (float)y_pred, zp = (float)z_pred, wy = (float)wy_d, wz = (float)wz_d;
+    int best = -1;
+    float bd2 = 0.0f;
+    if (!g) {
+        for (int j = 0; j < n; j++) {
+            float dy = cl[4 * j + 1] - yp, dz = cl[4 * j + 2] - zp;
+            if (!(fabsf(dy) <= wy && fabsf(dz) <= wz)) continue;
+            float a = dy * dy, b = dz * dz, d2 = a + b;
+            if (best < 0 || d2 < bd2 || (d2 == bd2 && j < best)) { best = j; bd2 = d2; }
+        }
+        return best;
+    }
+    if (n == 0) return -1;
+    const float m = 1e-3f; /* bin margin: makes the visited bins a superset of the fp32 window test */
+    int by0 = grid_bin1(yp - wy - m, g->y0, g->inv_cy, g->ny), by1 = grid_bin1(yp + wy + m, g->y0, g->inv_cy, g->ny);
+    int bz0 = grid_bin1(zp - wz - m, g->z0, g->inv_cz, g->nz), bz1 = grid_bin1(zp + wz + m, g->z0, g->inv_cz, g->nz);
+    for (int bz = bz0; bz <= bz1; bz++)
+        for (int k = g->bin_start[bz * g->ny + by0]; k < g->bin_start[bz * g->ny + by1 + 1]; k++) {
+            int j = g->perm[k];
+            float dy = cl[4 * j + 1] - yp, dz = cl[4 * j + 2] - zp;
+            if (!(fabsf(dy) <= wy && fabsf(dz) <= wz)) continue;
+            float a = dy * dy, b = dz * dz, d2 = a + b;
+            if (best < 0 || d2 < bd2 || (d2 == bd2 && j < best)) { best = j; bd2 = d2; }
+        }
+    return best;
+}
+
+static void pack_cov(const double P[25], double c[15]) {
+    int k = 0;
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j <= i; j++) c[k++] = P[i * 5 + j];
+}
+
+/* One direction of the pick-up loop (SURVEY 8(c) S5 phases A and B).  step = +1 / -1.  (p,P) at row *r_cur. */
+static void follow_dir(const orc_config *c, const float *clusters, const int32_t *ro, const orc_rowgrid *grids,
+                       int step, double p[5], double P[25], int *r_cur, double *chi2, int32_t *hits /*[R]*/,
+                       int *nhits, int *last_hit_row, double p_at_hit[5], double P_at_hit[25]) {
+    const int R = c->n_rows;
+    const double cB = curv_const(c), sy2 = (double)c->sigma_y * c->sigma_y, sz2 = (double)c->sigma_z * c->sigma_z;
+    const double tanh_ = tan((double)c->half_angle_rad);
+    int gap = 0, r = *r_cur;
+    for (;;) {
+        int rn = r + step;
+        if (rn < 0 || rn >= R) break;
+        double p1[5], P1[25];
+        if (orc_transport(p, P, (double)c->row_x[rn] - (double)c->row_x[r], cB, c->kf_max_sinphi, p1, P1, NULL)) break;
+        memcpy(p, p1, sizeof(p1));
+        memcpy(P, P1, sizeof(P1));
+        r = rn;
+        if (fabs(p[0]) > (double)c->row_x[r] * tanh_ + c->kf_edge_margin) break;
+        double wy = c->kf_gate_sigma * sqrt(P[0] + sy2), wz = c->kf_gate_sigma * sqrt(P[6] + sz2);
+        if (wy > c->kf_win_max) wy = c->kf_win_max;
+        if (wz > c->kf_win_max) wz = c->kf_win_max;
+        int n = ro[r + 1] - ro[r];
+        int j = pickup(clusters + 4 * (size_t)ro[r], n, grids ? &grids[r] : NULL, p[0], p[1], wy, wz);
+        if (j >= 0) {
+            const float *h = clusters + 4 * (size_t)(ro[r] + j);
+            *chi2 += orc_update(p, P, (double)h[1], (double)h[2], sy2, sz2);
+            hits[r] = ro[r] + j;
+            (*nhits)++;
+            gap = 0;
+            *last_hit_row = r;
+            if (p_at_hit) { memcpy(p_at_hit, p, 5 * sizeof(double)); memcpy(P_at_hit, P, 25 * sizeof(double)); }
+        } else {
+            gap++;
+            if (gap > c->kf_max_gap) break;
+        }
+    }
+    *r_cur = r;
+}
+
+/* Follow one candidate (global hit indices, rows increasing).  ro = row offsets of ITS instance [R+1] (global
+ * indices).  grids: per-row grids of the instance or NULL for the linear scan.  hits: [R], filled with the global
+ * cluster index attached in each row or -1. */
+void orc_follow_one(const orc_config *c, const float *clusters, const int32_t *ro, const orc_rowgrid *grids,
+                    const int32_t *cand, int n, orc_tracklet *t, int32_t *hits) {
+    const int R = c->n_rows;
+    const double cB = curv_const(c), sy2 = (double)c->sigma_y * c->sigma_y, sz2 = (double)c->sigma_z * c->sigma_z;
+    memset(t, 0, sizeof(*t));
+    for (int r = 0; r < R; r++) hits[r] = -1;
+    int rows[64];
+    for (int i = 0; i < n; i++) rows[i] = row_of(ro, R, cand[i]);
+    const int ii[3] = {0, n / 2, n - 1};
+    double sx[3], sy[3], sz[3];
+    for (int m = 0; m < 3; m++) {
+        const float *h = clusters + 4 * (size_t)cand[ii[m]];
+        sx[m] = (double)c->row_x[rows[ii[m]]];
+        sy[m] = (double)h[1];
+        sz[m] = (double)h[2];
+    }
+    double p[5], P[25];
+    orc_seed(sx, sy, sz, cB, p);
+    if (!(fabs(p[2]) <= c->kf_max_sinphi)) return;
+    memset(P, 0, sizeof(P));
+    for (int i = 0; i < 5; i++) P[i * 5 + i] = c->kf_p0[i];
+    double chi2 = 0.0;
+    int nhits = 0, r = rows[0];
+    /* phase A: candidate hits, then upward pick-up */
+    for (int i = 0; i < n; i++) {
+        if (i > 0) {
+            double p1[5], P1[25];
+            if (orc_transport(p, P, (double)c->row_x[rows[i]] - (double)c->row_x[r], cB, c->kf_max_sinphi, p1, P1, NULL))
+                return;
+            memcpy(p, p1, sizeof(p1));
+            memcpy(P, P1, sizeof(P1));
+            r = rows[i];
+        }
+        const float *h = clusters + 4 * (size_t)cand[i];
+        chi2 += orc_update(p, P, (double)h[1], (double)h[2], sy2, sz2);
+        hits[r] = cand[i];
+        nhits++;
+    }
+    int last_row = r, dummy = r;
+    follow_dir(c, clusters, ro, grids, +1, p, P, &r, &chi2, hits, &nhits, &last_row, NULL, NULL);
+    /* phase B: one step back to the start row, no update there, then downward pick-up */
+    {
+        double p1[5], P1[25];
+        if (orc_transport(p, P, (double)c->row_x[rows[0]] - (double)c->row_x[r], cB, c->kf_max_sinphi, p1, P1, NULL))
+            return;
+        memcpy(p, p1, sizeof(p1));
+        memcpy(P, P1, sizeof(P1));
+        r = rows[0];
+    }
+    double pr[5], Pr[25];
+    memcpy(pr, p, sizeof(pr));
+    memcpy(Pr, P, sizeof(Pr));
+    int first_row = rows[0];
+    dummy = first_row;
+    follow_dir(c, clusters, ro, grids, -1, p, P, &r, &chi2, hits, &nhits, &dummy, pr, Pr);
+    first_row = dummy;
+    t->ok = 1;
+    t->nhits = nhits;
+    t->first_row = first_row;
+    t->last_row = last_row;
+    t->ref_row = first_row;
+    memcpy(t->p, pr, sizeof(pr));
+    pack_cov(Pr, t->cov);
+    t->chi2 = chi2;
+}
+
+/* Follow all candidates.  cand_hits [n_cand][cand_max] global indices.  tracklets [n_cand]; trk_hits [n_cand][R]. */
+int orc_follow(const orc_config *c, const float *clusters, const int32_t *row_offsets, int32_t n_inst,
+               const int32_t *cand_hits, const int32_t *cand_n, int64_t n_cand, int32_t use_grid,
+               orc_tracklet *tracklets, int32_t *trk_hits) {
+    const int R = c->n_rows, M = c->cand_max_hits;
+    int64_t ci = 0;
+    for (int inst = 0; inst < n_inst && ci < n_cand; inst++) {
+        const int32_t *ro = row_offsets + (size_t)inst * R;
+        if (!(cand_hits[ci * M] < ro[R])) continue;
+        orc_rowgrid *grids = NULL;
+        if (use_grid) {
+            grids = (orc_rowgrid *)calloc((size_t)R, sizeof(orc_rowgrid));
+            for (int r = 0; r < R; r++) grid_build(&grids[r], c, inst, r, clusters + 4 * (size_t)ro[r], ro[r + 1] - ro[r]);
+        }
+        for (; ci < n_cand && cand_hits[ci * M] < ro[R]; ci++)
+            orc_follow_one(c, clusters, ro, grids, cand_hits + ci * M, cand_n[ci], &tracklets[ci], trk_hits + ci * R);
+        if (use_grid) {
+            for (int r = 0; r < R; r++) grid_free(&grids[r]);
+            free(grids);
+        }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ S6: tracklet selector */
+
+/* SURVEY 8(c) S6.  weight = (nhits, -candidate id); every cluster goes to the claiming tracklet of maximal weight;
+ * a tracklet keeps the hits it owns and becomes a final track iff kept >= sel_min_hits; final tracks in ascending
+ * candidate id.  Outputs: cluster_owner [n_clusters] final track index or -1; trk_cand [n_tracks]; trk_hit_offset
+ * [n_tracks+1]; trk_hit_list (kept hits, rows increasing).  Returns the number of final tracks (required count;
+ * nothing is written beyond trk_cap / hits_cap).  n_out[0] = n_tracks, n_out[1] = total kept hits. */
+void orc_select(const orc_config *c, int64_t n_clusters, const orc_tracklet *tracklets, const int32_t *trk_hits,
+                int64_t n_cand, int32_t *cluster_owner, int32_t *trk_cand, int64_t *trk_hit_offset,
+                int32_t *trk_hit_list, int64_t trk_cap, int64_t hits_cap, int64_t *n_out) {
+    const int R = c->n_rows;
+    int32_t *best = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_clusters > 0 ? n_clusters : 1));
+    for (int64_t h = 0; h < n_clusters; h++) { best[h] = -1; cluster_owner[h] = -1; }
+    for (int64_t ci = 0; ci < n_cand; ci++) {
+        if (!tracklets[ci].ok) continue;
+        for (int r = 0; r < R; r++) {
+            int32_t h = trk_hits[ci * R + r];
+            if (h < 0) continue;
+            int32_t b = best[h];
+            /* ascending ci: an earlier claimant wins ties, so replace only on strictly more hits */
+            if (b < 0 || tracklets[ci].nhits > tracklets[b].nhits) best[h] = (int32_t)ci;
+        }
+    }
+    int64_t nt = 0, nh = 0;
+    for (int64_t ci = 0; ci < n_cand; ci++) {
+        if (!tracklets[ci].ok) continue;
+        int kept = 0;
+        for (int r = 0; r < R; r++) {
+            int32_t h = trk_hits[ci * R + r];
+            if (h >= 0 && best[h] == ci) kept++;
+        }
+        if (kept < c->sel_min_hits) continue;
+        if (nt < trk_cap) {
+            trk_cand[nt] = (int32_t)ci;
+            trk_hit_offset[nt] = nh;
+        }
+        for (int r = 0; r < R; r++) {
+            int32_t h = trk_hits[ci * R + r];
+            if (h >= 0 && best[h] == ci) {
+                if (nt < trk_cap) cluster_owner[h] = (int32_t)nt;
+                if (nh < hits_cap && nt < trk_cap) trk_hit_list[nh] = h;
+                nh++;
+            }
+        }
+        nt++;
+    }
+    if (nt <= trk_cap) trk_hit_offset[nt] = nh;
+    n_out[0] = nt;
+    n_out[1] = nh;
+    free(best);
+}
+
+/* ------------------------------------------------------------------ whole chain, per instance (for timing) */
+
+/* Runs S1-S6 on every instance independently (optionally one OpenMP thread per instance) and reports only the
+ * totals: n_out = {n_start, n_cand, n_tracklets, n_tracks, n_track_hits}.  Used by bench.py's cpu_baseline leg:
+ * it executes exactly the stage functions above, instance by instance. */
+int orc_track_count(const orc_config *c, const float *clusters, const int32_t *row_offsets, int32_t n_inst,
+                    int32_t n_threads, int64_t *n_out) {
+    const int R = c->n_rows, M = c->cand_max_hits;
+    int64_t tot[5] = {0, 0, 0, 0, 0};
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 1) num_threads(n_threads > 0 ? n_threads : 1)
+#endif
+    for (int inst = 0; inst < n_inst; inst++) {
+        const int32_t *ro = row_offsets + (size_t)inst * R;
+        const int32_t base = ro[0];
+        const int64_t n = ro[R] - base;
+        /* re-base this instance to local indices so that the stage functions see a one-instance problem */
+        int32_t *lro = (int32_t *)malloc(sizeof(int32_t) * (size_t)(R + 1));
+        for (int r = 0; r <= R; r++) lro[r] = ro[r] - base;
+        const float *cl = clusters + 4 * (size_t)base;
+        size_t nn = (size_t)(n > 0 ? n : 1);
+        int32_t *up = (int32_t *)malloc(sizeof(int32_t) * nn), *dn = (int32_t *)malloc(sizeof(int32_t) * nn);
+        int32_t *cu = (int32_t *)malloc(sizeof(int32_t) * nn), *cd = (int32_t *)malloc(sizeof(int32_t) * nn);
+        orc_config ci = *c;
+        /* the instance's side (z>=0 / z<0) must survive the re-basing: keep inst % sectors_per_event */
+        int32_t *ro1 = lro;
+        /* orc_neighbours derives the side from the instance index; emulate by calling the per-row code directly */
+        {
+            orc_rowgrid *grids = (orc_rowgrid *)calloc((size_t)R, sizeof(orc_rowgrid));
+            for (int r = 0; r < R; r++) grid_build(&grids[r], &ci, inst, r, cl + 4 * (size_t)ro1[r], ro1[r + 1] - ro1[r]);
+            for (int r = 0; r < R; r++) {
+                int n_r = ro1[r + 1] - ro1[r];
+                if (r == 0 || r == R - 1) {
+                    for (int h = 0; h < n_r; h++) up[ro1[r] + h] = dn[ro1[r] + h] = -1;
+                    continue;
+                }
+                int32_t *ul = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_r + 1));
+                int32_t *dl = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_r + 1));
+                neighbours_row(&ci, cl + 4 * (size_t)ro1[r - 1], ro1[r] - ro1[r - 1], cl + 4 * (size_t)ro1[r], n_r,
+                               cl + 4 * (size_t)ro1[r + 1], ro1[r + 2] - ro1[r + 1], &grids[r - 1], &grids[r + 1], 1, ul, dl);
+                for (int h = 0; h < n_r; h++) {
+                    up[ro1[r] + h] = ul[h] < 0 ? -1 : ro1[r + 1] + ul[h];
+                    dn[ro1[r] + h] = dl[h] < 0 ? -1 : ro1[r - 1] + dl[h];
+                }
+                free(ul);
+                free(dl);
+            }
+            orc_clean(n, up, dn, cu, cd);
+            int64_t cnt[2];
+            orc_candidates(&ci, n, cu, cd, NULL, 0, NULL, NULL, 0, cnt);
+            int64_t nc = cnt[1];
+            int32_t *ch = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nc * M + 1));
+            int32_t *cn = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nc + 1));
+            int32_t *sh = (int32_t *)malloc(sizeof(int32_t) * (size_t)(cnt[0] + 1));
+            orc_candidates(&ci, n, cu, cd, sh, cnt[0], ch, cn, nc, cnt);
+            orc_tracklet *tl = (orc_tracklet *)malloc(sizeof(orc_tracklet) * (size_t)(nc + 1));
+            int32_t *th = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nc * R + 1));
+            int64_t ntl = 0;
+            for (int64_t k = 0; k < nc; k++) {
+                orc_follow_one(&ci, cl, ro1, grids, ch + k * M, cn[k], &tl[k], th + k * R);
+                ntl += tl[k].ok;
+            }
+            int32_t *owner = (int32_t *)malloc(sizeof(int32_t) * nn);
+            int32_t *tc = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nc + 1));
+            int64_t *tho = (int64_t *)malloc(sizeof(int64_t) * (size_t)(nc + 2));
+            int32_t *thl = (int32_t *)malloc(sizeof(int32_t) * nn);
+            int64_t so[2];
+            orc_select(&ci, n, tl, th, nc, owner, tc, tho, thl, nc + 1, (int64_t)nn, so);
+#ifdef _OPENMP
+#pragma omp critical
+#endif
+            {
+                tot[0] += cnt[0]; tot[1] += nc; tot[2] += ntl; tot[3] += so[0]; tot[4] += so[1];
+            }
+            free(owner); free(tc); free(tho); free(thl); free(tl); free(th); free(ch); free(cn); free(sh);
+            for (int r = 0; r < R; r++) grid_free(&grids[r]);
+            free(grids);
+        }
+        free(up); free(dn); free(cu); free(cd); free(lro);
+    }
+    for (int i = 0; i < 5; i++) n_out[i] = tot[i];
+    return 0;
+}
+
+int32_t orc_sizeof_tracklet(void) { return (int32_t)sizeof(orc_tracklet); }
+int32_t orc_sizeof_config(void) { return (int32_t)sizeof(orc_config); }
