@@ -1,0 +1,157 @@
+/*
+ * tpc_tracker.h -- C ABI of the B200-native TPC sector tracker (libtpctrk.so).
+ *
+ * The operation: the "sector tracker" of /root/reference/PAPER.md:25 (section 2, "Online Tracking in
+ * ALICE"): for every TPC sector individually, a Cellular Automaton forms and concatenates links of
+ * adjacent hits close to a straight line into track candidates of 4 to 10 hits, the track following fits
+ * the candidate, extrapolates it through the sector and picks up further clusters with a simplified
+ * Kalman filter, and a selection step assigns clusters to tracks dissolving ambiguities.  Only Bz is
+ * respected.  The stage list and the parameterisation (y, z, sinPhi, dz/ds, q/pt) are
+ * those of BASELINE.json `north_star`; every constant and formula the paper leaves open is fixed in
+ * DESIGN.md ("Readings"), identically for this library and for the CPU oracle in oracle/.
+ *
+ * Conventions.  Units cm, Tesla, GeV/c.  A "sector instance" is one sector of one event (or drift
+ * window); instance i has geometric sector i % sectors_per_event, and sectors >= sectors_per_event/2
+ * are the z < 0 side.  Clusters are in the sector-local frame: x = pad-row plane, y along the pad row,
+ * z along the drift.  Everything is asynchronous on the stream given by tpc_set_stream; the library
+ * never allocates device memory and never synchronises inside tpc_track_sectors.
+ *
+ * All functions return 0 on success or a negative TPC_ERR_* code; tpc_last_error() gives the text.
+ * There is no CPU fallback: without a CUDA device every call that touches the device fails with
+ * TPC_ERR_CUDA.
+ */
+#ifndef TPC_TRACKER_H
+#define TPC_TRACKER_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TPC_OK 0
+#define TPC_ERR_ARG (-1)       /* NULL / negative / misaligned argument */
+#define TPC_ERR_GEOMETRY (-2)  /* n_rows out of [3,255], rows not strictly increasing or not uniformly spaced */
+#define TPC_ERR_WORKSPACE (-3) /* workspace missing or smaller than tpc_workspace_bytes() */
+#define TPC_ERR_CUDA (-4)      /* a CUDA runtime call failed (text in tpc_last_error) */
+#define TPC_ERR_CAPACITY (-5)  /* tpc_check_counts: an output buffer was too small (results were saturated) */
+#define TPC_ERR_INPUT (-6)     /* tpc_check_counts: device-side input validation failed (row too long, ...) */
+
+#define TPC_CAND_MAX_HITS 10   /* stride of cand_hits (reading A7: "usually 4 to 10 hits") */
+#define TPC_N_COUNTS 8
+
+typedef struct tpc_tracker tpc_tracker_t; /* opaque, library-owned */
+
+/* Tunables.  Any field left 0 takes the default of DESIGN.md "Readings" (given in the comments). */
+typedef struct {
+    float nf_win_y, nf_win_z;  /* S2 neighbour window half-sizes [cm]: 2.0, 2.5 */
+    float nf_d2_max;           /* S2 cut on the squared second difference [cm^2]: 1.0 */
+    int32_t cand_min_hits;     /* S4 minimum chain length: 4 */
+    int32_t cand_max_hits;     /* S4 hits kept per candidate: 10 (<= TPC_CAND_MAX_HITS) */
+    float kf_p0[5];            /* S5 initial covariance diagonal: 1, 1, 0.1, 0.1, 10 */
+    float kf_gate_sigma;       /* S5 pick-up gate in sigmas: 4 */
+    float kf_win_max;          /* S5 pick-up gate cap [cm]: 3 */
+    int32_t kf_max_gap;        /* S5 consecutive rows without a hit before stopping: 5 */
+    float kf_max_sinphi;       /* S5 |sinPhi| limit: 0.95 */
+    float kf_edge_margin;      /* S5 stop when |y| exceeds the row half-width by this [cm]: 2 */
+    int32_t sel_min_hits;      /* S6 minimum hits kept by a final track: 10 */
+    float grid_cell_z;         /* S1 z-bin width of the per-row grid [cm]: 2.5.  Performance only: no result depends on it */
+} tpc_params_t;
+
+typedef struct {
+    int32_t n_rows;            /* pad rows per sector, 3..255 (159) */
+    const float* row_x;        /* HOST pointer [n_rows], strictly increasing, uniform pitch (1e-4 rel); copied */
+    int32_t sectors_per_event; /* 36 (even) */
+    float half_angle_rad;      /* sector half opening angle (10 deg): row half-width = row_x * tan(half_angle) */
+    float z_lo, z_hi;          /* z range of the z >= 0 side used for the grid (mirrored for z < 0): 0..250, or
+                                  -250..500 for drift windows.  Clusters outside are legal (clamped into edge bins) */
+    float sigma_y, sigma_z;    /* cluster errors used by the filter [cm] */
+    tpc_params_t params;
+} tpc_geometry_t;
+
+/*
+ * Output buffers: all caller-owned DEVICE memory; a NULL pointer skips that output (counts is required).
+ * Index values are GLOBAL cluster indices (position in the input array) unless stated; -1 = none.
+ * When a capacity is too small the library writes only what fits (never out of bounds) and `counts`
+ * still holds the REQUIRED numbers, so the caller can detect it after synchronising (tpc_check_counts).
+ */
+typedef struct {
+    /* S2/S3 (parity/debug) */
+    int32_t* link_up_raw; /* [n_clusters] best up-neighbour before cleaning */
+    int32_t* link_dn_raw; /* [n_clusters] */
+    int32_t* link_up;     /* [n_clusters] after cleaning (mutual links only) */
+    int32_t* link_dn;     /* [n_clusters] */
+    /* S4 */
+    int32_t* start_hits;  /* [start_capacity] ascending */
+    int64_t start_capacity;
+    int32_t* cand_hits;   /* [cand_capacity][TPC_CAND_MAX_HITS], unused slots -1; candidates in ascending start hit */
+    int32_t* cand_n;      /* [cand_capacity] hits stored, cand_min_hits..cand_max_hits */
+    int64_t cand_capacity;
+    /* S5 tracklets, one slot per candidate id (parity/debug) */
+    float* tl_params;     /* [tl_capacity][5] y, z, sinPhi, dz/ds, q/pt at row tl_rows[.][2] */
+    float* tl_cov;        /* [tl_capacity][15] lower triangle row-major: (0,0),(1,0),(1,1),(2,0),... */
+    float* tl_chi2;       /* [tl_capacity] */
+    int32_t* tl_nhits;    /* [tl_capacity] attached hits; 0 = the candidate produced no tracklet */
+    int32_t* tl_rows;     /* [tl_capacity][3] first row, last row, reference row */
+    int32_t* tl_hits;     /* [tl_capacity][n_rows] attached cluster per row or -1 */
+    int64_t tl_capacity;
+    /* S6 final tracks, ascending candidate id */
+    float* trk_params;    /* [trk_capacity][5] (those of the tracklet: no refit after hit removal) */
+    float* trk_cov;       /* [trk_capacity][15] */
+    float* trk_chi2;      /* [trk_capacity] */
+    float* trk_xref;      /* [trk_capacity] x of the reference row */
+    int32_t* trk_cand_id; /* [trk_capacity] */
+    int32_t* trk_nhits;   /* [trk_capacity] hits kept (>= sel_min_hits) */
+    int32_t* trk_sector;  /* [trk_capacity] sector instance */
+    int64_t* trk_hit_offset; /* [trk_capacity+1] CSR into trk_hits */
+    int32_t* trk_hits;    /* [trk_hits_capacity] kept hits, rows increasing */
+    int64_t trk_capacity, trk_hits_capacity;
+    int32_t* cluster_owner; /* [n_clusters] final track index or -1 */
+    /* device [TPC_N_COUNTS]: 0 n_start, 1 n_cand, 2 n_tracklets, 3 n_tracks, 4 n_track_hits,
+       5 input error flags (bit0: a row holds > 65535 clusters; bit1: > 2^23 candidates in one instance), 6-7 reserved.
+       Written by the last kernel of the call. */
+    int64_t* counts;
+} tpc_output_t;
+
+/* Create a tracker for one geometry and field.  Host-only work plus one small upload. */
+int tpc_tracker_create(const tpc_geometry_t* geom, float bz_tesla, tpc_tracker_t** out);
+void tpc_tracker_destroy(tpc_tracker_t* t);
+
+/* Bytes of device workspace tpc_track_sectors needs for inputs up to these sizes (candidates are bounded by
+   max_clusters / cand_min_hits, so no candidate count is needed). */
+size_t tpc_workspace_bytes(const tpc_tracker_t* t, int64_t max_clusters, int64_t max_sector_instances);
+/* The caller (PyTorch) owns the workspace; it must stay valid and unshared while a call is in flight. 256-B aligned. */
+int tpc_set_workspace(tpc_tracker_t* t, void* dev_ptr, size_t bytes);
+/* cudaStream_t as void*; NULL = the legacy default stream. */
+int tpc_set_stream(tpc_tracker_t* t, void* cuda_stream);
+
+/*
+ * Track all sector instances (stages S1-S6).  clusters_xyzw: DEVICE, 16-byte aligned, [n_clusters][4] =
+ * (x, y, z, w); x and w are carried but never read (the row gives x).  row_offsets: DEVICE int32
+ * [n_sector_instances * n_rows + 1], CSR, instance-major row-minor, row_offsets[0] = 0 and
+ * row_offsets[last] = n_clusters.  Clusters inside a row may be in any order.  n_clusters < 2^31.
+ * Asynchronous; one call in flight per tracker.
+ */
+int tpc_track_sectors(tpc_tracker_t* t, const float* clusters_xyzw, const int32_t* row_offsets,
+                      int32_t n_sector_instances, int64_t n_clusters, const tpc_output_t* out);
+
+/* After synchronising and copying `counts` to the host: TPC_OK, TPC_ERR_CAPACITY or TPC_ERR_INPUT. */
+int tpc_check_counts(const int64_t* counts_host, const tpc_output_t* out);
+
+/* Number of kernel launches the last tpc_track_sectors call enqueued (for bench.py's gpu_launches). */
+int32_t tpc_last_launch_count(const tpc_tracker_t* t);
+
+/* Optional per-stage timing of later calls: event_pairs = 1 records CUDA events around every stage;
+   tpc_stage_times_ms synchronises the stream and returns the milliseconds of the last call in
+   out_ms[TPC_N_STAGES] (order: bin, neighbours, clean, chains, follow, select). */
+#define TPC_N_STAGES 6
+int tpc_set_stage_timing(tpc_tracker_t* t, int32_t enable);
+int tpc_stage_times_ms(tpc_tracker_t* t, float* out_ms);
+
+const char* tpc_last_error(const tpc_tracker_t* t);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPC_TRACKER_H */

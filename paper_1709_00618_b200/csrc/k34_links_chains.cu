@@ -1,0 +1,186 @@
+// S3: neighbour cleaning (keep only mutual links; BASELINE.json north_star) and
+// S4: start hits + concatenation of links into track candidates "of usually 4 to 10 TPC hits" (Fig. 1b).
+// All integer work; results are unique, so they must equal the oracle bit for bit.
+//
+// Deterministic compaction without atomics-ordered output: candidates are numbered in ascending global index of
+// their start hit by (1) per-slab counts, (2) one exclusive scan over the S*R slab counts, (3) a ballot/popc
+// ranking inside each slab CTA.
+#include "tpc_common.cuh"
+
+namespace tpc {
+
+constexpr int kCleanThreads = 256;
+constexpr int kChainThreads = 128;
+constexpr int kScanThreads = 1024;
+
+// S3 + per-hit initialisation of the selector's claim word (fused here because this kernel streams over all hits).
+__global__ void __launch_bounds__(kCleanThreads)
+clean_links_kernel(int64_t n, const int32_t* __restrict__ up_raw, const int32_t* __restrict__ dn_raw,
+                   int32_t* __restrict__ up, int32_t* __restrict__ dn, uint32_t* __restrict__ claim) {
+    const int64_t h = (int64_t)blockIdx.x * kCleanThreads + threadIdx.x;
+    if (h >= n) return;
+    const int32_t u = up_raw[h], d = dn_raw[h];
+    up[h] = (u >= 0 && __ldg(&dn_raw[u]) == (int32_t)h) ? u : -1;
+    dn[h] = (d >= 0 && __ldg(&up_raw[d]) == (int32_t)h) ? d : -1;
+    claim[h] = 0u;
+}
+
+// S4 pass 1: per-hit flags (bit0 start hit, bit1 candidate) and per-slab counts.
+__global__ void __launch_bounds__(kChainThreads)
+chain_flags_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
+                   const int32_t* __restrict__ up, const int32_t* __restrict__ dn, uint8_t* __restrict__ flags,
+                   int2* __restrict__ slab_part) {
+    __shared__ int s_cnt[2];
+    const int slab = blockIdx.x;
+    const int base = row_offsets[slab], n = row_offsets[slab + 1] - base;
+    if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    int ns = 0, nc = 0;
+    for (int i = threadIdx.x; i < n; i += kChainThreads) {
+        const int h = base + i;
+        uint8_t f = 0;
+        int x = up[h];
+        if (x >= 0 && dn[h] < 0) {
+            f = 1;
+            int len = 2;  // h and x
+            while (len < g.cand_min && (x = __ldg(&up[x])) >= 0) len++;
+            if (x >= 0 && len >= g.cand_min) f = 3;
+        }
+        flags[h] = f;
+        ns += f & 1;
+        nc += f >> 1;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        ns += __shfl_xor_sync(0xffffffffu, ns, d);
+        nc += __shfl_xor_sync(0xffffffffu, nc, d);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&s_cnt[0], ns);
+        atomicAdd(&s_cnt[1], nc);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) slab_part[slab] = make_int2(s_cnt[0], s_cnt[1]);
+}
+
+// Exclusive scan of int2 partials by ONE CTA (m is a few thousand to a few hundred thousand entries); entry m
+// receives the totals, which also go to counts[c0], counts[c1].
+__global__ void __launch_bounds__(kScanThreads)
+scan_int2_kernel(int2* __restrict__ part, const int64_t* __restrict__ m_dev, int64_t m_div, int64_t m_cap,
+                 int64_t m_host, int64_t* __restrict__ counts, int c0, int c1) {
+    __shared__ int2 s_warp[kScanThreads / 32];
+    __shared__ int2 s_carry;
+    // number of entries: host value, or ceil(min(*m_dev, m_cap) / m_div) when m_dev is given (S6: device-side count)
+    const int64_t m = m_dev ? (min(*m_dev, m_cap) + m_div - 1) / m_div : m_host;
+    if (threadIdx.x == 0) s_carry = make_int2(0, 0);
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int64_t start = 0; start < m; start += kScanThreads) {
+        const int64_t i = start + threadIdx.x;
+        int2 v = i < m ? part[i] : make_int2(0, 0);
+        int2 incl = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            int a = __shfl_up_sync(0xffffffffu, incl.x, d), b = __shfl_up_sync(0xffffffffu, incl.y, d);
+            if (lane >= d) { incl.x += a; incl.y += b; }
+        }
+        if (lane == 31) s_warp[wid] = incl;
+        __syncthreads();
+        int2 off = s_carry;
+        for (int k = 0; k < wid; k++) { off.x += s_warp[k].x; off.y += s_warp[k].y; }
+        if (i < m) part[i] = make_int2(off.x + incl.x - v.x, off.y + incl.y - v.y);
+        __syncthreads();
+        if (threadIdx.x == kScanThreads - 1) s_carry = make_int2(off.x + incl.x, off.y + incl.y);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        part[m] = s_carry;
+        counts[c0] = s_carry.x;
+        counts[c1] = s_carry.y;
+    }
+}
+
+// S4 pass 2: ranked write of start hits and candidates.
+__global__ void __launch_bounds__(kChainThreads)
+chain_write_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
+                   const int32_t* __restrict__ up, const uint8_t* __restrict__ flags,
+                   const int2* __restrict__ slab_part, int32_t* __restrict__ start_hits, int64_t start_cap,
+                   int32_t* __restrict__ cand_hits, int32_t* __restrict__ cand_n, int32_t* __restrict__ cand_slab,
+                   int64_t cand_cap, int32_t* __restrict__ usr_cand_hits, int32_t* __restrict__ usr_cand_n,
+                   int64_t usr_cand_cap) {
+    __shared__ int2 s_warp[kChainThreads / 32];
+    const int slab = blockIdx.x;
+    const int base = row_offsets[slab], n = row_offsets[slab + 1] - base;
+    const int2 sb = slab_part[slab];
+    if (slab_part[slab + 1].x == sb.x) return;  // no start hit in this slab
+    int run_s = sb.x, run_c = sb.y;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int start = 0; start < n; start += kChainThreads) {
+        const int i = start + threadIdx.x;
+        const int h = base + i;
+        const uint8_t f = i < n ? flags[h] : 0;
+        const unsigned ms = __ballot_sync(0xffffffffu, f & 1), mc = __ballot_sync(0xffffffffu, f & 2);
+        if (lane == 0) s_warp[wid] = make_int2(__popc(ms), __popc(mc));
+        __syncthreads();
+        int os = run_s, oc = run_c, ts = 0, tc = 0;
+#pragma unroll
+        for (int k = 0; k < kChainThreads / 32; k++) {
+            const int2 v = s_warp[k];
+            if (k < wid) { os += v.x; oc += v.y; }
+            ts += v.x;
+            tc += v.y;
+        }
+        const unsigned below = (1u << lane) - 1u;
+        if (f & 1) {
+            const int64_t ps = os + __popc(ms & below);
+            if (start_hits && ps < start_cap) start_hits[ps] = h;
+        }
+        if (f & 2) {
+            const int64_t c = oc + __popc(mc & below);
+            int32_t hits[kCandMax];
+            int k = 0;
+            for (int x = h; x >= 0 && k < g.cand_max; x = __ldg(&up[x])) hits[k++] = x;
+            const int nh = k;
+            for (; k < kCandMax; k++) hits[k] = -1;
+            if (c < cand_cap) {
+#pragma unroll
+                for (int q = 0; q < kCandMax; q++) cand_hits[c * kCandMax + q] = hits[q];
+                cand_n[c] = nh;
+                cand_slab[c] = slab;
+            }
+            if (usr_cand_hits && c < usr_cand_cap) {
+#pragma unroll
+                for (int q = 0; q < kCandMax; q++) usr_cand_hits[c * kCandMax + q] = hits[q];
+            }
+            if (usr_cand_n && c < usr_cand_cap) usr_cand_n[c] = nh;
+        }
+        run_s += ts;
+        run_c += tc;
+        __syncthreads();
+    }
+}
+
+int launch_clean(const DevGeom&, const Workspace& w, const Problem& p, cudaStream_t s) {
+    if (p.n_clusters == 0) return 0;
+    clean_links_kernel<<<div_up(p.n_clusters, kCleanThreads), kCleanThreads, 0, s>>>(p.n_clusters, w.up_raw, w.dn_raw,
+                                                                                    w.up, w.dn, w.claim);
+    return 1;
+}
+
+void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m_cap, int64_t m_host, int64_t* counts,
+                      int c0, int c1, cudaStream_t s) {
+    scan_int2_kernel<<<1, kScanThreads, 0, s>>>(part, m_dev, m_div, m_cap, m_host, counts, c0, c1);
+}
+
+int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, cudaStream_t s) {
+    const int slabs = p.n_inst * g.R;
+    if (slabs == 0) return 0;
+    chain_flags_kernel<<<slabs, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.dn, w.flags, w.slab_part);
+    launch_scan_int2(w.slab_part, nullptr, 1, 0, slabs, w.counts, 0, 1, s);
+    chain_write_kernel<<<slabs, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.flags, w.slab_part, u.start_hits,
+                                                       u.start_cap, w.cand_hits, w.cand_n, w.cand_slab, w.Cmax,
+                                                       u.cand_hits, u.cand_n, u.cand_cap);
+    return 3;
+}
+
+}  // namespace tpc

@@ -1,0 +1,173 @@
+// fp32 Kalman-filter arithmetic of S5 (track following with "a simplified Kalman filter"; only Bz is
+// respected).  State p = (y, z, sinPhi, dz/ds, q/pt) at a pad-row plane x; covariance as the packed
+// lower triangle c00 c10 c11 c20 c21 c22 c30 c31 c32 c33 c40 c41 c42 c43 c44.  Formulas: DESIGN.md "S5".
+// Written from the formulas, not from the oracle's code: the oracle works on full 5x5 fp64 matrices with generic
+// loops, this file on the 15 packed fp32 entries with the sparse Jacobian multiplied out by hand.
+#pragma once
+#include "tpc_common.cuh"
+
+namespace tpc {
+
+struct KfState {
+    float y, z, s, t, k;
+    float c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
+};
+
+// asin(a)/a: arc length over chord for half-angle sine a
+__device__ __forceinline__ float asin_over(float a) {
+    const float a2 = a * a;
+    if (a2 < 0.01f)  // |a| < 0.1: series, truncation < 4e-10
+        return 1.0f + a2 * (1.0f / 6.0f + a2 * (3.0f / 40.0f + a2 * (15.0f / 336.0f)));
+    return asinf(a) / a;
+}
+
+// Transport to the plane x + dx along the exact helix for constant Bz.  Returns false (state untouched) when
+// |sinPhi| would leave [-max_s, max_s].
+__device__ __forceinline__ bool kf_transport(KfState& st, float dx, float cB, float max_s) {
+    const float s = st.s, t = st.t;
+    const float kap = cB * st.k;
+    const float kdx = kap * dx;
+    const float s1 = s + kdx;
+    if (fabsf(s) > max_s || fabsf(s1) > max_s) return false;
+    const float c0sq = (1.0f - s) * (1.0f + s), c1sq = (1.0f - s1) * (1.0f + s1);
+    const float ic0 = rsqrtf(c0sq), ic1 = rsqrtf(c1sq);
+    const float c0 = c0sq * ic0, c1 = c1sq * ic1;
+    const float tg = (s + s1) / (c0 + c1);
+    const float sec2 = fmaf(tg, tg, 1.0f);
+    const float chord = dx * sqrtf(sec2);
+    const float a = 0.5f * kap * chord;
+    const float dS = chord * asin_over(a);
+    // Jacobian entries (identity elsewhere)
+    const float f02 = dx * sec2 * 0.5f * (ic0 + ic1);
+    const float f04 = cB * dx * dx * sec2 * 0.5f * ic1;
+    const float f12 = t * dx * tg * ic0 * ic1;
+    const float f13 = dS;
+    float ddS;  // d(dS)/d(kappa) = (dx/c1 - dS)/kappa; cancels for small kappa*dx -> 2/3-point series there
+    if (fabsf(kdx) > 0.02f) {
+        ddS = (dx * ic1 - dS) / kap;
+    } else {
+        const float se = fmaf(2.0f / 3.0f, kdx, s);
+        const float ice = rsqrtf((1.0f - se) * (1.0f + se));
+        ddS = 0.5f * dx * dx * se * ice * ice * ice;
+    }
+    const float f14 = cB * t * ddS;
+    const float f24 = cB * dx;
+    st.y = fmaf(dx, tg, st.y);
+    st.z = fmaf(t, dS, st.z);
+    st.s = s1;
+    // P <- F P F^T, multiplied out for the lower triangle
+    const float n40 = st.c40 + f02 * st.c42 + f04 * st.c44;
+    const float n41 = st.c41 + f12 * st.c42 + f13 * st.c43 + f14 * st.c44;
+    const float n42 = st.c42 + f24 * st.c44;
+    const float n30 = st.c30 + f02 * st.c32 + f04 * st.c43;
+    const float n31 = st.c31 + f12 * st.c32 + f13 * st.c33 + f14 * st.c43;
+    const float n32 = st.c32 + f24 * st.c43;
+    const float a00 = st.c00 + f02 * st.c20 + f04 * st.c40;
+    const float a02 = st.c20 + f02 * st.c22 + f04 * st.c42;
+    const float a10 = st.c10 + f12 * st.c20 + f13 * st.c30 + f14 * st.c40;
+    const float a11 = st.c11 + f12 * st.c21 + f13 * st.c31 + f14 * st.c41;
+    const float a12 = st.c21 + f12 * st.c22 + f13 * st.c32 + f14 * st.c42;
+    const float a20 = st.c20 + f24 * st.c40;
+    const float a21 = st.c21 + f24 * st.c41;
+    const float a22 = st.c22 + f24 * st.c42;
+    st.c00 = a00 + f02 * a02 + f04 * n40;
+    st.c10 = a10 + f02 * a12 + f04 * n41;
+    st.c11 = a11 + f12 * a12 + f13 * n31 + f14 * n41;
+    st.c20 = a20 + f02 * a22 + f04 * n42;
+    st.c21 = a21 + f12 * a22 + f13 * n32 + f14 * n42;
+    st.c22 = a22 + f24 * n42;
+    st.c30 = n30;
+    st.c31 = n31;
+    st.c32 = n32;
+    st.c40 = n40;
+    st.c41 = n41;
+    st.c42 = n42;
+    return true;
+}
+
+// Two sequential scalar updates (y with sy2, then z with sz2); returns the chi2 increment.
+__device__ __forceinline__ float kf_update(KfState& st, float ym, float zm, float sy2, float sz2) {
+    float chi2;
+    {
+        const float inv = 1.0f / (st.c00 + sy2);
+        const float res = ym - st.y;
+        const float k0 = st.c00 * inv, k1 = st.c10 * inv, k2 = st.c20 * inv, k3 = st.c30 * inv, k4 = st.c40 * inv;
+        const float r = sy2 * inv;  // column 0 shrinks by sigma^2/S (no cancellation)
+        chi2 = res * res * inv;
+        st.y = fmaf(k0, res, st.y);
+        st.z = fmaf(k1, res, st.z);
+        st.s = fmaf(k2, res, st.s);
+        st.t = fmaf(k3, res, st.t);
+        st.k = fmaf(k4, res, st.k);
+        st.c11 = fmaf(-k1, st.c10, st.c11);
+        st.c21 = fmaf(-k2, st.c10, st.c21);
+        st.c22 = fmaf(-k2, st.c20, st.c22);
+        st.c31 = fmaf(-k3, st.c10, st.c31);
+        st.c32 = fmaf(-k3, st.c20, st.c32);
+        st.c33 = fmaf(-k3, st.c30, st.c33);
+        st.c41 = fmaf(-k4, st.c10, st.c41);
+        st.c42 = fmaf(-k4, st.c20, st.c42);
+        st.c43 = fmaf(-k4, st.c30, st.c43);
+        st.c44 = fmaf(-k4, st.c40, st.c44);
+        st.c00 *= r;
+        st.c10 *= r;
+        st.c20 *= r;
+        st.c30 *= r;
+        st.c40 *= r;
+    }
+    {
+        const float inv = 1.0f / (st.c11 + sz2);
+        const float res = zm - st.z;
+        const float k0 = st.c10 * inv, k1 = st.c11 * inv, k2 = st.c21 * inv, k3 = st.c31 * inv, k4 = st.c41 * inv;
+        const float r = sz2 * inv;
+        chi2 = fmaf(res * res, inv, chi2);
+        st.y = fmaf(k0, res, st.y);
+        st.z = fmaf(k1, res, st.z);
+        st.s = fmaf(k2, res, st.s);
+        st.t = fmaf(k3, res, st.t);
+        st.k = fmaf(k4, res, st.k);
+        st.c00 = fmaf(-k0, st.c10, st.c00);
+        st.c20 = fmaf(-k2, st.c10, st.c20);
+        st.c22 = fmaf(-k2, st.c21, st.c22);
+        st.c30 = fmaf(-k3, st.c10, st.c30);
+        st.c32 = fmaf(-k3, st.c21, st.c32);
+        st.c33 = fmaf(-k3, st.c31, st.c33);
+        st.c40 = fmaf(-k4, st.c10, st.c40);
+        st.c42 = fmaf(-k4, st.c21, st.c42);
+        st.c43 = fmaf(-k4, st.c31, st.c43);
+        st.c44 = fmaf(-k4, st.c41, st.c44);
+        st.c10 *= r;
+        st.c11 *= r;
+        st.c21 *= r;
+        st.c31 *= r;
+        st.c41 *= r;
+    }
+    return chi2;
+}
+
+// Seed: circle through three points in (x,y); dz/ds from the end points.  Returns false if |sinPhi| > max_s.
+__device__ __forceinline__ bool kf_seed(KfState& st, float x0, float y0, float z0, float x1, float y1, float x2,
+                                        float y2, float z2, float cB, float max_s, const float* p0) {
+    const float ax = x1 - x0, ay = y1 - y0, bx = x2 - x0, by = y2 - y0;
+    const float cross = ax * by - ay * bx;
+    const float d01 = sqrtf(ax * ax + ay * ay), d02 = sqrtf(bx * bx + by * by);
+    const float ex = x2 - x1, ey = y2 - y1;
+    const float d12 = sqrtf(ex * ex + ey * ey);
+    const float kap = 2.0f * cross / (d01 * d02 * d12);
+    // sin(theta01 - asin(kappa d01 / 2)) expanded: sin A cos B - cos A sin B, with sin A = ay/d01, cos A = ax/d01
+    const float sb = 0.5f * kap * d01;
+    const float cb = sqrtf((1.0f - sb) * (1.0f + sb));
+    const float sphi = (ay * cb - ax * sb) / d01;
+    if (!(fabsf(sphi) <= max_s)) return false;
+    const float S02 = d02 * asin_over(0.5f * kap * d02);
+    st.y = y0;
+    st.z = z0;
+    st.s = sphi;
+    st.t = (z2 - z0) / S02;
+    st.k = cB != 0.0f ? kap / cB : 0.0f;
+    st.c00 = p0[0]; st.c11 = p0[1]; st.c22 = p0[2]; st.c33 = p0[3]; st.c44 = p0[4];
+    st.c10 = st.c20 = st.c21 = st.c30 = st.c31 = st.c32 = st.c40 = st.c41 = st.c42 = st.c43 = 0.0f;
+    return true;
+}
+
+}  // namespace tpc

@@ -1,0 +1,114 @@
+// Internal declarations shared by the CUDA translation units of libtpctrk.so.  Not part of the ABI.
+// (The CPU oracle in oracle/ includes nothing from here.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tpc {
+
+constexpr int kCandMax = 10;      // TPC_CAND_MAX_HITS
+constexpr int kMaxRows = 255;
+constexpr int kMaxZBins = 2047;
+constexpr uint16_t kNoHit = 0xFFFFu;
+constexpr float kKappaPerTesla = 0.00299792458f;
+
+// Everything the kernels need to know about geometry and tunables.  Passed by value as a
+// __grid_constant__ kernel parameter (lives in the constant bank; uniform reads are free).
+struct DevGeom {
+    int R;          // pad rows
+    int RP;         // row stride of the per-tracklet hit table (R rounded up to 8)
+    int nz;         // z bins per row
+    int nzp;        // stride of the bin table (nz + 1 rounded up to 2)
+    int spe, spe_half;
+    float z0_a, z0_c;  // grid origin: z >= 0 side, z < 0 side
+    float inv_cz;
+    float nf_wy, nf_wz, nf_d2max;
+    int cand_min, cand_max;
+    float p0[5];
+    float gate, wmax;
+    int max_gap;
+    float max_s, edge_margin, tan_half;
+    int sel_min;
+    float sy2, sz2;
+    float cB;       // curvature per (q/pt): kappa = cB * q/pt
+    const float* row_x;  // device [R]
+};
+
+// Views into the caller's workspace (all device pointers), fixed per call.
+struct Workspace {
+    float2* hit_yz;       // [N]  (y, z) sorted by z bin inside every (instance,row) segment
+    uint16_t* hit_idx;    // [N]  local index (position in the row segment of the INPUT) of the sorted hit
+    uint16_t* bin_start;  // [S*R][nzp] first sorted position of every z bin, entry nz = row length
+    int32_t* up_raw;      // [N] global indices
+    int32_t* dn_raw;
+    int32_t* up;          // cleaned
+    int32_t* dn;
+    uint32_t* claim;      // [N] S6 best claiming weight
+    uint8_t* flags;       // [N] bit0 start hit, bit1 candidate
+    int2* slab_part;      // [S*R + 1] (starts, candidates) per slab, then their exclusive scan
+    int32_t* cand_hits;   // [Cmax][kCandMax]
+    int32_t* cand_n;      // [Cmax]
+    int32_t* cand_slab;   // [Cmax] instance * R + row of the start hit
+    float* tl_par;        // [Cmax][5]
+    float* tl_cov;        // [Cmax][15]
+    float* tl_chi2;       // [Cmax]
+    int32_t* tl_nhits;    // [Cmax]  0 = no tracklet
+    int32_t* tl_rows;     // [Cmax]  first | last << 8 | ref << 16
+    uint16_t* tl_rowhit;  // [Cmax][RP] local index of the attached hit per row (valid in first..last), kNoHit = none
+    int32_t* tl_kept;     // [Cmax]  hits won in the selector, 0 if rejected
+    int2* sel_part;       // [Cmax/64 + 2] (tracks, hits) per block of 64 tracklets, then exclusive scan
+    int64_t* counts;      // [8] internal copy of the output counts
+    int64_t Cmax;
+};
+
+struct Problem {
+    const float4* clusters;
+    const int32_t* row_offsets;
+    int32_t n_inst;
+    int64_t n_clusters;
+};
+
+__host__ __device__ inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// z bin of the per-row grid.  Monotone non-decreasing in z (one rounded subtraction, one rounded multiplication by
+// a positive constant, floor, clamp), which is all the superset arguments of S2 and S5 need.
+__device__ __forceinline__ int zbin(float z, float z0, float inv_cz, int nz) {
+    int b = __float2int_rd(__fmul_rn(__fsub_rn(z, z0), inv_cz));
+    return min(max(b, 0), nz - 1);
+}
+
+__device__ __forceinline__ float grid_z0(const DevGeom& g, int inst) {
+    return ((inst % g.spe) >= g.spe_half) ? g.z0_c : g.z0_a;
+}
+
+// ---- launchers (one per stage; each returns the number of kernels it enqueued) ----
+int launch_bin_rows(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s);
+int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s);
+int launch_clean(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s);
+struct ChainOut {  // optional user-facing S4 outputs (NULL = skip)
+    int32_t* start_hits;
+    int64_t start_cap;
+    int32_t* cand_hits;
+    int32_t* cand_n;
+    int64_t cand_cap;
+};
+int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, cudaStream_t s);
+void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m_cap, int64_t m_host, int64_t* counts,
+                      int c0, int c1, cudaStream_t s);
+int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, cudaStream_t s);
+
+struct SelectOut {  // mirrors the S6 part of tpc_output_t
+    float *trk_params, *trk_cov, *trk_chi2, *trk_xref;
+    int32_t *trk_cand_id, *trk_nhits, *trk_sector;
+    int64_t* trk_hit_offset;
+    int32_t* trk_hits;
+    int64_t trk_capacity, trk_hits_capacity;
+    int32_t* cluster_owner;
+    int64_t* counts;  // user counts (device)
+};
+int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const SelectOut& o, cudaStream_t s);
+// expands the compact tracklet hit table into global indices [Cmax_out][R] (parity/debug output)
+int launch_export_tracklets(const DevGeom& g, const Workspace& w, const Problem& p, int32_t* tl_hits, int32_t* tl_rows,
+                            int64_t cap, cudaStream_t s);
+
+}  // namespace tpc

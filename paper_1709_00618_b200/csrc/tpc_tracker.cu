@@ -1,0 +1,282 @@
+// C ABI of libtpctrk.so (include/tpc_tracker.h): handle, workspace carving, stage sequencing.
+// Host code only; every step of the hot path runs in the kernels of k1..k6.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/tpc_tracker.h"
+#include "tpc_common.cuh"
+
+using namespace tpc;
+
+struct tpc_tracker {
+    DevGeom g;
+    float* d_row_x = nullptr;
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;
+    int n_sm = 148;
+    int last_launches = 0;
+    bool timing = false;
+    cudaEvent_t ev[TPC_N_STAGES + 1] = {};
+    bool ev_valid = false;
+    std::string err;
+};
+
+static int fail(tpc_tracker* t, int code, const std::string& msg) {
+    if (t) t->err = msg;
+    return code;
+}
+
+static thread_local std::string g_create_err;
+
+template <typename T>
+static T dflt(T v, T d) { return v == (T)0 ? d : v; }
+
+extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_tracker_t** out) {
+    if (!geom || !out || !geom->row_x) { g_create_err = "NULL argument"; return TPC_ERR_ARG; }
+    *out = nullptr;
+    const int R = geom->n_rows;
+    if (R < 3 || R > kMaxRows) { g_create_err = "n_rows out of [3,255]"; return TPC_ERR_GEOMETRY; }
+    const double pitch = ((double)geom->row_x[R - 1] - (double)geom->row_x[0]) / (R - 1);
+    if (!(pitch > 0.0)) { g_create_err = "rows not increasing"; return TPC_ERR_GEOMETRY; }
+    for (int r = 1; r < R; r++) {
+        const double d = (double)geom->row_x[r] - (double)geom->row_x[r - 1];
+        if (!(d > 0.0) || std::fabs(d - pitch) > 1e-4 * pitch + 4e-5) {
+            g_create_err = "pad rows must be strictly increasing with uniform pitch (DESIGN.md reading A5)";
+            return TPC_ERR_GEOMETRY;
+        }
+    }
+    if (geom->sectors_per_event < 2 || (geom->sectors_per_event & 1) || !(geom->z_hi > geom->z_lo) ||
+        !(geom->sigma_y > 0.0f) || !(geom->sigma_z > 0.0f) || !(geom->half_angle_rad > 0.0f)) {
+        g_create_err = "bad sectors_per_event / z range / sigma / half angle";
+        return TPC_ERR_ARG;
+    }
+    const tpc_params_t& p = geom->params;
+    tpc_tracker* t = new (std::nothrow) tpc_tracker();
+    if (!t) { g_create_err = "out of host memory"; return TPC_ERR_ARG; }
+    DevGeom& g = t->g;
+    g.R = R;
+    g.RP = (R + 7) & ~7;
+    const float cz = dflt(p.grid_cell_z, 2.5f);
+    int nz = (int)std::ceil(((double)geom->z_hi - (double)geom->z_lo) / cz);
+    if (nz < 1) nz = 1;
+    if (nz > kMaxZBins) nz = kMaxZBins;
+    g.nz = nz;
+    g.nzp = (nz + 2) & ~1;
+    g.spe = geom->sectors_per_event;
+    g.spe_half = g.spe / 2;
+    g.z0_a = geom->z_lo;
+    g.z0_c = -geom->z_hi;
+    g.inv_cz = 1.0f / cz;
+    g.nf_wy = dflt(p.nf_win_y, 2.0f);
+    g.nf_wz = dflt(p.nf_win_z, 2.5f);
+    g.nf_d2max = dflt(p.nf_d2_max, 1.0f);
+    g.cand_min = dflt(p.cand_min_hits, 4);
+    g.cand_max = dflt(p.cand_max_hits, 10);
+    const float p0d[5] = {1.0f, 1.0f, 0.1f, 0.1f, 10.0f};
+    for (int i = 0; i < 5; i++) g.p0[i] = dflt(p.kf_p0[i], p0d[i]);
+    g.gate = dflt(p.kf_gate_sigma, 4.0f);
+    g.wmax = dflt(p.kf_win_max, 3.0f);
+    g.max_gap = dflt(p.kf_max_gap, 5);
+    g.max_s = dflt(p.kf_max_sinphi, 0.95f);
+    g.edge_margin = dflt(p.kf_edge_margin, 2.0f);
+    g.tan_half = (float)std::tan((double)geom->half_angle_rad);
+    g.sel_min = dflt(p.sel_min_hits, 10);
+    g.sy2 = (float)((double)geom->sigma_y * (double)geom->sigma_y);
+    g.sz2 = (float)((double)geom->sigma_z * (double)geom->sigma_z);
+    g.cB = (float)(-0.00299792458 * (double)bz);
+    if (g.cand_min < 2 || g.cand_max > kCandMax || g.cand_max < g.cand_min || g.cand_max < 3) {
+        delete t;
+        g_create_err = "cand_min_hits/cand_max_hits out of range (2 <= min <= max <= 10, max >= 3)";
+        return TPC_ERR_ARG;
+    }
+    cudaError_t e = cudaMalloc(&t->d_row_x, sizeof(float) * R);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_row_x, geom->row_x, sizeof(float) * R, cudaMemcpyHostToDevice);
+    int dev = 0;
+    if (e == cudaSuccess) e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&t->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) {
+        g_create_err = std::string("CUDA: ") + cudaGetErrorString(e);
+        if (t->d_row_x) cudaFree(t->d_row_x);
+        delete t;
+        return TPC_ERR_CUDA;
+    }
+    g.row_x = t->d_row_x;
+    *out = t;
+    return TPC_OK;
+}
+
+extern "C" void tpc_tracker_destroy(tpc_tracker_t* t) {
+    if (!t) return;
+    if (t->ev_valid)
+        for (auto& e : t->ev) cudaEventDestroy(e);
+    if (t->d_row_x) cudaFree(t->d_row_x);
+    delete t;
+}
+
+// ---- workspace carving: one function computes the layout for both sizing and use ----
+namespace {
+struct Carver {
+    char* base;
+    size_t off = 0;
+    template <typename T>
+    T* take(size_t n) {
+        off = (off + 255) & ~(size_t)255;
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
+    Carver c{static_cast<char*>(base)};
+    const size_t n = (size_t)(N > 0 ? N : 1), slabs = (size_t)(S > 0 ? S : 1) * g.R;
+    const size_t cmax = (size_t)(N / g.cand_min + 1);
+    Workspace v;
+    v.counts = c.take<int64_t>(TPC_N_COUNTS);
+    v.hit_yz = c.take<float2>(n);
+    v.hit_idx = c.take<uint16_t>(n);
+    v.bin_start = c.take<uint16_t>(slabs * g.nzp);
+    v.up_raw = c.take<int32_t>(n);
+    v.dn_raw = c.take<int32_t>(n);
+    v.up = c.take<int32_t>(n);
+    v.dn = c.take<int32_t>(n);
+    v.claim = c.take<uint32_t>(n);
+    v.flags = c.take<uint8_t>(n);
+    v.slab_part = c.take<int2>(slabs + 1);
+    v.cand_hits = c.take<int32_t>(cmax * kCandMax);
+    v.cand_n = c.take<int32_t>(cmax);
+    v.cand_slab = c.take<int32_t>(cmax);
+    v.tl_par = c.take<float>(cmax * 5);
+    v.tl_cov = c.take<float>(cmax * 15);
+    v.tl_chi2 = c.take<float>(cmax);
+    v.tl_nhits = c.take<int32_t>(cmax);
+    v.tl_rows = c.take<int32_t>(cmax);
+    v.tl_rowhit = c.take<uint16_t>(cmax * g.RP);
+    v.tl_kept = c.take<int32_t>(cmax);
+    v.sel_part = c.take<int2>(cmax / 64 + 2);
+    v.Cmax = (int64_t)cmax;
+    if (w) *w = v;
+    return (c.off + 255) & ~(size_t)255;
+}
+}  // namespace
+
+extern "C" size_t tpc_workspace_bytes(const tpc_tracker_t* t, int64_t max_clusters, int64_t max_inst) {
+    if (!t || max_clusters < 0 || max_inst < 0) return 0;
+    return carve(t->g, nullptr, max_clusters, max_inst, nullptr);
+}
+
+extern "C" int tpc_set_workspace(tpc_tracker_t* t, void* dev_ptr, size_t bytes) {
+    if (!t) return TPC_ERR_ARG;
+    if (!dev_ptr || ((uintptr_t)dev_ptr & 255)) return fail(t, TPC_ERR_ARG, "workspace must be non-NULL and 256-byte aligned");
+    t->ws = dev_ptr;
+    t->ws_bytes = bytes;
+    return TPC_OK;
+}
+
+extern "C" int tpc_set_stream(tpc_tracker_t* t, void* s) {
+    if (!t) return TPC_ERR_ARG;
+    t->stream = static_cast<cudaStream_t>(s);
+    return TPC_OK;
+}
+
+extern "C" int tpc_set_stage_timing(tpc_tracker_t* t, int32_t enable) {
+    if (!t) return TPC_ERR_ARG;
+    if (enable && !t->ev_valid) {
+        for (auto& e : t->ev)
+            if (cudaEventCreate(&e) != cudaSuccess) return fail(t, TPC_ERR_CUDA, "cudaEventCreate failed");
+        t->ev_valid = true;
+    }
+    t->timing = enable != 0;
+    return TPC_OK;
+}
+
+extern "C" int tpc_stage_times_ms(tpc_tracker_t* t, float* out_ms) {
+    if (!t || !out_ms) return TPC_ERR_ARG;
+    if (!t->ev_valid) return fail(t, TPC_ERR_ARG, "stage timing was not enabled");
+    cudaError_t e = cudaEventSynchronize(t->ev[TPC_N_STAGES]);
+    for (int i = 0; i < TPC_N_STAGES && e == cudaSuccess; i++) e = cudaEventElapsedTime(&out_ms[i], t->ev[i], t->ev[i + 1]);
+    if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, std::string("CUDA: ") + cudaGetErrorString(e));
+    return TPC_OK;
+}
+
+extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const int32_t* row_offsets, int32_t n_inst,
+                                 int64_t n_clusters, const tpc_output_t* out) {
+    if (!t) return TPC_ERR_ARG;
+    if (!out || !out->counts) return fail(t, TPC_ERR_ARG, "out and out->counts are required");
+    if (n_inst < 0 || n_clusters < 0 || n_clusters >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "bad sizes");
+    if ((int64_t)n_inst * t->g.R + 1 >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "too many sector instances");
+    if (n_clusters > 0 && (!clusters || !row_offsets || n_inst == 0)) return fail(t, TPC_ERR_ARG, "NULL input");
+    if ((uintptr_t)clusters & 15) return fail(t, TPC_ERR_ARG, "clusters must be 16-byte aligned");
+    Workspace w;
+    const size_t need = carve(t->g, t->ws, n_clusters, n_inst, &w);
+    if (!t->ws || need > t->ws_bytes) return fail(t, TPC_ERR_WORKSPACE, "workspace missing or too small");
+    cudaStream_t s = t->stream;
+    const DevGeom& g = t->g;
+    Problem p{reinterpret_cast<const float4*>(clusters), row_offsets, n_inst, n_clusters};
+    int launches = 0;
+    const bool tm = t->timing && t->ev_valid;
+    cudaMemsetAsync(w.counts, 0, sizeof(int64_t) * TPC_N_COUNTS, s);
+    if (out->cluster_owner && n_clusters > 0) cudaMemsetAsync(out->cluster_owner, 0xFF, sizeof(int32_t) * n_clusters, s);
+    if (tm) cudaEventRecord(t->ev[0], s);
+    launches += launch_bin_rows(g, w, p, s);
+    if (tm) cudaEventRecord(t->ev[1], s);
+    launches += launch_neighbours(g, w, p, s);
+    if (tm) cudaEventRecord(t->ev[2], s);
+    launches += launch_clean(g, w, p, s);
+    if (tm) cudaEventRecord(t->ev[3], s);
+    ChainOut co{out->start_hits, out->start_hits ? out->start_capacity : 0, out->cand_hits, out->cand_n,
+                (out->cand_hits || out->cand_n) ? out->cand_capacity : 0};
+    launches += launch_chains(g, w, p, co, s);
+    if (tm) cudaEventRecord(t->ev[4], s);
+    launches += launch_follow(g, w, p, t->n_sm, s);
+    if (tm) cudaEventRecord(t->ev[5], s);
+    SelectOut so{out->trk_params, out->trk_cov, out->trk_chi2, out->trk_xref, out->trk_cand_id, out->trk_nhits,
+                 out->trk_sector, out->trk_hit_offset, out->trk_hits, out->trk_capacity, out->trk_hits_capacity,
+                 out->cluster_owner, out->counts};
+    launches += launch_select(g, w, p, so, s);
+    if (tm) cudaEventRecord(t->ev[6], s);
+    // optional parity/debug copies (device to device, same stream)
+    if (n_clusters > 0) {
+        const size_t nb = sizeof(int32_t) * (size_t)n_clusters;
+        if (out->link_up_raw) cudaMemcpyAsync(out->link_up_raw, w.up_raw, nb, cudaMemcpyDeviceToDevice, s);
+        if (out->link_dn_raw) cudaMemcpyAsync(out->link_dn_raw, w.dn_raw, nb, cudaMemcpyDeviceToDevice, s);
+        if (out->link_up) cudaMemcpyAsync(out->link_up, w.up, nb, cudaMemcpyDeviceToDevice, s);
+        if (out->link_dn) cudaMemcpyAsync(out->link_dn, w.dn, nb, cudaMemcpyDeviceToDevice, s);
+        const int64_t tc = out->tl_capacity < w.Cmax ? out->tl_capacity : w.Cmax;
+        if (tc > 0) {
+            if (out->tl_params) cudaMemcpyAsync(out->tl_params, w.tl_par, sizeof(float) * 5 * tc, cudaMemcpyDeviceToDevice, s);
+            if (out->tl_cov) cudaMemcpyAsync(out->tl_cov, w.tl_cov, sizeof(float) * 15 * tc, cudaMemcpyDeviceToDevice, s);
+            if (out->tl_chi2) cudaMemcpyAsync(out->tl_chi2, w.tl_chi2, sizeof(float) * tc, cudaMemcpyDeviceToDevice, s);
+            if (out->tl_nhits) cudaMemcpyAsync(out->tl_nhits, w.tl_nhits, sizeof(int32_t) * tc, cudaMemcpyDeviceToDevice, s);
+            launches += launch_export_tracklets(g, w, p, out->tl_hits, out->tl_rows, tc, s);
+        }
+    }
+    t->last_launches = launches;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, std::string("CUDA: ") + cudaGetErrorString(e));
+    return TPC_OK;
+}
+
+extern "C" int tpc_check_counts(const int64_t* c, const tpc_output_t* out) {
+    if (!c || !out) return TPC_ERR_ARG;
+    if (c[5] != 0) return TPC_ERR_INPUT;
+    if (out->start_hits && c[0] > out->start_capacity) return TPC_ERR_CAPACITY;
+    if ((out->cand_hits || out->cand_n) && c[1] > out->cand_capacity) return TPC_ERR_CAPACITY;
+    if ((out->tl_params || out->tl_cov || out->tl_chi2 || out->tl_nhits || out->tl_rows || out->tl_hits) &&
+        c[1] > out->tl_capacity)
+        return TPC_ERR_CAPACITY;
+    if (c[3] > out->trk_capacity && (out->trk_params || out->trk_cov || out->trk_chi2 || out->trk_xref ||
+                                     out->trk_cand_id || out->trk_nhits || out->trk_sector || out->trk_hit_offset ||
+                                     out->trk_hits || out->cluster_owner))
+        return TPC_ERR_CAPACITY;
+    if (out->trk_hits && c[4] > out->trk_hits_capacity) return TPC_ERR_CAPACITY;
+    return TPC_OK;
+}
+
+extern "C" int32_t tpc_last_launch_count(const tpc_tracker_t* t) { return t ? t->last_launches : 0; }
+
+extern "C" const char* tpc_last_error(const tpc_tracker_t* t) { return t ? t->err.c_str() : g_create_err.c_str(); }

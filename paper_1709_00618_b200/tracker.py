@@ -1,0 +1,295 @@
+"""Thin Python binding of libtpctrk.so (include/tpc_tracker.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the hot path runs in the library's CUDA kernels.
+There is no fallback: if the shared library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtpctrk.so")
+
+CAND_MAX_HITS = 10
+N_COUNTS = 8
+N_STAGES = 6
+STAGE_NAMES = ("bin", "neighbours", "clean", "chains", "follow", "select")
+ERRORS = {-1: "TPC_ERR_ARG", -2: "TPC_ERR_GEOMETRY", -3: "TPC_ERR_WORKSPACE", -4: "TPC_ERR_CUDA",
+          -5: "TPC_ERR_CAPACITY", -6: "TPC_ERR_INPUT"}
+
+EXPORTS = ("tpc_tracker_create", "tpc_tracker_destroy", "tpc_workspace_bytes", "tpc_set_workspace", "tpc_set_stream",
+           "tpc_track_sectors", "tpc_check_counts", "tpc_last_launch_count", "tpc_set_stage_timing",
+           "tpc_stage_times_ms", "tpc_last_error")
+
+
+class TpcError(RuntimeError):
+    pass
+
+
+class Params(C.Structure):
+    _fields_ = [("nf_win_y", C.c_float), ("nf_win_z", C.c_float), ("nf_d2_max", C.c_float),
+                ("cand_min_hits", C.c_int32), ("cand_max_hits", C.c_int32), ("kf_p0", C.c_float * 5),
+                ("kf_gate_sigma", C.c_float), ("kf_win_max", C.c_float), ("kf_max_gap", C.c_int32),
+                ("kf_max_sinphi", C.c_float), ("kf_edge_margin", C.c_float), ("sel_min_hits", C.c_int32),
+                ("grid_cell_z", C.c_float)]
+
+
+class Geometry(C.Structure):
+    _fields_ = [("n_rows", C.c_int32), ("row_x", C.POINTER(C.c_float)), ("sectors_per_event", C.c_int32),
+                ("half_angle_rad", C.c_float), ("z_lo", C.c_float), ("z_hi", C.c_float), ("sigma_y", C.c_float),
+                ("sigma_z", C.c_float), ("params", Params)]
+
+
+_OUT_PTRS = ("link_up_raw", "link_dn_raw", "link_up", "link_dn")
+
+
+class Output(C.Structure):
+    _fields_ = [("link_up_raw", C.c_void_p), ("link_dn_raw", C.c_void_p), ("link_up", C.c_void_p),
+                ("link_dn", C.c_void_p), ("start_hits", C.c_void_p), ("start_capacity", C.c_int64),
+                ("cand_hits", C.c_void_p), ("cand_n", C.c_void_p), ("cand_capacity", C.c_int64),
+                ("tl_params", C.c_void_p), ("tl_cov", C.c_void_p), ("tl_chi2", C.c_void_p), ("tl_nhits", C.c_void_p),
+                ("tl_rows", C.c_void_p), ("tl_hits", C.c_void_p), ("tl_capacity", C.c_int64),
+                ("trk_params", C.c_void_p), ("trk_cov", C.c_void_p), ("trk_chi2", C.c_void_p),
+                ("trk_xref", C.c_void_p), ("trk_cand_id", C.c_void_p), ("trk_nhits", C.c_void_p),
+                ("trk_sector", C.c_void_p), ("trk_hit_offset", C.c_void_p), ("trk_hits", C.c_void_p),
+                ("trk_capacity", C.c_int64), ("trk_hits_capacity", C.c_int64), ("cluster_owner", C.c_void_p),
+                ("counts", C.c_void_p)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libtpctrk.so and declare the prototypes.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise TpcError(f"{LIB_PATH} not found: build it with `python -m paper_1709_00618_b200.build` "
+                       "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    lib.tpc_tracker_create.argtypes = [C.POINTER(Geometry), C.c_float, C.POINTER(C.c_void_p)]
+    lib.tpc_tracker_create.restype = C.c_int
+    lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
+    lib.tpc_tracker_destroy.restype = None
+    lib.tpc_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int64]
+    lib.tpc_workspace_bytes.restype = C.c_size_t
+    lib.tpc_set_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
+    lib.tpc_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+    lib.tpc_track_sectors.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.POINTER(Output)]
+    lib.tpc_check_counts.argtypes = [C.POINTER(C.c_int64), C.POINTER(Output)]
+    lib.tpc_last_launch_count.argtypes = [C.c_void_p]
+    lib.tpc_last_launch_count.restype = C.c_int32
+    lib.tpc_set_stage_timing.argtypes = [C.c_void_p, C.c_int32]
+    lib.tpc_stage_times_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    lib.tpc_last_error.argtypes = [C.c_void_p]
+    lib.tpc_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def make_geometry(row_x: np.ndarray, *, z_lo=0.0, z_hi=250.0, sigma_y=0.1, sigma_z=0.1, sectors_per_event=36,
+                  half_angle_rad=float(np.deg2rad(10.0)), **params):
+    """Returns (Geometry, keep-alive row_x array).  Unknown tunables raise; omitted ones take the defaults."""
+    rx = np.ascontiguousarray(row_x, dtype=np.float32)
+    g = Geometry()
+    g.n_rows = len(rx)
+    g.row_x = rx.ctypes.data_as(C.POINTER(C.c_float))
+    g.sectors_per_event = sectors_per_event
+    g.half_angle_rad = half_angle_rad
+    g.z_lo, g.z_hi, g.sigma_y, g.sigma_z = z_lo, z_hi, sigma_y, sigma_z
+    names = {f[0] for f in Params._fields_}
+    for k, v in params.items():
+        if k not in names:
+            raise TypeError(f"unknown tracker parameter {k!r}")
+        if k == "kf_p0":
+            for i in range(5):
+                g.params.kf_p0[i] = v[i]
+        else:
+            setattr(g.params, k, v)
+    return g, rx
+
+
+@dataclass
+class TrackResult:
+    """Host copies (numpy) of one call's outputs; fields not requested are None."""
+    counts: np.ndarray
+    link_up_raw: np.ndarray = None
+    link_dn_raw: np.ndarray = None
+    link_up: np.ndarray = None
+    link_dn: np.ndarray = None
+    start_hits: np.ndarray = None
+    cand_hits: np.ndarray = None
+    cand_n: np.ndarray = None
+    tl_params: np.ndarray = None
+    tl_cov: np.ndarray = None
+    tl_chi2: np.ndarray = None
+    tl_nhits: np.ndarray = None
+    tl_rows: np.ndarray = None
+    tl_hits: np.ndarray = None
+    trk_params: np.ndarray = None
+    trk_cov: np.ndarray = None
+    trk_chi2: np.ndarray = None
+    trk_xref: np.ndarray = None
+    trk_cand_id: np.ndarray = None
+    trk_nhits: np.ndarray = None
+    trk_sector: np.ndarray = None
+    trk_hit_offset: np.ndarray = None
+    trk_hits: np.ndarray = None
+    cluster_owner: np.ndarray = None
+
+    @property
+    def n_start(self): return int(self.counts[0])
+    @property
+    def n_cand(self): return int(self.counts[1])
+    @property
+    def n_tracklets(self): return int(self.counts[2])
+    @property
+    def n_tracks(self): return int(self.counts[3])
+    @property
+    def n_track_hits(self): return int(self.counts[4])
+
+
+class Tracker:
+    """tpc_tracker_create(geometry, Bz) + workspace/stream plumbing with torch tensors."""
+
+    def __init__(self, row_x, bz, *, device="cuda:0", **geom_kw):
+        import torch
+        if not torch.cuda.is_available():
+            raise TpcError("no CUDA device: the TPC tracker has no CPU path")
+        self._torch = torch
+        self.device = torch.device(device)
+        self.lib = load_library()
+        self.n_rows = len(row_x)
+        geom, self._rx = make_geometry(row_x, **geom_kw)
+        h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            rc = self.lib.tpc_tracker_create(C.byref(geom), C.c_float(bz), C.byref(h))
+        if rc != 0:
+            raise TpcError(f"tpc_tracker_create: {ERRORS.get(rc, rc)}: {self.lib.tpc_last_error(None).decode()}")
+        self._h = h
+        self._ws = None
+        self._out_keep = None
+
+    @classmethod
+    def for_event(cls, ev, **kw):
+        from . import datagen
+        return cls(datagen.row_x(ev.n_rows), ev.bz, z_lo=ev.z_lo, z_hi=ev.z_hi, sigma_y=ev.sigma_y,
+                   sigma_z=ev.sigma_z, **kw)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.tpc_tracker_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise TpcError(f"{what}: {ERRORS.get(rc, rc)}: {self.lib.tpc_last_error(self._h).decode()}")
+
+    def workspace_bytes(self, max_clusters, max_inst):
+        return int(self.lib.tpc_workspace_bytes(self._h, int(max_clusters), int(max_inst)))
+
+    def reserve(self, max_clusters, max_inst):
+        """Allocate (with torch) and attach a workspace large enough for these sizes."""
+        need = self.workspace_bytes(max_clusters, max_inst)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = self._torch.empty(need, dtype=self._torch.uint8, device=self.device)
+        self._check(self.lib.tpc_set_workspace(self._h, C.c_void_p(self._ws.data_ptr()), self._ws.numel()),
+                    "tpc_set_workspace")
+
+    def set_stream(self, stream=None):
+        s = stream if stream is not None else self._torch.cuda.current_stream(self.device)
+        self._check(self.lib.tpc_set_stream(self._h, C.c_void_p(s.cuda_stream)), "tpc_set_stream")
+
+    def set_stage_timing(self, enable=True):
+        self._check(self.lib.tpc_set_stage_timing(self._h, 1 if enable else 0), "tpc_set_stage_timing")
+
+    def stage_times_ms(self):
+        buf = (C.c_float * N_STAGES)()
+        self._check(self.lib.tpc_stage_times_ms(self._h, buf), "tpc_stage_times_ms")
+        return dict(zip(STAGE_NAMES, [float(x) for x in buf]))
+
+    @property
+    def last_launch_count(self):
+        return int(self.lib.tpc_last_launch_count(self._h))
+
+    # ---- device-level call: torch tensors in, torch tensors out, asynchronous ------------------------------------
+    def alloc_outputs(self, n_clusters, *, debug=False, cand_capacity=None, trk_capacity=None):
+        """Device output buffers as a dict of torch tensors (+ the ctypes struct).  debug=True adds every parity array."""
+        t = self._torch
+        dev = self.device
+        n = max(int(n_clusters), 1)
+        cc = int(cand_capacity if cand_capacity is not None else n // 4 + 1)
+        tc = int(trk_capacity if trk_capacity is not None else n // 10 + 1)
+        i32, f32, i64 = t.int32, t.float32, t.int64
+        bufs = dict(counts=t.zeros(N_COUNTS, dtype=i64, device=dev),
+                    trk_params=t.empty((tc, 5), dtype=f32, device=dev), trk_cov=t.empty((tc, 15), dtype=f32, device=dev),
+                    trk_chi2=t.empty(tc, dtype=f32, device=dev), trk_xref=t.empty(tc, dtype=f32, device=dev),
+                    trk_cand_id=t.empty(tc, dtype=i32, device=dev), trk_nhits=t.empty(tc, dtype=i32, device=dev),
+                    trk_sector=t.empty(tc, dtype=i32, device=dev), trk_hit_offset=t.empty(tc + 1, dtype=i64, device=dev),
+                    trk_hits=t.empty(n, dtype=i32, device=dev), cluster_owner=t.empty(n, dtype=i32, device=dev))
+        if debug:
+            for k in _OUT_PTRS:
+                bufs[k] = t.empty(n, dtype=i32, device=dev)
+            bufs.update(start_hits=t.empty(n, dtype=i32, device=dev),
+                        cand_hits=t.empty((cc, CAND_MAX_HITS), dtype=i32, device=dev),
+                        cand_n=t.empty(cc, dtype=i32, device=dev),
+                        tl_params=t.empty((cc, 5), dtype=f32, device=dev), tl_cov=t.empty((cc, 15), dtype=f32, device=dev),
+                        tl_chi2=t.empty(cc, dtype=f32, device=dev), tl_nhits=t.empty(cc, dtype=i32, device=dev),
+                        tl_rows=t.empty((cc, 3), dtype=i32, device=dev),
+                        tl_hits=t.empty((cc, self.n_rows), dtype=i32, device=dev))
+        o = Output()
+        for k, v in bufs.items():
+            setattr(o, k, v.data_ptr())
+        o.start_capacity = n if debug else 0
+        o.cand_capacity = cc if debug else 0
+        o.tl_capacity = cc if debug else 0
+        o.trk_capacity = tc
+        o.trk_hits_capacity = n
+        return bufs, o
+
+    def track_sectors_device(self, clusters, row_offsets, n_inst, out_struct):
+        """tpc_track_sectors on device tensors (float32 [N,4], int32 [n_inst*R+1]); asynchronous."""
+        n = int(clusters.shape[0])
+        self._check(self.lib.tpc_track_sectors(self._h, C.c_void_p(clusters.data_ptr()),
+                                               C.c_void_p(row_offsets.data_ptr()), int(n_inst), n,
+                                               C.byref(out_struct)), "tpc_track_sectors")
+
+    # ---- convenience: numpy in, numpy out (used by the parity tests) ----------------------------------------------
+    def track_sectors(self, clusters: np.ndarray, row_offsets: np.ndarray, n_inst: int, *, debug=False,
+                      cand_capacity=None, trk_capacity=None) -> TrackResult:
+        t = self._torch
+        cl = t.from_numpy(np.ascontiguousarray(clusters, np.float32).reshape(-1, 4)).to(self.device)
+        ro = t.from_numpy(np.ascontiguousarray(row_offsets, np.int32)).to(self.device)
+        n = int(cl.shape[0])
+        with t.cuda.device(self.device):
+            self.reserve(n, n_inst)
+            self.set_stream()
+            bufs, o = self.alloc_outputs(n, debug=debug, cand_capacity=cand_capacity, trk_capacity=trk_capacity)
+            self.track_sectors_device(cl, ro, n_inst, o)
+            t.cuda.synchronize(self.device)
+        counts = bufs["counts"].cpu().numpy()
+        cnt = (C.c_int64 * N_COUNTS)(*[int(x) for x in counts])
+        rc = self.lib.tpc_check_counts(cnt, C.byref(o))
+        if rc != 0:
+            raise TpcError(f"tpc_check_counts: {ERRORS.get(rc, rc)} counts={counts.tolist()}")
+        res = TrackResult(counts=counts)
+        nt, nh, nc, ns = res.n_tracks, res.n_track_hits, res.n_cand, res.n_start
+        cut = dict(trk_params=nt, trk_cov=nt, trk_chi2=nt, trk_xref=nt, trk_cand_id=nt, trk_nhits=nt, trk_sector=nt,
+                   trk_hit_offset=nt + 1, trk_hits=nh, cluster_owner=n, link_up_raw=n, link_dn_raw=n, link_up=n,
+                   link_dn=n, start_hits=ns, cand_hits=nc, cand_n=nc, tl_params=nc, tl_cov=nc, tl_chi2=nc, tl_nhits=nc,
+                   tl_rows=nc, tl_hits=nc)
+        for k, v in bufs.items():
+            if k != "counts":
+                setattr(res, k, v[:cut[k]].cpu().numpy())
+        return res

@@ -1,0 +1,78 @@
+"""GPU-vs-oracle comparison helpers (tests only).  The oracle is oracle/tpc_oracle.c; the GPU path is reached only
+through the C ABI (paper_1709_00618_b200.tracker)."""
+import numpy as np
+
+from oracle.tpc_oracle import Oracle
+
+# BASELINE.json north_star: "matched tracks must have fitted parameters within 1e-3 relative / 1e-4 absolute".
+PAR_RTOL = 1e-3
+PAR_ATOL = 1e-4
+MIN_SHARED = 0.995  # ">= 99.5 % of hit assignments" shared with the oracle
+
+
+def run_oracle(ev, **kw):
+    o = Oracle.for_event(ev, **kw)
+    return o.track(ev.clusters, ev.row_offsets, ev.n_inst)
+
+
+def assert_ca_bit_exact(g, o):
+    """S2, S3, S4: integer results are unique -> bit-exact."""
+    assert np.array_equal(g.link_up_raw, o.link_up_raw), "raw up links differ"
+    assert np.array_equal(g.link_dn_raw, o.link_dn_raw), "raw down links differ"
+    assert np.array_equal(g.link_up, o.link_up), "cleaned up links differ"
+    assert np.array_equal(g.link_dn, o.link_dn), "cleaned down links differ"
+    assert np.array_equal(g.start_hits, o.start_hits), "start hits differ"
+    assert g.n_start == len(o.start_hits) and g.n_cand == len(o.cand_n)
+    assert np.array_equal(g.cand_n, o.cand_n), "candidate lengths differ"
+    assert np.array_equal(g.cand_hits, o.cand_hits), "candidate hit lists differ"
+
+
+def tracklet_report(g, o):
+    """S5 comparison per candidate id (ids are identical on both sides because candidates are bit-exact)."""
+    ok_o = o.tracklets["ok"].astype(bool)
+    ok_g = g.tl_nhits > 0
+    both = ok_o & ok_g
+    same_hits = np.all(g.tl_hits == o.tracklet_hits, axis=1)
+    att_o = o.tracklet_hits >= 0
+    shared = ((g.tl_hits == o.tracklet_hits) & att_o)[both].sum()
+    total = max(att_o[both].sum(), (g.tl_hits >= 0)[both].sum())
+    ident = both & same_hits
+    po = o.tracklets["p"][ident]
+    pg = g.tl_params[ident].astype(np.float64)
+    excess = np.abs(pg - po) / (PAR_ATOL + PAR_RTOL * np.abs(po))  # <= 1 means inside the tolerance
+    return dict(n_cand=len(ok_o), ok_mismatch=int((ok_o != ok_g).sum()), identical_hit_lists=int(ident.sum()),
+                n_both=int(both.sum()), shared_frac=float(shared / max(total, 1)),
+                worst_param_excess=float(excess.max()) if excess.size else 0.0,
+                worst_by_param=excess.max(axis=0).tolist() if excess.size else [0.0] * 5,
+                nhits_equal=bool(np.array_equal(g.tl_nhits[ident], o.tracklets["nhits"][ident])),
+                rows_equal=bool(np.array_equal(g.tl_rows[ident][:, 0], o.tracklets["first_row"][ident])
+                                and np.array_equal(g.tl_rows[ident][:, 1], o.tracklets["last_row"][ident])))
+
+
+def final_track_report(g, o, n_clusters):
+    """S6: share of identical final cluster->track assignments, with tracks matched by candidate id."""
+    own_g = np.full(n_clusters, -1, np.int64)
+    own_o = np.full(n_clusters, -1, np.int64)
+    m = g.cluster_owner >= 0
+    own_g[m] = g.trk_cand_id[g.cluster_owner[m]]
+    m = o.cluster_owner >= 0
+    own_o[m] = o.trk_cand[o.cluster_owner[m]]
+    assigned = (own_g >= 0) | (own_o >= 0)
+    same = (own_g == own_o) & assigned
+    return dict(n_tracks_gpu=int(g.n_tracks), n_tracks_oracle=int(len(o.trk_cand)),
+                shared_assign_frac=float(same.sum() / max(assigned.sum(), 1)),
+                tracks_identical=bool(np.array_equal(g.trk_cand_id, o.trk_cand)))
+
+
+def assert_final_consistency(g, n_clusters):
+    """Internal consistency of the S6 outputs (holds at any size)."""
+    nt = g.n_tracks
+    off = g.trk_hit_offset
+    assert off[0] == 0 and off[nt] == g.n_track_hits and np.all(np.diff(off) == g.trk_nhits)
+    assert np.all(g.trk_nhits >= 10)
+    assert np.all(np.diff(g.trk_cand_id) > 0)
+    owner = g.cluster_owner
+    assert owner.shape[0] == n_clusters
+    trk_of_hit = np.repeat(np.arange(nt), g.trk_nhits)
+    assert np.array_equal(owner[g.trk_hits], trk_of_hit)
+    assert (owner >= 0).sum() == g.n_track_hits  # every owned cluster is listed exactly once
