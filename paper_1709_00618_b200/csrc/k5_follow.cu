@@ -16,6 +16,7 @@ struct FollowCtx {
     int slab_base;       // instance * R
     float z0;
     const float* s_rowx; // shared [R]
+    float yref, zref;    // the filter state holds (y - yref, z - zref): see follow_kernel
 };
 
 // Nearest cluster of the row inside the gate around the predicted (y,z); ties -> lowest local index.
@@ -65,14 +66,15 @@ __device__ __forceinline__ int follow_dir(const DevGeom& g, const FollowCtx& cx,
         const float xr = cx.s_rowx[rn];
         if (!kf_transport(st, xr - cx.s_rowx[r], g.cB, g.max_s)) break;
         r = rn;
-        if (fabsf(st.y) > fmaf(xr, g.tan_half, g.edge_margin)) break;
+        const float yp = st.y + cx.yref, zp = st.z + cx.zref;
+        if (fabsf(yp) > fmaf(xr, g.tan_half, g.edge_margin)) break;
         const float wy = fminf(g.wmax, g.gate * sqrtf(st.c00 + g.sy2));
         const float wz = fminf(g.wmax, g.gate * sqrtf(st.c11 + g.sz2));
         float ym, zm;
-        const int j = pick_up(g, cx, r, st.y, st.z, wy, wz, ym, zm);
+        const int j = pick_up(g, cx, r, yp, zp, wy, wz, ym, zm);
         if (j >= 0) {
             rowhit[r] = cx.hit_idx[cx.ro[r] + j];
-            chi2 += kf_update(st, ym, zm, g.sy2, g.sz2);
+            chi2 += kf_update(st, ym - cx.yref, zm - cx.zref, g.sy2, g.sz2);
             nhits++;
             gap = 0;
             last_hit_row = r;
@@ -116,9 +118,14 @@ follow_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clus
         // seed from hits 0, n/2, n-1
         const int i1 = n >> 1, i2 = n - 1;
         const float4 h0 = __ldg(&clusters[ch[0]]), h1 = __ldg(&clusters[ch[i1]]), h2 = __ldg(&clusters[ch[i2]]);
+        // The state carries y and z relative to the first candidate hit.  The model is translation invariant in y
+        // and z, so this is exact; it keeps the fp32 rounding of the two coordinates (ulp(20 cm), ulp(250 cm)) out
+        // of q/pt and sinPhi, whose sensitivity to position noise is ~50/cm on 10-row tracklets.
+        cx.yref = h0.y;
+        cx.zref = h0.z;
         KfState st;
-        if (!kf_seed(st, s_rowx[r0], h0.y, h0.z, s_rowx[r0 + i1], h1.y, s_rowx[r0 + i2], h2.y, h2.z, g.cB, g.max_s,
-                     g.p0))
+        if (!kf_seed(st, s_rowx[r0], 0.0f, 0.0f, s_rowx[r0 + i1], h1.y - cx.yref, s_rowx[r0 + i2], h2.y - cx.yref,
+                     h2.z - cx.zref, g.cB, g.max_s, g.p0))
             continue;
         float chi2 = 0.0f;
         int nhits = 0;
@@ -131,7 +138,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clus
                 break;
             }
             const float4 h = __ldg(&clusters[hg]);
-            chi2 += kf_update(st, h.y, h.z, g.sy2, g.sz2);
+            chi2 += kf_update(st, h.y - cx.yref, h.z - cx.zref, g.sy2, g.sz2);
             rowhit[r0 + i] = (uint16_t)(hg - cx.ro[r0 + i]);
             nhits++;
         }
@@ -145,7 +152,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clus
         int first_row = r0;
         follow_dir<-1>(g, cx, st, r0, chi2, nhits, first_row, rowhit, &rep);
         float* p = tl_par + c * 5;
-        p[0] = rep.y; p[1] = rep.z; p[2] = rep.s; p[3] = rep.t; p[4] = rep.k;
+        p[0] = rep.y + cx.yref; p[1] = rep.z + cx.zref; p[2] = rep.s; p[3] = rep.t; p[4] = rep.k;
         float* q = tl_cov + c * 15;
         q[0] = rep.c00; q[1] = rep.c10; q[2] = rep.c11; q[3] = rep.c20; q[4] = rep.c21; q[5] = rep.c22; q[6] = rep.c30;
         q[7] = rep.c31; q[8] = rep.c32; q[9] = rep.c33; q[10] = rep.c40; q[11] = rep.c41; q[12] = rep.c42;

@@ -42,13 +42,19 @@ __device__ __forceinline__ bool kf_transport(KfState& st, float dx, float cB, fl
     const float f04 = cB * dx * dx * sec2 * 0.5f * ic1;
     const float f12 = t * dx * tg * ic0 * ic1;
     const float f13 = dS;
-    float ddS;  // d(dS)/d(kappa) = (dx/c1 - dS)/kappa; cancels for small kappa*dx -> 2/3-point series there
-    if (fabsf(kdx) > 0.02f) {
-        ddS = (dx * ic1 - dS) / kap;
+    // d(dS)/d(kappa) = (dx/c1 - dS)/kappa.  That difference cancels for small kappa*dx, and this entry steers q/pt
+    // through the z residuals, so it is evaluated in a cancellation-free form: with m the chord direction
+    // (tan m = tg), h = kappa dS / 2 the half turning angle,
+    //   dx/c1 - dS = 2 [cos m (sin h - h cos h) + h sin m sin h] / (kappa c1),
+    // and sin h - h cos h = h^3/3 (1 - h^2/10 + h^4/280 - h^6/15120 ...).  Dividing by kappa analytically:
+    //   ddS = [tg dx dS / 2 + kappa dS^3 / (12 sqrt(sec2)) (1 - h^2/10 + ...)] / c1.
+    float ddS;
+    const float hh = 0.5f * kap * dS, h2 = hh * hh;
+    if (h2 < 0.09f) {
+        const float ser = 1.0f + h2 * (-0.1f + h2 * (1.0f / 280.0f - h2 * (1.0f / 15120.0f)));
+        ddS = (0.5f * tg * dx * dS + kap * dS * dS * dS * (1.0f / 12.0f) * rsqrtf(sec2) * ser) * ic1;
     } else {
-        const float se = fmaf(2.0f / 3.0f, kdx, s);
-        const float ice = rsqrtf((1.0f - se) * (1.0f + se));
-        ddS = 0.5f * dx * dx * se * ice * ice * ice;
+        ddS = (dx * ic1 - dS) / kap;
     }
     const float f14 = cB * t * ddS;
     const float f24 = cB * dx;
