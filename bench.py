@@ -1,0 +1,319 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the TPC sector tracker on the synthetic drift-window workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--windows NW] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (S1..S6, one tpc_track_sectors call) over one batch of NW CFG:4 drift
+windows (BASELINE.json configs[3]/[4]: 5 overlapping Pb-Pb events per window; 36*NW independent sector instances).
+`value` = clusters/s with the inputs resident in HBM; `e2e` = the same metric through tpc_track_sectors_host with
+pinned HOST buffers (upload, tracking and result download inside the timed region).
+N > 1 (torchrun): every rank tracks its own NW windows (weak scaling, no data-path collective).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1709_00618_b200 import datagen  # noqa: E402
+
+METRIC = "TPC clusters/sec tracked on 1 B200 (ms/event); achieved HBM GB/s vs peak"
+UNIT = "clusters/s"
+# algorithmic bytes the staged method moves per cluster (whole path / S5 only)
+BYTES_PER_CLUSTER_PATH = 130.0
+BYTES_PER_CLUSTER_S5 = 34.0
+# fp32 operations per unit of S5 work, counted from the formulas in csrc/kf_math.cuh
+FLOP_TRANSPORT, FLOP_UPDATE, FLOP_EXAMINE, FLOP_SEARCH = 150.0, 93.0, 7.0, 18.0
+FP32_LANES_PER_SM, N_SM = 128, 148
+# dram bytes per launch of follow_kernel per cluster, from the committed ncu --set full capture (profiles/); None
+# until a capture exists
+FOLLOW_DRAM_BYTES_PER_CLUSTER = None
+
+
+def _gen_window(seed):
+    return datagen.drift_window(seed)
+
+
+def make_batch(n_windows, seed0):
+    """NW CFG:4 windows, generated in parallel worker processes (before CUDA is touched)."""
+    seeds = [seed0 + i for i in range(n_windows)]
+    n_proc = max(1, min(n_windows, (os.cpu_count() or 2) // max(1, int(os.environ.get("LOCAL_WORLD_SIZE", "1")))))
+    if n_proc > 1:
+        import multiprocessing as mp
+        with mp.get_context("fork").Pool(n_proc) as pool:
+            evs = pool.map(_gen_window, seeds)
+    else:
+        evs = [_gen_window(s) for s in seeds]
+    return evs, datagen.concat_events(evs, name=f"cfg5_batch{n_windows}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(index)], stdout=subprocess.PIPE, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append((time.time(), ln.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons, power = [], None, set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [l for (ts, l) in self.lines if t0 <= ts <= t1 + 0.2] or [l for (_, l) in self.lines[-3:]]
+        for l in rows:
+            f = [x.strip() for x in l.split(",")]
+            try:
+                sm.append(float(f[0])); smax = float(f[1]); power.append(float(f[2]))
+            except Exception:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "power_w_max": max(power) if power else None, "samples": len(sm)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+def cpu_baseline(evs, budget_windows=1):
+    """The oracle as it stands, on the host cores, on a bounded sample (first windows of the batch)."""
+    from oracle.tpc_oracle import Oracle
+    ev = datagen.concat_events(evs[:budget_windows]) if budget_windows > 1 else evs[0]
+    cores = min(os.cpu_count() or 1, ev.n_inst)
+    o = Oracle.for_event(ev)
+    t = time.perf_counter()
+    c = o.track_count(ev.clusters, ev.row_offsets, ev.n_inst, n_threads=cores)
+    dt = time.perf_counter() - t
+    return {"value": ev.n_clusters / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{budget_windows} drift window(s) of the batch, {ev.n_clusters} clusters, {ev.n_inst} sector "
+                      f"instances, one OpenMP thread per instance up to all cores, {dt:.2f} s",
+            "tracks": c["n_tracks"]}, dt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the same workload recipe, each step a bounded sample (one window)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    evs, _ = make_batch(1, args.seed0)
+    times = []
+    info = None
+    for i in range(args.warmup + args.steps):
+        info, dt = cpu_baseline(evs, 1)
+        if i >= args.warmup:
+            times.append(dt)
+    n = evs[0].n_clusters
+    v = n * len(times) / sum(times)
+    info["value"] = v
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64 (Kalman filter) / f32 (neighbour search)",
+            "data": "synthetic", "config": {"workload": "cfg4_drift_window (bounded sample: 1 window per step)",
+                                            "clusters_per_step": n, "seed0": args.seed0},
+            "cpu_baseline": info,
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    t_gen = time.time()
+    evs, batch = make_batch(args.windows, args.seed0 + rank * args.windows)  # before CUDA init (fork)
+    t_gen = time.time() - t_gen
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_1709_00618_b200 import Tracker, physics
+    from paper_1709_00618_b200.tracker import HostPipeline
+    N, S = batch.n_clusters, batch.n_inst
+    trk = Tracker.for_event(batch, device=f"cuda:{local}")
+    h_cl = torch.from_numpy(batch.clusters).pin_memory()
+    h_ro = torch.from_numpy(batch.row_offsets).pin_memory()
+    d_cl = h_cl.to(dev)
+    d_ro = h_ro.to(dev)
+    trk.reserve(N, S)
+    trk.set_stream()
+    trk.set_stage_timing(True)
+    bufs, out = trk.alloc_outputs(N, trk_capacity=N // 20 + 64)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        trk.track_sectors_device(d_cl, d_ro, S, out)
+    barrier()
+    sampler = ClockSampler(local)
+    time.sleep(0.25)
+    # One CUDA-event pair per step on the launching stream; the steps are queued back to back.  When the batch
+    # (inputs + intermediates) could sit in the 126 MB L2, a 512 MB buffer is rewritten between steps (outside the
+    # event pairs) so that every step starts cold.
+    flush = (16 * N < 2 * 126e6)
+    fbuf = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if flush else None
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t0 = time.time()
+    for a, b in ev:
+        if flush:
+            fbuf.fill_(1)
+        a.record()
+        trk.track_sectors_device(d_cl, d_ro, S, out)
+        b.record()
+    torch.cuda.synchronize(dev)
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    launches = trk.last_launch_count * args.steps
+    if world > 1:
+        tt = torch.tensor([ms], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+        nn = torch.tensor([N], device=dev, dtype=torch.int64)
+        dist.all_reduce(nn)
+        n_total = int(nn.item())
+    else:
+        n_total = N
+    ms_step = ms / args.steps
+    value = n_total / (ms_step * 1e-3)
+    counts = bufs["counts"].cpu().numpy()
+    # per-stage device times of the timed calls (CUDA events recorded by the library on the launching stream)
+    k = min(args.steps, 32)
+    st = [trk.stage_times_ms(a) for a in range(k)]
+    stage_ms = {nme: float(np.mean([s[nme] for s in st])) for nme in st[0]}
+
+    # ---- end to end through the host-buffer entry point -------------------------------------------------------------
+    ipc = 36 * max(1, args.chunk_windows)
+    max_chunk = max(int(batch.row_offsets[min(i + ipc, S) * batch.n_rows] - batch.row_offsets[i * batch.n_rows])
+                    for i in range(0, S, ipc))
+    pipe = HostPipeline(trk, max_chunk, ipc, N, n_slots=args.slots)
+    trk.set_stage_timing(False)
+    for _ in range(max(1, min(args.warmup, 2))):
+        ho = pipe.run(h_cl, h_ro, S)
+    barrier()
+    tw = time.perf_counter()
+    for _ in range(args.steps):
+        ho = pipe.run(h_cl, h_ro, S)
+    torch.cuda.synchronize(dev)
+    e2e_ms = (time.perf_counter() - tw) * 1e3
+    if world > 1:
+        tt = torch.tensor([e2e_ms], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_ms = float(tt.item())
+    e2e_value = n_total / (e2e_ms / args.steps * 1e-3)
+    e2e_tracks = int(ho.totals[3])
+    launches_e2e = int(ho.n_launches)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    hbm_peak, sm_max, peak_src = measured_peaks()
+    fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12  # TFLOP/s
+    flops = (counts[6] * FLOP_TRANSPORT + counts[7] * FLOP_UPDATE + counts[8] * FLOP_EXAMINE + counts[9] * FLOP_SEARCH)
+    t_follow = stage_ms["follow"] * 1e-3
+    ach = flops / t_follow / 1e12
+    roof = {"kernel": "follow_kernel (S5 Kalman track following)", "bound": "alu", "achieved": ach, "peak": fp32_peak,
+            "unit": "TFLOP/s", "frac": ach / fp32_peak,
+            "traffic": None if FOLLOW_DRAM_BYTES_PER_CLUSTER is None else FOLLOW_DRAM_BYTES_PER_CLUSTER * N,
+            "peak_source": f"148 SM x 128 fp32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md)",
+            "avg_launch_ms": stage_ms["follow"], "share_of_step": stage_ms["follow"] / sum(stage_ms.values()),
+            "algorithmic_flop_per_launch": float(flops),
+            "work": {"transports": int(counts[6]), "updates": int(counts[7]), "clusters_examined": int(counts[8]),
+                     "searches": int(counts[9]), "row_steps_per_cluster": float(counts[6]) / N},
+            "hbm_view": {"bytes_per_cluster": BYTES_PER_CLUSTER_S5,
+                         "achieved_gbs": BYTES_PER_CLUSTER_S5 * N / t_follow / 1e9,
+                         "frac_of_hbm_peak": BYTES_PER_CLUSTER_S5 * N / t_follow / 1e9 / hbm_peak}}
+    path_gbs = BYTES_PER_CLUSTER_PATH * N / (ms_step * 1e-3) / 1e9
+    roof_path = {"bound": "hbm", "achieved": path_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": path_gbs / hbm_peak,
+                 "bytes_per_cluster_model": BYTES_PER_CLUSTER_PATH, "peak_source": peak_src,
+                 "frac_of_nominal_8TBs": path_gbs / 8000.0}
+    cpu, _ = cpu_baseline(evs, 1) if world == 1 else (None, 0)
+    own = bufs["cluster_owner"][:evs[0].n_clusters].cpu().numpy()
+    n_trk0 = int(own.max()) + 1 if (own >= 0).any() else 0
+    phys = physics.report(evs[0], own, n_trk0)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"cfg5 throughput batch: {args.windows} CFG:4 drift windows per GPU "
+                                   "(5 overlapping Pb-Pb-like events each) in one call",
+                       "windows_per_gpu": args.windows, "sector_instances_per_gpu": S, "clusters_per_gpu": N,
+                       "ms_per_window": ms_step / args.windows, "seed0": args.seed0,
+                       "l2": (f"inputs are {16 * N / 1e6:.0f} MB of float4; " +
+                              ("L2 flushed (512 MB write) before every timed step" if flush else
+                               "larger than twice the 126 MB L2, steps run back to back without a flush")),
+                       "generation_s": round(t_gen, 1)},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(ho.h2d_bytes),
+                    "d2h_bytes_per_step": int(ho.d2h_bytes), "ms_per_step": e2e_ms / args.steps,
+                    "chunks": int(ho.n_chunks), "slots": args.slots, "gpu_launches_per_step": launches_e2e,
+                    "tracks": e2e_tracks, "timer": "host perf_counter around the blocking C-ABI calls"},
+            "roofline": roof, "roofline_path_hbm": roof_path, "cpu_baseline": cpu,
+            "stage_ms": stage_ms,
+            "results": {"candidates": int(counts[1]), "tracklets": int(counts[2]), "tracks": int(counts[3]),
+                        "track_hits": int(counts[4]), "error_flags": int(counts[5])},
+            "physics_window0": phys}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--windows", type=int, default=16, help="CFG:4 drift windows per GPU and step")
+    ap.add_argument("--chunk-windows", type=int, default=2, help="windows per upload chunk in the e2e pipeline")
+    ap.add_argument("--slots", type=int, default=3)
+    ap.add_argument("--seed0", type=int, default=5001)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

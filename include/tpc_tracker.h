@@ -39,7 +39,7 @@ extern "C" {
 #define TPC_ERR_INPUT (-6)     /* tpc_check_counts: device-side input validation failed (row too long, ...) */
 
 #define TPC_CAND_MAX_HITS 10   /* stride of cand_hits (reading A7: "usually 4 to 10 hits") */
-#define TPC_N_COUNTS 8
+#define TPC_N_COUNTS 16
 
 typedef struct tpc_tracker tpc_tracker_t; /* opaque, library-owned */
 
@@ -109,7 +109,9 @@ typedef struct {
     int64_t trk_capacity, trk_hits_capacity;
     int32_t* cluster_owner; /* [n_clusters] final track index or -1 */
     /* device [TPC_N_COUNTS]: 0 n_start, 1 n_cand, 2 n_tracklets, 3 n_tracks, 4 n_track_hits,
-       5 input error flags (bit0: a row holds > 65535 clusters; bit1: > 2^23 candidates in one instance), 6-7 reserved.
+       5 input error flags (bit0: a row holds > 65535 clusters; bit1: > 2^23 candidates in one instance),
+       6 S5 transport steps executed, 7 S5 measurement updates, 8 clusters examined by the S5 pick-up search,
+       9 S5 pick-up searches (work counters for the roofline arithmetic), 10-15 reserved.
        Written by the last kernel of the call. */
     int64_t* counts;
 } tpc_output_t;
@@ -142,12 +144,51 @@ int tpc_check_counts(const int64_t* counts_host, const tpc_output_t* out);
 /* Number of kernel launches the last tpc_track_sectors call enqueued (for bench.py's gpu_launches). */
 int32_t tpc_last_launch_count(const tpc_tracker_t* t);
 
-/* Optional per-stage timing of later calls: event_pairs = 1 records CUDA events around every stage;
-   tpc_stage_times_ms synchronises the stream and returns the milliseconds of the last call in
-   out_ms[TPC_N_STAGES] (order: bin, neighbours, clean, chains, follow, select). */
+/* Optional per-stage timing: when enabled, every tpc_track_sectors call records CUDA events on its stream around
+   each stage (a ring of the last TPC_TIMING_RING calls).  tpc_stage_times_ms waits for the call `age` calls back
+   (0 = the last one) and returns its milliseconds in out_ms[TPC_N_STAGES]
+   (order: bin, neighbours, clean, chains, follow, select). */
 #define TPC_N_STAGES 6
+#define TPC_TIMING_RING 32
 int tpc_set_stage_timing(tpc_tracker_t* t, int32_t enable);
-int tpc_stage_times_ms(tpc_tracker_t* t, float* out_ms);
+int tpc_stage_times_ms(tpc_tracker_t* t, int32_t age, float* out_ms);
+
+/*
+ * Host-buffer entry point (BASELINE.json configs[4]: windows "streamed through the tracker in double-buffered
+ * chunks with cluster upload overlapped on a second CUDA stream").  The job is cut into chunks of
+ * inst_per_chunk sector instances; chunk i+1 is uploaded on h2d_stream while chunk i is tracked on
+ * compute_stream and the results of chunk i-1 return on d2h_stream.  Blocks until every result is on the host.
+ * h_clusters / h_row_offsets / the arrays in tpc_host_output_t should be pinned host memory (pageable memory
+ * works but serialises the copies).  Slots are caller-owned DEVICE buffers (allocate n_slots >= 2 of them); the
+ * workspace set by tpc_set_workspace is shared by all chunks and must cover the largest chunk.
+ */
+typedef struct {
+    float* clusters;      /* device [max_clusters][4] */
+    int32_t* row_offsets; /* device [max_instances * n_rows + 1] */
+    int64_t max_clusters;
+    int32_t max_instances;
+    tpc_output_t out;     /* device outputs of this slot: counts required; trk_* / cluster_owner as wanted */
+} tpc_slot_t;
+
+typedef struct {
+    /* HOST arrays for the whole job, NULL = not returned.  Indices are global: trk_hits hold positions in
+       h_clusters, cluster_owner holds positions in the job-wide track list, trk_sector the job-wide instance. */
+    float* trk_params;       /* [trk_capacity][5] */
+    float* trk_cov;          /* [trk_capacity][15] */
+    int32_t* trk_nhits;      /* [trk_capacity] */
+    int32_t* trk_sector;     /* [trk_capacity] */
+    int64_t* trk_hit_offset; /* [trk_capacity + 1] */
+    int32_t* trk_hits;       /* [trk_hits_capacity] */
+    int32_t* cluster_owner;  /* [n_clusters] */
+    int64_t trk_capacity, trk_hits_capacity;
+    int64_t totals[TPC_N_COUNTS]; /* written by the call: sums of the per-chunk counts */
+    int64_t n_chunks, n_launches, h2d_bytes, d2h_bytes; /* written by the call */
+} tpc_host_output_t;
+
+int tpc_track_sectors_host(tpc_tracker_t* t, const float* h_clusters_xyzw, const int32_t* h_row_offsets,
+                           int32_t n_sector_instances, int64_t n_clusters, int32_t inst_per_chunk,
+                           tpc_slot_t* slots, int32_t n_slots, void* h2d_stream, void* compute_stream,
+                           void* d2h_stream, tpc_host_output_t* hout);
 
 const char* tpc_last_error(const tpc_tracker_t* t);
 

@@ -26,6 +26,7 @@ SOURCES = {
     "k34_links_chains.cu": [],
     "k5_follow.cu": [],
     "k6_select.cu": [],
+    "host_pipeline.cu": [],
 }
 
 

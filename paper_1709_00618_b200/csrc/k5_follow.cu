@@ -19,15 +19,21 @@ struct FollowCtx {
     float yref, zref;    // the filter state holds (y - yref, z - zref): see follow_kernel
 };
 
+struct WorkCount {  // per-thread work counters (roofline arithmetic): summed into counts[6..9] at kernel end
+    unsigned transports, updates, examined, searches;
+};
+
 // Nearest cluster of the row inside the gate around the predicted (y,z); ties -> lowest local index.
 // Returns the sorted position (relative to the row start) or -1; (ym, zm) get its coordinates.
 __device__ __forceinline__ int pick_up(const DevGeom& g, const FollowCtx& cx, int r, float yp, float zp, float wy,
-                                       float wz, float& ym, float& zm) {
+                                       float wz, float& ym, float& zm, WorkCount& wc) {
     const int base = cx.ro[r];
     const uint16_t* tbl = cx.bin_start + (size_t)(cx.slab_base + r) * g.nzp;
     const float m = 1e-3f;  // bin margin: the visited bins are a superset of the rounded fp32 window test below
     const int b0 = zbin(zp - wz - m, cx.z0, g.inv_cz, g.nz), b1 = zbin(zp + wz + m, cx.z0, g.inv_cz, g.nz);
     const int j0 = tbl[b0], j1 = tbl[b1 + 1];
+    wc.searches++;
+    wc.examined += j1 - j0;
     int best = -1, best_idx = 0;
     float bd2 = 0.0f;
     const float2* yz = cx.hit_yz + base;
@@ -58,23 +64,25 @@ __device__ __forceinline__ int pick_up(const DevGeom& g, const FollowCtx& cx, in
 template <int STEP>
 __device__ __forceinline__ int follow_dir(const DevGeom& g, const FollowCtx& cx, KfState& st, int r, float& chi2,
                                           int& nhits, int& last_hit_row, uint16_t* __restrict__ rowhit,
-                                          KfState* at_hit) {
+                                          KfState* at_hit, WorkCount& wc) {
     int gap = 0;
     for (;;) {
         const int rn = r + STEP;
         if (rn < 0 || rn >= g.R) break;
         const float xr = cx.s_rowx[rn];
         if (!kf_transport(st, xr - cx.s_rowx[r], g.cB, g.max_s)) break;
+        wc.transports++;
         r = rn;
         const float yp = st.y + cx.yref, zp = st.z + cx.zref;
         if (fabsf(yp) > fmaf(xr, g.tan_half, g.edge_margin)) break;
         const float wy = fminf(g.wmax, g.gate * sqrtf(st.c00 + g.sy2));
         const float wz = fminf(g.wmax, g.gate * sqrtf(st.c11 + g.sz2));
         float ym, zm;
-        const int j = pick_up(g, cx, r, yp, zp, wy, wz, ym, zm);
+        const int j = pick_up(g, cx, r, yp, zp, wy, wz, ym, zm, wc);
         if (j >= 0) {
             rowhit[r] = cx.hit_idx[cx.ro[r] + j];
             chi2 += kf_update(st, ym - cx.yref, zm - cx.zref, g.sy2, g.sz2);
+            wc.updates++;
             nhits++;
             gap = 0;
             last_hit_row = r;
@@ -92,7 +100,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clus
               const int32_t* __restrict__ row_offsets, const float2* __restrict__ hit_yz,
               const uint16_t* __restrict__ hit_idx, const uint16_t* __restrict__ bin_start,
               const int32_t* __restrict__ cand_hits, const int32_t* __restrict__ cand_n,
-              const int32_t* __restrict__ cand_slab, const int64_t* __restrict__ counts, int64_t Cmax,
+              const int32_t* __restrict__ cand_slab, int64_t* __restrict__ counts, int64_t Cmax,
               float* __restrict__ tl_par, float* __restrict__ tl_cov, float* __restrict__ tl_chi2,
               int32_t* __restrict__ tl_nhits, int32_t* __restrict__ tl_rows, uint16_t* __restrict__ tl_rowhit) {
     __shared__ float s_rowx[kMaxRows + 1];
@@ -100,6 +108,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clus
     __syncthreads();
     const int64_t n_cand = min(counts[1], Cmax);
     const int64_t stride = (int64_t)gridDim.x * kFollowThreads;
+    WorkCount wc = {0u, 0u, 0u, 0u};
     for (int64_t c = (int64_t)blockIdx.x * kFollowThreads + threadIdx.x; c < n_cand; c += stride) {
         const int slab0 = cand_slab[c];
         const int inst = slab0 / g.R, r0 = slab0 - inst * g.R;
@@ -139,18 +148,21 @@ follow_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clus
             }
             const float4 h = __ldg(&clusters[hg]);
             chi2 += kf_update(st, h.y - cx.yref, h.z - cx.zref, g.sy2, g.sz2);
+            wc.transports += i > 0;
+            wc.updates++;
             rowhit[r0 + i] = (uint16_t)(hg - cx.ro[r0 + i]);
             nhits++;
         }
         if (!ok) continue;
         // ... then upward pick-up
         int last_row = r0 + n - 1;
-        const int r_top = follow_dir<+1>(g, cx, st, last_row, chi2, nhits, last_row, rowhit, nullptr);
+        const int r_top = follow_dir<+1>(g, cx, st, last_row, chi2, nhits, last_row, rowhit, nullptr, wc);
         // phase B: one step back to the start row (no update there), then downward pick-up
         if (!kf_transport(st, s_rowx[r0] - s_rowx[r_top], g.cB, g.max_s)) continue;
+        wc.transports++;
         KfState rep = st;
         int first_row = r0;
-        follow_dir<-1>(g, cx, st, r0, chi2, nhits, first_row, rowhit, &rep);
+        follow_dir<-1>(g, cx, st, r0, chi2, nhits, first_row, rowhit, &rep, wc);
         float* p = tl_par + c * 5;
         p[0] = rep.y + cx.yref; p[1] = rep.z + cx.zref; p[2] = rep.s; p[3] = rep.t; p[4] = rep.k;
         float* q = tl_cov + c * 15;
@@ -160,6 +172,14 @@ follow_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clus
         tl_chi2[c] = chi2;
         tl_rows[c] = first_row | (last_row << 8) | (first_row << 16);
         tl_nhits[c] = nhits;
+    }
+    // work counters: warp reduction, one atomic per warp and counter
+    unsigned v[4] = {wc.transports, wc.updates, wc.examined, wc.searches};
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], d);
+        if ((threadIdx.x & 31) == 0 && v[q]) atomicAdd((unsigned long long*)&counts[6 + q], (unsigned long long)v[q]);
     }
 }
 

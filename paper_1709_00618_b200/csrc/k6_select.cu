@@ -188,7 +188,7 @@ __global__ void finalize_counts_kernel(const int64_t* __restrict__ counts, const
     if (threadIdx.x == 0) {
         if (o.trk_hit_offset && counts[3] <= o.trk_capacity) o.trk_hit_offset[counts[3]] = counts[4];
     }
-    if (threadIdx.x < 8) o.counts[threadIdx.x] = counts[threadIdx.x];
+    if (threadIdx.x < 16) o.counts[threadIdx.x] = counts[threadIdx.x];
 }
 
 // defined in k34_links_chains.cu

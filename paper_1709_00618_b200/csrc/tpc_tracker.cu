@@ -8,27 +8,9 @@
 
 #include "../../include/tpc_tracker.h"
 #include "tpc_common.cuh"
+#include "tracker_handle.cuh"
 
 using namespace tpc;
-
-struct tpc_tracker {
-    DevGeom g;
-    float* d_row_x = nullptr;
-    void* ws = nullptr;
-    size_t ws_bytes = 0;
-    cudaStream_t stream = nullptr;
-    int n_sm = 148;
-    int last_launches = 0;
-    bool timing = false;
-    cudaEvent_t ev[TPC_N_STAGES + 1] = {};
-    bool ev_valid = false;
-    std::string err;
-};
-
-static int fail(tpc_tracker* t, int code, const std::string& msg) {
-    if (t) t->err = msg;
-    return code;
-}
 
 static thread_local std::string g_create_err;
 
@@ -112,7 +94,8 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
 extern "C" void tpc_tracker_destroy(tpc_tracker_t* t) {
     if (!t) return;
     if (t->ev_valid)
-        for (auto& e : t->ev) cudaEventDestroy(e);
+        for (auto& ring : t->ev)
+            for (auto& e : ring) cudaEventDestroy(e);
     if (t->d_row_x) cudaFree(t->d_row_x);
     delete t;
 }
@@ -186,19 +169,22 @@ extern "C" int tpc_set_stream(tpc_tracker_t* t, void* s) {
 extern "C" int tpc_set_stage_timing(tpc_tracker_t* t, int32_t enable) {
     if (!t) return TPC_ERR_ARG;
     if (enable && !t->ev_valid) {
-        for (auto& e : t->ev)
-            if (cudaEventCreate(&e) != cudaSuccess) return fail(t, TPC_ERR_CUDA, "cudaEventCreate failed");
+        for (auto& ring : t->ev)
+            for (auto& e : ring)
+                if (cudaEventCreate(&e) != cudaSuccess) return fail(t, TPC_ERR_CUDA, "cudaEventCreate failed");
         t->ev_valid = true;
     }
     t->timing = enable != 0;
     return TPC_OK;
 }
 
-extern "C" int tpc_stage_times_ms(tpc_tracker_t* t, float* out_ms) {
+extern "C" int tpc_stage_times_ms(tpc_tracker_t* t, int32_t age, float* out_ms) {
     if (!t || !out_ms) return TPC_ERR_ARG;
     if (!t->ev_valid) return fail(t, TPC_ERR_ARG, "stage timing was not enabled");
-    cudaError_t e = cudaEventSynchronize(t->ev[TPC_N_STAGES]);
-    for (int i = 0; i < TPC_N_STAGES && e == cudaSuccess; i++) e = cudaEventElapsedTime(&out_ms[i], t->ev[i], t->ev[i + 1]);
+    if (age < 0 || age >= TPC_TIMING_RING || age >= t->n_calls) return fail(t, TPC_ERR_ARG, "no timed call of that age");
+    cudaEvent_t* ev = t->ev[(t->n_calls - 1 - age) % TPC_TIMING_RING];
+    cudaError_t e = cudaEventSynchronize(ev[TPC_N_STAGES]);
+    for (int i = 0; i < TPC_N_STAGES && e == cudaSuccess; i++) e = cudaEventElapsedTime(&out_ms[i], ev[i], ev[i + 1]);
     if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, std::string("CUDA: ") + cudaGetErrorString(e));
     return TPC_OK;
 }
@@ -219,26 +205,28 @@ extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const 
     Problem p{reinterpret_cast<const float4*>(clusters), row_offsets, n_inst, n_clusters};
     int launches = 0;
     const bool tm = t->timing && t->ev_valid;
+    cudaEvent_t* ev = t->ev[t->n_calls % TPC_TIMING_RING];
+    if (tm) t->n_calls++;
     cudaMemsetAsync(w.counts, 0, sizeof(int64_t) * TPC_N_COUNTS, s);
     if (out->cluster_owner && n_clusters > 0) cudaMemsetAsync(out->cluster_owner, 0xFF, sizeof(int32_t) * n_clusters, s);
-    if (tm) cudaEventRecord(t->ev[0], s);
+    if (tm) cudaEventRecord(ev[0], s);
     launches += launch_bin_rows(g, w, p, s);
-    if (tm) cudaEventRecord(t->ev[1], s);
+    if (tm) cudaEventRecord(ev[1], s);
     launches += launch_neighbours(g, w, p, s);
-    if (tm) cudaEventRecord(t->ev[2], s);
+    if (tm) cudaEventRecord(ev[2], s);
     launches += launch_clean(g, w, p, s);
-    if (tm) cudaEventRecord(t->ev[3], s);
+    if (tm) cudaEventRecord(ev[3], s);
     ChainOut co{out->start_hits, out->start_hits ? out->start_capacity : 0, out->cand_hits, out->cand_n,
                 (out->cand_hits || out->cand_n) ? out->cand_capacity : 0};
     launches += launch_chains(g, w, p, co, s);
-    if (tm) cudaEventRecord(t->ev[4], s);
+    if (tm) cudaEventRecord(ev[4], s);
     launches += launch_follow(g, w, p, t->n_sm, s);
-    if (tm) cudaEventRecord(t->ev[5], s);
+    if (tm) cudaEventRecord(ev[5], s);
     SelectOut so{out->trk_params, out->trk_cov, out->trk_chi2, out->trk_xref, out->trk_cand_id, out->trk_nhits,
                  out->trk_sector, out->trk_hit_offset, out->trk_hits, out->trk_capacity, out->trk_hits_capacity,
                  out->cluster_owner, out->counts};
     launches += launch_select(g, w, p, so, s);
-    if (tm) cudaEventRecord(t->ev[6], s);
+    if (tm) cudaEventRecord(ev[6], s);
     // optional parity/debug copies (device to device, same stream)
     if (n_clusters > 0) {
         const size_t nb = sizeof(int32_t) * (size_t)n_clusters;

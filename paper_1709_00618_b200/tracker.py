@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtpctrk.so")
 
 CAND_MAX_HITS = 10
-N_COUNTS = 8
+N_COUNTS = 16
 N_STAGES = 6
 STAGE_NAMES = ("bin", "neighbours", "clean", "chains", "follow", "select")
 ERRORS = {-1: "TPC_ERR_ARG", -2: "TPC_ERR_GEOMETRY", -3: "TPC_ERR_WORKSPACE", -4: "TPC_ERR_CUDA",
@@ -23,7 +23,7 @@ ERRORS = {-1: "TPC_ERR_ARG", -2: "TPC_ERR_GEOMETRY", -3: "TPC_ERR_WORKSPACE", -4
 
 EXPORTS = ("tpc_tracker_create", "tpc_tracker_destroy", "tpc_workspace_bytes", "tpc_set_workspace", "tpc_set_stream",
            "tpc_track_sectors", "tpc_check_counts", "tpc_last_launch_count", "tpc_set_stage_timing",
-           "tpc_stage_times_ms", "tpc_last_error")
+           "tpc_stage_times_ms", "tpc_last_error", "tpc_track_sectors_host")
 
 
 class TpcError(RuntimeError):
@@ -60,6 +60,19 @@ class Output(C.Structure):
                 ("counts", C.c_void_p)]
 
 
+class Slot(C.Structure):
+    _fields_ = [("clusters", C.c_void_p), ("row_offsets", C.c_void_p), ("max_clusters", C.c_int64),
+                ("max_instances", C.c_int32), ("out", Output)]
+
+
+class HostOutput(C.Structure):
+    _fields_ = [("trk_params", C.c_void_p), ("trk_cov", C.c_void_p), ("trk_nhits", C.c_void_p),
+                ("trk_sector", C.c_void_p), ("trk_hit_offset", C.c_void_p), ("trk_hits", C.c_void_p),
+                ("cluster_owner", C.c_void_p), ("trk_capacity", C.c_int64), ("trk_hits_capacity", C.c_int64),
+                ("totals", C.c_int64 * 16), ("n_chunks", C.c_int64), ("n_launches", C.c_int64),
+                ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64)]
+
+
 _lib = None
 
 
@@ -85,9 +98,12 @@ def load_library():
     lib.tpc_last_launch_count.argtypes = [C.c_void_p]
     lib.tpc_last_launch_count.restype = C.c_int32
     lib.tpc_set_stage_timing.argtypes = [C.c_void_p, C.c_int32]
-    lib.tpc_stage_times_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    lib.tpc_stage_times_ms.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_float)]
     lib.tpc_last_error.argtypes = [C.c_void_p]
     lib.tpc_last_error.restype = C.c_char_p
+    lib.tpc_track_sectors_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_int32,
+                                           C.POINTER(Slot), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                           C.POINTER(HostOutput)]
     _lib = lib
     return lib
 
@@ -214,9 +230,10 @@ class Tracker:
     def set_stage_timing(self, enable=True):
         self._check(self.lib.tpc_set_stage_timing(self._h, 1 if enable else 0), "tpc_set_stage_timing")
 
-    def stage_times_ms(self):
+    def stage_times_ms(self, age=0):
+        """Milliseconds per stage of the timed call `age` calls back (0 = last)."""
         buf = (C.c_float * N_STAGES)()
-        self._check(self.lib.tpc_stage_times_ms(self._h, buf), "tpc_stage_times_ms")
+        self._check(self.lib.tpc_stage_times_ms(self._h, int(age), buf), "tpc_stage_times_ms")
         return dict(zip(STAGE_NAMES, [float(x) for x in buf]))
 
     @property
@@ -293,3 +310,65 @@ class Tracker:
             if k != "counts":
                 setattr(res, k, v[:cut[k]].cpu().numpy())
         return res
+
+
+class HostPipeline:
+    """Buffers for tpc_track_sectors_host: `n_slots` device slots (torch), pinned host result arrays, three streams.
+
+    The chunk loop, the stream/event choreography and every copy are inside the C library; this class only owns
+    memory and marshals pointers."""
+
+    def __init__(self, tracker: Tracker, max_chunk_clusters: int, inst_per_chunk: int, total_clusters: int, *,
+                 n_slots=2, trk_frac=0.05):
+        t = tracker._torch
+        self.trk = tracker
+        self.inst_per_chunk = int(inst_per_chunk)
+        dev = tracker.device
+        n = max(int(max_chunk_clusters), 1)
+        tc = int(n * trk_frac) + 64
+        i32, f32, i64 = t.int32, t.float32, t.int64
+        self._keep = []
+        self.slots = (Slot * n_slots)()
+        with t.cuda.device(dev):
+            for s in range(n_slots):
+                b = dict(clusters=t.empty((n, 4), dtype=f32, device=dev),
+                         row_offsets=t.empty(self.inst_per_chunk * tracker.n_rows + 1, dtype=i32, device=dev),
+                         counts=t.zeros(N_COUNTS, dtype=i64, device=dev),
+                         trk_params=t.empty((tc, 5), dtype=f32, device=dev), trk_cov=t.empty((tc, 15), dtype=f32, device=dev),
+                         trk_nhits=t.empty(tc, dtype=i32, device=dev), trk_sector=t.empty(tc, dtype=i32, device=dev),
+                         trk_hit_offset=t.empty(tc + 1, dtype=i64, device=dev), trk_hits=t.empty(n, dtype=i32, device=dev),
+                         cluster_owner=t.empty(n, dtype=i32, device=dev))
+                self._keep.append(b)
+                sl = self.slots[s]
+                sl.clusters, sl.row_offsets = b["clusters"].data_ptr(), b["row_offsets"].data_ptr()
+                sl.max_clusters, sl.max_instances = n, self.inst_per_chunk
+                for k in ("counts", "trk_params", "trk_cov", "trk_nhits", "trk_sector", "trk_hit_offset", "trk_hits",
+                          "cluster_owner"):
+                    setattr(sl.out, k, b[k].data_ptr())
+                sl.out.trk_capacity, sl.out.trk_hits_capacity = tc, n
+            tracker.reserve(n, self.inst_per_chunk)
+            self.streams = [t.cuda.Stream(device=dev) for _ in range(3)]
+        N = max(int(total_clusters), 1)
+        T = int(N * trk_frac) + 64
+        pin = dict(pin_memory=True)
+        self.host = dict(trk_params=t.empty((T, 5), dtype=f32, **pin), trk_cov=t.empty((T, 15), dtype=f32, **pin),
+                         trk_nhits=t.empty(T, dtype=i32, **pin), trk_sector=t.empty(T, dtype=i32, **pin),
+                         trk_hit_offset=t.empty(T + 1, dtype=i64, **pin), trk_hits=t.empty(N, dtype=i32, **pin),
+                         cluster_owner=t.empty(N, dtype=i32, **pin))
+        self.hout = HostOutput()
+        for k, v in self.host.items():
+            setattr(self.hout, k, v.data_ptr())
+        self.hout.trk_capacity, self.hout.trk_hits_capacity = T, N
+        self.n_slots = n_slots
+
+    def run(self, h_clusters, h_row_offsets, n_inst):
+        """h_clusters: pinned float32 torch tensor [N,4]; h_row_offsets: pinned int32 [n_inst*R+1].  Blocks."""
+        tr = self.trk
+        n = int(h_clusters.shape[0])
+        rc = tr.lib.tpc_track_sectors_host(tr._h, C.c_void_p(h_clusters.data_ptr()), C.c_void_p(h_row_offsets.data_ptr()),
+                                           int(n_inst), n, self.inst_per_chunk, self.slots, self.n_slots,
+                                           C.c_void_p(self.streams[0].cuda_stream),
+                                           C.c_void_p(self.streams[1].cuda_stream),
+                                           C.c_void_p(self.streams[2].cuda_stream), C.byref(self.hout))
+        tr._check(rc, "tpc_track_sectors_host")
+        return self.hout

@@ -109,3 +109,31 @@ def test_grid_cell_does_not_change_results():
         b = _gpu(ev, grid_cell_z=cz)
         for k in ("link_up_raw", "link_dn_raw", "cand_hits", "tl_hits", "tl_params", "cluster_owner"):
             assert np.array_equal(getattr(a, k), getattr(b, k)), (cz, k)
+
+
+def test_host_pipeline_equals_device_call():
+    """tpc_track_sectors_host (chunked, three streams, pinned buffers) == one tpc_track_sectors call on the batch."""
+    import torch
+    from paper_1709_00618_b200 import Tracker
+    from paper_1709_00618_b200.tracker import HostPipeline
+    evs = [dg.drift_window(seed=5101 + i, mean_tracks=120.0, cap_tracks=300) for i in range(5)]
+    batch = dg.concat_events(evs)
+    trk = Tracker.for_event(batch)
+    ref = trk.track_sectors(batch.clusters, batch.row_offsets, batch.n_inst)
+    h_cl = torch.from_numpy(batch.clusters).pin_memory()
+    h_ro = torch.from_numpy(batch.row_offsets).pin_memory()
+    for ipc, slots in ((36, 2), (72, 3), (36 * 5, 2), (7, 3)):
+        R = batch.n_rows
+        mx = max(int(batch.row_offsets[min(i + ipc, batch.n_inst) * R] - batch.row_offsets[i * R])
+                 for i in range(0, batch.n_inst, ipc))
+        pipe = HostPipeline(trk, mx, ipc, batch.n_clusters, n_slots=slots)
+        ho = pipe.run(h_cl, h_ro, batch.n_inst)
+        nt, nh = int(ho.totals[3]), int(ho.totals[4])
+        assert nt == ref.n_tracks and nh == ref.n_track_hits and int(ho.totals[1]) == ref.n_cand
+        assert np.array_equal(pipe.host["cluster_owner"].numpy()[:batch.n_clusters], ref.cluster_owner), (ipc, slots)
+        assert np.array_equal(pipe.host["trk_hits"].numpy()[:nh], ref.trk_hits)
+        assert np.array_equal(pipe.host["trk_hit_offset"].numpy()[:nt + 1], ref.trk_hit_offset)
+        assert np.array_equal(pipe.host["trk_params"].numpy()[:nt], ref.trk_params)
+        assert np.array_equal(pipe.host["trk_sector"].numpy()[:nt], ref.trk_sector)
+        assert ho.n_chunks == -(-batch.n_inst // ipc) and ho.h2d_bytes >= 16 * batch.n_clusters
+    trk.close()
