@@ -25,7 +25,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_1709_00618_b200 import datagen  # noqa: E402
+from paper_1709_00618_b200 import datagen, sharding  # noqa: E402
 
 METRIC = "TPC clusters/sec tracked on 1 B200 (ms/event); achieved HBM GB/s vs peak"
 UNIT = "clusters/s"
@@ -44,9 +44,9 @@ def _gen_window(seed):
     return datagen.drift_window(seed)
 
 
-def make_batch(n_windows, seed0):
+def make_batch(n_windows, seed0, rank=0):
     """NW CFG:4 windows, generated in parallel worker processes (before CUDA is touched)."""
-    seeds = [seed0 + i for i in range(n_windows)]
+    seeds = sharding.window_seeds(n_windows, seed0, rank)
     n_proc = max(1, min(n_windows, (os.cpu_count() or 2) // max(1, int(os.environ.get("LOCAL_WORLD_SIZE", "1")))))
     if n_proc > 1:
         import multiprocessing as mp
@@ -155,7 +155,7 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     t_gen = time.time()
-    evs, batch = make_batch(args.windows, args.seed0 + rank * args.windows)  # before CUDA init (fork)
+    evs, batch = make_batch(args.windows, args.seed0, rank)  # before CUDA init (fork)
     t_gen = time.time() - t_gen
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
@@ -205,15 +205,7 @@ def run_ours(args):
     clocks = sampler.stop(t0, t1)
     ms = sum(a.elapsed_time(b) for a, b in ev)
     launches = trk.last_launch_count * args.steps
-    if world > 1:
-        tt = torch.tensor([ms], device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-        nn = torch.tensor([N], device=dev, dtype=torch.int64)
-        dist.all_reduce(nn)
-        n_total = int(nn.item())
-    else:
-        n_total = N
+    ms, n_total = sharding.combine_step(ms, N, device=dev)  # max over ranks, total clusters (no data-path collective)
     ms_step = ms / args.steps
     value = n_total / (ms_step * 1e-3)
     counts = bufs["counts"].cpu().numpy()
@@ -236,10 +228,7 @@ def run_ours(args):
         ho = pipe.run(h_cl, h_ro, S)
     torch.cuda.synchronize(dev)
     e2e_ms = (time.perf_counter() - tw) * 1e3
-    if world > 1:
-        tt = torch.tensor([e2e_ms], device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_ms = float(tt.item())
+    e2e_ms, _ = sharding.combine_step(e2e_ms, N, device=dev)
     e2e_value = n_total / (e2e_ms / args.steps * 1e-3)
     e2e_tracks = int(ho.totals[3])
     launches_e2e = int(ho.n_launches)
