@@ -166,7 +166,8 @@ def run_ours(args):
     from paper_1709_00618_b200 import Tracker, physics
     from paper_1709_00618_b200.tracker import HostPipeline
     N, S = batch.n_clusters, batch.n_inst
-    trk = Tracker.for_event(batch, device=f"cuda:{local}")
+    tune = json.loads(args.tune) if args.tune else {}
+    trk = Tracker.for_event(batch, device=f"cuda:{local}", **tune)
     h_cl = torch.from_numpy(batch.clusters).pin_memory()
     h_ro = torch.from_numpy(batch.row_offsets).pin_memory()
     d_cl = h_cl.to(dev)
@@ -297,6 +298,7 @@ def main():
     ap.add_argument("--chunk-windows", type=int, default=2, help="windows per upload chunk in the e2e pipeline")
     ap.add_argument("--slots", type=int, default=3)
     ap.add_argument("--seed0", type=int, default=5001)
+    ap.add_argument("--tune", default="", help='JSON dict of performance-only tracker parameters, e.g. {"grid_cells_y": 8}')
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

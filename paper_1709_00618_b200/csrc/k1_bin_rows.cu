@@ -1,7 +1,7 @@
 // S1: per-pad-row grid binning (BASELINE.json north_star; the paper, does not describe it).
-// One CTA per (sector instance, pad row): counting sort of the row's clusters by z bin, done entirely in shared
-// memory, writing the sorted (y,z) pairs, their original local indices and the bin-start table.
-// The grid is an acceleration structure only; no result of S2..S6 depends on it.
+// One CTA per (sector instance, pad row): counting sort of the row's clusters by grid cell (z bin major, y strip
+// minor), done entirely in shared memory, writing the sorted (y,z) pairs, their original local indices and the
+// cell-start table.  The grid is an acceleration structure only; no result of S2..S6 depends on it.
 #include "tpc_common.cuh"
 
 namespace tpc {
@@ -12,10 +12,10 @@ __global__ void __launch_bounds__(kBinThreads)
 bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clusters,
                 const int32_t* __restrict__ row_offsets, float2* __restrict__ hit_yz, uint16_t* __restrict__ hit_idx,
                 uint16_t* __restrict__ bin_start, int64_t* __restrict__ counts) {
-    extern __shared__ uint32_t sm_hist[];  // [nz + 1] counts, then exclusive starts (running cursors in pass 2)
+    extern __shared__ __align__(16) uint32_t sm_hist[];  // [nzp] counts, then exclusive starts (cursors in pass 2)
     __shared__ uint32_t sm_warp[kBinThreads / 32];
     const int slab = blockIdx.x;
-    const int inst = slab / g.R;
+    const int inst = slab / g.R, r = slab - inst * g.R;
     const int base = row_offsets[slab];
     int n = row_offsets[slab + 1] - base;
     if (n > 65535) {  // local indices are 16 bit: flag and ignore the excess (documented in tpc_tracker.h)
@@ -23,20 +23,41 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
         n = 65535;
     }
     const float z0 = grid_z0(g, inst);
-    const int nz = g.nz;
-    for (int b = threadIdx.x; b <= nz; b += kBinThreads) sm_hist[b] = 0;
+    const float y0 = g.row_y0[r], inv_sy = g.row_inv_sy[r];
+    const int nzp = g.nzp;  // multiple of 8
+    uint4* hist4 = reinterpret_cast<uint4*>(sm_hist);
+    for (int b = threadIdx.x; b < nzp / 4; b += kBinThreads) hist4[b] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
-    // pass 1: histogram.  Coalesced float4 loads, 16 B per thread.
-    for (int i = threadIdx.x; i < n; i += kBinThreads) {
+    // pass 1: histogram.  Coalesced float4 loads, 16 B per thread; the cell ids stay in registers for pass 2
+    // when the row is short enough (two hits per thread), which is the normal case.
+    constexpr int kKeep = 2;
+    int key[kKeep];
+    float2 yz[kKeep];
+#pragma unroll
+    for (int k = 0; k < kKeep; k++) {
+        const int i = threadIdx.x + k * kBinThreads;
+        key[k] = -1;
+        if (i < n) {
+            const float4 c = __ldg(&clusters[base + i]);
+            key[k] = zbin(c.z, z0, g.inv_cz, g.nz) * g.ny + ybin(c.y, y0, inv_sy, g.ny);
+            yz[k] = make_float2(c.y, c.z);
+            atomicAdd(&sm_hist[key[k]], 1u);
+        }
+    }
+    for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {
         const float4 c = __ldg(&clusters[base + i]);
-        atomicAdd(&sm_hist[zbin(c.z, z0, g.inv_cz, nz)], 1u);
+        atomicAdd(&sm_hist[zbin(c.z, z0, g.inv_cz, g.nz) * g.ny + ybin(c.y, y0, inv_sy, g.ny)], 1u);
     }
     __syncthreads();
-    // exclusive scan of nz+1 entries: contiguous chunk per thread, warp scan of the chunk sums
-    const int per = (nz + 1 + kBinThreads - 1) / kBinThreads;
-    const int lo = threadIdx.x * per, hi = min(lo + per, nz + 1);
+    // exclusive scan of nzp entries: a contiguous chunk of 8-entry groups per thread, warp scan of the chunk sums
+    const int groups = nzp / 8;
+    const int per = (groups + kBinThreads - 1) / kBinThreads;
+    const int glo = min(threadIdx.x * per, groups), ghi = min(glo + per, groups);
     uint32_t sum = 0;
-    for (int b = lo; b < hi; b++) sum += sm_hist[b];
+    for (int q = glo; q < ghi; q++) {
+        const uint4 a = hist4[2 * q], b = hist4[2 * q + 1];
+        sum += a.x + a.y + a.z + a.w + b.x + b.y + b.z + b.w;
+    }
     uint32_t incl = sum;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
@@ -48,18 +69,29 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
     __syncthreads();
     uint32_t off = incl - sum;
     for (int k = 0; k < wid; k++) off += sm_warp[k];
-    uint16_t* tbl = bin_start + (size_t)slab * g.nzp;
-    for (int b = lo; b < hi; b++) {
-        uint32_t c = sm_hist[b];
-        sm_hist[b] = off;
-        tbl[b] = (uint16_t)off;
-        off += c;
+    uint4* tbl4 = reinterpret_cast<uint4*>(bin_start + (size_t)slab * nzp);  // 16-B aligned: nzp % 8 == 0
+    for (int q = glo; q < ghi; q++) {
+        uint4 a = hist4[2 * q], b = hist4[2 * q + 1];
+        uint32_t s0 = off, s1 = s0 + a.x, s2 = s1 + a.y, s3 = s2 + a.z, s4 = s3 + a.w, s5 = s4 + b.x, s6 = s5 + b.y,
+                 s7 = s6 + b.z;
+        off = s7 + b.w;
+        hist4[2 * q] = make_uint4(s0, s1, s2, s3);
+        hist4[2 * q + 1] = make_uint4(s4, s5, s6, s7);
+        tbl4[q] = make_uint4(s0 | (s1 << 16), s2 | (s3 << 16), s4 | (s5 << 16), s6 | (s7 << 16));
     }
     __syncthreads();
-    // pass 2: scatter (the clusters come from L1/L2 this time)
-    for (int i = threadIdx.x; i < n; i += kBinThreads) {
+    // pass 2: scatter
+#pragma unroll
+    for (int k = 0; k < kKeep; k++) {
+        if (key[k] >= 0) {
+            const uint32_t pos = atomicAdd(&sm_hist[key[k]], 1u);
+            hit_yz[base + pos] = yz[k];
+            hit_idx[base + pos] = (uint16_t)(threadIdx.x + k * kBinThreads);
+        }
+    }
+    for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {  // long rows: from L1/L2 this time
         const float4 c = __ldg(&clusters[base + i]);
-        const uint32_t pos = atomicAdd(&sm_hist[zbin(c.z, z0, g.inv_cz, nz)], 1u);
+        const uint32_t pos = atomicAdd(&sm_hist[zbin(c.z, z0, g.inv_cz, g.nz) * g.ny + ybin(c.y, y0, inv_sy, g.ny)], 1u);
         hit_yz[base + pos] = make_float2(c.y, c.z);
         hit_idx[base + pos] = (uint16_t)i;
     }
@@ -68,8 +100,14 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
 int launch_bin_rows(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s) {
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
-    bin_rows_kernel<<<slabs, kBinThreads, (g.nz + 1) * sizeof(uint32_t), s>>>(
-        g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.counts);
+    const size_t smem = (size_t)g.nzp * sizeof(uint32_t);
+    static size_t configured = 0;
+    if (smem > 48 * 1024 && smem > configured) {
+        cudaFuncSetAttribute(bin_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        configured = smem;
+    }
+    bin_rows_kernel<<<slabs, kBinThreads, smem, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
+                                                     w.counts);
     return 1;
 }
 

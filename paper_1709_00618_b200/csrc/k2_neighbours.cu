@@ -8,20 +8,85 @@
 // pre-rounded bounds, and the minimum is taken over (D, u, d) lexicographically, so the result does not depend on
 // the order in which the grid presents the hits.  This file is additionally compiled with -fmad=false.
 //
-// One CTA per (sector instance, pad row).  The sorted (y,z), the original indices and the bin tables of the two
-// adjacent rows are staged in shared memory (they are read ~10x per hit); rows too long for that are read in place.
+// One CTA per (sector instance, pad row).  The sorted (y,z), the original indices and the cell tables of the two
+// adjacent rows are staged in shared memory; rows or tables too long for that are read in place.  Per hit the
+// search is three flat loops instead of a nested one: window hits of row r+1, window hits of row r-1 (each through
+// the 2-D grid, a handful of candidates), then the pairs of the two short lists.
 #include "tpc_common.cuh"
 
 namespace tpc {
 
 constexpr int kNbThreads = 128;
-constexpr int kNbStageHits = 3584;  // max hits of row r-1 plus row r+1 staged in shared memory (10 B each)
+constexpr int kNbStageHits = 1024;  // max hits of row r-1 plus row r+1 staged in shared memory (10 B each)
+constexpr int kNbStageTbl = 4096;   // max table entries per row staged in shared memory (2 B each, two rows)
+constexpr int kNbList = 4;          // window hits per neighbour row kept in registers; more -> exact slow path
 
 struct RowView {
     const float2* yz;
     const uint16_t* idx;
     const uint16_t* tbl;
+    float y0, inv_sy;
 };
+
+struct Best {
+    float D;
+    int iu, id;  // local indices, -1 = none
+};
+
+__device__ __forceinline__ void consider(Best& b, float D, int iu, int id) {
+    if (b.iu < 0 || D < b.D || (D == b.D && (iu < b.iu || (iu == b.iu && id < b.id)))) {
+        b.D = D;
+        b.iu = iu;
+        b.id = id;
+    }
+}
+
+// Positions (in the sorted row) of the hits of `row` inside the window, newest in the low 16 bits; returns how many
+// there are (only the last four are kept).
+__device__ __forceinline__ int window_hits(const DevGeom& g, const RowView& row, float ylo, float yhi, float zlo,
+                                           float zhi, int zb0, int zb1, unsigned long long& list) {
+    const int ys0 = ybin(ylo, row.y0, row.inv_sy, g.ny), ys1 = ybin(yhi, row.y0, row.inv_sy, g.ny);
+    int cnt = 0;
+    list = 0ull;
+    for (int zb = zb0; zb <= zb1; zb++) {
+        const int j0 = row.tbl[zb * g.ny + ys0], j1 = row.tbl[zb * g.ny + ys1 + 1];
+        for (int j = j0; j < j1; j++) {
+            const float2 h = row.yz[j];
+            if (ylo <= h.x && h.x <= yhi && zlo <= h.y && h.y <= zhi) {
+                list = (list << 16) | (unsigned long long)j;
+                cnt++;
+            }
+        }
+    }
+    return cnt;
+}
+
+// Exact search without the register lists (more than kNbList window hits in a neighbour row: dense spots only).
+__device__ __noinline__ void search_dense(const DevGeom& g, const RowView& up, const RowView& dn, float y, float z,
+                                          float ylo, float yhi, float zlo, float zhi, int zb0, int zb1, Best& best) {
+    const int us0 = ybin(ylo, up.y0, up.inv_sy, g.ny), us1 = ybin(yhi, up.y0, up.inv_sy, g.ny);
+    const int ds0 = ybin(ylo, dn.y0, dn.inv_sy, g.ny), ds1 = ybin(yhi, dn.y0, dn.inv_sy, g.ny);
+    for (int zu = zb0; zu <= zb1; zu++) {
+        const int u0 = up.tbl[zu * g.ny + us0], u1 = up.tbl[zu * g.ny + us1 + 1];
+        for (int a = u0; a < u1; a++) {
+            const float2 u = up.yz[a];
+            if (!(ylo <= u.x && u.x <= yhi && zlo <= u.y && u.y <= zhi)) continue;
+            const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
+            const int iu = up.idx[a];
+            for (int zd = zb0; zd <= zb1; zd++) {
+                const int d0 = dn.tbl[zd * g.ny + ds0], d1 = dn.tbl[zd * g.ny + ds1 + 1];
+                for (int b = d0; b < d1; b++) {
+                    const float2 d = dn.yz[b];
+                    if (!(ylo <= d.x && d.x <= yhi && zlo <= d.y && d.y <= zhi)) continue;
+                    const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
+                    const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
+                    const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+                    if (D <= g.nf_d2max) consider(best, D, iu, dn.idx[b]);
+                }
+            }
+        }
+    }
+}
 
 __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const float2* my_yz,
                                            const uint16_t* my_idx, int n, float z0, int base, int base_up,
@@ -33,38 +98,33 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
         const float y = h.x, z = h.y;
         const float ylo = __fsub_rn(y, WY), yhi = __fadd_rn(y, WY);
         const float zlo = __fsub_rn(z, WZ), zhi = __fadd_rn(z, WZ);
-        const int b0 = zbin(zlo, z0, g.inv_cz, g.nz), b1 = zbin(zhi, z0, g.inv_cz, g.nz);
-        const int u0 = up.tbl[b0], u1 = up.tbl[b1 + 1];
-        const int d0 = dn.tbl[b0], d1 = dn.tbl[b1 + 1];
-        int bu = -1, bd = -1;
-        float bD = 0.0f;
-        for (int a = u0; a < u1; a++) {
-            const float2 u = up.yz[a];
-            if (!(ylo <= u.x && u.x <= yhi && zlo <= u.y && u.y <= zhi)) continue;
-            const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
-            const int iu = up.idx[a];
-            for (int b = d0; b < d1; b++) {
-                const float2 d = dn.yz[b];
-                if (!(ylo <= d.x && d.x <= yhi && zlo <= d.y && d.y <= zhi)) continue;
-                const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
-                const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
-                const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
-                if (!(D <= D2MAX)) continue;
-                bool better = bu < 0 || D < bD;
-                if (!better && D == bD) {
-                    const int id = dn.idx[b];
-                    better = iu < bu || (iu == bu && id < bd);
-                }
-                if (better) {
-                    bD = D;
-                    bu = iu;
-                    bd = dn.idx[b];
+        const int zb0 = zbin(zlo, z0, g.inv_cz, g.nz), zb1 = zbin(zhi, z0, g.inv_cz, g.nz);
+        unsigned long long lu, ld;
+        const int nu = window_hits(g, up, ylo, yhi, zlo, zhi, zb0, zb1, lu);
+        const int nd = window_hits(g, dn, ylo, yhi, zlo, zhi, zb0, zb1, ld);
+        Best best{0.0f, -1, -1};
+        if (nu > kNbList || nd > kNbList) {
+            search_dense(g, up, dn, y, z, ylo, yhi, zlo, zhi, zb0, zb1, best);
+        } else if (nd > 0) {
+            for (int a = 0; a < nu; a++, lu >>= 16) {
+                const int ja = (int)(lu & 0xffffull);
+                const float2 u = up.yz[ja];
+                const int iu = up.idx[ja];
+                const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
+                unsigned long long l = ld;
+                for (int b = 0; b < nd; b++, l >>= 16) {
+                    const int jb = (int)(l & 0xffffull);
+                    const float2 d = dn.yz[jb];
+                    const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
+                    const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
+                    const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+                    if (D <= D2MAX) consider(best, D, iu, dn.idx[jb]);
                 }
             }
         }
         const int me = base + my_idx[i];
-        link_up[me] = bu < 0 ? -1 : base_up + bu;
-        link_dn[me] = bd < 0 ? -1 : base_dn + bd;
+        link_up[me] = best.iu < 0 ? -1 : base_up + best.iu;
+        link_dn[me] = best.id < 0 ? -1 : base_dn + best.id;
     }
 }
 
@@ -85,57 +145,57 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
         for (int i = threadIdx.x; i < n; i += kNbThreads) link_up[base + i] = link_dn[base + i] = -1;
         return;
     }
+    if (n == 0) return;
     const int base_dn = row_offsets[slab - 1], base_up = row_offsets[slab + 1];
     const int n_dn = min(base - base_dn, 65535), n_up = min(row_offsets[slab + 2] - base_up, 65535);
     const float z0 = grid_z0(g, inst);
-    const uint16_t* tbl_up = bin_start + (size_t)(slab + 1) * g.nzp;
-    const uint16_t* tbl_dn = bin_start + (size_t)(slab - 1) * g.nzp;
-    RowView up, dn;
+    RowView up{hit_yz + base_up, hit_idx + base_up, bin_start + (size_t)(slab + 1) * g.nzp, g.row_y0[r + 1],
+               g.row_inv_sy[r + 1]};
+    RowView dn{hit_yz + base_dn, hit_idx + base_dn, bin_start + (size_t)(slab - 1) * g.nzp, g.row_y0[r - 1],
+               g.row_inv_sy[r - 1]};
+    // shared layout: tbl_up[nzp] tbl_dn[nzp] (if staged) | yz_up[n_up] yz_dn[n_dn] | idx_up[n_up] idx_dn[n_dn]
+    const bool stage_tbl = g.nzp <= kNbStageTbl;
+    uint4* s_tbl = reinterpret_cast<uint4*>(sm_raw);
+    float2* s_yz = reinterpret_cast<float2*>(sm_raw + (stage_tbl ? (size_t)g.nzp * 4 : 0));
+    uint16_t* s_idx = reinterpret_cast<uint16_t*>(s_yz + kNbStageHits);
+    if (stage_tbl) {
+        const int q = g.nzp / 8;  // 16-byte groups per table
+        const uint4* gu = reinterpret_cast<const uint4*>(up.tbl);
+        const uint4* gd = reinterpret_cast<const uint4*>(dn.tbl);
+        for (int i = threadIdx.x; i < q; i += kNbThreads) {
+            s_tbl[i] = __ldg(&gu[i]);
+            s_tbl[q + i] = __ldg(&gd[i]);
+        }
+        up.tbl = reinterpret_cast<const uint16_t*>(s_tbl);
+        dn.tbl = reinterpret_cast<const uint16_t*>(s_tbl + q);
+    }
     if (n_up + n_dn <= kNbStageHits) {
-        // shared layout: yz_up[n_up] yz_dn[n_dn] | tbl_up[nzp] tbl_dn[nzp] idx_up[n_up] idx_dn[n_dn]
-        float2* s_yz = reinterpret_cast<float2*>(sm_raw);
-        uint16_t* s_16 = reinterpret_cast<uint16_t*>(s_yz + kNbStageHits);
-        uint16_t* s_tu = s_16;
-        uint16_t* s_td = s_16 + g.nzp;
-        uint16_t* s_iu = s_td + g.nzp;
-        uint16_t* s_id = s_iu + n_up;
         for (int i = threadIdx.x; i < n_up; i += kNbThreads) {
-            s_yz[i] = __ldg(&hit_yz[base_up + i]);
-            s_iu[i] = __ldg(&hit_idx[base_up + i]);
+            s_yz[i] = __ldg(&up.yz[i]);
+            s_idx[i] = __ldg(&up.idx[i]);
         }
         for (int i = threadIdx.x; i < n_dn; i += kNbThreads) {
-            s_yz[n_up + i] = __ldg(&hit_yz[base_dn + i]);
-            s_id[i] = __ldg(&hit_idx[base_dn + i]);
+            s_yz[n_up + i] = __ldg(&dn.yz[i]);
+            s_idx[n_up + i] = __ldg(&dn.idx[i]);
         }
-        for (int i = threadIdx.x; i <= g.nz; i += kNbThreads) {
-            s_tu[i] = __ldg(&tbl_up[i]);
-            s_td[i] = __ldg(&tbl_dn[i]);
-        }
-        __syncthreads();
-        up = RowView{s_yz, s_iu, s_tu};
-        dn = RowView{s_yz + n_up, s_id, s_td};
-    } else {
-        up = RowView{hit_yz + base_up, hit_idx + base_up, tbl_up};
-        dn = RowView{hit_yz + base_dn, hit_idx + base_dn, tbl_dn};
+        up.yz = s_yz;
+        up.idx = s_idx;
+        dn.yz = s_yz + n_up;
+        dn.idx = s_idx + n_up;
     }
+    __syncthreads();
     search_row(g, up, dn, hit_yz + base, hit_idx + base, n, z0, base, base_up, base_dn, link_up, link_dn);
 }
 
 static size_t nb_smem_bytes(const DevGeom& g) {
-    return (size_t)kNbStageHits * sizeof(float2) + (size_t)(2 * g.nzp + kNbStageHits) * sizeof(uint16_t);
+    return (size_t)kNbStageHits * (sizeof(float2) + sizeof(uint16_t)) + (g.nzp <= kNbStageTbl ? (size_t)g.nzp * 4 : 0);
 }
 
 int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s) {
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
-    static bool configured = false;
-    const size_t smem = nb_smem_bytes(g);
-    if (!configured) {
-        cudaFuncSetAttribute(neighbours_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        configured = true;
-    }
-    neighbours_kernel<<<slabs, kNbThreads, smem, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.up_raw,
-                                                      w.dn_raw);
+    neighbours_kernel<<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
+                                                                  w.up_raw, w.dn_raw);
     return 1;
 }
 

@@ -2,196 +2,368 @@
 // TPC sector volume to pick up additional clusters and refine the fit using a simplified Kalman filter"
 // (Fig. 1c); constant Bz only.  Control flow: DESIGN.md "S5" (seed, phase A upward,
 // one-step back transport, phase B downward).  One thread per candidate, all arithmetic fp32 in registers.
+//
+// Execution model: persistent warps, every lane a small state machine that advances its
+// candidate by exactly ONE pad row per loop iteration whatever its phase (own hits / upward / back transport /
+// downward), so the lanes of a warp run the same transport-search-update code instead of diverging on phase and
+// track length.  A lane whose candidate has ended parks until a few lanes are parked, then those lanes write
+// their tracklets and take new candidates from the warp's chunk of the device-wide queue (consecutive candidate
+// ids start in neighbouring rows of one sector instance, which keeps the warp's loads in the same L1 lines).
 #include "kf_math.cuh"
 
 namespace tpc {
 
 constexpr int kFollowThreads = 128;
+constexpr int kFollowCtasPerSm = 8;
+constexpr int kFollowChunk = 64;   // candidates a warp takes from the queue at a time
+constexpr int kFollowReload = 4;   // parked lanes that trigger a write-out / refill phase
 
-struct FollowCtx {
-    const float2* hit_yz;
-    const uint16_t* hit_idx;
-    const uint16_t* bin_start;
-    const int32_t* ro;   // row offsets of this candidate's instance [R+1]
-    int slab_base;       // instance * R
-    float z0;
-    const float* s_rowx; // shared [R]
-    float yref, zref;    // the filter state holds (y - yref, z - zref): see follow_kernel
-};
+enum FollowMode : int { kCand = 0, kUp = 1, kBack = 2, kDown = 3, kDone = 4, kIdle = 5 };
 
 struct WorkCount {  // per-thread work counters (roofline arithmetic): summed into counts[6..9] at kernel end
     unsigned transports, updates, examined, searches;
 };
 
+struct FollowArgs {
+    const float4* clusters;
+    const int32_t* row_offsets;
+    const float2* hit_yz;
+    const uint16_t* hit_idx;
+    const uint16_t* bin_start;
+    const int32_t* cand_hits;
+    const int32_t* cand_n;
+    const int32_t* cand_slab;
+    int64_t* counts;
+    int64_t Cmax;
+    float* tl_par;
+    float* tl_cov;
+    float* tl_chi2;
+    int32_t* tl_nhits;
+    int32_t* tl_rows;
+    uint16_t* tl_rowhit;
+};
+
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// One hit of the pick-up search: inside the gate and nearer than the best so far?  Ties -> lowest local index.
+struct PickBest {
+    int j;       // sorted position of the best hit, -1 = none
+    int idx;     // its local index, -1 = not loaded yet
+    float d2, y, z;
+};
+
+__device__ __forceinline__ void pick_consider(PickBest& b, const uint16_t* __restrict__ idx, int j, bool valid,
+                                              float2 h, float yp, float zp, float wy, float wz) {
+    const float dy = __fsub_rn(h.x, yp), dz = __fsub_rn(h.y, zp);
+    const float d2 = __fadd_rn(__fmul_rn(dy, dy), __fmul_rn(dz, dz));
+    const bool in = valid && fabsf(dy) <= wy && fabsf(dz) <= wz;
+    bool better = in && d2 < b.d2;
+    int id = -1;
+    if (in && d2 == b.d2) {  // exact tie: lowest local index wins (rare)
+        id = idx[j];
+        if (b.idx < 0) b.idx = idx[b.j];
+        better = id < b.idx;
+    }
+    if (better) {
+        b.j = j;
+        b.idx = id;
+        b.d2 = d2;
+        b.y = h.x;
+        b.z = h.y;
+    }
+}
+
 // Nearest cluster of the row inside the gate around the predicted (y,z); ties -> lowest local index.
 // Returns the sorted position (relative to the row start) or -1; (ym, zm) get its coordinates.
-__device__ __forceinline__ int pick_up(const DevGeom& g, const FollowCtx& cx, int r, float yp, float zp, float wy,
-                                       float wz, float& ym, float& zm, WorkCount& wc) {
-    const int base = cx.ro[r];
-    const uint16_t* tbl = cx.bin_start + (size_t)(cx.slab_base + r) * g.nzp;
-    const float m = 1e-3f;  // bin margin: the visited bins are a superset of the rounded fp32 window test below
-    const int b0 = zbin(zp - wz - m, cx.z0, g.inv_cz, g.nz), b1 = zbin(zp + wz + m, cx.z0, g.inv_cz, g.nz);
-    const int j0 = tbl[b0], j1 = tbl[b1 + 1];
+// The grid cells visited are a superset of the rounded fp32 gate test (margin m, monotone bin functions).
+__device__ __forceinline__ int pick_up(const DevGeom& g, const float2* __restrict__ yz,
+                                       const uint16_t* __restrict__ idx, const uint16_t* __restrict__ tbl, float z0,
+                                       float y0, float inv_sy, float yp, float zp, float wy, float wz, float& ym,
+                                       float& zm, WorkCount& wc) {
+    const float m = 1e-3f;
+    const int zb0 = zbin(zp - wz - m, z0, g.inv_cz, g.nz), zb1 = zbin(zp + wz + m, z0, g.inv_cz, g.nz);
+    const int ys0 = ybin(yp - wy - m, y0, inv_sy, g.ny), ys1 = ybin(yp + wy + m, y0, inv_sy, g.ny) + 1;
+    // first and last z bin: the four table entries are independent loads
+    const uint16_t* ta = tbl + zb0 * g.ny;
+    const uint16_t* tb = tbl + zb1 * g.ny;
+    const int ja0 = ta[ys0], ja1 = ta[ys1];
+    int jb0 = 0, jb1 = 0;
+    if (zb1 > zb0) {
+        jb0 = tb[ys0];
+        jb1 = tb[ys1];
+    }
+    const int na = ja1 - ja0, nt = na + (jb1 - jb0);
     wc.searches++;
-    wc.examined += j1 - j0;
-    int best = -1, best_idx = 0;
-    float bd2 = 0.0f;
-    const float2* yz = cx.hit_yz + base;
-    for (int j = j0; j < j1; j++) {
-        const float2 h = yz[j];
-        const float dy = __fsub_rn(h.x, yp), dz = __fsub_rn(h.y, zp);
-        if (!(fabsf(dy) <= wy && fabsf(dz) <= wz)) continue;
-        const float d2 = __fadd_rn(__fmul_rn(dy, dy), __fmul_rn(dz, dz));
-        bool better = best < 0 || d2 < bd2;
-        int idx = -1;
-        if (!better && d2 == bd2) {
-            idx = cx.hit_idx[base + j];
-            if (best_idx < 0) best_idx = cx.hit_idx[base + best];
-            better = idx < best_idx;
+    wc.examined += nt;
+    PickBest b{-1, -1, __int_as_float(0x7f800000), 0.0f, 0.0f};
+    // the two ranges as one sequence, four hits per trip (independent loads: one memory round trip per trip)
+    for (int k = 0; k < nt; k += 4) {
+        int j[4];
+        float2 h[4];
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const int kk = min(k + q, nt - 1);
+            j[q] = kk < na ? ja0 + kk : jb0 + (kk - na);
+            h[q] = yz[j[q]];
         }
-        if (better) {
-            best = j;
-            best_idx = idx;  // -1 = not loaded yet
-            bd2 = d2;
-            ym = h.x;
-            zm = h.y;
-        }
+#pragma unroll
+        for (int q = 0; q < 4; q++) pick_consider(b, idx, j[q], k + q < nt, h[q], yp, zp, wy, wz);
     }
-    return best;
+    // z bins in between exist only when the cells are narrower than the gate (non-default grid_cell_z)
+    for (int zb = zb0 + 1; zb < zb1; zb++) {
+        const int j0 = tbl[zb * g.ny + ys0], j1 = tbl[zb * g.ny + ys1];
+        wc.examined += j1 - j0;
+        for (int j = j0; j < j1; j++) pick_consider(b, idx, j, true, yz[j], yp, zp, wy, wz);
+    }
+    ym = b.y;
+    zm = b.z;
+    return b.j;
 }
 
-// One direction of the pick-up loop.  Returns the last visited row.
-template <int STEP>
-__device__ __forceinline__ int follow_dir(const DevGeom& g, const FollowCtx& cx, KfState& st, int r, float& chi2,
-                                          int& nhits, int& last_hit_row, uint16_t* __restrict__ rowhit,
-                                          KfState* at_hit, WorkCount& wc) {
-    int gap = 0;
-    for (;;) {
-        const int rn = r + STEP;
-        if (rn < 0 || rn >= g.R) break;
-        const float xr = cx.s_rowx[rn];
-        if (!kf_transport(st, xr - cx.s_rowx[r], g.cB, g.max_s)) break;
-        wc.transports++;
-        r = rn;
-        const float yp = st.y + cx.yref, zp = st.z + cx.zref;
-        if (fabsf(yp) > fmaf(xr, g.tan_half, g.edge_margin)) break;
-        const float wy = fminf(g.wmax, g.gate * sqrtf(st.c00 + g.sy2));
-        const float wz = fminf(g.wmax, g.gate * sqrtf(st.c11 + g.sz2));
-        float ym, zm;
-        const int j = pick_up(g, cx, r, yp, zp, wy, wz, ym, zm, wc);
-        if (j >= 0) {
-            rowhit[r] = cx.hit_idx[cx.ro[r] + j];
-            chi2 += kf_update(st, ym - cx.yref, zm - cx.zref, g.sy2, g.sz2);
-            wc.updates++;
-            nhits++;
-            gap = 0;
-            last_hit_row = r;
-            if (at_hit) *at_hit = st;
-        } else {
-            rowhit[r] = kNoHit;
-            if (++gap > g.max_gap) break;
-        }
-    }
-    return r;
-}
-
-__global__ void __launch_bounds__(kFollowThreads)
-follow_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clusters,
-              const int32_t* __restrict__ row_offsets, const float2* __restrict__ hit_yz,
-              const uint16_t* __restrict__ hit_idx, const uint16_t* __restrict__ bin_start,
-              const int32_t* __restrict__ cand_hits, const int32_t* __restrict__ cand_n,
-              const int32_t* __restrict__ cand_slab, int64_t* __restrict__ counts, int64_t Cmax,
-              float* __restrict__ tl_par, float* __restrict__ tl_cov, float* __restrict__ tl_chi2,
-              int32_t* __restrict__ tl_nhits, int32_t* __restrict__ tl_rows, uint16_t* __restrict__ tl_rowhit) {
+__global__ void __launch_bounds__(kFollowThreads, kFollowCtasPerSm)
+follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowArgs a) {
     __shared__ float s_rowx[kMaxRows + 1];
-    for (int i = threadIdx.x; i < g.R; i += kFollowThreads) s_rowx[i] = g.row_x[i];
+    __shared__ float2 s_rowy[kMaxRows + 1];      // (y0, strips per cm) of the row's grid
+    __shared__ float4 s_rep[5][kFollowThreads];  // reported state of the lane's tracklet (see kDown below)
+    for (int i = threadIdx.x; i < g.R; i += kFollowThreads) {
+        s_rowx[i] = g.row_x[i];
+        s_rowy[i] = make_float2(g.row_y0[i], g.row_inv_sy[i]);
+    }
     __syncthreads();
-    const int64_t n_cand = min(counts[1], Cmax);
-    const int64_t stride = (int64_t)gridDim.x * kFollowThreads;
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const unsigned below = (1u << lane) - 1u;
+    const int n_cand = (int)min(a.counts[1], a.Cmax);
+    unsigned long long* queue = reinterpret_cast<unsigned long long*>(&a.counts[10]);
+    int wn = 0, we = 0;  // the warp's chunk [wn, we) of candidate ids (warp-uniform)
+    bool exhausted = false;
     WorkCount wc = {0u, 0u, 0u, 0u};
-    for (int64_t c = (int64_t)blockIdx.x * kFollowThreads + threadIdx.x; c < n_cand; c += stride) {
-        const int slab0 = cand_slab[c];
-        const int inst = slab0 / g.R, r0 = slab0 - inst * g.R;
-        const int n = cand_n[c];
-        FollowCtx cx;
-        cx.hit_yz = hit_yz;
-        cx.hit_idx = hit_idx;
-        cx.bin_start = bin_start;
-        cx.ro = row_offsets + (size_t)inst * g.R;
-        cx.slab_base = inst * g.R;
-        cx.z0 = grid_z0(g, inst);
-        cx.s_rowx = s_rowx;
-        const int32_t* ch = cand_hits + c * kCandMax;
-        uint16_t* rowhit = tl_rowhit + c * g.RP;
-        tl_nhits[c] = 0;  // overwritten at the end if a tracklet results
-        // seed from hits 0, n/2, n-1
-        const int i1 = n >> 1, i2 = n - 1;
-        const float4 h0 = __ldg(&clusters[ch[0]]), h1 = __ldg(&clusters[ch[i1]]), h2 = __ldg(&clusters[ch[i2]]);
-        // The state carries y and z relative to the first candidate hit.  The model is translation invariant in y
-        // and z, so this is exact; it keeps the fp32 rounding of the two coordinates (ulp(20 cm), ulp(250 cm)) out
-        // of q/pt and sinPhi, whose sensitivity to position noise is ~50/cm on 10-row tracklets.
-        cx.yref = h0.y;
-        cx.zref = h0.z;
-        KfState st;
-        if (!kf_seed(st, s_rowx[r0], 0.0f, 0.0f, s_rowx[r0 + i1], h1.y - cx.yref, s_rowx[r0 + i2], h2.y - cx.yref,
-                     h2.z - cx.zref, g.cB, g.max_s, g.p0))
-            continue;
-        float chi2 = 0.0f;
-        int nhits = 0;
-        // phase A: the candidate's own hits ...
-        bool ok = true;
-        for (int i = 0; i < n; i++) {
-            const int hg = ch[i];
-            if (i > 0 && !kf_transport(st, s_rowx[r0 + i] - s_rowx[r0 + i - 1], g.cB, g.max_s)) {
-                ok = false;
-                break;
+
+    // lane state
+    int mode = kIdle;
+    int c = 0, r = 0, r0 = 0, n = 0, i = 0, slab_base = 0;
+    int nhits = 0, gap = 0, first_row = 0, last_row = 0;
+    float yref = 0.0f, zref = 0.0f, z0 = 0.0f, chi2 = 0.0f;
+    KfState st = {};
+
+    for (;;) {
+        unsigned act = __ballot_sync(full, mode < kDone);
+        if (act == 0u || (!exhausted && 32 - __popc(act) >= kFollowReload)) {
+            // ---- write-out of ended candidates ----
+            if (mode == kDone) {
+                const float4 q0 = s_rep[0][threadIdx.x], q1 = s_rep[1][threadIdx.x], q2 = s_rep[2][threadIdx.x],
+                             q3 = s_rep[3][threadIdx.x], q4 = s_rep[4][threadIdx.x];
+                float* p = a.tl_par + (size_t)c * 5;
+                p[0] = q0.x + yref; p[1] = q0.y + zref; p[2] = q0.z; p[3] = q0.w; p[4] = q1.x;
+                float* q = a.tl_cov + (size_t)c * 15;
+                q[0] = q1.y; q[1] = q1.z; q[2] = q1.w; q[3] = q2.x; q[4] = q2.y; q[5] = q2.z; q[6] = q2.w;
+                q[7] = q3.x; q[8] = q3.y; q[9] = q3.z; q[10] = q3.w; q[11] = q4.x; q[12] = q4.y; q[13] = q4.z;
+                q[14] = q4.w;
+                a.tl_chi2[c] = chi2;
+                a.tl_rows[c] = first_row | (last_row << 8) | (first_row << 16);
+                a.tl_nhits[c] = nhits;
+                mode = kIdle;
             }
-            const float4 h = __ldg(&clusters[hg]);
-            chi2 += kf_update(st, h.y - cx.yref, h.z - cx.zref, g.sy2, g.sz2);
-            wc.transports += i > 0;
-            wc.updates++;
-            rowhit[r0 + i] = (uint16_t)(hg - cx.ro[r0 + i]);
-            nhits++;
+            // ---- refill ----
+            if (!exhausted) {
+                if (wn == we) {
+                    unsigned long long v = 0;
+                    if (lane == 0) v = atomicAdd(queue, (unsigned long long)kFollowChunk);
+                    v = __shfl_sync(full, v, 0);
+                    if (v >= (unsigned long long)n_cand) {
+                        exhausted = true;
+                    } else {
+                        wn = (int)v;
+                        we = min(wn + kFollowChunk, n_cand);
+                    }
+                }
+                const unsigned idle = __ballot_sync(full, mode == kIdle);
+                const int mine = wn + __popc(idle & below);
+                if (mode == kIdle && mine < we) {
+                    c = mine;
+                    const int slab0 = a.cand_slab[c];
+                    const int inst = slab0 / g.R;
+                    r0 = slab0 - inst * g.R;
+                    n = a.cand_n[c];
+                    slab_base = inst * g.R;
+                    z0 = grid_z0(g, inst);
+                    const int32_t* ch = a.cand_hits + (size_t)c * kCandMax;
+                    // seed from hits 0, n/2, n-1
+                    const int i1 = n >> 1, i2 = n - 1;
+                    const float4 h0 = __ldg(&a.clusters[ch[0]]), h1 = __ldg(&a.clusters[ch[i1]]),
+                                 h2 = __ldg(&a.clusters[ch[i2]]);
+                    // The state carries y and z relative to the first candidate hit.  The model is translation
+                    // invariant in y and z, so this is exact; it keeps the fp32 rounding of the two coordinates
+                    // (ulp(20 cm), ulp(250 cm)) out of q/pt and sinPhi, whose sensitivity to position noise is
+                    // ~50/cm on 10-row tracklets.
+                    yref = h0.y;
+                    zref = h0.z;
+                    if (kf_seed(st, s_rowx[r0], 0.0f, 0.0f, s_rowx[r0 + i1], h1.y - yref, s_rowx[r0 + i2], h2.y - yref,
+                                h2.z - zref, g.cB, g.max_s, g.p0)) {
+                        mode = kCand;
+                        i = 0;
+                        r = r0;
+                        chi2 = 0.0f;
+                        nhits = 0;
+                        gap = 0;
+                        first_row = r0;
+                        last_row = r0;
+                    } else {  // no tracklet: an all-zero record
+                        nhits = 0;
+                        chi2 = yref = zref = 0.0f;
+                        first_row = last_row = 0;
+#pragma unroll
+                        for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        mode = kDone;
+                    }
+                }
+                wn = min(we, wn + __popc(idle));
+            }
+            act = __ballot_sync(full, mode < kDone);
+            if (act == 0u && exhausted) break;
         }
-        if (!ok) continue;
-        // ... then upward pick-up
-        int last_row = r0 + n - 1;
-        const int r_top = follow_dir<+1>(g, cx, st, last_row, chi2, nhits, last_row, rowhit, nullptr, wc);
-        // phase B: one step back to the start row (no update there), then downward pick-up
-        if (!kf_transport(st, s_rowx[r0] - s_rowx[r_top], g.cB, g.max_s)) continue;
-        wc.transports++;
-        KfState rep = st;
-        int first_row = r0;
-        follow_dir<-1>(g, cx, st, r0, chi2, nhits, first_row, rowhit, &rep, wc);
-        float* p = tl_par + c * 5;
-        p[0] = rep.y + cx.yref; p[1] = rep.z + cx.zref; p[2] = rep.s; p[3] = rep.t; p[4] = rep.k;
-        float* q = tl_cov + c * 15;
-        q[0] = rep.c00; q[1] = rep.c10; q[2] = rep.c11; q[3] = rep.c20; q[4] = rep.c21; q[5] = rep.c22; q[6] = rep.c30;
-        q[7] = rep.c31; q[8] = rep.c32; q[9] = rep.c33; q[10] = rep.c40; q[11] = rep.c41; q[12] = rep.c42;
-        q[13] = rep.c43; q[14] = rep.c44;
-        tl_chi2[c] = chi2;
-        tl_rows[c] = first_row | (last_row << 8) | (first_row << 16);
-        tl_nhits[c] = nhits;
+        if (mode < kDone) {
+            // ---- one pad row ----
+            const int rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : (mode == kCand ? r0 + i : r + 1));
+            const int32_t row_base = a.row_offsets[slab_base + rn];
+            bool alive = true;
+            if (rn != r) {
+                if (kf_transport(st, s_rowx[rn] - s_rowx[r], g.cB, g.max_s)) {
+                    wc.transports++;
+                    r = rn;
+                } else {
+                    alive = false;
+                    if (mode == kUp) {
+                        mode = kBack;
+                    } else if (mode == kDown) {
+                        mode = kDone;
+                    } else {  // inside the candidate's own hits, or the back transport: no tracklet
+                        nhits = 0;
+                        chi2 = yref = zref = 0.0f;
+                        first_row = last_row = 0;
+#pragma unroll
+                        for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        mode = kDone;
+                    }
+                }
+            }
+            if (alive && mode == kBack) {
+                // phase B starts: the reported state is the back-transported one until a hit is attached
+                mode = r0 > 0 ? kDown : kDone;
+                gap = 0;
+                s_rep[0][threadIdx.x] = make_float4(st.y, st.z, st.s, st.t);
+                s_rep[1][threadIdx.x] = make_float4(st.k, st.c00, st.c10, st.c11);
+                s_rep[2][threadIdx.x] = make_float4(st.c20, st.c21, st.c22, st.c30);
+                s_rep[3][threadIdx.x] = make_float4(st.c31, st.c32, st.c33, st.c40);
+                s_rep[4][threadIdx.x] = make_float4(st.c41, st.c42, st.c43, st.c44);
+                alive = false;
+            }
+            if (alive) {
+                uint16_t* rowhit = a.tl_rowhit + (size_t)c * g.RP;
+                float ym = 0.0f, zm = 0.0f;
+                int li = -1;  // local index of the hit to attach
+                bool have = false;
+                bool stop = false;
+                if (mode == kCand) {
+                    const int hg = a.cand_hits[(size_t)c * kCandMax + i];
+                    const float4 h = __ldg(&a.clusters[hg]);
+                    ym = h.y;
+                    zm = h.z;
+                    li = hg - row_base;
+                    have = true;
+                } else {
+                    const float yp = st.y + yref, zp = st.z + zref;
+                    if (fabsf(yp) > fmaf(s_rowx[r], g.tan_half, g.edge_margin)) {
+                        stop = true;
+                        alive = false;
+                    } else {
+                        const float vy = st.c00 + g.sy2, vz = st.c11 + g.sz2;  // > 0: sigma > 0 (tpc_tracker_create)
+                        const float wy = fminf(g.wmax, g.gate * (vy * rsqrtf(vy)));
+                        const float wz = fminf(g.wmax, g.gate * (vz * rsqrtf(vz)));
+                        const float2 gy = s_rowy[r];
+                        const int j = pick_up(g, a.hit_yz + row_base, a.hit_idx + row_base,
+                                              a.bin_start + (size_t)(slab_base + r) * g.nzp, z0, gy.x, gy.y, yp, zp,
+                                              wy, wz, ym, zm, wc);
+                        have = j >= 0;  // (the index load below is not on the path to the update)
+                        if (have) li = a.hit_idx[row_base + j];
+                    }
+                }
+                if (alive) {
+                    if (have) {
+                        __stcs(&rowhit[r], (uint16_t)li);
+                        chi2 += kf_update(st, ym - yref, zm - zref, g.sy2, g.sz2);
+                        wc.updates++;
+                        nhits++;
+                        gap = 0;
+                        if (mode == kDown) {
+                            first_row = r;
+                            s_rep[0][threadIdx.x] = make_float4(st.y, st.z, st.s, st.t);
+                            s_rep[1][threadIdx.x] = make_float4(st.k, st.c00, st.c10, st.c11);
+                            s_rep[2][threadIdx.x] = make_float4(st.c20, st.c21, st.c22, st.c30);
+                            s_rep[3][threadIdx.x] = make_float4(st.c31, st.c32, st.c33, st.c40);
+                            s_rep[4][threadIdx.x] = make_float4(st.c41, st.c42, st.c43, st.c44);
+                        } else {
+                            last_row = r;
+                        }
+                    } else {
+                        __stcs(&rowhit[r], kNoHit);
+                        if (++gap > g.max_gap) stop = true;
+                    }
+                }
+                // where the next iteration goes
+                if (mode == kCand) {
+                    if (++i == n) mode = kUp;
+                }
+                if (mode == kUp) {
+                    if (stop || r + 1 >= g.R) mode = kBack;
+                } else if (mode == kDown) {
+                    if (stop || r == 0) mode = kDone;
+                }
+            }
+            if (mode == kUp || mode == kDown) {
+                // The lane searches row r+dir next and probably the rows after it.  Every search is two dependent loads
+                // (cell table, then hits) from lines no other lane has touched recently, so warm them up now: the
+                // table line three rows ahead and, through the table line two rows ahead (warmed an iteration ago), the
+                // hit line two rows ahead.
+                // Straight-line predictions with the curvature term; being wrong only costs time.
+                const int dir = mode == kUp ? 1 : -1;
+                const int r2 = min(max(r + 2 * dir, 0), g.R - 1), r3 = min(max(r + 3 * dir, 0), g.R - 1);
+                const float ic = rsqrtf((1.0f - st.s) * (1.0f + st.s));
+                const float tgp = st.s * ic, hk = 0.5f * g.cB * st.k * ic * ic * ic, tz = st.t * ic;
+                const float d2 = s_rowx[r2] - s_rowx[r], d3 = s_rowx[r3] - s_rowx[r];
+                const float ya = st.y + yref, za = st.z + zref;
+                const float y2 = ya + d2 * (tgp + hk * d2), z2 = za + d2 * tz;
+                const float y3 = ya + d3 * (tgp + hk * d3), z3 = za + d3 * tz;
+                const float2 g2 = s_rowy[r2], g3 = s_rowy[r3];
+                const uint16_t* t3 = a.bin_start + (size_t)(slab_base + r3) * g.nzp;
+                prefetch_l1(t3 + zbin(z3, z0, g.inv_cz, g.nz) * g.ny + ybin(y3, g3.x, g3.y, g.ny));
+                const uint16_t* t2 = a.bin_start + (size_t)(slab_base + r2) * g.nzp;
+                const int j2 = t2[zbin(z2, z0, g.inv_cz, g.nz) * g.ny + ybin(y2 - 0.5f, g2.x, g2.y, g.ny)];
+                const float2* h2 = a.hit_yz + a.row_offsets[slab_base + r2] + j2;
+                prefetch_l1(h2);
+                prefetch_l1(h2 + 3);
+            }
+        }
     }
     // work counters: warp reduction, one atomic per warp and counter
     unsigned v[4] = {wc.transports, wc.updates, wc.examined, wc.searches};
 #pragma unroll
     for (int q = 0; q < 4; q++) {
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], d);
-        if ((threadIdx.x & 31) == 0 && v[q]) atomicAdd((unsigned long long*)&counts[6 + q], (unsigned long long)v[q]);
+        for (int d = 16; d > 0; d >>= 1) v[q] += __shfl_xor_sync(full, v[q], d);
+        if (lane == 0 && v[q]) atomicAdd((unsigned long long*)&a.counts[6 + q], (unsigned long long)v[q]);
     }
 }
 
 int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, cudaStream_t s) {
     if (p.n_clusters == 0) return 0;
-    // grid-stride over the (device-side) candidate count: enough CTAs to fill the machine, capped by the bound
+    // persistent grid: every SM holds kFollowCtasPerSm CTAs, capped by the candidate bound
     int64_t want = div_up(w.Cmax, kFollowThreads);
-    int grid = (int)(want < (int64_t)n_sm * 16 ? want : (int64_t)n_sm * 16);
+    int grid = (int)(want < (int64_t)n_sm * kFollowCtasPerSm ? want : (int64_t)n_sm * kFollowCtasPerSm);
     if (grid < 1) grid = 1;
-    follow_kernel<<<grid, kFollowThreads, 0, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
-                                                  w.cand_hits, w.cand_n, w.cand_slab, w.counts, w.Cmax, w.tl_par,
-                                                  w.tl_cov, w.tl_chi2, w.tl_nhits, w.tl_rows, w.tl_rowhit);
+    FollowArgs a{p.clusters, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.cand_hits, w.cand_n, w.cand_slab,
+                 w.counts,   w.Cmax,        w.tl_par, w.tl_cov,  w.tl_chi2,   w.tl_nhits,  w.tl_rows, w.tl_rowhit};
+    follow_kernel<<<grid, kFollowThreads, 0, s>>>(g, a);
     return 1;
 }
 

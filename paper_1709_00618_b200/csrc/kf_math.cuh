@@ -32,9 +32,10 @@ __device__ __forceinline__ bool kf_transport(KfState& st, float dx, float cB, fl
     const float c0sq = (1.0f - s) * (1.0f + s), c1sq = (1.0f - s1) * (1.0f + s1);
     const float ic0 = rsqrtf(c0sq), ic1 = rsqrtf(c1sq);
     const float c0 = c0sq * ic0, c1 = c1sq * ic1;
-    const float tg = (s + s1) / (c0 + c1);
+    const float tg = __fdividef(s + s1, c0 + c1);
     const float sec2 = fmaf(tg, tg, 1.0f);
-    const float chord = dx * sqrtf(sec2);
+    const float isec = rsqrtf(sec2);  // sec2 >= 1
+    const float chord = dx * (sec2 * isec);
     const float a = 0.5f * kap * chord;
     const float dS = chord * asin_over(a);
     // Jacobian entries (identity elsewhere)
@@ -52,7 +53,7 @@ __device__ __forceinline__ bool kf_transport(KfState& st, float dx, float cB, fl
     const float hh = 0.5f * kap * dS, h2 = hh * hh;
     if (h2 < 0.09f) {
         const float ser = 1.0f + h2 * (-0.1f + h2 * (1.0f / 280.0f - h2 * (1.0f / 15120.0f)));
-        ddS = (0.5f * tg * dx * dS + kap * dS * dS * dS * (1.0f / 12.0f) * rsqrtf(sec2) * ser) * ic1;
+        ddS = (0.5f * tg * dx * dS + kap * dS * dS * dS * (1.0f / 12.0f) * isec * ser) * ic1;
     } else {
         ddS = (dx * ic1 - dS) / kap;
     }
@@ -95,7 +96,7 @@ __device__ __forceinline__ bool kf_transport(KfState& st, float dx, float cB, fl
 __device__ __forceinline__ float kf_update(KfState& st, float ym, float zm, float sy2, float sz2) {
     float chi2;
     {
-        const float inv = 1.0f / (st.c00 + sy2);
+        const float inv = __fdividef(1.0f, st.c00 + sy2);
         const float res = ym - st.y;
         const float k0 = st.c00 * inv, k1 = st.c10 * inv, k2 = st.c20 * inv, k3 = st.c30 * inv, k4 = st.c40 * inv;
         const float r = sy2 * inv;  // column 0 shrinks by sigma^2/S (no cancellation)
@@ -122,7 +123,7 @@ __device__ __forceinline__ float kf_update(KfState& st, float ym, float zm, floa
         st.c40 *= r;
     }
     {
-        const float inv = 1.0f / (st.c11 + sz2);
+        const float inv = __fdividef(1.0f, st.c11 + sz2);
         const float res = zm - st.z;
         const float k0 = st.c10 * inv, k1 = st.c11 * inv, k2 = st.c21 * inv, k3 = st.c31 * inv, k4 = st.c41 * inv;
         const float r = sz2 * inv;

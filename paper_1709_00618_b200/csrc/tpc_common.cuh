@@ -8,7 +8,7 @@ namespace tpc {
 
 constexpr int kCandMax = 10;      // TPC_CAND_MAX_HITS
 constexpr int kMaxRows = 255;
-constexpr int kMaxZBins = 2047;
+constexpr int kMaxCells = 16384;  // cells of one row's grid (positions and the table are 16 bit; S1 keeps 4 B/cell in smem)
 constexpr uint16_t kNoHit = 0xFFFFu;
 constexpr float kKappaPerTesla = 0.00299792458f;
 
@@ -18,7 +18,9 @@ struct DevGeom {
     int R;          // pad rows
     int RP;         // row stride of the per-tracklet hit table (R rounded up to 8)
     int nz;         // z bins per row
-    int nzp;        // stride of the bin table (nz + 1 rounded up to 2)
+    int ny;         // y strips per row
+    int ncell;      // nz * ny cells per row, cell id = zbin * ny + ystrip (a y range inside one z bin is contiguous)
+    int nzp;        // stride of the cell table (ncell + 1 rounded up to 16 entries = 32 B)
     int spe, spe_half;
     float z0_a, z0_c;  // grid origin: z >= 0 side, z < 0 side
     float inv_cz;
@@ -32,13 +34,15 @@ struct DevGeom {
     float sy2, sz2;
     float cB;       // curvature per (q/pt): kappa = cB * q/pt
     const float* row_x;  // device [R]
+    const float* row_y0;      // device [R] lower edge of the row's y grid: -(row half-width + 0.5 cm)
+    const float* row_inv_sy;  // device [R] strips per cm of that row
 };
 
 // Views into the caller's workspace (all device pointers), fixed per call.
 struct Workspace {
-    float2* hit_yz;       // [N]  (y, z) sorted by z bin inside every (instance,row) segment
+    float2* hit_yz;       // [N]  (y, z) sorted by grid cell inside every (instance,row) segment
     uint16_t* hit_idx;    // [N]  local index (position in the row segment of the INPUT) of the sorted hit
-    uint16_t* bin_start;  // [S*R][nzp] first sorted position of every z bin, entry nz = row length
+    uint16_t* bin_start;  // [S*R][nzp] first sorted position of every grid cell, entry ncell = row length
     int32_t* up_raw;      // [N] global indices
     int32_t* dn_raw;
     int32_t* up;          // cleaned
@@ -75,6 +79,12 @@ __host__ __device__ inline int div_up(int64_t a, int64_t b) { return (int)((a + 
 __device__ __forceinline__ int zbin(float z, float z0, float inv_cz, int nz) {
     int b = __float2int_rd(__fmul_rn(__fsub_rn(z, z0), inv_cz));
     return min(max(b, 0), nz - 1);
+}
+
+// y strip of the per-row grid: same construction, so monotone non-decreasing in y.
+__device__ __forceinline__ int ybin(float y, float y0, float inv_sy, int ny) {
+    int b = __float2int_rd(__fmul_rn(__fsub_rn(y, y0), inv_sy));
+    return min(max(b, 0), ny - 1);
 }
 
 __device__ __forceinline__ float grid_z0(const DevGeom& g, int inst) {

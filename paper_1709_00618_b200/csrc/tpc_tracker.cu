@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/tpc_tracker.h"
 #include "tpc_common.cuh"
@@ -42,12 +43,22 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     DevGeom& g = t->g;
     g.R = R;
     g.RP = (R + 7) & ~7;
-    const float cz = dflt(p.grid_cell_z, 2.5f);
+    // per-row 2-D grid: ny strips across the row, z bins of cz (performance only, no result depends on either).
+    // Default cz = 6.25 cm > 2 * max(kf_win_max, nf_win_z) + margins, so a search window touches at most 2 z bins.
+    int ny = dflt(p.grid_cells_y, 16);
+    if (ny < 1) ny = 1;
+    if (ny > 64) ny = 64;
+    float cz = dflt(p.grid_cell_z, 6.25f);
     int nz = (int)std::ceil(((double)geom->z_hi - (double)geom->z_lo) / cz);
     if (nz < 1) nz = 1;
-    if (nz > kMaxZBins) nz = kMaxZBins;
+    if ((int64_t)nz * ny > kMaxCells) {  // too fine: widen the z bins until the row grid fits
+        nz = kMaxCells / ny;
+        cz = (float)(((double)geom->z_hi - (double)geom->z_lo) / nz);
+    }
     g.nz = nz;
-    g.nzp = (nz + 2) & ~1;
+    g.ny = ny;
+    g.ncell = nz * ny;
+    g.nzp = (g.ncell + 1 + 15) & ~15;  // rows of the table start on 32-byte sectors
     g.spe = geom->sectors_per_event;
     g.spe_half = g.spe / 2;
     g.z0_a = geom->z_lo;
@@ -75,8 +86,15 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
         g_create_err = "cand_min_hits/cand_max_hits out of range (2 <= min <= max <= 10, max >= 3)";
         return TPC_ERR_ARG;
     }
-    cudaError_t e = cudaMalloc(&t->d_row_x, sizeof(float) * R);
-    if (e == cudaSuccess) e = cudaMemcpy(t->d_row_x, geom->row_x, sizeof(float) * R, cudaMemcpyHostToDevice);
+    std::vector<float> rows(3 * (size_t)R);
+    for (int r = 0; r < R; r++) {
+        const float hw = geom->row_x[r] * g.tan_half + 0.5f;  // half-width of the row's y grid
+        rows[r] = geom->row_x[r];
+        rows[R + r] = -hw;
+        rows[2 * R + r] = (float)ny / (2.0f * hw);
+    }
+    cudaError_t e = cudaMalloc(&t->d_row_x, sizeof(float) * 3 * R);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_row_x, rows.data(), sizeof(float) * 3 * R, cudaMemcpyHostToDevice);
     int dev = 0;
     if (e == cudaSuccess) e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&t->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -87,6 +105,8 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
         return TPC_ERR_CUDA;
     }
     g.row_x = t->d_row_x;
+    g.row_y0 = t->d_row_x + R;
+    g.row_inv_sy = t->d_row_x + 2 * R;
     *out = t;
     return TPC_OK;
 }

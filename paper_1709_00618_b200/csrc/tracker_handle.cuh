@@ -7,7 +7,7 @@
 
 struct tpc_tracker {
     tpc::DevGeom g;
-    float* d_row_x = nullptr;
+    float* d_row_x = nullptr;  // [3][R]: row_x, row_y0, row_inv_sy
     void* ws = nullptr;
     size_t ws_bytes = 0;
     cudaStream_t stream = nullptr;
