@@ -8,8 +8,8 @@
 // pre-rounded bounds, and the minimum is taken over (D, u, d) lexicographically, so the result does not depend on
 // the order in which the grid presents the hits.  This file is additionally compiled with -fmad=false.
 //
-// One CTA per (sector instance, pad row).  The sorted (y,z), the original indices and the cell tables of the two
-// adjacent rows are staged in shared memory; rows or tables too long for that are read in place.  Per hit the
+// One CTA per (sector instance, pad row).  The sorted (y,z) and the cell tables of the two adjacent rows are
+// staged in shared memory; rows or tables too long for that are read in place.  Per hit the
 // search is three flat loops instead of a nested one: window hits of row r+1, window hits of row r-1 (each through
 // the 2-D grid, a handful of candidates), then the pairs of the two short lists.
 #include "tpc_common.cuh"
@@ -17,7 +17,7 @@
 namespace tpc {
 
 constexpr int kNbThreads = 128;
-constexpr int kNbStageHits = 1024;  // max hits of row r-1 plus row r+1 staged in shared memory (10 B each)
+constexpr int kNbStageHits = 1024;  // max hits of row r-1 plus row r+1 staged in shared memory (8 B each)
 constexpr int kNbStageTbl = 4096;   // max table entries per row staged in shared memory (2 B each, two rows)
 constexpr int kNbList = 4;          // window hits per neighbour row kept in registers; more -> exact slow path
 
@@ -30,14 +30,22 @@ struct RowView {
 
 struct Best {
     float D;
-    int iu, id;  // local indices, -1 = none
+    int ju, jd;  // positions in the sorted rows r+1 / r-1, -1 = none
 };
 
-__device__ __forceinline__ void consider(Best& b, float D, int iu, int id) {
-    if (b.iu < 0 || D < b.D || (D == b.D && (iu < b.iu || (iu == b.iu && id < b.id)))) {
+// Keep the minimum over (D, local index of u, local index of d); the local indices (positions in the INPUT row
+// segments) are only loaded to break exact ties of D, so the result does not depend on the sorted order.
+__device__ __forceinline__ void consider(Best& b, float D, int ju, int jd, const uint16_t* __restrict__ idx_up,
+                                         const uint16_t* __restrict__ idx_dn) {
+    bool better = b.ju < 0 || D < b.D;
+    if (!better && D == b.D) {
+        const int iu = idx_up[ju], bu = idx_up[b.ju];
+        better = iu < bu || (iu == bu && idx_dn[jd] < idx_dn[b.jd]);
+    }
+    if (better) {
         b.D = D;
-        b.iu = iu;
-        b.id = id;
+        b.ju = ju;
+        b.jd = jd;
     }
 }
 
@@ -72,7 +80,6 @@ __device__ __noinline__ void search_dense(const DevGeom& g, const RowView& up, c
             const float2 u = up.yz[a];
             if (!(ylo <= u.x && u.x <= yhi && zlo <= u.y && u.y <= zhi)) continue;
             const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
-            const int iu = up.idx[a];
             for (int zd = zb0; zd <= zb1; zd++) {
                 const int d0 = dn.tbl[zd * g.ny + ds0], d1 = dn.tbl[zd * g.ny + ds1 + 1];
                 for (int b = d0; b < d1; b++) {
@@ -81,7 +88,7 @@ __device__ __noinline__ void search_dense(const DevGeom& g, const RowView& up, c
                     const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
                     const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
                     const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
-                    if (D <= g.nf_d2max) consider(best, D, iu, dn.idx[b]);
+                    if (D <= g.nf_d2max) consider(best, D, a, b, up.idx, dn.idx);
                 }
             }
         }
@@ -89,7 +96,7 @@ __device__ __noinline__ void search_dense(const DevGeom& g, const RowView& up, c
 }
 
 __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const float2* my_yz,
-                                           const uint16_t* my_idx, int n, float z0, int base, int base_up,
+                                           int n, float z0, int base, int base_up,
                                            int base_dn, int32_t* __restrict__ link_up,
                                            int32_t* __restrict__ link_dn) {
     const float WY = g.nf_wy, WZ = g.nf_wz, D2MAX = g.nf_d2max;
@@ -109,7 +116,6 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
             for (int a = 0; a < nu; a++, lu >>= 16) {
                 const int ja = (int)(lu & 0xffffull);
                 const float2 u = up.yz[ja];
-                const int iu = up.idx[ja];
                 const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
                 unsigned long long l = ld;
                 for (int b = 0; b < nd; b++, l >>= 16) {
@@ -118,13 +124,14 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
                     const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
                     const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
                     const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
-                    if (D <= D2MAX) consider(best, D, iu, dn.idx[jb]);
+                    if (D <= D2MAX) consider(best, D, ja, jb, up.idx, dn.idx);
                 }
             }
         }
-        const int me = base + my_idx[i];
-        link_up[me] = best.iu < 0 ? -1 : base_up + best.iu;
-        link_dn[me] = best.id < 0 ? -1 : base_dn + best.id;
+        // links live in SORTED space: entry base + i belongs to the i-th hit of the sorted row, values are sorted
+        // global positions; coalesced stores
+        link_up[base + i] = best.ju < 0 ? -1 : base_up + best.ju;
+        link_dn[base + i] = best.jd < 0 ? -1 : base_dn + best.jd;
     }
 }
 
@@ -153,11 +160,11 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
                g.row_inv_sy[r + 1]};
     RowView dn{hit_yz + base_dn, hit_idx + base_dn, bin_start + (size_t)(slab - 1) * g.nzp, g.row_y0[r - 1],
                g.row_inv_sy[r - 1]};
-    // shared layout: tbl_up[nzp] tbl_dn[nzp] (if staged) | yz_up[n_up] yz_dn[n_dn] | idx_up[n_up] idx_dn[n_dn]
+    // shared layout: tbl_up[nzp] tbl_dn[nzp] (if staged) | yz_up[n_up] yz_dn[n_dn]; the local indices are only read
+    // to break exact ties and stay in global memory
     const bool stage_tbl = g.nzp <= kNbStageTbl;
     uint4* s_tbl = reinterpret_cast<uint4*>(sm_raw);
     float2* s_yz = reinterpret_cast<float2*>(sm_raw + (stage_tbl ? (size_t)g.nzp * 4 : 0));
-    uint16_t* s_idx = reinterpret_cast<uint16_t*>(s_yz + kNbStageHits);
     if (stage_tbl) {
         const int q = g.nzp / 8;  // 16-byte groups per table
         const uint4* gu = reinterpret_cast<const uint4*>(up.tbl);
@@ -170,25 +177,17 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
         dn.tbl = reinterpret_cast<const uint16_t*>(s_tbl + q);
     }
     if (n_up + n_dn <= kNbStageHits) {
-        for (int i = threadIdx.x; i < n_up; i += kNbThreads) {
-            s_yz[i] = __ldg(&up.yz[i]);
-            s_idx[i] = __ldg(&up.idx[i]);
-        }
-        for (int i = threadIdx.x; i < n_dn; i += kNbThreads) {
-            s_yz[n_up + i] = __ldg(&dn.yz[i]);
-            s_idx[n_up + i] = __ldg(&dn.idx[i]);
-        }
+        for (int i = threadIdx.x; i < n_up; i += kNbThreads) s_yz[i] = __ldg(&up.yz[i]);
+        for (int i = threadIdx.x; i < n_dn; i += kNbThreads) s_yz[n_up + i] = __ldg(&dn.yz[i]);
         up.yz = s_yz;
-        up.idx = s_idx;
         dn.yz = s_yz + n_up;
-        dn.idx = s_idx + n_up;
     }
     __syncthreads();
-    search_row(g, up, dn, hit_yz + base, hit_idx + base, n, z0, base, base_up, base_dn, link_up, link_dn);
+    search_row(g, up, dn, hit_yz + base, n, z0, base, base_up, base_dn, link_up, link_dn);
 }
 
 static size_t nb_smem_bytes(const DevGeom& g) {
-    return (size_t)kNbStageHits * (sizeof(float2) + sizeof(uint16_t)) + (g.nzp <= kNbStageTbl ? (size_t)g.nzp * 4 : 0);
+    return (size_t)kNbStageHits * sizeof(float2) + (g.nzp <= kNbStageTbl ? (size_t)g.nzp * 4 : 0);
 }
 
 int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s) {

@@ -100,43 +100,81 @@ scan_int2_kernel(int2* __restrict__ part, const int64_t* __restrict__ m_dev, int
     }
 }
 
-// S4 pass 2: ranked write of start hits and candidates.
+// S4 pass 2: ranked write of start hits and candidates.  Links and flags live in sorted space, but start hits and
+// candidates are numbered in ascending INPUT index of the start hit, so the rank inside the slab is
+// taken over the input positions: one bit per input position in shared memory, popcount prefix per word.
+constexpr int kChainMaxBits = 8192;  // rows up to this length use the bitmaps; longer rows count by brute force
+constexpr int kChainWords = kChainMaxBits / 32;
+
 __global__ void __launch_bounds__(kChainThreads)
 chain_write_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
-                   const int32_t* __restrict__ up, const uint8_t* __restrict__ flags,
-                   const int2* __restrict__ slab_part, int32_t* __restrict__ start_hits, int64_t start_cap,
-                   int32_t* __restrict__ cand_hits, int32_t* __restrict__ cand_n, int32_t* __restrict__ cand_slab,
-                   int64_t cand_cap, int32_t* __restrict__ usr_cand_hits, int32_t* __restrict__ usr_cand_n,
-                   int64_t usr_cand_cap) {
-    __shared__ int2 s_warp[kChainThreads / 32];
+                   const uint16_t* __restrict__ hit_idx, const int32_t* __restrict__ up,
+                   const uint8_t* __restrict__ flags, const int2* __restrict__ slab_part,
+                   int32_t* __restrict__ start_hits, int64_t start_cap, int32_t* __restrict__ cand_hits,
+                   int32_t* __restrict__ cand_n, int32_t* __restrict__ cand_slab, int64_t cand_cap,
+                   int32_t* __restrict__ usr_cand_hits, int32_t* __restrict__ usr_cand_n, int64_t usr_cand_cap) {
+    __shared__ uint32_t s_bits[2][kChainWords];  // [0] start hits, [1] candidates, by input position
+    __shared__ uint16_t s_pre[2][kChainWords];   // set bits in the words before
     const int slab = blockIdx.x;
-    const int base = row_offsets[slab], n = row_offsets[slab + 1] - base;
+    const int base = row_offsets[slab], n = min(row_offsets[slab + 1] - base, 65535);
     const int2 sb = slab_part[slab];
     if (slab_part[slab + 1].x == sb.x) return;  // no start hit in this slab
-    int run_s = sb.x, run_c = sb.y;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    for (int start = 0; start < n; start += kChainThreads) {
-        const int i = start + threadIdx.x;
-        const int h = base + i;
-        const uint8_t f = i < n ? flags[h] : 0;
-        const unsigned ms = __ballot_sync(0xffffffffu, f & 1), mc = __ballot_sync(0xffffffffu, f & 2);
-        if (lane == 0) s_warp[wid] = make_int2(__popc(ms), __popc(mc));
+    const bool bitmap = n <= kChainMaxBits;
+    const int words = (n + 31) >> 5;
+    if (bitmap) {
+        for (int w = threadIdx.x; w < words; w += kChainThreads) s_bits[0][w] = s_bits[1][w] = 0u;
         __syncthreads();
-        int os = run_s, oc = run_c, ts = 0, tc = 0;
+        for (int i = threadIdx.x; i < n; i += kChainThreads) {
+            const uint8_t f = flags[base + i];
+            if (f) {
+                const int li = hit_idx[base + i];
+                atomicOr(&s_bits[0][li >> 5], 1u << (li & 31));
+                if (f & 2) atomicOr(&s_bits[1][li >> 5], 1u << (li & 31));
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x < 64) {  // warp 0: start hits, warp 1: candidates
+            const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
+            int carry = 0;
+            for (int w0 = 0; w0 < words; w0 += 32) {
+                const int w = w0 + lane;
+                const int v = w < words ? __popc(s_bits[q][w]) : 0;
+                int incl = v;
 #pragma unroll
-        for (int k = 0; k < kChainThreads / 32; k++) {
-            const int2 v = s_warp[k];
-            if (k < wid) { os += v.x; oc += v.y; }
-            ts += v.x;
-            tc += v.y;
+                for (int d = 1; d < 32; d <<= 1) {
+                    const int t = __shfl_up_sync(0xffffffffu, incl, d);
+                    if (lane >= d) incl += t;
+                }
+                if (w < words) s_pre[q][w] = (uint16_t)(carry + incl - v);
+                carry += __shfl_sync(0xffffffffu, incl, 31);
+            }
         }
-        const unsigned below = (1u << lane) - 1u;
-        if (f & 1) {
-            const int64_t ps = os + __popc(ms & below);
-            if (start_hits && ps < start_cap) start_hits[ps] = h;
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < n; i += kChainThreads) {
+        const int h = base + i;
+        const uint8_t f = flags[h];
+        if (!f) continue;
+        const int li = hit_idx[h];
+        int rs, rc;  // start hits / candidates of this slab with a smaller input position
+        if (bitmap) {
+            const unsigned below = (1u << (li & 31)) - 1u;
+            rs = s_pre[0][li >> 5] + __popc(s_bits[0][li >> 5] & below);
+            rc = s_pre[1][li >> 5] + __popc(s_bits[1][li >> 5] & below);
+        } else {
+            rs = rc = 0;
+            for (int k = 0; k < n; k++) {
+                const uint8_t fk = flags[base + k];
+                if (fk && hit_idx[base + k] < li) {
+                    rs++;
+                    rc += fk >> 1;
+                }
+            }
         }
+        const int64_t ps = sb.x + rs;
+        if (start_hits && ps < start_cap) start_hits[ps] = base + li;
         if (f & 2) {
-            const int64_t c = oc + __popc(mc & below);
+            const int64_t c = sb.y + rc;
             int32_t hits[kCandMax];
             int k = 0;
             for (int x = h; x >= 0 && k < g.cand_max; x = __ldg(&up[x])) hits[k++] = x;
@@ -148,16 +186,32 @@ chain_write_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict_
                 cand_n[c] = nh;
                 cand_slab[c] = slab;
             }
-            if (usr_cand_hits && c < usr_cand_cap) {
+            if (usr_cand_hits && c < usr_cand_cap) {  // user-facing copy: input-order global indices
 #pragma unroll
-                for (int q = 0; q < kCandMax; q++) usr_cand_hits[c * kCandMax + q] = hits[q];
+                for (int q = 0; q < kCandMax; q++)
+                    usr_cand_hits[c * kCandMax + q] =
+                        q < nh ? row_offsets[slab + q] + (int32_t)hit_idx[hits[q]] : -1;
             }
             if (usr_cand_n && c < usr_cand_cap) usr_cand_n[c] = nh;
         }
-        run_s += ts;
-        run_c += tc;
-        __syncthreads();
     }
+}
+
+// Parity/debug export of one link array: sorted space -> input-order positions and values.  dir = +1 / -1 is the
+// row offset of the link targets.
+__global__ void __launch_bounds__(kChainThreads)
+export_links_kernel(const int32_t* __restrict__ row_offsets, const uint16_t* __restrict__ hit_idx,
+                    const int32_t* __restrict__ link, int dir, int n_slabs, int32_t* __restrict__ out) {
+    const int slab = blockIdx.x;
+    const int base = row_offsets[slab], n_all = row_offsets[slab + 1] - base;
+    const int n = min(n_all, 65535);
+    const int tslab = min(max(slab + dir, 0), n_slabs - 1);
+    const int tbase = row_offsets[tslab];
+    for (int i = threadIdx.x; i < n; i += kChainThreads) {
+        const int32_t v = link[base + i];
+        out[base + hit_idx[base + i]] = v < 0 ? -1 : tbase + (int32_t)hit_idx[v];
+    }
+    for (int i = n + threadIdx.x; i < n_all; i += kChainThreads) out[base + i] = -1;
 }
 
 int launch_clean(const DevGeom&, const Workspace& w, const Problem& p, cudaStream_t s) {
@@ -177,10 +231,18 @@ int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const 
     if (slabs == 0) return 0;
     chain_flags_kernel<<<slabs, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.dn, w.flags, w.slab_part);
     launch_scan_int2(w.slab_part, nullptr, 1, 0, slabs, w.counts, 0, 1, s);
-    chain_write_kernel<<<slabs, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.flags, w.slab_part, u.start_hits,
+    chain_write_kernel<<<slabs, kChainThreads, 0, s>>>(g, p.row_offsets, w.hit_idx, w.up, w.flags, w.slab_part, u.start_hits,
                                                        u.start_cap, w.cand_hits, w.cand_n, w.cand_slab, w.Cmax,
                                                        u.cand_hits, u.cand_n, u.cand_cap);
     return 3;
+}
+
+int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link, int dir,
+                        int32_t* out, cudaStream_t s) {
+    const int slabs = p.n_inst * g.R;
+    if (slabs == 0 || !out) return 0;
+    export_links_kernel<<<slabs, kChainThreads, 0, s>>>(p.row_offsets, w.hit_idx, link, dir, slabs, out);
+    return 1;
 }
 
 }  // namespace tpc

@@ -25,7 +25,6 @@ struct WorkCount {  // per-thread work counters (roofline arithmetic): summed in
 };
 
 struct FollowArgs {
-    const float4* clusters;
     const int32_t* row_offsets;
     const float2* hit_yz;
     const uint16_t* hit_idx;
@@ -42,8 +41,6 @@ struct FollowArgs {
     int32_t* tl_rows;
     uint16_t* tl_rowhit;
 };
-
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // One hit of the pick-up search: inside the gate and nearer than the best so far?  Ties -> lowest local index.
 struct PickBest {
@@ -190,16 +187,15 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     const int32_t* ch = a.cand_hits + (size_t)c * kCandMax;
                     // seed from hits 0, n/2, n-1
                     const int i1 = n >> 1, i2 = n - 1;
-                    const float4 h0 = __ldg(&a.clusters[ch[0]]), h1 = __ldg(&a.clusters[ch[i1]]),
-                                 h2 = __ldg(&a.clusters[ch[i2]]);
+                    const float2 h0 = a.hit_yz[ch[0]], h1 = a.hit_yz[ch[i1]], h2 = a.hit_yz[ch[i2]];  // (y, z)
                     // The state carries y and z relative to the first candidate hit.  The model is translation
                     // invariant in y and z, so this is exact; it keeps the fp32 rounding of the two coordinates
                     // (ulp(20 cm), ulp(250 cm)) out of q/pt and sinPhi, whose sensitivity to position noise is
                     // ~50/cm on 10-row tracklets.
-                    yref = h0.y;
-                    zref = h0.z;
-                    if (kf_seed(st, s_rowx[r0], 0.0f, 0.0f, s_rowx[r0 + i1], h1.y - yref, s_rowx[r0 + i2], h2.y - yref,
-                                h2.z - zref, g.cB, g.max_s, g.p0)) {
+                    yref = h0.x;
+                    zref = h0.y;
+                    if (kf_seed(st, s_rowx[r0], 0.0f, 0.0f, s_rowx[r0 + i1], h1.x - yref, s_rowx[r0 + i2], h2.x - yref,
+                                h2.y - zref, g.cB, g.max_s, g.p0)) {
                         mode = kCand;
                         i = 0;
                         r = r0;
@@ -261,15 +257,15 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             if (alive) {
                 uint16_t* rowhit = a.tl_rowhit + (size_t)c * g.RP;
                 float ym = 0.0f, zm = 0.0f;
-                int li = -1;  // local index of the hit to attach
+                int li = -1;  // position of the hit to attach in the sorted row
                 bool have = false;
                 bool stop = false;
                 if (mode == kCand) {
-                    const int hg = a.cand_hits[(size_t)c * kCandMax + i];
-                    const float4 h = __ldg(&a.clusters[hg]);
-                    ym = h.y;
-                    zm = h.z;
-                    li = hg - row_base;
+                    const int hs = a.cand_hits[(size_t)c * kCandMax + i];  // sorted global position
+                    const float2 h = a.hit_yz[hs];
+                    ym = h.x;
+                    zm = h.y;
+                    li = hs - row_base;
                     have = true;
                 } else {
                     const float yp = st.y + yref, zp = st.z + zref;
@@ -284,8 +280,8 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         const int j = pick_up(g, a.hit_yz + row_base, a.hit_idx + row_base,
                                               a.bin_start + (size_t)(slab_base + r) * g.nzp, z0, gy.x, gy.y, yp, zp,
                                               wy, wz, ym, zm, wc);
-                        have = j >= 0;  // (the index load below is not on the path to the update)
-                        if (have) li = a.hit_idx[row_base + j];
+                        have = j >= 0;
+                        li = j;
                     }
                 }
                 if (alive) {
@@ -320,29 +316,6 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     if (stop || r == 0) mode = kDone;
                 }
             }
-            if (mode == kUp || mode == kDown) {
-                // The lane searches row r+dir next and probably the rows after it.  Every search is two dependent loads
-                // (cell table, then hits) from lines no other lane has touched recently, so warm them up now: the
-                // table line three rows ahead and, through the table line two rows ahead (warmed an iteration ago), the
-                // hit line two rows ahead.
-                // Straight-line predictions with the curvature term; being wrong only costs time.
-                const int dir = mode == kUp ? 1 : -1;
-                const int r2 = min(max(r + 2 * dir, 0), g.R - 1), r3 = min(max(r + 3 * dir, 0), g.R - 1);
-                const float ic = rsqrtf((1.0f - st.s) * (1.0f + st.s));
-                const float tgp = st.s * ic, hk = 0.5f * g.cB * st.k * ic * ic * ic, tz = st.t * ic;
-                const float d2 = s_rowx[r2] - s_rowx[r], d3 = s_rowx[r3] - s_rowx[r];
-                const float ya = st.y + yref, za = st.z + zref;
-                const float y2 = ya + d2 * (tgp + hk * d2), z2 = za + d2 * tz;
-                const float y3 = ya + d3 * (tgp + hk * d3), z3 = za + d3 * tz;
-                const float2 g2 = s_rowy[r2], g3 = s_rowy[r3];
-                const uint16_t* t3 = a.bin_start + (size_t)(slab_base + r3) * g.nzp;
-                prefetch_l1(t3 + zbin(z3, z0, g.inv_cz, g.nz) * g.ny + ybin(y3, g3.x, g3.y, g.ny));
-                const uint16_t* t2 = a.bin_start + (size_t)(slab_base + r2) * g.nzp;
-                const int j2 = t2[zbin(z2, z0, g.inv_cz, g.nz) * g.ny + ybin(y2 - 0.5f, g2.x, g2.y, g.ny)];
-                const float2* h2 = a.hit_yz + a.row_offsets[slab_base + r2] + j2;
-                prefetch_l1(h2);
-                prefetch_l1(h2 + 3);
-            }
         }
     }
     // work counters: warp reduction, one atomic per warp and counter
@@ -361,7 +334,7 @@ int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_
     int64_t want = div_up(w.Cmax, kFollowThreads);
     int grid = (int)(want < (int64_t)n_sm * kFollowCtasPerSm ? want : (int64_t)n_sm * kFollowCtasPerSm);
     if (grid < 1) grid = 1;
-    FollowArgs a{p.clusters, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.cand_hits, w.cand_n, w.cand_slab,
+    FollowArgs a{p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.cand_hits, w.cand_n, w.cand_slab,
                  w.counts,   w.Cmax,        w.tl_par, w.tl_cov,  w.tl_chi2,   w.tl_nhits,  w.tl_rows, w.tl_rowhit};
     follow_kernel<<<grid, kFollowThreads, 0, s>>>(g, a);
     return 1;

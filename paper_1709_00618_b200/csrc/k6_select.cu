@@ -114,7 +114,8 @@ write_tracks_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict
                     const uint16_t* __restrict__ tl_rowhit, const uint32_t* __restrict__ claim,
                     const int32_t* __restrict__ tl_kept, const int2* __restrict__ sel_part,
                     const float* __restrict__ tl_par, const float* __restrict__ tl_cov,
-                    const float* __restrict__ tl_chi2, int64_t* __restrict__ counts, int64_t Cmax, const SelectOut o) {
+                    const float* __restrict__ tl_chi2, const uint16_t* __restrict__ hit_idx,
+                    int64_t* __restrict__ counts, int64_t Cmax, const SelectOut o) {
     __shared__ int s_kept[kSelBlock];
     __shared__ int2 s_off[kSelBlock];
     const int64_t n_cand = min(counts[1], Cmax);
@@ -167,8 +168,8 @@ write_tracks_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict
                 if (r <= v.last) {
                     const uint16_t li = v.rowhit[r];
                     if (li != kNoHit) {
-                        const int hh = v.ro[r] + li;
-                        if (claim[hh] == v.w) gh = hh;
+                        const int hh = v.ro[r] + li;  // sorted space; the outputs take the input-order index
+                        if (claim[hh] == v.w) gh = v.ro[r] + (int)hit_idx[hh];
                     }
                 }
                 const unsigned m = __ballot_sync(0xffffffffu, gh >= 0);
@@ -209,7 +210,7 @@ int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const 
         launch_scan_int2(w.sel_part, w.counts + 1, kSelBlock, w.Cmax, 0, w.counts, 3, 4, s);
         write_tracks_kernel<<<grid_b, kSelThreads, 0, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows, w.cand_slab,
                                                            w.slab_part, w.tl_rowhit, w.claim, w.tl_kept, w.sel_part,
-                                                           w.tl_par, w.tl_cov, w.tl_chi2, w.counts, w.Cmax, o);
+                                                           w.tl_par, w.tl_cov, w.tl_chi2, w.hit_idx, w.counts, w.Cmax, o);
         launches += 4;
     }
     finalize_counts_kernel<<<1, 32, 0, s>>>(w.counts, o);
@@ -220,7 +221,8 @@ int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const 
 __global__ void export_tracklets_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
                                         const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_rows,
                                         const int32_t* __restrict__ cand_slab,
-                                        const uint16_t* __restrict__ tl_rowhit, const int64_t* __restrict__ counts,
+                                        const uint16_t* __restrict__ tl_rowhit,
+                                        const uint16_t* __restrict__ hit_idx, const int64_t* __restrict__ counts,
                                         int64_t cap, int32_t* __restrict__ out_hits, int32_t* __restrict__ out_rows) {
     const int64_t n_cand = min(counts[1], cap);
     const int lane = threadIdx.x & 31;
@@ -237,7 +239,7 @@ __global__ void export_tracklets_kernel(const __grid_constant__ DevGeom g, const
                 int gh = -1;
                 if (nh && r >= first && r <= last) {
                     const uint16_t li = tl_rowhit[c * g.RP + r];
-                    if (li != kNoHit) gh = ro[r] + li;
+                    if (li != kNoHit) gh = ro[r] + (int)hit_idx[ro[r] + li];
                 }
                 out_hits[c * g.R + r] = gh;
             }
@@ -252,7 +254,7 @@ int launch_export_tracklets(const DevGeom& g, const Workspace& w, const Problem&
     const int64_t warps = div_up(c, 8);
     const int grid = (int)(warps < 148 * 16 ? warps : 148 * 16);
     export_tracklets_kernel<<<grid, 256, 0, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows, w.cand_slab, w.tl_rowhit,
-                                                 w.counts, c, tl_hits, tl_rows);
+                                                 w.hit_idx, w.counts, c, tl_hits, tl_rows);
     return 1;
 }
 

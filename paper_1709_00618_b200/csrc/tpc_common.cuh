@@ -43,7 +43,9 @@ struct Workspace {
     float2* hit_yz;       // [N]  (y, z) sorted by grid cell inside every (instance,row) segment
     uint16_t* hit_idx;    // [N]  local index (position in the row segment of the INPUT) of the sorted hit
     uint16_t* bin_start;  // [S*R][nzp] first sorted position of every grid cell, entry ncell = row length
-    int32_t* up_raw;      // [N] global indices
+    // Index spaces: everything below that is indexed by hit or holds hit indices uses SORTED global positions
+    // (row start + position in the sorted row); the user-facing outputs are translated back through hit_idx.
+    int32_t* up_raw;      // [N] S2 links
     int32_t* dn_raw;
     int32_t* up;          // cleaned
     int32_t* dn;
@@ -58,7 +60,7 @@ struct Workspace {
     float* tl_chi2;       // [Cmax]
     int32_t* tl_nhits;    // [Cmax]  0 = no tracklet
     int32_t* tl_rows;     // [Cmax]  first | last << 8 | ref << 16
-    uint16_t* tl_rowhit;  // [Cmax][RP] local index of the attached hit per row (valid in first..last), kNoHit = none
+    uint16_t* tl_rowhit;  // [Cmax][RP] position in the sorted row of the attached hit (valid in first..last), kNoHit = none
     int32_t* tl_kept;     // [Cmax]  hits won in the selector, 0 if rejected
     int2* sel_part;       // [Cmax/64 + 2] (tracks, hits) per block of 64 tracklets, then exclusive scan
     int64_t* counts;      // [8] internal copy of the output counts
@@ -105,6 +107,9 @@ struct ChainOut {  // optional user-facing S4 outputs (NULL = skip)
 int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, cudaStream_t s);
 void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m_cap, int64_t m_host, int64_t* counts,
                       int c0, int c1, cudaStream_t s);
+// parity/debug: a link array of the workspace (sorted space) as input-order indices; dir = row offset of the targets
+int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link, int dir,
+                        int32_t* out, cudaStream_t s);
 int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, cudaStream_t s);
 
 struct SelectOut {  // mirrors the S6 part of tpc_output_t

@@ -249,11 +249,10 @@ extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const 
     if (tm) cudaEventRecord(ev[6], s);
     // optional parity/debug copies (device to device, same stream)
     if (n_clusters > 0) {
-        const size_t nb = sizeof(int32_t) * (size_t)n_clusters;
-        if (out->link_up_raw) cudaMemcpyAsync(out->link_up_raw, w.up_raw, nb, cudaMemcpyDeviceToDevice, s);
-        if (out->link_dn_raw) cudaMemcpyAsync(out->link_dn_raw, w.dn_raw, nb, cudaMemcpyDeviceToDevice, s);
-        if (out->link_up) cudaMemcpyAsync(out->link_up, w.up, nb, cudaMemcpyDeviceToDevice, s);
-        if (out->link_dn) cudaMemcpyAsync(out->link_dn, w.dn, nb, cudaMemcpyDeviceToDevice, s);
+        launches += launch_export_links(g, w, p, w.up_raw, +1, out->link_up_raw, s);
+        launches += launch_export_links(g, w, p, w.dn_raw, -1, out->link_dn_raw, s);
+        launches += launch_export_links(g, w, p, w.up, +1, out->link_up, s);
+        launches += launch_export_links(g, w, p, w.dn, -1, out->link_dn, s);
         const int64_t tc = out->tl_capacity < w.Cmax ? out->tl_capacity : w.Cmax;
         if (tc > 0) {
             if (out->tl_params) cudaMemcpyAsync(out->tl_params, w.tl_par, sizeof(float) * 5 * tc, cudaMemcpyDeviceToDevice, s);
