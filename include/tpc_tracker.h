@@ -112,7 +112,8 @@ typedef struct {
     /* device [TPC_N_COUNTS]: 0 n_start, 1 n_cand, 2 n_tracklets, 3 n_tracks, 4 n_track_hits,
        5 input error flags (bit0: a row holds > 65535 clusters; bit1: > 2^23 candidates in one instance),
        6 S5 transport steps executed, 7 S5 measurement updates, 8 clusters examined by the S5 pick-up search,
-       9 S5 pick-up searches (work counters for the roofline arithmetic), 10-15 reserved.
+       9 S5 pick-up searches (work counters for the roofline arithmetic; 6-9 stay 0 unless
+       tpc_set_work_counters enabled them), 10-15 reserved.
        Written by the last kernel of the call. */
     int64_t* counts;
 } tpc_output_t;
@@ -144,6 +145,10 @@ int tpc_check_counts(const int64_t* counts_host, const tpc_output_t* out);
 
 /* Number of kernel launches the last tpc_track_sectors call enqueued (for bench.py's gpu_launches). */
 int32_t tpc_last_launch_count(const tpc_tracker_t* t);
+
+/* Work counters of S5 (counts[6..9]): off by default.  When enabled, the follower runs a variant that also counts its
+   transport steps, updates, searches and examined clusters; the results are unchanged, the call is a little slower. */
+int tpc_set_work_counters(tpc_tracker_t* t, int32_t enable);
 
 /* Optional per-stage timing: when enabled, every tpc_track_sectors call records CUDA events on its stream around
    each stage (a ring of the last TPC_TIMING_RING calls).  tpc_stage_times_ms waits for the call `age` calls back

@@ -16,6 +16,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libtpctrk.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+# extra nvcc flags for every translation unit, e.g. TPC_NVCC_FLAGS="-DTPC_FOLLOW_CTAS=8" (kernel tuning switches)
+EXTRA = os.environ.get("TPC_NVCC_FLAGS", "").split()
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-Wall", "-Xptxas", "-v"]
@@ -45,7 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     log = []
     for src, extra in SOURCES.items():
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
-        cmd = [NVCC, *ARCH, *COMMON, *extra, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [NVCC, *ARCH, *COMMON, *extra, *EXTRA, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         log.append("$ " + " ".join(cmd) + "\n" + r.stdout + r.stderr)
         if r.returncode != 0:

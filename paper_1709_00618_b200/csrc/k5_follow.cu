@@ -9,20 +9,30 @@
 // track length.  A lane whose candidate has ended parks until a few lanes are parked, then those lanes write
 // their tracklets and take new candidates from the warp's chunk of the device-wide queue (consecutive candidate
 // ids start in neighbouring rows of one sector instance, which keeps the warp's loads in the same L1 lines).
+//
+// Latency: a row step is a dependent chain  transport -> cell table -> hits -> update.  The two memory round trips
+// are taken off that chain by looking ahead: the row a lane visits next is known when the current step ends, and
+// its position there is known to a few mm by linear extrapolation, so the step ends by (1) loading the next row's
+// offset, (2) prefetching the cell-table sector of the row after next, and (3) reading the next row's table entry
+// (prefetched one step earlier) to prefetch the sector of its first candidate hit.  The prefetches are hints only:
+// the search itself recomputes everything from the transported state.
 #include "kf_math.cuh"
+
+#ifndef TPC_FOLLOW_CTAS
+#define TPC_FOLLOW_CTAS 6
+#endif
+#ifndef TPC_FOLLOW_LA
+#define TPC_FOLLOW_LA 0  // look-ahead depth: 0 none, 1 next row's table sector, 2 table two rows ahead + next row's hits
+#endif
 
 namespace tpc {
 
 constexpr int kFollowThreads = 128;
-constexpr int kFollowCtasPerSm = 8;
+constexpr int kFollowCtasPerSm = TPC_FOLLOW_CTAS;
 constexpr int kFollowChunk = 64;   // candidates a warp takes from the queue at a time
 constexpr int kFollowReload = 4;   // parked lanes that trigger a write-out / refill phase
 
 enum FollowMode : int { kCand = 0, kUp = 1, kBack = 2, kDown = 3, kDone = 4, kIdle = 5 };
-
-struct WorkCount {  // per-thread work counters (roofline arithmetic): summed into counts[6..9] at kernel end
-    unsigned transports, updates, examined, searches;
-};
 
 struct FollowArgs {
     const int32_t* row_offsets;
@@ -42,103 +52,71 @@ struct FollowArgs {
     uint16_t* tl_rowhit;
 };
 
-// One hit of the pick-up search: inside the gate and nearer than the best so far?  Ties -> lowest local index.
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// The best hit of the pick-up search so far.
 struct PickBest {
     int j;       // sorted position of the best hit, -1 = none
-    int idx;     // its local index, -1 = not loaded yet
     float d2, y, z;
 };
 
+// One hit of the pick-up search: inside the gate and nearer than the best so far?  Ties -> lowest local index.
+// The decision arithmetic is individually rounded fp32 (both sides decide in fp32).
 __device__ __forceinline__ void pick_consider(PickBest& b, const uint16_t* __restrict__ idx, int j, bool valid,
                                               float2 h, float yp, float zp, float wy, float wz) {
     const float dy = __fsub_rn(h.x, yp), dz = __fsub_rn(h.y, zp);
     const float d2 = __fadd_rn(__fmul_rn(dy, dy), __fmul_rn(dz, dz));
     const bool in = valid && fabsf(dy) <= wy && fabsf(dz) <= wz;
     bool better = in && d2 < b.d2;
-    int id = -1;
-    if (in && d2 == b.d2) {  // exact tie: lowest local index wins (rare)
-        id = idx[j];
-        if (b.idx < 0) b.idx = idx[b.j];
-        better = id < b.idx;
-    }
+    if (in && d2 == b.d2 && j != b.j) better = idx[j] < idx[b.j];  // exact tie (rare): lowest local index wins
     if (better) {
         b.j = j;
-        b.idx = id;
         b.d2 = d2;
         b.y = h.x;
         b.z = h.y;
     }
 }
 
-// Nearest cluster of the row inside the gate around the predicted (y,z); ties -> lowest local index.
-// Returns the sorted position (relative to the row start) or -1; (ym, zm) get its coordinates.
-// The grid cells visited are a superset of the rounded fp32 gate test (margin m, monotone bin functions).
-__device__ __forceinline__ int pick_up(const DevGeom& g, const float2* __restrict__ yz,
-                                       const uint16_t* __restrict__ idx, const uint16_t* __restrict__ tbl, float z0,
-                                       float y0, float inv_sy, float yp, float zp, float wy, float wz, float& ym,
-                                       float& zm, WorkCount& wc) {
-    const float m = 1e-3f;
-    const int zb0 = zbin(zp - wz - m, z0, g.inv_cz, g.nz), zb1 = zbin(zp + wz + m, z0, g.inv_cz, g.nz);
-    const int ys0 = ybin(yp - wy - m, y0, inv_sy, g.ny), ys1 = ybin(yp + wy + m, y0, inv_sy, g.ny) + 1;
-    // first and last z bin: the four table entries are independent loads
-    const uint16_t* ta = tbl + zb0 * g.ny;
-    const uint16_t* tb = tbl + zb1 * g.ny;
-    const int ja0 = ta[ys0], ja1 = ta[ys1];
-    int jb0 = 0, jb1 = 0;
-    if (zb1 > zb0) {
-        jb0 = tb[ys0];
-        jb1 = tb[ys1];
-    }
-    const int na = ja1 - ja0, nt = na + (jb1 - jb0);
-    wc.searches++;
-    wc.examined += nt;
-    PickBest b{-1, -1, __int_as_float(0x7f800000), 0.0f, 0.0f};
-    // the two ranges as one sequence, four hits per trip (independent loads: one memory round trip per trip)
-    for (int k = 0; k < nt; k += 4) {
-        int j[4];
-        float2 h[4];
-#pragma unroll
-        for (int q = 0; q < 4; q++) {
-            const int kk = min(k + q, nt - 1);
-            j[q] = kk < na ? ja0 + kk : jb0 + (kk - na);
-            h[q] = yz[j[q]];
-        }
-#pragma unroll
-        for (int q = 0; q < 4; q++) pick_consider(b, idx, j[q], k + q < nt, h[q], yp, zp, wy, wz);
-    }
-    // z bins in between exist only when the cells are narrower than the gate (non-default grid_cell_z)
-    for (int zb = zb0 + 1; zb < zb1; zb++) {
-        const int j0 = tbl[zb * g.ny + ys0], j1 = tbl[zb * g.ny + ys1];
-        wc.examined += j1 - j0;
-        for (int j = j0; j < j1; j++) pick_consider(b, idx, j, true, yz[j], yp, zp, wy, wz);
-    }
-    ym = b.y;
-    zm = b.z;
-    return b.j;
+__device__ __forceinline__ void store_report(float4 (*s_rep)[kFollowThreads], const KfState& st) {
+    s_rep[0][threadIdx.x] = make_float4(st.y, st.z, st.s, st.t);
+    s_rep[1][threadIdx.x] = make_float4(st.k, st.c00, st.c10, st.c11);
+    s_rep[2][threadIdx.x] = make_float4(st.c20, st.c21, st.c22, st.c30);
+    s_rep[3][threadIdx.x] = make_float4(st.c31, st.c32, st.c33, st.c40);
+    s_rep[4][threadIdx.x] = make_float4(st.c41, st.c42, st.c43, st.c44);
 }
 
+__device__ __forceinline__ void zero_report(float4 (*s_rep)[kFollowThreads]) {
+#pragma unroll
+    for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+}
+
+// kCount: also accumulate the work counters counts[6..9] (roofline arithmetic; tpc_set_work_counters).  They are a
+// property of the input, so the timed runs use the variant without them.
+template <bool kCount>
 __global__ void __launch_bounds__(kFollowThreads, kFollowCtasPerSm)
 follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowArgs a) {
     __shared__ float s_rowx[kMaxRows + 1];
     __shared__ float2 s_rowy[kMaxRows + 1];      // (y0, strips per cm) of the row's grid
     __shared__ float4 s_rep[5][kFollowThreads];  // reported state of the lane's tracklet (see kDown below)
-    for (int i = threadIdx.x; i < g.R; i += kFollowThreads) {
-        s_rowx[i] = g.row_x[i];
-        s_rowy[i] = make_float2(g.row_y0[i], g.row_inv_sy[i]);
+    for (int q = threadIdx.x; q < g.R; q += kFollowThreads) {
+        s_rowx[q] = g.row_x[q];
+        s_rowy[q] = make_float2(g.row_y0[q], g.row_inv_sy[q]);
     }
     __syncthreads();
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    const unsigned below = (1u << lane) - 1u;
     const int n_cand = (int)min(a.counts[1], a.Cmax);
     unsigned long long* queue = reinterpret_cast<unsigned long long*>(&a.counts[10]);
     int wn = 0, we = 0;  // the warp's chunk [wn, we) of candidate ids (warp-uniform)
     bool exhausted = false;
-    WorkCount wc = {0u, 0u, 0u, 0u};
+    unsigned n_tr = 0, n_up = 0, n_ex = 0, n_se = 0;  // work counters (kCount only)
 
     // lane state
     int mode = kIdle;
-    int c = 0, r = 0, r0 = 0, n = 0, i = 0, slab_base = 0;
+    int c = 0, slab_base = 0;
+    int r = 0, rn = 0, rb = 0;      // row of the state, row of the coming step and its offset in the hit arrays
+    int r0 = 0, n = 0, i = 0;       // start row, candidate length, next own hit
+    int hsn = 0;                    // sorted global position of the candidate's next own hit
     int nhits = 0, gap = 0, first_row = 0, last_row = 0;
     float yref = 0.0f, zref = 0.0f, z0 = 0.0f, chi2 = 0.0f;
     KfState st = {};
@@ -175,7 +153,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     }
                 }
                 const unsigned idle = __ballot_sync(full, mode == kIdle);
-                const int mine = wn + __popc(idle & below);
+                const int mine = wn + __popc(idle & ((1u << lane) - 1u));
                 if (mode == kIdle && mine < we) {
                     c = mine;
                     const int slab0 = a.cand_slab[c];
@@ -187,7 +165,9 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     const int32_t* ch = a.cand_hits + (size_t)c * kCandMax;
                     // seed from hits 0, n/2, n-1
                     const int i1 = n >> 1, i2 = n - 1;
-                    const float2 h0 = a.hit_yz[ch[0]], h1 = a.hit_yz[ch[i1]], h2 = a.hit_yz[ch[i2]];  // (y, z)
+                    hsn = ch[0];
+                    const float2 h0 = a.hit_yz[hsn], h1 = a.hit_yz[ch[i1]], h2 = a.hit_yz[ch[i2]];  // (y, z)
+                    rb = a.row_offsets[slab_base + r0];
                     // The state carries y and z relative to the first candidate hit.  The model is translation
                     // invariant in y and z, so this is exact; it keeps the fp32 rounding of the two coordinates
                     // (ulp(20 cm), ulp(250 cm)) out of q/pt and sinPhi, whose sensitivity to position noise is
@@ -198,7 +178,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                                 h2.y - zref, g.cB, g.max_s, g.p0)) {
                         mode = kCand;
                         i = 0;
-                        r = r0;
+                        r = rn = r0;
                         chi2 = 0.0f;
                         nhits = 0;
                         gap = 0;
@@ -208,8 +188,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         nhits = 0;
                         chi2 = yref = zref = 0.0f;
                         first_row = last_row = 0;
-#pragma unroll
-                        for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        zero_report(s_rep);
                         mode = kDone;
                     }
                 }
@@ -219,13 +198,20 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             if (act == 0u && exhausted) break;
         }
         if (mode < kDone) {
-            // ---- one pad row ----
-            const int rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : (mode == kCand ? r0 + i : r + 1));
-            const int32_t row_base = a.row_offsets[slab_base + rn];
+            // ---- one pad row: transport to row rn (offset rb), attach a hit, decide where to go next ----
             bool alive = true;
+            bool la = false;             // look-ahead possible: this step moved by one row in the running direction
+            float dyp = 0.0f, dzp = 0.0f;  // displacement of that move
+            float wy = 1.0f, wz = 1.0f;    // gate of this step's search (look-ahead guess otherwise)
+            float2 hc = make_float2(0.0f, 0.0f);
+            if (mode == kCand) hc = a.hit_yz[hsn];  // issued before the transport arithmetic
             if (rn != r) {
+                const float yb = st.y, zb = st.z;
                 if (kf_transport(st, s_rowx[rn] - s_rowx[r], g.cB, g.max_s)) {
-                    wc.transports++;
+                    if (kCount) n_tr++;
+                    dyp = st.y - yb;
+                    dzp = st.z - zb;
+                    la = mode != kBack;
                     r = rn;
                 } else {
                     alive = false;
@@ -237,8 +223,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         nhits = 0;
                         chi2 = yref = zref = 0.0f;
                         first_row = last_row = 0;
-#pragma unroll
-                        for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        zero_report(s_rep);
                         mode = kDone;
                     }
                 }
@@ -247,57 +232,78 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 // phase B starts: the reported state is the back-transported one until a hit is attached
                 mode = r0 > 0 ? kDown : kDone;
                 gap = 0;
-                s_rep[0][threadIdx.x] = make_float4(st.y, st.z, st.s, st.t);
-                s_rep[1][threadIdx.x] = make_float4(st.k, st.c00, st.c10, st.c11);
-                s_rep[2][threadIdx.x] = make_float4(st.c20, st.c21, st.c22, st.c30);
-                s_rep[3][threadIdx.x] = make_float4(st.c31, st.c32, st.c33, st.c40);
-                s_rep[4][threadIdx.x] = make_float4(st.c41, st.c42, st.c43, st.c44);
+                store_report(s_rep, st);
                 alive = false;
             }
             if (alive) {
-                uint16_t* rowhit = a.tl_rowhit + (size_t)c * g.RP;
-                float ym = 0.0f, zm = 0.0f;
-                int li = -1;  // position of the hit to attach in the sorted row
-                bool have = false;
+                float ym = hc.x, zm = hc.y;
+                int li = hsn - rb;  // position of the hit to attach in the sorted row
+                bool have = true;
                 bool stop = false;
-                if (mode == kCand) {
-                    const int hs = a.cand_hits[(size_t)c * kCandMax + i];  // sorted global position
-                    const float2 h = a.hit_yz[hs];
-                    ym = h.x;
-                    zm = h.y;
-                    li = hs - row_base;
-                    have = true;
-                } else {
+                if (mode != kCand) {
                     const float yp = st.y + yref, zp = st.z + zref;
                     if (fabsf(yp) > fmaf(s_rowx[r], g.tan_half, g.edge_margin)) {
                         stop = true;
                         alive = false;
                     } else {
-                        const float vy = st.c00 + g.sy2, vz = st.c11 + g.sz2;  // > 0: sigma > 0 (tpc_tracker_create)
-                        const float wy = fminf(g.wmax, g.gate * (vy * rsqrtf(vy)));
-                        const float wz = fminf(g.wmax, g.gate * (vz * rsqrtf(vz)));
+                        // gate: 4 sigma of the predicted residual, capped (sigma > 0: tpc_tracker_create)
+                        wy = fminf(g.wmax, g.gate * sqrtf(st.c00 + g.sy2));
+                        wz = fminf(g.wmax, g.gate * sqrtf(st.c11 + g.sz2));
+                        // The cells visited are a superset of the rounded fp32 gate test (margin m, monotone bins).
+                        const float m = 1e-3f;
                         const float2 gy = s_rowy[r];
-                        const int j = pick_up(g, a.hit_yz + row_base, a.hit_idx + row_base,
-                                              a.bin_start + (size_t)(slab_base + r) * g.nzp, z0, gy.x, gy.y, yp, zp,
-                                              wy, wz, ym, zm, wc);
-                        have = j >= 0;
-                        li = j;
+                        const int zb0 = zbin(zp - wz - m, z0, g.inv_cz, g.nz), zb1 = zbin(zp + wz + m, z0, g.inv_cz, g.nz);
+                        const int ys0 = ybin(yp - wy - m, gy.x, gy.y, g.ny), ys1 = ybin(yp + wy + m, gy.x, gy.y, g.ny) + 1;
+                        const uint16_t* tbl = a.bin_start + (size_t)(slab_base + r) * g.nzp;
+                        const float2* yz = a.hit_yz + rb;
+                        const uint16_t* idx = a.hit_idx + rb;
+                        // first and last z bin: the four table entries are independent loads
+                        const uint16_t* ta = tbl + zb0 * g.ny;
+                        const uint16_t* tb = tbl + zb1 * g.ny;
+                        const int ja0 = ta[ys0], ja1 = ta[ys1];
+                        int jb0 = 0, jb1 = 0;
+                        if (zb1 > zb0) {
+                            jb0 = tb[ys0];
+                            jb1 = tb[ys1];
+                        }
+                        const int na = ja1 - ja0, nt = na + (jb1 - jb0);
+                        if (kCount) {
+                            n_se++;
+                            n_ex += nt;
+                        }
+                        PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f};
+                        // the two ranges as one sequence, two hits per trip (independent loads)
+                        for (int k = 0; k < nt; k += 2) {
+                            const int k1 = min(k + 1, nt - 1);
+                            const int j0 = k < na ? ja0 + k : jb0 + (k - na);
+                            const int j1 = k1 < na ? ja0 + k1 : jb0 + (k1 - na);
+                            const float2 h0 = yz[j0], h1 = yz[j1];
+                            pick_consider(b, idx, j0, true, h0, yp, zp, wy, wz);
+                            pick_consider(b, idx, j1, k + 1 < nt, h1, yp, zp, wy, wz);
+                        }
+                        // z bins in between exist only when the cells are narrower than the gate (non-default grid_cell_z)
+                        for (int zb = zb0 + 1; zb < zb1; zb++) {
+                            const int j0 = tbl[zb * g.ny + ys0], j1 = tbl[zb * g.ny + ys1];
+                            if (kCount) n_ex += j1 - j0;
+                            for (int j = j0; j < j1; j++) pick_consider(b, idx, j, true, yz[j], yp, zp, wy, wz);
+                        }
+                        ym = b.y;
+                        zm = b.z;
+                        li = b.j;
+                        have = b.j >= 0;
                     }
                 }
                 if (alive) {
+                    uint16_t* rowhit = a.tl_rowhit + (size_t)c * g.RP;
                     if (have) {
                         __stcs(&rowhit[r], (uint16_t)li);
                         chi2 += kf_update(st, ym - yref, zm - zref, g.sy2, g.sz2);
-                        wc.updates++;
+                        if (kCount) n_up++;
                         nhits++;
                         gap = 0;
                         if (mode == kDown) {
                             first_row = r;
-                            s_rep[0][threadIdx.x] = make_float4(st.y, st.z, st.s, st.t);
-                            s_rep[1][threadIdx.x] = make_float4(st.k, st.c00, st.c10, st.c11);
-                            s_rep[2][threadIdx.x] = make_float4(st.c20, st.c21, st.c22, st.c30);
-                            s_rep[3][threadIdx.x] = make_float4(st.c31, st.c32, st.c33, st.c40);
-                            s_rep[4][threadIdx.x] = make_float4(st.c41, st.c42, st.c43, st.c44);
+                            store_report(s_rep, st);
                         } else {
                             last_row = r;
                         }
@@ -316,19 +322,45 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     if (stop || r == 0) mode = kDone;
                 }
             }
+            // ---- set up the next step: its row, the row's offset, the candidate's next own hit; look ahead ----
+            if (mode < kDone) {
+                rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : (mode == kCand ? r0 + i : r + 1));
+                rb = a.row_offsets[slab_base + rn];
+                if (mode == kCand) {
+                    hsn = a.cand_hits[(size_t)c * kCandMax + i];
+                } else if (TPC_FOLLOW_LA > 0 && la && mode != kBack) {
+                    // the coming steps search rows rn, rn + dir near the linear extrapolation of this step's move
+                    const float ye = st.y + yref + dyp - wy, ze = st.z + zref + dzp - wz;
+                    const float2 gy1 = s_rowy[rn];
+                    const int cell1 = zbin(ze, z0, g.inv_cz, g.nz) * g.ny + ybin(ye, gy1.x, gy1.y, g.ny);
+                    const uint16_t* t1 = a.bin_start + (size_t)(slab_base + rn) * g.nzp + cell1;
+                    if (TPC_FOLLOW_LA == 1) {
+                        prefetch_l1(t1);
+                    } else {
+                        const int r2 = 2 * rn - r;
+                        if (r2 >= 0 && r2 < g.R) {
+                            const float2 gy2 = s_rowy[r2];
+                            const int cell2 = zbin(ze + dzp, z0, g.inv_cz, g.nz) * g.ny + ybin(ye + dyp, gy2.x, gy2.y, g.ny);
+                            prefetch_l1(a.bin_start + (size_t)(slab_base + r2) * g.nzp + cell2);
+                        }
+                        prefetch_l1(a.hit_yz + rb + *t1);
+                    }
+                }
+            }
         }
     }
-    // work counters: warp reduction, one atomic per warp and counter
-    unsigned v[4] = {wc.transports, wc.updates, wc.examined, wc.searches};
+    if (kCount) {  // work counters: warp reduction, one atomic per warp and counter
+        unsigned v[4] = {n_tr, n_up, n_ex, n_se};
 #pragma unroll
-    for (int q = 0; q < 4; q++) {
+        for (int q = 0; q < 4; q++) {
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1) v[q] += __shfl_xor_sync(full, v[q], d);
-        if (lane == 0 && v[q]) atomicAdd((unsigned long long*)&a.counts[6 + q], (unsigned long long)v[q]);
+            for (int d = 16; d > 0; d >>= 1) v[q] += __shfl_xor_sync(full, v[q], d);
+            if (lane == 0 && v[q]) atomicAdd((unsigned long long*)&a.counts[6 + q], (unsigned long long)v[q]);
+        }
     }
 }
 
-int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, cudaStream_t s) {
+int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, bool count_work, cudaStream_t s) {
     if (p.n_clusters == 0) return 0;
     // persistent grid: every SM holds kFollowCtasPerSm CTAs, capped by the candidate bound
     int64_t want = div_up(w.Cmax, kFollowThreads);
@@ -336,7 +368,10 @@ int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_
     if (grid < 1) grid = 1;
     FollowArgs a{p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.cand_hits, w.cand_n, w.cand_slab,
                  w.counts,   w.Cmax,        w.tl_par, w.tl_cov,  w.tl_chi2,   w.tl_nhits,  w.tl_rows, w.tl_rowhit};
-    follow_kernel<<<grid, kFollowThreads, 0, s>>>(g, a);
+    if (count_work)
+        follow_kernel<true><<<grid, kFollowThreads, 0, s>>>(g, a);
+    else
+        follow_kernel<false><<<grid, kFollowThreads, 0, s>>>(g, a);
     return 1;
 }
 

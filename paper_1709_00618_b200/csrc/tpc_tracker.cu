@@ -186,6 +186,12 @@ extern "C" int tpc_set_stream(tpc_tracker_t* t, void* s) {
     return TPC_OK;
 }
 
+extern "C" int tpc_set_work_counters(tpc_tracker_t* t, int32_t enable) {
+    if (!t) return TPC_ERR_ARG;
+    t->count_work = enable != 0;
+    return TPC_OK;
+}
+
 extern "C" int tpc_set_stage_timing(tpc_tracker_t* t, int32_t enable) {
     if (!t) return TPC_ERR_ARG;
     if (enable && !t->ev_valid) {
@@ -240,7 +246,7 @@ extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const 
                 (out->cand_hits || out->cand_n) ? out->cand_capacity : 0};
     launches += launch_chains(g, w, p, co, s);
     if (tm) cudaEventRecord(ev[4], s);
-    launches += launch_follow(g, w, p, t->n_sm, s);
+    launches += launch_follow(g, w, p, t->n_sm, t->count_work, s);
     if (tm) cudaEventRecord(ev[5], s);
     SelectOut so{out->trk_params, out->trk_cov, out->trk_chi2, out->trk_xref, out->trk_cand_id, out->trk_nhits,
                  out->trk_sector, out->trk_hit_offset, out->trk_hits, out->trk_capacity, out->trk_hits_capacity,

@@ -14,6 +14,7 @@ struct tpc_tracker {
     int n_sm = 148;
     int last_launches = 0;
     bool timing = false;
+    bool count_work = false;  // S5 work counters counts[6..9] (tpc_set_work_counters)
     cudaEvent_t ev[TPC_TIMING_RING][TPC_N_STAGES + 1] = {};
     bool ev_valid = false;
     int64_t n_calls = 0;  // timed calls so far (ring position = n_calls % TPC_TIMING_RING)
