@@ -9,28 +9,20 @@
 // track length.  A lane whose candidate has ended parks until a few lanes are parked, then those lanes write
 // their tracklets and take new candidates from the warp's chunk of the device-wide queue (consecutive candidate
 // ids start in neighbouring rows of one sector instance, which keeps the warp's loads in the same L1 lines).
-//
-// Latency: a row step is a dependent chain  transport -> cell table -> hits -> update.  The two memory round trips
-// are taken off that chain by looking ahead: the row a lane visits next is known when the current step ends, and
-// its position there is known to a few mm by linear extrapolation, so the step ends by (1) loading the next row's
-// offset, (2) prefetching the cell-table sector of the row after next, and (3) reading the next row's table entry
-// (prefetched one step earlier) to prefetch the sector of its first candidate hit.  The prefetches are hints only:
-// the search itself recomputes everything from the transported state.
 #include "kf_math.cuh"
 
 #ifndef TPC_FOLLOW_CTAS
 #define TPC_FOLLOW_CTAS 6
 #endif
-#ifndef TPC_FOLLOW_LA
-#define TPC_FOLLOW_LA 0  // look-ahead depth: 0 none, 1 next row's table sector, 2 table two rows ahead + next row's hits
-#endif
-
 namespace tpc {
 
 constexpr int kFollowThreads = 128;
 constexpr int kFollowCtasPerSm = TPC_FOLLOW_CTAS;
 constexpr int kFollowChunk = 64;   // candidates a warp takes from the queue at a time
-constexpr int kFollowReload = 4;   // parked lanes that trigger a write-out / refill phase
+#ifndef TPC_FOLLOW_RELOAD
+#define TPC_FOLLOW_RELOAD 4
+#endif
+constexpr int kFollowReload = TPC_FOLLOW_RELOAD;  // parked lanes that trigger a write-out / refill phase
 
 enum FollowMode : int { kCand = 0, kUp = 1, kBack = 2, kDown = 3, kDone = 4, kIdle = 5 };
 
@@ -52,29 +44,38 @@ struct FollowArgs {
     uint16_t* tl_rowhit;
 };
 
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-
 // The best hit of the pick-up search so far.
 struct PickBest {
     int j;       // sorted position of the best hit, -1 = none
     float d2, y, z;
 };
 
+// Exact tie between two hits of the search (only duplicated clusters produce one): the lowest local index wins.
+__device__ __noinline__ bool tie_lower_index(const uint16_t* __restrict__ idx, unsigned ja, unsigned jb) {
+    return idx[ja] < idx[jb];
+}
+
 // One hit of the pick-up search: inside the gate and nearer than the best so far?  Ties -> lowest local index.
 // The decision arithmetic is individually rounded fp32 (both sides decide in fp32).
-__device__ __forceinline__ void pick_consider(PickBest& b, const uint16_t* __restrict__ idx, int j, bool valid,
-                                              float2 h, float yp, float zp, float wy, float wz) {
+__device__ __forceinline__ void pick_consider(PickBest& b, const uint16_t* __restrict__ idx, unsigned rb, int j,
+                                              bool valid, float2 h, float yp, float zp, float wy, float wz) {
     const float dy = __fsub_rn(h.x, yp), dz = __fsub_rn(h.y, zp);
     const float d2 = __fadd_rn(__fmul_rn(dy, dy), __fmul_rn(dz, dz));
     const bool in = valid && fabsf(dy) <= wy && fabsf(dz) <= wz;
     bool better = in && d2 < b.d2;
-    if (in && d2 == b.d2 && j != b.j) better = idx[j] < idx[b.j];  // exact tie (rare): lowest local index wins
+    if (in && d2 == b.d2 && j != b.j) better = tie_lower_index(idx, rb + (unsigned)j, rb + (unsigned)b.j);
     if (better) {
         b.j = j;
         b.d2 = d2;
         b.y = h.x;
         b.z = h.y;
     }
+}
+
+__device__ __forceinline__ float sqrt_fast(float x) {  // x > 0, normal range
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
 }
 
 __device__ __forceinline__ void store_report(float4 (*s_rep)[kFollowThreads], const KfState& st) {
@@ -200,18 +201,11 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
         if (mode < kDone) {
             // ---- one pad row: transport to row rn (offset rb), attach a hit, decide where to go next ----
             bool alive = true;
-            bool la = false;             // look-ahead possible: this step moved by one row in the running direction
-            float dyp = 0.0f, dzp = 0.0f;  // displacement of that move
-            float wy = 1.0f, wz = 1.0f;    // gate of this step's search (look-ahead guess otherwise)
             float2 hc = make_float2(0.0f, 0.0f);
             if (mode == kCand) hc = a.hit_yz[hsn];  // issued before the transport arithmetic
             if (rn != r) {
-                const float yb = st.y, zb = st.z;
                 if (kf_transport(st, s_rowx[rn] - s_rowx[r], g.cB, g.max_s)) {
                     if (kCount) n_tr++;
-                    dyp = st.y - yb;
-                    dzp = st.z - zb;
-                    la = mode != kBack;
                     r = rn;
                 } else {
                     alive = false;
@@ -238,7 +232,6 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             if (alive) {
                 float ym = hc.x, zm = hc.y;
                 int li = hsn - rb;  // position of the hit to attach in the sorted row
-                bool have = true;
                 bool stop = false;
                 if (mode != kCand) {
                     const float yp = st.y + yref, zp = st.z + zref;
@@ -247,56 +240,59 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         alive = false;
                     } else {
                         // gate: 4 sigma of the predicted residual, capped (sigma > 0: tpc_tracker_create)
-                        wy = fminf(g.wmax, g.gate * sqrtf(st.c00 + g.sy2));
-                        wz = fminf(g.wmax, g.gate * sqrtf(st.c11 + g.sz2));
+                        const float wy = fminf(g.wmax, g.gate * sqrt_fast(st.c00 + g.sy2));
+                        const float wz = fminf(g.wmax, g.gate * sqrt_fast(st.c11 + g.sz2));
                         // The cells visited are a superset of the rounded fp32 gate test (margin m, monotone bins).
                         const float m = 1e-3f;
                         const float2 gy = s_rowy[r];
                         const int zb0 = zbin(zp - wz - m, z0, g.inv_cz, g.nz), zb1 = zbin(zp + wz + m, z0, g.inv_cz, g.nz);
                         const int ys0 = ybin(yp - wy - m, gy.x, gy.y, g.ny), ys1 = ybin(yp + wy + m, gy.x, gy.y, g.ny) + 1;
-                        const uint16_t* tbl = a.bin_start + (size_t)(slab_base + r) * g.nzp;
-                        const float2* yz = a.hit_yz + rb;
-                        const uint16_t* idx = a.hit_idx + rb;
-                        // first and last z bin: the four table entries are independent loads
-                        const uint16_t* ta = tbl + zb0 * g.ny;
-                        const uint16_t* tb = tbl + zb1 * g.ny;
-                        const int ja0 = ta[ys0], ja1 = ta[ys1];
+                        // one index per table entry (32-bit arithmetic, one wide multiply-add per address)
+                        const unsigned tb0 = (unsigned)(slab_base + r) * (unsigned)g.nzp;
+                        const unsigned ia = tb0 + (unsigned)(zb0 * g.ny), ib = tb0 + (unsigned)(zb1 * g.ny);
+                        const int ja0 = a.bin_start[ia + ys0], ja1 = a.bin_start[ia + ys1];
                         int jb0 = 0, jb1 = 0;
                         if (zb1 > zb0) {
-                            jb0 = tb[ys0];
-                            jb1 = tb[ys1];
+                            jb0 = a.bin_start[ib + ys0];
+                            jb1 = a.bin_start[ib + ys1];
                         }
                         const int na = ja1 - ja0, nt = na + (jb1 - jb0);
                         if (kCount) {
                             n_se++;
                             n_ex += nt;
                         }
+                        // The two ranges form one sequence k = 0..nt-1.  Its first two hits are examined in line
+                        // (most searches see one or two); the loop below takes the rest one by one.
+                        const int d = jb0 - na;  // position of sequence element k >= na is k + d
+                        const int j0 = na > 0 ? ja0 : jb0;
+                        const int j1 = na > 1 ? ja0 + 1 : 1 + d;
+                        const unsigned urb = (unsigned)rb;
+                        const float2 h0 = a.hit_yz[urb + (unsigned)(nt > 0 ? j0 : 0)];
+                        const float2 h1 = a.hit_yz[urb + (unsigned)(nt > 1 ? j1 : 0)];
                         PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f};
-                        // the two ranges as one sequence, two hits per trip (independent loads)
-                        for (int k = 0; k < nt; k += 2) {
-                            const int k1 = min(k + 1, nt - 1);
-                            const int j0 = k < na ? ja0 + k : jb0 + (k - na);
-                            const int j1 = k1 < na ? ja0 + k1 : jb0 + (k1 - na);
-                            const float2 h0 = yz[j0], h1 = yz[j1];
-                            pick_consider(b, idx, j0, true, h0, yp, zp, wy, wz);
-                            pick_consider(b, idx, j1, k + 1 < nt, h1, yp, zp, wy, wz);
+                        pick_consider(b, a.hit_idx, urb, j0, nt > 0, h0, yp, zp, wy, wz);
+                        pick_consider(b, a.hit_idx, urb, j1, nt > 1, h1, yp, zp, wy, wz);
+                        for (int k = 2; k < nt; k++) {
+                            const int j = k < na ? ja0 + k : k + d;
+                            pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
                         }
                         // z bins in between exist only when the cells are narrower than the gate (non-default grid_cell_z)
                         for (int zb = zb0 + 1; zb < zb1; zb++) {
-                            const int j0 = tbl[zb * g.ny + ys0], j1 = tbl[zb * g.ny + ys1];
-                            if (kCount) n_ex += j1 - j0;
-                            for (int j = j0; j < j1; j++) pick_consider(b, idx, j, true, yz[j], yp, zp, wy, wz);
+                            const unsigned im = tb0 + (unsigned)(zb * g.ny);
+                            const int jm0 = a.bin_start[im + ys0], jm1 = a.bin_start[im + ys1];
+                            if (kCount) n_ex += jm1 - jm0;
+                            for (int j = jm0; j < jm1; j++)
+                                pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
                         }
                         ym = b.y;
                         zm = b.z;
                         li = b.j;
-                        have = b.j >= 0;
                     }
                 }
                 if (alive) {
-                    uint16_t* rowhit = a.tl_rowhit + (size_t)c * g.RP;
-                    if (have) {
-                        __stcs(&rowhit[r], (uint16_t)li);
+                    const unsigned ih = (unsigned)c * (unsigned)g.RP + (unsigned)r;
+                    __stcs(&a.tl_rowhit[ih], (uint16_t)li);  // li = -1 stores kNoHit
+                    if (li >= 0) {
                         chi2 += kf_update(st, ym - yref, zm - zref, g.sy2, g.sz2);
                         if (kCount) n_up++;
                         nhits++;
@@ -307,9 +303,8 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         } else {
                             last_row = r;
                         }
-                    } else {
-                        __stcs(&rowhit[r], kNoHit);
-                        if (++gap > g.max_gap) stop = true;
+                    } else if (++gap > g.max_gap) {
+                        stop = true;
                     }
                 }
                 // where the next iteration goes
@@ -322,30 +317,11 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     if (stop || r == 0) mode = kDone;
                 }
             }
-            // ---- set up the next step: its row, the row's offset, the candidate's next own hit; look ahead ----
+            // ---- set up the next step: its row, the row's offset, the candidate's next own hit ----
             if (mode < kDone) {
                 rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : (mode == kCand ? r0 + i : r + 1));
                 rb = a.row_offsets[slab_base + rn];
-                if (mode == kCand) {
-                    hsn = a.cand_hits[(size_t)c * kCandMax + i];
-                } else if (TPC_FOLLOW_LA > 0 && la && mode != kBack) {
-                    // the coming steps search rows rn, rn + dir near the linear extrapolation of this step's move
-                    const float ye = st.y + yref + dyp - wy, ze = st.z + zref + dzp - wz;
-                    const float2 gy1 = s_rowy[rn];
-                    const int cell1 = zbin(ze, z0, g.inv_cz, g.nz) * g.ny + ybin(ye, gy1.x, gy1.y, g.ny);
-                    const uint16_t* t1 = a.bin_start + (size_t)(slab_base + rn) * g.nzp + cell1;
-                    if (TPC_FOLLOW_LA == 1) {
-                        prefetch_l1(t1);
-                    } else {
-                        const int r2 = 2 * rn - r;
-                        if (r2 >= 0 && r2 < g.R) {
-                            const float2 gy2 = s_rowy[r2];
-                            const int cell2 = zbin(ze + dzp, z0, g.inv_cz, g.nz) * g.ny + ybin(ye + dyp, gy2.x, gy2.y, g.ny);
-                            prefetch_l1(a.bin_start + (size_t)(slab_base + r2) * g.nzp + cell2);
-                        }
-                        prefetch_l1(a.hit_yz + rb + *t1);
-                    }
-                }
+                if (mode == kCand) hsn = a.cand_hits[(unsigned)c * (unsigned)kCandMax + (unsigned)i];
             }
         }
     }
