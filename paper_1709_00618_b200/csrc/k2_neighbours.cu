@@ -9,9 +9,9 @@
 // the order in which the grid presents the hits.  This file is additionally compiled with -fmad=false.
 //
 // One CTA per (sector instance, pad row).  The sorted (y,z) and the cell tables of the two adjacent rows are
-// staged in shared memory; rows or tables too long for that are read in place.  Per hit the
-// search is three flat loops instead of a nested one: window hits of row r+1, window hits of row r-1 (each through
-// the 2-D grid, a handful of candidates), then the pairs of the two short lists.
+// staged in shared memory; rows or tables too long for that are read in place.  Per hit the search is two flat
+// loops: the window hits of row r-1 (a handful, through the 2-D grid) are collected in registers, then every window
+// hit of row r+1 is paired with them.
 #include "tpc_common.cuh"
 
 namespace tpc {
@@ -49,24 +49,28 @@ __device__ __forceinline__ void consider(Best& b, float D, int ju, int jd, const
     }
 }
 
-// Positions (in the sorted row) of the hits of `row` inside the window, newest in the low 16 bits; returns how many
-// there are (only the last four are kept).
-__device__ __forceinline__ int window_hits(const DevGeom& g, const RowView& row, float ylo, float yhi, float zlo,
-                                           float zhi, int zb0, int zb1, unsigned long long& list) {
-    const int ys0 = ybin(ylo, row.y0, row.inv_sy, g.ny), ys1 = ybin(yhi, row.y0, row.inv_sy, g.ny);
-    int cnt = 0;
-    list = 0ull;
-    for (int zb = zb0; zb <= zb1; zb++) {
-        const int j0 = row.tbl[zb * g.ny + ys0], j1 = row.tbl[zb * g.ny + ys1 + 1];
-        for (int j = j0; j < j1; j++) {
-            const float2 h = row.yz[j];
-            if (ylo <= h.x && h.x <= yhi && zlo <= h.y && h.y <= zhi) {
-                list = (list << 16) | (unsigned long long)j;
-                cnt++;
-            }
-        }
+// The cells a window touches in one neighbour row, as ONE sequence of nt sorted positions: the first na start at a0
+// (z bin zb0, strips ys0..ys1 are contiguous in the sorted row), the rest at b0 (z bin zb1 when the window crosses a
+// bin edge).  Valid for zb1 - zb0 <= 1 (the default grid: bins wider than the window).
+struct CellSeq {
+    int a0, na, b0, nt;
+};
+
+__device__ __forceinline__ CellSeq window_cells(const DevGeom& g, const RowView& row, float ylo, float yhi, int zb0,
+                                                int zb1) {
+    const int ys0 = ybin(ylo, row.y0, row.inv_sy, g.ny), ys1 = ybin(yhi, row.y0, row.inv_sy, g.ny) + 1;
+    const uint16_t* ta = row.tbl + zb0 * g.ny;
+    CellSeq c;
+    c.a0 = ta[ys0];
+    c.na = (int)ta[ys1] - c.a0;
+    c.b0 = 0;
+    c.nt = c.na;
+    if (zb1 > zb0) {
+        const uint16_t* tb = row.tbl + zb1 * g.ny;
+        c.b0 = tb[ys0];
+        c.nt += (int)tb[ys1] - c.b0;
     }
-    return cnt;
+    return c;
 }
 
 // Exact search without the register lists (more than kNbList window hits in a neighbour row: dense spots only).
@@ -106,27 +110,53 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
         const float ylo = __fsub_rn(y, WY), yhi = __fadd_rn(y, WY);
         const float zlo = __fsub_rn(z, WZ), zhi = __fadd_rn(z, WZ);
         const int zb0 = zbin(zlo, z0, g.inv_cz, g.nz), zb1 = zbin(zhi, z0, g.inv_cz, g.nz);
-        unsigned long long lu, ld;
-        const int nu = window_hits(g, up, ylo, yhi, zlo, zhi, zb0, zb1, lu);
-        const int nd = window_hits(g, dn, ylo, yhi, zlo, zhi, zb0, zb1, ld);
         Best best{0.0f, -1, -1};
-        if (nu > kNbList || nd > kNbList) {
-            search_dense(g, up, dn, y, z, ylo, yhi, zlo, zhi, zb0, zb1, best);
-        } else if (nd > 0) {
-            for (int a = 0; a < nu; a++, lu >>= 16) {
-                const int ja = (int)(lu & 0xffffull);
-                const float2 u = up.yz[ja];
-                const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
-                unsigned long long l = ld;
-                for (int b = 0; b < nd; b++, l >>= 16) {
-                    const int jb = (int)(l & 0xffffull);
-                    const float2 d = dn.yz[jb];
-                    const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
-                    const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
-                    const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
-                    if (D <= D2MAX) consider(best, D, ja, jb, up.idx, dn.idx);
+        bool dense = zb1 - zb0 > 1;
+        if (!dense) {
+            // Two flat loops (one per neighbour row) over the handful of hits in the touched cells.  Row r-1 first:
+            // its window hits (at most kNbList = 4) stay in registers as (y - y_d, z - z_d) plus their positions,
+            // newest first; then every window hit of row r+1 is paired with them.
+            const CellSeq cd = window_cells(g, dn, ylo, yhi, zb0, zb1);
+            const CellSeq cu = window_cells(g, up, ylo, yhi, zb0, zb1);
+            float t2a = 0.0f, t2b = 0.0f, t2c = 0.0f, t2d = 0.0f, t4a = 0.0f, t4b = 0.0f, t4c = 0.0f, t4d = 0.0f;
+            unsigned long long ld = 0ull;
+            int nd = 0;
+            const int dshift = cd.b0 - cd.na;
+            for (int k = 0; k < cd.nt; k++) {
+                const int j = k < cd.na ? cd.a0 + k : k + dshift;
+                const float2 d = dn.yz[j];
+                if (ylo <= d.x && d.x <= yhi && zlo <= d.y && d.y <= zhi) {
+                    t2d = t2c; t2c = t2b; t2b = t2a; t2a = __fsub_rn(y, d.x);
+                    t4d = t4c; t4c = t4b; t4b = t4a; t4a = __fsub_rn(z, d.y);
+                    ld = (ld << 16) | (unsigned long long)j;
+                    nd++;
                 }
             }
+            dense = nd > kNbList;
+            if (!dense && nd > 0) {
+                const int ushift = cu.b0 - cu.na;
+                for (int k = 0; k < cu.nt; k++) {
+                    const int ja = k < cu.na ? cu.a0 + k : k + ushift;
+                    const float2 u = up.yz[ja];
+                    if (!(ylo <= u.x && u.x <= yhi && zlo <= u.y && u.y <= zhi)) continue;
+                    const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
+#define TPC_NB_PAIR(T2, T4, Q)                                                                      \
+    if (nd > Q) {                                                                                   \
+        const float ey = __fsub_rn(t1, T2), ez = __fsub_rn(t3, T4);                                 \
+        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                            \
+        if (D <= D2MAX) consider(best, D, ja, (int)((ld >> (16 * Q)) & 0xffffull), up.idx, dn.idx); \
+    }
+                    TPC_NB_PAIR(t2a, t4a, 0)
+                    TPC_NB_PAIR(t2b, t4b, 1)
+                    TPC_NB_PAIR(t2c, t4c, 2)
+                    TPC_NB_PAIR(t2d, t4d, 3)
+#undef TPC_NB_PAIR
+                }
+            }
+        }
+        if (dense) {  // more than kNbList window hits in row r-1, or a grid finer than the window: exact slow path
+            best = Best{0.0f, -1, -1};
+            search_dense(g, up, dn, y, z, ylo, yhi, zlo, zhi, zb0, zb1, best);
         }
         // links live in SORTED space: entry base + i belongs to the i-th hit of the sorted row, values are sorted
         // global positions; coalesced stores

@@ -42,6 +42,7 @@ struct FollowArgs {
     int32_t* tl_nhits;
     int32_t* tl_rows;
     uint16_t* tl_rowhit;
+    uint32_t* tl_sel;  // S6 record of the tracklet (k6_select.cu), zeroed here
 };
 
 // The best hit of the pick-up search so far.
@@ -138,6 +139,8 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 a.tl_chi2[c] = chi2;
                 a.tl_rows[c] = first_row | (last_row << 8) | (first_row << 16);
                 a.tl_nhits[c] = nhits;
+                uint4* rec = reinterpret_cast<uint4*>(a.tl_sel + (size_t)c * g.sel_stride);
+                for (int q4i = 0; q4i < g.sel_stride / 4; q4i++) rec[q4i] = make_uint4(0u, 0u, 0u, 0u);
                 mode = kIdle;
             }
             // ---- refill ----
@@ -343,7 +346,8 @@ int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_
     int grid = (int)(want < (int64_t)n_sm * kFollowCtasPerSm ? want : (int64_t)n_sm * kFollowCtasPerSm);
     if (grid < 1) grid = 1;
     FollowArgs a{p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.cand_hits, w.cand_n, w.cand_slab,
-                 w.counts,   w.Cmax,        w.tl_par, w.tl_cov,  w.tl_chi2,   w.tl_nhits,  w.tl_rows, w.tl_rowhit};
+                 w.counts,   w.Cmax,        w.tl_par, w.tl_cov,  w.tl_chi2,   w.tl_nhits,  w.tl_rows, w.tl_rowhit,
+                 w.tl_sel};
     if (count_work)
         follow_kernel<true><<<grid, kFollowThreads, 0, s>>>(g, a);
     else

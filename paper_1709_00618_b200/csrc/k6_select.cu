@@ -3,46 +3,32 @@
 // hits (ties: lowest candidate id); a tracklet keeps the hits it won and becomes a final track iff it keeps
 // >= sel_min hits; final tracks are numbered in ascending candidate id.  Integer-only, so results are unique.
 //
-// Warp per tracklet (the row-indexed hit table of one tracklet is one coalesced 2*R-byte read); claim by a 32-bit
-// atomicMax on the packed weight (nhits << 23 | inverted candidate id local to the sector instance); deterministic
-// numbering through per-block counts + one scan + in-block prefix.
+// claim (tracklet-centric): one 32-bit atomicMax of the packed weight (nhits << 23 | inverted candidate id local to
+// the sector instance) per attached hit.  A warp takes 32 consecutive tracklets: every lane loads one header
+// (coalesced), then the warp walks the 32 row-indexed hit tables, 4 rows per lane and 8-byte load.  The pass is bound
+// by the SM's issue rate for scattered atomics (~1.3 cycles per lane, B300_MICROARCH.md "Atomics").
+// Everything after it is HIT-centric: every pass streams over the hits once (coalesced) and touches one 32-byte
+// record per claimed hit:
+//   mark      per hit: winner tracklet from the claim word -> set the row's bit in the winner's kept-row mask
+//   count     per tracklet: kept = popcount(mask), tracks/hits per block of 256 tracklets, then one scan
+//   finalize  per tracklet: track index and first hit position (deterministic: ascending candidate id), track record
+//   write     per hit: owner and the track's hit list entry (rank = kept rows below, from the mask)
 #include "tpc_common.cuh"
 
 namespace tpc {
 
 constexpr int kSelThreads = 256;
-constexpr int kSelWarps = kSelThreads / 32;
-constexpr int kSelBlock = 64;  // tracklets per CTA work item
-constexpr int kSelPerWarp = kSelBlock / kSelWarps;
+constexpr int kSelBlock = kSelThreads;  // tracklets per CTA in the tracklet-centric passes
+constexpr int kHitThreads = 128;        // hit-centric passes: one CTA per (sector instance, pad row)
+constexpr unsigned kFull = 0xffffffffu;
 
-struct TlView {
-    int inst, first, last;
-    uint32_t w;
-    const uint16_t* rowhit;
-    const int32_t* ro;
-};
-
-__device__ __forceinline__ bool load_tracklet(const DevGeom& g, int64_t c, const int32_t* __restrict__ row_offsets,
-                                              const int32_t* __restrict__ tl_nhits,
-                                              const int32_t* __restrict__ tl_rows,
-                                              const int32_t* __restrict__ cand_slab,
-                                              const int2* __restrict__ slab_part,
-                                              const uint16_t* __restrict__ tl_rowhit, int64_t* counts, TlView& v) {
-    const int nh = tl_nhits[c];
-    if (nh == 0) return false;
-    const int rows = tl_rows[c];
-    v.first = rows & 0xff;
-    v.last = (rows >> 8) & 0xff;
-    v.inst = cand_slab[c] / g.R;
-    const int64_t lcid = c - slab_part[(size_t)v.inst * g.R].y;  // candidate ordinal inside its sector instance
-    if (lcid > 0x7FFFFF) atomicOr((unsigned long long*)&counts[5], 2ull);
-    v.w = ((uint32_t)nh << 23) | (uint32_t)(0x7FFFFF - (lcid & 0x7FFFFF));
-    v.rowhit = tl_rowhit + c * g.RP;
-    v.ro = row_offsets + (size_t)v.inst * g.R;
-    return true;
+__device__ __forceinline__ int64_t winner_of(uint32_t w, int64_t cand_base) {
+    return cand_base + (int64_t)(0x7FFFFFu - (w & 0x7FFFFFu));
 }
 
-__global__ void __launch_bounds__(kSelThreads)
+constexpr int kClaimThreads = 256;
+
+__global__ void __launch_bounds__(kClaimThreads)
 claim_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
              const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_rows,
              const int32_t* __restrict__ cand_slab, const int2* __restrict__ slab_part,
@@ -50,49 +36,91 @@ claim_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_
              int64_t Cmax) {
     const int64_t n_cand = min(counts[1], Cmax);
     const int lane = threadIdx.x & 31;
-    const int64_t warp0 = (int64_t)blockIdx.x * kSelWarps + (threadIdx.x >> 5);
-    for (int64_t c = warp0; c < n_cand; c += (int64_t)gridDim.x * kSelWarps) {
-        TlView v;
-        if (!load_tracklet(g, c, row_offsets, tl_nhits, tl_rows, cand_slab, slab_part, tl_rowhit, counts, v)) continue;
-        for (int r = v.first + lane; r <= v.last; r += 32) {
-            const uint16_t li = v.rowhit[r];
-            if (li != kNoHit) atomicMax(&claim[v.ro[r] + li], v.w);
+    const int64_t stride = (int64_t)gridDim.x * kClaimThreads;
+    for (int64_t c0 = (int64_t)blockIdx.x * kClaimThreads + (threadIdx.x & ~31); c0 < n_cand; c0 += stride) {
+        // header of the lane's tracklet
+        uint32_t my_w = 0u;
+        int my_rows = 0, my_inst = 0;
+        if (c0 + lane < n_cand) {
+            const int64_t c = c0 + lane;
+            const int nh = tl_nhits[c];
+            my_rows = tl_rows[c];
+            my_inst = cand_slab[c] / g.R;
+            if (nh > 0) {
+                const int64_t lcid = c - slab_part[(size_t)my_inst * g.R].y;  // candidate ordinal inside its instance
+                if (lcid > 0x7FFFFF) atomicOr((unsigned long long*)&counts[5], 2ull);
+                my_w = ((uint32_t)nh << 23) | (uint32_t)(0x7FFFFF - (lcid & 0x7FFFFF));
+            }
+        }
+        for (unsigned todo = __ballot_sync(kFull, my_w != 0u); todo; todo &= todo - 1) {
+            const int k = __ffs(todo) - 1;
+            const uint32_t w = __shfl_sync(kFull, my_w, k);
+            const int rows = __shfl_sync(kFull, my_rows, k), inst = __shfl_sync(kFull, my_inst, k);
+            const int first = rows & 0xff, last = (rows >> 8) & 0xff;
+            const uint16_t* rh = tl_rowhit + (size_t)(c0 + k) * g.RP;
+            const int32_t* ro = row_offsets + (size_t)inst * g.R;
+            for (int rq = (first & ~127) + 4 * lane; rq <= last; rq += 128) {
+                if (rq + 3 < first) continue;
+                const uint2 v = *reinterpret_cast<const uint2*>(rh + rq);  // RP % 8 == 0: in bounds, 8-byte aligned
+                const uint32_t li[4] = {v.x & 0xffffu, v.x >> 16, v.y & 0xffffu, v.y >> 16};
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    const int r = rq + j;
+                    if (r >= first && r <= last && li[j] != kNoHit) atomicMax(&claim[ro[r] + (int)li[j]], w);
+                }
+            }
         }
     }
 }
 
+__global__ void __launch_bounds__(kHitThreads)
+mark_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
+            const int2* __restrict__ slab_part, const uint32_t* __restrict__ claim, uint32_t* __restrict__ tl_sel) {
+    const int slab = blockIdx.x;
+    const int inst = slab / g.R, r = slab - inst * g.R;
+    const int base = row_offsets[slab], n = row_offsets[slab + 1] - base;
+    if (n == 0) return;
+    const int64_t cand_base = slab_part[(size_t)inst * g.R].y;
+    const uint32_t bit = 1u << (r & 31);
+    for (int i = threadIdx.x; i < n; i += kHitThreads) {
+        const uint32_t w = claim[base + i];
+        if (w) atomicOr(&tl_sel[winner_of(w, cand_base) * g.sel_stride + (r >> 5)], bit);
+    }
+}
+
+// kept hits of tracklet c from its mask (0 if below sel_min)
+__device__ __forceinline__ int kept_of(const DevGeom& g, const uint32_t* __restrict__ tl_sel, int64_t c) {
+    const uint4* rec = reinterpret_cast<const uint4*>(tl_sel + c * g.sel_stride);
+    int kept = 0;
+    for (int q = 0; q < g.sel_words; q += 4) {  // words past sel_words inside the last uint4 are masked below
+        const uint4 v = rec[q >> 2];
+        kept += __popc(v.x);
+        if (q + 1 < g.sel_words) kept += __popc(v.y);
+        if (q + 2 < g.sel_words) kept += __popc(v.z);
+        if (q + 3 < g.sel_words) kept += __popc(v.w);
+    }
+    return kept < g.sel_min ? 0 : kept;
+}
+
 __global__ void __launch_bounds__(kSelThreads)
-count_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
-             const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_rows,
-             const int32_t* __restrict__ cand_slab, const int2* __restrict__ slab_part,
-             const uint16_t* __restrict__ tl_rowhit, const uint32_t* __restrict__ claim,
-             int32_t* __restrict__ tl_kept, int2* __restrict__ sel_part, int64_t* __restrict__ counts, int64_t Cmax) {
+count_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ tl_nhits,
+             const uint32_t* __restrict__ tl_sel, int2* __restrict__ sel_part, int64_t* __restrict__ counts,
+             int64_t Cmax) {
     __shared__ int s_cnt[3];
     const int64_t n_cand = min(counts[1], Cmax);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
     for (int64_t blk = blockIdx.x; blk * kSelBlock < n_cand; blk += gridDim.x) {
         if (threadIdx.x < 3) s_cnt[threadIdx.x] = 0;
         __syncthreads();
-        int n_trk = 0, n_hit = 0, n_tl = 0;
-        for (int i = 0; i < kSelPerWarp; i++) {
-            const int64_t c = blk * kSelBlock + wid * kSelPerWarp + i;
-            if (c >= n_cand) break;
-            TlView v;
-            int kept = 0;
-            if (load_tracklet(g, c, row_offsets, tl_nhits, tl_rows, cand_slab, slab_part, tl_rowhit, counts, v)) {
-                n_tl++;
-                for (int r = v.first + lane; r <= v.last; r += 32) {
-                    const uint16_t li = v.rowhit[r];
-                    if (li != kNoHit && claim[v.ro[r] + li] == v.w) kept++;
-                }
-#pragma unroll
-                for (int d = 16; d > 0; d >>= 1) kept += __shfl_xor_sync(0xffffffffu, kept, d);
-                if (kept < g.sel_min) kept = 0;
-            }
-            if (lane == 0) tl_kept[c] = kept;
-            n_trk += kept > 0;
-            n_hit += kept;
+        const int64_t c = blk * kSelBlock + threadIdx.x;
+        int kept = 0, have = 0;
+        if (c < n_cand && tl_nhits[c] > 0) {
+            have = 1;
+            kept = kept_of(g, tl_sel, c);
         }
+        const int n_trk = __reduce_add_sync(kFull, kept > 0 ? 1 : 0);
+        const int n_hit = __reduce_add_sync(kFull, kept);
+        const int n_tl = __reduce_add_sync(kFull, have);
         if (lane == 0) {
             atomicAdd(&s_cnt[0], n_trk);
             atomicAdd(&s_cnt[1], n_hit);
@@ -107,81 +135,88 @@ count_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_
     }
 }
 
+struct FinalIn {
+    const int32_t* tl_nhits;
+    const int32_t* tl_rows;
+    const int32_t* cand_slab;
+    const float* tl_par;
+    const float* tl_cov;
+    const float* tl_chi2;
+    const int2* sel_part;
+    uint32_t* tl_sel;
+    int64_t* counts;
+    int64_t Cmax;
+};
+
 __global__ void __launch_bounds__(kSelThreads)
-write_tracks_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
-                    const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_rows,
-                    const int32_t* __restrict__ cand_slab, const int2* __restrict__ slab_part,
-                    const uint16_t* __restrict__ tl_rowhit, const uint32_t* __restrict__ claim,
-                    const int32_t* __restrict__ tl_kept, const int2* __restrict__ sel_part,
-                    const float* __restrict__ tl_par, const float* __restrict__ tl_cov,
-                    const float* __restrict__ tl_chi2, const uint16_t* __restrict__ hit_idx,
-                    int64_t* __restrict__ counts, int64_t Cmax, const SelectOut o) {
-    __shared__ int s_kept[kSelBlock];
-    __shared__ int2 s_off[kSelBlock];
-    const int64_t n_cand = min(counts[1], Cmax);
+finalize_tracks_kernel(const __grid_constant__ DevGeom g, const FinalIn a, const SelectOut o) {
+    __shared__ int2 s_warp[kSelThreads / 32];
+    const int64_t n_cand = min(a.counts[1], a.Cmax);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     for (int64_t blk = blockIdx.x; blk * kSelBlock < n_cand; blk += gridDim.x) {
-        if (threadIdx.x < kSelBlock) {
-            const int64_t c = blk * kSelBlock + threadIdx.x;
-            s_kept[threadIdx.x] = c < n_cand ? tl_kept[c] : 0;
-        }
-        __syncthreads();
-        if (wid == 0) {  // exclusive prefix over the 64 tracklets of the block (two per lane)
-            const int k0 = s_kept[2 * lane], k1 = s_kept[2 * lane + 1];
-            int t = (k0 > 0) + (k1 > 0), h = k0 + k1;
-            int ti = t, hi = h;
+        const int64_t c = blk * kSelBlock + threadIdx.x;
+        int kept = 0;
+        if (c < n_cand && a.tl_nhits[c] > 0) kept = kept_of(g, a.tl_sel, c);
+        // exclusive prefix of (tracks, hits) inside the block: warp scan + warp totals
+        const int t = kept > 0 ? 1 : 0;
+        int ti = t, hi = kept;
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const int a = __shfl_up_sync(0xffffffffu, ti, d), b = __shfl_up_sync(0xffffffffu, hi, d);
-                if (lane >= d) { ti += a; hi += b; }
-            }
-            s_off[2 * lane] = make_int2(ti - t, hi - h);
-            s_off[2 * lane + 1] = make_int2(ti - t + (k0 > 0), hi - h + k0);
+        for (int d = 1; d < 32; d <<= 1) {
+            const int x = __shfl_up_sync(kFull, ti, d), y = __shfl_up_sync(kFull, hi, d);
+            if (lane >= d) { ti += x; hi += y; }
         }
+        if (lane == 31) s_warp[wid] = make_int2(ti, hi);
         __syncthreads();
-        const int2 base = sel_part[blk];
-        for (int i = 0; i < kSelPerWarp; i++) {
-            const int q = wid * kSelPerWarp + i;
-            const int64_t c = blk * kSelBlock + q;
-            if (c >= n_cand || s_kept[q] == 0) continue;
-            const int64_t trk = (int64_t)base.x + s_off[q].x;
-            const int64_t h0 = (int64_t)base.y + s_off[q].y;
-            TlView v;
-            load_tracklet(g, c, row_offsets, tl_nhits, tl_rows, cand_slab, slab_part, tl_rowhit, counts, v);
-            const bool fits = trk < o.trk_capacity;
-            if (fits) {
-                if (o.trk_params && lane < 5) o.trk_params[trk * 5 + lane] = tl_par[c * 5 + lane];
-                if (o.trk_cov && lane < 15) o.trk_cov[trk * 15 + lane] = tl_cov[c * 15 + lane];
-                if (lane == 0) {
-                    if (o.trk_chi2) o.trk_chi2[trk] = tl_chi2[c];
-                    if (o.trk_xref) o.trk_xref[trk] = g.row_x[(tl_rows[c] >> 16) & 0xff];
-                    if (o.trk_cand_id) o.trk_cand_id[trk] = (int32_t)c;
-                    if (o.trk_nhits) o.trk_nhits[trk] = s_kept[q];
-                    if (o.trk_sector) o.trk_sector[trk] = v.inst;
-                    if (o.trk_hit_offset) o.trk_hit_offset[trk] = h0;
-                }
-            }
-            int run = 0;
-            for (int rb = v.first; rb <= v.last; rb += 32) {
-                const int r = rb + lane;
-                int gh = -1;
-                if (r <= v.last) {
-                    const uint16_t li = v.rowhit[r];
-                    if (li != kNoHit) {
-                        const int hh = v.ro[r] + li;  // sorted space; the outputs take the input-order index
-                        if (claim[hh] == v.w) gh = v.ro[r] + (int)hit_idx[hh];
-                    }
-                }
-                const unsigned m = __ballot_sync(0xffffffffu, gh >= 0);
-                if (gh >= 0 && fits) {
-                    const int64_t pos = h0 + run + __popc(m & ((1u << lane) - 1u));
-                    if (o.trk_hits && pos < o.trk_hits_capacity) o.trk_hits[pos] = gh;
-                    if (o.cluster_owner) o.cluster_owner[gh] = (int32_t)trk;
-                }
-                run += __popc(m);
-            }
-        }
+        int2 off = a.sel_part[blk];
+        for (int k = 0; k < wid; k++) { off.x += s_warp[k].x; off.y += s_warp[k].y; }
         __syncthreads();
+        if (c >= n_cand) continue;
+        const int64_t trk = (int64_t)off.x + ti - t;
+        const int64_t h0 = (int64_t)off.y + hi - kept;
+        const bool is_trk = kept > 0 && trk < o.trk_capacity;
+        uint32_t* rec = a.tl_sel + c * g.sel_stride;
+        rec[g.sel_words] = is_trk ? (uint32_t)trk : 0xFFFFFFFFu;
+        rec[g.sel_words + 1] = (uint32_t)h0;
+        if (!is_trk) continue;
+        const int rows = a.tl_rows[c];
+        if (o.trk_params)
+#pragma unroll
+            for (int q = 0; q < 5; q++) o.trk_params[trk * 5 + q] = a.tl_par[c * 5 + q];
+        if (o.trk_cov)
+#pragma unroll
+            for (int q = 0; q < 15; q++) o.trk_cov[trk * 15 + q] = a.tl_cov[c * 15 + q];
+        if (o.trk_chi2) o.trk_chi2[trk] = a.tl_chi2[c];
+        if (o.trk_xref) o.trk_xref[trk] = g.row_x[(rows >> 16) & 0xff];
+        if (o.trk_cand_id) o.trk_cand_id[trk] = (int32_t)c;
+        if (o.trk_nhits) o.trk_nhits[trk] = kept;
+        if (o.trk_sector) o.trk_sector[trk] = a.cand_slab[c] / g.R;
+        if (o.trk_hit_offset) o.trk_hit_offset[trk] = h0;
+    }
+}
+
+__global__ void __launch_bounds__(kHitThreads)
+write_hits_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
+                  const int2* __restrict__ slab_part, const uint32_t* __restrict__ claim,
+                  const uint32_t* __restrict__ tl_sel, const uint16_t* __restrict__ hit_idx, const SelectOut o) {
+    const int slab = blockIdx.x;
+    const int inst = slab / g.R, r = slab - inst * g.R;
+    const int base = row_offsets[slab], n = min(row_offsets[slab + 1] - base, 65535);
+    if (n == 0) return;
+    const int64_t cand_base = slab_part[(size_t)inst * g.R].y;
+    const int wq = r >> 5;
+    const uint32_t below = (1u << (r & 31)) - 1u;
+    for (int i = threadIdx.x; i < n; i += kHitThreads) {
+        const uint32_t w = claim[base + i];
+        if (!w) continue;
+        const uint32_t* rec = tl_sel + winner_of(w, cand_base) * g.sel_stride;
+        const uint32_t trk = rec[g.sel_words];
+        if (trk == 0xFFFFFFFFu) continue;  // the winner is not a final track: the hit stays unassigned
+        int rank = __popc(rec[wq] & below);
+        for (int q = 0; q < wq; q++) rank += __popc(rec[q]);
+        const int gi = base + (int)hit_idx[base + i];  // sorted space -> input-order index
+        if (o.cluster_owner) o.cluster_owner[gi] = (int32_t)trk;
+        const int64_t pos = (int64_t)rec[g.sel_words + 1] + rank;
+        if (o.trk_hits && pos < o.trk_hits_capacity) o.trk_hits[pos] = gi;
     }
 }
 
@@ -199,19 +234,19 @@ void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m
 int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const SelectOut& o, cudaStream_t s) {
     int launches = 0;
     if (p.n_clusters > 0) {
+        const int slabs = p.n_inst * g.R;
         const int64_t blocks = div_up(w.Cmax, kSelBlock);
-        const int grid_b = (int)(blocks < 148 * 16 ? blocks : 148 * 16);
-        const int64_t warps = div_up(w.Cmax, kSelWarps);
-        const int grid_w = (int)(warps < 148 * 16 ? warps : 148 * 16);
-        claim_kernel<<<grid_w, kSelThreads, 0, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows, w.cand_slab, w.slab_part,
+        const int grid = (int)(blocks < 148 * 8 ? blocks : 148 * 8);
+        claim_kernel<<<grid, kClaimThreads, 0, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows, w.cand_slab, w.slab_part,
                                                     w.tl_rowhit, w.claim, w.counts, w.Cmax);
-        count_kernel<<<grid_b, kSelThreads, 0, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows, w.cand_slab, w.slab_part,
-                                                    w.tl_rowhit, w.claim, w.tl_kept, w.sel_part, w.counts, w.Cmax);
+        mark_kernel<<<slabs, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel);
+        count_kernel<<<grid, kSelThreads, 0, s>>>(g, w.tl_nhits, w.tl_sel, w.sel_part, w.counts, w.Cmax);
         launch_scan_int2(w.sel_part, w.counts + 1, kSelBlock, w.Cmax, 0, w.counts, 3, 4, s);
-        write_tracks_kernel<<<grid_b, kSelThreads, 0, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows, w.cand_slab,
-                                                           w.slab_part, w.tl_rowhit, w.claim, w.tl_kept, w.sel_part,
-                                                           w.tl_par, w.tl_cov, w.tl_chi2, w.hit_idx, w.counts, w.Cmax, o);
-        launches += 4;
+        const FinalIn a{w.tl_nhits, w.tl_rows, w.cand_slab, w.tl_par, w.tl_cov, w.tl_chi2, w.sel_part, w.tl_sel,
+                        w.counts,   w.Cmax};
+        finalize_tracks_kernel<<<grid, kSelThreads, 0, s>>>(g, a, o);
+        write_hits_kernel<<<slabs, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel, w.hit_idx, o);
+        launches += 6;
     }
     finalize_counts_kernel<<<1, 32, 0, s>>>(w.counts, o);
     return launches + 1;

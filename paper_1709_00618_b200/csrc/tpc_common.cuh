@@ -17,6 +17,8 @@ constexpr float kKappaPerTesla = 0.00299792458f;
 struct DevGeom {
     int R;          // pad rows
     int RP;         // row stride of the per-tracklet hit table (R rounded up to 8)
+    int sel_words;  // 32-bit words of a tracklet's kept-row mask (S6): ceil(R / 32)
+    int sel_stride; // words per S6 tracklet record: mask, track index, first hit position; multiple of 4 (16 B)
     int nz;         // z bins per row
     int ny;         // y strips per row
     int ncell;      // nz * ny cells per row, cell id = zbin * ny + ystrip (a y range inside one z bin is contiguous)
@@ -61,8 +63,8 @@ struct Workspace {
     int32_t* tl_nhits;    // [Cmax]  0 = no tracklet
     int32_t* tl_rows;     // [Cmax]  first | last << 8 | ref << 16
     uint16_t* tl_rowhit;  // [Cmax][RP] position in the sorted row of the attached hit (valid in first..last), kNoHit = none
-    int32_t* tl_kept;     // [Cmax]  hits won in the selector, 0 if rejected
-    int2* sel_part;       // [Cmax/64 + 2] (tracks, hits) per block of 64 tracklets, then exclusive scan
+    uint32_t* tl_sel;     // [Cmax][sel_stride] S6 record: kept-row mask, final track index (or ~0), first hit position
+    int2* sel_part;       // [Cmax/64 + 2] (tracks, hits) per block of 256 tracklets, then exclusive scan
     int64_t* counts;      // [8] internal copy of the output counts
     int64_t Cmax;
 };

@@ -43,6 +43,8 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     DevGeom& g = t->g;
     g.R = R;
     g.RP = (R + 7) & ~7;
+    g.sel_words = (R + 31) / 32;
+    g.sel_stride = (g.sel_words + 2 + 3) & ~3;
     // per-row 2-D grid: ny strips across the row, z bins of cz (performance only, no result depends on either).
     // Default cz = 6.25 cm > 2 * max(kf_win_max, nf_win_z) + margins, so a search window touches at most 2 z bins.
     int ny = dflt(p.grid_cells_y, 16);
@@ -159,7 +161,7 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.tl_nhits = c.take<int32_t>(cmax);
     v.tl_rows = c.take<int32_t>(cmax);
     v.tl_rowhit = c.take<uint16_t>(cmax * g.RP);
-    v.tl_kept = c.take<int32_t>(cmax);
+    v.tl_sel = c.take<uint32_t>(cmax * g.sel_stride);
     v.sel_part = c.take<int2>(cmax / 64 + 2);
     v.Cmax = (int64_t)cmax;
     if (w) *w = v;
