@@ -3,28 +3,44 @@
 // (Fig. 1c); constant Bz only.  Control flow: DESIGN.md "S5" (seed, phase A upward,
 // one-step back transport, phase B downward).  One thread per candidate, all arithmetic fp32 in registers.
 //
-// Execution model: persistent warps, every lane a small state machine that advances its
-// candidate by exactly ONE pad row per loop iteration whatever its phase (own hits / upward / back transport /
-// downward), so the lanes of a warp run the same transport-search-update code instead of diverging on phase and
-// track length.  A lane whose candidate has ended parks until a few lanes are parked, then those lanes write
-// their tracklets and take new candidates from the warp's chunk of the device-wide queue (consecutive candidate
-// ids start in neighbouring rows of one sector instance, which keeps the warp's loads in the same L1 lines).
+// Two kernels:
+//  * fit_candidates_kernel: seed + Kalman fit of the candidate's own 4..10 hits.  Every address is known up front, so
+//    all loads of a candidate are in flight together; the state after the last own hit goes to tl_state.
+//  * follow_kernel: the row-by-row extrapolation.  Persistent warps, every lane a small state machine that advances
+//    its candidate by ONE pad row per loop iteration (upward / back transport / downward), with the lanes refilled
+//    from a device-wide queue as candidates end.  The two dependent memory round trips of a pick-up search (cell
+//    table -> hits) are taken off the critical path by a two-stage software pipeline: the cell-table entries of the
+//    row TWO steps ahead and the first two hits of the row ONE step ahead are loaded speculatively for a window
+//    around the linearly extrapolated position, widened by a margin.  At the step itself the exact window is
+//    computed; if its cells are covered by the speculated ones (almost always) the preloaded data are used --
+//    examining a superset of cells is harmless because every hit still passes the exact gate test (the grid is an
+//    acceleration structure only) -- otherwise the step falls back to direct loads.
 #include "kf_math.cuh"
 
 #ifndef TPC_FOLLOW_CTAS
-#define TPC_FOLLOW_CTAS 6
+#define TPC_FOLLOW_CTAS 5
+#endif
+#ifndef TPC_FOLLOW_RELOAD
+#define TPC_FOLLOW_RELOAD 4
 #endif
 namespace tpc {
 
 constexpr int kFollowThreads = 128;
 constexpr int kFollowCtasPerSm = TPC_FOLLOW_CTAS;
-constexpr int kFollowChunk = 64;   // candidates a warp takes from the queue at a time
-#ifndef TPC_FOLLOW_RELOAD
-#define TPC_FOLLOW_RELOAD 4
-#endif
+constexpr int kFollowChunk = 64;                  // candidates a warp takes from the queue at a time
 constexpr int kFollowReload = TPC_FOLLOW_RELOAD;  // parked lanes that trigger a write-out / refill phase
+constexpr int kFitThreads = 128;
+#ifndef TPC_SPEC_HITS
+#define TPC_SPEC_HITS 4
+#endif
+#ifndef TPC_SPEC_MARGIN
+#define TPC_SPEC_MARGIN 0.25f
+#endif
+constexpr int kSpecHits = TPC_SPEC_HITS;          // hits of the coming window fetched ahead
+constexpr float kSpecMargin = TPC_SPEC_MARGIN;  // [cm] widening of the speculated window (performance only)
+constexpr float kCellMargin = 1e-3f;  // [cm] the visited cells are a superset of the rounded fp32 gate test
 
-enum FollowMode : int { kCand = 0, kUp = 1, kBack = 2, kDown = 3, kDone = 4, kIdle = 5 };
+enum FollowMode : int { kUp = 0, kBack = 1, kDown = 2, kDone = 3, kIdle = 4 };
 
 struct FollowArgs {
     const int32_t* row_offsets;
@@ -36,6 +52,7 @@ struct FollowArgs {
     const int32_t* cand_slab;
     int64_t* counts;
     int64_t Cmax;
+    float4* tl_state;  // [6][Cmax] state after the candidate's own hits (fit kernel -> follow kernel)
     float* tl_par;
     float* tl_cov;
     float* tl_chi2;
@@ -44,6 +61,116 @@ struct FollowArgs {
     uint16_t* tl_rowhit;
     uint32_t* tl_sel;  // S6 record of the tracklet (k6_select.cu), zeroed here
 };
+
+__device__ __forceinline__ void zero_tracklet(const DevGeom& g, const FollowArgs& a, int c) {
+    float* p = a.tl_par + (size_t)c * 5;
+#pragma unroll
+    for (int q = 0; q < 5; q++) p[q] = 0.0f;
+    float* v = a.tl_cov + (size_t)c * 15;
+#pragma unroll
+    for (int q = 0; q < 15; q++) v[q] = 0.0f;
+    a.tl_chi2[c] = 0.0f;
+    a.tl_rows[c] = 0;
+    a.tl_nhits[c] = 0;
+    uint4* rec = reinterpret_cast<uint4*>(a.tl_sel + (size_t)c * g.sel_stride);
+    for (int q = 0; q < g.sel_stride / 4; q++) rec[q] = make_uint4(0u, 0u, 0u, 0u);
+}
+
+// ---- fit of the candidate's own hits -----------------------------------------------------------------------------
+template <bool kCount>
+__global__ void __launch_bounds__(kFitThreads)
+fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowArgs a) {
+    const int n_cand = (int)min(a.counts[1], a.Cmax);
+    const int c = blockIdx.x * kFitThreads + threadIdx.x;
+    unsigned n_tr = 0, n_up = 0;
+    if (c < n_cand) {
+        const int slab0 = a.cand_slab[c];
+        const int inst = slab0 / g.R;
+        const int r0 = slab0 - inst * g.R;
+        const int n = a.cand_n[c];
+        // the candidate's hits: sorted global positions (5 x 8-byte loads), coordinates and row offsets
+        int pos[kCandMax];
+        const int2* ch = reinterpret_cast<const int2*>(a.cand_hits + (size_t)c * kCandMax);
+#pragma unroll
+        for (int q = 0; q < kCandMax / 2; q++) {
+            const int2 v = ch[q];
+            pos[2 * q] = v.x;
+            pos[2 * q + 1] = v.y;
+        }
+        float2 h[kCandMax];
+        int rb[kCandMax];
+        float x[kCandMax];
+#pragma unroll
+        for (int q = 0; q < kCandMax; q++) {
+            h[q] = make_float2(0.0f, 0.0f);
+            rb[q] = 0;
+            x[q] = 0.0f;
+            if (q < n) {
+                h[q] = a.hit_yz[pos[q]];
+                rb[q] = a.row_offsets[slab0 + q];
+                x[q] = g.row_x[r0 + q];
+            }
+        }
+        // seed from hits 0, n/2, n-1.  The state carries y and z relative to the first candidate hit: the model is
+        // translation invariant in y and z, so this is exact, and it keeps the fp32 rounding of the two
+        // coordinates (ulp(20 cm), ulp(250 cm)) out of q/pt and sinPhi.
+        const int i1 = n >> 1, i2 = n - 1;
+        float2 h1 = h[0], h2 = h[0];
+        float x1 = x[0], x2 = x[0];
+#pragma unroll
+        for (int q = 1; q < kCandMax; q++) {
+            if (q == i1) { h1 = h[q]; x1 = x[q]; }
+            if (q == i2) { h2 = h[q]; x2 = x[q]; }
+        }
+        const float yref = h[0].x, zref = h[0].y;
+        KfState st;
+        bool ok = kf_seed(st, x[0], 0.0f, 0.0f, x1, h1.x - yref, x2, h2.x - yref, h2.y - zref, g.cB, g.max_s, g.p0);
+        float chi2 = 0.0f;
+        if (ok) {
+#pragma unroll
+            for (int q = 0; q < kCandMax; q++) {
+                if (q < n && ok) {
+                    if (q > 0) {
+                        ok = kf_transport(st, x[q] - x[q - 1], g.cB, g.max_s);
+                        if (kCount && ok) n_tr++;
+                    }
+                    if (ok) {
+                        chi2 += kf_update(st, h[q].x - yref, h[q].y - zref, g.sy2, g.sz2);
+                        if (kCount) n_up++;
+                    }
+                }
+            }
+        }
+        float4* ts = a.tl_state + c;
+        const size_t cs = (size_t)a.Cmax;
+        if (ok) {
+            ts[0] = make_float4(st.y, st.z, st.s, st.t);
+            ts[cs] = make_float4(st.k, st.c00, st.c10, st.c11);
+            ts[2 * cs] = make_float4(st.c20, st.c21, st.c22, st.c30);
+            ts[3 * cs] = make_float4(st.c31, st.c32, st.c33, st.c40);
+            ts[4 * cs] = make_float4(st.c41, st.c42, st.c43, st.c44);
+            ts[5 * cs] = make_float4(yref, zref, chi2, __int_as_float(n));
+            uint16_t* rh = a.tl_rowhit + (size_t)c * g.RP + r0;
+#pragma unroll
+            for (int q = 0; q < kCandMax; q++)
+                if (q < n) __stcs(&rh[q], (uint16_t)(pos[q] - rb[q]));
+        } else {  // no tracklet: an all-zero record, and the follower skips the candidate
+            ts[5 * cs] = make_float4(0.0f, 0.0f, 0.0f, __int_as_float(0));
+            zero_tracklet(g, a, c);
+        }
+    }
+    if (kCount) {
+        const unsigned full = 0xffffffffu;
+        n_tr = __reduce_add_sync(full, n_tr);
+        n_up = __reduce_add_sync(full, n_up);
+        if ((threadIdx.x & 31) == 0) {
+            if (n_tr) atomicAdd((unsigned long long*)&a.counts[6], (unsigned long long)n_tr);
+            if (n_up) atomicAdd((unsigned long long*)&a.counts[7], (unsigned long long)n_up);
+        }
+    }
+}
+
+// ---- row-by-row following ------------------------------------------------------------------------------------------
 
 // The best hit of the pick-up search so far.
 struct PickBest {
@@ -64,14 +191,20 @@ __device__ __forceinline__ void pick_consider(PickBest& b, const uint16_t* __res
     const float d2 = __fadd_rn(__fmul_rn(dy, dy), __fmul_rn(dz, dz));
     const bool in = valid && fabsf(dy) <= wy && fabsf(dz) <= wz;
     bool better = in && d2 < b.d2;
-    if (in && d2 == b.d2 && j != b.j) better = tie_lower_index(idx, rb + (unsigned)j, rb + (unsigned)b.j);
-    if (better) {
-        b.j = j;
-        b.d2 = d2;
-        b.y = h.x;
-        b.z = h.y;
-    }
+    if (in && d2 == b.d2) better = tie_lower_index(idx, rb + (unsigned)j, rb + (unsigned)b.j);  // b.d2 finite: b.j >= 0
+    b.j = better ? j : b.j;
+    b.d2 = better ? d2 : b.d2;
+    b.y = better ? h.x : b.y;
+    b.z = better ? h.y : b.z;
 }
+
+// Speculative hit loads go straight to shared memory (cp.async, 8 bytes): no register is tied up while they fly.
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 __device__ __forceinline__ float sqrt_fast(float x) {  // x > 0, normal range
     float r;
@@ -87,9 +220,37 @@ __device__ __forceinline__ void store_report(float4 (*s_rep)[kFollowThreads], co
     s_rep[4][threadIdx.x] = make_float4(st.c41, st.c42, st.c43, st.c44);
 }
 
-__device__ __forceinline__ void zero_report(float4 (*s_rep)[kFollowThreads]) {
-#pragma unroll
-    for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+// The cells of a search window in one row: z bins zb0 and (if two) zb0 + 1, strips ys0 .. ys1 - 1; packed
+// ys0 | ys1 << 8 | zb0 << 16 | two << 31.  kNoCells = not usable (window wider than two z bins).
+constexpr unsigned kNoCells = 0xffffffffu;
+
+struct Window {
+    int zb0, zb1, ys0, ys1;  // ys1 exclusive
+};
+
+__device__ __forceinline__ Window window_cells(const DevGeom& g, float2 gy, float z0, float yp, float zp, float wy,
+                                               float wz) {
+    Window w;
+    w.zb0 = zbin(zp - wz, z0, g.inv_cz, g.nz);
+    w.zb1 = zbin(zp + wz, z0, g.inv_cz, g.nz);
+    w.ys0 = ybin(yp - wy, gy.x, gy.y, g.ny);
+    w.ys1 = ybin(yp + wy, gy.x, gy.y, g.ny) + 1;
+    return w;
+}
+
+// The window's hits as one sequence of nt sorted positions: the first na start at ja0, element k >= na sits at k + d.
+struct HitSeq {
+    int ja0, na, nt, d;
+};
+
+__device__ __forceinline__ HitSeq hit_seq(unsigned tab0, unsigned tab1, bool two) {
+    HitSeq s;
+    s.ja0 = (int)(tab0 & 0xffffu);
+    s.na = (int)(tab0 >> 16) - s.ja0;
+    const int jb0 = (int)(tab1 & 0xffffu);
+    s.nt = s.na + (two ? (int)(tab1 >> 16) - jb0 : 0);
+    s.d = jb0 - s.na;
+    return s;
 }
 
 // kCount: also accumulate the work counters counts[6..9] (roofline arithmetic; tpc_set_work_counters).  They are a
@@ -100,6 +261,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
     __shared__ float s_rowx[kMaxRows + 1];
     __shared__ float2 s_rowy[kMaxRows + 1];      // (y0, strips per cm) of the row's grid
     __shared__ float4 s_rep[5][kFollowThreads];  // reported state of the lane's tracklet (see kDown below)
+    __shared__ float2 s_hit[kSpecHits][kFollowThreads];  // speculative copies of the coming window's first hits
     for (int q = threadIdx.x; q < g.R; q += kFollowThreads) {
         s_rowx[q] = g.row_x[q];
         s_rowy[q] = make_float2(g.row_y0[q], g.row_inv_sy[q]);
@@ -108,6 +270,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int n_cand = (int)min(a.counts[1], a.Cmax);
+    const size_t cs = (size_t)a.Cmax;
     unsigned long long* queue = reinterpret_cast<unsigned long long*>(&a.counts[10]);
     int wn = 0, we = 0;  // the warp's chunk [wn, we) of candidate ids (warp-uniform)
     bool exhausted = false;
@@ -116,12 +279,18 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
     // lane state
     int mode = kIdle;
     int c = 0, slab_base = 0;
-    int r = 0, rn = 0, rb = 0;      // row of the state, row of the coming step and its offset in the hit arrays
-    int r0 = 0, n = 0, i = 0;       // start row, candidate length, next own hit
-    int hsn = 0;                    // sorted global position of the candidate's next own hit
+    int r = 0, rn = 0, r0 = 0;  // row of the state, row of the coming step, start row
     int nhits = 0, gap = 0, first_row = 0, last_row = 0;
     float yref = 0.0f, zref = 0.0f, z0 = 0.0f, chi2 = 0.0f;
     KfState st = {};
+    // Speculation pipeline.  Slot A belongs to the coming step (row rn): packed cell-table entries, the cells they
+    // were read for, the row's offset and the first two hits of the window.  Slot B holds the raw cell-table loads
+    // issued last for the row after that (or for rn itself while the pipeline fills); its registers are not
+    // touched before the iteration after the one that issued them, so no load is waited for where it is issued.
+    bool tabA_ok = false, hitA_ok = false, tabB_ok = false;
+    unsigned cellsA = kNoCells, cellsB = kNoCells, tabA0 = 0u, tabA1 = 0u;
+    unsigned tB00 = 0u, tB01 = 0u, tB10 = 0u, tB11 = 0u;
+    int rbA = 0, rbB = 0;
 
     for (;;) {
         unsigned act = __ballot_sync(full, mode < kDone);
@@ -160,40 +329,31 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 const int mine = wn + __popc(idle & ((1u << lane) - 1u));
                 if (mode == kIdle && mine < we) {
                     c = mine;
-                    const int slab0 = a.cand_slab[c];
-                    const int inst = slab0 / g.R;
-                    r0 = slab0 - inst * g.R;
-                    n = a.cand_n[c];
-                    slab_base = inst * g.R;
-                    z0 = grid_z0(g, inst);
-                    const int32_t* ch = a.cand_hits + (size_t)c * kCandMax;
-                    // seed from hits 0, n/2, n-1
-                    const int i1 = n >> 1, i2 = n - 1;
-                    hsn = ch[0];
-                    const float2 h0 = a.hit_yz[hsn], h1 = a.hit_yz[ch[i1]], h2 = a.hit_yz[ch[i2]];  // (y, z)
-                    rb = a.row_offsets[slab_base + r0];
-                    // The state carries y and z relative to the first candidate hit.  The model is translation
-                    // invariant in y and z, so this is exact; it keeps the fp32 rounding of the two coordinates
-                    // (ulp(20 cm), ulp(250 cm)) out of q/pt and sinPhi, whose sensitivity to position noise is
-                    // ~50/cm on 10-row tracklets.
-                    yref = h0.x;
-                    zref = h0.y;
-                    if (kf_seed(st, s_rowx[r0], 0.0f, 0.0f, s_rowx[r0 + i1], h1.x - yref, s_rowx[r0 + i2], h2.x - yref,
-                                h2.y - zref, g.cB, g.max_s, g.p0)) {
-                        mode = kCand;
-                        i = 0;
-                        r = rn = r0;
-                        chi2 = 0.0f;
-                        nhits = 0;
+                    const float4* ts = a.tl_state + c;
+                    const float4 t5 = ts[5 * cs];
+                    const int n = __float_as_int(t5.w);
+                    if (n > 0) {  // n == 0: the fit of the candidate's own hits failed, nothing to follow
+                        const float4 t0 = ts[0], t1 = ts[cs], t2 = ts[2 * cs], t3 = ts[3 * cs], t4 = ts[4 * cs];
+                        const int slab0 = a.cand_slab[c];
+                        const int inst = slab0 / g.R;
+                        r0 = slab0 - inst * g.R;
+                        slab_base = inst * g.R;
+                        z0 = grid_z0(g, inst);
+                        st.y = t0.x; st.z = t0.y; st.s = t0.z; st.t = t0.w;
+                        st.k = t1.x; st.c00 = t1.y; st.c10 = t1.z; st.c11 = t1.w;
+                        st.c20 = t2.x; st.c21 = t2.y; st.c22 = t2.z; st.c30 = t2.w;
+                        st.c31 = t3.x; st.c32 = t3.y; st.c33 = t3.z; st.c40 = t3.w;
+                        st.c41 = t4.x; st.c42 = t4.y; st.c43 = t4.z; st.c44 = t4.w;
+                        yref = t5.x;
+                        zref = t5.y;
+                        chi2 = t5.z;
+                        nhits = n;
                         gap = 0;
                         first_row = r0;
-                        last_row = r0;
-                    } else {  // no tracklet: an all-zero record
-                        nhits = 0;
-                        chi2 = yref = zref = 0.0f;
-                        first_row = last_row = 0;
-                        zero_report(s_rep);
-                        mode = kDone;
+                        r = last_row = r0 + n - 1;
+                        mode = r + 1 < g.R ? kUp : kBack;
+                        rn = mode == kUp ? r + 1 : r0;
+                        tabA_ok = hitA_ok = tabB_ok = false;
                     }
                 }
                 wn = min(we, wn + __popc(idle));
@@ -201,130 +361,162 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             act = __ballot_sync(full, mode < kDone);
             if (act == 0u && exhausted) break;
         }
-        if (mode < kDone) {
-            // ---- one pad row: transport to row rn (offset rb), attach a hit, decide where to go next ----
-            bool alive = true;
-            float2 hc = make_float2(0.0f, 0.0f);
-            if (mode == kCand) hc = a.hit_yz[hsn];  // issued before the transport arithmetic
-            if (rn != r) {
-                if (kf_transport(st, s_rowx[rn] - s_rowx[r], g.cB, g.max_s)) {
-                    if (kCount) n_tr++;
-                    r = rn;
-                } else {
-                    alive = false;
-                    if (mode == kUp) {
-                        mode = kBack;
-                    } else if (mode == kDown) {
-                        mode = kDone;
-                    } else {  // inside the candidate's own hits, or the back transport: no tracklet
-                        nhits = 0;
-                        chi2 = yref = zref = 0.0f;
-                        first_row = last_row = 0;
-                        zero_report(s_rep);
-                        mode = kDone;
+        if (mode < kDone && (mode == kBack || hitA_ok)) {
+            // ---- one pad row: transport to row rn, attach a hit, decide where to go next.  Written as one
+            // straight path with flags: the lanes of a warp differ in phase, and every branch taken by a few
+            // lanes costs the whole warp its instructions.
+            const bool is_back = mode == kBack;
+            const bool t_ok = kf_transport(st, s_rowx[rn] - s_rowx[r], g.cB, g.max_s);
+            if (kCount && t_ok) n_tr++;
+            r = t_ok ? rn : r;
+            const float yp = st.y + yref, zp = st.z + zref;
+            const bool inside = fabsf(yp) <= fmaf(s_rowx[r], g.tan_half, g.edge_margin);
+            const bool search = t_ok && !is_back && inside;
+            int li = -1;
+            if (search) {
+                // gate: 4 sigma of the predicted residual, capped (sigma > 0: tpc_tracker_create)
+                const float wy = fminf(g.wmax, g.gate * sqrt_fast(st.c00 + g.sy2));
+                const float wz = fminf(g.wmax, g.gate * sqrt_fast(st.c11 + g.sz2));
+                const Window w = window_cells(g, s_rowy[r], z0, yp, zp, wy + kCellMargin, wz + kCellMargin);
+                // are the exact window's cells covered by the speculated ones?
+                const int sy0 = (int)(cellsA & 0xffu), sy1 = (int)((cellsA >> 8) & 0xffu);
+                const int sz0 = (int)((cellsA >> 16) & 0x7fffu);
+                bool two = (cellsA >> 31) != 0u;
+                const bool spec = cellsA != kNoCells && sy0 <= w.ys0 && w.ys1 <= sy1 && sz0 <= w.zb0 &&
+                                  w.zb1 <= sz0 + (int)two;
+                unsigned tab0 = tabA0, tab1 = tabA1;
+                const unsigned urb = (unsigned)rbA;
+                const unsigned tb0 = (unsigned)(slab_base + r) * (unsigned)g.nzp;
+                if (!spec) {  // direct loads of the exact window's cell-table entries
+                    const unsigned ia = tb0 + (unsigned)(w.zb0 * g.ny), ib = tb0 + (unsigned)(w.zb1 * g.ny);
+                    two = w.zb1 > w.zb0;
+                    const unsigned t00 = a.bin_start[ia + w.ys0], t01 = a.bin_start[ia + w.ys1];
+                    unsigned t10 = 0u, t11 = 0u;
+                    if (two) {
+                        t10 = a.bin_start[ib + w.ys0];
+                        t11 = a.bin_start[ib + w.ys1];
                     }
+                    tab0 = t00 | (t01 << 16);
+                    tab1 = t10 | (t11 << 16);
                 }
-            }
-            if (alive && mode == kBack) {
-                // phase B starts: the reported state is the back-transported one until a hit is attached
-                mode = r0 > 0 ? kDown : kDone;
-                gap = 0;
-                store_report(s_rep, st);
-                alive = false;
-            }
-            if (alive) {
-                float ym = hc.x, zm = hc.y;
-                int li = hsn - rb;  // position of the hit to attach in the sorted row
-                bool stop = false;
-                if (mode != kCand) {
-                    const float yp = st.y + yref, zp = st.z + zref;
-                    if (fabsf(yp) > fmaf(s_rowx[r], g.tan_half, g.edge_margin)) {
-                        stop = true;
-                        alive = false;
-                    } else {
-                        // gate: 4 sigma of the predicted residual, capped (sigma > 0: tpc_tracker_create)
-                        const float wy = fminf(g.wmax, g.gate * sqrt_fast(st.c00 + g.sy2));
-                        const float wz = fminf(g.wmax, g.gate * sqrt_fast(st.c11 + g.sz2));
-                        // The cells visited are a superset of the rounded fp32 gate test (margin m, monotone bins).
-                        const float m = 1e-3f;
-                        const float2 gy = s_rowy[r];
-                        const int zb0 = zbin(zp - wz - m, z0, g.inv_cz, g.nz), zb1 = zbin(zp + wz + m, z0, g.inv_cz, g.nz);
-                        const int ys0 = ybin(yp - wy - m, gy.x, gy.y, g.ny), ys1 = ybin(yp + wy + m, gy.x, gy.y, g.ny) + 1;
-                        // one index per table entry (32-bit arithmetic, one wide multiply-add per address)
-                        const unsigned tb0 = (unsigned)(slab_base + r) * (unsigned)g.nzp;
-                        const unsigned ia = tb0 + (unsigned)(zb0 * g.ny), ib = tb0 + (unsigned)(zb1 * g.ny);
-                        const int ja0 = a.bin_start[ia + ys0], ja1 = a.bin_start[ia + ys1];
-                        int jb0 = 0, jb1 = 0;
-                        if (zb1 > zb0) {
-                            jb0 = a.bin_start[ib + ys0];
-                            jb1 = a.bin_start[ib + ys1];
-                        }
-                        const int na = ja1 - ja0, nt = na + (jb1 - jb0);
-                        if (kCount) {
-                            n_se++;
-                            n_ex += nt;
-                        }
-                        // The two ranges form one sequence k = 0..nt-1.  Its first two hits are examined in line
-                        // (most searches see one or two); the loop below takes the rest one by one.
-                        const int d = jb0 - na;  // position of sequence element k >= na is k + d
-                        const int j0 = na > 0 ? ja0 : jb0;
-                        const int j1 = na > 1 ? ja0 + 1 : 1 + d;
-                        const unsigned urb = (unsigned)rb;
-                        const float2 h0 = a.hit_yz[urb + (unsigned)(nt > 0 ? j0 : 0)];
-                        const float2 h1 = a.hit_yz[urb + (unsigned)(nt > 1 ? j1 : 0)];
-                        PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f};
-                        pick_consider(b, a.hit_idx, urb, j0, nt > 0, h0, yp, zp, wy, wz);
-                        pick_consider(b, a.hit_idx, urb, j1, nt > 1, h1, yp, zp, wy, wz);
-                        for (int k = 2; k < nt; k++) {
-                            const int j = k < na ? ja0 + k : k + d;
+                const HitSeq q = hit_seq(tab0, tab1, two);
+                if (kCount) {
+                    n_se++;
+                    n_ex += q.nt;
+                }
+                // The window's hits form one sequence k = 0..nt-1, element k at sorted position seq_pos(k).  The
+                // first kSpecHits come from the speculative copies in shared memory, the rest (rare) one by one.
+                PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f};
+                int k0 = 0;
+                if (spec) {
+                    cp_async_wait_all();
+#pragma unroll
+                    for (int k = 0; k < kSpecHits; k++) {
+                        const int j = k < q.na ? q.ja0 + k : k + q.d;
+                        pick_consider(b, a.hit_idx, urb, j, k < q.nt, s_hit[k][threadIdx.x], yp, zp, wy, wz);
+                    }
+                    k0 = kSpecHits;
+                }
+                for (int k = k0; k < q.nt; k++) {
+                    const int j = k < q.na ? q.ja0 + k : k + q.d;
+                    pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
+                }
+                // z bins in between exist only when the cells are narrower than the gate (non-default
+                // grid_cell_z); such windows are never speculated
+                if (!spec)
+                    for (int zb = w.zb0 + 1; zb < w.zb1; zb++) {
+                        const unsigned im = tb0 + (unsigned)(zb * g.ny);
+                        const int jm0 = a.bin_start[im + w.ys0], jm1 = a.bin_start[im + w.ys1];
+                        if (kCount) n_ex += jm1 - jm0;
+                        for (int j = jm0; j < jm1; j++)
                             pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
-                        }
-                        // z bins in between exist only when the cells are narrower than the gate (non-default grid_cell_z)
-                        for (int zb = zb0 + 1; zb < zb1; zb++) {
-                            const unsigned im = tb0 + (unsigned)(zb * g.ny);
-                            const int jm0 = a.bin_start[im + ys0], jm1 = a.bin_start[im + ys1];
-                            if (kCount) n_ex += jm1 - jm0;
-                            for (int j = jm0; j < jm1; j++)
-                                pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
-                        }
-                        ym = b.y;
-                        zm = b.z;
-                        li = b.j;
                     }
-                }
-                if (alive) {
-                    const unsigned ih = (unsigned)c * (unsigned)g.RP + (unsigned)r;
-                    __stcs(&a.tl_rowhit[ih], (uint16_t)li);  // li = -1 stores kNoHit
-                    if (li >= 0) {
-                        chi2 += kf_update(st, ym - yref, zm - zref, g.sy2, g.sz2);
-                        if (kCount) n_up++;
-                        nhits++;
-                        gap = 0;
-                        if (mode == kDown) {
-                            first_row = r;
-                            store_report(s_rep, st);
-                        } else {
-                            last_row = r;
-                        }
-                    } else if (++gap > g.max_gap) {
-                        stop = true;
-                    }
-                }
-                // where the next iteration goes
-                if (mode == kCand) {
-                    if (++i == n) mode = kUp;
-                }
-                if (mode == kUp) {
-                    if (stop || r + 1 >= g.R) mode = kBack;
-                } else if (mode == kDown) {
-                    if (stop || r == 0) mode = kDone;
+                li = b.j;
+                __stcs(&a.tl_rowhit[(unsigned)c * (unsigned)g.RP + (unsigned)r], (uint16_t)li);  // -1 = kNoHit
+                if (li >= 0) {
+                    chi2 += kf_update(st, b.y - yref, b.z - zref, g.sy2, g.sz2);
+                    if (kCount) n_up++;
                 }
             }
-            // ---- set up the next step: its row, the row's offset, the candidate's next own hit ----
-            if (mode < kDone) {
-                rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : (mode == kCand ? r0 + i : r + 1));
-                rb = a.row_offsets[slab_base + rn];
-                if (mode == kCand) hsn = a.cand_hits[(unsigned)c * (unsigned)kCandMax + (unsigned)i];
+            // bookkeeping of the step, as selects
+            const bool hit = li >= 0;
+            const bool down = mode == kDown;
+            nhits += hit ? 1 : 0;
+            gap = hit ? 0 : gap + (search ? 1 : 0);
+            first_row = (hit && down) ? r : first_row;
+            last_row = (hit && !down) ? r : last_row;
+            if ((hit && down) || (is_back && t_ok)) store_report(s_rep, st);  // reported state: see kDown / kBack
+            const bool stop = !t_ok || !inside || gap > g.max_gap;
+            int next;
+            if (is_back) {
+                next = (t_ok && r0 > 0) ? kDown : kDone;
+                gap = 0;
+                if (!t_ok) {  // the back transport failed: no tracklet, an all-zero record
+                    nhits = 0;
+                    chi2 = yref = zref = 0.0f;
+                    first_row = last_row = 0;
+#pragma unroll
+                    for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                }
+            } else if (down) {
+                next = (stop || r == 0) ? kDone : kDown;
+            } else {
+                next = (stop || r + 1 >= g.R) ? kBack : kUp;
+            }
+            const bool flush = next != mode;
+            mode = next;
+            tabB_ok = tabB_ok && !flush;
+            tabA_ok = hitA_ok = false;  // slot A is consumed (or stale)
+            rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : r + 1);
+        }
+        // ---- speculation pipeline: advance and issue (no load issued here is consumed in this iteration) ----
+        if (mode == kUp || mode == kDown) {
+            if (!tabA_ok && tabB_ok) {  // slot B (issued in an earlier iteration) becomes slot A
+                tabA0 = tB00 | (tB01 << 16);
+                tabA1 = tB10 | (tB11 << 16);
+                cellsA = cellsB;
+                rbA = rbB;
+                tabA_ok = true;
+                tabB_ok = false;
+            }
+            if (tabA_ok && !hitA_ok) {  // first hits of the speculated window of row rn -> shared memory
+                if (cellsA != kNoCells) {
+                    const HitSeq q = hit_seq(tabA0, tabA1, (cellsA >> 31) != 0u);
+                    cp_async_wait_all();  // copies of a window that was not used must not land after the new ones
+#pragma unroll
+                    for (int k = 0; k < kSpecHits; k++)
+                        if (k < q.nt)
+                            cp_async8(&s_hit[k][threadIdx.x],
+                                      &a.hit_yz[(unsigned)rbA + (unsigned)(k < q.na ? q.ja0 + k : k + q.d)]);
+                    cp_async_commit();
+                }
+                hitA_ok = true;
+            }
+            const int tr = tabA_ok ? (mode == kUp ? rn + 1 : rn - 1) : rn;  // the next row not yet in slot A
+            if (!tabB_ok && tr >= 0 && tr < g.R) {
+                // window around the position extrapolated linearly from the current state, widened
+                const float ic = rsqrtf((1.0f - st.s) * (1.0f + st.s));
+                const float dxk = s_rowx[tr] - s_rowx[r];
+                const float yq = fmaf(dxk, st.s * ic, st.y + yref), zq = fmaf(dxk, st.t * ic, st.z + zref);
+                const float wy = fminf(g.wmax, g.gate * sqrt_fast(st.c00 + g.sy2)) + kSpecMargin;
+                const float wz = fminf(g.wmax, g.gate * sqrt_fast(st.c11 + g.sz2)) + kSpecMargin;
+                const Window w = window_cells(g, s_rowy[tr], z0, yq, zq, wy, wz);
+                const unsigned tb0 = (unsigned)(slab_base + tr) * (unsigned)g.nzp;
+                rbB = a.row_offsets[slab_base + tr];
+                if (w.zb1 - w.zb0 <= 1) {
+                    const unsigned ia = tb0 + (unsigned)(w.zb0 * g.ny);
+                    tB00 = a.bin_start[ia + w.ys0];
+                    tB01 = a.bin_start[ia + w.ys1];
+                    if (w.zb1 > w.zb0) {
+                        tB10 = a.bin_start[ia + g.ny + w.ys0];
+                        tB11 = a.bin_start[ia + g.ny + w.ys1];
+                    }
+                    cellsB = (unsigned)w.ys0 | ((unsigned)w.ys1 << 8) | ((unsigned)w.zb0 << 16) |
+                             (w.zb1 > w.zb0 ? 0x80000000u : 0u);
+                } else {
+                    cellsB = kNoCells;
+                }
+                tabB_ok = true;
             }
         }
     }
@@ -332,8 +524,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
         unsigned v[4] = {n_tr, n_up, n_ex, n_se};
 #pragma unroll
         for (int q = 0; q < 4; q++) {
-#pragma unroll
-            for (int d = 16; d > 0; d >>= 1) v[q] += __shfl_xor_sync(full, v[q], d);
+            v[q] = __reduce_add_sync(full, v[q]);
             if (lane == 0 && v[q]) atomicAdd((unsigned long long*)&a.counts[6 + q], (unsigned long long)v[q]);
         }
     }
@@ -341,18 +532,22 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
 
 int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, bool count_work, cudaStream_t s) {
     if (p.n_clusters == 0) return 0;
+    FollowArgs a{p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.cand_hits, w.cand_n,    w.cand_slab, w.counts, w.Cmax,
+                 w.tl_state,    w.tl_par, w.tl_cov,  w.tl_chi2,   w.tl_nhits,  w.tl_rows,  w.tl_rowhit, w.tl_sel};
+    // the candidate count lives on the device: both grids are sized by its bound and bounded by it inside
+    const int fit_grid = div_up(w.Cmax, kFitThreads);
     // persistent grid: every SM holds kFollowCtasPerSm CTAs, capped by the candidate bound
-    int64_t want = div_up(w.Cmax, kFollowThreads);
+    const int64_t want = div_up(w.Cmax, kFollowThreads);
     int grid = (int)(want < (int64_t)n_sm * kFollowCtasPerSm ? want : (int64_t)n_sm * kFollowCtasPerSm);
     if (grid < 1) grid = 1;
-    FollowArgs a{p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.cand_hits, w.cand_n, w.cand_slab,
-                 w.counts,   w.Cmax,        w.tl_par, w.tl_cov,  w.tl_chi2,   w.tl_nhits,  w.tl_rows, w.tl_rowhit,
-                 w.tl_sel};
-    if (count_work)
+    if (count_work) {
+        fit_candidates_kernel<true><<<fit_grid, kFitThreads, 0, s>>>(g, a);
         follow_kernel<true><<<grid, kFollowThreads, 0, s>>>(g, a);
-    else
+    } else {
+        fit_candidates_kernel<false><<<fit_grid, kFitThreads, 0, s>>>(g, a);
         follow_kernel<false><<<grid, kFollowThreads, 0, s>>>(g, a);
-    return 1;
+    }
+    return 2;
 }
 
 }  // namespace tpc

@@ -57,6 +57,7 @@ struct Workspace {
     int32_t* cand_hits;   // [Cmax][kCandMax]
     int32_t* cand_n;      // [Cmax]
     int32_t* cand_slab;   // [Cmax] instance * R + row of the start hit
+    float4* tl_state;     // [6][Cmax] S5: state after the candidate's own hits (fit kernel -> follow kernel)
     float* tl_par;        // [Cmax][5]
     float* tl_cov;        // [Cmax][15]
     float* tl_chi2;       // [Cmax]

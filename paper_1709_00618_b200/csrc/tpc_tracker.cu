@@ -46,11 +46,12 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     g.sel_words = (R + 31) / 32;
     g.sel_stride = (g.sel_words + 2 + 3) & ~3;
     // per-row 2-D grid: ny strips across the row, z bins of cz (performance only, no result depends on either).
-    // Default cz = 6.25 cm > 2 * max(kf_win_max, nf_win_z) + margins, so a search window touches at most 2 z bins.
+    // Default cz = 6.75 cm > 2 * (kf_win_max + the follower's speculation margin), so a search window touches at most
+    // 2 z bins.
     int ny = dflt(p.grid_cells_y, 16);
     if (ny < 1) ny = 1;
     if (ny > 64) ny = 64;
-    float cz = dflt(p.grid_cell_z, 6.25f);
+    float cz = dflt(p.grid_cell_z, 6.75f);
     int nz = (int)std::ceil(((double)geom->z_hi - (double)geom->z_lo) / cz);
     if (nz < 1) nz = 1;
     if ((int64_t)nz * ny > kMaxCells) {  // too fine: widen the z bins until the row grid fits
@@ -155,6 +156,7 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.cand_hits = c.take<int32_t>(cmax * kCandMax);
     v.cand_n = c.take<int32_t>(cmax);
     v.cand_slab = c.take<int32_t>(cmax);
+    v.tl_state = c.take<float4>(cmax * 6);
     v.tl_par = c.take<float>(cmax * 5);
     v.tl_cov = c.take<float>(cmax * 15);
     v.tl_chi2 = c.take<float>(cmax);
