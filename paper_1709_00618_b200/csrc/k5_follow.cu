@@ -17,14 +17,18 @@
 //    acceleration structure only) -- otherwise the step falls back to direct loads.
 #include "kf_math.cuh"
 
+#ifndef TPC_FOLLOW_SPEC
+#define TPC_FOLLOW_SPEC 0
+#endif
 #ifndef TPC_FOLLOW_CTAS
-#define TPC_FOLLOW_CTAS 5
+#define TPC_FOLLOW_CTAS (TPC_FOLLOW_SPEC ? 5 : 7)
 #endif
 #ifndef TPC_FOLLOW_RELOAD
 #define TPC_FOLLOW_RELOAD 4
 #endif
 namespace tpc {
 
+constexpr bool kFollowSpec = TPC_FOLLOW_SPEC != 0;  // speculative load pipeline on/off (performance only)
 constexpr int kFollowThreads = 128;
 constexpr int kFollowCtasPerSm = TPC_FOLLOW_CTAS;
 constexpr int kFollowChunk = 64;                  // candidates a warp takes from the queue at a time
@@ -255,7 +259,7 @@ __device__ __forceinline__ HitSeq hit_seq(unsigned tab0, unsigned tab1, bool two
 
 // kCount: also accumulate the work counters counts[6..9] (roofline arithmetic; tpc_set_work_counters).  They are a
 // property of the input, so the timed runs use the variant without them.
-template <bool kCount>
+template <bool kCount, bool kSpec>
 __global__ void __launch_bounds__(kFollowThreads, kFollowCtasPerSm)
 follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowArgs a) {
     __shared__ float s_rowx[kMaxRows + 1];
@@ -354,6 +358,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         mode = r + 1 < g.R ? kUp : kBack;
                         rn = mode == kUp ? r + 1 : r0;
                         tabA_ok = hitA_ok = tabB_ok = false;
+                        if (!kSpec) rbA = a.row_offsets[slab_base + rn];
                     }
                 }
                 wn = min(we, wn + __popc(idle));
@@ -361,7 +366,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             act = __ballot_sync(full, mode < kDone);
             if (act == 0u && exhausted) break;
         }
-        if (mode < kDone && (mode == kBack || hitA_ok)) {
+        if (mode < kDone && (!kSpec || mode == kBack || hitA_ok)) {
             // ---- one pad row: transport to row rn, attach a hit, decide where to go next.  Written as one
             // straight path with flags: the lanes of a warp differ in phase, and every branch taken by a few
             // lanes costs the whole warp its instructions.
@@ -382,7 +387,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 const int sy0 = (int)(cellsA & 0xffu), sy1 = (int)((cellsA >> 8) & 0xffu);
                 const int sz0 = (int)((cellsA >> 16) & 0x7fffu);
                 bool two = (cellsA >> 31) != 0u;
-                const bool spec = cellsA != kNoCells && sy0 <= w.ys0 && w.ys1 <= sy1 && sz0 <= w.zb0 &&
+                const bool spec = kSpec && cellsA != kNoCells && sy0 <= w.ys0 && w.ys1 <= sy1 && sz0 <= w.zb0 &&
                                   w.zb1 <= sz0 + (int)two;
                 unsigned tab0 = tabA0, tab1 = tabA1;
                 const unsigned urb = (unsigned)rbA;
@@ -407,8 +412,15 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 // The window's hits form one sequence k = 0..nt-1, element k at sorted position seq_pos(k).  The
                 // first kSpecHits come from the speculative copies in shared memory, the rest (rare) one by one.
                 PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f};
-                int k0 = 0;
-                if (spec) {
+                int k0 = 2;
+                if (!spec) {  // direct loads of the first two hits
+                    float2 h0 = make_float2(0.0f, 0.0f), h1 = h0;
+                    const int j0 = q.na > 0 ? q.ja0 : q.d, j1 = q.na > 1 ? q.ja0 + 1 : 1 + q.d;
+                    if (q.nt > 0) h0 = a.hit_yz[urb + (unsigned)j0];
+                    if (q.nt > 1) h1 = a.hit_yz[urb + (unsigned)j1];
+                    pick_consider(b, a.hit_idx, urb, j0, q.nt > 0, h0, yp, zp, wy, wz);
+                    pick_consider(b, a.hit_idx, urb, j1, q.nt > 1, h1, yp, zp, wy, wz);
+                } else {
                     cp_async_wait_all();
 #pragma unroll
                     for (int k = 0; k < kSpecHits; k++) {
@@ -469,8 +481,10 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             tabA_ok = hitA_ok = false;  // slot A is consumed (or stale)
             rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : r + 1);
         }
-        // ---- speculation pipeline: advance and issue (no load issued here is consumed in this iteration) ----
-        if (mode == kUp || mode == kDown) {
+        if (!kSpec) {
+            if (mode < kDone) rbA = a.row_offsets[slab_base + rn];  // offset of the coming row, one step ahead
+        } else if (mode == kUp || mode == kDown) {
+            // ---- speculation pipeline: advance and issue (no load issued here is consumed in this iteration) ----
             if (!tabA_ok && tabB_ok) {  // slot B (issued in an earlier iteration) becomes slot A
                 tabA0 = tB00 | (tB01 << 16);
                 tabA1 = tB10 | (tB11 << 16);
@@ -538,14 +552,15 @@ int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_
     const int fit_grid = div_up(w.Cmax, kFitThreads);
     // persistent grid: every SM holds kFollowCtasPerSm CTAs, capped by the candidate bound
     const int64_t want = div_up(w.Cmax, kFollowThreads);
-    int grid = (int)(want < (int64_t)n_sm * kFollowCtasPerSm ? want : (int64_t)n_sm * kFollowCtasPerSm);
+    const int per_sm = kFollowCtasPerSm;
+    int grid = (int)(want < (int64_t)n_sm * per_sm ? want : (int64_t)n_sm * per_sm);
     if (grid < 1) grid = 1;
     if (count_work) {
         fit_candidates_kernel<true><<<fit_grid, kFitThreads, 0, s>>>(g, a);
-        follow_kernel<true><<<grid, kFollowThreads, 0, s>>>(g, a);
+        follow_kernel<true, kFollowSpec><<<grid, kFollowThreads, 0, s>>>(g, a);
     } else {
         fit_candidates_kernel<false><<<fit_grid, kFitThreads, 0, s>>>(g, a);
-        follow_kernel<false><<<grid, kFollowThreads, 0, s>>>(g, a);
+        follow_kernel<false, kFollowSpec><<<grid, kFollowThreads, 0, s>>>(g, a);
     }
     return 2;
 }
