@@ -56,8 +56,8 @@ typedef struct {
     float kf_max_sinphi;       /* S5 |sinPhi| limit: 0.95 */
     float kf_edge_margin;      /* S5 stop when |y| exceeds the row half-width by this [cm]: 2 */
     int32_t sel_min_hits;      /* S6 minimum hits kept by a final track: 10 */
-    float grid_cell_z;         /* S1 z-bin width of the per-row grid [cm]: 6.25.  Performance only: no result depends on it */
-    int32_t grid_cells_y;      /* S1 strips across a pad row (1..64): 16.  Performance only */
+    float grid_cell_z;         /* S1 z-bin width of the per-row grid [cm]: 6.75.  Performance only: no result depends on it */
+    int32_t grid_cells_y;      /* S1 strips across a pad row (1..64): 12.  Performance only */
 } tpc_params_t;
 
 typedef struct {

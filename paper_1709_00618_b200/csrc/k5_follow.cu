@@ -40,6 +40,10 @@ constexpr int kFitThreads = 128;
 #ifndef TPC_SPEC_MARGIN
 #define TPC_SPEC_MARGIN 0.25f
 #endif
+#ifndef TPC_DIRECT_HITS
+#define TPC_DIRECT_HITS 3
+#endif
+constexpr int kDirectHits = TPC_DIRECT_HITS;      // hits of a window examined in line (the rest in a loop)
 constexpr int kSpecHits = TPC_SPEC_HITS;          // hits of the coming window fetched ahead
 constexpr float kSpecMargin = TPC_SPEC_MARGIN;  // [cm] widening of the speculated window (performance only)
 constexpr float kCellMargin = 1e-3f;  // [cm] the visited cells are a superset of the rounded fp32 gate test
@@ -412,14 +416,19 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 // The window's hits form one sequence k = 0..nt-1, element k at sorted position seq_pos(k).  The
                 // first kSpecHits come from the speculative copies in shared memory, the rest (rare) one by one.
                 PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f};
-                int k0 = 2;
-                if (!spec) {  // direct loads of the first two hits
-                    float2 h0 = make_float2(0.0f, 0.0f), h1 = h0;
-                    const int j0 = q.na > 0 ? q.ja0 : q.d, j1 = q.na > 1 ? q.ja0 + 1 : 1 + q.d;
-                    if (q.nt > 0) h0 = a.hit_yz[urb + (unsigned)j0];
-                    if (q.nt > 1) h1 = a.hit_yz[urb + (unsigned)j1];
-                    pick_consider(b, a.hit_idx, urb, j0, q.nt > 0, h0, yp, zp, wy, wz);
-                    pick_consider(b, a.hit_idx, urb, j1, q.nt > 1, h1, yp, zp, wy, wz);
+                int k0 = kDirectHits;
+                if (!spec) {  // direct loads of the first hits, all in flight together
+                    float2 h[kDirectHits];
+                    int j[kDirectHits];
+#pragma unroll
+                    for (int k = 0; k < kDirectHits; k++) {
+                        j[k] = k < q.na ? q.ja0 + k : k + q.d;
+                        h[k] = make_float2(0.0f, 0.0f);
+                        if (k < q.nt) h[k] = a.hit_yz[urb + (unsigned)j[k]];
+                    }
+#pragma unroll
+                    for (int k = 0; k < kDirectHits; k++)
+                        pick_consider(b, a.hit_idx, urb, j[k], k < q.nt, h[k], yp, zp, wy, wz);
                 } else {
                     cp_async_wait_all();
 #pragma unroll

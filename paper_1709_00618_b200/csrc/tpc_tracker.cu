@@ -48,7 +48,7 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     // per-row 2-D grid: ny strips across the row, z bins of cz (performance only, no result depends on either).
     // Default cz = 6.75 cm > 2 * (kf_win_max + the follower's speculation margin), so a search window touches at most
     // 2 z bins.
-    int ny = dflt(p.grid_cells_y, 16);
+    int ny = dflt(p.grid_cells_y, 12);
     if (ny < 1) ny = 1;
     if (ny > 64) ny = 64;
     float cz = dflt(p.grid_cell_z, 6.75f);
