@@ -11,7 +11,7 @@ constexpr int kBinThreads = 128;
 __global__ void __launch_bounds__(kBinThreads)
 bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clusters,
                 const int32_t* __restrict__ row_offsets, float2* __restrict__ hit_yz, uint16_t* __restrict__ hit_idx,
-                uint16_t* __restrict__ bin_start, int64_t* __restrict__ counts) {
+                uint16_t* __restrict__ hit_pos, uint16_t* __restrict__ bin_start, int64_t* __restrict__ counts) {
     extern __shared__ __align__(16) uint32_t sm_hist[];  // [nzp] counts, then exclusive starts (cursors in pass 2)
     __shared__ uint32_t sm_warp[kBinThreads / 32];
     const int slab = blockIdx.x;
@@ -87,6 +87,7 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
             const uint32_t pos = atomicAdd(&sm_hist[key[k]], 1u);
             hit_yz[base + pos] = yz[k];
             hit_idx[base + pos] = (uint16_t)(threadIdx.x + k * kBinThreads);
+            hit_pos[base + threadIdx.x + k * kBinThreads] = (uint16_t)pos;  // inverse permutation, coalesced
         }
     }
     for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {  // long rows: from L1/L2 this time
@@ -94,6 +95,7 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
         const uint32_t pos = atomicAdd(&sm_hist[zbin(c.z, z0, g.inv_cz, g.nz) * g.ny + ybin(c.y, y0, inv_sy, g.ny)], 1u);
         hit_yz[base + pos] = make_float2(c.y, c.z);
         hit_idx[base + pos] = (uint16_t)i;
+        hit_pos[base + i] = (uint16_t)pos;
     }
 }
 
@@ -106,7 +108,7 @@ int launch_bin_rows(const DevGeom& g, const Workspace& w, const Problem& p, cuda
         cudaFuncSetAttribute(bin_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    bin_rows_kernel<<<slabs, kBinThreads, smem, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
+    bin_rows_kernel<<<slabs, kBinThreads, smem, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx, w.hit_pos, w.bin_start,
                                                      w.counts);
     return 1;
 }

@@ -100,100 +100,56 @@ scan_int2_kernel(int2* __restrict__ part, const int64_t* __restrict__ m_dev, int
     }
 }
 
-// S4 pass 2: ranked write of start hits and candidates.  Links and flags live in sorted space, but start hits and
-// candidates are numbered in ascending INPUT index of the start hit, so the rank inside the slab is
-// taken over the input positions: one bit per input position in shared memory, popcount prefix per word.
-constexpr int kChainMaxBits = 8192;  // rows up to this length use the bitmaps; longer rows count by brute force
-constexpr int kChainWords = kChainMaxBits / 32;
-
+// S4 pass 2: ranked write of the start hits and of the candidates' start positions.  Links and flags live in sorted
+// space, but start hits and candidates are numbered in ascending INPUT index of the start hit, so the
+// CTA walks its row in input order (through S1's inverse permutation hit_pos) and ranks with ballot/popc prefixes.
+// The candidate's hit list itself (the first <= 10 chain hits) is read off the links by the S5 fit kernel, one thread
+// per candidate, where the walk runs at full lane occupancy.
 __global__ void __launch_bounds__(kChainThreads)
-chain_write_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
-                   const uint16_t* __restrict__ hit_idx, const int32_t* __restrict__ up,
+chain_write_kernel(const int32_t* __restrict__ row_offsets, const uint16_t* __restrict__ hit_pos,
                    const uint8_t* __restrict__ flags, const int2* __restrict__ slab_part,
-                   int32_t* __restrict__ start_hits, int64_t start_cap, int32_t* __restrict__ cand_hits,
-                   int32_t* __restrict__ cand_n, int32_t* __restrict__ cand_slab, int64_t cand_cap,
-                   int32_t* __restrict__ usr_cand_hits, int32_t* __restrict__ usr_cand_n, int64_t usr_cand_cap) {
-    __shared__ uint32_t s_bits[2][kChainWords];  // [0] start hits, [1] candidates, by input position
-    __shared__ uint16_t s_pre[2][kChainWords];   // set bits in the words before
+                   int32_t* __restrict__ start_hits, int64_t start_cap, int32_t* __restrict__ cand_start,
+                   int32_t* __restrict__ cand_slab, int64_t cand_cap) {
+    __shared__ int2 s_warp[kChainThreads / 32];
     const int slab = blockIdx.x;
-    const int base = row_offsets[slab], n = min(row_offsets[slab + 1] - base, 65535);
     const int2 sb = slab_part[slab];
     if (slab_part[slab + 1].x == sb.x) return;  // no start hit in this slab
-    const bool bitmap = n <= kChainMaxBits;
-    const int words = (n + 31) >> 5;
-    if (bitmap) {
-        for (int w = threadIdx.x; w < words; w += kChainThreads) s_bits[0][w] = s_bits[1][w] = 0u;
-        __syncthreads();
-        for (int i = threadIdx.x; i < n; i += kChainThreads) {
-            const uint8_t f = flags[base + i];
-            if (f) {
-                const int li = hit_idx[base + i];
-                atomicOr(&s_bits[0][li >> 5], 1u << (li & 31));
-                if (f & 2) atomicOr(&s_bits[1][li >> 5], 1u << (li & 31));
-            }
+    const int base = row_offsets[slab], n = min(row_offsets[slab + 1] - base, 65535);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    int2 carry = sb;  // (start hits, candidates) before the current chunk
+    for (int i0 = 0; i0 < n; i0 += kChainThreads) {
+        const int i = i0 + threadIdx.x;  // input position
+        int pos = 0;
+        uint8_t f = 0;
+        if (i < n) {
+            pos = hit_pos[base + i];
+            f = flags[base + pos];
         }
+        const unsigned ms = __ballot_sync(0xffffffffu, f & 1), mc = __ballot_sync(0xffffffffu, f & 2);
+        if (lane == 0) s_warp[wid] = make_int2(__popc(ms), __popc(mc));
         __syncthreads();
-        if (threadIdx.x < 64) {  // warp 0: start hits, warp 1: candidates
-            const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
-            int carry = 0;
-            for (int w0 = 0; w0 < words; w0 += 32) {
-                const int w = w0 + lane;
-                const int v = w < words ? __popc(s_bits[q][w]) : 0;
-                int incl = v;
+        int2 off = carry, tot = carry;
 #pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const int t = __shfl_up_sync(0xffffffffu, incl, d);
-                    if (lane >= d) incl += t;
-                }
-                if (w < words) s_pre[q][w] = (uint16_t)(carry + incl - v);
-                carry += __shfl_sync(0xffffffffu, incl, 31);
-            }
+        for (int k = 0; k < kChainThreads / 32; k++) {
+            const int2 v = s_warp[k];
+            if (k < wid) { off.x += v.x; off.y += v.y; }
+            tot.x += v.x;
+            tot.y += v.y;
         }
-        __syncthreads();
-    }
-    for (int i = threadIdx.x; i < n; i += kChainThreads) {
-        const int h = base + i;
-        const uint8_t f = flags[h];
-        if (!f) continue;
-        const int li = hit_idx[h];
-        int rs, rc;  // start hits / candidates of this slab with a smaller input position
-        if (bitmap) {
-            const unsigned below = (1u << (li & 31)) - 1u;
-            rs = s_pre[0][li >> 5] + __popc(s_bits[0][li >> 5] & below);
-            rc = s_pre[1][li >> 5] + __popc(s_bits[1][li >> 5] & below);
-        } else {
-            rs = rc = 0;
-            for (int k = 0; k < n; k++) {
-                const uint8_t fk = flags[base + k];
-                if (fk && hit_idx[base + k] < li) {
-                    rs++;
-                    rc += fk >> 1;
+        carry = tot;
+        if (f) {
+            const int64_t ps = off.x + __popc(ms & lt);
+            if (start_hits && ps < start_cap) start_hits[ps] = base + i;
+            if (f & 2) {
+                const int64_t c = off.y + __popc(mc & lt);
+                if (c < cand_cap) {
+                    cand_start[c] = base + pos;
+                    cand_slab[c] = slab;
                 }
             }
         }
-        const int64_t ps = sb.x + rs;
-        if (start_hits && ps < start_cap) start_hits[ps] = base + li;
-        if (f & 2) {
-            const int64_t c = sb.y + rc;
-            int32_t hits[kCandMax];
-            int k = 0;
-            for (int x = h; x >= 0 && k < g.cand_max; x = __ldg(&up[x])) hits[k++] = x;
-            const int nh = k;
-            for (; k < kCandMax; k++) hits[k] = -1;
-            if (c < cand_cap) {
-#pragma unroll
-                for (int q = 0; q < kCandMax; q++) cand_hits[c * kCandMax + q] = hits[q];
-                cand_n[c] = nh;
-                cand_slab[c] = slab;
-            }
-            if (usr_cand_hits && c < usr_cand_cap) {  // user-facing copy: input-order global indices
-#pragma unroll
-                for (int q = 0; q < kCandMax; q++)
-                    usr_cand_hits[c * kCandMax + q] =
-                        q < nh ? row_offsets[slab + q] + (int32_t)hit_idx[hits[q]] : -1;
-            }
-            if (usr_cand_n && c < usr_cand_cap) usr_cand_n[c] = nh;
-        }
+        __syncthreads();
     }
 }
 
@@ -231,9 +187,8 @@ int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const 
     if (slabs == 0) return 0;
     chain_flags_kernel<<<slabs, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.dn, w.flags, w.slab_part);
     launch_scan_int2(w.slab_part, nullptr, 1, 0, slabs, w.counts, 0, 1, s);
-    chain_write_kernel<<<slabs, kChainThreads, 0, s>>>(g, p.row_offsets, w.hit_idx, w.up, w.flags, w.slab_part, u.start_hits,
-                                                       u.start_cap, w.cand_hits, w.cand_n, w.cand_slab, w.Cmax,
-                                                       u.cand_hits, u.cand_n, u.cand_cap);
+    chain_write_kernel<<<slabs, kChainThreads, 0, s>>>(p.row_offsets, w.hit_pos, w.flags, w.slab_part, u.start_hits,
+                                                       u.start_cap, w.cand_start, w.cand_slab, w.Cmax);
     return 3;
 }
 

@@ -55,9 +55,12 @@ struct FollowArgs {
     const float2* hit_yz;
     const uint16_t* hit_idx;
     const uint16_t* bin_start;
-    const int32_t* cand_hits;
-    const int32_t* cand_n;
+    const int32_t* up;          // cleaned up-links (sorted space)
+    const int32_t* cand_start;  // sorted global position of the candidate's start hit
     const int32_t* cand_slab;
+    int32_t* usr_cand_hits;     // optional user-facing S4 outputs (input-order global indices), NULL = skip
+    int32_t* usr_cand_n;
+    int64_t usr_cand_cap;
     int64_t* counts;
     int64_t Cmax;
     float4* tl_state;  // [6][Cmax] state after the candidate's own hits (fit kernel -> follow kernel)
@@ -95,15 +98,15 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
         const int slab0 = a.cand_slab[c];
         const int inst = slab0 / g.R;
         const int r0 = slab0 - inst * g.R;
-        const int n = a.cand_n[c];
-        // the candidate's hits: sorted global positions (5 x 8-byte loads), coordinates and row offsets
+        // S4 concatenation: the candidate's hits are the first <= cand_max hits of the chain of up-links that
+        // starts at its start hit (sorted global positions); the walk is 9 dependent 4-byte loads per thread
         int pos[kCandMax];
-        const int2* ch = reinterpret_cast<const int2*>(a.cand_hits + (size_t)c * kCandMax);
+        pos[0] = a.cand_start[c];
+        int n = 1;
 #pragma unroll
-        for (int q = 0; q < kCandMax / 2; q++) {
-            const int2 v = ch[q];
-            pos[2 * q] = v.x;
-            pos[2 * q + 1] = v.y;
+        for (int q = 1; q < kCandMax; q++) {
+            pos[q] = (pos[q - 1] >= 0 && q < g.cand_max) ? a.up[pos[q - 1]] : -1;
+            n += pos[q] >= 0 ? 1 : 0;
         }
         float2 h[kCandMax];
         int rb[kCandMax];
@@ -130,6 +133,12 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
             if (q == i1) { h1 = h[q]; x1 = x[q]; }
             if (q == i2) { h2 = h[q]; x2 = x[q]; }
         }
+        if (a.usr_cand_hits && c < a.usr_cand_cap) {  // parity/user copy: input-order global indices
+#pragma unroll
+            for (int q = 0; q < kCandMax; q++)
+                a.usr_cand_hits[(size_t)c * kCandMax + q] = q < n ? rb[q] + (int)a.hit_idx[pos[q]] : -1;
+        }
+        if (a.usr_cand_n && c < a.usr_cand_cap) a.usr_cand_n[c] = n;
         const float yref = h[0].x, zref = h[0].y;
         KfState st;
         bool ok = kf_seed(st, x[0], 0.0f, 0.0f, x1, h1.x - yref, x2, h2.x - yref, h2.y - zref, g.cB, g.max_s, g.p0);
@@ -553,10 +562,12 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
     }
 }
 
-int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, bool count_work, cudaStream_t s) {
+int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, int n_sm, bool count_work,
+                  cudaStream_t s) {
     if (p.n_clusters == 0) return 0;
-    FollowArgs a{p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start, w.cand_hits, w.cand_n,    w.cand_slab, w.counts, w.Cmax,
-                 w.tl_state,    w.tl_par, w.tl_cov,  w.tl_chi2,   w.tl_nhits,  w.tl_rows,  w.tl_rowhit, w.tl_sel};
+    FollowArgs a{p.row_offsets, w.hit_yz,  w.hit_idx,   w.bin_start, w.up,      w.cand_start, w.cand_slab,
+                 u.cand_hits,   u.cand_n,  u.cand_cap,  w.counts,    w.Cmax,    w.tl_state,   w.tl_par,
+                 w.tl_cov,      w.tl_chi2, w.tl_nhits,  w.tl_rows,   w.tl_rowhit, w.tl_sel};
     // the candidate count lives on the device: both grids are sized by its bound and bounded by it inside
     const int fit_grid = div_up(w.Cmax, kFitThreads);
     // persistent grid: every SM holds kFollowCtasPerSm CTAs, capped by the candidate bound

@@ -44,6 +44,7 @@ struct DevGeom {
 struct Workspace {
     float2* hit_yz;       // [N]  (y, z) sorted by grid cell inside every (instance,row) segment
     uint16_t* hit_idx;    // [N]  local index (position in the row segment of the INPUT) of the sorted hit
+    uint16_t* hit_pos;    // [N]  inverse of hit_idx: position in the sorted row of the hit with that local index
     uint16_t* bin_start;  // [S*R][nzp] first sorted position of every grid cell, entry ncell = row length
     // Index spaces: everything below that is indexed by hit or holds hit indices uses SORTED global positions
     // (row start + position in the sorted row); the user-facing outputs are translated back through hit_idx.
@@ -54,8 +55,7 @@ struct Workspace {
     uint32_t* claim;      // [N] S6 best claiming weight
     uint8_t* flags;       // [N] bit0 start hit, bit1 candidate
     int2* slab_part;      // [S*R + 1] (starts, candidates) per slab, then their exclusive scan
-    int32_t* cand_hits;   // [Cmax][kCandMax]
-    int32_t* cand_n;      // [Cmax]
+    int32_t* cand_start;  // [Cmax] sorted global position of the candidate's start hit (S4); the chain is walked in S5
     int32_t* cand_slab;   // [Cmax] instance * R + row of the start hit
     float4* tl_state;     // [6][Cmax] S5: state after the candidate's own hits (fit kernel -> follow kernel)
     float* tl_par;        // [Cmax][5]
@@ -113,7 +113,8 @@ void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m
 // parity/debug: a link array of the workspace (sorted space) as input-order indices; dir = row offset of the targets
 int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link, int dir,
                         int32_t* out, cudaStream_t s);
-int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, bool count_work, cudaStream_t s);
+int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, int n_sm, bool count_work,
+                  cudaStream_t s);
 
 struct SelectOut {  // mirrors the S6 part of tpc_output_t
     float *trk_params, *trk_cov, *trk_chi2, *trk_xref;

@@ -145,6 +145,7 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.counts = c.take<int64_t>(TPC_N_COUNTS);
     v.hit_yz = c.take<float2>(n);
     v.hit_idx = c.take<uint16_t>(n);
+    v.hit_pos = c.take<uint16_t>(n);
     v.bin_start = c.take<uint16_t>(slabs * g.nzp);
     v.up_raw = c.take<int32_t>(n);
     v.dn_raw = c.take<int32_t>(n);
@@ -153,8 +154,7 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.claim = c.take<uint32_t>(n);
     v.flags = c.take<uint8_t>(n);
     v.slab_part = c.take<int2>(slabs + 1);
-    v.cand_hits = c.take<int32_t>(cmax * kCandMax);
-    v.cand_n = c.take<int32_t>(cmax);
+    v.cand_start = c.take<int32_t>(cmax);
     v.cand_slab = c.take<int32_t>(cmax);
     v.tl_state = c.take<float4>(cmax * 6);
     v.tl_par = c.take<float>(cmax * 5);
@@ -250,7 +250,7 @@ extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const 
                 (out->cand_hits || out->cand_n) ? out->cand_capacity : 0};
     launches += launch_chains(g, w, p, co, s);
     if (tm) cudaEventRecord(ev[4], s);
-    launches += launch_follow(g, w, p, t->n_sm, t->count_work, s);
+    launches += launch_follow(g, w, p, co, t->n_sm, t->count_work, s);
     if (tm) cudaEventRecord(ev[5], s);
     SelectOut so{out->trk_params, out->trk_cov, out->trk_chi2, out->trk_xref, out->trk_cand_id, out->trk_nhits,
                  out->trk_sector, out->trk_hit_offset, out->trk_hits, out->trk_capacity, out->trk_hits_capacity,
