@@ -33,20 +33,23 @@ struct Best {
     int ju, jd;  // positions in the sorted rows r+1 / r-1, -1 = none
 };
 
-// Keep the minimum over (D, local index of u, local index of d); the local indices (positions in the INPUT row
-// segments) are only loaded to break exact ties of D, so the result does not depend on the sorted order.
-__device__ __forceinline__ void consider(Best& b, float D, int ju, int jd, const uint16_t* __restrict__ idx_up,
-                                         const uint16_t* __restrict__ idx_dn) {
-    bool better = b.ju < 0 || D < b.D;
-    if (!better && D == b.D) {
-        const int iu = idx_up[ju], bu = idx_up[b.ju];
-        better = iu < bu || (iu == bu && idx_dn[jd] < idx_dn[b.jd]);
-    }
-    if (better) {
-        b.D = D;
-        b.ju = ju;
-        b.jd = jd;
-    }
+// Exact tie of D between two admissible pairs (duplicated clusters only): the lower (local index of u, local index
+// of d) wins.  Local indices = positions in the INPUT row segments, so the result does not depend on the sorted order.
+__device__ __noinline__ bool tie_lower(const uint16_t* __restrict__ idx_up, const uint16_t* __restrict__ idx_dn, int ju,
+                                       int jd, int bu, int bd) {
+    const int iu = idx_up[ju], ibu = idx_up[bu];
+    return iu < ibu || (iu == ibu && idx_dn[jd] < idx_dn[bd]);
+}
+
+// Keep the minimum over (D, local index of u, local index of d).  Straight-line code: `adm` says whether the pair
+// exists and is admissible; b.D starts at +inf, so an exact tie implies a previous admissible pair.
+__device__ __forceinline__ void consider(Best& b, bool adm, float D, int ju, int jd,
+                                         const uint16_t* __restrict__ idx_up, const uint16_t* __restrict__ idx_dn) {
+    bool better = adm && D < b.D;
+    if (adm && D == b.D) better = tie_lower(idx_up, idx_dn, ju, jd, b.ju, b.jd);
+    b.D = better ? D : b.D;
+    b.ju = better ? ju : b.ju;
+    b.jd = better ? jd : b.jd;
 }
 
 // The cells a window touches in one neighbour row, as ONE sequence of nt sorted positions: the first na start at a0
@@ -92,11 +95,15 @@ __device__ __noinline__ void search_dense(const DevGeom& g, const RowView& up, c
                     const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
                     const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
                     const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
-                    if (D <= g.nf_d2max) consider(best, D, a, b, up.idx, dn.idx);
+                    consider(best, D <= g.nf_d2max, D, a, b, up.idx, dn.idx);
                 }
             }
         }
     }
+}
+
+__device__ __forceinline__ bool in_window(float2 h, float ylo, float yhi, float zlo, float zhi) {
+    return ylo <= h.x && h.x <= yhi && zlo <= h.y && h.y <= zhi;
 }
 
 __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const float2* my_yz,
@@ -104,59 +111,74 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
                                            int base_dn, int32_t* __restrict__ link_up,
                                            int32_t* __restrict__ link_dn) {
     const float WY = g.nf_wy, WZ = g.nf_wz, D2MAX = g.nf_d2max;
+    const float kInf = __int_as_float(0x7f800000);
     for (int i = threadIdx.x; i < n; i += kNbThreads) {
         const float2 h = my_yz[i];
         const float y = h.x, z = h.y;
         const float ylo = __fsub_rn(y, WY), yhi = __fadd_rn(y, WY);
         const float zlo = __fsub_rn(z, WZ), zhi = __fadd_rn(z, WZ);
         const int zb0 = zbin(zlo, z0, g.inv_cz, g.nz), zb1 = zbin(zhi, z0, g.inv_cz, g.nz);
-        Best best{0.0f, -1, -1};
-        bool dense = zb1 - zb0 > 1;
-        if (!dense) {
-            // Two flat loops (one per neighbour row) over the handful of hits in the touched cells.  Row r-1 first:
-            // its window hits (at most kNbList = 4) stay in registers as (y - y_d, z - z_d) plus their positions,
-            // newest first; then every window hit of row r+1 is paired with them.
+        Best best{kInf, -1, -1};
+        if (zb1 - zb0 > 1) {  // a grid finer than the window (non-default grid_cell_z): generic exact search
+            search_dense(g, up, dn, y, z, ylo, yhi, zlo, zhi, zb0, zb1, best);
+        } else {
+            // Flat loops over the handful of hits in the touched cells.  Row r-1 first: its window hits (the newest
+            // kNbList = 4) stay in registers as (y - y_d, z - z_d) plus their positions; then every window hit of
+            // row r+1 is paired with them.  All straight-line code with predicates: the lanes of a warp see
+            // different hit counts, and branches taken by a few lanes cost the whole warp.
             const CellSeq cd = window_cells(g, dn, ylo, yhi, zb0, zb1);
             const CellSeq cu = window_cells(g, up, ylo, yhi, zb0, zb1);
             float t2a = 0.0f, t2b = 0.0f, t2c = 0.0f, t2d = 0.0f, t4a = 0.0f, t4b = 0.0f, t4c = 0.0f, t4d = 0.0f;
             unsigned long long ld = 0ull;
             int nd = 0;
-            const int dshift = cd.b0 - cd.na;
+            const int dshift = cd.b0 - cd.na, ushift = cu.b0 - cu.na;
             for (int k = 0; k < cd.nt; k++) {
                 const int j = k < cd.na ? cd.a0 + k : k + dshift;
                 const float2 d = dn.yz[j];
-                if (ylo <= d.x && d.x <= yhi && zlo <= d.y && d.y <= zhi) {
-                    t2d = t2c; t2c = t2b; t2b = t2a; t2a = __fsub_rn(y, d.x);
-                    t4d = t4c; t4c = t4b; t4b = t4a; t4a = __fsub_rn(z, d.y);
-                    ld = (ld << 16) | (unsigned long long)j;
-                    nd++;
-                }
+                const bool in = in_window(d, ylo, yhi, zlo, zhi);
+                t2d = in ? t2c : t2d; t2c = in ? t2b : t2c; t2b = in ? t2a : t2b; t2a = in ? __fsub_rn(y, d.x) : t2a;
+                t4d = in ? t4c : t4d; t4c = in ? t4b : t4c; t4b = in ? t4a : t4b; t4a = in ? __fsub_rn(z, d.y) : t4a;
+                ld = in ? ((ld << 16) | (unsigned long long)j) : ld;
+                nd += in ? 1 : 0;
             }
-            dense = nd > kNbList;
-            if (!dense && nd > 0) {
-                const int ushift = cu.b0 - cu.na;
-                for (int k = 0; k < cu.nt; k++) {
+            if (nd <= kNbList) {
+                for (int k = 0; k < (nd > 0 ? cu.nt : 0); k++) {
                     const int ja = k < cu.na ? cu.a0 + k : k + ushift;
                     const float2 u = up.yz[ja];
-                    if (!(ylo <= u.x && u.x <= yhi && zlo <= u.y && u.y <= zhi)) continue;
+                    const bool uin = in_window(u, ylo, yhi, zlo, zhi);
                     const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
-#define TPC_NB_PAIR(T2, T4, Q)                                                                      \
-    if (nd > Q) {                                                                                   \
-        const float ey = __fsub_rn(t1, T2), ez = __fsub_rn(t3, T4);                                 \
-        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                            \
-        if (D <= D2MAX) consider(best, D, ja, (int)((ld >> (16 * Q)) & 0xffffull), up.idx, dn.idx); \
+#define TPC_NB_PAIR(T2, T4, Q)                                                                                   \
+    {                                                                                                            \
+        const float ey = __fsub_rn(t1, T2), ez = __fsub_rn(t3, T4);                                              \
+        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                                         \
+        consider(best, uin && nd > Q && D <= D2MAX, D, ja, (int)((ld >> (16 * Q)) & 0xffffull), up.idx, dn.idx); \
     }
                     TPC_NB_PAIR(t2a, t4a, 0)
                     TPC_NB_PAIR(t2b, t4b, 1)
-                    TPC_NB_PAIR(t2c, t4c, 2)
-                    TPC_NB_PAIR(t2d, t4d, 3)
+                    if (nd > 2) {
+                        TPC_NB_PAIR(t2c, t4c, 2)
+                        TPC_NB_PAIR(t2d, t4d, 3)
+                    }
 #undef TPC_NB_PAIR
                 }
+            } else {
+                // more than kNbList window hits in row r-1 (dense spots): pair every window hit of row r+1 with a
+                // second pass over the row r-1 cells
+                for (int k = 0; k < cu.nt; k++) {
+                    const int ja = k < cu.na ? cu.a0 + k : k + ushift;
+                    const float2 u = up.yz[ja];
+                    if (!in_window(u, ylo, yhi, zlo, zhi)) continue;
+                    const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
+                    for (int q = 0; q < cd.nt; q++) {
+                        const int jb = q < cd.na ? cd.a0 + q : q + dshift;
+                        const float2 d = dn.yz[jb];
+                        const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
+                        const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
+                        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+                        consider(best, in_window(d, ylo, yhi, zlo, zhi) && D <= D2MAX, D, ja, jb, up.idx, dn.idx);
+                    }
+                }
             }
-        }
-        if (dense) {  // more than kNbList window hits in row r-1, or a grid finer than the window: exact slow path
-            best = Best{0.0f, -1, -1};
-            search_dense(g, up, dn, y, z, ylo, yhi, zlo, zhi, zb0, zb1, best);
         }
         // links live in SORTED space: entry base + i belongs to the i-th hit of the sorted row, values are sorted
         // global positions; coalesced stores
