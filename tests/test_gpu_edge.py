@@ -1,0 +1,132 @@
+"""GPU edge cases and full-size parity: empty and ragged inputs, exact duplicates (tie-breaks), dense spots (the slow
+paths of S2 and S5), capacity overflow, and the bench's own workload (full CFG:4 windows) against the oracle."""
+import dataclasses
+import json
+import os
+
+import numpy as np
+import pytest
+
+from paper_1709_00618_b200 import datagen as dg
+
+from parity_util import (MIN_SHARED, assert_ca_bit_exact, assert_final_consistency, final_track_report, run_oracle,
+                         tracklet_report)
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu(ev, **kw):
+    from paper_1709_00618_b200 import Tracker
+    trk = Tracker.for_event(ev)
+    res = trk.track_sectors(ev.clusters, ev.row_offsets, ev.n_inst, debug=True, **kw)
+    trk.close()
+    return res
+
+
+def _rebuild(ev, clusters, rows, inst=None):
+    """An Event with the given clusters; rows (and instances) say where each goes.  Order inside a row = given order."""
+    inst = np.zeros(len(rows), np.int64) if inst is None else np.asarray(inst, np.int64)
+    slab = inst * ev.n_rows + np.asarray(rows, np.int64)
+    order = np.argsort(slab, kind="stable")
+    ro = np.zeros(ev.n_inst * ev.n_rows + 1, np.int32)
+    np.add.at(ro, slab + 1, 1)
+    ro = np.cumsum(ro).astype(np.int32)
+    cl = np.ascontiguousarray(clusters[order], np.float32)
+    return dataclasses.replace(ev, clusters=cl, row_offsets=ro, labels=np.full(len(cl), -1, np.int32), truth={})
+
+
+def _rows_of(ev):
+    return np.repeat(np.arange(ev.n_inst * ev.n_rows), np.diff(ev.row_offsets)) % ev.n_rows
+
+
+def _check(ev, max_ok_mismatch=0):
+    o = run_oracle(ev)
+    g = _gpu(ev)
+    assert_ca_bit_exact(g, o)
+    tr = tracklet_report(g, o)
+    fr = final_track_report(g, o, ev.n_clusters)
+    assert_final_consistency(g, ev.n_clusters)
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/parity_report.jsonl", "a") as f:
+        f.write(json.dumps(dict(case=ev.name, n_clusters=ev.n_clusters, **tr, **fr)) + "\n")
+    assert tr["ok_mismatch"] <= max_ok_mismatch, tr
+    assert tr["shared_frac"] >= MIN_SHARED and tr["worst_param_excess"] <= 1.0, tr
+    if fr["n_tracks_gpu"] or fr["n_tracks_oracle"]:
+        assert fr["shared_assign_frac"] >= MIN_SHARED, fr
+    return g, o
+
+
+def test_empty_input():
+    ev = dg.single_sector(seed=1001)
+    empty = _rebuild(ev, ev.clusters[:0], np.zeros(0, np.int64))
+    g = _gpu(empty)
+    assert g.counts[:6].tolist() == [0, 0, 0, 0, 0, 0]
+    assert g.cluster_owner.shape == (0,) and g.trk_hit_offset[0] == 0
+
+
+def test_ragged_rows_few_hits():
+    """Most rows empty: hits only in rows 0..14 and 140..158, one row with a single hit."""
+    ev = dg.single_sector(seed=1011)
+    rows = _rows_of(ev)
+    keep = (rows <= 14) | (rows >= 140)
+    keep[np.flatnonzero(rows == 3)[1:]] = False
+    rag = _rebuild(ev, ev.clusters[keep], rows[keep])
+    g, o = _check(rag)
+    assert g.n_tracks == len(o.trk_cand) and g.n_tracks > 0
+
+
+def test_short_tracks_only_no_final_track():
+    """Tracks of 8 rows: candidates and tracklets exist, but no tracklet reaches sel_min = 10 hits."""
+    ev = dg.single_sector(seed=1012, noise=0.0)
+    rows = _rows_of(ev)
+    keep = (rows >= 40) & (rows < 48)
+    sh = _rebuild(ev, ev.clusters[keep], rows[keep])
+    g, o = _check(sh)
+    assert g.n_cand > 0 and g.n_tracks == 0 and np.all(g.cluster_owner == -1)
+
+
+def test_exact_duplicates_tie_breaks():
+    """Every cluster twice: every D and every pick-up distance ties exactly, so the lowest-index rules decide."""
+    ev = dg.single_sector(seed=1013, n_tracks=60)
+    rows = _rows_of(ev)
+    cl = np.concatenate([ev.clusters, ev.clusters])
+    dup = _rebuild(ev, cl, np.concatenate([rows, rows]))
+    _check(dup)
+
+
+def test_dense_spot_slow_paths():
+    """> 4 window hits in the neighbour rows and > 3 hits in the follower's gate: the loops behind the in-line paths."""
+    ev = dg.single_sector(seed=1014, n_tracks=40)
+    rows = _rows_of(ev)
+    rng = np.random.default_rng(77)
+    extra_rows = np.repeat(np.arange(60, 75), 12)
+    x = dg.row_x(ev.n_rows)[extra_rows]
+    blob = np.stack([x, rng.uniform(-1.0, 1.0, len(x)), rng.uniform(99.0, 101.5, len(x)),
+                     np.full(len(x), -1.0)], axis=1).astype(np.float32)
+    dense = _rebuild(ev, np.concatenate([ev.clusters, blob]), np.concatenate([rows, extra_rows]))
+    _check(dense)
+
+
+def test_capacity_overflow_is_reported_not_written():
+    from paper_1709_00618_b200 import Tracker
+    from paper_1709_00618_b200.tracker import TpcError
+    ev = dg.single_sector(seed=1001)
+    full = _gpu(ev)
+    assert full.n_tracks > 4
+    trk = Tracker.for_event(ev)
+    with pytest.raises(TpcError, match="CAPACITY"):
+        trk.track_sectors(ev.clusters, ev.row_offsets, ev.n_inst, trk_capacity=3)
+    trk.close()
+
+
+def test_full_size_drift_windows_against_oracle():
+    """The bench's workload at full size: two full CFG:4 windows (5 overlapping events each, 72 sector instances),
+    in the launch configuration bench.py times (one tpc_track_sectors call on the batch)."""
+    evs = [dg.drift_window(seed=5001 + i) for i in range(2)]
+    batch = dg.concat_events(evs)
+    assert batch.n_clusters > 1_000_000
+    # A tracklet exists or not by threshold tests on the fitted state (|sinPhi| <= 0.95 in a transport): fp64 in the
+    # oracle, fp32 in the kernels (A12/A13), so at this size a handful of the ~130 k candidates may fall on
+    # the other side; they count against the 99.5 % shared-assignment bar like any other difference.
+    g, o = _check(batch, max_ok_mismatch=batch.n_clusters // 200_000)
+    assert abs(g.n_tracks - len(o.trk_cand)) <= 5
