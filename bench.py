@@ -37,7 +37,7 @@ FLOP_TRANSPORT, FLOP_UPDATE, FLOP_EXAMINE, FLOP_SEARCH = 150.0, 93.0, 7.0, 18.0
 FP32_LANES_PER_SM, N_SM = 128, 148
 # dram bytes per launch of follow_kernel per cluster, from the committed ncu --set full capture (profiles/); None
 # until a capture exists
-FOLLOW_DRAM_BYTES_PER_CLUSTER = None
+FOLLOW_DRAM_BYTES_PER_CLUSTER = 338.5  # profiles/r1c_full_kernels.md: (5.773 + 0.465) GB per launch / 18,427,708 clusters
 
 
 def _gen_window(seed):
@@ -221,6 +221,20 @@ def run_ours(args):
     st = [trk.stage_times_ms(a) for a in range(k)]  # the untimed counting call above recorded no events
     stage_ms = {nme: float(np.mean([s[nme] for s in st])) for nme in st[0]}
 
+    # ---- latency of ONE drift window (CFG:4) alone on the GPU: L2 flushed before every call ----------------------
+    n0, s0 = evs[0].n_clusters, evs[0].n_inst
+    fb1 = fbuf if fbuf is not None else torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    ev1 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+    trk.track_sectors_device(d_cl[:n0], d_ro[:s0 * batch.n_rows + 1], s0, out)
+    for a, b in ev1:
+        fb1.fill_(1)
+        a.record()
+        trk.track_sectors_device(d_cl[:n0], d_ro[:s0 * batch.n_rows + 1], s0, out)
+        b.record()
+    torch.cuda.synchronize(dev)
+    one_ms = float(np.median([a.elapsed_time(b) for a, b in ev1]))
+    del fb1
+
     # ---- end to end through the host-buffer entry point -------------------------------------------------------------
     ipc = 36 * max(1, args.chunk_windows)
     max_chunk = max(int(batch.row_offsets[min(i + ipc, S) * batch.n_rows] - batch.row_offsets[i * batch.n_rows])
@@ -246,17 +260,22 @@ def run_ours(args):
         return
     hbm_peak, sm_max, peak_src = measured_peaks()
     fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12  # TFLOP/s
-    flops = (counts[6] * FLOP_TRANSPORT + counts[7] * FLOP_UPDATE + counts[8] * FLOP_EXAMINE + counts[9] * FLOP_SEARCH)
+    # follow_kernel alone: the work of the fit kernel (the candidates' own hits, counts[11..12]) is not its work
+    tr_f, up_f = int(counts[6] - counts[11]), int(counts[7] - counts[12])
+    flops = (tr_f * FLOP_TRANSPORT + up_f * FLOP_UPDATE + counts[8] * FLOP_EXAMINE + counts[9] * FLOP_SEARCH)
     t_follow = stage_ms["follow"] * 1e-3
     ach = flops / t_follow / 1e12
-    roof = {"kernel": "follow_kernel (S5 Kalman track following)", "bound": "alu", "achieved": ach, "peak": fp32_peak,
+    roof = {"kernel": "follow_kernel (S5 Kalman track following, row-by-row extrapolation)", "bound": "alu", "achieved": ach, "peak": fp32_peak,
             "unit": "TFLOP/s", "frac": ach / fp32_peak,
             "traffic": None if FOLLOW_DRAM_BYTES_PER_CLUSTER is None else FOLLOW_DRAM_BYTES_PER_CLUSTER * N,
+            "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of follow_kernel per launch on the "
+                              "default workload (profiles/r1c_full_kernels.md), scaled by the cluster count",
             "peak_source": f"148 SM x 128 fp32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md)",
             "avg_launch_ms": stage_ms["follow"], "share_of_step": stage_ms["follow"] / sum(stage_ms.values()),
             "algorithmic_flop_per_launch": float(flops),
-            "work": {"transports": int(counts[6]), "updates": int(counts[7]), "clusters_examined": int(counts[8]),
-                     "searches": int(counts[9]), "row_steps_per_cluster": float(counts[6]) / N},
+            "work": {"transports": tr_f, "updates": up_f, "clusters_examined": int(counts[8]),
+                     "searches": int(counts[9]), "fit_kernel_transports": int(counts[11]),
+                     "fit_kernel_updates": int(counts[12]), "row_steps_per_cluster": float(counts[6]) / N},
             "hbm_view": {"bytes_per_cluster": BYTES_PER_CLUSTER_S5,
                          "achieved_gbs": BYTES_PER_CLUSTER_S5 * N / t_follow / 1e9,
                          "frac_of_hbm_peak": BYTES_PER_CLUSTER_S5 * N / t_follow / 1e9 / hbm_peak}}
@@ -286,6 +305,8 @@ def run_ours(args):
                     "tracks": e2e_tracks, "timer": "host perf_counter around the blocking C-ABI calls"},
             "roofline": roof, "roofline_path_hbm": roof_path, "cpu_baseline": cpu,
             "stage_ms": stage_ms,
+            "single_window": {"workload": "cfg4: one drift window alone (36 sector instances), L2 flushed", "ms": one_ms,
+                              "clusters": n0, "clusters_per_s": n0 / (one_ms * 1e-3)},
             "results": {"candidates": int(counts[1]), "tracklets": int(counts[2]), "tracks": int(counts[3]),
                         "track_hits": int(counts[4]), "error_flags": int(counts[5])},
             "physics_window0": phys}

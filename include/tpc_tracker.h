@@ -113,7 +113,8 @@ typedef struct {
        5 input error flags (bit0: a row holds > 65535 clusters; bit1: > 2^23 candidates in one instance),
        6 S5 transport steps executed, 7 S5 measurement updates, 8 clusters examined by the S5 pick-up search,
        9 S5 pick-up searches (work counters for the roofline arithmetic; 6-9 stay 0 unless
-       tpc_set_work_counters enabled them), 10-15 reserved.
+       tpc_set_work_counters enabled them), 10 internal, 11/12 the part of 6/7 spent on the candidates' own
+       hits (fit kernel), 13-15 reserved.
        Written by the last kernel of the call. */
     int64_t* counts;
 } tpc_output_t;
@@ -153,8 +154,9 @@ int tpc_set_work_counters(tpc_tracker_t* t, int32_t enable);
 /* Optional per-stage timing: when enabled, every tpc_track_sectors call records CUDA events on its stream around
    each stage (a ring of the last TPC_TIMING_RING calls).  tpc_stage_times_ms waits for the call `age` calls back
    (0 = the last one) and returns its milliseconds in out_ms[TPC_N_STAGES]
-   (order: bin, neighbours, clean, chains, follow, select). */
-#define TPC_N_STAGES 6
+   (order: bin, neighbours, clean, chains, fit, follow, select; fit = the candidates' own hits, follow = the
+   row-by-row extrapolation, both S5). */
+#define TPC_N_STAGES 7
 #define TPC_TIMING_RING 32
 int tpc_set_stage_timing(tpc_tracker_t* t, int32_t enable);
 int tpc_stage_times_ms(tpc_tracker_t* t, int32_t age, float* out_ms);

@@ -75,10 +75,18 @@ scan_int2_kernel(int2* __restrict__ part, const int64_t* __restrict__ m_dev, int
     if (threadIdx.x == 0) s_carry = make_int2(0, 0);
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    for (int64_t start = 0; start < m; start += kScanThreads) {
-        const int64_t i = start + threadIdx.x;
-        int2 v = i < m ? part[i] : make_int2(0, 0);
-        int2 incl = v;
+    constexpr int kPer = 4;  // consecutive entries per thread and round
+    for (int64_t start = 0; start < m; start += kScanThreads * kPer) {
+        const int64_t i0 = start + (int64_t)threadIdx.x * kPer;
+        int2 v[kPer];
+        int2 sum = make_int2(0, 0);
+#pragma unroll
+        for (int q = 0; q < kPer; q++) {
+            v[q] = i0 + q < m ? part[i0 + q] : make_int2(0, 0);
+            sum.x += v[q].x;
+            sum.y += v[q].y;
+        }
+        int2 incl = sum;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             int a = __shfl_up_sync(0xffffffffu, incl.x, d), b = __shfl_up_sync(0xffffffffu, incl.y, d);
@@ -88,9 +96,15 @@ scan_int2_kernel(int2* __restrict__ part, const int64_t* __restrict__ m_dev, int
         __syncthreads();
         int2 off = s_carry;
         for (int k = 0; k < wid; k++) { off.x += s_warp[k].x; off.y += s_warp[k].y; }
-        if (i < m) part[i] = make_int2(off.x + incl.x - v.x, off.y + incl.y - v.y);
+        int2 run = make_int2(off.x + incl.x - sum.x, off.y + incl.y - sum.y);
+#pragma unroll
+        for (int q = 0; q < kPer; q++) {
+            if (i0 + q < m) part[i0 + q] = run;
+            run.x += v[q].x;
+            run.y += v[q].y;
+        }
         __syncthreads();
-        if (threadIdx.x == kScanThreads - 1) s_carry = make_int2(off.x + incl.x, off.y + incl.y);
+        if (threadIdx.x == kScanThreads - 1) s_carry = run;
         __syncthreads();
     }
     if (threadIdx.x == 0) {

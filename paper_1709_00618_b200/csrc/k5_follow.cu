@@ -183,6 +183,8 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
         if ((threadIdx.x & 31) == 0) {
             if (n_tr) atomicAdd((unsigned long long*)&a.counts[6], (unsigned long long)n_tr);
             if (n_up) atomicAdd((unsigned long long*)&a.counts[7], (unsigned long long)n_up);
+            if (n_tr) atomicAdd((unsigned long long*)&a.counts[11], (unsigned long long)n_tr);
+            if (n_up) atomicAdd((unsigned long long*)&a.counts[12], (unsigned long long)n_up);
         }
     }
 }
@@ -562,27 +564,36 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
     }
 }
 
-int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, int n_sm, bool count_work,
-                  cudaStream_t s) {
+static FollowArgs follow_args(const Workspace& w, const Problem& p, const ChainOut& u) {
+    return FollowArgs{p.row_offsets, w.hit_yz,  w.hit_idx,  w.bin_start, w.up,        w.cand_start, w.cand_slab,
+                      u.cand_hits,   u.cand_n,  u.cand_cap, w.counts,    w.Cmax,      w.tl_state,   w.tl_par,
+                      w.tl_cov,      w.tl_chi2, w.tl_nhits, w.tl_rows,   w.tl_rowhit, w.tl_sel};
+}
+
+int launch_fit(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, bool count_work, cudaStream_t s) {
     if (p.n_clusters == 0) return 0;
-    FollowArgs a{p.row_offsets, w.hit_yz,  w.hit_idx,   w.bin_start, w.up,      w.cand_start, w.cand_slab,
-                 u.cand_hits,   u.cand_n,  u.cand_cap,  w.counts,    w.Cmax,    w.tl_state,   w.tl_par,
-                 w.tl_cov,      w.tl_chi2, w.tl_nhits,  w.tl_rows,   w.tl_rowhit, w.tl_sel};
-    // the candidate count lives on the device: both grids are sized by its bound and bounded by it inside
-    const int fit_grid = div_up(w.Cmax, kFitThreads);
+    const FollowArgs a = follow_args(w, p, u);
+    // the candidate count lives on the device: the grid is sized by its bound and bounded by it inside
+    const int grid = div_up(w.Cmax, kFitThreads);
+    if (count_work)
+        fit_candidates_kernel<true><<<grid, kFitThreads, 0, s>>>(g, a);
+    else
+        fit_candidates_kernel<false><<<grid, kFitThreads, 0, s>>>(g, a);
+    return 1;
+}
+
+int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, bool count_work, cudaStream_t s) {
+    if (p.n_clusters == 0) return 0;
+    const FollowArgs a = follow_args(w, p, ChainOut{nullptr, 0, nullptr, nullptr, 0});
     // persistent grid: every SM holds kFollowCtasPerSm CTAs, capped by the candidate bound
     const int64_t want = div_up(w.Cmax, kFollowThreads);
-    const int per_sm = kFollowCtasPerSm;
-    int grid = (int)(want < (int64_t)n_sm * per_sm ? want : (int64_t)n_sm * per_sm);
+    int grid = (int)(want < (int64_t)n_sm * kFollowCtasPerSm ? want : (int64_t)n_sm * kFollowCtasPerSm);
     if (grid < 1) grid = 1;
-    if (count_work) {
-        fit_candidates_kernel<true><<<fit_grid, kFitThreads, 0, s>>>(g, a);
+    if (count_work)
         follow_kernel<true, kFollowSpec><<<grid, kFollowThreads, 0, s>>>(g, a);
-    } else {
-        fit_candidates_kernel<false><<<fit_grid, kFitThreads, 0, s>>>(g, a);
+    else
         follow_kernel<false, kFollowSpec><<<grid, kFollowThreads, 0, s>>>(g, a);
-    }
-    return 2;
+    return 1;
 }
 
 }  // namespace tpc

@@ -113,8 +113,8 @@ void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m
 // parity/debug: a link array of the workspace (sorted space) as input-order indices; dir = row offset of the targets
 int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link, int dir,
                         int32_t* out, cudaStream_t s);
-int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, int n_sm, bool count_work,
-                  cudaStream_t s);
+int launch_fit(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, bool count_work, cudaStream_t s);
+int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, bool count_work, cudaStream_t s);
 
 struct SelectOut {  // mirrors the S6 part of tpc_output_t
     float *trk_params, *trk_cov, *trk_chi2, *trk_xref;

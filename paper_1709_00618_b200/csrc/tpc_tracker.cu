@@ -250,13 +250,15 @@ extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const 
                 (out->cand_hits || out->cand_n) ? out->cand_capacity : 0};
     launches += launch_chains(g, w, p, co, s);
     if (tm) cudaEventRecord(ev[4], s);
-    launches += launch_follow(g, w, p, co, t->n_sm, t->count_work, s);
+    launches += launch_fit(g, w, p, co, t->count_work, s);
     if (tm) cudaEventRecord(ev[5], s);
+    launches += launch_follow(g, w, p, t->n_sm, t->count_work, s);
+    if (tm) cudaEventRecord(ev[6], s);
     SelectOut so{out->trk_params, out->trk_cov, out->trk_chi2, out->trk_xref, out->trk_cand_id, out->trk_nhits,
                  out->trk_sector, out->trk_hit_offset, out->trk_hits, out->trk_capacity, out->trk_hits_capacity,
                  out->cluster_owner, out->counts};
     launches += launch_select(g, w, p, so, s);
-    if (tm) cudaEventRecord(ev[6], s);
+    if (tm) cudaEventRecord(ev[7], s);
     // optional parity/debug copies (device to device, same stream)
     if (n_clusters > 0) {
         launches += launch_export_links(g, w, p, w.up_raw, +1, out->link_up_raw, s);
