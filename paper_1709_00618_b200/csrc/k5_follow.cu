@@ -449,9 +449,11 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     }
                     k0 = kSpecHits;
                 }
-                for (int k = k0; k < q.nt; k++) {
+                for (int k = k0; k < q.nt; k++) {  // few lanes get here: test the gate first, most hits fail it
                     const int j = k < q.na ? q.ja0 + k : k + q.d;
-                    pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
+                    const float2 h = a.hit_yz[urb + (unsigned)j];
+                    if (fabsf(__fsub_rn(h.x, yp)) <= wy && fabsf(__fsub_rn(h.y, zp)) <= wz)
+                        pick_consider(b, a.hit_idx, urb, j, true, h, yp, zp, wy, wz);
                 }
                 // z bins in between exist only when the cells are narrower than the gate (non-default
                 // grid_cell_z); such windows are never speculated
