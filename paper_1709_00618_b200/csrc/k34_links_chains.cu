@@ -25,18 +25,19 @@ clean_links_kernel(int64_t n, const int32_t* __restrict__ up_raw, const int32_t*
     claim[h] = 0u;
 }
 
-// S4 pass 1: per-hit flags (bit0 start hit, bit1 candidate) and per-slab counts.
+// S4 pass 1: per-hit flags (bit0 start hit, bit1 candidate) and per-slab counts.  One WARP per (instance,row) slab:
+// a slab is ~200 hits and a short chain of dependent loads, so what bounds these passes is how many slabs an SM has
+// in flight -- 64 with a warp each against 16 with a 128-thread CTA each -- and a warp needs no barrier.
 __global__ void __launch_bounds__(kChainThreads)
 chain_flags_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
                    const int32_t* __restrict__ up, const int32_t* __restrict__ dn, uint8_t* __restrict__ flags,
-                   int2* __restrict__ slab_part) {
-    __shared__ int s_cnt[2];
-    const int slab = blockIdx.x;
+                   int2* __restrict__ slab_part, int n_slabs) {
+    const int slab = blockIdx.x * (kChainThreads / 32) + (threadIdx.x >> 5);
+    if (slab >= n_slabs) return;
+    const int lane = threadIdx.x & 31;
     const int base = row_offsets[slab], n = row_offsets[slab + 1] - base;
-    if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0;
-    __syncthreads();
     int ns = 0, nc = 0;
-    for (int i = threadIdx.x; i < n; i += kChainThreads) {
+    for (int i = lane; i < n; i += 32) {
         const int h = base + i;
         uint8_t f = 0;
         int x = up[h];
@@ -50,17 +51,9 @@ chain_flags_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict_
         ns += f & 1;
         nc += f >> 1;
     }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        ns += __shfl_xor_sync(0xffffffffu, ns, d);
-        nc += __shfl_xor_sync(0xffffffffu, nc, d);
-    }
-    if ((threadIdx.x & 31) == 0) {
-        atomicAdd(&s_cnt[0], ns);
-        atomicAdd(&s_cnt[1], nc);
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) slab_part[slab] = make_int2(s_cnt[0], s_cnt[1]);
+    ns = __reduce_add_sync(0xffffffffu, ns);
+    nc = __reduce_add_sync(0xffffffffu, nc);
+    if (lane == 0) slab_part[slab] = make_int2(ns, nc);
 }
 
 // Exclusive scan of int2 partials by ONE CTA (m is a few thousand to a few hundred thousand entries); entry m
@@ -123,17 +116,17 @@ __global__ void __launch_bounds__(kChainThreads)
 chain_write_kernel(const int32_t* __restrict__ row_offsets, const uint16_t* __restrict__ hit_pos,
                    const uint8_t* __restrict__ flags, const int2* __restrict__ slab_part,
                    int32_t* __restrict__ start_hits, int64_t start_cap, int32_t* __restrict__ cand_start,
-                   int32_t* __restrict__ cand_slab, int64_t cand_cap) {
-    __shared__ int2 s_warp[kChainThreads / 32];
-    const int slab = blockIdx.x;
+                   int32_t* __restrict__ cand_slab, int64_t cand_cap, int n_slabs) {
+    const int slab = blockIdx.x * (kChainThreads / 32) + (threadIdx.x >> 5);  // one warp per slab
+    if (slab >= n_slabs) return;
     const int2 sb = slab_part[slab];
     if (slab_part[slab + 1].x == sb.x) return;  // no start hit in this slab
     const int base = row_offsets[slab], n = min(row_offsets[slab + 1] - base, 65535);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
-    int2 carry = sb;  // (start hits, candidates) before the current chunk
-    for (int i0 = 0; i0 < n; i0 += kChainThreads) {
-        const int i = i0 + threadIdx.x;  // input position
+    int2 carry = sb;  // (start hits, candidates) before the current 32 input positions
+    for (int i0 = 0; i0 < n; i0 += 32) {
+        const int i = i0 + lane;  // input position
         int pos = 0;
         uint8_t f = 0;
         if (i < n) {
@@ -141,29 +134,19 @@ chain_write_kernel(const int32_t* __restrict__ row_offsets, const uint16_t* __re
             f = flags[base + pos];
         }
         const unsigned ms = __ballot_sync(0xffffffffu, f & 1), mc = __ballot_sync(0xffffffffu, f & 2);
-        if (lane == 0) s_warp[wid] = make_int2(__popc(ms), __popc(mc));
-        __syncthreads();
-        int2 off = carry, tot = carry;
-#pragma unroll
-        for (int k = 0; k < kChainThreads / 32; k++) {
-            const int2 v = s_warp[k];
-            if (k < wid) { off.x += v.x; off.y += v.y; }
-            tot.x += v.x;
-            tot.y += v.y;
-        }
-        carry = tot;
         if (f) {
-            const int64_t ps = off.x + __popc(ms & lt);
+            const int64_t ps = carry.x + __popc(ms & lt);
             if (start_hits && ps < start_cap) start_hits[ps] = base + i;
             if (f & 2) {
-                const int64_t c = off.y + __popc(mc & lt);
+                const int64_t c = carry.y + __popc(mc & lt);
                 if (c < cand_cap) {
                     cand_start[c] = base + pos;
                     cand_slab[c] = slab;
                 }
             }
         }
-        __syncthreads();
+        carry.x += __popc(ms);
+        carry.y += __popc(mc);
     }
 }
 
@@ -199,10 +182,11 @@ void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m
 int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, cudaStream_t s) {
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
-    chain_flags_kernel<<<slabs, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.dn, w.flags, w.slab_part);
+    const int grid = div_up(slabs, kChainThreads / 32);
+    chain_flags_kernel<<<grid, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.dn, w.flags, w.slab_part, slabs);
     launch_scan_int2(w.slab_part, nullptr, 1, 0, slabs, w.counts, 0, 1, s);
-    chain_write_kernel<<<slabs, kChainThreads, 0, s>>>(p.row_offsets, w.hit_pos, w.flags, w.slab_part, u.start_hits,
-                                                       u.start_cap, w.cand_start, w.cand_slab, w.Cmax);
+    chain_write_kernel<<<grid, kChainThreads, 0, s>>>(p.row_offsets, w.hit_pos, w.flags, w.slab_part, u.start_hits,
+                                                      u.start_cap, w.cand_start, w.cand_slab, w.Cmax, slabs);
     return 3;
 }
 

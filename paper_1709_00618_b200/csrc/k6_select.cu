@@ -19,7 +19,7 @@ namespace tpc {
 
 constexpr int kSelThreads = 256;
 constexpr int kSelBlock = kSelThreads;  // tracklets per CTA in the tracklet-centric passes
-constexpr int kHitThreads = 128;        // hit-centric passes: one CTA per (sector instance, pad row)
+constexpr int kHitThreads = 256;        // hit-centric passes: one WARP per (sector instance, pad row)
 constexpr unsigned kFull = 0xffffffffu;
 
 __device__ __forceinline__ int64_t winner_of(uint32_t w, int64_t cand_base) {
@@ -75,14 +75,16 @@ claim_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_
 
 __global__ void __launch_bounds__(kHitThreads)
 mark_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
-            const int2* __restrict__ slab_part, const uint32_t* __restrict__ claim, uint32_t* __restrict__ tl_sel) {
-    const int slab = blockIdx.x;
+            const int2* __restrict__ slab_part, const uint32_t* __restrict__ claim, uint32_t* __restrict__ tl_sel,
+            int n_slabs) {
+    const int slab = blockIdx.x * (kHitThreads / 32) + (threadIdx.x >> 5);  // one warp per slab
+    if (slab >= n_slabs) return;
     const int inst = slab / g.R, r = slab - inst * g.R;
     const int base = row_offsets[slab], n = row_offsets[slab + 1] - base;
     if (n == 0) return;
     const int64_t cand_base = slab_part[(size_t)inst * g.R].y;
     const uint32_t bit = 1u << (r & 31);
-    for (int i = threadIdx.x; i < n; i += kHitThreads) {
+    for (int i = threadIdx.x & 31; i < n; i += 32) {
         const uint32_t w = claim[base + i];
         if (w) atomicOr(&tl_sel[winner_of(w, cand_base) * g.sel_stride + (r >> 5)], bit);
     }
@@ -197,15 +199,17 @@ finalize_tracks_kernel(const __grid_constant__ DevGeom g, const FinalIn a, const
 __global__ void __launch_bounds__(kHitThreads)
 write_hits_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
                   const int2* __restrict__ slab_part, const uint32_t* __restrict__ claim,
-                  const uint32_t* __restrict__ tl_sel, const uint16_t* __restrict__ hit_idx, const SelectOut o) {
-    const int slab = blockIdx.x;
+                  const uint32_t* __restrict__ tl_sel, const uint16_t* __restrict__ hit_idx, const SelectOut o,
+                  int n_slabs) {
+    const int slab = blockIdx.x * (kHitThreads / 32) + (threadIdx.x >> 5);  // one warp per slab
+    if (slab >= n_slabs) return;
     const int inst = slab / g.R, r = slab - inst * g.R;
     const int base = row_offsets[slab], n = min(row_offsets[slab + 1] - base, 65535);
     if (n == 0) return;
     const int64_t cand_base = slab_part[(size_t)inst * g.R].y;
     const int wq = r >> 5;
     const uint32_t below = (1u << (r & 31)) - 1u;
-    for (int i = threadIdx.x; i < n; i += kHitThreads) {
+    for (int i = threadIdx.x & 31; i < n; i += 32) {
         const uint32_t w = claim[base + i];
         if (!w) continue;
         const uint32_t* rec = tl_sel + winner_of(w, cand_base) * g.sel_stride;
@@ -239,13 +243,15 @@ int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const 
         const int grid = (int)(blocks < 148 * 8 ? blocks : 148 * 8);
         claim_kernel<<<grid, kClaimThreads, 0, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows, w.cand_slab, w.slab_part,
                                                     w.tl_rowhit, w.claim, w.counts, w.Cmax);
-        mark_kernel<<<slabs, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel);
+        const int hgrid = div_up(slabs, kHitThreads / 32);
+        mark_kernel<<<hgrid, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel, slabs);
         count_kernel<<<grid, kSelThreads, 0, s>>>(g, w.tl_nhits, w.tl_sel, w.sel_part, w.counts, w.Cmax);
         launch_scan_int2(w.sel_part, w.counts + 1, kSelBlock, w.Cmax, 0, w.counts, 3, 4, s);
         const FinalIn a{w.tl_nhits, w.tl_rows, w.cand_slab, w.tl_par, w.tl_cov, w.tl_chi2, w.sel_part, w.tl_sel,
                         w.counts,   w.Cmax};
         finalize_tracks_kernel<<<grid, kSelThreads, 0, s>>>(g, a, o);
-        write_hits_kernel<<<slabs, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel, w.hit_idx, o);
+        write_hits_kernel<<<hgrid, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel, w.hit_idx, o,
+                                                        slabs);
         launches += 6;
     }
     finalize_counts_kernel<<<1, 32, 0, s>>>(w.counts, o);
