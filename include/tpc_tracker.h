@@ -58,6 +58,9 @@ typedef struct {
     int32_t sel_min_hits;      /* S6 minimum hits kept by a final track: 10 */
     float grid_cell_z;         /* S1 z-bin width of the per-row grid [cm]: 6.75.  Performance only: no result depends on it */
     int32_t grid_cells_y;      /* S1 strips across a pad row (1..64): 12.  Performance only */
+    int32_t nf_bridge_rows;    /* S2: 0 (default) links join adjacent pad rows only (BASELINE.json north_star);
+                                  1 = a hit without an admissible adjacent pair may take one partner two rows away
+                                  (single missing rows are bridged; reading A2') */
 } tpc_params_t;
 
 typedef struct {

@@ -52,6 +52,8 @@ typedef struct {
     int32_t sel_min_hits;
     float grid_cell_y, grid_cell_z;
     double bz;
+    int32_t nf_bridge_rows;      /* 0: links join adjacent rows only; 1: a single missing row may be bridged (A2') */
+    int32_t pad_;
 } orc_config;
 
 typedef struct {               /* one tracklet (S5 output) */
@@ -124,63 +126,138 @@ static void grid_free(orc_rowgrid *g) {
 
 /* ------------------------------------------------------------------ S2: neighbour finder */
 
-/* SURVEY 8(c) S2.  cl_* point at the first cluster (x,y,z,w) of rows r-1, r, r+1; indices written are
- * LOCAL to the rows (position within the row segment of the input array), -1 if none.
- * use_grid = 0: brute force over all (u,d); 1: visit only bins overlapping the window.  Both apply the
- * identical exact tests, so they must agree bit for bit (pin: tests/test_oracle_ca.py). */
-static void neighbours_row(const orc_config *c, const float *cl_dn, int n_dn, const float *cl_r, int n_r,
-                           const float *cl_up, int n_up, const orc_rowgrid *g_dn, const orc_rowgrid *g_up,
-                           int use_grid, int32_t *up_loc, int32_t *dn_loc) {
-    const float WY = c->nf_win_y, WZ = c->nf_win_z, D2MAX = c->nf_d2_max;
-    int32_t *ulist = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_up + 1));
-    int32_t *dlist = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_dn + 1));
-    for (int h = 0; h < n_r; h++) {
-        const float y = cl_r[4 * h + 1], z = cl_r[4 * h + 2];
-        const float ylo = y - WY, yhi = y + WY, zlo = z - WZ, zhi = z + WZ;
-        int nu = 0, nd = 0;
-        for (int pass = 0; pass < 2; pass++) {
-            const float *cl = pass ? cl_dn : cl_up;
-            int n = pass ? n_dn : n_up;
-            const orc_rowgrid *g = pass ? g_dn : g_up;
-            int32_t *list = pass ? dlist : ulist;
-            int cnt = 0;
-            if (!use_grid) {
-                for (int j = 0; j < n; j++) {
-                    float yj = cl[4 * j + 1], zj = cl[4 * j + 2];
-                    if (ylo <= yj && yj <= yhi && zlo <= zj && zj <= zhi) list[cnt++] = j;
-                }
-            } else if (n > 0) {
-                int by0 = grid_bin1(ylo, g->y0, g->inv_cy, g->ny), by1 = grid_bin1(yhi, g->y0, g->inv_cy, g->ny);
-                int bz0 = grid_bin1(zlo, g->z0, g->inv_cz, g->nz), bz1 = grid_bin1(zhi, g->z0, g->inv_cz, g->nz);
-                for (int bz = bz0; bz <= bz1; bz++)
-                    for (int k = g->bin_start[bz * g->ny + by0]; k < g->bin_start[bz * g->ny + by1 + 1]; k++) {
-                        int j = g->perm[k];
-                        float yj = cl[4 * j + 1], zj = cl[4 * j + 2];
-                        if (ylo <= yj && yj <= yhi && zlo <= zj && zj <= zhi) list[cnt++] = j;
-                    }
-            }
-            if (pass) nd = cnt; else nu = cnt;
+/* Hits of one row inside the window [ylo,yhi] x [zlo,zhi] (pure comparisons against pre-rounded bounds), as local
+ * indices (positions within the row segment of the input array).  use_grid = 0: all hits of the row are tested;
+ * 1: only the bins overlapping the window.  Both apply the identical exact test, so they must agree
+ * (pin: tests/test_oracle_ca.py). */
+static int window_list(const float *cl, int n, const orc_rowgrid *g, int use_grid, float ylo, float yhi, float zlo,
+                       float zhi, int32_t *list) {
+    int cnt = 0;
+    if (!use_grid) {
+        for (int j = 0; j < n; j++) {
+            float yj = cl[4 * j + 1], zj = cl[4 * j + 2];
+            if (ylo <= yj && yj <= yhi && zlo <= zj && zj <= zhi) list[cnt++] = j;
         }
-        /* minimum over (D, u, d) lexicographically: independent of the visiting order */
-        int bu = -1, bd = -1;
-        float bD = 0.0f;
-        for (int a = 0; a < nu; a++)
-            for (int b = 0; b < nd; b++) {
-                int u = ulist[a], d = dlist[b];
-                float t1 = cl_up[4 * u + 1] - y, t2 = y - cl_dn[4 * d + 1], ey = t1 - t2;
-                float t3 = cl_up[4 * u + 2] - z, t4 = z - cl_dn[4 * d + 2], ez = t3 - t4;
-                float pyy = ey * ey, pzz = ez * ez;
-                float D = pyy + pzz;
-                if (!(D <= D2MAX)) continue;
-                if (bu < 0 || D < bD || (D == bD && (u < bu || (u == bu && d < bd)))) {
-                    bD = D; bu = u; bd = d;
+    } else if (n > 0) {
+        int by0 = grid_bin1(ylo, g->y0, g->inv_cy, g->ny), by1 = grid_bin1(yhi, g->y0, g->inv_cy, g->ny);
+        int bz0 = grid_bin1(zlo, g->z0, g->inv_cz, g->nz), bz1 = grid_bin1(zhi, g->z0, g->inv_cz, g->nz);
+        for (int bz = bz0; bz <= bz1; bz++)
+            for (int k = g->bin_start[bz * g->ny + by0]; k < g->bin_start[bz * g->ny + by1 + 1]; k++) {
+                int j = g->perm[k];
+                float yj = cl[4 * j + 1], zj = cl[4 * j + 2];
+                if (ylo <= yj && yj <= yhi && zlo <= zj && zj <= zhi) list[cnt++] = j;
+            }
+    }
+    return cnt;
+}
+
+/* SURVEY 8(c) S2 for one sector instance (ro = its row offsets [R+1], indices of `clusters`); link_up/link_dn are
+ * written at those indices and hold such indices, -1 if none.  All fp32, every operation individually rounded
+ * (this file is compiled with -ffp-contract=off).
+ *
+ * Class 0 (the reading of BASELINE.json north_star, "adjacent pad rows"): u in row r+1, d in row r-1, both inside
+ * the window of half-widths (WY, WZ) around the hit; D = (t1 - t2)^2 + (t3 - t4)^2 with t1 = y_u - y, t2 = y - y_d,
+ * t3 = z_u - z, t4 = z - z_d; admissible iff D <= D2MAX; minimum over (D, u, d).
+ *
+ * Class 1 (nf_bridge_rows = 1, reading A2': "bridge single missing rows"): only for
+ * a hit with NO admissible class-0 pair.  One of the two partners may lie two rows away (a row without a usable
+ * cluster is skipped): (du, dd) = (1, 2): u in row r+1, d in row r-2, or (2, 1): u in row r+2, d in row r-1.  The
+ * partner two rows away is searched in the doubled window (2 WY, 2 WZ; exact doubling).  The deviation from a
+ * straight line for unequal spacing is dd * (u - h) - du * (h - d):
+ *     (1,2): ey = (t1 + t1) - t2,   (2,1): ey = t1 - (t2 + t2),   same for z;   D = ey*ey + ez*ez.
+ * Its variance for cluster errors sigma is 14 sigma^2 against 6 sigma^2 for class 0, so the cut is
+ * D <= 2.25 * D2MAX (2.25 is exact in binary; the same ~4 sigma).  Minimum over (D, du, u, d) lexicographically. */
+static void neighbours_instance(const orc_config *c, const float *clusters, const int32_t *ro,
+                                const orc_rowgrid *grids, int use_grid, int32_t *link_up, int32_t *link_dn) {
+    const int R = c->n_rows;
+    const float WY = c->nf_win_y, WZ = c->nf_win_z, D2MAX = c->nf_d2_max;
+    const float WY2 = WY + WY, WZ2 = WZ + WZ, D2MAX1 = D2MAX * 2.25f;
+    int nmax = 1;
+    for (int r = 0; r < R; r++)
+        if (ro[r + 1] - ro[r] > nmax) nmax = ro[r + 1] - ro[r];
+    int32_t *ulist = (int32_t *)malloc(sizeof(int32_t) * (size_t)nmax);
+    int32_t *dlist = (int32_t *)malloc(sizeof(int32_t) * (size_t)nmax);
+    int32_t *xlist = (int32_t *)malloc(sizeof(int32_t) * (size_t)nmax);
+#define ROWCL(rr) (clusters + 4 * (size_t)ro[rr])
+#define ROWN(rr) (ro[(rr) + 1] - ro[rr])
+#define ROWG(rr) (use_grid ? &grids[rr] : (const orc_rowgrid *)0)
+    for (int r = 0; r < R; r++) {
+        const int n_r = ROWN(r);
+        const float *cl_r = ROWCL(r);
+        for (int h = 0; h < n_r; h++) {
+            int32_t lu = -1, ld = -1;
+            if (r >= 1 && r <= R - 2) { /* rows 0 and R-1 never own links (reading A6) */
+                const float y = cl_r[4 * h + 1], z = cl_r[4 * h + 2];
+                const float ylo = y - WY, yhi = y + WY, zlo = z - WZ, zhi = z + WZ;
+                const float *cl_up = ROWCL(r + 1), *cl_dn = ROWCL(r - 1);
+                const int nu = window_list(cl_up, ROWN(r + 1), ROWG(r + 1), use_grid, ylo, yhi, zlo, zhi, ulist);
+                const int nd = window_list(cl_dn, ROWN(r - 1), ROWG(r - 1), use_grid, ylo, yhi, zlo, zhi, dlist);
+                /* class 0: minimum over (D, u, d) lexicographically: independent of the visiting order */
+                int bu = -1, bd = -1, bdu = 1, bdd = 1;
+                float bD = 0.0f;
+                for (int a = 0; a < nu; a++)
+                    for (int b = 0; b < nd; b++) {
+                        int u = ulist[a], d = dlist[b];
+                        float t1 = cl_up[4 * u + 1] - y, t2 = y - cl_dn[4 * d + 1], ey = t1 - t2;
+                        float t3 = cl_up[4 * u + 2] - z, t4 = z - cl_dn[4 * d + 2], ez = t3 - t4;
+                        float pyy = ey * ey, pzz = ez * ez;
+                        float D = pyy + pzz;
+                        if (!(D <= D2MAX)) continue;
+                        if (bu < 0 || D < bD || (D == bD && (u < bu || (u == bu && d < bd)))) {
+                            bD = D; bu = u; bd = d;
+                        }
+                    }
+                if (bu < 0 && c->nf_bridge_rows) {
+                    const float ylo2 = y - WY2, yhi2 = y + WY2, zlo2 = z - WZ2, zhi2 = z + WZ2;
+                    if (r - 2 >= 0) { /* (du, dd) = (1, 2) */
+                        const float *cl_d2 = ROWCL(r - 2);
+                        const int nx = window_list(cl_d2, ROWN(r - 2), ROWG(r - 2), use_grid, ylo2, yhi2, zlo2, zhi2, xlist);
+                        for (int a = 0; a < nu; a++)
+                            for (int b = 0; b < nx; b++) {
+                                int u = ulist[a], d = xlist[b];
+                                float t1 = cl_up[4 * u + 1] - y, t2 = y - cl_d2[4 * d + 1], ey = (t1 + t1) - t2;
+                                float t3 = cl_up[4 * u + 2] - z, t4 = z - cl_d2[4 * d + 2], ez = (t3 + t3) - t4;
+                                float pyy = ey * ey, pzz = ez * ez;
+                                float D = pyy + pzz;
+                                if (!(D <= D2MAX1)) continue;
+                                if (bu < 0 || D < bD || (D == bD && (u < bu || (u == bu && d < bd)))) {
+                                    bD = D; bu = u; bd = d; bdu = 1; bdd = 2;
+                                }
+                            }
+                    }
+                    if (r + 2 <= R - 1) { /* (du, dd) = (2, 1); on an exact tie of D the (1, 2) pair found above stays */
+                        const float *cl_u2 = ROWCL(r + 2);
+                        const int nx = window_list(cl_u2, ROWN(r + 2), ROWG(r + 2), use_grid, ylo2, yhi2, zlo2, zhi2, xlist);
+                        for (int a = 0; a < nx; a++)
+                            for (int b = 0; b < nd; b++) {
+                                int u = xlist[a], d = dlist[b];
+                                float t1 = cl_u2[4 * u + 1] - y, t2 = y - cl_dn[4 * d + 1], ey = t1 - (t2 + t2);
+                                float t3 = cl_u2[4 * u + 2] - z, t4 = z - cl_dn[4 * d + 2], ez = t3 - (t4 + t4);
+                                float pyy = ey * ey, pzz = ez * ez;
+                                float D = pyy + pzz;
+                                if (!(D <= D2MAX1)) continue;
+                                if (bu < 0 || D < bD ||
+                                    (D == bD && bdu == 2 && (u < bu || (u == bu && d < bd)))) {
+                                    bD = D; bu = u; bd = d; bdu = 2; bdd = 1;
+                                }
+                            }
+                    }
+                }
+                if (bu >= 0) {
+                    lu = ro[r + bdu] + bu;
+                    ld = ro[r - bdd] + bd;
                 }
             }
-        up_loc[h] = bu;
-        dn_loc[h] = bd;
+            link_up[ro[r] + h] = lu;
+            link_dn[ro[r] + h] = ld;
+        }
     }
+#undef ROWCL
+#undef ROWN
+#undef ROWG
     free(ulist);
     free(dlist);
+    free(xlist);
 }
 
 /* Raw links for all instances.  link_up/link_dn: [n_clusters] GLOBAL cluster indices or -1. */
@@ -192,24 +269,7 @@ int orc_neighbours(const orc_config *c, const float *clusters, const int32_t *ro
         orc_rowgrid *grids = (orc_rowgrid *)calloc((size_t)R, sizeof(orc_rowgrid));
         if (use_grid)
             for (int r = 0; r < R; r++) grid_build(&grids[r], c, inst, r, clusters + 4 * (size_t)ro[r], ro[r + 1] - ro[r]);
-        for (int r = 0; r < R; r++) {
-            int n_r = ro[r + 1] - ro[r];
-            if (r == 0 || r == R - 1) {
-                for (int h = 0; h < n_r; h++) link_up[ro[r] + h] = link_dn[ro[r] + h] = -1;
-                continue;
-            }
-            int n_dn = ro[r] - ro[r - 1], n_up = ro[r + 2] - ro[r + 1];
-            int32_t *ul = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_r + 1));
-            int32_t *dl = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_r + 1));
-            neighbours_row(c, clusters + 4 * (size_t)ro[r - 1], n_dn, clusters + 4 * (size_t)ro[r], n_r,
-                           clusters + 4 * (size_t)ro[r + 1], n_up, &grids[r - 1], &grids[r + 1], use_grid, ul, dl);
-            for (int h = 0; h < n_r; h++) {
-                link_up[ro[r] + h] = ul[h] < 0 ? -1 : ro[r + 1] + ul[h];
-                link_dn[ro[r] + h] = dl[h] < 0 ? -1 : ro[r - 1] + dl[h];
-            }
-            free(ul);
-            free(dl);
-        }
+        neighbours_instance(c, clusters, ro, grids, use_grid, link_up, link_dn);
         if (use_grid)
             for (int r = 0; r < R; r++) grid_free(&grids[r]);
         free(grids);
@@ -615,23 +675,7 @@ int orc_track_count(const orc_config *c, const float *clusters, const int32_t *r
         {
             orc_rowgrid *grids = (orc_rowgrid *)calloc((size_t)R, sizeof(orc_rowgrid));
             for (int r = 0; r < R; r++) grid_build(&grids[r], &ci, inst, r, cl + 4 * (size_t)ro1[r], ro1[r + 1] - ro1[r]);
-            for (int r = 0; r < R; r++) {
-                int n_r = ro1[r + 1] - ro1[r];
-                if (r == 0 || r == R - 1) {
-                    for (int h = 0; h < n_r; h++) up[ro1[r] + h] = dn[ro1[r] + h] = -1;
-                    continue;
-                }
-                int32_t *ul = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_r + 1));
-                int32_t *dl = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_r + 1));
-                neighbours_row(&ci, cl + 4 * (size_t)ro1[r - 1], ro1[r] - ro1[r - 1], cl + 4 * (size_t)ro1[r], n_r,
-                               cl + 4 * (size_t)ro1[r + 1], ro1[r + 2] - ro1[r + 1], &grids[r - 1], &grids[r + 1], 1, ul, dl);
-                for (int h = 0; h < n_r; h++) {
-                    up[ro1[r] + h] = ul[h] < 0 ? -1 : ro1[r + 1] + ul[h];
-                    dn[ro1[r] + h] = dl[h] < 0 ? -1 : ro1[r - 1] + dl[h];
-                }
-                free(ul);
-                free(dl);
-            }
+            neighbours_instance(&ci, cl, ro1, grids, 1, up, dn);
             orc_clean(n, up, dn, cu, cd);
             int64_t cnt[2];
             orc_candidates(&ci, n, cu, cd, NULL, 0, NULL, NULL, 0, cnt);

@@ -37,6 +37,7 @@ class Config(C.Structure):
         ("kf_gate_sigma", C.c_double), ("kf_win_max", C.c_double), ("kf_max_gap", C.c_int32),
         ("kf_max_sinphi", C.c_double), ("kf_edge_margin", C.c_double), ("sel_min_hits", C.c_int32),
         ("grid_cell_y", C.c_float), ("grid_cell_z", C.c_float), ("bz", C.c_double),
+        ("nf_bridge_rows", C.c_int32), ("pad_", C.c_int32),
     ]
 
 
@@ -90,7 +91,7 @@ class Oracle:
                  half_angle_rad=float(np.deg2rad(10.0)), nf_win_y=2.0, nf_win_z=2.5, nf_d2_max=1.0, cand_min_hits=4,
                  cand_max_hits=CAND_MAX, kf_p0=(1.0, 1.0, 0.1, 0.1, 10.0), kf_gate_sigma=4.0, kf_win_max=3.0,
                  kf_max_gap=5, kf_max_sinphi=0.95, kf_edge_margin=2.0, sel_min_hits=10, grid_cell_y=4.0,
-                 grid_cell_z=5.0):
+                 grid_cell_z=5.0, nf_bridge_rows=0):
         self._row_x = np.ascontiguousarray(row_x, dtype=np.float32)
         c = Config()
         c.n_rows = len(self._row_x)
@@ -105,6 +106,7 @@ class Oracle:
         c.kf_gate_sigma, c.kf_win_max, c.kf_max_gap = kf_gate_sigma, kf_win_max, kf_max_gap
         c.kf_max_sinphi, c.kf_edge_margin, c.sel_min_hits = kf_max_sinphi, kf_edge_margin, sel_min_hits
         c.grid_cell_y, c.grid_cell_z, c.bz = grid_cell_y, grid_cell_z, bz
+        c.nf_bridge_rows = int(nf_bridge_rows)
         self.cfg = c
         self.n_rows = c.n_rows
         self.bz = bz

@@ -102,13 +102,82 @@ __device__ __noinline__ void search_dense(const DevGeom& g, const RowView& up, c
     }
 }
 
+// ---- class 1 (reading A2', nf_bridge_rows = 1): a hit WITHOUT an admissible adjacent pair may take one partner two
+// rows away, so that a single missing row does not break the chain.  (du, dd) = (1, 2): u in row r+1, d in row r-2;
+// (2, 1): u in row r+2, d in row r-1.  The partner two rows away is searched in the doubled window; the deviation is
+// dd * (u - h) - du * (h - d), i.e. (t1 + t1) - t2 resp. t1 - (t2 + t2); cut at 2.25 * d2max; minimum over
+// (D, du, local index of u, local index of d).  Exact evaluation order: DESIGN.md "S2 class 1".  Rare (hits next to
+// a missing cluster, and noise), so it is a plain out-of-line nested search over the grid cells.
+struct BestBridge {
+    float D;
+    int ju, jd, du;  // positions in the sorted rows r+du / r-(3-du); ju < 0 = none
+};
+
+template <bool kFarIsUp>
+__device__ __forceinline__ void bridge_pairs(const DevGeom& g, const RowView& nearr, const RowView& farr, float y, float z,
+                                             float z0, BestBridge& best) {
+    const float WY = g.nf_wy, WZ = g.nf_wz, WY2 = __fadd_rn(WY, WY), WZ2 = __fadd_rn(WZ, WZ);
+    const float dmax = __fmul_rn(g.nf_d2max, 2.25f);
+    const float ylo = __fsub_rn(y, WY), yhi = __fadd_rn(y, WY), zlo = __fsub_rn(z, WZ), zhi = __fadd_rn(z, WZ);
+    const float ylo2 = __fsub_rn(y, WY2), yhi2 = __fadd_rn(y, WY2), zlo2 = __fsub_rn(z, WZ2), zhi2 = __fadd_rn(z, WZ2);
+    const int nz0 = zbin(zlo, z0, g.inv_cz, g.nz), nz1 = zbin(zhi, z0, g.inv_cz, g.nz);
+    const int fz0 = zbin(zlo2, z0, g.inv_cz, g.nz), fz1 = zbin(zhi2, z0, g.inv_cz, g.nz);
+    const int ns0 = ybin(ylo, nearr.y0, nearr.inv_sy, g.ny), ns1 = ybin(yhi, nearr.y0, nearr.inv_sy, g.ny);
+    const int fs0 = ybin(ylo2, farr.y0, farr.inv_sy, g.ny), fs1 = ybin(yhi2, farr.y0, farr.inv_sy, g.ny);
+    const int du = kFarIsUp ? 2 : 1;
+    for (int zn = nz0; zn <= nz1; zn++) {
+        const int a0 = nearr.tbl[zn * g.ny + ns0], a1 = nearr.tbl[zn * g.ny + ns1 + 1];
+        for (int a = a0; a < a1; a++) {
+            const float2 p = nearr.yz[a];
+            if (!(ylo <= p.x && p.x <= yhi && zlo <= p.y && p.y <= zhi)) continue;
+            for (int zf = fz0; zf <= fz1; zf++) {
+                const int b0 = farr.tbl[zf * g.ny + fs0], b1 = farr.tbl[zf * g.ny + fs1 + 1];
+                for (int b = b0; b < b1; b++) {
+                    const float2 q = farr.yz[b];
+                    if (!(ylo2 <= q.x && q.x <= yhi2 && zlo2 <= q.y && q.y <= zhi2)) continue;
+                    // u = the upper partner, d = the lower one
+                    const float2 u = kFarIsUp ? q : p, d = kFarIsUp ? p : q;
+                    const int ju = kFarIsUp ? b : a, jd = kFarIsUp ? a : b;
+                    const float t1 = __fsub_rn(u.x, y), t2 = __fsub_rn(y, d.x);
+                    const float t3 = __fsub_rn(u.y, z), t4 = __fsub_rn(z, d.y);
+                    const float ey = kFarIsUp ? __fsub_rn(t1, __fadd_rn(t2, t2)) : __fsub_rn(__fadd_rn(t1, t1), t2);
+                    const float ez = kFarIsUp ? __fsub_rn(t3, __fadd_rn(t4, t4)) : __fsub_rn(__fadd_rn(t3, t3), t4);
+                    const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+                    if (!(D <= dmax)) continue;
+                    bool better = best.ju < 0 || D < best.D;
+                    if (!better && D == best.D && du == best.du) {  // (1,2) beats (2,1) on a tie; same kind: indices
+                        const uint16_t* iu = kFarIsUp ? farr.idx : nearr.idx;
+                        const uint16_t* id = kFarIsUp ? nearr.idx : farr.idx;
+                        const int cu = iu[ju], bu = iu[best.ju];
+                        better = cu < bu || (cu == bu && id[jd] < id[best.jd]);
+                    }
+                    if (better) {
+                        best.D = D;
+                        best.ju = ju;
+                        best.jd = jd;
+                        best.du = du;
+                    }
+                }
+            }
+        }
+    }
+}
+
+__device__ __noinline__ void search_bridge(const DevGeom& g, const RowView& up, const RowView& dn, const RowView& up2,
+                                           const RowView& dn2, bool has_up2, bool has_dn2, float y, float z, float z0,
+                                           BestBridge& best) {
+    if (has_dn2) bridge_pairs<false>(g, up, dn2, y, z, z0, best);  // (du, dd) = (1, 2) first: it wins exact ties
+    if (has_up2) bridge_pairs<true>(g, dn, up2, y, z, z0, best);   // (du, dd) = (2, 1)
+}
+
 __device__ __forceinline__ bool in_window(float2 h, float ylo, float yhi, float zlo, float zhi) {
     return ylo <= h.x && h.x <= yhi && zlo <= h.y && h.y <= zhi;
 }
 
-__device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const float2* my_yz,
-                                           int n, float z0, int base, int base_up,
-                                           int base_dn, int32_t* __restrict__ link_up,
+__device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const RowView up2,
+                                           const RowView dn2, bool has_up2, bool has_dn2, const float2* my_yz,
+                                           int n, float z0, int base, int base_up, int base_dn, int base_up2,
+                                           int base_dn2, int32_t* __restrict__ link_up,
                                            int32_t* __restrict__ link_dn) {
     const float WY = g.nf_wy, WZ = g.nf_wz, D2MAX = g.nf_d2max;
     const float kInf = __int_as_float(0x7f800000);
@@ -182,8 +251,18 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
         }
         // links live in SORTED space: entry base + i belongs to the i-th hit of the sorted row, values are sorted
         // global positions; coalesced stores
-        link_up[base + i] = best.ju < 0 ? -1 : base_up + best.ju;
-        link_dn[base + i] = best.jd < 0 ? -1 : base_dn + best.jd;
+        int lu = best.ju < 0 ? -1 : base_up + best.ju;
+        int ld = best.jd < 0 ? -1 : base_dn + best.jd;
+        if (g.bridge && best.ju < 0) {  // class 1: no admissible adjacent pair
+            BestBridge bb{kInf, -1, -1, 1};
+            search_bridge(g, up, dn, up2, dn2, has_up2, has_dn2, y, z, z0, bb);
+            if (bb.ju >= 0) {
+                lu = (bb.du == 2 ? base_up2 : base_up) + bb.ju;
+                ld = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
+            }
+        }
+        link_up[base + i] = lu;
+        link_dn[base + i] = ld;
     }
 }
 
@@ -235,7 +314,16 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
         dn.yz = s_yz + n_up;
     }
     __syncthreads();
-    search_row(g, up, dn, hit_yz + base, n, z0, base, base_up, base_dn, link_up, link_dn);
+    // rows two away (class 1 only): read in place
+    const bool has_up2 = r + 2 <= g.R - 1, has_dn2 = r - 2 >= 0;
+    const int base_up2 = has_up2 ? row_offsets[slab + 2] : 0, base_dn2 = has_dn2 ? row_offsets[slab - 2] : 0;
+    const int ru2 = has_up2 ? r + 2 : r, rd2 = has_dn2 ? r - 2 : r;
+    const RowView up2{hit_yz + base_up2, hit_idx + base_up2, bin_start + (size_t)(slab + (has_up2 ? 2 : 0)) * g.nzp,
+                      g.row_y0[ru2], g.row_inv_sy[ru2]};
+    const RowView dn2{hit_yz + base_dn2, hit_idx + base_dn2, bin_start + (size_t)(slab - (has_dn2 ? 2 : 0)) * g.nzp,
+                      g.row_y0[rd2], g.row_inv_sy[rd2]};
+    search_row(g, up, dn, up2, dn2, has_up2, has_dn2, hit_yz + base, n, z0, base, base_up, base_dn, base_up2, base_dn2,
+               link_up, link_dn);
 }
 
 static size_t nb_smem_bytes(const DevGeom& g) {

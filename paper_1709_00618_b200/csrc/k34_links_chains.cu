@@ -158,10 +158,13 @@ export_links_kernel(const int32_t* __restrict__ row_offsets, const uint16_t* __r
     const int slab = blockIdx.x;
     const int base = row_offsets[slab], n_all = row_offsets[slab + 1] - base;
     const int n = min(n_all, 65535);
-    const int tslab = min(max(slab + dir, 0), n_slabs - 1);
-    const int tbase = row_offsets[tslab];
+    // the target lies in the adjacent row, or two rows away where S2 bridged a missing row (reading A2'); row offsets
+    // of a neighbouring instance are never selected because a link stays inside its instance
+    const int t1 = min(max(slab + dir, 0), n_slabs - 1), t2 = min(max(slab + 2 * dir, 0), n_slabs - 1);
+    const int b1 = row_offsets[t1], b2 = row_offsets[t2], e1 = row_offsets[t1 + 1];
     for (int i = threadIdx.x; i < n; i += kChainThreads) {
         const int32_t v = link[base + i];
+        const int tbase = (v >= b1 && v < e1) ? b1 : b2;
         out[base + hit_idx[base + i]] = v < 0 ? -1 : tbase + (int32_t)hit_idx[v];
     }
     for (int i = n + threadIdx.x; i < n_all; i += kChainThreads) out[base + i] = -1;

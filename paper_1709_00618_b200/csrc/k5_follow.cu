@@ -109,17 +109,32 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
             n += pos[q] >= 0 ? 1 : 0;
         }
         float2 h[kCandMax];
-        int rb[kCandMax];
+        int rb[kCandMax];   // offset of the hit's row
+        int row[kCandMax];  // its pad row: consecutive, or one row skipped where S2 bridged a missing row (A2')
         float x[kCandMax];
+        const int slab_base0 = slab0 - r0;
 #pragma unroll
         for (int q = 0; q < kCandMax; q++) {
             h[q] = make_float2(0.0f, 0.0f);
             rb[q] = 0;
+            row[q] = r0;
             x[q] = 0.0f;
             if (q < n) {
                 h[q] = a.hit_yz[pos[q]];
-                rb[q] = a.row_offsets[slab0 + q];
-                x[q] = g.row_x[r0 + q];
+                if (q == 0) {
+                    rb[q] = a.row_offsets[slab0];
+                } else {
+                    row[q] = row[q - 1] + 1;
+                    rb[q] = a.row_offsets[slab_base0 + row[q]];
+                    if (g.bridge) {
+                        const int nb2 = a.row_offsets[slab_base0 + row[q] + 1];  // row[q] + 1 <= R: a valid entry
+                        if (pos[q] >= nb2) {
+                            row[q]++;
+                            rb[q] = nb2;
+                        }
+                    }
+                }
+                x[q] = g.row_x[row[q]];
             }
         }
         // seed from hits 0, n/2, n-1.  The state carries y and z relative to the first candidate hit: the model is
@@ -166,11 +181,16 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
             ts[2 * cs] = make_float4(st.c20, st.c21, st.c22, st.c30);
             ts[3 * cs] = make_float4(st.c31, st.c32, st.c33, st.c40);
             ts[4 * cs] = make_float4(st.c41, st.c42, st.c43, st.c44);
-            ts[5 * cs] = make_float4(yref, zref, chi2, __int_as_float(n));
-            uint16_t* rh = a.tl_rowhit + (size_t)c * g.RP + r0;
+            int span = 0;  // last own row - start row
+            uint16_t* rh = a.tl_rowhit + (size_t)c * g.RP;
 #pragma unroll
             for (int q = 0; q < kCandMax; q++)
-                if (q < n) __stcs(&rh[q], (uint16_t)(pos[q] - rb[q]));
+                if (q < n) {
+                    __stcs(&rh[row[q]], (uint16_t)(pos[q] - rb[q]));
+                    if (q > 0 && row[q] - row[q - 1] == 2) __stcs(&rh[row[q] - 1], kNoHit);  // the bridged row
+                    span = row[q] - r0;
+                }
+            ts[5 * cs] = make_float4(yref, zref, chi2, __int_as_float(n | (span << 8)));
         } else {  // no tracklet: an all-zero record, and the follower skips the candidate
             ts[5 * cs] = make_float4(0.0f, 0.0f, 0.0f, __int_as_float(0));
             zero_tracklet(g, a, c);
@@ -350,7 +370,8 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     c = mine;
                     const float4* ts = a.tl_state + c;
                     const float4 t5 = ts[5 * cs];
-                    const int n = __float_as_int(t5.w);
+                    const int nbits = __float_as_int(t5.w);  // own hits | (last own row - start row) << 8
+                    const int n = nbits & 0xff;
                     if (n > 0) {  // n == 0: the fit of the candidate's own hits failed, nothing to follow
                         const float4 t0 = ts[0], t1 = ts[cs], t2 = ts[2 * cs], t3 = ts[3 * cs], t4 = ts[4 * cs];
                         const int slab0 = a.cand_slab[c];
@@ -369,7 +390,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         nhits = n;
                         gap = 0;
                         first_row = r0;
-                        r = last_row = r0 + n - 1;
+                        r = last_row = r0 + (nbits >> 8);
                         mode = r + 1 < g.R ? kUp : kBack;
                         rn = mode == kUp ? r + 1 : r0;
                         tabA_ok = hitA_ok = tabB_ok = false;

@@ -27,6 +27,7 @@ struct DevGeom {
     float z0_a, z0_c;  // grid origin: z >= 0 side, z < 0 side
     float inv_cz;
     float nf_wy, nf_wz, nf_d2max;
+    int bridge;     // S2: 1 = a single missing row may be bridged (reading A2')
     int cand_min, cand_max;
     float p0[5];
     float gate, wmax;

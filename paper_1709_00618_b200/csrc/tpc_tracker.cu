@@ -70,6 +70,7 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     g.nf_wy = dflt(p.nf_win_y, 2.0f);
     g.nf_wz = dflt(p.nf_win_z, 2.5f);
     g.nf_d2max = dflt(p.nf_d2_max, 1.0f);
+    g.bridge = p.nf_bridge_rows != 0 ? 1 : 0;
     g.cand_min = dflt(p.cand_min_hits, 4);
     g.cand_max = dflt(p.cand_max_hits, 10);
     const float p0d[5] = {1.0f, 1.0f, 0.1f, 0.1f, 10.0f};

@@ -35,7 +35,7 @@ class Params(C.Structure):
                 ("cand_min_hits", C.c_int32), ("cand_max_hits", C.c_int32), ("kf_p0", C.c_float * 5),
                 ("kf_gate_sigma", C.c_float), ("kf_win_max", C.c_float), ("kf_max_gap", C.c_int32),
                 ("kf_max_sinphi", C.c_float), ("kf_edge_margin", C.c_float), ("sel_min_hits", C.c_int32),
-                ("grid_cell_z", C.c_float), ("grid_cells_y", C.c_int32)]
+                ("grid_cell_z", C.c_float), ("grid_cells_y", C.c_int32), ("nf_bridge_rows", C.c_int32)]
 
 
 class Geometry(C.Structure):

@@ -35,8 +35,8 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_binding_structs_match_header_sizes():
     from paper_1709_00618_b200 import tracker
-    # tpc_params_t: 3 f + 2 i + 5 f + 2 f + 1 i + 2 f + 1 i + 1 f + 1 i = 18 words
-    assert C.sizeof(tracker.Params) == 18 * 4
+    # tpc_params_t: 3 f + 2 i + 5 f + 2 f + 1 i + 2 f + 1 i + 1 f + 2 i = 19 words
+    assert C.sizeof(tracker.Params) == 19 * 4
     raw = 8 + 8 + 4 * 6 + C.sizeof(tracker.Params)  # n_rows(+pad), ptr, spe..sigma, params
     assert C.sizeof(tracker.Geometry) == (raw + 7) // 8 * 8  # tail padding to the pointer alignment
     assert C.sizeof(tracker.Output) % 8 == 0
