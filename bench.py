@@ -235,6 +235,35 @@ def run_ours(args):
     one_ms = float(np.median([a.elapsed_time(b) for a, b in ev1]))
     del fb1
 
+    # ---- the same batch with S2 row bridging on (reading A2'; not the headline reading) ------
+    trk_b = Tracker.for_event(batch, device=f"cuda:{local}", nf_bridge_rows=1, **tune)
+    trk_b.reserve(N, S)
+    trk_b.set_stream()
+    trk_b.set_stage_timing(True)
+    for _ in range(2):
+        trk_b.track_sectors_device(d_cl, d_ro, S, out)
+    evb = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)]
+    for a, b in evb:
+        a.record()
+        trk_b.track_sectors_device(d_cl, d_ro, S, out)
+        b.record()
+    torch.cuda.synchronize(dev)
+    bridge_ms = float(np.mean([a.elapsed_time(b) for a, b in evb]))
+    cb = bufs["counts"].cpu().numpy()
+    stb = [trk_b.stage_times_ms(a) for a in range(3)]
+    own_b = bufs["cluster_owner"][:evs[0].n_clusters].cpu().numpy()
+    bridge = {"reading": "nf_bridge_rows=1: a hit without an admissible adjacent pair may take one partner two rows "
+                         "away (DESIGN.md A2'); parity-tested against the oracle like the default reading",
+              "value": N / (bridge_ms * 1e-3), "unit": UNIT, "ms_per_step": bridge_ms,
+              "stage_ms": {nme: float(np.mean([x[nme] for x in stb])) for nme in stb[0]},
+              "results": {"candidates": int(cb[1]), "tracklets": int(cb[2]), "tracks": int(cb[3]),
+                          "track_hits": int(cb[4])},
+              "physics_window0": physics.report(evs[0], own_b, int(own_b.max()) + 1 if (own_b >= 0).any() else 0)}
+    trk_b.close()
+    # restore the default reading's outputs of window 0 for the physics report below
+    trk.track_sectors_device(d_cl[:n0], d_ro[:s0 * batch.n_rows + 1], s0, out)
+    torch.cuda.synchronize(dev)
+
     # ---- end to end through the host-buffer entry point -------------------------------------------------------------
     ipc = 36 * max(1, args.chunk_windows)
     max_chunk = max(int(batch.row_offsets[min(i + ipc, S) * batch.n_rows] - batch.row_offsets[i * batch.n_rows])
@@ -305,6 +334,7 @@ def run_ours(args):
                     "tracks": e2e_tracks, "timer": "host perf_counter around the blocking C-ABI calls"},
             "roofline": roof, "roofline_path_hbm": roof_path, "cpu_baseline": cpu,
             "stage_ms": stage_ms,
+            "next1_bridge_rows": bridge,
             "single_window": {"workload": "cfg4: one drift window alone (36 sector instances), L2 flushed", "ms": one_ms,
                               "clusters": n0, "clusters_per_s": n0 / (one_ms * 1e-3)},
             "results": {"candidates": int(counts[1]), "tracklets": int(counts[2]), "tracks": int(counts[3]),

@@ -113,6 +113,19 @@ struct BestBridge {
     int ju, jd, du;  // positions in the sorted rows r+du / r-(3-du); ju < 0 = none
 };
 
+// Minimum over (D, du, local index of u, local index of d) for class 1, straight-line; b.D starts at +inf, b.du at 1,
+// the (1,2) pairs are all considered before the (2,1) pairs, so a (2,1) pair never replaces a (1,2) pair on a tie.
+__device__ __forceinline__ void consider_bridge(BestBridge& b, bool adm, float D, int du, int ju, int jd,
+                                                const uint16_t* __restrict__ idx_up,
+                                                const uint16_t* __restrict__ idx_dn) {
+    bool better = adm && D < b.D;
+    if (adm && D == b.D && du == b.du) better = tie_lower(idx_up, idx_dn, ju, jd, b.ju, b.jd);
+    b.D = better ? D : b.D;
+    b.ju = better ? ju : b.ju;
+    b.jd = better ? jd : b.jd;
+    b.du = better ? du : b.du;
+}
+
 template <bool kFarIsUp>
 __device__ __forceinline__ void bridge_pairs(const DevGeom& g, const RowView& nearr, const RowView& farr, float y, float z,
                                              float z0, BestBridge& best) {
@@ -174,6 +187,7 @@ __device__ __forceinline__ bool in_window(float2 h, float ylo, float yhi, float 
     return ylo <= h.x && h.x <= yhi && zlo <= h.y && h.y <= zhi;
 }
 
+template <bool kBridge>
 __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const RowView up2,
                                            const RowView dn2, bool has_up2, bool has_dn2, const float2* my_yz,
                                            int n, float z0, int base, int base_up, int base_dn, int base_up2,
@@ -188,7 +202,12 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
         const float zlo = __fsub_rn(z, WZ), zhi = __fadd_rn(z, WZ);
         const int zb0 = zbin(zlo, z0, g.inv_cz, g.nz), zb1 = zbin(zhi, z0, g.inv_cz, g.nz);
         Best best{kInf, -1, -1};
-        if (zb1 - zb0 > 1) {  // a grid finer than the window (non-default grid_cell_z): generic exact search
+        // row r-1 window hits (the newest kNbList = 4) as (y - y_d, z - z_d) plus their positions
+        float t2a = 0.0f, t2b = 0.0f, t2c = 0.0f, t2d = 0.0f, t4a = 0.0f, t4b = 0.0f, t4c = 0.0f, t4d = 0.0f;
+        unsigned long long ld = 0ull;
+        int nd = 0;
+        const bool coarse = zb1 - zb0 <= 1;
+        if (!coarse) {  // a grid finer than the window (non-default grid_cell_z): generic exact search
             search_dense(g, up, dn, y, z, ylo, yhi, zlo, zhi, zb0, zb1, best);
         } else {
             // Flat loops over the handful of hits in the touched cells.  Row r-1 first: its window hits (the newest
@@ -197,9 +216,6 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
             // different hit counts, and branches taken by a few lanes cost the whole warp.
             const CellSeq cd = window_cells(g, dn, ylo, yhi, zb0, zb1);
             const CellSeq cu = window_cells(g, up, ylo, yhi, zb0, zb1);
-            float t2a = 0.0f, t2b = 0.0f, t2c = 0.0f, t2d = 0.0f, t4a = 0.0f, t4b = 0.0f, t4c = 0.0f, t4d = 0.0f;
-            unsigned long long ld = 0ull;
-            int nd = 0;
             const int dshift = cd.b0 - cd.na, ushift = cu.b0 - cu.na;
             for (int k = 0; k < cd.nt; k++) {
                 const int j = k < cd.na ? cd.a0 + k : k + dshift;
@@ -252,20 +268,99 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
         // links live in SORTED space: entry base + i belongs to the i-th hit of the sorted row, values are sorted
         // global positions; coalesced stores
         int lu = best.ju < 0 ? -1 : base_up + best.ju;
-        int ld = best.jd < 0 ? -1 : base_dn + best.jd;
-        if (g.bridge && best.ju < 0) {  // class 1: no admissible adjacent pair
+        int ldn = best.jd < 0 ? -1 : base_dn + best.jd;
+        if (kBridge && best.ju < 0) {  // class 1 (reading A2'): no admissible adjacent pair
             BestBridge bb{kInf, -1, -1, 1};
-            search_bridge(g, up, dn, up2, dn2, has_up2, has_dn2, y, z, z0, bb);
+            bool generic = !coarse;
+            if (coarse) {
+                // row r+1 window hits into registers as (y_u - y, z_u - z), like the row r-1 list above
+                const CellSeq cu = window_cells(g, up, ylo, yhi, zb0, zb1);
+                const int ushift = cu.b0 - cu.na;
+                float t1a = 0.0f, t1b = 0.0f, t1c = 0.0f, t1d = 0.0f, t3a = 0.0f, t3b = 0.0f, t3c = 0.0f, t3d = 0.0f;
+                unsigned long long lup = 0ull;
+                int nu = 0;
+                for (int k = 0; k < cu.nt; k++) {
+                    const int j = k < cu.na ? cu.a0 + k : k + ushift;
+                    const float2 u = up.yz[j];
+                    const bool in = in_window(u, ylo, yhi, zlo, zhi);
+                    t1d = in ? t1c : t1d; t1c = in ? t1b : t1c; t1b = in ? t1a : t1b; t1a = in ? __fsub_rn(u.x, y) : t1a;
+                    t3d = in ? t3c : t3d; t3c = in ? t3b : t3c; t3b = in ? t3a : t3b; t3a = in ? __fsub_rn(u.y, z) : t3a;
+                    lup = in ? ((lup << 16) | (unsigned long long)j) : lup;
+                    nu += in ? 1 : 0;
+                }
+                generic = nu > kNbList || nd > kNbList;
+                if (!generic && (nu > 0 || nd > 0)) {
+                    const float WY2 = __fadd_rn(WY, WY), WZ2 = __fadd_rn(WZ, WZ), dmax = __fmul_rn(D2MAX, 2.25f);
+                    const float ylo2 = __fsub_rn(y, WY2), yhi2 = __fadd_rn(y, WY2);
+                    const float zlo2 = __fsub_rn(z, WZ2), zhi2 = __fadd_rn(z, WZ2);
+                    const int fz0 = zbin(zlo2, z0, g.inv_cz, g.nz), fz1 = zbin(zhi2, z0, g.inv_cz, g.nz);
+                    if (nu > 0 && has_dn2) {  // (du, dd) = (1, 2): u from the row r+1 list, d in row r-2
+                        const int fs0 = ybin(ylo2, dn2.y0, dn2.inv_sy, g.ny), fs1 = ybin(yhi2, dn2.y0, dn2.inv_sy, g.ny) + 1;
+                        for (int zf = fz0; zf <= fz1; zf++) {
+                            const int b1 = dn2.tbl[zf * g.ny + fs1];
+                            for (int b = dn2.tbl[zf * g.ny + fs0]; b < b1; b++) {
+                                const float2 d = dn2.yz[b];
+                                const bool din = in_window(d, ylo2, yhi2, zlo2, zhi2);
+                                const float t2 = __fsub_rn(y, d.x), t4 = __fsub_rn(z, d.y);
+#define TPC_NB_BRIDGE_A(T1, T3, Q)                                                                           \
+    {                                                                                                        \
+        const float ey = __fsub_rn(__fadd_rn(T1, T1), t2), ez = __fsub_rn(__fadd_rn(T3, T3), t4);            \
+        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                                     \
+        consider_bridge(bb, din && nu > Q && D <= dmax, D, 1, (int)((lup >> (16 * Q)) & 0xffffull), b, up.idx, \
+                        dn2.idx);                                                                            \
+    }
+                                TPC_NB_BRIDGE_A(t1a, t3a, 0)
+                                if (nu > 1) {
+                                    TPC_NB_BRIDGE_A(t1b, t3b, 1)
+                                    TPC_NB_BRIDGE_A(t1c, t3c, 2)
+                                    TPC_NB_BRIDGE_A(t1d, t3d, 3)
+                                }
+#undef TPC_NB_BRIDGE_A
+                            }
+                        }
+                    }
+                    if (nd > 0 && has_up2) {  // (du, dd) = (2, 1): u in row r+2, d from the row r-1 list
+                        const int fs0 = ybin(ylo2, up2.y0, up2.inv_sy, g.ny), fs1 = ybin(yhi2, up2.y0, up2.inv_sy, g.ny) + 1;
+                        for (int zf = fz0; zf <= fz1; zf++) {
+                            const int a1 = up2.tbl[zf * g.ny + fs1];
+                            for (int a = up2.tbl[zf * g.ny + fs0]; a < a1; a++) {
+                                const float2 u = up2.yz[a];
+                                const bool uin = in_window(u, ylo2, yhi2, zlo2, zhi2);
+                                const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
+#define TPC_NB_BRIDGE_B(T2, T4, Q)                                                                          \
+    {                                                                                                       \
+        const float ey = __fsub_rn(t1, __fadd_rn(T2, T2)), ez = __fsub_rn(t3, __fadd_rn(T4, T4));           \
+        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                                    \
+        consider_bridge(bb, uin && nd > Q && D <= dmax, D, 2, a, (int)((ld >> (16 * Q)) & 0xffffull), up2.idx, \
+                        dn.idx);                                                                            \
+    }
+                                TPC_NB_BRIDGE_B(t2a, t4a, 0)
+                                if (nd > 1) {
+                                    TPC_NB_BRIDGE_B(t2b, t4b, 1)
+                                    TPC_NB_BRIDGE_B(t2c, t4c, 2)
+                                    TPC_NB_BRIDGE_B(t2d, t4d, 3)
+                                }
+#undef TPC_NB_BRIDGE_B
+                            }
+                        }
+                    }
+                }
+            }
+            if (generic) {  // dense spot or a fine grid: plain nested search
+                bb = BestBridge{kInf, -1, -1, 1};
+                search_bridge(g, up, dn, up2, dn2, has_up2, has_dn2, y, z, z0, bb);
+            }
             if (bb.ju >= 0) {
                 lu = (bb.du == 2 ? base_up2 : base_up) + bb.ju;
-                ld = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
+                ldn = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
             }
         }
         link_up[base + i] = lu;
-        link_dn[base + i] = ld;
+        link_dn[base + i] = ldn;
     }
 }
 
+template <bool kBridge>
 __global__ void __launch_bounds__(kNbThreads)
 neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
                   const float2* __restrict__ hit_yz, const uint16_t* __restrict__ hit_idx,
@@ -322,7 +417,7 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
                       g.row_y0[ru2], g.row_inv_sy[ru2]};
     const RowView dn2{hit_yz + base_dn2, hit_idx + base_dn2, bin_start + (size_t)(slab - (has_dn2 ? 2 : 0)) * g.nzp,
                       g.row_y0[rd2], g.row_inv_sy[rd2]};
-    search_row(g, up, dn, up2, dn2, has_up2, has_dn2, hit_yz + base, n, z0, base, base_up, base_dn, base_up2, base_dn2,
+    search_row<kBridge>(g, up, dn, up2, dn2, has_up2, has_dn2, hit_yz + base, n, z0, base, base_up, base_dn, base_up2, base_dn2,
                link_up, link_dn);
 }
 
@@ -333,8 +428,12 @@ static size_t nb_smem_bytes(const DevGeom& g) {
 int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s) {
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
-    neighbours_kernel<<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
-                                                                  w.up_raw, w.dn_raw);
+    if (g.bridge)
+        neighbours_kernel<true><<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
+                                                                            w.bin_start, w.up_raw, w.dn_raw);
+    else
+        neighbours_kernel<false><<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
+                                                                             w.bin_start, w.up_raw, w.dn_raw);
     return 1;
 }
 
