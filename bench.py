@@ -236,7 +236,7 @@ def run_ours(args):
     del fb1
 
     # ---- the same batch with S2 row bridging on (reading A2'; not the headline reading) ------
-    trk_b = Tracker.for_event(batch, device=f"cuda:{local}", nf_bridge_rows=1, **tune)
+    trk_b = Tracker.for_event(batch, device=f"cuda:{local}", **{**tune, "nf_bridge_rows": 1})
     trk_b.reserve(N, S)
     trk_b.set_stream()
     trk_b.set_stage_timing(True)

@@ -187,12 +187,142 @@ __device__ __forceinline__ bool in_window(float2 h, float ylo, float yhi, float 
     return ylo <= h.x && h.x <= yhi && zlo <= h.y && h.y <= zhi;
 }
 
+constexpr int kNbTodo = 1024;  // class-1 hits of a row deferred to the second phase (more are searched in place)
+
+// Window hits of one adjacent row as a register list: (first coordinate difference, second) of the newest four,
+// their sorted positions (newest in the low 16 bits), and how many there are.
+struct NearList {
+    float pa, pb, pc, pd, qa, qb, qc, qd;
+    unsigned long long pos;
+    int n;
+};
+
+// kUp: the list holds (y_u - y, z_u - z) of row r+1; else (y - y_d, z - z_d) of row r-1.
+template <bool kUp>
+__device__ __forceinline__ NearList near_list(const DevGeom& g, const RowView& row, float y, float z, float ylo,
+                                              float yhi, float zlo, float zhi, int zb0, int zb1) {
+    const CellSeq c = window_cells(g, row, ylo, yhi, zb0, zb1);
+    const int shift = c.b0 - c.na;
+    NearList l{0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0ull, 0};
+    for (int k = 0; k < c.nt; k++) {
+        const int j = k < c.na ? c.a0 + k : k + shift;
+        const float2 h = row.yz[j];
+        const bool in = in_window(h, ylo, yhi, zlo, zhi);
+        const float p = kUp ? __fsub_rn(h.x, y) : __fsub_rn(y, h.x), q = kUp ? __fsub_rn(h.y, z) : __fsub_rn(z, h.y);
+        l.pd = in ? l.pc : l.pd; l.pc = in ? l.pb : l.pc; l.pb = in ? l.pa : l.pb; l.pa = in ? p : l.pa;
+        l.qd = in ? l.qc : l.qd; l.qc = in ? l.qb : l.qc; l.qb = in ? l.qa : l.qb; l.qa = in ? q : l.qa;
+        l.pos = in ? ((l.pos << 16) | (unsigned long long)j) : l.pos;
+        l.n += in ? 1 : 0;
+    }
+    return l;
+}
+
+// The cells of the doubled window in a row two away, as one sequence of up to three contiguous ranges.
+struct FarSeq {
+    int s0, n0, s1, n1, s2, nt;
+};
+
+__device__ __forceinline__ FarSeq far_cells(const DevGeom& g, const RowView& row, float ylo2, float yhi2, int fz0,
+                                            int fz1) {
+    const int fs0 = ybin(ylo2, row.y0, row.inv_sy, g.ny), fs1 = ybin(yhi2, row.y0, row.inv_sy, g.ny) + 1;
+    FarSeq f{0, 0, 0, 0, 0, 0};
+    f.s0 = row.tbl[fz0 * g.ny + fs0];
+    f.n0 = (int)row.tbl[fz0 * g.ny + fs1] - f.s0;
+    f.nt = f.n0;
+    if (fz1 > fz0) {
+        f.s1 = row.tbl[(fz0 + 1) * g.ny + fs0];
+        f.n1 = (int)row.tbl[(fz0 + 1) * g.ny + fs1] - f.s1;
+        f.nt += f.n1;
+    }
+    if (fz1 > fz0 + 1) {
+        f.s2 = row.tbl[(fz0 + 2) * g.ny + fs0];
+        f.nt += (int)row.tbl[(fz0 + 2) * g.ny + fs1] - f.s2;
+    }
+    return f;
+}
+
+__device__ __forceinline__ int far_pos(const FarSeq& f, int k) {
+    return k < f.n0 ? f.s0 + k : (k < f.n0 + f.n1 ? f.s1 + (k - f.n0) : f.s2 + (k - f.n0 - f.n1));
+}
+
+// Class-1 search of one hit (see above search_bridge for the reading).  Flat loops over the cells of the rows two
+// away, paired with the register lists of the adjacent rows; dense spots and fine grids take the nested search.
+__device__ __forceinline__ BestBridge bridge_hit(const DevGeom& g, const RowView& up, const RowView& dn,
+                                                 const RowView& up2, const RowView& dn2, bool has_up2, bool has_dn2,
+                                                 float y, float z, float z0) {
+    const float WY = g.nf_wy, WZ = g.nf_wz;
+    const float kInf = __int_as_float(0x7f800000);
+    BestBridge bb{kInf, -1, -1, 1};
+    const float ylo = __fsub_rn(y, WY), yhi = __fadd_rn(y, WY), zlo = __fsub_rn(z, WZ), zhi = __fadd_rn(z, WZ);
+    const int zb0 = zbin(zlo, z0, g.inv_cz, g.nz), zb1 = zbin(zhi, z0, g.inv_cz, g.nz);
+    const float WY2 = __fadd_rn(WY, WY), WZ2 = __fadd_rn(WZ, WZ), dmax = __fmul_rn(g.nf_d2max, 2.25f);
+    const float ylo2 = __fsub_rn(y, WY2), yhi2 = __fadd_rn(y, WY2), zlo2 = __fsub_rn(z, WZ2), zhi2 = __fadd_rn(z, WZ2);
+    const int fz0 = zbin(zlo2, z0, g.inv_cz, g.nz), fz1 = zbin(zhi2, z0, g.inv_cz, g.nz);
+    bool generic = zb1 - zb0 > 1 || fz1 - fz0 > 2;
+    if (!generic) {
+        const NearList lu = near_list<true>(g, up, y, z, ylo, yhi, zlo, zhi, zb0, zb1);
+        const NearList ld = near_list<false>(g, dn, y, z, ylo, yhi, zlo, zhi, zb0, zb1);
+        generic = lu.n > kNbList || ld.n > kNbList;
+        if (!generic && lu.n > 0 && has_dn2) {  // (du, dd) = (1, 2): u from the row r+1 list, d in row r-2
+            const FarSeq f = far_cells(g, dn2, ylo2, yhi2, fz0, fz1);
+            for (int k = 0; k < f.nt; k++) {
+                const int b = far_pos(f, k);
+                const float2 d = dn2.yz[b];
+                const bool din = in_window(d, ylo2, yhi2, zlo2, zhi2);
+                const float t2 = __fsub_rn(y, d.x), t4 = __fsub_rn(z, d.y);
+#define TPC_NB_BRIDGE_A(T1, T3, Q)                                                                             \
+    {                                                                                                          \
+        const float ey = __fsub_rn(__fadd_rn(T1, T1), t2), ez = __fsub_rn(__fadd_rn(T3, T3), t4);              \
+        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                                       \
+        consider_bridge(bb, din && lu.n > Q && D <= dmax, D, 1, (int)((lu.pos >> (16 * Q)) & 0xffffull), b, up.idx, \
+                        dn2.idx);                                                                              \
+    }
+                TPC_NB_BRIDGE_A(lu.pa, lu.qa, 0)
+                if (lu.n > 1) {
+                    TPC_NB_BRIDGE_A(lu.pb, lu.qb, 1)
+                    TPC_NB_BRIDGE_A(lu.pc, lu.qc, 2)
+                    TPC_NB_BRIDGE_A(lu.pd, lu.qd, 3)
+                }
+#undef TPC_NB_BRIDGE_A
+            }
+        }
+        if (!generic && ld.n > 0 && has_up2) {  // (du, dd) = (2, 1): u in row r+2, d from the row r-1 list
+            const FarSeq f = far_cells(g, up2, ylo2, yhi2, fz0, fz1);
+            for (int k = 0; k < f.nt; k++) {
+                const int a = far_pos(f, k);
+                const float2 u = up2.yz[a];
+                const bool uin = in_window(u, ylo2, yhi2, zlo2, zhi2);
+                const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
+#define TPC_NB_BRIDGE_B(T2, T4, Q)                                                                             \
+    {                                                                                                          \
+        const float ey = __fsub_rn(t1, __fadd_rn(T2, T2)), ez = __fsub_rn(t3, __fadd_rn(T4, T4));              \
+        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                                       \
+        consider_bridge(bb, uin && ld.n > Q && D <= dmax, D, 2, a, (int)((ld.pos >> (16 * Q)) & 0xffffull), up2.idx, \
+                        dn.idx);                                                                               \
+    }
+                TPC_NB_BRIDGE_B(ld.pa, ld.qa, 0)
+                if (ld.n > 1) {
+                    TPC_NB_BRIDGE_B(ld.pb, ld.qb, 1)
+                    TPC_NB_BRIDGE_B(ld.pc, ld.qc, 2)
+                    TPC_NB_BRIDGE_B(ld.pd, ld.qd, 3)
+                }
+#undef TPC_NB_BRIDGE_B
+            }
+        }
+    }
+    if (generic) {
+        bb = BestBridge{kInf, -1, -1, 1};
+        search_bridge(g, up, dn, up2, dn2, has_up2, has_dn2, y, z, z0, bb);
+    }
+    return bb;
+}
+
 template <bool kBridge>
 __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const RowView up2,
                                            const RowView dn2, bool has_up2, bool has_dn2, const float2* my_yz,
                                            int n, float z0, int base, int base_up, int base_dn, int base_up2,
                                            int base_dn2, int32_t* __restrict__ link_up,
-                                           int32_t* __restrict__ link_dn) {
+                                           int32_t* __restrict__ link_dn, unsigned* s_ntodo, uint16_t* s_todo) {
     const float WY = g.nf_wy, WZ = g.nf_wz, D2MAX = g.nf_d2max;
     const float kInf = __int_as_float(0x7f800000);
     for (int i = threadIdx.x; i < n; i += kNbThreads) {
@@ -269,94 +399,35 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
         // global positions; coalesced stores
         int lu = best.ju < 0 ? -1 : base_up + best.ju;
         int ldn = best.jd < 0 ? -1 : base_dn + best.jd;
-        if (kBridge && best.ju < 0) {  // class 1 (reading A2'): no admissible adjacent pair
-            BestBridge bb{kInf, -1, -1, 1};
-            bool generic = !coarse;
-            if (coarse) {
-                // row r+1 window hits into registers as (y_u - y, z_u - z), like the row r-1 list above
-                const CellSeq cu = window_cells(g, up, ylo, yhi, zb0, zb1);
-                const int ushift = cu.b0 - cu.na;
-                float t1a = 0.0f, t1b = 0.0f, t1c = 0.0f, t1d = 0.0f, t3a = 0.0f, t3b = 0.0f, t3c = 0.0f, t3d = 0.0f;
-                unsigned long long lup = 0ull;
-                int nu = 0;
-                for (int k = 0; k < cu.nt; k++) {
-                    const int j = k < cu.na ? cu.a0 + k : k + ushift;
-                    const float2 u = up.yz[j];
-                    const bool in = in_window(u, ylo, yhi, zlo, zhi);
-                    t1d = in ? t1c : t1d; t1c = in ? t1b : t1c; t1b = in ? t1a : t1b; t1a = in ? __fsub_rn(u.x, y) : t1a;
-                    t3d = in ? t3c : t3d; t3c = in ? t3b : t3c; t3b = in ? t3a : t3b; t3a = in ? __fsub_rn(u.y, z) : t3a;
-                    lup = in ? ((lup << 16) | (unsigned long long)j) : lup;
-                    nu += in ? 1 : 0;
+        if (kBridge && best.ju < 0) {
+            // class 1 (reading A2'): no admissible adjacent pair.  About one hit in five gets here, so the search is
+            // deferred: the hit goes on a list in shared memory and the list is worked off with all lanes busy
+            const unsigned slot = atomicAdd(s_ntodo, 1u);
+            if (slot < (unsigned)kNbTodo) {
+                s_todo[slot] = (uint16_t)i;
+            } else {  // list full (very long rows): search now
+                const BestBridge bb = bridge_hit(g, up, dn, up2, dn2, has_up2, has_dn2, y, z, z0);
+                if (bb.ju >= 0) {
+                    lu = (bb.du == 2 ? base_up2 : base_up) + bb.ju;
+                    ldn = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
                 }
-                generic = nu > kNbList || nd > kNbList;
-                if (!generic && (nu > 0 || nd > 0)) {
-                    const float WY2 = __fadd_rn(WY, WY), WZ2 = __fadd_rn(WZ, WZ), dmax = __fmul_rn(D2MAX, 2.25f);
-                    const float ylo2 = __fsub_rn(y, WY2), yhi2 = __fadd_rn(y, WY2);
-                    const float zlo2 = __fsub_rn(z, WZ2), zhi2 = __fadd_rn(z, WZ2);
-                    const int fz0 = zbin(zlo2, z0, g.inv_cz, g.nz), fz1 = zbin(zhi2, z0, g.inv_cz, g.nz);
-                    if (nu > 0 && has_dn2) {  // (du, dd) = (1, 2): u from the row r+1 list, d in row r-2
-                        const int fs0 = ybin(ylo2, dn2.y0, dn2.inv_sy, g.ny), fs1 = ybin(yhi2, dn2.y0, dn2.inv_sy, g.ny) + 1;
-                        for (int zf = fz0; zf <= fz1; zf++) {
-                            const int b1 = dn2.tbl[zf * g.ny + fs1];
-                            for (int b = dn2.tbl[zf * g.ny + fs0]; b < b1; b++) {
-                                const float2 d = dn2.yz[b];
-                                const bool din = in_window(d, ylo2, yhi2, zlo2, zhi2);
-                                const float t2 = __fsub_rn(y, d.x), t4 = __fsub_rn(z, d.y);
-#define TPC_NB_BRIDGE_A(T1, T3, Q)                                                                           \
-    {                                                                                                        \
-        const float ey = __fsub_rn(__fadd_rn(T1, T1), t2), ez = __fsub_rn(__fadd_rn(T3, T3), t4);            \
-        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                                     \
-        consider_bridge(bb, din && nu > Q && D <= dmax, D, 1, (int)((lup >> (16 * Q)) & 0xffffull), b, up.idx, \
-                        dn2.idx);                                                                            \
-    }
-                                TPC_NB_BRIDGE_A(t1a, t3a, 0)
-                                if (nu > 1) {
-                                    TPC_NB_BRIDGE_A(t1b, t3b, 1)
-                                    TPC_NB_BRIDGE_A(t1c, t3c, 2)
-                                    TPC_NB_BRIDGE_A(t1d, t3d, 3)
-                                }
-#undef TPC_NB_BRIDGE_A
-                            }
-                        }
-                    }
-                    if (nd > 0 && has_up2) {  // (du, dd) = (2, 1): u in row r+2, d from the row r-1 list
-                        const int fs0 = ybin(ylo2, up2.y0, up2.inv_sy, g.ny), fs1 = ybin(yhi2, up2.y0, up2.inv_sy, g.ny) + 1;
-                        for (int zf = fz0; zf <= fz1; zf++) {
-                            const int a1 = up2.tbl[zf * g.ny + fs1];
-                            for (int a = up2.tbl[zf * g.ny + fs0]; a < a1; a++) {
-                                const float2 u = up2.yz[a];
-                                const bool uin = in_window(u, ylo2, yhi2, zlo2, zhi2);
-                                const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
-#define TPC_NB_BRIDGE_B(T2, T4, Q)                                                                          \
-    {                                                                                                       \
-        const float ey = __fsub_rn(t1, __fadd_rn(T2, T2)), ez = __fsub_rn(t3, __fadd_rn(T4, T4));           \
-        const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                                    \
-        consider_bridge(bb, uin && nd > Q && D <= dmax, D, 2, a, (int)((ld >> (16 * Q)) & 0xffffull), up2.idx, \
-                        dn.idx);                                                                            \
-    }
-                                TPC_NB_BRIDGE_B(t2a, t4a, 0)
-                                if (nd > 1) {
-                                    TPC_NB_BRIDGE_B(t2b, t4b, 1)
-                                    TPC_NB_BRIDGE_B(t2c, t4c, 2)
-                                    TPC_NB_BRIDGE_B(t2d, t4d, 3)
-                                }
-#undef TPC_NB_BRIDGE_B
-                            }
-                        }
-                    }
-                }
-            }
-            if (generic) {  // dense spot or a fine grid: plain nested search
-                bb = BestBridge{kInf, -1, -1, 1};
-                search_bridge(g, up, dn, up2, dn2, has_up2, has_dn2, y, z, z0, bb);
-            }
-            if (bb.ju >= 0) {
-                lu = (bb.du == 2 ? base_up2 : base_up) + bb.ju;
-                ldn = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
             }
         }
         link_up[base + i] = lu;
         link_dn[base + i] = ldn;
+    }
+    if (kBridge) {
+        __syncthreads();
+        const int n_todo = min((int)*s_ntodo, kNbTodo);
+        for (int t = threadIdx.x; t < n_todo; t += kNbThreads) {
+            const int i = s_todo[t];
+            const float2 h = my_yz[i];
+            const BestBridge bb = bridge_hit(g, up, dn, up2, dn2, has_up2, has_dn2, h.x, h.y, z0);
+            if (bb.ju >= 0) {
+                link_up[base + i] = (bb.du == 2 ? base_up2 : base_up) + bb.ju;
+                link_dn[base + i] = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
+            }
+        }
     }
 }
 
@@ -367,6 +438,9 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
                   const uint16_t* __restrict__ bin_start, int32_t* __restrict__ link_up,
                   int32_t* __restrict__ link_dn) {
     extern __shared__ __align__(16) unsigned char sm_raw[];
+    __shared__ unsigned s_ntodo;
+    __shared__ uint16_t s_todo[kBridge ? kNbTodo : 1];
+    if (threadIdx.x == 0) s_ntodo = 0u;
     const int slab = blockIdx.x;
     const int inst = slab / g.R, r = slab - inst * g.R;
     const int base = row_offsets[slab];
@@ -418,7 +492,7 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
     const RowView dn2{hit_yz + base_dn2, hit_idx + base_dn2, bin_start + (size_t)(slab - (has_dn2 ? 2 : 0)) * g.nzp,
                       g.row_y0[rd2], g.row_inv_sy[rd2]};
     search_row<kBridge>(g, up, dn, up2, dn2, has_up2, has_dn2, hit_yz + base, n, z0, base, base_up, base_dn, base_up2, base_dn2,
-               link_up, link_dn);
+               link_up, link_dn, &s_ntodo, s_todo);
 }
 
 static size_t nb_smem_bytes(const DevGeom& g) {
