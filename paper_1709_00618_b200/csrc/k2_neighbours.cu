@@ -187,7 +187,6 @@ __device__ __forceinline__ bool in_window(float2 h, float ylo, float yhi, float 
     return ylo <= h.x && h.x <= yhi && zlo <= h.y && h.y <= zhi;
 }
 
-constexpr int kNbTodo = 1024;  // class-1 hits of a row deferred to the second phase (more are searched in place)
 
 // Window hits of one adjacent row as a register list: (first coordinate difference, second) of the newest four,
 // their sorted positions (newest in the low 16 bits), and how many there are.
@@ -317,12 +316,9 @@ __device__ __forceinline__ BestBridge bridge_hit(const DevGeom& g, const RowView
     return bb;
 }
 
-template <bool kBridge>
-__device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const RowView up2,
-                                           const RowView dn2, bool has_up2, bool has_dn2, const float2* my_yz,
-                                           int n, float z0, int base, int base_up, int base_dn, int base_up2,
-                                           int base_dn2, int32_t* __restrict__ link_up,
-                                           int32_t* __restrict__ link_dn, unsigned* s_ntodo, uint16_t* s_todo) {
+__device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const float2* my_yz,
+                                           int n, float z0, int base, int base_up, int base_dn,
+                                           int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
     const float WY = g.nf_wy, WZ = g.nf_wz, D2MAX = g.nf_d2max;
     const float kInf = __int_as_float(0x7f800000);
     for (int i = threadIdx.x; i < n; i += kNbThreads) {
@@ -399,48 +395,17 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
         // global positions; coalesced stores
         int lu = best.ju < 0 ? -1 : base_up + best.ju;
         int ldn = best.jd < 0 ? -1 : base_dn + best.jd;
-        if (kBridge && best.ju < 0) {
-            // class 1 (reading A2'): no admissible adjacent pair.  About one hit in five gets here, so the search is
-            // deferred: the hit goes on a list in shared memory and the list is worked off with all lanes busy
-            const unsigned slot = atomicAdd(s_ntodo, 1u);
-            if (slot < (unsigned)kNbTodo) {
-                s_todo[slot] = (uint16_t)i;
-            } else {  // list full (very long rows): search now
-                const BestBridge bb = bridge_hit(g, up, dn, up2, dn2, has_up2, has_dn2, y, z, z0);
-                if (bb.ju >= 0) {
-                    lu = (bb.du == 2 ? base_up2 : base_up) + bb.ju;
-                    ldn = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
-                }
-            }
-        }
         link_up[base + i] = lu;
         link_dn[base + i] = ldn;
     }
-    if (kBridge) {
-        __syncthreads();
-        const int n_todo = min((int)*s_ntodo, kNbTodo);
-        for (int t = threadIdx.x; t < n_todo; t += kNbThreads) {
-            const int i = s_todo[t];
-            const float2 h = my_yz[i];
-            const BestBridge bb = bridge_hit(g, up, dn, up2, dn2, has_up2, has_dn2, h.x, h.y, z0);
-            if (bb.ju >= 0) {
-                link_up[base + i] = (bb.du == 2 ? base_up2 : base_up) + bb.ju;
-                link_dn[base + i] = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
-            }
-        }
-    }
 }
 
-template <bool kBridge>
 __global__ void __launch_bounds__(kNbThreads)
 neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
                   const float2* __restrict__ hit_yz, const uint16_t* __restrict__ hit_idx,
                   const uint16_t* __restrict__ bin_start, int32_t* __restrict__ link_up,
                   int32_t* __restrict__ link_dn) {
     extern __shared__ __align__(16) unsigned char sm_raw[];
-    __shared__ unsigned s_ntodo;
-    __shared__ uint16_t s_todo[kBridge ? kNbTodo : 1];
-    if (threadIdx.x == 0) s_ntodo = 0u;
     const int slab = blockIdx.x;
     const int inst = slab / g.R, r = slab - inst * g.R;
     const int base = row_offsets[slab];
@@ -483,16 +448,72 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
         dn.yz = s_yz + n_up;
     }
     __syncthreads();
-    // rows two away (class 1 only): read in place
+    search_row(g, up, dn, hit_yz + base, n, z0, base, base_up, base_dn, link_up, link_dn);
+}
+
+// Class 1 (reading A2', nf_bridge_rows = 1) as its own pass: one WARP per (instance,row) slab reads the row's raw
+// up-links, queues the hits without an adjacent pair (about one in five) and searches 32 of them at a time, so the
+// lanes stay busy and the tuned class-0 kernel above is untouched.  All rows are read in place (L2).
+constexpr int kBrThreads = 128;
+
+__global__ void __launch_bounds__(kBrThreads)
+bridge_links_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
+                    const float2* __restrict__ hit_yz, const uint16_t* __restrict__ hit_idx,
+                    const uint16_t* __restrict__ bin_start, int32_t* __restrict__ link_up,
+                    int32_t* __restrict__ link_dn, int n_slabs) {
+    __shared__ uint16_t s_queue[kBrThreads / 32][64];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int slab = blockIdx.x * (kBrThreads / 32) + wid;
+    if (slab >= n_slabs) return;
+    const int inst = slab / g.R, r = slab - inst * g.R;
+    if (r == 0 || r == g.R - 1) return;  // first and last row never own links (reading A6)
+    const int base = row_offsets[slab];
+    const int n = min(row_offsets[slab + 1] - base, 65535);
+    if (n == 0) return;
+    const float z0 = grid_z0(g, inst);
     const bool has_up2 = r + 2 <= g.R - 1, has_dn2 = r - 2 >= 0;
+    const int base_dn = row_offsets[slab - 1], base_up = row_offsets[slab + 1];
     const int base_up2 = has_up2 ? row_offsets[slab + 2] : 0, base_dn2 = has_dn2 ? row_offsets[slab - 2] : 0;
     const int ru2 = has_up2 ? r + 2 : r, rd2 = has_dn2 ? r - 2 : r;
+    const RowView up{hit_yz + base_up, hit_idx + base_up, bin_start + (size_t)(slab + 1) * g.nzp, g.row_y0[r + 1],
+                     g.row_inv_sy[r + 1]};
+    const RowView dn{hit_yz + base_dn, hit_idx + base_dn, bin_start + (size_t)(slab - 1) * g.nzp, g.row_y0[r - 1],
+                     g.row_inv_sy[r - 1]};
     const RowView up2{hit_yz + base_up2, hit_idx + base_up2, bin_start + (size_t)(slab + (has_up2 ? 2 : 0)) * g.nzp,
                       g.row_y0[ru2], g.row_inv_sy[ru2]};
     const RowView dn2{hit_yz + base_dn2, hit_idx + base_dn2, bin_start + (size_t)(slab - (has_dn2 ? 2 : 0)) * g.nzp,
                       g.row_y0[rd2], g.row_inv_sy[rd2]};
-    search_row<kBridge>(g, up, dn, up2, dn2, has_up2, has_dn2, hit_yz + base, n, z0, base, base_up, base_dn, base_up2, base_dn2,
-               link_up, link_dn, &s_ntodo, s_todo);
+    uint16_t* queue = s_queue[wid];
+    const unsigned lt = (1u << lane) - 1u;
+    int qn = 0;  // queued hits (warp-uniform), < 32 between rounds
+    for (int i0 = 0; i0 < n || qn > 0; i0 += 32) {
+        const int i = i0 + lane;
+        const bool need = i < n && link_up[base + i] < 0;
+        const unsigned m = __ballot_sync(0xffffffffu, need);
+        if (need) queue[qn + __popc(m & lt)] = (uint16_t)i;
+        qn += __popc(m);
+        __syncwarp();
+        const bool last = i0 + 32 >= n;
+        if (qn >= 32 || (last && qn > 0)) {
+            const int take = min(qn, 32);
+            if (lane < take) {
+                const int j = queue[lane];
+                const float2 h = hit_yz[base + j];
+                const BestBridge bb = bridge_hit(g, up, dn, up2, dn2, has_up2, has_dn2, h.x, h.y, z0);
+                if (bb.ju >= 0) {
+                    link_up[base + j] = (bb.du == 2 ? base_up2 : base_up) + bb.ju;
+                    link_dn[base + j] = (bb.du == 2 ? base_dn : base_dn2) + bb.jd;
+                }
+            }
+            __syncwarp();
+            const uint16_t moved = lane + 32 < qn ? queue[lane + 32] : (uint16_t)0;
+            __syncwarp();
+            if (lane + 32 < qn) queue[lane] = moved;
+            qn -= take;
+            __syncwarp();
+        }
+        if (last && qn == 0) break;
+    }
 }
 
 static size_t nb_smem_bytes(const DevGeom& g) {
@@ -502,12 +523,13 @@ static size_t nb_smem_bytes(const DevGeom& g) {
 int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s) {
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
-    if (g.bridge)
-        neighbours_kernel<true><<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
-                                                                            w.bin_start, w.up_raw, w.dn_raw);
-    else
-        neighbours_kernel<false><<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
-                                                                             w.bin_start, w.up_raw, w.dn_raw);
+    neighbours_kernel<<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
+                                                                  w.up_raw, w.dn_raw);
+    if (g.bridge) {  // class 1 (reading A2'): a second, light pass over the hits that found no adjacent pair
+        bridge_links_kernel<<<div_up(slabs, kBrThreads / 32), kBrThreads, 0, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
+                                                                                  w.bin_start, w.up_raw, w.dn_raw, slabs);
+        return 2;
+    }
     return 1;
 }
 
