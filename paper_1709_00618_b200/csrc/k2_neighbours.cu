@@ -244,6 +244,14 @@ __device__ __forceinline__ int far_pos(const FarSeq& f, int k) {
     return k < f.n0 ? f.s0 + k : (k < f.n0 + f.n1 ? f.s1 + (k - f.n0) : f.s2 + (k - f.n0 - f.n1));
 }
 
+#ifndef TPC_NB_FAR
+#define TPC_NB_FAR 1
+#endif
+#ifndef TPC_BR_CTAS
+#define TPC_BR_CTAS 8
+#endif
+constexpr int kNbFar = TPC_NB_FAR;  // hits of a row two away fetched together before they are examined
+
 // Class-1 search of one hit (see above search_bridge for the reading).  Flat loops over the cells of the rows two
 // away, paired with the register lists of the adjacent rows; dense spots and fine grids take the nested search.
 __device__ __forceinline__ BestBridge bridge_hit(const DevGeom& g, const RowView& up, const RowView& dn,
@@ -264,10 +272,22 @@ __device__ __forceinline__ BestBridge bridge_hit(const DevGeom& g, const RowView
         generic = lu.n > kNbList || ld.n > kNbList;
         if (!generic && lu.n > 0 && has_dn2) {  // (du, dd) = (1, 2): u from the row r+1 list, d in row r-2
             const FarSeq f = far_cells(g, dn2, ylo2, yhi2, fz0, fz1);
+            float2 fh[kNbFar];  // the first far hits are loaded together (one memory round trip), then examined
+#pragma unroll
+            for (int k = 0; k < kNbFar; k++) fh[k] = k < f.nt ? dn2.yz[far_pos(f, k)] : make_float2(0.0f, 0.0f);
+#pragma unroll 1
             for (int k = 0; k < f.nt; k++) {
                 const int b = far_pos(f, k);
-                const float2 d = dn2.yz[b];
+                float2 d;
+                if (k < kNbFar) {
+                    d = fh[0];
+#pragma unroll
+                    for (int q = 0; q < kNbFar - 1; q++) fh[q] = fh[q + 1];  // shift: no dynamic register indexing
+                } else {
+                    d = dn2.yz[b];
+                }
                 const bool din = in_window(d, ylo2, yhi2, zlo2, zhi2);
+                if (!din) continue;  // the cells cover several times the window: most far hits end here
                 const float t2 = __fsub_rn(y, d.x), t4 = __fsub_rn(z, d.y);
 #define TPC_NB_BRIDGE_A(T1, T3, Q)                                                                             \
     {                                                                                                          \
@@ -287,10 +307,22 @@ __device__ __forceinline__ BestBridge bridge_hit(const DevGeom& g, const RowView
         }
         if (!generic && ld.n > 0 && has_up2) {  // (du, dd) = (2, 1): u in row r+2, d from the row r-1 list
             const FarSeq f = far_cells(g, up2, ylo2, yhi2, fz0, fz1);
+            float2 fh[kNbFar];
+#pragma unroll
+            for (int k = 0; k < kNbFar; k++) fh[k] = k < f.nt ? up2.yz[far_pos(f, k)] : make_float2(0.0f, 0.0f);
+#pragma unroll 1
             for (int k = 0; k < f.nt; k++) {
                 const int a = far_pos(f, k);
-                const float2 u = up2.yz[a];
+                float2 u;
+                if (k < kNbFar) {
+                    u = fh[0];
+#pragma unroll
+                    for (int q = 0; q < kNbFar - 1; q++) fh[q] = fh[q + 1];
+                } else {
+                    u = up2.yz[a];
+                }
                 const bool uin = in_window(u, ylo2, yhi2, zlo2, zhi2);
+                if (!uin) continue;
                 const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
 #define TPC_NB_BRIDGE_B(T2, T4, Q)                                                                             \
     {                                                                                                          \
@@ -456,7 +488,7 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
 // lanes stay busy and the tuned class-0 kernel above is untouched.  All rows are read in place (L2).
 constexpr int kBrThreads = 128;
 
-__global__ void __launch_bounds__(kBrThreads)
+__global__ void __launch_bounds__(kBrThreads, TPC_BR_CTAS)
 bridge_links_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
                     const float2* __restrict__ hit_yz, const uint16_t* __restrict__ hit_idx,
                     const uint16_t* __restrict__ bin_start, int32_t* __restrict__ link_up,
