@@ -28,8 +28,11 @@
  * chain invariants; Jacobian == central finite differences; forward+backward transport is the
  * identity; Bz->0 limit is the straight line; zero-smear fits reproduce the generating helix to
  * 1e-6; pulls ~ N(0,1) and chi2/ndf ~ 1; a one-shot weighted least-squares fit (numpy) equals
- * the filter result.  Parity unpinned: the absolute values of the tuning constants (window sizes,
- * D2 cut, gate, gap, selector threshold) -- the paper gives none (readings A3,A4,A9,A11).
+ * the filter result; for the optional class-1 links of S2 (nf_bridge_rows, reading A2'):
+ * grid == brute force, hand-placed lines with one / two missing rows, the cut the 2.25 factor
+ * implies (tests/test_oracle_bridge.py).  Parity unpinned: the absolute values of the tuning
+ * constants (window sizes, D2 cuts, gate, gap, selector threshold) -- the paper gives none
+ * (readings A2',A3,A4,A9,A11).
  */
 #include <math.h>
 #include <stdint.h>
