@@ -31,7 +31,10 @@ namespace tpc {
 constexpr bool kFollowSpec = TPC_FOLLOW_SPEC != 0;  // speculative load pipeline on/off (performance only)
 constexpr int kFollowThreads = 128;
 constexpr int kFollowCtasPerSm = TPC_FOLLOW_CTAS;
-constexpr int kFollowChunk = 64;                  // candidates a warp takes from the queue at a time
+#ifndef TPC_FOLLOW_CHUNK
+#define TPC_FOLLOW_CHUNK 0
+#endif
+constexpr int kFollowChunk = TPC_FOLLOW_CHUNK;  // candidates a warp takes from the queue at a time; 0 = as many as it has idle lanes
 constexpr int kFollowReload = TPC_FOLLOW_RELOAD;  // parked lanes that trigger a write-out / refill phase
 constexpr int kFitThreads = 128;
 #ifndef TPC_SPEC_HITS
@@ -353,18 +356,21 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             }
             // ---- refill ----
             if (!exhausted) {
+                const unsigned idle = __ballot_sync(full, mode == kIdle);
                 if (wn == we) {
+                    // kFollowChunk = 0: take exactly as many ids as there are idle lanes (best balance at the end of
+                    // the queue: no warp sits on ids it cannot start yet)
+                    const int take = kFollowChunk > 0 ? kFollowChunk : __popc(idle);
                     unsigned long long v = 0;
-                    if (lane == 0) v = atomicAdd(queue, (unsigned long long)kFollowChunk);
+                    if (lane == 0) v = atomicAdd(queue, (unsigned long long)take);
                     v = __shfl_sync(full, v, 0);
                     if (v >= (unsigned long long)n_cand) {
                         exhausted = true;
                     } else {
                         wn = (int)v;
-                        we = min(wn + kFollowChunk, n_cand);
+                        we = min(wn + take, n_cand);
                     }
                 }
-                const unsigned idle = __ballot_sync(full, mode == kIdle);
                 const int mine = wn + __popc(idle & ((1u << lane) - 1u));
                 if (mode == kIdle && mine < we) {
                     c = mine;
