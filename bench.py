@@ -351,7 +351,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--windows", type=int, default=16, help="CFG:4 drift windows per GPU and step")
+    ap.add_argument("--windows", type=int, default=100, help="CFG:4 drift windows per GPU and step")
     ap.add_argument("--chunk-windows", type=int, default=2, help="windows per upload chunk in the e2e pipeline")
     ap.add_argument("--slots", type=int, default=3)
     ap.add_argument("--seed0", type=int, default=5001)

@@ -116,8 +116,8 @@ typedef struct {
        5 input error flags (bit0: a row holds > 65535 clusters; bit1: > 2^23 candidates in one instance),
        6 S5 transport steps executed, 7 S5 measurement updates, 8 clusters examined by the S5 pick-up search,
        9 S5 pick-up searches (work counters for the roofline arithmetic; 6-9 stay 0 unless
-       tpc_set_work_counters enabled them), 10 internal, 11/12 the part of 6/7 spent on the candidates' own
-       hits (fit kernel), 13-15 reserved.
+       tpc_set_work_counters enabled them), 10 and 13 internal, 11/12 the part of 6/7 spent on the candidates' own
+       hits (fit kernel), 14-15 reserved.
        Written by the last kernel of the call. */
     int64_t* counts;
 } tpc_output_t;

@@ -36,8 +36,15 @@ claim_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_
              int64_t Cmax) {
     const int64_t n_cand = min(counts[1], Cmax);
     const int lane = threadIdx.x & 31;
-    const int64_t stride = (int64_t)gridDim.x * kClaimThreads;
-    for (int64_t c0 = (int64_t)blockIdx.x * kClaimThreads + (threadIdx.x & ~31); c0 < n_cand; c0 += stride) {
+    // Chunks of 32 tracklets are handed out in order from a device-wide counter (counts[13]), so the tracklets in
+    // flight -- and with them the claim words being updated -- stay a compact window of candidate ids that the L2
+    // holds; with a fixed grid stride the warps drift apart and at 100 windows the atomics thrash the L2.
+    unsigned long long* next = reinterpret_cast<unsigned long long*>(&counts[13]);
+    for (;;) {
+        unsigned long long t = 0;
+        if (lane == 0) t = atomicAdd(next, 32ull);
+        const int64_t c0 = (int64_t)__shfl_sync(kFull, t, 0);
+        if (c0 >= n_cand) break;
         // header of the lane's tracklet
         uint32_t my_w = 0u;
         int my_rows = 0, my_inst = 0;
@@ -61,7 +68,8 @@ claim_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_
             const int32_t* ro = row_offsets + (size_t)inst * g.R;
             for (int rq = (first & ~127) + 4 * lane; rq <= last; rq += 128) {
                 if (rq + 3 < first) continue;
-                const uint2 v = *reinterpret_cast<const uint2*>(rh + rq);  // RP % 8 == 0: in bounds, 8-byte aligned
+                const uint2 v = __ldcs(reinterpret_cast<const uint2*>(rh + rq));  // streamed once (evict-first): keep the L2 for
+                                                                         // the claim words; RP % 8 == 0: in bounds, aligned
                 const uint32_t li[4] = {v.x & 0xffffu, v.x >> 16, v.y & 0xffffu, v.y >> 16};
 #pragma unroll
                 for (int j = 0; j < 4; j++) {
