@@ -177,6 +177,77 @@ int launch_clean(const DevGeom&, const Workspace& w, const Problem& p, cudaStrea
     return 1;
 }
 
+// Two-level scan for long inputs (the per-slab counts: ~570 k entries at 100 windows, where one CTA takes 0.43 ms):
+// every CTA scans a tile of 4096 entries in place and reports its total; the tile totals go through the one-CTA scan;
+// a last pass adds the tile offsets.
+constexpr int kTile = kScanThreads * 4;
+
+__global__ void __launch_bounds__(kScanThreads)
+scan_tiles_kernel(int2* __restrict__ part, int64_t m, int2* __restrict__ tile_sums) {
+    __shared__ int2 s_warp[kScanThreads / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t i0 = (int64_t)blockIdx.x * kTile + (int64_t)threadIdx.x * 4;
+    int2 v[4];
+    int2 sum = make_int2(0, 0);
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        v[q] = i0 + q < m ? part[i0 + q] : make_int2(0, 0);
+        sum.x += v[q].x;
+        sum.y += v[q].y;
+    }
+    int2 incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int a = __shfl_up_sync(0xffffffffu, incl.x, d), b = __shfl_up_sync(0xffffffffu, incl.y, d);
+        if (lane >= d) { incl.x += a; incl.y += b; }
+    }
+    if (lane == 31) s_warp[wid] = incl;
+    __syncthreads();
+    int2 off = make_int2(0, 0), tot = make_int2(0, 0);
+#pragma unroll
+    for (int k = 0; k < kScanThreads / 32; k++) {
+        const int2 w = s_warp[k];
+        if (k < wid) { off.x += w.x; off.y += w.y; }
+        tot.x += w.x;
+        tot.y += w.y;
+    }
+    int2 run = make_int2(off.x + incl.x - sum.x, off.y + incl.y - sum.y);
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        if (i0 + q < m) part[i0 + q] = run;
+        run.x += v[q].x;
+        run.y += v[q].y;
+    }
+    if (threadIdx.x == 0) tile_sums[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(256)
+add_tile_offsets_kernel(int2* __restrict__ part, int64_t m, const int2* __restrict__ tile_sums, int n_tiles) {
+    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (i < m) {
+        const int2 o = tile_sums[i / kTile];
+        int2 v = part[i];
+        v.x += o.x;
+        v.y += o.y;
+        part[i] = v;
+    } else if (i == m) {
+        part[m] = tile_sums[n_tiles];  // the totals
+    }
+}
+
+// returns the kernels launched
+int launch_scan_int2_long(int2* part, int64_t m, int2* tile_sums, int64_t* counts, int c0, int c1, cudaStream_t s) {
+    if (m <= 4 * kTile) {
+        scan_int2_kernel<<<1, kScanThreads, 0, s>>>(part, nullptr, 1, 0, m, counts, c0, c1);
+        return 1;
+    }
+    const int n_tiles = div_up(m, kTile);
+    scan_tiles_kernel<<<n_tiles, kScanThreads, 0, s>>>(part, m, tile_sums);
+    scan_int2_kernel<<<1, kScanThreads, 0, s>>>(tile_sums, nullptr, 1, 0, n_tiles, counts, c0, c1);
+    add_tile_offsets_kernel<<<div_up(m + 1, 256), 256, 0, s>>>(part, m, tile_sums, n_tiles);
+    return 3;
+}
+
 void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m_cap, int64_t m_host, int64_t* counts,
                       int c0, int c1, cudaStream_t s) {
     scan_int2_kernel<<<1, kScanThreads, 0, s>>>(part, m_dev, m_div, m_cap, m_host, counts, c0, c1);
@@ -187,10 +258,10 @@ int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const 
     if (slabs == 0) return 0;
     const int grid = div_up(slabs, kChainThreads / 32);
     chain_flags_kernel<<<grid, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.dn, w.flags, w.slab_part, slabs);
-    launch_scan_int2(w.slab_part, nullptr, 1, 0, slabs, w.counts, 0, 1, s);
+    const int scans = launch_scan_int2_long(w.slab_part, slabs, w.scan_tmp, w.counts, 0, 1, s);
     chain_write_kernel<<<grid, kChainThreads, 0, s>>>(p.row_offsets, w.hit_pos, w.flags, w.slab_part, u.start_hits,
                                                       u.start_cap, w.cand_start, w.cand_slab, w.Cmax, slabs);
-    return 3;
+    return 2 + scans;
 }
 
 int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link, int dir,

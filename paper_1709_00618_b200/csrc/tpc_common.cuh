@@ -55,6 +55,7 @@ struct Workspace {
     int32_t* dn;
     uint32_t* claim;      // [N] S6 best claiming weight
     uint8_t* flags;       // [N] bit0 start hit, bit1 candidate
+    int2* scan_tmp;       // [S*R / 4096 + 2] tile totals of the two-level scan over slab_part
     int2* slab_part;      // [S*R + 1] (starts, candidates) per slab, then their exclusive scan
     int32_t* cand_start;  // [Cmax] sorted global position of the candidate's start hit (S4); the chain is walked in S5
     int32_t* cand_slab;   // [Cmax] instance * R + row of the start hit

@@ -155,6 +155,7 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.claim = c.take<uint32_t>(n);
     v.flags = c.take<uint8_t>(n);
     v.slab_part = c.take<int2>(slabs + 1);
+    v.scan_tmp = c.take<int2>(slabs / 4096 + 2);
     v.cand_start = c.take<int32_t>(cmax);
     v.cand_slab = c.take<int32_t>(cmax);
     v.tl_state = c.take<float4>(cmax * 6);

@@ -120,9 +120,10 @@ def test_capacity_overflow_is_reported_not_written():
 
 
 def test_full_size_drift_windows_against_oracle():
-    """The bench's workload at full size: two full CFG:4 windows (5 overlapping events each, 72 sector instances),
-    in the launch configuration bench.py times (one tpc_track_sectors call on the batch)."""
-    evs = [dg.drift_window(seed=5001 + i) for i in range(2)]
+    """The bench's workload at full size: three full CFG:4 windows (5 overlapping events each, 108 sector instances:
+    enough slabs for the two-level scan of the long-input path), in the launch configuration bench.py times (one
+    tpc_track_sectors call on the batch)."""
+    evs = [dg.drift_window(seed=5001 + i) for i in range(3)]
     batch = dg.concat_events(evs)
     assert batch.n_clusters > 1_000_000
     # A tracklet exists or not by threshold tests on the fitted state (|sinPhi| <= 0.95 in a transport): fp64 in the
