@@ -37,7 +37,7 @@ FLOP_TRANSPORT, FLOP_UPDATE, FLOP_EXAMINE, FLOP_SEARCH = 150.0, 93.0, 7.0, 18.0
 FP32_LANES_PER_SM, N_SM = 128, 148
 # dram bytes per launch of follow_kernel per cluster, from the committed ncu --set full capture (profiles/); None
 # until a capture exists
-FOLLOW_DRAM_BYTES_PER_CLUSTER = 336.7  # profiles/r1d_full_kernels.md: (5.739 + 0.465) GB per launch / 18,427,708 clusters
+FOLLOW_DRAM_BYTES_PER_CLUSTER = 120.3  # profiles/r1h_full_kernels.md: (11.0 + 2.98) GB per launch / 116,186,372 clusters
 
 
 def _gen_window(seed):
@@ -298,7 +298,7 @@ def run_ours(args):
             "unit": "TFLOP/s", "frac": ach / fp32_peak,
             "traffic": None if FOLLOW_DRAM_BYTES_PER_CLUSTER is None else FOLLOW_DRAM_BYTES_PER_CLUSTER * N,
             "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of follow_kernel per launch on the "
-                              "default workload (profiles/r1d_full_kernels.md), scaled by the cluster count",
+                              "default workload (profiles/r1h_full_kernels.md), scaled by the cluster count",
             "peak_source": f"148 SM x 128 fp32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md)",
             "avg_launch_ms": stage_ms["follow"], "share_of_step": stage_ms["follow"] / sum(stage_ms.values()),
             "algorithmic_flop_per_launch": float(flops),

@@ -91,8 +91,11 @@ __device__ __forceinline__ void zero_tracklet(const DevGeom& g, const FollowArgs
 }
 
 // ---- fit of the candidate's own hits -----------------------------------------------------------------------------
+#ifndef TPC_FIT_CTAS
+#define TPC_FIT_CTAS 4
+#endif
 template <bool kCount>
-__global__ void __launch_bounds__(kFitThreads)
+__global__ void __launch_bounds__(kFitThreads, TPC_FIT_CTAS)
 fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowArgs a) {
     const int n_cand = (int)min(a.counts[1], a.Cmax);
     const int c = blockIdx.x * kFitThreads + threadIdx.x;
