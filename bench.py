@@ -40,7 +40,17 @@ FP32_LANES_PER_SM, N_SM = 128, 148
 FOLLOW_DRAM_BYTES_PER_CLUSTER = 120.3  # profiles/r1h_full_kernels.md: (11.0 + 2.98) GB per launch / 116,186,372 clusters
 
 
+WORKLOAD = "cfg5"  # set from --workload before the batch is generated (module global: the worker processes fork)
+WORKLOADS = {"cfg5": "CFG:4 drift windows (5 overlapping Pb-Pb-like events each)",
+             "cfg3": "CFG:3 central Pb-Pb-like events (8,000 primaries + 20 % secondaries, 10 % noise)",
+             "cfg2": "CFG:2 peripheral Pb-Pb-like events (1,000 primaries, 5 % noise)"}
+
+
 def _gen_window(seed):
+    if WORKLOAD == "cfg3":
+        return datagen.central_event(seed)
+    if WORKLOAD == "cfg2":
+        return datagen.full_event(seed)
     return datagen.drift_window(seed)
 
 
@@ -117,7 +127,16 @@ def cpu_baseline(evs, budget_windows=1):
     t = time.perf_counter()
     c = o.track_count(ev.clusters, ev.row_offsets, ev.n_inst, n_threads=cores)
     dt = time.perf_counter() - t
+    # the same oracle on ONE core, on one sector instance of the sample (S8d: single-threaded and all-core figures)
+    R = ev.n_rows
+    i_big = int(np.argmax(np.diff(ev.row_offsets[::R])))
+    lo, hi = int(ev.row_offsets[i_big * R]), int(ev.row_offsets[(i_big + 1) * R])
+    ro1 = (ev.row_offsets[i_big * R:(i_big + 1) * R + 1] - lo).astype(np.int32)
+    t1 = time.perf_counter()
+    o.track_count(ev.clusters[lo:hi], ro1, 1, n_threads=1)
+    dt1 = time.perf_counter() - t1
     return {"value": ev.n_clusters / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "single_core_value": (hi - lo) / dt1,
             "sample": f"{budget_windows} drift window(s) of the batch, {ev.n_clusters} clusters, {ev.n_inst} sector "
                       f"instances, one OpenMP thread per instance up to all cores, {dt:.2f} s",
             "tracks": c["n_tracks"]}, dt
@@ -319,8 +338,8 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"cfg5 throughput batch: {args.windows} CFG:4 drift windows per GPU "
-                                   "(5 overlapping Pb-Pb-like events each) in one call",
+            "config": {"workload": f"{'cfg5 throughput batch' if WORKLOAD == 'cfg5' else WORKLOAD + ' batch'}: "
+                                   f"{args.windows} {WORKLOADS[WORKLOAD]} per GPU in one call",
                        "windows_per_gpu": args.windows, "sector_instances_per_gpu": S, "clusters_per_gpu": N,
                        "ms_per_window": ms_step / args.windows, "seed0": args.seed0,
                        "l2": (f"inputs are {16 * N / 1e6:.0f} MB of float4; " +
@@ -354,9 +373,14 @@ def main():
     ap.add_argument("--windows", type=int, default=100, help="CFG:4 drift windows per GPU and step")
     ap.add_argument("--chunk-windows", type=int, default=2, help="windows per upload chunk in the e2e pipeline")
     ap.add_argument("--slots", type=int, default=3)
+    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS),
+                    help="what --windows counts: drift windows (default, the headline), or CFG:3 / CFG:2 events for the "
+                         "linear-scaling check of PAPER.md:33")
     ap.add_argument("--seed0", type=int, default=5001)
     ap.add_argument("--tune", default="", help='JSON dict of performance-only tracker parameters, e.g. {"grid_cells_y": 8}')
     args = ap.parse_args()
+    global WORKLOAD
+    WORKLOAD = args.workload
     if args.impl == "reference":
         run_reference(args)
     else:
