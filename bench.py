@@ -371,7 +371,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--windows", type=int, default=100, help="CFG:4 drift windows per GPU and step")
-    ap.add_argument("--chunk-windows", type=int, default=2, help="windows per upload chunk in the e2e pipeline")
+    ap.add_argument("--chunk-windows", type=int, default=5, help="windows per upload chunk in the e2e pipeline")
     ap.add_argument("--slots", type=int, default=3)
     ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS),
                     help="what --windows counts: drift windows (default, the headline), or CFG:3 / CFG:2 events for the "

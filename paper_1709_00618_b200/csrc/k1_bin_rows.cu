@@ -8,7 +8,10 @@ namespace tpc {
 
 constexpr int kBinThreads = 128;
 
-__global__ void __launch_bounds__(kBinThreads)
+#ifndef TPC_BIN_CTAS
+#define TPC_BIN_CTAS 16
+#endif
+__global__ void __launch_bounds__(kBinThreads, TPC_BIN_CTAS)
 bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clusters,
                 const int32_t* __restrict__ row_offsets, float2* __restrict__ hit_yz, uint16_t* __restrict__ hit_idx,
                 uint16_t* __restrict__ hit_pos, uint16_t* __restrict__ bin_start, int64_t* __restrict__ counts) {
