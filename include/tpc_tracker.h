@@ -144,6 +144,16 @@ int tpc_set_stream(tpc_tracker_t* t, void* cuda_stream);
 int tpc_track_sectors(tpc_tracker_t* t, const float* clusters_xyzw, const int32_t* row_offsets,
                       int32_t n_sector_instances, int64_t n_clusters, const tpc_output_t* out);
 
+/*
+ * Compact cluster input.  x and w of a cluster are never read (the row gives x), so half of
+ * the 16 bytes per cluster is dead weight on the PCIe upload and in S1's read.  With TPC_INPUT_YZ the `clusters`
+ * argument of tpc_track_sectors / tpc_track_sectors_host (and tpc_slot_t.clusters) is [n_clusters][2] = (y, z),
+ * 8-byte aligned; results are bit-identical to the TPC_INPUT_XYZW call on the same (y, z).  Default: TPC_INPUT_XYZW.
+ */
+#define TPC_INPUT_XYZW 0
+#define TPC_INPUT_YZ 1
+int tpc_set_input_layout(tpc_tracker_t* t, int32_t layout);
+
 /* After synchronising and copying `counts` to the host: TPC_OK, TPC_ERR_CAPACITY or TPC_ERR_INPUT. */
 int tpc_check_counts(const int64_t* counts_host, const tpc_output_t* out);
 

@@ -68,6 +68,7 @@ extern "C" int tpc_track_sectors_host(tpc_tracker_t* t, const float* h_cl, const
         return fail(t, TPC_ERR_ARG, "bad argument");
     if (n_clusters > 0 && !h_cl) return fail(t, TPC_ERR_ARG, "NULL clusters");
     const int R = t->g.R;
+    const int64_t fpc = t->input_yz ? 2 : 4;  // floats per cluster in h_cl and in the slots' cluster buffers
     cudaStream_t s_in = static_cast<cudaStream_t>(h2d_stream), s_cmp = static_cast<cudaStream_t>(compute_stream),
                  s_out = static_cast<cudaStream_t>(d2h_stream);
     std::vector<Chunk> chunks;
@@ -161,8 +162,9 @@ extern "C" int tpc_track_sectors_host(tpc_tracker_t* t, const float* h_cl, const
         // upload: the slot's inputs are free once the chunk that used them last has been tracked
         if (i >= n_slots) CK(cudaStreamWaitEvent(s_in, ev_cmp[s], 0));
         if (c.n_cl > 0) {
-            CK(cudaMemcpyAsync(slots[s].clusters, h_cl + 4 * c.cl0, sizeof(float) * 4 * c.n_cl, cudaMemcpyHostToDevice, s_in));
-            up_bytes += (int64_t)sizeof(float) * 4 * c.n_cl;
+            // TPC_INPUT_YZ: 2 floats per cluster instead of 4 (tpc_set_input_layout)
+            CK(cudaMemcpyAsync(slots[s].clusters, h_cl + fpc * c.cl0, sizeof(float) * fpc * c.n_cl, cudaMemcpyHostToDevice, s_in));
+            up_bytes += (int64_t)sizeof(float) * fpc * c.n_cl;
         }
         const int64_t n_ro = (int64_t)c.n_inst * R + 1;
         CK(cudaMemcpyAsync(slots[s].row_offsets, h_ro + (int64_t)c.inst0 * R, sizeof(int32_t) * n_ro, cudaMemcpyHostToDevice, s_in));

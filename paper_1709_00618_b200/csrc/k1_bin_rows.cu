@@ -11,8 +11,18 @@ constexpr int kBinThreads = 128;
 #ifndef TPC_BIN_CTAS
 #define TPC_BIN_CTAS 16
 #endif
+// (y, z) of input cluster i: from the (x, y, z, w) records, or from the compact (y, z) input (tpc_set_input_layout)
+template <bool kYZ>
+__device__ __forceinline__ float2 load_yz(const float4* __restrict__ clusters, const float2* __restrict__ yz, int i) {
+    if (kYZ) return __ldg(&yz[i]);
+    const float4 c = __ldg(&clusters[i]);
+    return make_float2(c.y, c.z);
+}
+
+template <bool kYZ>
 __global__ void __launch_bounds__(kBinThreads, TPC_BIN_CTAS)
 bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clusters,
+                const float2* __restrict__ clusters_yz,
                 const int32_t* __restrict__ row_offsets, float2* __restrict__ hit_yz, uint16_t* __restrict__ hit_idx,
                 uint16_t* __restrict__ hit_pos, uint16_t* __restrict__ bin_start, int64_t* __restrict__ counts) {
     extern __shared__ __align__(16) uint32_t sm_hist[];  // [nzp] counts, then exclusive starts (cursors in pass 2)
@@ -41,15 +51,15 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
         const int i = threadIdx.x + k * kBinThreads;
         key[k] = -1;
         if (i < n) {
-            const float4 c = __ldg(&clusters[base + i]);
-            key[k] = zbin(c.z, z0, g.inv_cz, g.nz) * g.ny + ybin(c.y, y0, inv_sy, g.ny);
-            yz[k] = make_float2(c.y, c.z);
+            const float2 c = load_yz<kYZ>(clusters, clusters_yz, base + i);
+            key[k] = zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny);
+            yz[k] = c;
             atomicAdd(&sm_hist[key[k]], 1u);
         }
     }
     for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {
-        const float4 c = __ldg(&clusters[base + i]);
-        atomicAdd(&sm_hist[zbin(c.z, z0, g.inv_cz, g.nz) * g.ny + ybin(c.y, y0, inv_sy, g.ny)], 1u);
+        const float2 c = load_yz<kYZ>(clusters, clusters_yz, base + i);
+        atomicAdd(&sm_hist[zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny)], 1u);
     }
     __syncthreads();
     // exclusive scan of nzp entries: a contiguous chunk of 8-entry groups per thread, warp scan of the chunk sums
@@ -94,9 +104,9 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
         }
     }
     for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {  // long rows: from L1/L2 this time
-        const float4 c = __ldg(&clusters[base + i]);
-        const uint32_t pos = atomicAdd(&sm_hist[zbin(c.z, z0, g.inv_cz, g.nz) * g.ny + ybin(c.y, y0, inv_sy, g.ny)], 1u);
-        hit_yz[base + pos] = make_float2(c.y, c.z);
+        const float2 c = load_yz<kYZ>(clusters, clusters_yz, base + i);
+        const uint32_t pos = atomicAdd(&sm_hist[zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny)], 1u);
+        hit_yz[base + pos] = c;
         hit_idx[base + pos] = (uint16_t)i;
         hit_pos[base + i] = (uint16_t)pos;
     }
@@ -108,11 +118,16 @@ int launch_bin_rows(const DevGeom& g, const Workspace& w, const Problem& p, cuda
     const size_t smem = (size_t)g.nzp * sizeof(uint32_t);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(bin_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(bin_rows_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(bin_rows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    bin_rows_kernel<<<slabs, kBinThreads, smem, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx, w.hit_pos, w.bin_start,
-                                                     w.counts);
+    if (p.clusters_yz)
+        bin_rows_kernel<true><<<slabs, kBinThreads, smem, s>>>(g, nullptr, p.clusters_yz, p.row_offsets, w.hit_yz,
+                                                               w.hit_idx, w.hit_pos, w.bin_start, w.counts);
+    else
+        bin_rows_kernel<false><<<slabs, kBinThreads, smem, s>>>(g, p.clusters, nullptr, p.row_offsets, w.hit_yz,
+                                                                w.hit_idx, w.hit_pos, w.bin_start, w.counts);
     return 1;
 }
 

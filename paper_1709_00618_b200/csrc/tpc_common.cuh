@@ -73,7 +73,8 @@ struct Workspace {
 };
 
 struct Problem {
-    const float4* clusters;
+    const float4* clusters;   // (x, y, z, w), or NULL when the input is compact
+    const float2* clusters_yz;  // compact input (y, z), or NULL
     const int32_t* row_offsets;
     int32_t n_inst;
     int64_t n_clusters;

@@ -192,6 +192,13 @@ extern "C" int tpc_set_stream(tpc_tracker_t* t, void* s) {
     return TPC_OK;
 }
 
+extern "C" int tpc_set_input_layout(tpc_tracker_t* t, int32_t layout) {
+    if (!t) return TPC_ERR_ARG;
+    if (layout != TPC_INPUT_XYZW && layout != TPC_INPUT_YZ) return fail(t, TPC_ERR_ARG, "unknown input layout");
+    t->input_yz = layout == TPC_INPUT_YZ;
+    return TPC_OK;
+}
+
 extern "C" int tpc_set_work_counters(tpc_tracker_t* t, int32_t enable) {
     if (!t) return TPC_ERR_ARG;
     t->count_work = enable != 0;
@@ -228,13 +235,15 @@ extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const 
     if (n_inst < 0 || n_clusters < 0 || n_clusters >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "bad sizes");
     if ((int64_t)n_inst * t->g.R + 1 >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "too many sector instances");
     if (n_clusters > 0 && (!clusters || !row_offsets || n_inst == 0)) return fail(t, TPC_ERR_ARG, "NULL input");
-    if ((uintptr_t)clusters & 15) return fail(t, TPC_ERR_ARG, "clusters must be 16-byte aligned");
+    if ((uintptr_t)clusters & (t->input_yz ? 7 : 15))
+        return fail(t, TPC_ERR_ARG, "clusters must be 16-byte aligned (8-byte for TPC_INPUT_YZ)");
     Workspace w;
     const size_t need = carve(t->g, t->ws, n_clusters, n_inst, &w);
     if (!t->ws || need > t->ws_bytes) return fail(t, TPC_ERR_WORKSPACE, "workspace missing or too small");
     cudaStream_t s = t->stream;
     const DevGeom& g = t->g;
-    Problem p{reinterpret_cast<const float4*>(clusters), row_offsets, n_inst, n_clusters};
+    Problem p{t->input_yz ? nullptr : reinterpret_cast<const float4*>(clusters),
+              t->input_yz ? reinterpret_cast<const float2*>(clusters) : nullptr, row_offsets, n_inst, n_clusters};
     int launches = 0;
     const bool tm = t->timing && t->ev_valid;
     cudaEvent_t* ev = t->ev[t->n_calls % TPC_TIMING_RING];

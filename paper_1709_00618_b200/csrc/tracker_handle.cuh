@@ -14,6 +14,7 @@ struct tpc_tracker {
     int n_sm = 148;
     int last_launches = 0;
     bool timing = false;
+    bool input_yz = false;    // clusters are (y, z) pairs instead of (x, y, z, w) (tpc_set_input_layout)
     bool count_work = false;  // S5 work counters counts[6..9] (tpc_set_work_counters)
     cudaEvent_t ev[TPC_TIMING_RING][TPC_N_STAGES + 1] = {};
     bool ev_valid = false;

@@ -23,7 +23,8 @@ ERRORS = {-1: "TPC_ERR_ARG", -2: "TPC_ERR_GEOMETRY", -3: "TPC_ERR_WORKSPACE", -4
 
 EXPORTS = ("tpc_tracker_create", "tpc_tracker_destroy", "tpc_workspace_bytes", "tpc_set_workspace", "tpc_set_stream",
            "tpc_track_sectors", "tpc_check_counts", "tpc_last_launch_count", "tpc_set_stage_timing",
-           "tpc_stage_times_ms", "tpc_last_error", "tpc_track_sectors_host", "tpc_set_work_counters")
+           "tpc_stage_times_ms", "tpc_last_error", "tpc_track_sectors_host", "tpc_set_work_counters",
+           "tpc_set_input_layout")
 
 
 class TpcError(RuntimeError):
@@ -99,6 +100,7 @@ def load_library():
     lib.tpc_last_launch_count.restype = C.c_int32
     lib.tpc_set_stage_timing.argtypes = [C.c_void_p, C.c_int32]
     lib.tpc_set_work_counters.argtypes = [C.c_void_p, C.c_int32]
+    lib.tpc_set_input_layout.argtypes = [C.c_void_p, C.c_int32]
     lib.tpc_stage_times_ms.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_float)]
     lib.tpc_last_error.argtypes = [C.c_void_p]
     lib.tpc_last_error.restype = C.c_char_p
@@ -234,6 +236,10 @@ class Tracker:
     def set_work_counters(self, enable=True):
         """counts[6..9] (S5 transports / updates / examined clusters / searches) are only filled when enabled."""
         self._check(self.lib.tpc_set_work_counters(self._h, 1 if enable else 0), "tpc_set_work_counters")
+
+    def set_input_layout(self, yz=False):
+        """yz=True: `clusters` of the track calls is [N,2] = (y, z) instead of [N,4] = (x, y, z, w) (TPC_INPUT_YZ)."""
+        self._check(self.lib.tpc_set_input_layout(self._h, 1 if yz else 0), "tpc_set_input_layout")
 
     def stage_times_ms(self, age=0):
         """Milliseconds per stage of the timed call `age` calls back (0 = last)."""

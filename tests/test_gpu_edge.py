@@ -131,3 +131,41 @@ def test_full_size_drift_windows_against_oracle():
     # the other side; they count against the 99.5 % shared-assignment bar like any other difference.
     g, o = _check(batch, max_ok_mismatch=batch.n_clusters // 200_000)
     assert abs(g.n_tracks - len(o.trk_cand)) <= 5
+
+
+def test_compact_yz_input_equals_xyzw():
+    """TPC_INPUT_YZ (clusters as (y, z) pairs, half the upload) gives bit-identical results: device call and host
+    pipeline."""
+    import torch
+    from paper_1709_00618_b200 import Tracker
+    from paper_1709_00618_b200.tracker import HostPipeline
+    evs = [dg.drift_window(seed=5301 + i, mean_tracks=150.0, cap_tracks=400) for i in range(3)]
+    batch = dg.concat_events(evs)
+    trk = Tracker.for_event(batch)
+    ref = trk.track_sectors(batch.clusters, batch.row_offsets, batch.n_inst)
+    yz = np.ascontiguousarray(batch.clusters[:, 1:3])
+    dev = trk.device
+    d_yz = torch.from_numpy(yz).to(dev)
+    d_ro = torch.from_numpy(batch.row_offsets).to(dev)
+    trk.set_input_layout(yz=True)
+    trk.reserve(batch.n_clusters, batch.n_inst)
+    trk.set_stream()
+    bufs, out = trk.alloc_outputs(batch.n_clusters)
+    trk.track_sectors_device(d_yz, d_ro, batch.n_inst, out)
+    torch.cuda.synchronize(dev)
+    assert bufs["counts"].cpu().numpy()[:5].tolist() == ref.counts[:5].tolist()
+    assert np.array_equal(bufs["cluster_owner"].cpu().numpy(), ref.cluster_owner)
+    assert np.array_equal(bufs["trk_params"][:ref.n_tracks].cpu().numpy(), ref.trk_params)
+    # host pipeline on the compact host buffer
+    h_yz = torch.from_numpy(yz).pin_memory()
+    h_ro = torch.from_numpy(batch.row_offsets).pin_memory()
+    R = batch.n_rows
+    mx = max(int(batch.row_offsets[min(i + 36, batch.n_inst) * R] - batch.row_offsets[i * R])
+             for i in range(0, batch.n_inst, 36))
+    pipe = HostPipeline(trk, mx, 36, batch.n_clusters, n_slots=2)
+    ho = pipe.run(h_yz, h_ro, batch.n_inst)
+    assert int(ho.totals[3]) == ref.n_tracks and ho.h2d_bytes < 8 * batch.n_clusters + 8 * len(batch.row_offsets)
+    assert np.array_equal(pipe.host["cluster_owner"].numpy()[:batch.n_clusters], ref.cluster_owner)
+    assert np.array_equal(pipe.host["trk_hits"].numpy()[:ref.n_track_hits], ref.trk_hits)
+    trk.set_input_layout(yz=False)
+    trk.close()
