@@ -169,3 +169,10 @@ def test_compact_yz_input_equals_xyzw():
     assert np.array_equal(pipe.host["trk_hits"].numpy()[:ref.n_track_hits], ref.trk_hits)
     trk.set_input_layout(yz=False)
     trk.close()
+
+
+def test_full_size_central_event_against_oracle():
+    """CFG:3 at full size: 8,000 primaries + 20 % secondaries, 10 % noise, ~1.5 M clusters, ~260 hits per row."""
+    ev = dg.central_event(seed=3001)
+    assert ev.n_clusters > 1_000_000
+    _check(ev, max_ok_mismatch=ev.n_clusters // 200_000)
