@@ -27,12 +27,17 @@
  * and helical tracks link to their own neighbours and are recovered with all hits; cleaning and
  * chain invariants; Jacobian == central finite differences; forward+backward transport is the
  * identity; Bz->0 limit is the straight line; zero-smear fits reproduce the generating helix to
- * 1e-6; pulls ~ N(0,1) and chi2/ndf ~ 1; a one-shot weighted least-squares fit (numpy) equals
- * the filter result; for the optional class-1 links of S2 (nf_bridge_rows, reading A2'):
- * grid == brute force, hand-placed lines with one / two missing rows, the cut the 2.25 factor
- * implies (tests/test_oracle_bridge.py).  Parity unpinned: the absolute values of the tuning
- * constants (window sizes, D2 cuts, gate, gap, selector threshold) -- the paper gives none
- * (readings A2',A3,A4,A9,A11).
+ * 1e-6; pulls ~ N(0,1) and chi2/ndf ~ 1; in the linear regime (Bz = 0, residuals of 1e-6 cm)
+ * the sequential filter equals a one-shot weighted least-squares fit with the prior folded in
+ * (numpy, state and covariance); the pick-up and stop rules of pickup() / follow_dir() on
+ * hand-placed straight tracks: nearest of several clusters in the gate, lowest local index on
+ * an exact tie, gate = 4 sigma capped at 3 cm, 5 empty rows bridged / 6 stop / a hit resets the
+ * count, stop at the first row beyond the sector edge + margin (tests/test_oracle_follow_rules.py);
+ * for the optional class-1 links of S2 (nf_bridge_rows, reading A2'): grid == brute force,
+ * hand-placed lines with one / two missing rows, the cut the 2.25 factor implies, the exact tie
+ * between the two kinds (tests/test_oracle_bridge.py).  Parity unpinned: the absolute values of
+ * the tuning constants (window sizes, D2 cuts, gate, gap, selector threshold) -- the paper gives
+ * none (readings A2',A3,A4,A9,A11).
  */
 #include <math.h>
 #include <stdint.h>

@@ -112,3 +112,30 @@ def test_bridging_halves_the_candidates_and_keeps_the_tracks():
     assert len(b.cand_n) < 0.6 * len(a.cand_n)
     assert abs(len(b.trk_cand) - len(a.trk_cand)) <= 0.03 * len(a.trk_cand)
     assert (b.cluster_owner >= 0).sum() >= 0.98 * (a.cluster_owner >= 0).sum()
+
+
+def test_exact_tie_between_the_two_kinds_prefers_the_pair_with_the_near_upper_partner():
+    """Reading A2': minimum over (D, du, u, d).  Hit h = (0, 100) in row 50; row 51 holds u1 = 1.5 (local index 1,
+    behind a far-away cluster), row 49 d1 = 1.5, row 48 d2 = -3, row 52 u2 = -3 (local index 0).  The adjacent pair
+    (u1, d1) deviates by 3 cm -> inadmissible; both bridged pairs are exactly straight:
+        (du, dd) = (1, 2): 2 (u1 - h) - (h - d2) = 3 - 3 = 0;   (2, 1): (u2 - h) - 2 (h - d1) = -3 + 3 = 0.
+    The tie goes to du = 1 although the other pair's upper partner has the lower local index."""
+    def links(d2_y):
+        rows = {48: [(d2_y, 100.0)], 49: [(1.5, 100.0)], 50: [(0.0, 100.0)], 51: [(-15.0, 100.0), (1.5, 100.0)],
+                52: [(-3.0, 100.0)]}
+        cl, ro = _event_from_rows(rows)
+        idx = {(int(r), k): int(ro[r]) + k for r in rows for k in range(len(rows[r]))}
+        for use_grid in (True, False):
+            up, dn = Oracle(RX, 0.0, nf_bridge_rows=1).neighbours(cl, ro, 1, use_grid=use_grid)
+            got = (int(up[idx[50, 0]]), int(dn[idx[50, 0]]))
+            assert use_grid or got == first
+            first = got
+        up0, _ = Oracle(RX, 0.0).neighbours(cl, ro, 1)
+        assert up0[idx[50, 0]] == -1  # no admissible adjacent pair: class 1 is what links it
+        return got, idx
+
+    got, idx = links(-3.0)
+    assert got == (idx[51, 1], idx[48, 0])
+    # D decides before the kind does: with d2 = -3.25 the (1, 2) pair deviates by 0.25 cm, the (2, 1) pair by 0
+    got, idx = links(-3.25)
+    assert got == (idx[52, 0], idx[49, 0])
