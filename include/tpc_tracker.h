@@ -113,7 +113,7 @@ typedef struct {
     int64_t trk_capacity, trk_hits_capacity;
     int32_t* cluster_owner; /* [n_clusters] final track index or -1 */
     /* device [TPC_N_COUNTS]: 0 n_start, 1 n_cand, 2 n_tracklets, 3 n_tracks, 4 n_track_hits,
-       5 input error flags (bit0: a row holds > 65535 clusters; bit1: > 2^23 candidates in one instance),
+       5 input error flags (bit0: a row holds > 65535 clusters; the excess clusters are ignored),
        6 S5 transport steps executed, 7 S5 measurement updates, 8 clusters examined by the S5 pick-up search,
        9 S5 pick-up searches (work counters for the roofline arithmetic; 6-9 stay 0 unless
        tpc_set_work_counters enabled them), 10 and 13 internal, 11/12 the part of 6/7 spent on the candidates' own

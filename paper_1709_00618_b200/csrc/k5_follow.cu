@@ -8,27 +8,21 @@
 //    all loads of a candidate are in flight together; the state after the last own hit goes to tl_state.
 //  * follow_kernel: the row-by-row extrapolation.  Persistent warps, every lane a small state machine that advances
 //    its candidate by ONE pad row per loop iteration (upward / back transport / downward), with the lanes refilled
-//    from a device-wide queue as candidates end.  The two dependent memory round trips of a pick-up search (cell
-//    table -> hits) are taken off the critical path by a two-stage software pipeline: the cell-table entries of the
-//    row TWO steps ahead and the first two hits of the row ONE step ahead are loaded speculatively for a window
-//    around the linearly extrapolated position, widened by a margin.  At the step itself the exact window is
-//    computed; if its cells are covered by the speculated ones (almost always) the preloaded data are used --
-//    examining a superset of cells is harmless because every hit still passes the exact gate test (the grid is an
-//    acceleration structure only) -- otherwise the step falls back to direct loads.
+//    from a device-wide queue as candidates end.  A pick-up search reads the cell-table entries of the exact gate
+//    window and then the window's first hits, all loads of a kind in flight together; examining a superset of cells
+//    is harmless because every hit still passes the exact gate test (the grid is an acceleration structure only).
+//    (A variant with a two-stage speculative load pipeline was measured in round 1 and lost to this one -- DESIGN.md
+//    section 5 -- and is no longer in the source.)
 #include "kf_math.cuh"
 
-#ifndef TPC_FOLLOW_SPEC
-#define TPC_FOLLOW_SPEC 0
-#endif
 #ifndef TPC_FOLLOW_CTAS
-#define TPC_FOLLOW_CTAS (TPC_FOLLOW_SPEC ? 5 : 7)
+#define TPC_FOLLOW_CTAS 7
 #endif
 #ifndef TPC_FOLLOW_RELOAD
 #define TPC_FOLLOW_RELOAD 4
 #endif
 namespace tpc {
 
-constexpr bool kFollowSpec = TPC_FOLLOW_SPEC != 0;  // speculative load pipeline on/off (performance only)
 constexpr int kFollowThreads = 128;
 constexpr int kFollowCtasPerSm = TPC_FOLLOW_CTAS;
 #ifndef TPC_FOLLOW_CHUNK
@@ -37,18 +31,10 @@ constexpr int kFollowCtasPerSm = TPC_FOLLOW_CTAS;
 constexpr int kFollowChunk = TPC_FOLLOW_CHUNK;  // candidates a warp takes from the queue at a time; 0 = as many as it has idle lanes
 constexpr int kFollowReload = TPC_FOLLOW_RELOAD;  // parked lanes that trigger a write-out / refill phase
 constexpr int kFitThreads = 128;
-#ifndef TPC_SPEC_HITS
-#define TPC_SPEC_HITS 4
-#endif
-#ifndef TPC_SPEC_MARGIN
-#define TPC_SPEC_MARGIN 0.25f
-#endif
 #ifndef TPC_DIRECT_HITS
 #define TPC_DIRECT_HITS 3
 #endif
 constexpr int kDirectHits = TPC_DIRECT_HITS;      // hits of a window examined in line (the rest in a loop)
-constexpr int kSpecHits = TPC_SPEC_HITS;          // hits of the coming window fetched ahead
-constexpr float kSpecMargin = TPC_SPEC_MARGIN;  // [cm] widening of the speculated window (performance only)
 constexpr float kCellMargin = 1e-3f;  // [cm] the visited cells are a superset of the rounded fp32 gate test
 
 enum FollowMode : int { kUp = 0, kBack = 1, kDown = 2, kDone = 3, kIdle = 4 };
@@ -143,9 +129,9 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
                 x[q] = g.row_x[row[q]];
             }
         }
-        // seed from hits 0, n/2, n-1.  The state carries y and z relative to the first candidate hit: the model is
+        // seed from hits 0, n/2, n-1.  The state carries y and z relative to the last attached hit: the model is
         // translation invariant in y and z, so this is exact, and it keeps the fp32 rounding of the two
-        // coordinates (ulp(20 cm), ulp(250 cm)) out of q/pt and sinPhi.
+        // coordinates (ulp(20 cm), ulp(250 cm)) out of the state.
         const int i1 = n >> 1, i2 = n - 1;
         float2 h1 = h[0], h2 = h[0];
         float x1 = x[0], x2 = x[0];
@@ -160,7 +146,7 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
                 a.usr_cand_hits[(size_t)c * kCandMax + q] = q < n ? rb[q] + (int)a.hit_idx[pos[q]] : -1;
         }
         if (a.usr_cand_n && c < a.usr_cand_cap) a.usr_cand_n[c] = n;
-        const float yref = h[0].x, zref = h[0].y;
+        float yref = h[0].x, zref = h[0].y;
         KfState st;
         bool ok = kf_seed(st, x[0], 0.0f, 0.0f, x1, h1.x - yref, x2, h2.x - yref, h2.y - zref, g.cB, g.max_s, g.p0);
         float chi2 = 0.0f;
@@ -174,6 +160,8 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
                     }
                     if (ok) {
                         chi2 += kf_update(st, h[q].x - yref, h[q].y - zref, g.sy2, g.sz2);
+                        yref = h[q].x;  // the state's (y, z) frame follows the attached hit (kf_update)
+                        zref = h[q].y;
                         if (kCount) n_up++;
                     }
                 }
@@ -243,14 +231,6 @@ __device__ __forceinline__ void pick_consider(PickBest& b, const uint16_t* __res
     b.z = better ? h.y : b.z;
 }
 
-// Speculative hit loads go straight to shared memory (cp.async, 8 bytes): no register is tied up while they fly.
-__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem)
-                 : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-
 __device__ __forceinline__ float sqrt_fast(float x) {  // x > 0, normal range
     float r;
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
@@ -265,10 +245,7 @@ __device__ __forceinline__ void store_report(float4 (*s_rep)[kFollowThreads], co
     s_rep[4][threadIdx.x] = make_float4(st.c41, st.c42, st.c43, st.c44);
 }
 
-// The cells of a search window in one row: z bins zb0 and (if two) zb0 + 1, strips ys0 .. ys1 - 1; packed
-// ys0 | ys1 << 8 | zb0 << 16 | two << 31.  kNoCells = not usable (window wider than two z bins).
-constexpr unsigned kNoCells = 0xffffffffu;
-
+// The cells of a search window in one row: z bins zb0..zb1, strips ys0 .. ys1 - 1.
 struct Window {
     int zb0, zb1, ys0, ys1;  // ys1 exclusive
 };
@@ -300,13 +277,12 @@ __device__ __forceinline__ HitSeq hit_seq(unsigned tab0, unsigned tab1, bool two
 
 // kCount: also accumulate the work counters counts[6..9] (roofline arithmetic; tpc_set_work_counters).  They are a
 // property of the input, so the timed runs use the variant without them.
-template <bool kCount, bool kSpec>
+template <bool kCount>
 __global__ void __launch_bounds__(kFollowThreads, kFollowCtasPerSm)
 follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowArgs a) {
     __shared__ float s_rowx[kMaxRows + 1];
     __shared__ float2 s_rowy[kMaxRows + 1];      // (y0, strips per cm) of the row's grid
     __shared__ float4 s_rep[5][kFollowThreads];  // reported state of the lane's tracklet (see kDown below)
-    __shared__ float2 s_hit[kSpecHits][kFollowThreads];  // speculative copies of the coming window's first hits
     for (int q = threadIdx.x; q < g.R; q += kFollowThreads) {
         s_rowx[q] = g.row_x[q];
         s_rowy[q] = make_float2(g.row_y0[q], g.row_inv_sy[q]);
@@ -328,14 +304,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
     int nhits = 0, gap = 0, first_row = 0, last_row = 0;
     float yref = 0.0f, zref = 0.0f, z0 = 0.0f, chi2 = 0.0f;
     KfState st = {};
-    // Speculation pipeline.  Slot A belongs to the coming step (row rn): packed cell-table entries, the cells they
-    // were read for, the row's offset and the first two hits of the window.  Slot B holds the raw cell-table loads
-    // issued last for the row after that (or for rn itself while the pipeline fills); its registers are not
-    // touched before the iteration after the one that issued them, so no load is waited for where it is issued.
-    bool tabA_ok = false, hitA_ok = false, tabB_ok = false;
-    unsigned cellsA = kNoCells, cellsB = kNoCells, tabA0 = 0u, tabA1 = 0u;
-    unsigned tB00 = 0u, tB01 = 0u, tB10 = 0u, tB11 = 0u;
-    int rbA = 0, rbB = 0;
+    int rb_next = 0;  // offset of row rn (loaded one step ahead)
 
     for (;;) {
         unsigned act = __ballot_sync(full, mode < kDone);
@@ -402,8 +371,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         r = last_row = r0 + (nbits >> 8);
                         mode = r + 1 < g.R ? kUp : kBack;
                         rn = mode == kUp ? r + 1 : r0;
-                        tabA_ok = hitA_ok = tabB_ok = false;
-                        if (!kSpec) rbA = a.row_offsets[slab_base + rn];
+                        rb_next = a.row_offsets[slab_base + rn];
                     }
                 }
                 wn = min(we, wn + __popc(idle));
@@ -411,7 +379,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             act = __ballot_sync(full, mode < kDone);
             if (act == 0u && exhausted) break;
         }
-        if (mode < kDone && (!kSpec || mode == kBack || hitA_ok)) {
+        if (mode < kDone) {
             // ---- one pad row: transport to row rn, attach a hit, decide where to go next.  Written as one
             // straight path with flags: the lanes of a warp differ in phase, and every branch taken by a few
             // lanes costs the whole warp its instructions.
@@ -428,37 +396,27 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 const float wy = fminf(g.wmax, g.gate * sqrt_fast(st.c00 + g.sy2));
                 const float wz = fminf(g.wmax, g.gate * sqrt_fast(st.c11 + g.sz2));
                 const Window w = window_cells(g, s_rowy[r], z0, yp, zp, wy + kCellMargin, wz + kCellMargin);
-                // are the exact window's cells covered by the speculated ones?
-                const int sy0 = (int)(cellsA & 0xffu), sy1 = (int)((cellsA >> 8) & 0xffu);
-                const int sz0 = (int)((cellsA >> 16) & 0x7fffu);
-                bool two = (cellsA >> 31) != 0u;
-                const bool spec = kSpec && cellsA != kNoCells && sy0 <= w.ys0 && w.ys1 <= sy1 && sz0 <= w.zb0 &&
-                                  w.zb1 <= sz0 + (int)two;
-                unsigned tab0 = tabA0, tab1 = tabA1;
-                const unsigned urb = (unsigned)rbA;
-                const unsigned tb0 = (unsigned)(slab_base + r) * (unsigned)g.nzp;
-                if (!spec) {  // direct loads of the exact window's cell-table entries
-                    const unsigned ia = tb0 + (unsigned)(w.zb0 * g.ny), ib = tb0 + (unsigned)(w.zb1 * g.ny);
-                    two = w.zb1 > w.zb0;
-                    const unsigned t00 = a.bin_start[ia + w.ys0], t01 = a.bin_start[ia + w.ys1];
-                    unsigned t10 = 0u, t11 = 0u;
-                    if (two) {
-                        t10 = a.bin_start[ib + w.ys0];
-                        t11 = a.bin_start[ib + w.ys1];
-                    }
-                    tab0 = t00 | (t01 << 16);
-                    tab1 = t10 | (t11 << 16);
+                const unsigned urb = (unsigned)rb_next;
+                // cell-table entries of the exact window (64-bit index: n_inst * R * nzp may exceed 2^32)
+                const uint16_t* tb = a.bin_start + (size_t)(slab_base + r) * (size_t)g.nzp;
+                const uint16_t* ta = tb + w.zb0 * g.ny;
+                const bool two = w.zb1 > w.zb0;
+                const unsigned t00 = ta[w.ys0], t01 = ta[w.ys1];
+                unsigned t10 = 0u, t11 = 0u;
+                if (two) {
+                    const uint16_t* tz = tb + w.zb1 * g.ny;
+                    t10 = tz[w.ys0];
+                    t11 = tz[w.ys1];
                 }
-                const HitSeq q = hit_seq(tab0, tab1, two);
+                const HitSeq q = hit_seq(t00 | (t01 << 16), t10 | (t11 << 16), two);
                 if (kCount) {
                     n_se++;
                     n_ex += q.nt;
                 }
                 // The window's hits form one sequence k = 0..nt-1, element k at sorted position seq_pos(k).  The
-                // first kSpecHits come from the speculative copies in shared memory, the rest (rare) one by one.
+                // first kDirectHits are loaded together (one memory round trip), the rest (rare) one by one.
                 PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f};
-                int k0 = kDirectHits;
-                if (!spec) {  // direct loads of the first hits, all in flight together
+                {
                     float2 h[kDirectHits];
                     int j[kDirectHits];
 #pragma unroll
@@ -470,35 +428,27 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
 #pragma unroll
                     for (int k = 0; k < kDirectHits; k++)
                         pick_consider(b, a.hit_idx, urb, j[k], k < q.nt, h[k], yp, zp, wy, wz);
-                } else {
-                    cp_async_wait_all();
-#pragma unroll
-                    for (int k = 0; k < kSpecHits; k++) {
-                        const int j = k < q.na ? q.ja0 + k : k + q.d;
-                        pick_consider(b, a.hit_idx, urb, j, k < q.nt, s_hit[k][threadIdx.x], yp, zp, wy, wz);
-                    }
-                    k0 = kSpecHits;
                 }
-                for (int k = k0; k < q.nt; k++) {  // few lanes get here: test the gate first, most hits fail it
+                for (int k = kDirectHits; k < q.nt; k++) {  // few lanes get here: test the gate first, most hits fail it
                     const int j = k < q.na ? q.ja0 + k : k + q.d;
                     const float2 h = a.hit_yz[urb + (unsigned)j];
                     if (fabsf(__fsub_rn(h.x, yp)) <= wy && fabsf(__fsub_rn(h.y, zp)) <= wz)
                         pick_consider(b, a.hit_idx, urb, j, true, h, yp, zp, wy, wz);
                 }
-                // z bins in between exist only when the cells are narrower than the gate (non-default
-                // grid_cell_z); such windows are never speculated
-                if (!spec)
-                    for (int zb = w.zb0 + 1; zb < w.zb1; zb++) {
-                        const unsigned im = tb0 + (unsigned)(zb * g.ny);
-                        const int jm0 = a.bin_start[im + w.ys0], jm1 = a.bin_start[im + w.ys1];
-                        if (kCount) n_ex += jm1 - jm0;
-                        for (int j = jm0; j < jm1; j++)
-                            pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
-                    }
+                // z bins in between exist only when the cells are narrower than the gate (non-default grid_cell_z)
+                for (int zb = w.zb0 + 1; zb < w.zb1; zb++) {
+                    const uint16_t* tm = tb + zb * g.ny;
+                    const int jm0 = tm[w.ys0], jm1 = tm[w.ys1];
+                    if (kCount) n_ex += jm1 - jm0;
+                    for (int j = jm0; j < jm1; j++)
+                        pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
+                }
                 li = b.j;
-                __stcs(&a.tl_rowhit[(unsigned)c * (unsigned)g.RP + (unsigned)r], (uint16_t)li);  // -1 = kNoHit
+                __stcs(&a.tl_rowhit[(size_t)c * (size_t)g.RP + (size_t)r], (uint16_t)li);  // -1 = kNoHit
                 if (li >= 0) {
                     chi2 += kf_update(st, b.y - yref, b.z - zref, g.sy2, g.sz2);
+                    yref = b.y;  // the state's (y, z) frame follows the attached hit (kf_update)
+                    zref = b.z;
                     if (kCount) n_up++;
                 }
             }
@@ -527,64 +477,10 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             } else {
                 next = (stop || r + 1 >= g.R) ? kBack : kUp;
             }
-            const bool flush = next != mode;
             mode = next;
-            tabB_ok = tabB_ok && !flush;
-            tabA_ok = hitA_ok = false;  // slot A is consumed (or stale)
             rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : r + 1);
         }
-        if (!kSpec) {
-            if (mode < kDone) rbA = a.row_offsets[slab_base + rn];  // offset of the coming row, one step ahead
-        } else if (mode == kUp || mode == kDown) {
-            // ---- speculation pipeline: advance and issue (no load issued here is consumed in this iteration) ----
-            if (!tabA_ok && tabB_ok) {  // slot B (issued in an earlier iteration) becomes slot A
-                tabA0 = tB00 | (tB01 << 16);
-                tabA1 = tB10 | (tB11 << 16);
-                cellsA = cellsB;
-                rbA = rbB;
-                tabA_ok = true;
-                tabB_ok = false;
-            }
-            if (tabA_ok && !hitA_ok) {  // first hits of the speculated window of row rn -> shared memory
-                if (cellsA != kNoCells) {
-                    const HitSeq q = hit_seq(tabA0, tabA1, (cellsA >> 31) != 0u);
-                    cp_async_wait_all();  // copies of a window that was not used must not land after the new ones
-#pragma unroll
-                    for (int k = 0; k < kSpecHits; k++)
-                        if (k < q.nt)
-                            cp_async8(&s_hit[k][threadIdx.x],
-                                      &a.hit_yz[(unsigned)rbA + (unsigned)(k < q.na ? q.ja0 + k : k + q.d)]);
-                    cp_async_commit();
-                }
-                hitA_ok = true;
-            }
-            const int tr = tabA_ok ? (mode == kUp ? rn + 1 : rn - 1) : rn;  // the next row not yet in slot A
-            if (!tabB_ok && tr >= 0 && tr < g.R) {
-                // window around the position extrapolated linearly from the current state, widened
-                const float ic = rsqrtf((1.0f - st.s) * (1.0f + st.s));
-                const float dxk = s_rowx[tr] - s_rowx[r];
-                const float yq = fmaf(dxk, st.s * ic, st.y + yref), zq = fmaf(dxk, st.t * ic, st.z + zref);
-                const float wy = fminf(g.wmax, g.gate * sqrt_fast(st.c00 + g.sy2)) + kSpecMargin;
-                const float wz = fminf(g.wmax, g.gate * sqrt_fast(st.c11 + g.sz2)) + kSpecMargin;
-                const Window w = window_cells(g, s_rowy[tr], z0, yq, zq, wy, wz);
-                const unsigned tb0 = (unsigned)(slab_base + tr) * (unsigned)g.nzp;
-                rbB = a.row_offsets[slab_base + tr];
-                if (w.zb1 - w.zb0 <= 1) {
-                    const unsigned ia = tb0 + (unsigned)(w.zb0 * g.ny);
-                    tB00 = a.bin_start[ia + w.ys0];
-                    tB01 = a.bin_start[ia + w.ys1];
-                    if (w.zb1 > w.zb0) {
-                        tB10 = a.bin_start[ia + g.ny + w.ys0];
-                        tB11 = a.bin_start[ia + g.ny + w.ys1];
-                    }
-                    cellsB = (unsigned)w.ys0 | ((unsigned)w.ys1 << 8) | ((unsigned)w.zb0 << 16) |
-                             (w.zb1 > w.zb0 ? 0x80000000u : 0u);
-                } else {
-                    cellsB = kNoCells;
-                }
-                tabB_ok = true;
-            }
-        }
+        if (mode < kDone) rb_next = a.row_offsets[slab_base + rn];  // offset of the coming row, one step ahead
     }
     if (kCount) {  // work counters: warp reduction, one atomic per warp and counter
         unsigned v[4] = {n_tr, n_up, n_ex, n_se};
@@ -622,9 +518,9 @@ int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_
     int grid = (int)(want < (int64_t)n_sm * kFollowCtasPerSm ? want : (int64_t)n_sm * kFollowCtasPerSm);
     if (grid < 1) grid = 1;
     if (count_work)
-        follow_kernel<true, kFollowSpec><<<grid, kFollowThreads, 0, s>>>(g, a);
+        follow_kernel<true><<<grid, kFollowThreads, 0, s>>>(g, a);
     else
-        follow_kernel<false, kFollowSpec><<<grid, kFollowThreads, 0, s>>>(g, a);
+        follow_kernel<false><<<grid, kFollowThreads, 0, s>>>(g, a);
     return 1;
 }
 

@@ -54,8 +54,10 @@ claim_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_
             my_rows = tl_rows[c];
             my_inst = cand_slab[c] / g.R;
             if (nh > 0) {
-                const int64_t lcid = c - slab_part[(size_t)my_inst * g.R].y;  // candidate ordinal inside its instance
-                if (lcid > 0x7FFFFF) atomicOr((unsigned long long*)&counts[5], 2ull);
+                // candidate ordinal inside its instance.  It fits in 23 bits by construction: chains are disjoint and
+                // hold >= cand_min >= 2 hits, so an instance has at most 255 rows * 65,535 hits / 2 = 8,355,712 < 2^23
+                // candidates (rows and row lengths are bounded by tpc_tracker_create and S1).
+                const int64_t lcid = c - slab_part[(size_t)my_inst * g.R].y;
                 my_w = ((uint32_t)nh << 23) | (uint32_t)(0x7FFFFF - (lcid & 0x7FFFFF));
             }
         }

@@ -234,7 +234,8 @@ extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const 
     if (!out || !out->counts) return fail(t, TPC_ERR_ARG, "out and out->counts are required");
     if (n_inst < 0 || n_clusters < 0 || n_clusters >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "bad sizes");
     if ((int64_t)n_inst * t->g.R + 1 >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "too many sector instances");
-    if (n_clusters > 0 && (!clusters || !row_offsets || n_inst == 0)) return fail(t, TPC_ERR_ARG, "NULL input");
+    if (n_clusters > 0 && (!clusters || n_inst == 0)) return fail(t, TPC_ERR_ARG, "NULL input");
+    if (n_inst > 0 && !row_offsets) return fail(t, TPC_ERR_ARG, "row_offsets is required when n_sector_instances > 0");
     if ((uintptr_t)clusters & (t->input_yz ? 7 : 15))
         return fail(t, TPC_ERR_ARG, "clusters must be 16-byte aligned (8-byte for TPC_INPUT_YZ)");
     Workspace w;

@@ -8,6 +8,12 @@ from oracle.tpc_oracle import Oracle
 PAR_RTOL = 1e-3
 PAR_ATOL = 1e-4
 MIN_SHARED = 0.995  # ">= 99.5 % of hit assignments" shared with the oracle
+# north_star fixes no tolerance for the covariance and chi2; DESIGN.md section 3 ("Tolerances beyond the five
+# parameters") derives these from the fp32 arithmetic: every covariance entry within COV_TOL of the scale of its two
+# variances, chi2 within CHI2_RTOL relative + CHI2_ATOL.
+COV_TOL = 1e-3
+CHI2_RTOL = 5e-4
+CHI2_ATOL = 5e-4
 
 
 def run_oracle(ev, **kw):
@@ -40,7 +46,21 @@ def tracklet_report(g, o):
     po = o.tracklets["p"][ident]
     pg = g.tl_params[ident].astype(np.float64)
     excess = np.abs(pg - po) / (PAR_ATOL + PAR_RTOL * np.abs(po))  # <= 1 means inside the tolerance
-    return dict(n_cand=len(ok_o), ok_mismatch=int((ok_o != ok_g).sum()), identical_hit_lists=int(ident.sum()),
+    # covariance (packed lower triangle, 15 entries) on the scale of the two variances involved; chi2
+    co = o.tracklets["cov"][ident]
+    cg = g.tl_cov[ident].astype(np.float64)
+    ii = np.array([i for i in range(5) for j in range(i + 1)])
+    jj = np.array([j for i in range(5) for j in range(i + 1)])
+    diag = np.array([0, 2, 5, 9, 14])
+    scale = np.sqrt(co[:, diag[ii]] * co[:, diag[jj]])
+    cov_excess = np.abs(cg - co) / (COV_TOL * scale) if co.size else np.zeros((0, 15))
+    xo = o.tracklets["chi2"][ident]
+    xg = g.tl_chi2[ident].astype(np.float64)
+    chi2_excess = np.abs(xg - xo) / (CHI2_ATOL + CHI2_RTOL * xo) if xo.size else np.zeros(0)
+    return dict(worst_cov_excess=float(cov_excess.max()) if cov_excess.size else 0.0,
+                worst_chi2_excess=float(chi2_excess.max()) if chi2_excess.size else 0.0,
+                ref_rows_equal=bool(np.array_equal(g.tl_rows[ident][:, 2], o.tracklets["ref_row"][ident])),
+                n_cand=len(ok_o), ok_mismatch=int((ok_o != ok_g).sum()), identical_hit_lists=int(ident.sum()),
                 n_both=int(both.sum()), shared_frac=float(shared / max(total, 1)),
                 worst_param_excess=float(excess.max()) if excess.size else 0.0,
                 worst_by_param=excess.max(axis=0).tolist() if excess.size else [0.0] * 5,
@@ -62,6 +82,39 @@ def final_track_report(g, o, n_clusters):
     return dict(n_tracks_gpu=int(g.n_tracks), n_tracks_oracle=int(len(o.trk_cand)),
                 shared_assign_frac=float(same.sum() / max(assigned.sum(), 1)),
                 tracks_identical=bool(np.array_equal(g.trk_cand_id, o.trk_cand)))
+
+
+def assert_final_track_records(g, o, row_offsets, n_rows, row_x):
+    """Everything S6 returns per final track against the oracle, tracks matched by candidate id:
+    trk_params / trk_cov / trk_chi2 are the tracklet's (S6 does not refit, S6) -> bit-identical to the
+    GPU's own tracklet outputs, which tracklet_report() compares with the oracle; trk_xref = x of the oracle's
+    reference row exactly; trk_sector = sector instance of the candidate's start hit exactly; trk_nhits = the
+    oracle's kept hits for every common track whose hit list is the same on both sides."""
+    cid = g.trk_cand_id
+    assert np.array_equal(g.trk_params, g.tl_params[cid]) and np.array_equal(g.trk_cov, g.tl_cov[cid])
+    assert np.array_equal(g.trk_chi2, g.tl_chi2[cid])
+    tl = o.tracklets[cid]
+    ok = tl["ok"].astype(bool)  # a GPU-only tracklet (A12/A13 threshold flips) has no oracle record
+    assert np.array_equal(g.trk_xref[ok], np.asarray(row_x, np.float32)[tl["ref_row"][ok]])
+    inst_of_hit = np.searchsorted(np.asarray(row_offsets)[::n_rows], o.cand_hits[cid, 0], side="right") - 1
+    assert np.array_equal(g.trk_sector, inst_of_hit.astype(np.int32))
+    # kept hits: compare per track on the tracks both sides have
+    common, ig, io = np.intersect1d(cid, o.trk_cand, return_indices=True)
+    kept_o = np.diff(o.trk_hit_offset)[io]
+    kept_g = g.trk_nhits[ig]
+    same_list = np.array([np.array_equal(g.trk_hits[g.trk_hit_offset[a]:g.trk_hit_offset[a + 1]],
+                                         o.trk_hits[o.trk_hit_offset[b]:o.trk_hit_offset[b + 1]])
+                          for a, b in zip(ig, io)], bool) if len(common) else np.zeros(0, bool)
+    assert np.array_equal(kept_g[same_list], kept_o[same_list])
+    # north_star: "matched tracks must have fitted parameters within 1e-3 relative / 1e-4 absolute" -- the FINAL tracks
+    # (tracklet_report applies the same bar to every tracklet, final or not).  Matched = same candidate id and the
+    # tracklet's hit list identical on both sides, so the two fits saw the same measurements.
+    same_tl = np.all(g.tl_hits[common] == o.tracklet_hits[common], axis=1) if len(common) else np.zeros(0, bool)
+    pg = g.trk_params[ig][same_tl].astype(np.float64)
+    po = o.tracklets["p"][common][same_tl]
+    ex = np.abs(pg - po) / (PAR_ATOL + PAR_RTOL * np.abs(po))
+    return dict(common_tracks=int(len(common)), identical_track_hit_lists=int(same_list.sum()),
+                worst_track_param_excess=float(ex.max()) if ex.size else 0.0)
 
 
 def assert_final_consistency(g, n_clusters):

@@ -9,8 +9,8 @@ import pytest
 
 from paper_1709_00618_b200 import datagen as dg
 
-from parity_util import (MIN_SHARED, assert_ca_bit_exact, assert_final_consistency, final_track_report, run_oracle,
-                         tracklet_report)
+from parity_util import (MIN_SHARED, assert_ca_bit_exact, assert_final_consistency, assert_final_track_records,
+                         final_track_report, run_oracle, tracklet_report)
 
 pytestmark = pytest.mark.gpu
 
@@ -46,11 +46,15 @@ def _check(ev, max_ok_mismatch=0):
     tr = tracklet_report(g, o)
     fr = final_track_report(g, o, ev.n_clusters)
     assert_final_consistency(g, ev.n_clusters)
+    rec = assert_final_track_records(g, o, ev.row_offsets, ev.n_rows, dg.row_x(ev.n_rows))
     os.makedirs("gpurun_out", exist_ok=True)
     with open("gpurun_out/parity_report.jsonl", "a") as f:
-        f.write(json.dumps(dict(case=ev.name, n_clusters=ev.n_clusters, **tr, **fr)) + "\n")
+        f.write(json.dumps(dict(case=ev.name, n_clusters=ev.n_clusters, **tr, **fr, **rec)) + "\n")
     assert tr["ok_mismatch"] <= max_ok_mismatch, tr
     assert tr["shared_frac"] >= MIN_SHARED and tr["worst_param_excess"] <= 1.0, tr
+    assert rec["worst_track_param_excess"] <= 1.0, rec
+    assert tr["nhits_equal"] and tr["rows_equal"] and tr["ref_rows_equal"], tr
+    assert tr["worst_cov_excess"] <= 1.0 and tr["worst_chi2_excess"] <= 1.0, tr
     if fr["n_tracks_gpu"] or fr["n_tracks_oracle"]:
         assert fr["shared_assign_frac"] >= MIN_SHARED, fr
     return g, o
@@ -129,8 +133,9 @@ def test_full_size_drift_windows_against_oracle():
     # A tracklet exists or not by threshold tests on the fitted state (|sinPhi| <= 0.95 in a transport): fp64 in the
     # oracle, fp32 in the kernels (A12/A13), so at this size a handful of the ~130 k candidates may fall on
     # the other side; they count against the 99.5 % shared-assignment bar like any other difference.
-    g, o = _check(batch, max_ok_mismatch=batch.n_clusters // 200_000)
-    assert abs(g.n_tracks - len(o.trk_cand)) <= 5
+    # Observed: 1 of 130,252 candidates (round 1); the allowance is observed + 1.
+    g, o = _check(batch, max_ok_mismatch=2)
+    assert abs(g.n_tracks - len(o.trk_cand)) <= 2
 
 
 def test_compact_yz_input_equals_xyzw():
@@ -175,4 +180,73 @@ def test_full_size_central_event_against_oracle():
     """CFG:3 at full size: 8,000 primaries + 20 % secondaries, 10 % noise, ~1.5 M clusters, ~260 hits per row."""
     ev = dg.central_event(seed=3001)
     assert ev.n_clusters > 1_000_000
-    _check(ev, max_ok_mismatch=ev.n_clusters // 200_000)
+    _check(ev, max_ok_mismatch=2)  # observed 1 of 73,605 tracklets (A12/A13 threshold in fp32 vs fp64), + 1
+
+
+def test_dense_rows_unstaged_neighbour_search():
+    """Rows of 700-1000 hits (2,000 tracks in one sector): rows r-1 and r+1 together exceed the 1,024 hits S2 stages
+    in shared memory, so the neighbour rows are read in place; more than two hits per thread in S1."""
+    ev = dg.single_sector(seed=1031, n_tracks=2000)
+    n_row = np.diff(ev.row_offsets)
+    assert (n_row[:-2] + n_row[2:]).max() > 1024 and n_row.max() > 600
+    _check(ev)
+
+
+def test_many_nearly_empty_instances():
+    """3,600 sector instances with a handful of tracks each: the per-instance bookkeeping (cell tables, slab scans,
+    candidate bases) at a large instance count and tiny rows."""
+    evs = [dg.full_event(seed=2100 + i, n_prim=12, noise=0.0) for i in range(100)]
+    batch = dg.concat_events(evs)
+    assert batch.n_inst == 3600
+    g, o = _check(batch)
+    assert g.n_tracks > 500
+
+
+def test_row_longer_than_16_bit_limit_is_flagged():
+    """A pad row with more than 65,535 clusters cannot be indexed by the 16-bit local positions: the call flags it
+    (counts[5] bit 0 -> TPC_ERR_INPUT from tpc_check_counts), stays inside its buffers and leaves the tracker usable."""
+    from paper_1709_00618_b200 import Tracker
+    from paper_1709_00618_b200.tracker import TpcError
+    ev = dg.single_sector(seed=1001)
+    rows = _rows_of(ev)
+    rng = np.random.default_rng(3)
+    n_big = 66_000
+    x = np.full(n_big, dg.row_x(ev.n_rows)[100])
+    blob = np.stack([x, rng.uniform(-30, 30, n_big), rng.uniform(0, 250, n_big), np.full(n_big, -1.0)],
+                    axis=1).astype(np.float32)
+    big = _rebuild(ev, np.concatenate([ev.clusters, blob]), np.concatenate([rows, np.full(n_big, 100)]))
+    assert np.diff(big.row_offsets).max() > 65_535
+    trk = Tracker.for_event(big)
+    with pytest.raises(TpcError, match="TPC_ERR_INPUT"):
+        trk.track_sectors(big.clusters, big.row_offsets, big.n_inst, debug=True)
+    ok = trk.track_sectors(ev.clusters, ev.row_offsets, ev.n_inst, debug=True)  # same handle, legal input
+    o = run_oracle(ev)
+    assert_ca_bit_exact(ok, o)
+    trk.close()
+
+
+def test_null_row_offsets_is_rejected():
+    """n_sector_instances > 0 with row_offsets == NULL must be an argument error, not a device fault."""
+    import ctypes as C
+    import torch
+    from paper_1709_00618_b200 import Tracker
+    ev = dg.single_sector(seed=1001)
+    trk = Tracker.for_event(ev)
+    trk.reserve(16, 1)
+    trk.set_stream()
+    bufs, out = trk.alloc_outputs(16)
+    rc = trk.lib.tpc_track_sectors(trk._h, None, None, 1, 0, C.byref(out))
+    assert rc == -1
+    torch.cuda.synchronize()
+    trk.close()
+
+
+def test_twenty_drift_windows_against_oracle():
+    """20 full CFG:4 windows in one call (720 sector instances, ~23 M clusters): the parameter tolerance at a fifth of
+    the bench size (the worst excess grows with the sample; DESIGN.md section 6 quotes this figure)."""
+    evs = [dg.drift_window(seed=5001 + i) for i in range(20)]
+    batch = dg.concat_events(evs)
+    assert batch.n_clusters > 15_000_000
+    # A12/A13 threshold flips: observed 1 per ~130 k candidates -> ~8 expected in ~1 M; allowance 12
+    g, o = _check(batch, max_ok_mismatch=12)
+    assert abs(g.n_tracks - len(o.trk_cand)) <= 8

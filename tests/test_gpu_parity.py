@@ -11,8 +11,8 @@ import pytest
 
 from paper_1709_00618_b200 import datagen as dg
 
-from parity_util import (MIN_SHARED, assert_ca_bit_exact, assert_final_consistency, final_track_report, run_oracle,
-                         tracklet_report)
+from parity_util import (MIN_SHARED, assert_ca_bit_exact, assert_final_consistency, assert_final_track_records,
+                         final_track_report, run_oracle, tracklet_report)
 
 pytestmark = pytest.mark.gpu
 
@@ -25,21 +25,24 @@ def _gpu(ev, **kw):
     return res
 
 
-def _full_parity(ev, label):
+def _full_parity(ev, label, check_cov=True):
     o = run_oracle(ev)
     g = _gpu(ev)
     assert_ca_bit_exact(g, o)
     tr = tracklet_report(g, o)
     fr = final_track_report(g, o, ev.n_clusters)
     assert_final_consistency(g, ev.n_clusters)
-    rep = dict(case=label, n_clusters=ev.n_clusters, **tr, **fr)
+    rec = assert_final_track_records(g, o, ev.row_offsets, ev.n_rows, dg.row_x(ev.n_rows))
+    rep = dict(case=label, n_clusters=ev.n_clusters, **tr, **fr, **rec)
     os.makedirs("gpurun_out", exist_ok=True)
     with open("gpurun_out/parity_report.jsonl", "a") as f:
         f.write(json.dumps(rep) + "\n")
     assert tr["ok_mismatch"] == 0, rep
     assert tr["shared_frac"] >= MIN_SHARED, rep
-    assert tr["worst_param_excess"] <= 1.0, rep
-    assert tr["nhits_equal"] and tr["rows_equal"], rep
+    assert tr["worst_param_excess"] <= 1.0 and rec["worst_track_param_excess"] <= 1.0, rep
+    assert tr["nhits_equal"] and tr["rows_equal"] and tr["ref_rows_equal"], rep
+    if check_cov:
+        assert tr["worst_cov_excess"] <= 1.0 and tr["worst_chi2_excess"] <= 1.0, rep
     assert fr["shared_assign_frac"] >= MIN_SHARED, rep
     assert int(g.counts[2]) == int(o.tracklets["ok"].sum())
     return g, o, rep
@@ -56,7 +59,10 @@ def test_cfg1_other_seeds(seed):
 
 def test_cfg1_variants_zero_field_zero_smear():
     _full_parity(dg.single_sector(seed=1004, bz=0.0), "cfg1_bz0")
-    _full_parity(dg.single_sector(seed=1005, sigma_y=0.0, sigma_z=0.0, noise=0.0), "cfg1_clean")
+    # zero smear: the cluster error handed to the filter is 1e-3 cm, a few ulp of the fp32 coordinates themselves, so
+    # residuals (chi2) and the covariance built from them are rounding noise of the INPUT on both sides; the hit
+    # lists and the five parameters are still held to the bar
+    _full_parity(dg.single_sector(seed=1005, sigma_y=0.0, sigma_z=0.0, noise=0.0), "cfg1_clean", check_cov=False)
 
 
 def test_cfg2_peripheral_event():
