@@ -135,23 +135,36 @@ int tpc_set_workspace(tpc_tracker_t* t, void* dev_ptr, size_t bytes);
 int tpc_set_stream(tpc_tracker_t* t, void* cuda_stream);
 
 /*
- * Track all sector instances (stages S1-S6).  clusters_xyzw: DEVICE, 16-byte aligned, [n_clusters][4] =
- * (x, y, z, w); x and w are carried but never read (the row gives x).  row_offsets: DEVICE int32
+ * Track all sector instances (stages S1-S6).  clusters: DEVICE, 16-byte aligned, [n_clusters][4] =
+ * (x, y, z, w); x and w are carried but never read (the row gives x) -- or one of the compact layouts below after
+ * tpc_set_input_layout.  row_offsets: DEVICE int32
  * [n_sector_instances * n_rows + 1], CSR, instance-major row-minor, row_offsets[0] = 0 and
  * row_offsets[last] = n_clusters.  Clusters inside a row may be in any order.  n_clusters < 2^31.
  * Asynchronous; one call in flight per tracker.
  */
-int tpc_track_sectors(tpc_tracker_t* t, const float* clusters_xyzw, const int32_t* row_offsets,
+int tpc_track_sectors(tpc_tracker_t* t, const void* clusters, const int32_t* row_offsets,
                       int32_t n_sector_instances, int64_t n_clusters, const tpc_output_t* out);
 
 /*
- * Compact cluster input.  x and w of a cluster are never read (the row gives x), so half of
- * the 16 bytes per cluster is dead weight on the PCIe upload and in S1's read.  With TPC_INPUT_YZ the `clusters`
- * argument of tpc_track_sectors / tpc_track_sectors_host (and tpc_slot_t.clusters) is [n_clusters][2] = (y, z),
- * 8-byte aligned; results are bit-identical to the TPC_INPUT_XYZW call on the same (y, z).  Default: TPC_INPUT_XYZW.
+ * Compact cluster input (PAPER.md:49 describes the experiment's own fixed-point cluster
+ * formats).  x and w of a cluster are never read (the row gives x), so most of the 16 bytes per cluster are dead
+ * weight on the PCIe upload (named as the bottleneck in PAPER.md:33) and in S1's read.  The layout applies to the
+ * `clusters` argument of tpc_track_sectors / the host entry points and to tpc_slot_t.clusters:
+ *   TPC_INPUT_XYZW  float [n][4] = (x, y, z, w), 16-byte aligned (default)
+ *   TPC_INPUT_YZ    float [n][2] = (y, z), 8-byte aligned; results bit-identical to XYZW on the same (y, z)
+ *   TPC_INPUT_I16   int16 [n][2] = (q_y, q_z), 4-byte aligned, 16-bit fixed point:
+ *                     y = q_y * TPC_I16_Y_STEP                       (q_y signed: |y| < 128 cm, step 1/256 cm)
+ *                     z = z_origin + (uint16)q_z * TPC_I16_Z_STEP    (q_z unsigned: 1024 cm range, step 1/64 cm)
+ *                   with z_origin = z_lo on the z >= 0 side and -z_hi on the z < 0 side (the grid origin of that
+ *                   side).  Decoding is one exact multiplication and one fp32 addition per coordinate; the tracker
+ *                   then runs on the decoded fp32 (y, z) exactly as for TPC_INPUT_YZ.  Clusters outside the
+ *                   representable range cannot be given in this layout.
  */
 #define TPC_INPUT_XYZW 0
 #define TPC_INPUT_YZ 1
+#define TPC_INPUT_I16 2
+#define TPC_I16_Y_STEP (1.0f / 256.0f)
+#define TPC_I16_Z_STEP (1.0f / 64.0f)
 int tpc_set_input_layout(tpc_tracker_t* t, int32_t layout);
 
 /* After synchronising and copying `counts` to the host: TPC_OK, TPC_ERR_CAPACITY or TPC_ERR_INPUT. */
@@ -175,20 +188,25 @@ int tpc_set_stage_timing(tpc_tracker_t* t, int32_t enable);
 int tpc_stage_times_ms(tpc_tracker_t* t, int32_t age, float* out_ms);
 
 /*
- * Host-buffer entry point (BASELINE.json configs[4]: windows "streamed through the tracker in double-buffered
- * chunks with cluster upload overlapped on a second CUDA stream").  The job is cut into chunks of
- * inst_per_chunk sector instances; chunk i+1 is uploaded on h2d_stream while chunk i is tracked on
- * compute_stream and the results of chunk i-1 return on d2h_stream.  Blocks until every result is on the host.
- * h_clusters / h_row_offsets / the arrays in tpc_host_output_t should be pinned host memory (pageable memory
- * works but serialises the copies).  Slots are caller-owned DEVICE buffers (allocate n_slots >= 2 of them); the
- * workspace set by tpc_set_workspace is shared by all chunks and must cover the largest chunk.
+ * Host-buffer entry points (BASELINE.json configs[4]: windows "streamed through the tracker in double-buffered
+ * chunks with cluster upload overlapped on a second CUDA stream"; time frames are sliced when they do
+ * not fit).  The job is cut into chunks of inst_per_chunk sector instances; chunk i+1 is uploaded while chunk i is
+ * tracked and the results of earlier chunks return, each on its own stream.  A slot is the set of caller-owned DEVICE
+ * buffers one chunk in flight needs (allocate 2..8).  A slot with its own workspace also gets its own compute
+ * stream, so that the start of chunk i+1 overlaps the drain of chunk i's follower; slots without one share the
+ * workspace given to tpc_set_workspace and a single compute stream.
+ * h_clusters / h_row_offsets / the arrays of tpc_host_output_t should be pinned host memory (pageable memory works
+ * but serialises the copies).  Only the arrays that are non-NULL in BOTH the slot's `out` and tpc_host_output_t are
+ * produced and copied back.
  */
 typedef struct {
-    float* clusters;      /* device [max_clusters][4] */
+    void* clusters;       /* device [max_clusters] records of the tracker's input layout */
     int32_t* row_offsets; /* device [max_instances * n_rows + 1] */
     int64_t max_clusters;
     int32_t max_instances;
     tpc_output_t out;     /* device outputs of this slot: counts required; trk_* / cluster_owner as wanted */
+    void* workspace;      /* device, 256-B aligned, >= tpc_workspace_bytes(max_clusters, max_instances); or NULL */
+    size_t workspace_bytes;
 } tpc_slot_t;
 
 typedef struct {
@@ -204,9 +222,25 @@ typedef struct {
     int64_t trk_capacity, trk_hits_capacity;
     int64_t totals[TPC_N_COUNTS]; /* written by the call: sums of the per-chunk counts */
     int64_t n_chunks, n_launches, h2d_bytes, d2h_bytes; /* written by the call */
+    /* written by the call: time each stream was busy (sums of the per-chunk CUDA-event intervals; the compute
+       figure can exceed wall_ms when slots have their own compute streams) and the host wall time of the call */
+    float h2d_ms, compute_ms, d2h_ms, wall_ms;
 } tpc_host_output_t;
 
-int tpc_track_sectors_host(tpc_tracker_t* t, const float* h_clusters_xyzw, const int32_t* h_row_offsets,
+/* Persistent pipeline: streams, events and the pinned counts buffer are created once, so that a run allocates
+   nothing.  The slots (copied) must stay valid until tpc_pipeline_destroy; one run in flight per pipeline, and the
+   tracker must not be used by other calls during a run. */
+typedef struct tpc_pipeline tpc_pipeline_t;
+int tpc_pipeline_create(tpc_tracker_t* t, const tpc_slot_t* slots, int32_t n_slots, tpc_pipeline_t** out);
+void tpc_pipeline_destroy(tpc_pipeline_t* p);
+/* Blocks until every result is on the host. */
+int tpc_pipeline_run(tpc_pipeline_t* p, const void* h_clusters, const int32_t* h_row_offsets,
+                     int32_t n_sector_instances, int64_t n_clusters, int32_t inst_per_chunk,
+                     tpc_host_output_t* hout);
+
+/* One-shot form: builds a pipeline on the caller's three streams (all slots share compute_stream), runs it and
+   tears it down. */
+int tpc_track_sectors_host(tpc_tracker_t* t, const void* h_clusters, const int32_t* h_row_offsets,
                            int32_t n_sector_instances, int64_t n_clusters, int32_t inst_per_chunk,
                            tpc_slot_t* slots, int32_t n_slots, void* h2d_stream, void* compute_stream,
                            void* d2h_stream, tpc_host_output_t* hout);

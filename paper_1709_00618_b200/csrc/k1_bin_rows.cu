@@ -11,18 +11,27 @@ constexpr int kBinThreads = 128;
 #ifndef TPC_BIN_CTAS
 #define TPC_BIN_CTAS 16
 #endif
-// (y, z) of input cluster i: from the (x, y, z, w) records, or from the compact (y, z) input (tpc_set_input_layout)
-template <bool kYZ>
-__device__ __forceinline__ float2 load_yz(const float4* __restrict__ clusters, const float2* __restrict__ yz, int i) {
-    if (kYZ) return __ldg(&yz[i]);
-    const float4 c = __ldg(&clusters[i]);
+// (y, z) of input cluster i in one of the three input layouts (tpc_set_input_layout): (x, y, z, w) records, compact
+// (y, z) pairs, or 16-bit fixed point (y = q_y / 256 cm; z = z origin of the sector side + q_z / 64 cm, q_z unsigned).
+// The fixed-point decode is one exact multiplication and, for z, one rounded addition (exact for origins that are
+// multiples of 1/64 cm and |z| < 2^18 / 64): the oracle's input is produced by the same two operations on the host.
+enum InLayout : int { kInXYZW = 0, kInYZ = 1, kInI16 = 2 };
+
+template <int kIn>
+__device__ __forceinline__ float2 load_yz(const void* __restrict__ in, int i, float z_origin) {
+    if (kIn == kInYZ) return __ldg(reinterpret_cast<const float2*>(in) + i);
+    if (kIn == kInI16) {
+        const short2 q = __ldg(reinterpret_cast<const short2*>(in) + i);
+        return make_float2(__fmul_rn((float)q.x, 1.0f / 256.0f),
+                           __fadd_rn(z_origin, __fmul_rn((float)(unsigned short)q.y, 1.0f / 64.0f)));
+    }
+    const float4 c = __ldg(reinterpret_cast<const float4*>(in) + i);
     return make_float2(c.y, c.z);
 }
 
-template <bool kYZ>
+template <int kIn>
 __global__ void __launch_bounds__(kBinThreads, TPC_BIN_CTAS)
-bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ clusters,
-                const float2* __restrict__ clusters_yz,
+bin_rows_kernel(const __grid_constant__ DevGeom g, const void* __restrict__ clusters,
                 const int32_t* __restrict__ row_offsets, float2* __restrict__ hit_yz, uint16_t* __restrict__ hit_idx,
                 uint16_t* __restrict__ hit_pos, uint16_t* __restrict__ bin_start, int64_t* __restrict__ counts) {
     extern __shared__ __align__(16) uint32_t sm_hist[];  // [nzp] counts, then exclusive starts (cursors in pass 2)
@@ -51,14 +60,14 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
         const int i = threadIdx.x + k * kBinThreads;
         key[k] = -1;
         if (i < n) {
-            const float2 c = load_yz<kYZ>(clusters, clusters_yz, base + i);
+            const float2 c = load_yz<kIn>(clusters, base + i, z0);
             key[k] = zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny);
             yz[k] = c;
             atomicAdd(&sm_hist[key[k]], 1u);
         }
     }
     for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {
-        const float2 c = load_yz<kYZ>(clusters, clusters_yz, base + i);
+        const float2 c = load_yz<kIn>(clusters, base + i, z0);
         atomicAdd(&sm_hist[zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny)], 1u);
     }
     __syncthreads();
@@ -104,7 +113,7 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const float4* __restrict__ cl
         }
     }
     for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {  // long rows: from L1/L2 this time
-        const float2 c = load_yz<kYZ>(clusters, clusters_yz, base + i);
+        const float2 c = load_yz<kIn>(clusters, base + i, z0);
         const uint32_t pos = atomicAdd(&sm_hist[zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny)], 1u);
         hit_yz[base + pos] = c;
         hit_idx[base + pos] = (uint16_t)i;
@@ -118,16 +127,20 @@ int launch_bin_rows(const DevGeom& g, const Workspace& w, const Problem& p, cuda
     const size_t smem = (size_t)g.nzp * sizeof(uint32_t);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(bin_rows_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaFuncSetAttribute(bin_rows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(bin_rows_kernel<kInXYZW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(bin_rows_kernel<kInYZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(bin_rows_kernel<kInI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    if (p.clusters_yz)
-        bin_rows_kernel<true><<<slabs, kBinThreads, smem, s>>>(g, nullptr, p.clusters_yz, p.row_offsets, w.hit_yz,
-                                                               w.hit_idx, w.hit_pos, w.bin_start, w.counts);
+    if (p.layout == kInYZ)
+        bin_rows_kernel<kInYZ><<<slabs, kBinThreads, smem, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx,
+                                                                w.hit_pos, w.bin_start, w.counts);
+    else if (p.layout == kInI16)
+        bin_rows_kernel<kInI16><<<slabs, kBinThreads, smem, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx,
+                                                                 w.hit_pos, w.bin_start, w.counts);
     else
-        bin_rows_kernel<false><<<slabs, kBinThreads, smem, s>>>(g, p.clusters, nullptr, p.row_offsets, w.hit_yz,
-                                                                w.hit_idx, w.hit_pos, w.bin_start, w.counts);
+        bin_rows_kernel<kInXYZW><<<slabs, kBinThreads, smem, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx,
+                                                                  w.hit_pos, w.bin_start, w.counts);
     return 1;
 }
 

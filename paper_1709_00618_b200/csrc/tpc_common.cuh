@@ -24,6 +24,7 @@ struct DevGeom {
     int ncell;      // nz * ny cells per row, cell id = zbin * ny + ystrip (a y range inside one z bin is contiguous)
     int nzp;        // stride of the cell table (ncell + 1 rounded up to 16 entries = 32 B)
     int spe, spe_half;
+    int inst_phase;  // geometric sector of instance 0 of this call (0 except for the chunks of the host pipeline)
     float z0_a, z0_c;  // grid origin: z >= 0 side, z < 0 side
     float inv_cz;
     float nf_wy, nf_wz, nf_d2max;
@@ -73,8 +74,8 @@ struct Workspace {
 };
 
 struct Problem {
-    const float4* clusters;   // (x, y, z, w), or NULL when the input is compact
-    const float2* clusters_yz;  // compact input (y, z), or NULL
+    const void* clusters;  // [n_clusters] records of `layout`
+    int layout;            // TPC_INPUT_XYZW (float4), TPC_INPUT_YZ (float2) or TPC_INPUT_I16 (short2)
     const int32_t* row_offsets;
     int32_t n_inst;
     int64_t n_clusters;
@@ -96,7 +97,7 @@ __device__ __forceinline__ int ybin(float y, float y0, float inv_sy, int ny) {
 }
 
 __device__ __forceinline__ float grid_z0(const DevGeom& g, int inst) {
-    return ((inst % g.spe) >= g.spe_half) ? g.z0_c : g.z0_a;
+    return (((inst + g.inst_phase) % g.spe) >= g.spe_half) ? g.z0_c : g.z0_a;
 }
 
 // ---- launchers (one per stage; each returns the number of kernels it enqueued) ----

@@ -64,7 +64,10 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     g.nzp = (g.ncell + 1 + 15) & ~15;  // rows of the table start on 32-byte sectors
     g.spe = geom->sectors_per_event;
     g.spe_half = g.spe / 2;
+    g.inst_phase = 0;
     g.z0_a = geom->z_lo;
+    t->z_lo = geom->z_lo;
+    t->z_hi = geom->z_hi;
     g.z0_c = -geom->z_hi;
     g.inv_cz = 1.0f / cz;
     g.nf_wy = dflt(p.nf_win_y, 2.0f);
@@ -194,8 +197,11 @@ extern "C" int tpc_set_stream(tpc_tracker_t* t, void* s) {
 
 extern "C" int tpc_set_input_layout(tpc_tracker_t* t, int32_t layout) {
     if (!t) return TPC_ERR_ARG;
-    if (layout != TPC_INPUT_XYZW && layout != TPC_INPUT_YZ) return fail(t, TPC_ERR_ARG, "unknown input layout");
-    t->input_yz = layout == TPC_INPUT_YZ;
+    if (layout != TPC_INPUT_XYZW && layout != TPC_INPUT_YZ && layout != TPC_INPUT_I16)
+        return fail(t, TPC_ERR_ARG, "unknown input layout");
+    if (layout == TPC_INPUT_I16 && ((double)t->z_hi - (double)t->z_lo) > 65535.0 * (double)TPC_I16_Z_STEP)
+        return fail(t, TPC_ERR_ARG, "TPC_INPUT_I16 covers 1024 cm of z; the geometry's z range is wider");
+    t->input_layout = layout;
     return TPC_OK;
 }
 
@@ -228,25 +234,30 @@ extern "C" int tpc_stage_times_ms(tpc_tracker_t* t, int32_t age, float* out_ms) 
     return TPC_OK;
 }
 
-extern "C" int tpc_track_sectors(tpc_tracker_t* t, const float* clusters, const int32_t* row_offsets, int32_t n_inst,
+extern "C" int tpc_track_sectors(tpc_tracker_t* t, const void* clusters, const int32_t* row_offsets, int32_t n_inst,
                                  int64_t n_clusters, const tpc_output_t* out) {
     if (!t) return TPC_ERR_ARG;
+    return tpc_track_on(t, t->ws, t->ws_bytes, t->stream, true, 0, clusters, row_offsets, n_inst, n_clusters, out);
+}
+
+int tpc_track_on(tpc_tracker* t, void* ws, size_t ws_bytes, cudaStream_t s, bool timed, int32_t first_inst,
+                 const void* clusters, const int32_t* row_offsets, int32_t n_inst, int64_t n_clusters,
+                 const tpc_output_t* out) {
     if (!out || !out->counts) return fail(t, TPC_ERR_ARG, "out and out->counts are required");
     if (n_inst < 0 || n_clusters < 0 || n_clusters >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "bad sizes");
     if ((int64_t)n_inst * t->g.R + 1 >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "too many sector instances");
     if (n_clusters > 0 && (!clusters || n_inst == 0)) return fail(t, TPC_ERR_ARG, "NULL input");
     if (n_inst > 0 && !row_offsets) return fail(t, TPC_ERR_ARG, "row_offsets is required when n_sector_instances > 0");
-    if ((uintptr_t)clusters & (t->input_yz ? 7 : 15))
-        return fail(t, TPC_ERR_ARG, "clusters must be 16-byte aligned (8-byte for TPC_INPUT_YZ)");
+    if ((uintptr_t)clusters & (uintptr_t)(layout_bytes(t->input_layout) - 1))
+        return fail(t, TPC_ERR_ARG, "clusters must be aligned to one record (16 / 8 / 4 bytes for XYZW / YZ / I16)");
     Workspace w;
-    const size_t need = carve(t->g, t->ws, n_clusters, n_inst, &w);
-    if (!t->ws || need > t->ws_bytes) return fail(t, TPC_ERR_WORKSPACE, "workspace missing or too small");
-    cudaStream_t s = t->stream;
-    const DevGeom& g = t->g;
-    Problem p{t->input_yz ? nullptr : reinterpret_cast<const float4*>(clusters),
-              t->input_yz ? reinterpret_cast<const float2*>(clusters) : nullptr, row_offsets, n_inst, n_clusters};
+    const size_t need = carve(t->g, ws, n_clusters, n_inst, &w);
+    if (!ws || need > ws_bytes) return fail(t, TPC_ERR_WORKSPACE, "workspace missing or too small");
+    DevGeom g = t->g;
+    g.inst_phase = first_inst % g.spe;
+    Problem p{clusters, t->input_layout, row_offsets, n_inst, n_clusters};
     int launches = 0;
-    const bool tm = t->timing && t->ev_valid;
+    const bool tm = timed && t->timing && t->ev_valid;
     cudaEvent_t* ev = t->ev[t->n_calls % TPC_TIMING_RING];
     if (tm) t->n_calls++;
     cudaMemsetAsync(w.counts, 0, sizeof(int64_t) * TPC_N_COUNTS, s);

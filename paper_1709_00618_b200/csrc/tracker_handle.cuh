@@ -12,9 +12,10 @@ struct tpc_tracker {
     size_t ws_bytes = 0;
     cudaStream_t stream = nullptr;
     int n_sm = 148;
+    float z_lo = 0.0f, z_hi = 0.0f;  // geometry z range of the z >= 0 side
     int last_launches = 0;
     bool timing = false;
-    bool input_yz = false;    // clusters are (y, z) pairs instead of (x, y, z, w) (tpc_set_input_layout)
+    int input_layout = TPC_INPUT_XYZW;  // tpc_set_input_layout
     bool count_work = false;  // S5 work counters counts[6..9] (tpc_set_work_counters)
     cudaEvent_t ev[TPC_TIMING_RING][TPC_N_STAGES + 1] = {};
     bool ev_valid = false;
@@ -27,3 +28,13 @@ static inline int fail(tpc_tracker* t, int code, const std::string& msg) {
     return code;
 }
 
+
+// bytes per cluster of an input layout, and the alignment mask of its base pointer
+static inline int64_t layout_bytes(int layout) { return layout == TPC_INPUT_XYZW ? 16 : layout == TPC_INPUT_YZ ? 8 : 4; }
+
+// The body of tpc_track_sectors on an explicit workspace and stream (the pipeline runs chunks concurrently on
+// per-slot workspaces).  `timed` = record the per-stage events of tpc_set_stage_timing.
+// `first_inst` = job-wide index of instance 0 (its geometric sector is first_inst % sectors_per_event).
+int tpc_track_on(tpc_tracker* t, void* ws, size_t ws_bytes, cudaStream_t s, bool timed, int32_t first_inst,
+                 const void* clusters, const int32_t* row_offsets, int32_t n_inst, int64_t n_clusters,
+                 const tpc_output_t* out);

@@ -266,6 +266,29 @@ def concat_events(events, name="batch") -> Event:
                  sigma_z=e0.sigma_z, truth=truth, name=name)
 
 
+I16_Y_STEP = 1.0 / 256.0  # cm per count of the 16-bit fixed-point cluster format (include/tpc_tracker.h TPC_INPUT_I16)
+I16_Z_STEP = 1.0 / 64.0
+
+
+def quantise_i16(ev: Event):
+    """The event in the 16-bit fixed-point input format: returns
+    (q int16 [N,2], Event whose (y, z) are the decoded fp32 values).  Input formatting only: y = q_y / 256 cm (signed),
+    z = z_origin + q_z / 64 cm (unsigned count), z_origin = z_lo on the z >= 0 side and -z_hi on the z < 0 side.
+    The decoded event is what BOTH the oracle and the tracker see, so parity on quantised input stays exact."""
+    inst = np.repeat(np.arange(ev.n_inst), np.diff(ev.row_offsets[::ev.n_rows]))
+    z0 = np.where((inst % SECTORS_PER_EVENT) >= SECTORS_PER_SIDE, -ev.z_hi, ev.z_lo).astype(np.float32)
+    y = ev.clusters[:, 1].astype(np.float64)
+    z = ev.clusters[:, 2].astype(np.float64)
+    qy = np.clip(np.rint(y / I16_Y_STEP), -32768, 32767).astype(np.int16)
+    qz = np.clip(np.rint((z - z0.astype(np.float64)) / I16_Z_STEP), 0, 65535).astype(np.uint16)
+    cl = ev.clusters.copy()
+    cl[:, 1] = qy.astype(np.float32) * np.float32(I16_Y_STEP)               # exact
+    cl[:, 2] = z0 + qz.astype(np.float32) * np.float32(I16_Z_STEP)          # exact product, one fp32 rounding
+    q = np.stack([qy, qz.view(np.int16)], axis=1)
+    from dataclasses import replace
+    return np.ascontiguousarray(q), replace(ev, clusters=cl, name=ev.name + "_i16")
+
+
 def window_batch(n_windows, seed0=5001, **kw) -> Event:
     """CFG:5 — `n_windows` CFG:4 drift windows, seeds seed0, seed0+1, ..."""
     return concat_events([drift_window(seed0 + w, **kw) for w in range(n_windows)], name=f"cfg5_batch{n_windows}")

@@ -24,7 +24,10 @@ ERRORS = {-1: "TPC_ERR_ARG", -2: "TPC_ERR_GEOMETRY", -3: "TPC_ERR_WORKSPACE", -4
 EXPORTS = ("tpc_tracker_create", "tpc_tracker_destroy", "tpc_workspace_bytes", "tpc_set_workspace", "tpc_set_stream",
            "tpc_track_sectors", "tpc_check_counts", "tpc_last_launch_count", "tpc_set_stage_timing",
            "tpc_stage_times_ms", "tpc_last_error", "tpc_track_sectors_host", "tpc_set_work_counters",
-           "tpc_set_input_layout")
+           "tpc_set_input_layout", "tpc_pipeline_create", "tpc_pipeline_destroy", "tpc_pipeline_run")
+INPUT_LAYOUTS = {"xyzw": 0, "yz": 1, "i16": 2}       # TPC_INPUT_*
+LAYOUT_BYTES = {"xyzw": 16, "yz": 8, "i16": 4}
+I16_Y_STEP, I16_Z_STEP = 1.0 / 256.0, 1.0 / 64.0     # TPC_I16_*_STEP
 
 
 class TpcError(RuntimeError):
@@ -63,7 +66,8 @@ class Output(C.Structure):
 
 class Slot(C.Structure):
     _fields_ = [("clusters", C.c_void_p), ("row_offsets", C.c_void_p), ("max_clusters", C.c_int64),
-                ("max_instances", C.c_int32), ("out", Output)]
+                ("max_instances", C.c_int32), ("out", Output), ("workspace", C.c_void_p),
+                ("workspace_bytes", C.c_size_t)]
 
 
 class HostOutput(C.Structure):
@@ -71,7 +75,8 @@ class HostOutput(C.Structure):
                 ("trk_sector", C.c_void_p), ("trk_hit_offset", C.c_void_p), ("trk_hits", C.c_void_p),
                 ("cluster_owner", C.c_void_p), ("trk_capacity", C.c_int64), ("trk_hits_capacity", C.c_int64),
                 ("totals", C.c_int64 * 16), ("n_chunks", C.c_int64), ("n_launches", C.c_int64),
-                ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64)]
+                ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64), ("h2d_ms", C.c_float), ("compute_ms", C.c_float),
+                ("d2h_ms", C.c_float), ("wall_ms", C.c_float)]
 
 
 _lib = None
@@ -107,6 +112,11 @@ def load_library():
     lib.tpc_track_sectors_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_int32,
                                            C.POINTER(Slot), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.POINTER(HostOutput)]
+    lib.tpc_pipeline_create.argtypes = [C.c_void_p, C.POINTER(Slot), C.c_int32, C.POINTER(C.c_void_p)]
+    lib.tpc_pipeline_destroy.argtypes = [C.c_void_p]
+    lib.tpc_pipeline_destroy.restype = None
+    lib.tpc_pipeline_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_int32,
+                                     C.POINTER(HostOutput)]
     _lib = lib
     return lib
 
@@ -193,6 +203,7 @@ class Tracker:
         self._h = h
         self._ws = None
         self._out_keep = None
+        self.input_layout = "xyzw"
 
     @classmethod
     def for_event(cls, ev, **kw):
@@ -237,9 +248,10 @@ class Tracker:
         """counts[6..9] (S5 transports / updates / examined clusters / searches) are only filled when enabled."""
         self._check(self.lib.tpc_set_work_counters(self._h, 1 if enable else 0), "tpc_set_work_counters")
 
-    def set_input_layout(self, yz=False):
-        """yz=True: `clusters` of the track calls is [N,2] = (y, z) instead of [N,4] = (x, y, z, w) (TPC_INPUT_YZ)."""
-        self._check(self.lib.tpc_set_input_layout(self._h, 1 if yz else 0), "tpc_set_input_layout")
+    def set_input_layout(self, layout="xyzw"):
+        """`clusters` of the track calls: "xyzw" float32 [N,4]; "yz" float32 [N,2]; "i16" int16 [N,2] fixed point."""
+        self.input_layout = layout
+        self._check(self.lib.tpc_set_input_layout(self._h, INPUT_LAYOUTS[layout]), "tpc_set_input_layout")
 
     def stage_times_ms(self, age=0):
         """Milliseconds per stage of the timed call `age` calls back (0 = last)."""
@@ -297,7 +309,11 @@ class Tracker:
     def track_sectors(self, clusters: np.ndarray, row_offsets: np.ndarray, n_inst: int, *, debug=False,
                       cand_capacity=None, trk_capacity=None) -> TrackResult:
         t = self._torch
-        cl = t.from_numpy(np.ascontiguousarray(clusters, np.float32).reshape(-1, 4)).to(self.device)
+        if self.input_layout == "i16":
+            cl = t.from_numpy(np.ascontiguousarray(clusters, np.int16).reshape(-1, 2)).to(self.device)
+        else:
+            cl = t.from_numpy(np.ascontiguousarray(clusters, np.float32)
+                              .reshape(-1, 4 if self.input_layout == "xyzw" else 2)).to(self.device)
         ro = t.from_numpy(np.ascontiguousarray(row_offsets, np.int32)).to(self.device)
         n = int(cl.shape[0])
         with t.cuda.device(self.device):
@@ -324,62 +340,89 @@ class Tracker:
 
 
 class HostPipeline:
-    """Buffers for tpc_track_sectors_host: `n_slots` device slots (torch), pinned host result arrays, three streams.
+    """Buffers and the persistent pipeline handle for tpc_pipeline_run: `n_slots` device slots (torch), each with its
+    own workspace, and pinned host result arrays for the outputs named in `want`.
 
     The chunk loop, the stream/event choreography and every copy are inside the C library; this class only owns
     memory and marshals pointers."""
 
+    RESULTS = ("trk_params", "trk_cov", "trk_nhits", "trk_sector", "trk_hit_offset", "trk_hits", "cluster_owner")
+
     def __init__(self, tracker: Tracker, max_chunk_clusters: int, inst_per_chunk: int, total_clusters: int, *,
-                 n_slots=2, trk_frac=0.05):
+                 n_slots=2, trk_frac=0.05, want=RESULTS, slot_workspaces=True):
         t = tracker._torch
         self.trk = tracker
         self.inst_per_chunk = int(inst_per_chunk)
         dev = tracker.device
         n = max(int(max_chunk_clusters), 1)
         tc = int(n * trk_frac) + 64
-        i32, f32, i64 = t.int32, t.float32, t.int64
+        i32, f32, i64, u8 = t.int32, t.float32, t.int64, t.uint8
         self._keep = []
         self.slots = (Slot * n_slots)()
+        ws_bytes = tracker.workspace_bytes(n, self.inst_per_chunk)
+        shapes = dict(trk_params=((tc, 5), f32), trk_cov=((tc, 15), f32), trk_nhits=((tc,), i32),
+                      trk_sector=((tc,), i32), trk_hit_offset=((tc + 1,), i64), trk_hits=((n,), i32),
+                      cluster_owner=((n,), i32))
         with t.cuda.device(dev):
             for s in range(n_slots):
-                b = dict(clusters=t.empty((n, 4), dtype=f32, device=dev),
+                b = dict(clusters=t.empty(n * LAYOUT_BYTES[tracker.input_layout], dtype=u8, device=dev),
                          row_offsets=t.empty(self.inst_per_chunk * tracker.n_rows + 1, dtype=i32, device=dev),
-                         counts=t.zeros(N_COUNTS, dtype=i64, device=dev),
-                         trk_params=t.empty((tc, 5), dtype=f32, device=dev), trk_cov=t.empty((tc, 15), dtype=f32, device=dev),
-                         trk_nhits=t.empty(tc, dtype=i32, device=dev), trk_sector=t.empty(tc, dtype=i32, device=dev),
-                         trk_hit_offset=t.empty(tc + 1, dtype=i64, device=dev), trk_hits=t.empty(n, dtype=i32, device=dev),
-                         cluster_owner=t.empty(n, dtype=i32, device=dev))
+                         counts=t.zeros(N_COUNTS, dtype=i64, device=dev))
+                for k in want:
+                    b[k] = t.empty(shapes[k][0], dtype=shapes[k][1], device=dev)
+                if slot_workspaces:
+                    b["workspace"] = t.empty(ws_bytes, dtype=u8, device=dev)
                 self._keep.append(b)
                 sl = self.slots[s]
                 sl.clusters, sl.row_offsets = b["clusters"].data_ptr(), b["row_offsets"].data_ptr()
                 sl.max_clusters, sl.max_instances = n, self.inst_per_chunk
-                for k in ("counts", "trk_params", "trk_cov", "trk_nhits", "trk_sector", "trk_hit_offset", "trk_hits",
-                          "cluster_owner"):
+                sl.out.counts = b["counts"].data_ptr()
+                for k in want:
                     setattr(sl.out, k, b[k].data_ptr())
                 sl.out.trk_capacity, sl.out.trk_hits_capacity = tc, n
-            tracker.reserve(n, self.inst_per_chunk)
-            self.streams = [t.cuda.Stream(device=dev) for _ in range(3)]
+                if slot_workspaces:
+                    sl.workspace, sl.workspace_bytes = b["workspace"].data_ptr(), ws_bytes
+            if not slot_workspaces:
+                tracker.reserve(n, self.inst_per_chunk)
         N = max(int(total_clusters), 1)
         T = int(N * trk_frac) + 64
-        pin = dict(pin_memory=True)
-        self.host = dict(trk_params=t.empty((T, 5), dtype=f32, **pin), trk_cov=t.empty((T, 15), dtype=f32, **pin),
-                         trk_nhits=t.empty(T, dtype=i32, **pin), trk_sector=t.empty(T, dtype=i32, **pin),
-                         trk_hit_offset=t.empty(T + 1, dtype=i64, **pin), trk_hits=t.empty(N, dtype=i32, **pin),
-                         cluster_owner=t.empty(N, dtype=i32, **pin))
+        hshapes = dict(trk_params=((T, 5), f32), trk_cov=((T, 15), f32), trk_nhits=((T,), i32), trk_sector=((T,), i32),
+                       trk_hit_offset=((T + 1,), i64), trk_hits=((N,), i32), cluster_owner=((N,), i32))
+        self.host = {k: t.empty(hshapes[k][0], dtype=hshapes[k][1], pin_memory=True) for k in want}
         self.hout = HostOutput()
         for k, v in self.host.items():
             setattr(self.hout, k, v.data_ptr())
         self.hout.trk_capacity, self.hout.trk_hits_capacity = T, N
         self.n_slots = n_slots
+        h = C.c_void_p()
+        with t.cuda.device(dev):
+            tracker._check(tracker.lib.tpc_pipeline_create(tracker._h, self.slots, n_slots, C.byref(h)),
+                           "tpc_pipeline_create")
+        self._p = h
+
+    def close(self):
+        if getattr(self, "_p", None):
+            self.trk.lib.tpc_pipeline_destroy(self._p)
+            self._p = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
     def run(self, h_clusters, h_row_offsets, n_inst):
-        """h_clusters: pinned float32 torch tensor [N,4]; h_row_offsets: pinned int32 [n_inst*R+1].  Blocks."""
+        """h_clusters: pinned torch tensor of the tracker's input layout ([N,4] f32 / [N,2] f32 / [N,2] i16);
+        h_row_offsets: pinned int32 [n_inst*R+1].  Blocks.  Returns a snapshot (plain Python numbers) of what the
+        call wrote into its tpc_host_output_t."""
         tr = self.trk
         n = int(h_clusters.shape[0])
-        rc = tr.lib.tpc_track_sectors_host(tr._h, C.c_void_p(h_clusters.data_ptr()), C.c_void_p(h_row_offsets.data_ptr()),
-                                           int(n_inst), n, self.inst_per_chunk, self.slots, self.n_slots,
-                                           C.c_void_p(self.streams[0].cuda_stream),
-                                           C.c_void_p(self.streams[1].cuda_stream),
-                                           C.c_void_p(self.streams[2].cuda_stream), C.byref(self.hout))
-        tr._check(rc, "tpc_track_sectors_host")
-        return self.hout
+        with tr._torch.cuda.device(tr.device):
+            rc = tr.lib.tpc_pipeline_run(self._p, C.c_void_p(h_clusters.data_ptr()),
+                                         C.c_void_p(h_row_offsets.data_ptr()), int(n_inst), n, self.inst_per_chunk,
+                                         C.byref(self.hout))
+        tr._check(rc, "tpc_pipeline_run")
+        ho = self.hout
+        return dict(totals=[int(x) for x in ho.totals], n_chunks=int(ho.n_chunks), n_launches=int(ho.n_launches),
+                    h2d_bytes=int(ho.h2d_bytes), d2h_bytes=int(ho.d2h_bytes), h2d_ms=float(ho.h2d_ms),
+                    compute_ms=float(ho.compute_ms), d2h_ms=float(ho.d2h_ms), wall_ms=float(ho.wall_ms))

@@ -40,6 +40,10 @@ def test_binding_structs_match_header_sizes():
     raw = 8 + 8 + 4 * 6 + C.sizeof(tracker.Params)  # n_rows(+pad), ptr, spe..sigma, params
     assert C.sizeof(tracker.Geometry) == (raw + 7) // 8 * 8  # tail padding to the pointer alignment
     assert C.sizeof(tracker.Output) % 8 == 0
+    # tpc_slot_t: 2 ptr + int64 + int32(+pad) + tpc_output_t + ptr + size_t
+    assert C.sizeof(tracker.Slot) == 8 * 4 + C.sizeof(tracker.Output) + 16
+    # tpc_host_output_t: 7 ptr + 2 int64 + 16 int64 + 4 int64 + 4 float
+    assert C.sizeof(tracker.HostOutput) == 8 * (7 + 2 + 16 + 4) + 16
 
 
 def test_no_cpu_fallback_without_device(lib):

@@ -138,42 +138,58 @@ def test_full_size_drift_windows_against_oracle():
     assert abs(g.n_tracks - len(o.trk_cand)) <= 2
 
 
-def test_compact_yz_input_equals_xyzw():
-    """TPC_INPUT_YZ (clusters as (y, z) pairs, half the upload) gives bit-identical results: device call and host
-    pipeline."""
+def test_compact_inputs_and_host_pipeline_against_oracle_full_window():
+    """One full CFG:4 window through every input layout and both entry points, each compared with the ORACLE:
+    (y, z) pairs (TPC_INPUT_YZ) must reproduce the float4 result bit for bit; 16-bit fixed point (TPC_INPUT_I16) is
+    compared with the oracle run on the decoded coordinates (the quantisation is applied before either side sees the
+    clusters, so links and candidates stay bit-exact); the chunked host pipeline returns the same job-wide arrays."""
     import torch
     from paper_1709_00618_b200 import Tracker
     from paper_1709_00618_b200.tracker import HostPipeline
-    evs = [dg.drift_window(seed=5301 + i, mean_tracks=150.0, cap_tracks=400) for i in range(3)]
-    batch = dg.concat_events(evs)
-    trk = Tracker.for_event(batch)
-    ref = trk.track_sectors(batch.clusters, batch.row_offsets, batch.n_inst)
-    yz = np.ascontiguousarray(batch.clusters[:, 1:3])
-    dev = trk.device
-    d_yz = torch.from_numpy(yz).to(dev)
-    d_ro = torch.from_numpy(batch.row_offsets).to(dev)
-    trk.set_input_layout(yz=True)
-    trk.reserve(batch.n_clusters, batch.n_inst)
-    trk.set_stream()
-    bufs, out = trk.alloc_outputs(batch.n_clusters)
-    trk.track_sectors_device(d_yz, d_ro, batch.n_inst, out)
-    torch.cuda.synchronize(dev)
-    assert bufs["counts"].cpu().numpy()[:5].tolist() == ref.counts[:5].tolist()
-    assert np.array_equal(bufs["cluster_owner"].cpu().numpy(), ref.cluster_owner)
-    assert np.array_equal(bufs["trk_params"][:ref.n_tracks].cpu().numpy(), ref.trk_params)
-    # host pipeline on the compact host buffer
-    h_yz = torch.from_numpy(yz).pin_memory()
-    h_ro = torch.from_numpy(batch.row_offsets).pin_memory()
-    R = batch.n_rows
-    mx = max(int(batch.row_offsets[min(i + 36, batch.n_inst) * R] - batch.row_offsets[i * R])
-             for i in range(0, batch.n_inst, 36))
-    pipe = HostPipeline(trk, mx, 36, batch.n_clusters, n_slots=2)
-    ho = pipe.run(h_yz, h_ro, batch.n_inst)
-    assert int(ho.totals[3]) == ref.n_tracks and ho.h2d_bytes < 8 * batch.n_clusters + 8 * len(batch.row_offsets)
-    assert np.array_equal(pipe.host["cluster_owner"].numpy()[:batch.n_clusters], ref.cluster_owner)
-    assert np.array_equal(pipe.host["trk_hits"].numpy()[:ref.n_track_hits], ref.trk_hits)
-    trk.set_input_layout(yz=False)
-    trk.close()
+    ev = dg.drift_window(seed=5003)
+    assert ev.n_clusters > 300_000
+    g_ref, o_ref = _check(ev, max_ok_mismatch=1)
+    q, ev_q = dg.quantise_i16(ev)
+    assert np.abs(ev_q.clusters[:, 1:3] - ev.clusters[:, 1:3]).max() <= 0.5 / 64 + 1e-4
+    o_q = run_oracle(ev_q)
+    R = ev.n_rows
+    for layout, data, o in (("yz", np.ascontiguousarray(ev.clusters[:, 1:3]), o_ref), ("i16", q, o_q)):
+        trk = Tracker.for_event(ev)
+        trk.set_input_layout(layout)
+        g = trk.track_sectors(data, ev.row_offsets, ev.n_inst, debug=True)
+        assert_ca_bit_exact(g, o)
+        tr = tracklet_report(g, o)
+        fr = final_track_report(g, o, ev.n_clusters)
+        assert_final_consistency(g, ev.n_clusters)
+        assert_final_track_records(g, o, ev.row_offsets, R, dg.row_x(R))
+        assert tr["ok_mismatch"] <= 1 and tr["shared_frac"] >= MIN_SHARED and tr["worst_param_excess"] <= 1.0, tr
+        assert tr["worst_cov_excess"] <= 1.0 and tr["worst_chi2_excess"] <= 1.0, tr
+        assert fr["shared_assign_frac"] >= MIN_SHARED, fr
+        if layout == "yz":  # same (y, z) as the float4 call: identical bits
+            for k in ("link_up_raw", "cand_hits", "tl_hits", "tl_params", "tl_cov", "trk_params", "cluster_owner"):
+                assert np.array_equal(getattr(g, k), getattr(g_ref, k)), k
+        # the chunked host pipeline on this layout: 7 chunks of 6 sector instances (the last one ragged), 3 slots
+        h_in = torch.from_numpy(data).pin_memory()
+        h_ro = torch.from_numpy(ev.row_offsets).pin_memory()
+        ipc = 5
+        mx = max(int(ev.row_offsets[min(i + ipc, ev.n_inst) * R] - ev.row_offsets[i * R])
+                 for i in range(0, ev.n_inst, ipc))
+        pipe = HostPipeline(trk, mx, ipc, ev.n_clusters, n_slots=3)
+        ho = pipe.run(h_in, h_ro, ev.n_inst)
+        nt, nh = ho["totals"][3], ho["totals"][4]
+        assert nt == g.n_tracks and nh == g.n_track_hits
+        assert ho["h2d_bytes"] == data.itemsize * 2 * ev.n_clusters + 4 * (ev.n_inst * R + ho["n_chunks"])
+        own = pipe.host["cluster_owner"].numpy()[:ev.n_clusters]
+        assert np.array_equal(own, g.cluster_owner)
+        assert np.array_equal(pipe.host["trk_hits"].numpy()[:nh], g.trk_hits)
+        assert np.array_equal(pipe.host["trk_params"].numpy()[:nt], g.trk_params)
+        # ... and directly against the oracle: final assignment by candidate id
+        own_o = np.where(o.cluster_owner >= 0, o.trk_cand[np.maximum(o.cluster_owner, 0)], -1)
+        own_g = np.where(own >= 0, g.trk_cand_id[np.maximum(own, 0)], -1)
+        assigned = (own_o >= 0) | (own_g >= 0)
+        assert ((own_o == own_g) & assigned).sum() >= MIN_SHARED * assigned.sum()
+        pipe.close()
+        trk.close()
 
 
 def test_full_size_central_event_against_oracle():

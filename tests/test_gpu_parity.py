@@ -118,28 +118,57 @@ def test_grid_cell_does_not_change_results():
 
 
 def test_host_pipeline_equals_device_call():
-    """tpc_track_sectors_host (chunked, three streams, pinned buffers) == one tpc_track_sectors call on the batch."""
+    """tpc_pipeline_run (chunked, per-slot workspaces and compute streams, pinned buffers) and the one-shot
+    tpc_track_sectors_host (three caller streams, shared workspace) == one tpc_track_sectors call on the batch."""
+    import ctypes as C
     import torch
     from paper_1709_00618_b200 import Tracker
-    from paper_1709_00618_b200.tracker import HostPipeline
+    from paper_1709_00618_b200.tracker import HostOutput, HostPipeline
     evs = [dg.drift_window(seed=5101 + i, mean_tracks=120.0, cap_tracks=300) for i in range(5)]
     batch = dg.concat_events(evs)
     trk = Tracker.for_event(batch)
     ref = trk.track_sectors(batch.clusters, batch.row_offsets, batch.n_inst)
     h_cl = torch.from_numpy(batch.clusters).pin_memory()
     h_ro = torch.from_numpy(batch.row_offsets).pin_memory()
-    for ipc, slots in ((36, 2), (72, 3), (36 * 5, 2), (7, 3)):
-        R = batch.n_rows
+    R = batch.n_rows
+
+    def same(pipe, ho, tag):
+        nt, nh = ho["totals"][3], ho["totals"][4]
+        assert nt == ref.n_tracks and nh == ref.n_track_hits and ho["totals"][1] == ref.n_cand, tag
+        assert np.array_equal(pipe.host["cluster_owner"].numpy()[:batch.n_clusters], ref.cluster_owner), tag
+        assert np.array_equal(pipe.host["trk_hits"].numpy()[:nh], ref.trk_hits), tag
+        assert np.array_equal(pipe.host["trk_hit_offset"].numpy()[:nt + 1], ref.trk_hit_offset), tag
+        assert np.array_equal(pipe.host["trk_params"].numpy()[:nt], ref.trk_params), tag
+        assert np.array_equal(pipe.host["trk_cov"].numpy()[:nt], ref.trk_cov), tag
+        assert np.array_equal(pipe.host["trk_nhits"].numpy()[:nt], ref.trk_nhits), tag
+        assert np.array_equal(pipe.host["trk_sector"].numpy()[:nt], ref.trk_sector), tag
+
+    for ipc, slots, own_ws in ((36, 2, True), (72, 3, True), (36 * 5, 2, True), (7, 3, True), (36, 2, False), (50, 4, False)):
         mx = max(int(batch.row_offsets[min(i + ipc, batch.n_inst) * R] - batch.row_offsets[i * R])
                  for i in range(0, batch.n_inst, ipc))
-        pipe = HostPipeline(trk, mx, ipc, batch.n_clusters, n_slots=slots)
-        ho = pipe.run(h_cl, h_ro, batch.n_inst)
-        nt, nh = int(ho.totals[3]), int(ho.totals[4])
-        assert nt == ref.n_tracks and nh == ref.n_track_hits and int(ho.totals[1]) == ref.n_cand
-        assert np.array_equal(pipe.host["cluster_owner"].numpy()[:batch.n_clusters], ref.cluster_owner), (ipc, slots)
-        assert np.array_equal(pipe.host["trk_hits"].numpy()[:nh], ref.trk_hits)
-        assert np.array_equal(pipe.host["trk_hit_offset"].numpy()[:nt + 1], ref.trk_hit_offset)
-        assert np.array_equal(pipe.host["trk_params"].numpy()[:nt], ref.trk_params)
-        assert np.array_equal(pipe.host["trk_sector"].numpy()[:nt], ref.trk_sector)
-        assert ho.n_chunks == -(-batch.n_inst // ipc) and ho.h2d_bytes >= 16 * batch.n_clusters
+        pipe = HostPipeline(trk, mx, ipc, batch.n_clusters, n_slots=slots, slot_workspaces=own_ws)
+        for rep in range(2):  # a pipeline is reusable
+            ho = pipe.run(h_cl, h_ro, batch.n_inst)
+            same(pipe, ho, (ipc, slots, own_ws, rep))
+        assert ho["n_chunks"] == -(-batch.n_inst // ipc)
+        assert ho["h2d_bytes"] == 16 * batch.n_clusters + 4 * (batch.n_inst * R + ho["n_chunks"])
+        assert ho["wall_ms"] > 0 and ho["h2d_ms"] > 0 and ho["compute_ms"] > 0 and ho["d2h_ms"] > 0
+        if not own_ws:  # the one-shot entry point on the same slots, caller's streams
+            for k in pipe.host.values():
+                k.zero_()
+            st = [torch.cuda.Stream() for _ in range(3)]
+            hout = pipe.hout
+            rc = trk.lib.tpc_track_sectors_host(trk._h, C.c_void_p(h_cl.data_ptr()), C.c_void_p(h_ro.data_ptr()),
+                                                batch.n_inst, batch.n_clusters, ipc, pipe.slots, slots,
+                                                C.c_void_p(st[0].cuda_stream), C.c_void_p(st[1].cuda_stream),
+                                                C.c_void_p(st[2].cuda_stream), C.byref(hout))
+            assert rc == 0
+            same(pipe, dict(totals=[int(x) for x in hout.totals]), ("one-shot", ipc))
+        pipe.close()
+    # only the requested results are produced and copied: owner alone
+    pipe = HostPipeline(trk, batch.n_clusters, batch.n_inst, batch.n_clusters, n_slots=2, want=("cluster_owner",))
+    ho = pipe.run(h_cl, h_ro, batch.n_inst)
+    assert np.array_equal(pipe.host["cluster_owner"].numpy()[:batch.n_clusters], ref.cluster_owner)
+    assert ho["d2h_bytes"] == 4 * batch.n_clusters + 8 * 16 * ho["n_chunks"]
+    pipe.close()
     trk.close()
