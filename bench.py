@@ -35,9 +35,11 @@ BYTES_PER_CLUSTER_S5 = 34.0
 # fp32 operations per unit of S5 work, counted from the formulas in csrc/kf_math.cuh
 FLOP_TRANSPORT, FLOP_UPDATE, FLOP_EXAMINE, FLOP_SEARCH = 150.0, 93.0, 7.0, 18.0
 FP32_LANES_PER_SM, N_SM = 128, 148
-# dram bytes per launch of follow_kernel per cluster, from the committed ncu --set full capture (profiles/); None
-# until a capture exists
-FOLLOW_DRAM_BYTES_PER_CLUSTER = 120.3  # profiles/r1h_full_kernels.md: (11.0 + 2.98) GB per launch / 116,186,372 clusters
+# ncu dram bytes per launch of the dominant kernel: read from the JSON committed next to the profile it was taken
+# from (it names the commit, the workload and the cluster count); reported only when this run's workload matches.
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+# results the e2e runs bring back: the fitted tracks and the cluster -> track assignment (once)
+E2E_WANT = ("cluster_owner", "trk_params", "trk_nhits", "trk_sector")
 
 
 WORKLOAD = "cfg5"  # set from --workload before the batch is generated (module global: the worker processes fork)
@@ -167,12 +169,69 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def measured_traffic(workload, windows, n_clusters):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, or None if no capture of this
+    workload is committed."""
+    try:
+        with open(TRAFFIC_JSON) as f:
+            d = json.load(f)
+    except Exception:
+        return None, "no committed ncu capture"
+    if d.get("workload") != workload or int(d.get("windows", -1)) != int(windows) or int(d.get("n_clusters", -1)) != int(n_clusters):
+        return None, f"committed capture is for {d.get('workload')} x {d.get('windows')} windows; not this workload"
+    return float(d["dram_bytes_per_launch"]), f"{d['source']} (commit {d.get('commit', '?')})"
+
+
+def run_e2e(torch, trk, dev, layout, host_in, h_ro, batch, args, combine):
+    """The whole job through tpc_pipeline_run from pinned HOST buffers: upload, tracking and download of the results
+    inside the timed region (host clock around the blocking calls)."""
+    from paper_1709_00618_b200.tracker import HostPipeline
+    S, N = batch.n_inst, batch.n_clusters
+    ipc = 36 * max(1, args.chunk_windows)
+    max_chunk = max(int(batch.row_offsets[min(i + ipc, S) * batch.n_rows] - batch.row_offsets[i * batch.n_rows])
+                    for i in range(0, S, ipc))
+    trk.set_input_layout(layout)
+    pipe = HostPipeline(trk, max_chunk, ipc, N, n_slots=args.slots, want=E2E_WANT)
+    for _ in range(max(1, min(args.warmup, 2))):
+        pipe.run(host_in, h_ro, S)
+    torch.cuda.synchronize(dev)
+    runs = []
+    tw = time.perf_counter()
+    for _ in range(args.steps):
+        runs.append(pipe.run(host_in, h_ro, S))  # a snapshot per run (plain numbers)
+    torch.cuda.synchronize(dev)
+    ms = (time.perf_counter() - tw) * 1e3
+    ms, n_total = combine(ms, N)
+    r = runs[-1]
+    k = len(runs)
+    out = {"value": n_total / (ms / k * 1e-3), "unit": UNIT, "h2d_bytes_per_step": r["h2d_bytes"],
+           "d2h_bytes_per_step": r["d2h_bytes"], "ms_per_step": ms / k,
+           "h2d_ms": float(np.mean([x["h2d_ms"] for x in runs])),
+           "compute_ms": float(np.mean([x["compute_ms"] for x in runs])),
+           "d2h_ms": float(np.mean([x["d2h_ms"] for x in runs])),
+           "h2d_gbs": r["h2d_bytes"] / max(np.mean([x["h2d_ms"] for x in runs]), 1e-9) / 1e6,
+           "d2h_gbs": r["d2h_bytes"] / max(np.mean([x["d2h_ms"] for x in runs]), 1e-9) / 1e6,
+           "chunks": r["n_chunks"], "slots": args.slots, "windows_per_chunk": args.chunk_windows,
+           "gpu_launches_per_step": r["n_launches"], "tracks": r["totals"][3],
+           "input": {"xyzw": "TPC_INPUT_XYZW: float4 (x, y, z, w), 16 B/cluster",
+                     "yz": "TPC_INPUT_YZ: fp32 (y, z) pairs, 8 B/cluster",
+                     "i16": "TPC_INPUT_I16: 16-bit fixed point (y/256 cm, z/64 cm), 4 B/cluster"}[layout],
+           "results": "cluster_owner (4 B/cluster) + trk_params, trk_nhits, trk_sector per track",
+           "busy": "h2d_ms / compute_ms / d2h_ms = time each stream was busy per step (CUDA events inside the "
+                   "library; compute counts concurrent chunks twice); the largest one bounds the step",
+           "timer": "host perf_counter around the blocking C-ABI calls"}
+    pipe.close()
+    trk.set_input_layout("xyzw")
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    skip = set(x for x in args.skip.split(",") if x)
     t_gen = time.time()
     evs, batch = make_batch(args.windows, args.seed0, rank)  # before CUDA init (fork)
     t_gen = time.time() - t_gen
@@ -183,7 +242,6 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     from paper_1709_00618_b200 import Tracker, physics
-    from paper_1709_00618_b200.tracker import HostPipeline
     N, S = batch.n_clusters, batch.n_inst
     tune = json.loads(args.tune) if args.tune else {}
     trk = Tracker.for_event(batch, device=f"cuda:{local}", **tune)
@@ -239,85 +297,68 @@ def run_ours(args):
     k = min(args.steps, 32)
     st = [trk.stage_times_ms(a) for a in range(k)]  # the untimed counting call above recorded no events
     stage_ms = {nme: float(np.mean([s[nme] for s in st])) for nme in st[0]}
+    own = bufs["cluster_owner"][:evs[0].n_clusters].cpu().numpy()  # window 0 of the default reading (physics report)
+
+    # ---- end to end through the host-buffer entry point (tpc_pipeline_run) -------------------------------------------
+    combine = lambda ms_, n_: sharding.combine_step(ms_, n_, device=dev)  # noqa: E731
+    e2e = e2e_xyzw = e2e_yz = None
+    if "e2e" not in skip:
+        # the streaming configuration the library recommends: 16-bit fixed-point clusters (4 B/cluster up)
+        q16, _ = datagen.quantise_i16(batch)
+        h_q = torch.from_numpy(q16).pin_memory()
+        e2e = run_e2e(torch, trk, dev, "i16", h_q, h_ro, batch, args, combine)
+        del h_q, q16
+        e2e_xyzw = run_e2e(torch, trk, dev, "xyzw", h_cl, h_ro, batch, args, combine)
+        h_yz = torch.from_numpy(np.ascontiguousarray(batch.clusters[:, 1:3])).pin_memory()
+        e2e_yz = run_e2e(torch, trk, dev, "yz", h_yz, h_ro, batch, args, combine)
+        del h_yz
 
     # ---- latency of ONE drift window (CFG:4) alone on the GPU: L2 flushed before every call ----------------------
-    n0, s0 = evs[0].n_clusters, evs[0].n_inst
-    fb1 = fbuf if fbuf is not None else torch.empty(512 << 20, dtype=torch.uint8, device=dev)
-    ev1 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
-    trk.track_sectors_device(d_cl[:n0], d_ro[:s0 * batch.n_rows + 1], s0, out)
-    for a, b in ev1:
-        fb1.fill_(1)
-        a.record()
+    single = None
+    if "single" not in skip:
+        n0, s0 = evs[0].n_clusters, evs[0].n_inst
+        fb1 = fbuf if fbuf is not None else torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+        ev1 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+        trk.set_stream()
         trk.track_sectors_device(d_cl[:n0], d_ro[:s0 * batch.n_rows + 1], s0, out)
-        b.record()
-    torch.cuda.synchronize(dev)
-    one_ms = float(np.median([a.elapsed_time(b) for a, b in ev1]))
-    del fb1
+        for a, b in ev1:
+            fb1.fill_(1)
+            a.record()
+            trk.track_sectors_device(d_cl[:n0], d_ro[:s0 * batch.n_rows + 1], s0, out)
+            b.record()
+        torch.cuda.synchronize(dev)
+        one_ms = float(np.median([a.elapsed_time(b) for a, b in ev1]))
+        del fb1
+        single = {"workload": "cfg4: one drift window alone (36 sector instances), L2 flushed", "ms": one_ms,
+                  "clusters": n0, "clusters_per_s": n0 / (one_ms * 1e-3)}
 
     # ---- the same batch with S2 row bridging on (reading A2'; not the headline reading) ------
-    trk_b = Tracker.for_event(batch, device=f"cuda:{local}", **{**tune, "nf_bridge_rows": 1})
-    trk_b.reserve(N, S)
-    trk_b.set_stream()
-    trk_b.set_stage_timing(True)
-    for _ in range(2):
-        trk_b.track_sectors_device(d_cl, d_ro, S, out)
-    evb = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)]
-    for a, b in evb:
-        a.record()
-        trk_b.track_sectors_device(d_cl, d_ro, S, out)
-        b.record()
-    torch.cuda.synchronize(dev)
-    bridge_ms = float(np.mean([a.elapsed_time(b) for a, b in evb]))
-    cb = bufs["counts"].cpu().numpy()
-    stb = [trk_b.stage_times_ms(a) for a in range(3)]
-    own_b = bufs["cluster_owner"][:evs[0].n_clusters].cpu().numpy()
-    bridge = {"reading": "nf_bridge_rows=1: a hit without an admissible adjacent pair may take one partner two rows "
-                         "away (DESIGN.md A2'); parity-tested against the oracle like the default reading",
-              "value": N / (bridge_ms * 1e-3), "unit": UNIT, "ms_per_step": bridge_ms,
-              "stage_ms": {nme: float(np.mean([x[nme] for x in stb])) for nme in stb[0]},
-              "results": {"candidates": int(cb[1]), "tracklets": int(cb[2]), "tracks": int(cb[3]),
-                          "track_hits": int(cb[4])},
-              "physics_window0": physics.report(evs[0], own_b, int(own_b.max()) + 1 if (own_b >= 0).any() else 0)}
-    trk_b.close()
-    # restore the default reading's outputs of window 0 for the physics report below
-    trk.track_sectors_device(d_cl[:n0], d_ro[:s0 * batch.n_rows + 1], s0, out)
-    torch.cuda.synchronize(dev)
-
-    # ---- end to end through the host-buffer entry point -------------------------------------------------------------
-    ipc = 36 * max(1, args.chunk_windows)
-    max_chunk = max(int(batch.row_offsets[min(i + ipc, S) * batch.n_rows] - batch.row_offsets[i * batch.n_rows])
-                    for i in range(0, S, ipc))
-    pipe = HostPipeline(trk, max_chunk, ipc, N, n_slots=args.slots)
-    trk.set_stage_timing(False)
-    for _ in range(max(1, min(args.warmup, 2))):
-        ho = pipe.run(h_cl, h_ro, S)
-    barrier()
-    tw = time.perf_counter()
-    for _ in range(args.steps):
-        ho = pipe.run(h_cl, h_ro, S)
-    torch.cuda.synchronize(dev)
-    e2e_ms = (time.perf_counter() - tw) * 1e3
-    e2e_ms, _ = sharding.combine_step(e2e_ms, N, device=dev)
-    e2e_value = n_total / (e2e_ms / args.steps * 1e-3)
-    e2e_tracks = int(ho.totals[3])
-    launches_e2e = int(ho.n_launches)
-
-    # the same pipeline fed with the compact (y, z) input (TPC_INPUT_YZ): half the upload
-    h_yz = torch.from_numpy(np.ascontiguousarray(batch.clusters[:, 1:3])).pin_memory()
-    trk.set_input_layout(yz=True)
-    hc = pipe.run(h_yz, h_ro, S)
-    barrier()
-    tw = time.perf_counter()
-    for _ in range(args.steps):
-        hc = pipe.run(h_yz, h_ro, S)
-    torch.cuda.synchronize(dev)
-    yz_ms = (time.perf_counter() - tw) * 1e3
-    yz_ms, _ = sharding.combine_step(yz_ms, N, device=dev)
-    e2e_yz = {"value": n_total / (yz_ms / args.steps * 1e-3), "unit": UNIT, "ms_per_step": yz_ms / args.steps,
-              "h2d_bytes_per_step": int(hc.h2d_bytes), "d2h_bytes_per_step": int(hc.d2h_bytes),
-              "tracks": int(hc.totals[3]), "input": "TPC_INPUT_YZ: clusters as (y, z) pairs; results identical"}
-    trk.set_input_layout(yz=False)
-    del h_yz
+    bridge = None
+    if "bridge" not in skip:
+        trk_b = Tracker.for_event(batch, device=f"cuda:{local}", **{**tune, "nf_bridge_rows": 1})
+        trk_b.reserve(N, S)
+        trk_b.set_stream()
+        trk_b.set_stage_timing(True)
+        for _ in range(2):
+            trk_b.track_sectors_device(d_cl, d_ro, S, out)
+        evb = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)]
+        for a, b in evb:
+            a.record()
+            trk_b.track_sectors_device(d_cl, d_ro, S, out)
+            b.record()
+        torch.cuda.synchronize(dev)
+        bridge_ms = float(np.mean([a.elapsed_time(b) for a, b in evb]))
+        cb = bufs["counts"].cpu().numpy()
+        stb = [trk_b.stage_times_ms(a) for a in range(3)]
+        own_b = bufs["cluster_owner"][:evs[0].n_clusters].cpu().numpy()
+        bridge = {"reading": "nf_bridge_rows=1: a hit without an admissible adjacent pair may take one partner two "
+                             "rows away (DESIGN.md A2'); parity-tested against the oracle like the default reading",
+                  "value": N / (bridge_ms * 1e-3), "unit": UNIT, "ms_per_step": bridge_ms,
+                  "stage_ms": {nme: float(np.mean([x[nme] for x in stb])) for nme in stb[0]},
+                  "results": {"candidates": int(cb[1]), "tracklets": int(cb[2]), "tracks": int(cb[3]),
+                              "track_hits": int(cb[4])},
+                  "physics_window0": physics.report(evs[0], own_b, int(own_b.max()) + 1 if (own_b >= 0).any() else 0)}
+        trk_b.close()
 
     if rank != 0:
         if world > 1:
@@ -330,12 +371,12 @@ def run_ours(args):
     flops = (tr_f * FLOP_TRANSPORT + up_f * FLOP_UPDATE + counts[8] * FLOP_EXAMINE + counts[9] * FLOP_SEARCH)
     t_follow = stage_ms["follow"] * 1e-3
     ach = flops / t_follow / 1e12
-    roof = {"kernel": "follow_kernel (S5 Kalman track following, row-by-row extrapolation)", "bound": "alu", "achieved": ach, "peak": fp32_peak,
-            "unit": "TFLOP/s", "frac": ach / fp32_peak,
-            "traffic": None if FOLLOW_DRAM_BYTES_PER_CLUSTER is None else FOLLOW_DRAM_BYTES_PER_CLUSTER * N,
-            "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of follow_kernel per launch on the "
-                              "default workload (profiles/r1h_full_kernels.md), scaled by the cluster count",
-            "peak_source": f"148 SM x 128 fp32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md)",
+    traffic, traffic_src = measured_traffic(WORKLOAD, args.windows, N)
+    roof = {"kernel": "follow_kernel (S5 Kalman track following, row-by-row extrapolation)", "bound": "alu",
+            "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s", "frac": ach / fp32_peak,
+            "traffic": traffic, "traffic_source": traffic_src,
+            "peak_source": f"NOMINAL, not measured: 148 SM x 128 fp32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md); "
+                           "MEASURED_PEAKS.json holds no fp32 ALU figure",
             "avg_launch_ms": stage_ms["follow"], "share_of_step": stage_ms["follow"] / sum(stage_ms.values()),
             "algorithmic_flop_per_launch": float(flops),
             "work": {"transports": tr_f, "updates": up_f, "clusters_examined": int(counts[8]),
@@ -348,8 +389,9 @@ def run_ours(args):
     roof_path = {"bound": "hbm", "achieved": path_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": path_gbs / hbm_peak,
                  "bytes_per_cluster_model": BYTES_PER_CLUSTER_PATH, "peak_source": peak_src,
                  "frac_of_nominal_8TBs": path_gbs / 8000.0}
-    cpu, _ = cpu_baseline(evs, 1) if world == 1 else (None, 0)
-    own = bufs["cluster_owner"][:evs[0].n_clusters].cpu().numpy()
+    cpu = None
+    if world == 1 and "cpu" not in skip:
+        cpu, _ = cpu_baseline(evs, 1)
     n_trk0 = int(own.max()) + 1 if (own >= 0).any() else 0
     phys = physics.report(evs[0], own, n_trk0)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -364,19 +406,13 @@ def run_ours(args):
                                "larger than twice the 126 MB L2, steps run back to back without a flush")),
                        "generation_s": round(t_gen, 1)},
             "clocks": clocks, "gpu_launches": launches,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(ho.h2d_bytes),
-                    "d2h_bytes_per_step": int(ho.d2h_bytes), "ms_per_step": e2e_ms / args.steps,
-                    "chunks": int(ho.n_chunks), "slots": args.slots, "gpu_launches_per_step": launches_e2e,
-                    "tracks": e2e_tracks, "timer": "host perf_counter around the blocking C-ABI calls"},
-            "e2e_compact_input": e2e_yz,
+            "e2e": e2e, "e2e_xyzw_f32": e2e_xyzw, "e2e_yz_f32": e2e_yz,
             "roofline": roof, "roofline_path_hbm": roof_path, "cpu_baseline": cpu,
-            "stage_ms": stage_ms,
-            "next1_bridge_rows": bridge,
-            "single_window": {"workload": "cfg4: one drift window alone (36 sector instances), L2 flushed", "ms": one_ms,
-                              "clusters": n0, "clusters_per_s": n0 / (one_ms * 1e-3)},
+            "stage_ms": stage_ms, "single_window": single,
             "results": {"candidates": int(counts[1]), "tracklets": int(counts[2]), "tracks": int(counts[3]),
                         "track_hits": int(counts[4]), "error_flags": int(counts[5])},
-            "physics_window0": phys}
+            "physics_window0": phys,
+            "next1_bridge_rows": bridge}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -389,13 +425,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--windows", type=int, default=100, help="CFG:4 drift windows per GPU and step")
-    ap.add_argument("--chunk-windows", type=int, default=5, help="windows per upload chunk in the e2e pipeline")
+    ap.add_argument("--chunk-windows", type=int, default=10, help="windows per upload chunk in the e2e pipeline")
     ap.add_argument("--slots", type=int, default=3)
     ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS),
                     help="what --windows counts: drift windows (default, the headline), or CFG:3 / CFG:2 events for the "
                          "linear-scaling check of PAPER.md:33")
     ap.add_argument("--seed0", type=int, default=5001)
     ap.add_argument("--tune", default="", help='JSON dict of performance-only tracker parameters, e.g. {"grid_cells_y": 8}')
+    ap.add_argument("--skip", default="", help="comma list of optional sections to leave out: e2e,single,bridge,cpu")
     args = ap.parse_args()
     global WORKLOAD
     WORKLOAD = args.workload
