@@ -159,6 +159,32 @@ static int window_list(const float *cl, int n, const orc_rowgrid *g, int use_gri
     return cnt;
 }
 
+/* Reading A5' (SURVEY 8(f) NEXT-2 "non-uniform pad-row pitch with the weighted second difference"): the
+ * pad rows need not be equally spaced (the real TPC has three pad lengths).  For row r with steps du = x[r+1] - x[r]
+ * and dd = x[r] - x[r-1], three points are collinear iff dd (u - h) - du (h - d) = 0; normalised so that equal steps
+ * give the plain second difference:   e = wu (u - h) - wd (h - d),  wu = 2 dd / (du + dd),  wd = 2 du / (du + dd).
+ * The search window is a slope bound (reading A3), so it scales with the step: the half-sizes towards row r+1 are
+ * (WY su, WZ su), su = du / p_ref, towards row r-1 (WY sd, WZ sd), sd = dd / p_ref, p_ref = mean pitch.
+ * A step within 1e-4 p_ref + 4e-5 cm of p_ref counts as p_ref (factor exactly 1; both steps such -> wu = wd = 1), so
+ * every geometry that passes the uniformity test of the default reading keeps that reading's arithmetic bit for bit.
+ * Computed in double from the fp32 row_x, rounded to fp32. */
+static void row_step_factors(const orc_config *c, int r, float *wu, float *wd, float *su, float *sd) {
+    const int R = c->n_rows;
+    const double pref = ((double)c->row_x[R - 1] - (double)c->row_x[0]) / (R - 1);
+    const double du = (double)c->row_x[r + 1] - (double)c->row_x[r], dd = (double)c->row_x[r] - (double)c->row_x[r - 1];
+    const double tol = 1e-4 * pref + 4e-5;
+    const int ureg = fabs(du - pref) <= tol, dreg = fabs(dd - pref) <= tol;
+    *su = ureg ? 1.0f : (float)(du / pref);
+    *sd = dreg ? 1.0f : (float)(dd / pref);
+    if (ureg && dreg) {
+        *wu = 1.0f;
+        *wd = 1.0f;
+    } else {
+        *wu = (float)(2.0 * dd / (du + dd));
+        *wd = (float)(2.0 * du / (du + dd));
+    }
+}
+
 /* SURVEY 8(c) S2 for one sector instance (ro = its row offsets [R+1], indices of `clusters`); link_up/link_dn are
  * written at those indices and hold such indices, -1 if none.  All fp32, every operation individually rounded
  * (this file is compiled with -ffp-contract=off).
@@ -167,7 +193,8 @@ static int window_list(const float *cl, int n, const orc_rowgrid *g, int use_gri
  * the window of half-widths (WY, WZ) around the hit; D = (t1 - t2)^2 + (t3 - t4)^2 with t1 = y_u - y, t2 = y - y_d,
  * t3 = z_u - z, t4 = z - z_d; admissible iff D <= D2MAX; minimum over (D, u, d).
  *
- * Class 1 (nf_bridge_rows = 1, reading A2': "bridge single missing rows"): only for
+ * Class 1 (nf_bridge_rows = 1, reading A2': "bridge single missing rows"; defined for
+ * equally spaced rows only -- the library rejects it with a non-uniform pitch): only for
  * a hit with NO admissible class-0 pair.  One of the two partners may lie two rows away (a row without a usable
  * cluster is skipped): (du, dd) = (1, 2): u in row r+1, d in row r-2, or (2, 1): u in row r+2, d in row r-1.  The
  * partner two rows away is searched in the doubled window (2 WY, 2 WZ; exact doubling).  The deviation from a
@@ -192,22 +219,30 @@ static void neighbours_instance(const orc_config *c, const float *clusters, cons
     for (int r = 0; r < R; r++) {
         const int n_r = ROWN(r);
         const float *cl_r = ROWCL(r);
+        float wu = 1.0f, wd = 1.0f, su = 1.0f, sd = 1.0f;
+        if (r >= 1 && r <= R - 2) row_step_factors(c, r, &wu, &wd, &su, &sd);
         for (int h = 0; h < n_r; h++) {
             int32_t lu = -1, ld = -1;
             if (r >= 1 && r <= R - 2) { /* rows 0 and R-1 never own links (reading A6) */
                 const float y = cl_r[4 * h + 1], z = cl_r[4 * h + 2];
-                const float ylo = y - WY, yhi = y + WY, zlo = z - WZ, zhi = z + WZ;
+                /* window towards row r+1 and towards row r-1 (reading A5': the half-sizes scale with the row step;
+                 * su = sd = 1 and wu = wd = 1 for equally spaced rows, where x * 1.0f is exact) */
+                const float WYu = WY * su, WZu = WZ * su, WYd = WY * sd, WZd = WZ * sd;
+                const float ylo = y - WYu, yhi = y + WYu, zlo = z - WZu, zhi = z + WZu;
+                const float ylo_d = y - WYd, yhi_d = y + WYd, zlo_d = z - WZd, zhi_d = z + WZd;
                 const float *cl_up = ROWCL(r + 1), *cl_dn = ROWCL(r - 1);
                 const int nu = window_list(cl_up, ROWN(r + 1), ROWG(r + 1), use_grid, ylo, yhi, zlo, zhi, ulist);
-                const int nd = window_list(cl_dn, ROWN(r - 1), ROWG(r - 1), use_grid, ylo, yhi, zlo, zhi, dlist);
+                const int nd = window_list(cl_dn, ROWN(r - 1), ROWG(r - 1), use_grid, ylo_d, yhi_d, zlo_d, zhi_d, dlist);
                 /* class 0: minimum over (D, u, d) lexicographically: independent of the visiting order */
                 int bu = -1, bd = -1, bdu = 1, bdd = 1;
                 float bD = 0.0f;
                 for (int a = 0; a < nu; a++)
                     for (int b = 0; b < nd; b++) {
                         int u = ulist[a], d = dlist[b];
-                        float t1 = cl_up[4 * u + 1] - y, t2 = y - cl_dn[4 * d + 1], ey = t1 - t2;
-                        float t3 = cl_up[4 * u + 2] - z, t4 = z - cl_dn[4 * d + 2], ez = t3 - t4;
+                        float t1 = cl_up[4 * u + 1] - y, t2 = y - cl_dn[4 * d + 1];
+                        float t3 = cl_up[4 * u + 2] - z, t4 = z - cl_dn[4 * d + 2];
+                        float a1 = wu * t1, a2 = wd * t2, ey = a1 - a2;
+                        float a3 = wu * t3, a4 = wd * t4, ez = a3 - a4;
                         float pyy = ey * ey, pzz = ez * ez;
                         float D = pyy + pzz;
                         if (!(D <= D2MAX)) continue;

@@ -115,7 +115,7 @@ class Oracle:
     @classmethod
     def for_event(cls, ev, **kw):
         from paper_1709_00618_b200 import datagen
-        return cls(datagen.row_x(ev.n_rows), ev.bz, z_lo=ev.z_lo, z_hi=ev.z_hi, sigma_y=ev.sigma_y,
+        return cls(ev.row_x, ev.bz, z_lo=ev.z_lo, z_hi=ev.z_hi, sigma_y=ev.sigma_y,
                    sigma_z=ev.sigma_z, **kw)
 
     # ---- stages -------------------------------------------------------------------------------------------

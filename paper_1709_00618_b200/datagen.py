@@ -38,6 +38,14 @@ def row_x(n_rows: int = N_ROWS) -> np.ndarray:
     return (X_FIRST + r * ((X_LAST - X_FIRST) / (n_rows - 1))).astype(np.float32)
 
 
+def row_x_three_pad_sizes() -> np.ndarray:
+    """159 pad rows with three pad lengths, as in the real TPC read-out chambers ("real TPC has 3
+    pad sizes"): 63 rows of 0.75 cm, 64 rows of 1.0 cm, 32 rows of 1.5 cm, first row at 85 cm.  Used by the
+    non-uniform-pitch reading A5'."""
+    steps = np.concatenate([np.full(63, 0.75), np.full(64, 1.0), np.full(31, 1.5)])
+    return (X_FIRST + np.concatenate([[0.0], np.cumsum(steps)])).astype(np.float32)
+
+
 @dataclass
 class Event:
     """One tracker input: `n_inst` sector instances, CSR over (instance, row)."""
@@ -54,6 +62,11 @@ class Event:
     sigma_z: float
     truth: dict = field(default_factory=dict)  # per-track generator parameters (arrays indexed by label)
     name: str = ""
+    rx: np.ndarray = None  # pad-row radii if they are not the uniform default (reading A5')
+
+    @property
+    def row_x(self) -> np.ndarray:
+        return row_x(self.n_rows) if self.rx is None else self.rx
 
     @property
     def n_clusters(self) -> int:
@@ -137,9 +150,9 @@ def _crossings(trk, bz, rx, sectors):
     return tuple(np.concatenate([o[i] for o in out]) for i in range(5))
 
 
-def gen_clusters(rng, n_prim, n_sec, *, bz, eff, sigma_y, sigma_z, noise, single_sector, n_rows=N_ROWS):
+def gen_clusters(rng, n_prim, n_sec, *, bz, eff, sigma_y, sigma_z, noise, single_sector, n_rows=N_ROWS, rx=None):
     """One collision: returns (inst, row, y, z, label) arrays + per-track truth. Noise label = -1."""
-    rx = row_x(n_rows)
+    rx = row_x(n_rows) if rx is None else rx
     trk = _tracks(rng, n_prim, n_sec, single_sector=single_sector)
     sectors = [0] if single_sector else range(SECTORS_PER_SIDE)
     sec, row, y, z, ti = _crossings(trk, bz, rx, sectors)
@@ -168,7 +181,7 @@ def gen_clusters(rng, n_prim, n_sec, *, bz, eff, sigma_y, sigma_z, noise, single
     return inst, row, y, z, ti, trk
 
 
-def _assemble(parts, truths, *, n_inst, n_rows, bz, z_lo, z_hi, sigma_y, sigma_z, name, inst_base=None):
+def _assemble(parts, truths, *, n_inst, n_rows, bz, z_lo, z_hi, sigma_y, sigma_z, name, inst_base=None, rx=None):
     """Merge per-collision cluster lists, sort per (instance,row) by (z,y) (A19), build the CSR table."""
     inst = np.concatenate([p[0] for p in parts])
     row = np.concatenate([p[1] for p in parts])
@@ -181,38 +194,39 @@ def _assemble(parts, truths, *, n_inst, n_rows, bz, z_lo, z_hi, sigma_y, sigma_z
     counts = np.bincount(key, minlength=n_inst * n_rows)
     offs = np.zeros(n_inst * n_rows + 1, np.int64)
     np.cumsum(counts, out=offs[1:])
-    rx = row_x(n_rows)
+    rx_ = row_x(n_rows) if rx is None else rx
     cl = np.empty((y.size, 4), np.float32)
-    cl[:, 0] = rx[key % n_rows]
+    cl[:, 0] = rx_[key % n_rows]
     cl[:, 1] = y
     cl[:, 2] = z
     cl[:, 3] = lab.astype(np.float32)
     truth = {k: np.concatenate([t[k] for t in truths]) for k in truths[0]} if truths else {}
     return Event(clusters=cl, row_offsets=offs.astype(np.int32), labels=lab.astype(np.int32), n_inst=n_inst,
-                 n_rows=n_rows, bz=bz, z_lo=z_lo, z_hi=z_hi, sigma_y=sigma_y, sigma_z=sigma_z, truth=truth, name=name)
+                 n_rows=n_rows, bz=bz, z_lo=z_lo, z_hi=z_hi, sigma_y=sigma_y, sigma_z=sigma_z, truth=truth, name=name,
+                 rx=rx)
 
 
 def single_sector(seed=1001, n_tracks=200, *, bz=0.5, sigma_y=0.1, sigma_z=0.1, noise=0.02, eff=1.0,
-                  n_rows=N_ROWS) -> Event:
+                  n_rows=N_ROWS, rx=None) -> Event:
     """CFG:1 — one sector, 200 helices from the origin, smear 0.1 cm, 2 % noise (A14)."""
     rng = _rng(seed)
     inst, row, y, z, ti, trk = gen_clusters(rng, n_tracks, 0, bz=bz, eff=eff, sigma_y=sigma_y, sigma_z=sigma_z,
-                                            noise=noise, single_sector=True, n_rows=n_rows)
+                                            noise=noise, single_sector=True, n_rows=n_rows, rx=rx)
     trk = dict(trk, z_shift=np.zeros(n_tracks))
     return _assemble([(inst, row, y, z, ti)], [trk], n_inst=1, n_rows=n_rows, bz=bz, z_lo=0.0, z_hi=Z_MAX,
-                     sigma_y=max(sigma_y, 1e-3), sigma_z=max(sigma_z, 1e-3), name="cfg1_single_sector")
+                     sigma_y=max(sigma_y, 1e-3), sigma_z=max(sigma_z, 1e-3), name="cfg1_single_sector", rx=rx)
 
 
 def full_event(seed=2001, n_prim=1000, *, sec_frac=0.0, bz=0.5, eff=0.95, sigma_y=0.1, sigma_z=0.1, noise=0.05,
-               name="cfg2_peripheral") -> Event:
+               name="cfg2_peripheral", rx=None) -> Event:
     """CFG:2 (defaults) / CFG:3 (`central_event`) — 36 sectors, one collision."""
     rng = _rng(seed)
     n_sec = int(round(n_prim * sec_frac))
     inst, row, y, z, ti, trk = gen_clusters(rng, n_prim, n_sec, bz=bz, eff=eff, sigma_y=sigma_y, sigma_z=sigma_z,
-                                            noise=noise, single_sector=False)
+                                            noise=noise, single_sector=False, rx=rx)
     trk = dict(trk, z_shift=np.zeros(n_prim + n_sec))
     return _assemble([(inst, row, y, z, ti)], [trk], n_inst=SECTORS_PER_EVENT, n_rows=N_ROWS, bz=bz, z_lo=0.0,
-                     z_hi=Z_MAX, sigma_y=sigma_y, sigma_z=sigma_z, name=name)
+                     z_hi=Z_MAX, sigma_y=sigma_y, sigma_z=sigma_z, name=name, rx=rx)
 
 
 def central_event(seed=3001, n_prim=8000) -> Event:
@@ -263,7 +277,7 @@ def concat_events(events, name="batch") -> Event:
     return Event(clusters=cl, row_offsets=np.concatenate(offs).astype(np.int32), labels=lab,
                  n_inst=sum(e.n_inst for e in events), n_rows=e0.n_rows, bz=e0.bz,
                  z_lo=min(e.z_lo for e in events), z_hi=max(e.z_hi for e in events), sigma_y=e0.sigma_y,
-                 sigma_z=e0.sigma_z, truth=truth, name=name)
+                 sigma_z=e0.sigma_z, truth=truth, name=name, rx=e0.rx)
 
 
 I16_Y_STEP = 1.0 / 256.0  # cm per count of the 16-bit fixed-point cluster format (include/tpc_tracker.h TPC_INPUT_I16)
@@ -295,13 +309,14 @@ def window_batch(n_windows, seed0=5001, **kw) -> Event:
 
 
 def from_tracks(trk: dict, *, bz, sigma_y=0.0, sigma_z=0.0, eff=1.0, noise=0.0, seed=7, single=True,
-                fp64_coords=False):
+                fp64_coords=False, rx=None):
     """Test helper: clusters of explicitly given tracks (dict with pt, eta, q, phi0, x0, y0, z0).
 
     Zero-smear / zero-noise / Bz=0 variants of CFG:1 used by the pins.  With
     `fp64_coords` the un-rounded fp64 (y, z) are returned next to the Event."""
     rng = _rng(seed)
-    rx = row_x()
+    rx_arg = rx
+    rx = row_x() if rx is None else rx
     trk = {k: np.asarray(v, dtype=np.float64) for k, v in trk.items()}
     sectors = [0] if single else range(SECTORS_PER_SIDE)
     sec, row, y, z, ti = _crossings(trk, bz, rx, sectors)
@@ -330,7 +345,7 @@ def from_tracks(trk: dict, *, bz, sigma_y=0.0, sigma_z=0.0, eff=1.0, noise=0.0, 
     ev = _assemble([(inst, row, y, z, ti)], [dict(trk, z_shift=np.zeros(len(trk["pt"])),
                                                   primary=np.ones(len(trk["pt"]), bool))],
                    n_inst=n_inst, n_rows=N_ROWS, bz=bz, z_lo=0.0, z_hi=Z_MAX, sigma_y=max(sigma_y, 1e-3),
-                   sigma_z=max(sigma_z, 1e-3), name="explicit_tracks")
+                   sigma_z=max(sigma_z, 1e-3), name="explicit_tracks", rx=rx_arg)
     if fp64_coords:
         return ev, y[order], z[order]
     return ev

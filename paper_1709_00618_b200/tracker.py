@@ -208,7 +208,7 @@ class Tracker:
     @classmethod
     def for_event(cls, ev, **kw):
         from . import datagen
-        return cls(datagen.row_x(ev.n_rows), ev.bz, z_lo=ev.z_lo, z_hi=ev.z_hi, sigma_y=ev.sigma_y,
+        return cls(ev.row_x, ev.bz, z_lo=ev.z_lo, z_hi=ev.z_hi, sigma_y=ev.sigma_y,
                    sigma_z=ev.sigma_z, **kw)
 
     def close(self):
