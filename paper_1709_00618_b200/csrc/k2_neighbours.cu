@@ -76,24 +76,42 @@ __device__ __forceinline__ CellSeq window_cells(const DevGeom& g, const RowView&
     return c;
 }
 
-// Exact search without the register lists (more than kNbList window hits in a neighbour row: dense spots only).
+// Search window of one hit towards one neighbour row: pre-rounded bounds and the z bins they touch.
+struct Win {
+    float ylo, yhi, zlo, zhi;
+    int zb0, zb1;
+};
+
+__device__ __forceinline__ Win make_win(const DevGeom& g, float y, float z, float wy, float wz, float z0) {
+    Win w;
+    w.ylo = __fsub_rn(y, wy);
+    w.yhi = __fadd_rn(y, wy);
+    w.zlo = __fsub_rn(z, wz);
+    w.zhi = __fadd_rn(z, wz);
+    w.zb0 = zbin(w.zlo, z0, g.inv_cz, g.nz);
+    w.zb1 = zbin(w.zhi, z0, g.inv_cz, g.nz);
+    return w;
+}
+
+// Exact search without the register lists (more than kNbList window hits in a neighbour row, or a grid finer than the
+// window).  wu / wd: weights of the two first differences (reading A5'; 1 on equally spaced rows).
 __device__ __noinline__ void search_dense(const DevGeom& g, const RowView& up, const RowView& dn, float y, float z,
-                                          float ylo, float yhi, float zlo, float zhi, int zb0, int zb1, Best& best) {
-    const int us0 = ybin(ylo, up.y0, up.inv_sy, g.ny), us1 = ybin(yhi, up.y0, up.inv_sy, g.ny);
-    const int ds0 = ybin(ylo, dn.y0, dn.inv_sy, g.ny), ds1 = ybin(yhi, dn.y0, dn.inv_sy, g.ny);
-    for (int zu = zb0; zu <= zb1; zu++) {
+                                          const Win& U, const Win& W, float wu, float wd, Best& best) {
+    const int us0 = ybin(U.ylo, up.y0, up.inv_sy, g.ny), us1 = ybin(U.yhi, up.y0, up.inv_sy, g.ny);
+    const int ds0 = ybin(W.ylo, dn.y0, dn.inv_sy, g.ny), ds1 = ybin(W.yhi, dn.y0, dn.inv_sy, g.ny);
+    for (int zu = U.zb0; zu <= U.zb1; zu++) {
         const int u0 = up.tbl[zu * g.ny + us0], u1 = up.tbl[zu * g.ny + us1 + 1];
         for (int a = u0; a < u1; a++) {
             const float2 u = up.yz[a];
-            if (!(ylo <= u.x && u.x <= yhi && zlo <= u.y && u.y <= zhi)) continue;
-            const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
-            for (int zd = zb0; zd <= zb1; zd++) {
+            if (!(U.ylo <= u.x && u.x <= U.yhi && U.zlo <= u.y && u.y <= U.zhi)) continue;
+            const float a1 = __fmul_rn(wu, __fsub_rn(u.x, y)), a3 = __fmul_rn(wu, __fsub_rn(u.y, z));
+            for (int zd = W.zb0; zd <= W.zb1; zd++) {
                 const int d0 = dn.tbl[zd * g.ny + ds0], d1 = dn.tbl[zd * g.ny + ds1 + 1];
                 for (int b = d0; b < d1; b++) {
                     const float2 d = dn.yz[b];
-                    if (!(ylo <= d.x && d.x <= yhi && zlo <= d.y && d.y <= zhi)) continue;
-                    const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
-                    const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
+                    if (!(W.ylo <= d.x && d.x <= W.yhi && W.zlo <= d.y && d.y <= W.zhi)) continue;
+                    const float ey = __fsub_rn(a1, __fmul_rn(wd, __fsub_rn(y, d.x)));
+                    const float ez = __fsub_rn(a3, __fmul_rn(wd, __fsub_rn(z, d.y)));
                     const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
                     consider(best, D <= g.nf_d2max, D, a, b, up.idx, dn.idx);
                 }
@@ -348,39 +366,53 @@ __device__ __forceinline__ BestBridge bridge_hit(const DevGeom& g, const RowView
     return bb;
 }
 
+// r = pad row of the hits (1..R-2).  Reading A5': the window towards row r+1 / r-1 has half-sizes (WY, WZ) * su / sd
+// and the deviation is wu (u - h) - wd (h - d); all four factors are exactly 1 on equally spaced rows, where this is
+// the plain second difference of the default reading (x * 1.0f is exact).
+// kUniform: all rows equally spaced -- the factors are all 1, so the multiplications and the second window are
+// skipped (same bits: x * 1.0f is exact); the launcher picks the variant from the geometry.
+template <bool kUniform>
+__device__ __forceinline__ float wmul(float w, float x) { return kUniform ? x : __fmul_rn(w, x); }
+
+template <bool kUniform>
 __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, const RowView dn, const float2* my_yz,
-                                           int n, float z0, int base, int base_up, int base_dn,
+                                           int n, int r, float z0, int base, int base_up, int base_dn,
                                            int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
-    const float WY = g.nf_wy, WZ = g.nf_wz, D2MAX = g.nf_d2max;
+    const float D2MAX = g.nf_d2max;
+    const float wu = kUniform ? 1.0f : g.row_wu[r], wd = kUniform ? 1.0f : g.row_wd[r];
+    const float WYu = kUniform ? g.nf_wy : __fmul_rn(g.nf_wy, g.row_su[r]);
+    const float WZu = kUniform ? g.nf_wz : __fmul_rn(g.nf_wz, g.row_su[r]);
+    const float WYd = kUniform ? g.nf_wy : __fmul_rn(g.nf_wy, g.row_sd[r]);
+    const float WZd = kUniform ? g.nf_wz : __fmul_rn(g.nf_wz, g.row_sd[r]);
     const float kInf = __int_as_float(0x7f800000);
     for (int i = threadIdx.x; i < n; i += kNbThreads) {
         const float2 h = my_yz[i];
         const float y = h.x, z = h.y;
-        const float ylo = __fsub_rn(y, WY), yhi = __fadd_rn(y, WY);
-        const float zlo = __fsub_rn(z, WZ), zhi = __fadd_rn(z, WZ);
-        const int zb0 = zbin(zlo, z0, g.inv_cz, g.nz), zb1 = zbin(zhi, z0, g.inv_cz, g.nz);
+        const Win U = make_win(g, y, z, WYu, WZu, z0);
+        const Win W = kUniform ? U : make_win(g, y, z, WYd, WZd, z0);
         Best best{kInf, -1, -1};
-        // row r-1 window hits (the newest kNbList = 4) as (y - y_d, z - z_d) plus their positions
+        // row r-1 window hits (the newest kNbList = 4) as wd * (y - y_d), wd * (z - z_d) plus their positions
         float t2a = 0.0f, t2b = 0.0f, t2c = 0.0f, t2d = 0.0f, t4a = 0.0f, t4b = 0.0f, t4c = 0.0f, t4d = 0.0f;
         unsigned long long ld = 0ull;
         int nd = 0;
-        const bool coarse = zb1 - zb0 <= 1;
+        const bool coarse = U.zb1 - U.zb0 <= 1 && W.zb1 - W.zb0 <= 1;
         if (!coarse) {  // a grid finer than the window (non-default grid_cell_z): generic exact search
-            search_dense(g, up, dn, y, z, ylo, yhi, zlo, zhi, zb0, zb1, best);
+            search_dense(g, up, dn, y, z, U, W, wu, wd, best);
         } else {
             // Flat loops over the handful of hits in the touched cells.  Row r-1 first: its window hits (the newest
-            // kNbList = 4) stay in registers as (y - y_d, z - z_d) plus their positions; then every window hit of
-            // row r+1 is paired with them.  All straight-line code with predicates: the lanes of a warp see
-            // different hit counts, and branches taken by a few lanes cost the whole warp.
-            const CellSeq cd = window_cells(g, dn, ylo, yhi, zb0, zb1);
-            const CellSeq cu = window_cells(g, up, ylo, yhi, zb0, zb1);
+            // kNbList = 4) stay in registers plus their positions; then every window hit of row r+1 is paired with
+            // them.  All straight-line code with predicates: the lanes of a warp see different hit counts, and
+            // branches taken by a few lanes cost the whole warp.
+            const CellSeq cd = window_cells(g, dn, W.ylo, W.yhi, W.zb0, W.zb1);
+            const CellSeq cu = window_cells(g, up, U.ylo, U.yhi, U.zb0, U.zb1);
             const int dshift = cd.b0 - cd.na, ushift = cu.b0 - cu.na;
             for (int k = 0; k < cd.nt; k++) {
                 const int j = k < cd.na ? cd.a0 + k : k + dshift;
                 const float2 d = dn.yz[j];
-                const bool in = in_window(d, ylo, yhi, zlo, zhi);
-                t2d = in ? t2c : t2d; t2c = in ? t2b : t2c; t2b = in ? t2a : t2b; t2a = in ? __fsub_rn(y, d.x) : t2a;
-                t4d = in ? t4c : t4d; t4c = in ? t4b : t4c; t4b = in ? t4a : t4b; t4a = in ? __fsub_rn(z, d.y) : t4a;
+                const bool in = in_window(d, W.ylo, W.yhi, W.zlo, W.zhi);
+                const float a2 = wmul<kUniform>(wd, __fsub_rn(y, d.x)), a4 = wmul<kUniform>(wd, __fsub_rn(z, d.y));
+                t2d = in ? t2c : t2d; t2c = in ? t2b : t2c; t2b = in ? t2a : t2b; t2a = in ? a2 : t2a;
+                t4d = in ? t4c : t4d; t4c = in ? t4b : t4c; t4b = in ? t4a : t4b; t4a = in ? a4 : t4a;
                 ld = in ? ((ld << 16) | (unsigned long long)j) : ld;
                 nd += in ? 1 : 0;
             }
@@ -388,8 +420,8 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
                 for (int k = 0; k < (nd > 0 ? cu.nt : 0); k++) {
                     const int ja = k < cu.na ? cu.a0 + k : k + ushift;
                     const float2 u = up.yz[ja];
-                    const bool uin = in_window(u, ylo, yhi, zlo, zhi);
-                    const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
+                    const bool uin = in_window(u, U.ylo, U.yhi, U.zlo, U.zhi);
+                    const float t1 = wmul<kUniform>(wu, __fsub_rn(u.x, y)), t3 = wmul<kUniform>(wu, __fsub_rn(u.y, z));
 #define TPC_NB_PAIR(T2, T4, Q)                                                                                   \
     {                                                                                                            \
         const float ey = __fsub_rn(t1, T2), ez = __fsub_rn(t3, T4);                                              \
@@ -410,15 +442,15 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
                 for (int k = 0; k < cu.nt; k++) {
                     const int ja = k < cu.na ? cu.a0 + k : k + ushift;
                     const float2 u = up.yz[ja];
-                    if (!in_window(u, ylo, yhi, zlo, zhi)) continue;
-                    const float t1 = __fsub_rn(u.x, y), t3 = __fsub_rn(u.y, z);
+                    if (!in_window(u, U.ylo, U.yhi, U.zlo, U.zhi)) continue;
+                    const float t1 = wmul<kUniform>(wu, __fsub_rn(u.x, y)), t3 = wmul<kUniform>(wu, __fsub_rn(u.y, z));
                     for (int q = 0; q < cd.nt; q++) {
                         const int jb = q < cd.na ? cd.a0 + q : q + dshift;
                         const float2 d = dn.yz[jb];
-                        const float t2 = __fsub_rn(y, d.x), ey = __fsub_rn(t1, t2);
-                        const float t4 = __fsub_rn(z, d.y), ez = __fsub_rn(t3, t4);
+                        const float ey = __fsub_rn(t1, wmul<kUniform>(wd, __fsub_rn(y, d.x)));
+                        const float ez = __fsub_rn(t3, wmul<kUniform>(wd, __fsub_rn(z, d.y)));
                         const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
-                        consider(best, in_window(d, ylo, yhi, zlo, zhi) && D <= D2MAX, D, ja, jb, up.idx, dn.idx);
+                        consider(best, in_window(d, W.ylo, W.yhi, W.zlo, W.zhi) && D <= D2MAX, D, ja, jb, up.idx, dn.idx);
                     }
                 }
             }
@@ -432,6 +464,7 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
     }
 }
 
+template <bool kUniform>
 __global__ void __launch_bounds__(kNbThreads)
 neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
                   const float2* __restrict__ hit_yz, const uint16_t* __restrict__ hit_idx,
@@ -480,7 +513,7 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
         dn.yz = s_yz + n_up;
     }
     __syncthreads();
-    search_row(g, up, dn, hit_yz + base, n, z0, base, base_up, base_dn, link_up, link_dn);
+    search_row<kUniform>(g, up, dn, hit_yz + base, n, r, z0, base, base_up, base_dn, link_up, link_dn);
 }
 
 // Class 1 (reading A2', nf_bridge_rows = 1) as its own pass: one WARP per (instance,row) slab reads the row's raw
@@ -555,8 +588,12 @@ static size_t nb_smem_bytes(const DevGeom& g) {
 int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s) {
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
-    neighbours_kernel<<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
-                                                                  w.up_raw, w.dn_raw);
+    if (g.uniform_pitch)
+        neighbours_kernel<true><<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
+                                                                            w.bin_start, w.up_raw, w.dn_raw);
+    else
+        neighbours_kernel<false><<<slabs, kNbThreads, nb_smem_bytes(g), s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
+                                                                             w.bin_start, w.up_raw, w.dn_raw);
     if (g.bridge) {  // class 1 (reading A2'): a second, light pass over the hits that found no adjacent pair
         bridge_links_kernel<<<div_up(slabs, kBrThreads / 32), kBrThreads, 0, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
                                                                                   w.bin_start, w.up_raw, w.dn_raw, slabs);

@@ -40,6 +40,13 @@ struct DevGeom {
     const float* row_x;  // device [R]
     const float* row_y0;      // device [R] lower edge of the row's y grid: -(row half-width + 0.5 cm)
     const float* row_inv_sy;  // device [R] strips per cm of that row
+    // S2 with a non-uniform row pitch (reading A5'): weights of the two first differences and scale of the search
+    // window towards row r+1 / r-1; all exactly 1 on equally spaced rows
+    int uniform_pitch;        // 1: every step factor below is exactly 1 (the S2 kernel skips them)
+    const float* row_wu;      // device [R]
+    const float* row_wd;
+    const float* row_su;
+    const float* row_sd;
 };
 
 // Views into the caller's workspace (all device pointers), fixed per call.

@@ -23,14 +23,23 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     *out = nullptr;
     const int R = geom->n_rows;
     if (R < 3 || R > kMaxRows) { g_create_err = "n_rows out of [3,255]"; return TPC_ERR_GEOMETRY; }
+    // Rows must be strictly increasing.  Equal spacing is no longer required (reading A5'): S2 weights its
+    // two first differences by the row steps and scales its window with them; a step within 1e-4 p + 4e-5 cm of the
+    // mean pitch p counts as p, so that equally spaced rows keep the arithmetic of the default reading bit for bit.
     const double pitch = ((double)geom->row_x[R - 1] - (double)geom->row_x[0]) / (R - 1);
     if (!(pitch > 0.0)) { g_create_err = "rows not increasing"; return TPC_ERR_GEOMETRY; }
+    bool uniform = true;
     for (int r = 1; r < R; r++) {
         const double d = (double)geom->row_x[r] - (double)geom->row_x[r - 1];
-        if (!(d > 0.0) || std::fabs(d - pitch) > 1e-4 * pitch + 4e-5) {
-            g_create_err = "pad rows must be strictly increasing with uniform pitch (DESIGN.md reading A5)";
+        if (!(d > 0.0)) {
+            g_create_err = "pad rows must be strictly increasing";
             return TPC_ERR_GEOMETRY;
         }
+        if (std::fabs(d - pitch) > 1e-4 * pitch + 4e-5) uniform = false;
+    }
+    if (!uniform && geom->params.nf_bridge_rows != 0) {
+        g_create_err = "nf_bridge_rows (reading A2') is defined for equally spaced pad rows only";
+        return TPC_ERR_GEOMETRY;
     }
     if (geom->sectors_per_event < 2 || (geom->sectors_per_event & 1) || !(geom->z_hi > geom->z_lo) ||
         !(geom->sigma_y > 0.0f) || !(geom->sigma_z > 0.0f) || !(geom->half_angle_rad > 0.0f)) {
@@ -93,15 +102,29 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
         g_create_err = "cand_min_hits/cand_max_hits out of range (2 <= min <= max <= 10, max >= 3)";
         return TPC_ERR_ARG;
     }
-    std::vector<float> rows(3 * (size_t)R);
+    constexpr int kRowTables = 7;  // row_x, row_y0, row_inv_sy, row_wu, row_wd, row_su, row_sd
+    std::vector<float> rows(kRowTables * (size_t)R, 1.0f);
     for (int r = 0; r < R; r++) {
         const float hw = geom->row_x[r] * g.tan_half + 0.5f;  // half-width of the row's y grid
         rows[r] = geom->row_x[r];
         rows[R + r] = -hw;
         rows[2 * R + r] = (float)ny / (2.0f * hw);
+        if (r >= 1 && r <= R - 2) {  // step factors of reading A5' (rows 0 and R-1 own no links)
+            const double up = (double)geom->row_x[r + 1] - (double)geom->row_x[r];
+            const double dn = (double)geom->row_x[r] - (double)geom->row_x[r - 1];
+            const double tol = 1e-4 * pitch + 4e-5;
+            const bool up_reg = std::fabs(up - pitch) <= tol, dn_reg = std::fabs(dn - pitch) <= tol;
+            if (!(up_reg && dn_reg)) {
+                rows[3 * R + r] = (float)(2.0 * dn / (up + dn));
+                rows[4 * R + r] = (float)(2.0 * up / (up + dn));
+            }
+            if (!up_reg) rows[5 * R + r] = (float)(up / pitch);
+            if (!dn_reg) rows[6 * R + r] = (float)(dn / pitch);
+        }
     }
-    cudaError_t e = cudaMalloc(&t->d_row_x, sizeof(float) * 3 * R);
-    if (e == cudaSuccess) e = cudaMemcpy(t->d_row_x, rows.data(), sizeof(float) * 3 * R, cudaMemcpyHostToDevice);
+    cudaError_t e = cudaMalloc(&t->d_row_x, sizeof(float) * kRowTables * R);
+    if (e == cudaSuccess)
+        e = cudaMemcpy(t->d_row_x, rows.data(), sizeof(float) * kRowTables * R, cudaMemcpyHostToDevice);
     int dev = 0;
     if (e == cudaSuccess) e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&t->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -114,6 +137,11 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     g.row_x = t->d_row_x;
     g.row_y0 = t->d_row_x + R;
     g.row_inv_sy = t->d_row_x + 2 * R;
+    g.uniform_pitch = uniform ? 1 : 0;
+    g.row_wu = t->d_row_x + 3 * R;
+    g.row_wd = t->d_row_x + 4 * R;
+    g.row_su = t->d_row_x + 5 * R;
+    g.row_sd = t->d_row_x + 6 * R;
     *out = t;
     return TPC_OK;
 }

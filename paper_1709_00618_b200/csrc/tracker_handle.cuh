@@ -7,7 +7,7 @@
 
 struct tpc_tracker {
     tpc::DevGeom g;
-    float* d_row_x = nullptr;  // [3][R]: row_x, row_y0, row_inv_sy
+    float* d_row_x = nullptr;  // [7][R]: row_x, row_y0, row_inv_sy, row_wu, row_wd, row_su, row_sd
     void* ws = nullptr;
     size_t ws_bytes = 0;
     cudaStream_t stream = nullptr;

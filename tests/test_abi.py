@@ -58,10 +58,13 @@ def test_no_cpu_fallback_without_device(lib):
 def test_geometry_validation_is_host_side(lib):
     from paper_1709_00618_b200 import tracker
     rx = np.linspace(85.0, 247.0, 159).astype(np.float32)
-    bad = rx.copy()
-    bad[50] += 0.3  # non-uniform pitch -> reading A5
-    for arr, n, want in ((bad, 159, -2), (rx, 2, -2), (rx[::-1].copy(), 159, -2)):
-        geom, keep = tracker.make_geometry(arr[:n] if n < len(arr) else arr)
+    flat = rx.copy()
+    flat[50] = flat[49]  # not strictly increasing
+    uneven = rx.copy()
+    uneven[50] += 0.3  # non-uniform pitch: accepted (reading A5') unless row bridging (reading A2') is asked for
+    for arr, n, want, kw in ((flat, 159, -2, {}), (rx, 2, -2, {}), (rx[::-1].copy(), 159, -2, {}),
+                             (uneven, 159, -2, dict(nf_bridge_rows=1))):
+        geom, keep = tracker.make_geometry(arr[:n] if n < len(arr) else arr, **kw)
         geom.n_rows = n
         h = C.c_void_p()
         rc = lib.tpc_tracker_create(C.byref(geom), C.c_float(0.5), C.byref(h))
