@@ -499,6 +499,12 @@ static int pickup(const float *cl, int n, const orc_rowgrid *g, double y_pred, d
     return best;
 }
 
+static void unpack_cov_c(const double c[15], double P[25]) {
+    int k = 0;
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j <= i; j++) { P[i * 5 + j] = c[k]; P[j * 5 + i] = c[k]; k++; }
+}
+
 static void pack_cov(const double P[25], double c[15]) {
     int k = 0;
     for (int i = 0; i < 5; i++)
@@ -758,3 +764,253 @@ int orc_track_count(const orc_config *c, const float *clusters, const int32_t *r
 
 int32_t orc_sizeof_tracklet(void) { return (int32_t)sizeof(orc_tracklet); }
 int32_t orc_sizeof_config(void) { return (int32_t)sizeof(orc_config); }
+
+/* ================================================================== PHASE 2: sector merger + refit
+ *
+ * PAPER.md:27 "The second phase merges the track segments found in the individual sectors to final tracks and
+ * performs a track refit" (PAPER.md:33 names a GPU prototype of this fit).  The paper gives
+ * no rule for either step; the reading is fixed in DESIGN.md ("Phase 2", readings M1-M4):
+ *  M1 refit of one segment = the S5 filter over the hits the track KEPT in S6 only, each used once: seed from the
+ *     kept hits (first, middle, last in row order) at the innermost hit, transport that state in one step to the
+ *     outermost hit's row, reset the covariance to the prior P0, then filter inward hit by hit (transport, update).
+ *     The state after the innermost hit is reported.  Any failed transport (|sinPhi| > max) -> no refit (ok = 0).
+ *  M2 frame change between neighbouring sectors = exact rotation of the helix state about the beam axis by
+ *     alpha = (sector difference) * 2 * half_angle; the rotated state sits at x' = x cos(alpha) + y sin(alpha) of the
+ *     new frame (no longer a pad-row plane) and is transported to a row from there.
+ *  M3 matching: segment B continues segment A outward iff same event/window (instance / sectors_per_event), same z
+ *     side, neighbouring sectors (cyclic), first_row(B) > last_row(A), first_row(B) - last_row(A) <= 10; B's
+ *     refitted state at its innermost hit, rotated into A's frame and transported to A's outermost row, must pass
+ *     |dy| <= 2 cm and |dz| <= 2 cm against A's outermost HIT; among those B the one with the smallest dy^2 + dz^2
+ *     (tie: lowest track index) is A's successor candidate, likewise every B picks its best A; a link exists iff the
+ *     choice is mutual.
+ *  M4 merged track = maximal chain of links, ordered inside out.  Its fit: M1 on the outermost segment, then at that
+ *     segment's innermost hit the state is rotated (M2) into the next segment's frame, transported to that segment's
+ *     outermost hit row, and the filter continues inward; reported at the innermost hit of the innermost segment, in
+ *     its frame.  chi2 and the hit count run over the whole chain.  Merged tracks are listed in ascending index of
+ *     their innermost segment.
+ */
+
+/* M2.  p at plane x of the old frame -> p1 at plane *x1 of the frame rotated by +alpha about the beam axis (the new
+ * frame's x axis points alpha further in azimuth).  P (5x5, row-major) -> P1 = J P J^T with the exact Jacobian of the
+ * map "state on the plane x = const of the old frame -> state on the plane x' = const of the new frame":
+ * a variation of y moves the point along the old plane; it is brought back to the new plane by sliding along the
+ * track, which scales y by cos(phi)/cos(phi'), shifts z by the dz/ds of that slide and turns the direction by the
+ * curvature over it.  J (row-major) may be NULL.  Returns 0 on success, 1 (outputs untouched) if |sinPhi| exceeds
+ * max_sinphi before or after the rotation or the rotated direction points backwards (cos <= 0). */
+int orc_rotate(const double p[5], const double P[25], double x, double alpha, double cB, double max_sinphi,
+               double p1[5], double P1[25], double *x1, double J_out[25]) {
+    const double ca = cos(alpha), sa = sin(alpha);
+    const double s = p[2];
+    if (fabs(s) > max_sinphi) return 1;
+    const double c = sqrt(1.0 - s * s);
+    /* new frame: x' = x cos(a) + y sin(a), y' = -x sin(a) + y cos(a); direction angle phi' = phi - alpha */
+    const double s1 = s * ca - c * sa, c1 = c * ca + s * sa;
+    if (fabs(s1) > max_sinphi || c1 <= 0.0) return 1;
+    *x1 = x * ca + p[0] * sa;
+    p1[0] = -x * sa + p[0] * ca;
+    p1[1] = p[1];
+    p1[2] = s1;
+    p1[3] = p[3];
+    p1[4] = p[4];
+    /* Jacobian at fixed new plane x' = *x1.  A shift dy of the point along the old plane changes x' by dy sin(a);
+     * sliding back along the track by path length ds = -dy sin(a) / c1 (so that x' is restored) gives
+     *   dy' = dy cos(a) + ds s1 = dy (cos(a) c1 - sin(a) s1) / c1 = dy c / c1,
+     *   dz' = ds t = -dy sin(a) t / c1,   d(sinPhi') = c1 kappa ds = -dy sin(a) kappa   (kappa = cB k). */
+    double J[25];
+    for (int i = 0; i < 25; i++) J[i] = (i % 6 == 0) ? 1.0 : 0.0;
+    J[0 * 5 + 0] = c / c1;
+    J[1 * 5 + 0] = -sa * p[3] / c1;
+    J[2 * 5 + 0] = -sa * cB * p[4];
+    J[2 * 5 + 2] = c1 / c; /* d sin(phi - a) / d sin(phi) = cos(phi - a) / cos(phi) */
+    double JP[25], Pn[25];
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j < 5; j++) {
+            double acc = 0.0;
+            for (int m = 0; m < 5; m++) acc += J[i * 5 + m] * P[m * 5 + j];
+            JP[i * 5 + j] = acc;
+        }
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j < 5; j++) {
+            double acc = 0.0;
+            for (int m = 0; m < 5; m++) acc += JP[i * 5 + m] * J[j * 5 + m];
+            Pn[i * 5 + j] = acc;
+        }
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j < 5; j++) P1[i * 5 + j] = 0.5 * (Pn[i * 5 + j] + Pn[j * 5 + i]);
+    if (J_out) memcpy(J_out, J, sizeof(J));
+    return 0;
+}
+
+/* One segment of a merged track for orc_refit_chain: its sector-local frame (azimuth index) and its kept hits. */
+typedef struct {
+    int32_t sector;   /* geometric sector 0 .. sectors_per_event-1 (frame of the hits) */
+    int32_t n;        /* kept hits */
+    const int32_t *rows; /* [n] pad rows, increasing */
+    const float *y;   /* [n] */
+    const float *z;   /* [n] */
+} orc_segment;
+
+typedef struct {
+    int32_t ok, nhits, nseg, first_row; /* first_row: innermost row of the innermost segment = reference row */
+    double p[5], cov[15], chi2;
+} orc_fit;
+
+static double sector_alpha(const orc_config *c, int from_sector, int to_sector) {
+    /* rotation angle from the frame of from_sector to the frame of to_sector, both on the same z side */
+    const int half = c->sectors_per_event / 2;
+    int d = (to_sector % half) - (from_sector % half);
+    if (d > half / 2) d -= half;
+    if (d < -half / 2) d += half;
+    return 2.0 * (double)c->half_angle_rad * d;
+}
+
+/* M1 + M4: fit of a chain of segments given inside out (seg[0] innermost).  n_seg = 1 is the plain refit of one
+ * track's kept hits. */
+void orc_refit_chain(const orc_config *c, const orc_segment *seg, int n_seg, orc_fit *f) {
+    const double cB = curv_const(c), sy2 = (double)c->sigma_y * c->sigma_y, sz2 = (double)c->sigma_z * c->sigma_z;
+    memset(f, 0, sizeof(*f));
+    f->nseg = n_seg;
+    const orc_segment *o = &seg[n_seg - 1]; /* outermost segment: seed and start there */
+    if (o->n < 3) return;
+    const int ii[3] = {0, o->n / 2, o->n - 1};
+    double sx[3], sy[3], sz[3];
+    for (int m = 0; m < 3; m++) {
+        sx[m] = (double)c->row_x[o->rows[ii[m]]];
+        sy[m] = (double)o->y[ii[m]];
+        sz[m] = (double)o->z[ii[m]];
+    }
+    double p[5], P[25], p1[5], P1[25];
+    orc_seed(sx, sy, sz, cB, p);
+    if (!(fabs(p[2]) <= c->kf_max_sinphi)) return;
+    memset(P, 0, sizeof(P));
+    for (int i = 0; i < 5; i++) P[i * 5 + i] = c->kf_p0[i];
+    /* one step from the seed's plane (innermost hit of the outermost segment) to its outermost hit; only the state
+     * is kept, the covariance restarts from the prior there */
+    double x = (double)c->row_x[o->rows[o->n - 1]];
+    if (o->n > 1) {
+        if (orc_transport(p, P, x - sx[0], cB, c->kf_max_sinphi, p1, P1, NULL)) return;
+        memcpy(p, p1, sizeof(p1));
+    }
+    memset(P, 0, sizeof(P));
+    for (int i = 0; i < 5; i++) P[i * 5 + i] = c->kf_p0[i];
+    double chi2 = 0.0;
+    int nhits = 0;
+    for (int s = n_seg - 1; s >= 0; s--) {
+        const orc_segment *g = &seg[s];
+        if (s < n_seg - 1) { /* M2: into this segment's frame, then to its outermost hit's row */
+            double xr;
+            if (orc_rotate(p, P, x, sector_alpha(c, seg[s + 1].sector, g->sector), cB, c->kf_max_sinphi, p1, P1, &xr, NULL))
+                return;
+            memcpy(p, p1, sizeof(p1));
+            memcpy(P, P1, sizeof(P1));
+            x = xr;
+        }
+        for (int i = g->n - 1; i >= 0; i--) {
+            const double xi = (double)c->row_x[g->rows[i]];
+            if (xi != x) {
+                if (orc_transport(p, P, xi - x, cB, c->kf_max_sinphi, p1, P1, NULL)) return;
+                memcpy(p, p1, sizeof(p1));
+                memcpy(P, P1, sizeof(P1));
+                x = xi;
+            }
+            chi2 += orc_update(p, P, (double)g->y[i], (double)g->z[i], sy2, sz2);
+            nhits++;
+        }
+    }
+    f->ok = 1;
+    f->nhits = nhits;
+    f->first_row = seg[0].rows[0];
+    memcpy(f->p, p, sizeof(p));
+    pack_cov(P, f->cov);
+    f->chi2 = chi2;
+}
+
+/* Phase 2 on the S6 output (final tracks with their kept hits as global cluster indices, rows increasing).
+ * trk_inst[t] = sector instance of track t.  Outputs: seg_fit [n_tracks] (M1 of every track alone), seg_next /
+ * seg_prev [n_tracks] (M3 links, -1 none), merged tracks (M4) in ascending innermost segment: m_first [<= n_tracks],
+ * m_fit.  Returns the number of merged tracks. */
+int64_t orc_phase2(const orc_config *c, const float *clusters, const int32_t *row_offsets, int32_t n_inst,
+                   int64_t n_tracks, const int32_t *trk_inst, const int64_t *trk_hit_offset, const int32_t *trk_hits,
+                   orc_fit *seg_fit, int32_t *seg_next, int32_t *seg_prev, int32_t *m_first, orc_fit *m_fit) {
+    const int R = c->n_rows, spe = c->sectors_per_event, half = spe / 2;
+    const double cB = curv_const(c);
+    const int64_t nh_all = n_tracks > 0 ? trk_hit_offset[n_tracks] : 0;
+    int32_t *rows = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nh_all + 1));
+    float *hy = (float *)malloc(sizeof(float) * (size_t)(nh_all + 1));
+    float *hz = (float *)malloc(sizeof(float) * (size_t)(nh_all + 1));
+    orc_segment *segs = (orc_segment *)malloc(sizeof(orc_segment) * (size_t)(n_tracks + 1));
+    for (int64_t t = 0; t < n_tracks; t++) {
+        const int32_t *ro = row_offsets + (size_t)trk_inst[t] * R;
+        for (int64_t k = trk_hit_offset[t]; k < trk_hit_offset[t + 1]; k++) {
+            rows[k] = row_of(ro, R, trk_hits[k]);
+            hy[k] = clusters[4 * (size_t)trk_hits[k] + 1];
+            hz[k] = clusters[4 * (size_t)trk_hits[k] + 2];
+        }
+        segs[t].sector = trk_inst[t] % spe;
+        segs[t].n = (int32_t)(trk_hit_offset[t + 1] - trk_hit_offset[t]);
+        segs[t].rows = rows + trk_hit_offset[t];
+        segs[t].y = hy + trk_hit_offset[t];
+        segs[t].z = hz + trk_hit_offset[t];
+        orc_refit_chain(c, &segs[t], 1, &seg_fit[t]); /* M1 */
+        seg_next[t] = seg_prev[t] = -1;
+    }
+    /* M3: best successor of every A, best predecessor of every B, then mutual choices.  Tracks of one window are
+     * contiguous in t (instances ascending), so the scan over B is limited to that window. */
+    int32_t *best_next = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_tracks + 1));
+    int32_t *best_prev = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_tracks + 1));
+    double *best_prev_d2 = (double *)malloc(sizeof(double) * (size_t)(n_tracks + 1));
+    for (int64_t t = 0; t < n_tracks; t++) { best_next[t] = best_prev[t] = -1; best_prev_d2[t] = 0.0; }
+    int64_t w0 = 0;
+    while (w0 < n_tracks) {
+        int64_t w1 = w0;
+        while (w1 < n_tracks && trk_inst[w1] / spe == trk_inst[w0] / spe) w1++;
+        for (int64_t a = w0; a < w1; a++) {
+            const orc_segment *A = &segs[a];
+            const int side_a = A->sector >= half, la = A->rows[A->n - 1];
+            double bd2 = 0.0;
+            for (int64_t b = w0; b < w1; b++) {
+                const orc_segment *B = &segs[b];
+                if (b == a || !seg_fit[b].ok || (B->sector >= half) != side_a) continue;
+                int ds = (B->sector % half) - (A->sector % half);
+                if (ds < 0) ds += half;
+                if (ds != 1 && ds != half - 1) continue; /* neighbouring sectors, cyclic */
+                const int fb = B->rows[0];
+                if (!(fb > la && fb - la <= 10)) continue;
+                double p1[5], P1[25], p2[5], P2[25], P0[25], xr;
+                unpack_cov_c(seg_fit[b].cov, P0);
+                if (orc_rotate(seg_fit[b].p, P0, (double)c->row_x[fb], sector_alpha(c, B->sector, A->sector), cB,
+                               c->kf_max_sinphi, p1, P1, &xr, NULL))
+                    continue;
+                if (orc_transport(p1, P1, (double)c->row_x[la] - xr, cB, c->kf_max_sinphi, p2, P2, NULL)) continue;
+                const double dy = p2[0] - (double)A->y[A->n - 1], dz = p2[1] - (double)A->z[A->n - 1];
+                if (!(fabs(dy) <= 2.0 && fabs(dz) <= 2.0)) continue;
+                const double d2 = dy * dy + dz * dz;
+                if (best_next[a] < 0 || d2 < bd2) { best_next[a] = (int32_t)b; bd2 = d2; } /* b ascending: ties keep the lower */
+                if (best_prev[b] < 0 || d2 < best_prev_d2[b]) { best_prev[b] = (int32_t)a; best_prev_d2[b] = d2; }
+            }
+        }
+        w0 = w1;
+    }
+    for (int64_t a = 0; a < n_tracks; a++)
+        if (best_next[a] >= 0 && best_prev[best_next[a]] == a) {
+            seg_next[a] = best_next[a];
+            seg_prev[best_next[a]] = (int32_t)a;
+        }
+    /* M4: chains, inside out, in ascending innermost segment */
+    int64_t nm = 0;
+    orc_segment chain[64];
+    for (int64_t t = 0; t < n_tracks; t++) {
+        if (seg_prev[t] >= 0) continue; /* not an innermost segment */
+        int n = 0;
+        for (int32_t x = (int32_t)t; x >= 0 && n < 64; x = seg_next[x]) chain[n++] = segs[x];
+        m_first[nm] = (int32_t)t;
+        if (n == 1) m_fit[nm] = seg_fit[t];
+        else orc_refit_chain(c, chain, n, &m_fit[nm]);
+        nm++;
+    }
+    free(rows); free(hy); free(hz); free(segs); free(best_next); free(best_prev); free(best_prev_d2);
+    return nm;
+}
+
+int32_t orc_sizeof_fit(void) { return (int32_t)sizeof(orc_fit); }
+int32_t orc_sizeof_segment(void) { return (int32_t)sizeof(orc_segment); }

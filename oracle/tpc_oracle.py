@@ -50,6 +50,24 @@ TRACKLET_DTYPE = np.dtype([("ok", "<i4"), ("nhits", "<i4"), ("first_row", "<i4")
                            ("ref_row", "<i4"), ("_pad", "<i4"), ("p", "<f8", (5,)), ("cov", "<f8", (15,)),
                            ("chi2", "<f8")])
 
+FIT_DTYPE = np.dtype([("ok", "<i4"), ("nhits", "<i4"), ("nseg", "<i4"), ("first_row", "<i4"), ("p", "<f8", (5,)),
+                      ("cov", "<f8", (15,)), ("chi2", "<f8")])
+
+
+class Segment(C.Structure):
+    _fields_ = [("sector", C.c_int32), ("n", C.c_int32), ("rows", C.POINTER(C.c_int32)), ("y", C.POINTER(C.c_float)),
+                ("z", C.POINTER(C.c_float))]
+
+
+@dataclass
+class Phase2Result:
+    seg_fit: np.ndarray    # FIT_DTYPE [n_tracks]: refit of every final track alone (kept hits only)
+    seg_next: np.ndarray   # [n_tracks] track that continues this one outward in the neighbouring sector, or -1
+    seg_prev: np.ndarray
+    m_first: np.ndarray    # [n_merged] innermost segment (track index) of every merged track, ascending
+    m_fit: np.ndarray      # FIT_DTYPE [n_merged]
+
+
 _lib = None
 
 
@@ -60,6 +78,8 @@ def lib():
         assert _lib.orc_sizeof_tracklet() == C.sizeof(Tracklet) == TRACKLET_DTYPE.itemsize
         assert _lib.orc_sizeof_config() == C.sizeof(Config)
         _lib.orc_update.restype = C.c_double
+        _lib.orc_phase2.restype = C.c_int64
+        assert _lib.orc_sizeof_fit() == FIT_DTYPE.itemsize and _lib.orc_sizeof_segment() == C.sizeof(Segment)
     return _lib
 
 
@@ -234,6 +254,59 @@ class Oracle:
         lib().orc_seed(_p(x, C.c_double), _p(y, C.c_double), _p(z, C.c_double), C.c_double(self.c_b),
                        _p(p, C.c_double))
         return p
+
+
+    # ---- phase 2: sector merger + refit -------------------------------------------------
+    def rotate(self, p, P, x, alpha, want_jac=False):
+        """State on the plane x of one sector frame -> state in the frame rotated by +alpha (reading M2).  Returns
+        (p1, P1, x1[, J]) or None."""
+        p = np.ascontiguousarray(p, np.float64)
+        P = np.ascontiguousarray(P, np.float64).reshape(25)
+        p1, P1, J = np.empty(5), np.empty(25), np.empty(25)
+        x1 = C.c_double()
+        rc = lib().orc_rotate(_p(p, C.c_double), _p(P, C.c_double), C.c_double(x), C.c_double(alpha),
+                              C.c_double(self.c_b), C.c_double(self.cfg.kf_max_sinphi), _p(p1, C.c_double),
+                              _p(P1, C.c_double), C.byref(x1), _p(J, C.c_double))
+        if rc:
+            return None
+        out = (p1, P1.reshape(5, 5), x1.value)
+        return out + (J.reshape(5, 5),) if want_jac else out
+
+    def refit_chain(self, segments):
+        """segments: list of (sector, rows, y, z) inside out, rows increasing (readings M1, M4).  Returns a FIT_DTYPE
+        record."""
+        keep, segs = [], (Segment * len(segments))()
+        for i, (sec, rows, y, z) in enumerate(segments):
+            r = np.ascontiguousarray(rows, np.int32)
+            yy = np.ascontiguousarray(y, np.float32)
+            zz = np.ascontiguousarray(z, np.float32)
+            keep.append((r, yy, zz))
+            segs[i].sector, segs[i].n = int(sec), len(r)
+            segs[i].rows, segs[i].y, segs[i].z = _p(r, C.c_int32), _p(yy, C.c_float), _p(zz, C.c_float)
+        f = np.zeros(1, FIT_DTYPE)
+        lib().orc_refit_chain(C.byref(self.cfg), segs, C.c_int(len(segments)), C.c_void_p(f.ctypes.data))
+        return f[0]
+
+    def phase2(self, clusters, row_offsets, n_inst, res: "OracleResult") -> Phase2Result:
+        """Merger + refit on the final tracks of `res` (an OracleResult of the same input)."""
+        cl = np.ascontiguousarray(clusters, np.float32)
+        ro = np.ascontiguousarray(row_offsets, np.int32)
+        nt = len(res.trk_cand)
+        inst = (np.searchsorted(ro[::self.n_rows], res.cand_hits[res.trk_cand, 0], side="right") - 1).astype(np.int32) \
+            if nt else np.zeros(0, np.int32)
+        inst = np.ascontiguousarray(inst)
+        off = np.ascontiguousarray(res.trk_hit_offset, np.int64)
+        hits = np.ascontiguousarray(res.trk_hits, np.int32)
+        seg_fit = np.zeros(max(nt, 1), FIT_DTYPE)
+        m_fit = np.zeros(max(nt, 1), FIT_DTYPE)
+        nxt = np.full(max(nt, 1), -1, np.int32)
+        prv = np.full(max(nt, 1), -1, np.int32)
+        mf = np.full(max(nt, 1), -1, np.int32)
+        nm = lib().orc_phase2(C.byref(self.cfg), _p(cl, C.c_float), _p(ro, C.c_int32), C.c_int32(n_inst),
+                              C.c_int64(nt), _p(inst, C.c_int32), _p(off, C.c_int64), _p(hits, C.c_int32),
+                              C.c_void_p(seg_fit.ctypes.data), _p(nxt, C.c_int32), _p(prv, C.c_int32),
+                              _p(mf, C.c_int32), C.c_void_p(m_fit.ctypes.data)) if nt else 0
+        return Phase2Result(seg_fit[:nt], nxt[:nt], prv[:nt], mf[:nm], m_fit[:nm])
 
 
 def unpack_cov(c15):
