@@ -245,6 +245,45 @@ int tpc_track_sectors_host(tpc_tracker_t* t, const void* h_clusters, const int32
                            tpc_slot_t* slots, int32_t n_slots, void* h2d_stream, void* compute_stream,
                            void* d2h_stream, tpc_host_output_t* hout);
 
+/*
+ * Phase 2: sector merger + track refit ("The second phase merges the track segments found in the
+ * individual sectors to final tracks and performs a track refit"; PAPER.md:33 names a GPU prototype of this fit;
+ * SURVEY.md 8(f) NEXT-3).  Readings M1-M4 of DESIGN.md:
+ *   refit     every final track is fitted again over the hits it KEPT in S6 (seed at the innermost kept hit, one step
+ *             to the outermost, prior reset, filter inward); this replaces S6's "parameters of the tracklet, lost
+ *             hits included".
+ *   merge     segment B continues segment A outward iff same event/window, same z side, neighbouring sectors,
+ *             first_row(B) in (last_row(A), last_row(A) + 10], and B's refitted state at its innermost hit, rotated
+ *             into A's frame and transported to A's outermost row, lies within 2 cm in y and z of A's outermost hit;
+ *             nearest candidate, mutual choice.
+ *   merged    a chain of segments gets ONE fit: filter from the outermost hit of the outermost segment inward,
+ *             rotating the state and covariance at every sector boundary; reported at the innermost hit of the
+ *             innermost segment, in that segment's frame.
+ * tpc_merge_refit works on the final tracks of the LAST tpc_track_sectors call of this tracker: it reads that call's
+ * workspace and its row_offsets array, so it must follow it (same stream; asynchronous) before the workspace is
+ * reused, and row_offsets must still be valid and unchanged.  Track indices are
+ * those of that call (positions in trk_*).  All pointers: caller-owned DEVICE memory, NULL = skipped, counts2 required.
+ */
+typedef struct {
+    int32_t* seg_next;   /* [n_tracks] track that continues this one outward in the neighbouring sector, or -1 */
+    int32_t* seg_prev;   /* [n_tracks] the inverse link */
+    int32_t* seg_ok;     /* [n_tracks] 1 = the refit of this track alone succeeded (0: |sinPhi| limit hit; keep trk_params) */
+    float* seg_params;   /* [n_tracks][5] refit of the track's kept hits, at its innermost kept hit */
+    float* seg_cov;      /* [n_tracks][15] */
+    float* seg_chi2;     /* [n_tracks] */
+    int32_t* mtrk_first; /* [mtrk_capacity] innermost segment (track index) of merged track m; ascending */
+    int32_t* mtrk_nseg;  /* [mtrk_capacity] segments in the chain (1 = not merged) */
+    int32_t* mtrk_nhits; /* [mtrk_capacity] kept hits of the whole chain */
+    int32_t* mtrk_ok;    /* [mtrk_capacity] 1 = the chain fit succeeded */
+    float* mtrk_params;  /* [mtrk_capacity][5] at the innermost hit of the innermost segment, in its sector frame */
+    float* mtrk_cov;     /* [mtrk_capacity][15] */
+    float* mtrk_chi2;    /* [mtrk_capacity] */
+    int64_t mtrk_capacity;
+    int64_t* counts2;    /* device [4]: merged tracks (required count), links, failed track refits, failed chain fits */
+} tpc_phase2_output_t;
+
+int tpc_merge_refit(tpc_tracker_t* t, const tpc_phase2_output_t* out);
+
 const char* tpc_last_error(const tpc_tracker_t* t);
 
 #ifdef __cplusplus

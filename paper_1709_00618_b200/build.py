@@ -28,6 +28,7 @@ SOURCES = {
     "k34_links_chains.cu": [],
     "k5_follow.cu": [],
     "k6_select.cu": [],
+    "k7_phase2.cu": [],
     "host_pipeline.cu": [],
 }
 

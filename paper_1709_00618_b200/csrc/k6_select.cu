@@ -158,6 +158,8 @@ struct FinalIn {
     uint32_t* tl_sel;
     int64_t* counts;
     int64_t Cmax;
+    int32_t* trk_cand;  // [Tmax] workspace copy of the track -> candidate map (phase 2)
+    int64_t Tmax;
 };
 
 __global__ void __launch_bounds__(kSelThreads)
@@ -189,6 +191,7 @@ finalize_tracks_kernel(const __grid_constant__ DevGeom g, const FinalIn a, const
         uint32_t* rec = a.tl_sel + c * g.sel_stride;
         rec[g.sel_words] = is_trk ? (uint32_t)trk : 0xFFFFFFFFu;
         rec[g.sel_words + 1] = (uint32_t)h0;
+        if (kept > 0 && trk < a.Tmax) a.trk_cand[trk] = (int32_t)c;
         if (!is_trk) continue;
         const int rows = a.tl_rows[c];
         if (o.trk_params)
@@ -258,7 +261,7 @@ int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const 
         count_kernel<<<grid, kSelThreads, 0, s>>>(g, w.tl_nhits, w.tl_sel, w.sel_part, w.counts, w.Cmax);
         launch_scan_int2(w.sel_part, w.counts + 1, kSelBlock, w.Cmax, 0, w.counts, 3, 4, s);
         const FinalIn a{w.tl_nhits, w.tl_rows, w.cand_slab, w.tl_par, w.tl_cov, w.tl_chi2, w.sel_part, w.tl_sel,
-                        w.counts,   w.Cmax};
+                        w.counts,   w.Cmax,    w.trk_cand,  w.Tmax};
         finalize_tracks_kernel<<<grid, kSelThreads, 0, s>>>(g, a, o);
         write_hits_kernel<<<hgrid, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel, w.hit_idx, o,
                                                         slabs);

@@ -158,6 +158,47 @@ __device__ __forceinline__ float kf_update(KfState& st, float ym, float zm, floa
     return chi2;
 }
 
+// Change of sector frame (phase 2, reading M2): the state on the plane x of one sector-local frame becomes the state
+// on the plane x1 of the frame rotated by +alpha about the beam axis (ca = cos alpha, sa = sin alpha).  y_abs is the
+// ABSOLUTE y of the state (the kernels carry st.y relative to a reference); on return st.y is the absolute y in the
+// new frame.  Exact rotation; the Jacobian of "state on the old plane -> state on the fixed new plane" has four
+// non-trivial entries: sliding back to the plane along the track scales y by cos(phi)/cos(phi'), shifts z by the
+// dz/ds of the slide and turns the direction by the curvature over it.  Returns false (state untouched) if
+// |sinPhi| leaves [-max_s, max_s] or the rotated direction points backwards.
+__device__ __forceinline__ bool kf_rotate(KfState& st, float y_abs, float x, float ca, float sa, float cB, float max_s,
+                                          float& x1) {
+    const float s = st.s;
+    if (fabsf(s) > max_s) return false;
+    const float c = sqrtf((1.0f - s) * (1.0f + s));
+    const float s1 = s * ca - c * sa, c1 = c * ca + s * sa;
+    if (fabsf(s1) > max_s || c1 <= 0.0f) return false;
+    const float ic1 = 1.0f / c1;
+    const float j00 = c * ic1, j10 = -sa * st.t * ic1, j20 = -sa * cB * st.k, j22 = c1 / c;
+    x1 = x * ca + y_abs * sa;
+    st.y = -x * sa + y_abs * ca;
+    st.s = s1;
+    // P <- J P J^T for rows y' = j00 y, z' = z + j10 y, s' = j20 y + j22 s (t, k unchanged)
+    const float a20 = j20 * st.c00 + j22 * st.c20;  // cov(s', y)
+    const float n11 = st.c11 + j10 * (2.0f * st.c10 + j10 * st.c00);
+    const float n21 = j20 * st.c10 + j22 * st.c21 + j10 * a20;
+    const float n22 = j20 * (j20 * st.c00 + 2.0f * j22 * st.c20) + j22 * j22 * st.c22;
+    const float n31 = st.c31 + j10 * st.c30, n32 = j20 * st.c30 + j22 * st.c32;
+    const float n41 = st.c41 + j10 * st.c40, n42 = j20 * st.c40 + j22 * st.c42;
+    st.c10 = j00 * (st.c10 + j10 * st.c00);
+    st.c00 = j00 * j00 * st.c00;
+    st.c11 = n11;
+    st.c20 = j00 * a20;
+    st.c21 = n21;
+    st.c22 = n22;
+    st.c30 = j00 * st.c30;
+    st.c31 = n31;
+    st.c32 = n32;
+    st.c40 = j00 * st.c40;
+    st.c41 = n41;
+    st.c42 = n42;
+    return true;
+}
+
 // Seed: circle through three points in (x,y); dz/ds from the end points.  Returns false if |sinPhi| > max_s.
 __device__ __forceinline__ bool kf_seed(KfState& st, float x0, float y0, float z0, float x1, float y1, float x2,
                                         float y2, float z2, float cB, float max_s, const float* p0) {

@@ -35,6 +35,7 @@ struct DevGeom {
     int max_gap;
     float max_s, edge_margin, tan_half;
     int sel_min;
+    float cos_2h, sin_2h;  // rotation between neighbouring sector frames: angle 2 * half_angle
     float sy2, sz2;
     float cB;       // curvature per (q/pt): kappa = cB * q/pt
     const float* row_x;  // device [R]
@@ -78,6 +79,21 @@ struct Workspace {
     int2* sel_part;       // [Cmax/64 + 2] (tracks, hits) per block of 256 tracklets, then exclusive scan
     int64_t* counts;      // [8] internal copy of the output counts
     int64_t Cmax;
+    // phase 2 (k7_phase2.cu), indexed by final track; Tmax = N / sel_min + 1 bounds the tracks (disjoint kept hits)
+    int64_t Tmax;
+    int32_t* trk_cand;    // [Tmax] candidate id of the final track (written by S6)
+    float* p2_par;        // [Tmax][5]  refit of the track's kept hits alone (reading M1)
+    float* p2_cov;        // [Tmax][15]
+    float* p2_chi2;       // [Tmax]
+    int4* p2_info;        // [Tmax] ok, first row, last row, kept hits
+    float2* p2_last;      // [Tmax] (y, z) of the outermost kept hit
+    int32_t* p2_first;    // [S + 1] first track of every sector instance
+    unsigned long long* p2_best_prev;  // [Tmax] (d2 bits << 32 | predecessor) minimum, ~0 = none
+    int32_t* p2_best_next;             // [Tmax]
+    int32_t* p2_next;     // [Tmax] links (reading M3)
+    int32_t* p2_prev;
+    int2* p2_part;        // [Tmax/256 + 2] heads per block of 256 tracks, then exclusive scan (.x)
+    int64_t* p2_counts;   // [4] merged tracks, links, failed segment refits, failed chain fits
 };
 
 struct Problem {
@@ -138,6 +154,15 @@ struct SelectOut {  // mirrors the S6 part of tpc_output_t
 };
 int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const SelectOut& o, cudaStream_t s);
 // expands the compact tracklet hit table into global indices [Cmax_out][R] (parity/debug output)
+struct Phase2Out {  // mirrors tpc_phase2_output_t
+    int32_t *seg_next, *seg_prev, *seg_ok;
+    float *seg_params, *seg_cov, *seg_chi2;
+    int32_t *mtrk_first, *mtrk_nseg, *mtrk_nhits, *mtrk_ok;
+    float *mtrk_params, *mtrk_cov, *mtrk_chi2;
+    int64_t mtrk_capacity;
+    int64_t* counts2;
+};
+int launch_phase2(const DevGeom& g, const Workspace& w, const Problem& p, const Phase2Out& o, cudaStream_t s);
 int launch_export_tracklets(const DevGeom& g, const Workspace& w, const Problem& p, int32_t* tl_hits, int32_t* tl_rows,
                             int64_t cap, cudaStream_t s);
 

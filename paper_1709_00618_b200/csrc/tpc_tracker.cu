@@ -94,6 +94,8 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     g.edge_margin = dflt(p.kf_edge_margin, 2.0f);
     g.tan_half = (float)std::tan((double)geom->half_angle_rad);
     g.sel_min = dflt(p.sel_min_hits, 10);
+    g.cos_2h = (float)std::cos(2.0 * (double)geom->half_angle_rad);
+    g.sin_2h = (float)std::sin(2.0 * (double)geom->half_angle_rad);
     g.sy2 = (float)((double)geom->sigma_y * (double)geom->sigma_y);
     g.sz2 = (float)((double)geom->sigma_z * (double)geom->sigma_z);
     g.cB = (float)(-0.00299792458 * (double)bz);
@@ -199,6 +201,21 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.tl_sel = c.take<uint32_t>(cmax * g.sel_stride);
     v.sel_part = c.take<int2>(cmax / 64 + 2);
     v.Cmax = (int64_t)cmax;
+    const size_t tmax = (size_t)(N / (g.sel_min > 0 ? g.sel_min : 1) + 1);
+    v.Tmax = (int64_t)tmax;
+    v.trk_cand = c.take<int32_t>(tmax);
+    v.p2_par = c.take<float>(tmax * 5);
+    v.p2_cov = c.take<float>(tmax * 15);
+    v.p2_chi2 = c.take<float>(tmax);
+    v.p2_info = c.take<int4>(tmax);
+    v.p2_last = c.take<float2>(tmax);
+    v.p2_first = c.take<int32_t>((size_t)(S > 0 ? S : 1) + 1);
+    v.p2_best_prev = c.take<unsigned long long>(tmax);
+    v.p2_best_next = c.take<int32_t>(tmax);
+    v.p2_next = c.take<int32_t>(tmax);
+    v.p2_prev = c.take<int32_t>(tmax);
+    v.p2_part = c.take<int2>(tmax / 256 + 2);
+    v.p2_counts = c.take<int64_t>(4);
     if (w) *w = v;
     return (c.off + 255) & ~(size_t)255;
 }
@@ -326,6 +343,31 @@ int tpc_track_on(tpc_tracker* t, void* ws, size_t ws_bytes, cudaStream_t s, bool
         }
     }
     t->last_launches = launches;
+    t->last_ws = ws;
+    t->last_ws_bytes = ws_bytes;
+    t->last_stream = s;
+    t->last_first_inst = first_inst;
+    t->last_row_offsets = row_offsets;
+    t->last_n_inst = n_inst;
+    t->last_n_clusters = n_clusters;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, std::string("CUDA: ") + cudaGetErrorString(e));
+    return TPC_OK;
+}
+
+extern "C" int tpc_merge_refit(tpc_tracker_t* t, const tpc_phase2_output_t* out) {
+    if (!t) return TPC_ERR_ARG;
+    if (!out || !out->counts2) return fail(t, TPC_ERR_ARG, "out and out->counts2 are required");
+    if (!t->last_ws) return fail(t, TPC_ERR_ARG, "tpc_merge_refit needs a preceding tpc_track_sectors call on this tracker");
+    Workspace w;
+    carve(t->g, t->last_ws, t->last_n_clusters, t->last_n_inst, &w);
+    DevGeom g = t->g;
+    g.inst_phase = t->last_first_inst % g.spe;
+    Problem p{nullptr, t->input_layout, t->last_row_offsets, t->last_n_inst, t->last_n_clusters};
+    const Phase2Out o{out->seg_next, out->seg_prev, out->seg_ok, out->seg_params, out->seg_cov, out->seg_chi2,
+                      out->mtrk_first, out->mtrk_nseg, out->mtrk_nhits, out->mtrk_ok, out->mtrk_params, out->mtrk_cov,
+                      out->mtrk_chi2, out->mtrk_capacity, out->counts2};
+    t->last_launches = launch_phase2(g, w, p, o, t->last_stream);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, std::string("CUDA: ") + cudaGetErrorString(e));
     return TPC_OK;

@@ -14,6 +14,13 @@ struct tpc_tracker {
     int n_sm = 148;
     float z_lo = 0.0f, z_hi = 0.0f;  // geometry z range of the z >= 0 side
     int last_launches = 0;
+    // the problem of the last tpc_track_sectors call: tpc_merge_refit (phase 2) reads its workspace
+    void* last_ws = nullptr;
+    size_t last_ws_bytes = 0;
+    cudaStream_t last_stream = nullptr;
+    int32_t last_first_inst = 0, last_n_inst = 0;
+    const int32_t* last_row_offsets = nullptr;
+    int64_t last_n_clusters = 0;
     bool timing = false;
     int input_layout = TPC_INPUT_XYZW;  // tpc_set_input_layout
     bool count_work = false;  // S5 work counters counts[6..9] (tpc_set_work_counters)

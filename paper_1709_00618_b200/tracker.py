@@ -24,7 +24,8 @@ ERRORS = {-1: "TPC_ERR_ARG", -2: "TPC_ERR_GEOMETRY", -3: "TPC_ERR_WORKSPACE", -4
 EXPORTS = ("tpc_tracker_create", "tpc_tracker_destroy", "tpc_workspace_bytes", "tpc_set_workspace", "tpc_set_stream",
            "tpc_track_sectors", "tpc_check_counts", "tpc_last_launch_count", "tpc_set_stage_timing",
            "tpc_stage_times_ms", "tpc_last_error", "tpc_track_sectors_host", "tpc_set_work_counters",
-           "tpc_set_input_layout", "tpc_pipeline_create", "tpc_pipeline_destroy", "tpc_pipeline_run")
+           "tpc_set_input_layout", "tpc_pipeline_create", "tpc_pipeline_destroy", "tpc_pipeline_run",
+           "tpc_merge_refit")
 INPUT_LAYOUTS = {"xyzw": 0, "yz": 1, "i16": 2}       # TPC_INPUT_*
 LAYOUT_BYTES = {"xyzw": 16, "yz": 8, "i16": 4}
 I16_Y_STEP, I16_Z_STEP = 1.0 / 256.0, 1.0 / 64.0     # TPC_I16_*_STEP
@@ -62,6 +63,14 @@ class Output(C.Structure):
                 ("trk_sector", C.c_void_p), ("trk_hit_offset", C.c_void_p), ("trk_hits", C.c_void_p),
                 ("trk_capacity", C.c_int64), ("trk_hits_capacity", C.c_int64), ("cluster_owner", C.c_void_p),
                 ("counts", C.c_void_p)]
+
+
+class Phase2Output(C.Structure):
+    _fields_ = [("seg_next", C.c_void_p), ("seg_prev", C.c_void_p), ("seg_ok", C.c_void_p), ("seg_params", C.c_void_p),
+                ("seg_cov", C.c_void_p), ("seg_chi2", C.c_void_p), ("mtrk_first", C.c_void_p), ("mtrk_nseg", C.c_void_p),
+                ("mtrk_nhits", C.c_void_p), ("mtrk_ok", C.c_void_p), ("mtrk_params", C.c_void_p),
+                ("mtrk_cov", C.c_void_p), ("mtrk_chi2", C.c_void_p), ("mtrk_capacity", C.c_int64),
+                ("counts2", C.c_void_p)]
 
 
 class Slot(C.Structure):
@@ -112,6 +121,7 @@ def load_library():
     lib.tpc_track_sectors_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_int32,
                                            C.POINTER(Slot), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.POINTER(HostOutput)]
+    lib.tpc_merge_refit.argtypes = [C.c_void_p, C.POINTER(Phase2Output)]
     lib.tpc_pipeline_create.argtypes = [C.c_void_p, C.POINTER(Slot), C.c_int32, C.POINTER(C.c_void_p)]
     lib.tpc_pipeline_destroy.argtypes = [C.c_void_p]
     lib.tpc_pipeline_destroy.restype = None
@@ -305,6 +315,43 @@ class Tracker:
                                                C.c_void_p(row_offsets.data_ptr()), int(n_inst), n,
                                                C.byref(out_struct)), "tpc_track_sectors")
 
+    # ---- phase 2: sector merger + refit on the final tracks of the last track_sectors call ------------------------
+    def alloc_phase2(self, n_tracks):
+        """Device buffers for tpc_merge_refit sized for n_tracks final tracks (+ the ctypes struct)."""
+        t = self._torch
+        dev = self.device
+        n = max(int(n_tracks), 1)
+        i32, f32, i64 = t.int32, t.float32, t.int64
+        bufs = dict(seg_next=t.empty(n, dtype=i32, device=dev), seg_prev=t.empty(n, dtype=i32, device=dev),
+                    seg_ok=t.empty(n, dtype=i32, device=dev), seg_params=t.empty((n, 5), dtype=f32, device=dev),
+                    seg_cov=t.empty((n, 15), dtype=f32, device=dev), seg_chi2=t.empty(n, dtype=f32, device=dev),
+                    mtrk_first=t.empty(n, dtype=i32, device=dev), mtrk_nseg=t.empty(n, dtype=i32, device=dev),
+                    mtrk_nhits=t.empty(n, dtype=i32, device=dev), mtrk_ok=t.empty(n, dtype=i32, device=dev),
+                    mtrk_params=t.empty((n, 5), dtype=f32, device=dev), mtrk_cov=t.empty((n, 15), dtype=f32, device=dev),
+                    mtrk_chi2=t.empty(n, dtype=f32, device=dev), counts2=t.zeros(4, dtype=i64, device=dev))
+        o = Phase2Output()
+        for k, v in bufs.items():
+            setattr(o, k, v.data_ptr())
+        o.mtrk_capacity = n
+        return bufs, o
+
+    def merge_refit_device(self, out_struct):
+        """tpc_merge_refit on the tracks of the last track call of this tracker; asynchronous."""
+        self._check(self.lib.tpc_merge_refit(self._h, C.byref(out_struct)), "tpc_merge_refit")
+
+    def merge_refit(self, n_tracks):
+        """numpy results of phase 2 for the last track_sectors() call (its workspace is still attached)."""
+        t = self._torch
+        with t.cuda.device(self.device):
+            bufs, o = self.alloc_phase2(n_tracks)
+            self.merge_refit_device(o)
+            t.cuda.synchronize(self.device)
+        c2 = bufs["counts2"].cpu().numpy()
+        nm = int(c2[0])
+        res = {k: v.cpu().numpy()[:(nm if k.startswith("mtrk") else n_tracks)] for k, v in bufs.items() if k != "counts2"}
+        res["counts2"] = c2
+        return res
+
     # ---- convenience: numpy in, numpy out (used by the parity tests) ----------------------------------------------
     def track_sectors(self, clusters: np.ndarray, row_offsets: np.ndarray, n_inst: int, *, debug=False,
                       cand_capacity=None, trk_capacity=None) -> TrackResult:
@@ -316,6 +363,7 @@ class Tracker:
                               .reshape(-1, 4 if self.input_layout == "xyzw" else 2)).to(self.device)
         ro = t.from_numpy(np.ascontiguousarray(row_offsets, np.int32)).to(self.device)
         n = int(cl.shape[0])
+        self._last_inputs = (cl, ro)  # tpc_merge_refit reads the row offsets of the last call: keep them alive
         with t.cuda.device(self.device):
             self.reserve(n, n_inst)
             self.set_stream()
