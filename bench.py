@@ -299,6 +299,28 @@ def run_ours(args):
     stage_ms = {nme: float(np.mean([s[nme] for s in st])) for nme in st[0]}
     own = bufs["cluster_owner"][:evs[0].n_clusters].cpu().numpy()  # window 0 of the default reading (physics report)
 
+    # ---- phase 2 on the same batch: sector merger + refit of the final tracks -----------------
+    phase2 = None
+    if "phase2" not in skip:
+        n_trk = int(counts[3])
+        p2bufs, p2o = trk.alloc_phase2(n_trk)
+        evp = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)]
+        trk.set_stream()
+        trk.merge_refit_device(p2o)  # the last call on d_cl/d_ro is still the tracked one
+        for a, b in evp:
+            a.record()
+            trk.merge_refit_device(p2o)
+            b.record()
+        torch.cuda.synchronize(dev)
+        c2 = p2bufs["counts2"].cpu().numpy()
+        p2_ms = float(np.mean([a.elapsed_time(b) for a, b in evp]))
+        phase2 = {"what": "tpc_merge_refit on the final tracks of the step: refit of every track's kept hits, matching "
+                          "across sector boundaries, one fit per merged track (DESIGN.md readings M1-M4)",
+                  "ms": p2_ms, "tracks_in": n_trk, "merged_tracks": int(c2[0]), "links": int(c2[1]),
+                  "failed_track_refits": int(c2[2]), "failed_chain_fits": int(c2[3]),
+                  "gpu_launches": trk.last_launch_count, "share_of_step_plus_phase2": p2_ms / (p2_ms + ms_step)}
+        del p2bufs
+
     # ---- end to end through the host-buffer entry point (tpc_pipeline_run) -------------------------------------------
     combine = lambda ms_, n_: sharding.combine_step(ms_, n_, device=dev)  # noqa: E731
     e2e = e2e_xyzw = e2e_yz = None
@@ -408,7 +430,7 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": launches,
             "e2e": e2e, "e2e_xyzw_f32": e2e_xyzw, "e2e_yz_f32": e2e_yz,
             "roofline": roof, "roofline_path_hbm": roof_path, "cpu_baseline": cpu,
-            "stage_ms": stage_ms, "single_window": single,
+            "stage_ms": stage_ms, "phase2_merge_refit": phase2, "single_window": single,
             "results": {"candidates": int(counts[1]), "tracklets": int(counts[2]), "tracks": int(counts[3]),
                         "track_hits": int(counts[4]), "error_flags": int(counts[5])},
             "physics_window0": phys,
@@ -432,7 +454,7 @@ def main():
                          "linear-scaling check of PAPER.md:33")
     ap.add_argument("--seed0", type=int, default=5001)
     ap.add_argument("--tune", default="", help='JSON dict of performance-only tracker parameters, e.g. {"grid_cells_y": 8}')
-    ap.add_argument("--skip", default="", help="comma list of optional sections to leave out: e2e,single,bridge,cpu")
+    ap.add_argument("--skip", default="", help="comma list of optional sections to leave out: e2e,phase2,single,bridge,cpu")
     args = ap.parse_args()
     global WORKLOAD
     WORKLOAD = args.workload
