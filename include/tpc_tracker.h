@@ -180,9 +180,9 @@ int tpc_set_work_counters(tpc_tracker_t* t, int32_t enable);
 /* Optional per-stage timing: when enabled, every tpc_track_sectors call records CUDA events on its stream around
    each stage (a ring of the last TPC_TIMING_RING calls).  tpc_stage_times_ms waits for the call `age` calls back
    (0 = the last one) and returns its milliseconds in out_ms[TPC_N_STAGES]
-   (order: bin, neighbours, clean, chains, fit, follow, select; fit = the candidates' own hits, follow = the
-   row-by-row extrapolation, both S5). */
-#define TPC_N_STAGES 7
+   (order: bin, neighbours, chains, fit, follow, select; chains = S3 cleaning fused with S4, fit = the candidates'
+   own hits, follow = the row-by-row extrapolation, both S5). */
+#define TPC_N_STAGES 6
 #define TPC_TIMING_RING 32
 int tpc_set_stage_timing(tpc_tracker_t* t, int32_t enable);
 int tpc_stage_times_ms(tpc_tracker_t* t, int32_t age, float* out_ms);

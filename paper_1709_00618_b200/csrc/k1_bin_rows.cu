@@ -34,7 +34,10 @@ __global__ void __launch_bounds__(kBinThreads, TPC_BIN_CTAS)
 bin_rows_kernel(const __grid_constant__ DevGeom g, const void* __restrict__ clusters,
                 const int32_t* __restrict__ row_offsets, float2* __restrict__ hit_yz, uint16_t* __restrict__ hit_idx,
                 uint16_t* __restrict__ hit_pos, uint16_t* __restrict__ bin_start, int64_t* __restrict__ counts) {
-    extern __shared__ __align__(16) uint32_t sm_hist[];  // [nzp] counts, then exclusive starts (cursors in pass 2)
+    // Cell counters are 16 bit, two per 32-bit word (a row holds <= 65,535 hits, so neither half can carry into the
+    // other): half the shared memory, half the zeroing and half the scan work of 32-bit counters, and the scanned
+    // words ARE the uint16 cell table that goes to global memory.
+    extern __shared__ __align__(16) uint32_t sm_hist[];  // [nzp / 2] packed counts, then exclusive starts (cursors)
     __shared__ uint32_t sm_warp[kBinThreads / 32];
     const int slab = blockIdx.x;
     const int inst = slab / g.R, r = slab - inst * g.R;
@@ -46,12 +49,12 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const void* __restrict__ clus
     }
     const float z0 = grid_z0(g, inst);
     const float y0 = g.row_y0[r], inv_sy = g.row_inv_sy[r];
-    const int nzp = g.nzp;  // multiple of 8
+    const int nw = g.nzp / 2;  // packed words; nzp % 16 == 0, so nw % 8 == 0
     uint4* hist4 = reinterpret_cast<uint4*>(sm_hist);
-    for (int b = threadIdx.x; b < nzp / 4; b += kBinThreads) hist4[b] = make_uint4(0u, 0u, 0u, 0u);
+    for (int b = threadIdx.x; b < nw / 4; b += kBinThreads) hist4[b] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
-    // pass 1: histogram.  Coalesced float4 loads, 16 B per thread; the cell ids stay in registers for pass 2
-    // when the row is short enough (two hits per thread), which is the normal case.
+    // pass 1: histogram.  Coalesced loads; the cell ids stay in registers for pass 2 when the row is short enough
+    // (two hits per thread), which is the normal case.
     constexpr int kKeep = 2;
     int key[kKeep];
     float2 yz[kKeep];
@@ -63,22 +66,25 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const void* __restrict__ clus
             const float2 c = load_yz<kIn>(clusters, base + i, z0);
             key[k] = zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny);
             yz[k] = c;
-            atomicAdd(&sm_hist[key[k]], 1u);
+            atomicAdd(&sm_hist[key[k] >> 1], (key[k] & 1) ? 0x10000u : 1u);
         }
     }
     for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {
         const float2 c = load_yz<kIn>(clusters, base + i, z0);
-        atomicAdd(&sm_hist[zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny)], 1u);
+        const int kk = zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny);
+        atomicAdd(&sm_hist[kk >> 1], (kk & 1) ? 0x10000u : 1u);
     }
     __syncthreads();
-    // exclusive scan of nzp entries: a contiguous chunk of 8-entry groups per thread, warp scan of the chunk sums
-    const int groups = nzp / 8;
+    // exclusive scan of the nzp counters: a contiguous chunk of 4-word groups (8 cells) per thread, warp scan of the
+    // chunk sums
+    const int groups = nw / 4;
     const int per = (groups + kBinThreads - 1) / kBinThreads;
     const int glo = min(threadIdx.x * per, groups), ghi = min(glo + per, groups);
     uint32_t sum = 0;
     for (int q = glo; q < ghi; q++) {
-        const uint4 a = hist4[2 * q], b = hist4[2 * q + 1];
-        sum += a.x + a.y + a.z + a.w + b.x + b.y + b.z + b.w;
+        const uint4 a = hist4[q];
+        const uint32_t t = a.x + a.y + a.z + a.w;  // sums of the low and of the high halves, each <= 65,535
+        sum += (t & 0xffffu) + (t >> 16);
     }
     uint32_t incl = sum;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -91,22 +97,25 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const void* __restrict__ clus
     __syncthreads();
     uint32_t off = incl - sum;
     for (int k = 0; k < wid; k++) off += sm_warp[k];
-    uint4* tbl4 = reinterpret_cast<uint4*>(bin_start + (size_t)slab * nzp);  // 16-B aligned: nzp % 8 == 0
+    uint4* tbl4 = reinterpret_cast<uint4*>(bin_start + (size_t)slab * g.nzp);  // 16-B aligned: nzp % 8 == 0
     for (int q = glo; q < ghi; q++) {
-        uint4 a = hist4[2 * q], b = hist4[2 * q + 1];
-        uint32_t s0 = off, s1 = s0 + a.x, s2 = s1 + a.y, s3 = s2 + a.z, s4 = s3 + a.w, s5 = s4 + b.x, s6 = s5 + b.y,
-                 s7 = s6 + b.z;
-        off = s7 + b.w;
-        hist4[2 * q] = make_uint4(s0, s1, s2, s3);
-        hist4[2 * q + 1] = make_uint4(s4, s5, s6, s7);
-        tbl4[q] = make_uint4(s0 | (s1 << 16), s2 | (s3 << 16), s4 | (s5 << 16), s6 | (s7 << 16));
+        const uint4 a = hist4[q];
+        uint4 o;
+        uint32_t lo, hi;
+        lo = a.x & 0xffffu; hi = a.x >> 16; o.x = off | ((off + lo) << 16); off += lo + hi;
+        lo = a.y & 0xffffu; hi = a.y >> 16; o.y = off | ((off + lo) << 16); off += lo + hi;
+        lo = a.z & 0xffffu; hi = a.z >> 16; o.z = off | ((off + lo) << 16); off += lo + hi;
+        lo = a.w & 0xffffu; hi = a.w >> 16; o.w = off | ((off + lo) << 16); off += lo + hi;
+        hist4[q] = o;
+        tbl4[q] = o;
     }
     __syncthreads();
-    // pass 2: scatter
+    // pass 2: scatter (the packed start of a cell is its cursor: atomicAdd returns the word before the increment)
 #pragma unroll
     for (int k = 0; k < kKeep; k++) {
         if (key[k] >= 0) {
-            const uint32_t pos = atomicAdd(&sm_hist[key[k]], 1u);
+            const uint32_t w = atomicAdd(&sm_hist[key[k] >> 1], (key[k] & 1) ? 0x10000u : 1u);
+            const uint32_t pos = (key[k] & 1) ? (w >> 16) : (w & 0xffffu);
             hit_yz[base + pos] = yz[k];
             hit_idx[base + pos] = (uint16_t)(threadIdx.x + k * kBinThreads);
             hit_pos[base + threadIdx.x + k * kBinThreads] = (uint16_t)pos;  // inverse permutation, coalesced
@@ -114,7 +123,9 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const void* __restrict__ clus
     }
     for (int i = threadIdx.x + kKeep * kBinThreads; i < n; i += kBinThreads) {  // long rows: from L1/L2 this time
         const float2 c = load_yz<kIn>(clusters, base + i, z0);
-        const uint32_t pos = atomicAdd(&sm_hist[zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny)], 1u);
+        const int kk = zbin(c.y, z0, g.inv_cz, g.nz) * g.ny + ybin(c.x, y0, inv_sy, g.ny);
+        const uint32_t w = atomicAdd(&sm_hist[kk >> 1], (kk & 1) ? 0x10000u : 1u);
+        const uint32_t pos = (kk & 1) ? (w >> 16) : (w & 0xffffu);
         hit_yz[base + pos] = c;
         hit_idx[base + pos] = (uint16_t)i;
         hit_pos[base + i] = (uint16_t)pos;
@@ -124,7 +135,7 @@ bin_rows_kernel(const __grid_constant__ DevGeom g, const void* __restrict__ clus
 int launch_bin_rows(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s) {
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
-    const size_t smem = (size_t)g.nzp * sizeof(uint32_t);
+    const size_t smem = (size_t)g.nzp * sizeof(uint16_t);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
         cudaFuncSetAttribute(bin_rows_kernel<kInXYZW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

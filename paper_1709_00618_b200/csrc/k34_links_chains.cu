@@ -1,4 +1,4 @@
-// S3: neighbour cleaning (keep only mutual links; BASELINE.json north_star) and
+// S3: neighbour cleaning (keep only mutual links; BASELINE.json north_star), fused into the first pass of
 // S4: start hits + concatenation of links into track candidates "of usually 4 to 10 TPC hits" (Fig. 1b).
 // All integer work; results are unique, so they must equal the oracle bit for bit.
 //
@@ -9,29 +9,23 @@
 
 namespace tpc {
 
-constexpr int kCleanThreads = 256;
 constexpr int kChainThreads = 128;
 constexpr int kScanThreads = 1024;
 
-// S3 + per-hit initialisation of the selector's claim word (fused here because this kernel streams over all hits).
-__global__ void __launch_bounds__(kCleanThreads)
-clean_links_kernel(int64_t n, const int32_t* __restrict__ up_raw, const int32_t* __restrict__ dn_raw,
-                   int32_t* __restrict__ up, int32_t* __restrict__ dn, uint32_t* __restrict__ claim) {
-    const int64_t h = (int64_t)blockIdx.x * kCleanThreads + threadIdx.x;
-    if (h >= n) return;
-    const int32_t u = up_raw[h], d = dn_raw[h];
-    up[h] = (u >= 0 && __ldg(&dn_raw[u]) == (int32_t)h) ? u : -1;
-    dn[h] = (d >= 0 && __ldg(&up_raw[d]) == (int32_t)h) ? d : -1;
-    claim[h] = 0u;
-}
-
-// S4 pass 1: per-hit flags (bit0 start hit, bit1 candidate) and per-slab counts.  One WARP per (instance,row) slab:
-// a slab is ~200 hits and a short chain of dependent loads, so what bounds these passes is how many slabs an SM has
-// in flight -- 64 with a warp each against 16 with a 128-thread CTA each -- and a warp needs no barrier.
+// S3 + S4 pass 1, fused (SURVEY.md 8(d) budgets S3 with its neighbours; the raw links were written, read
+// back, cleaned, written again and read a third time).  Per hit: the cleaned links are computed on the fly from the
+// raw arrays -- cu = up_raw[h] if dn_raw[up_raw[h]] == h, cd likewise (reading S3: mutual links only) -- only the
+// cleaned up-link is materialised (the S5 fit kernel walks it), plus the flags (bit0 start hit, bit1 candidate), the
+// per-slab counts and the selector's claim word.  A start hit's chain is walked on the raw arrays with the same
+// mutuality test, because the cleaned links of later rows may not have been written yet by their warps.
+// One WARP per (instance,row) slab: a slab is ~200 hits and a short chain of dependent loads, so what bounds this
+// pass is how many slabs an SM has in flight -- 64 with a warp each against 16 with a 128-thread CTA each -- and a
+// warp needs no barrier.
 __global__ void __launch_bounds__(kChainThreads)
-chain_flags_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
-                   const int32_t* __restrict__ up, const int32_t* __restrict__ dn, uint8_t* __restrict__ flags,
-                   int2* __restrict__ slab_part, int n_slabs) {
+clean_flags_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
+                   const int32_t* __restrict__ up_raw, const int32_t* __restrict__ dn_raw, int32_t* __restrict__ up,
+                   uint32_t* __restrict__ claim, uint8_t* __restrict__ flags, int2* __restrict__ slab_part,
+                   int n_slabs) {
     const int slab = blockIdx.x * (kChainThreads / 32) + (threadIdx.x >> 5);
     if (slab >= n_slabs) return;
     const int lane = threadIdx.x & 31;
@@ -39,12 +33,22 @@ chain_flags_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict_
     int ns = 0, nc = 0;
     for (int i = lane; i < n; i += 32) {
         const int h = base + i;
+        const int32_t u = up_raw[h], d = dn_raw[h];
+        const int32_t cu = (u >= 0 && __ldg(&dn_raw[u]) == h) ? u : -1;
+        const bool has_cd = d >= 0 && __ldg(&up_raw[d]) == h;
+        up[h] = cu;
+        claim[h] = 0u;
         uint8_t f = 0;
-        int x = up[h];
-        if (x >= 0 && dn[h] < 0) {
+        if (cu >= 0 && !has_cd) {
             f = 1;
-            int len = 2;  // h and x
-            while (len < g.cand_min && (x = __ldg(&up[x])) >= 0) len++;
+            int len = 2;  // h and cu
+            int x = cu;
+            while (len < g.cand_min) {
+                const int nx = __ldg(&up_raw[x]);
+                if (nx < 0 || __ldg(&dn_raw[nx]) != x) { x = -1; break; }
+                x = nx;
+                len++;
+            }
             if (x >= 0 && len >= g.cand_min) f = 3;
         }
         flags[h] = f;
@@ -152,9 +156,11 @@ chain_write_kernel(const int32_t* __restrict__ row_offsets, const uint16_t* __re
 
 // Parity/debug export of one link array: sorted space -> input-order positions and values.  dir = +1 / -1 is the
 // row offset of the link targets.
+// `mutual` != NULL: the link is kept only if mutual[link] points back (the cleaned link computed on the fly, reading S3).
 __global__ void __launch_bounds__(kChainThreads)
 export_links_kernel(const int32_t* __restrict__ row_offsets, const uint16_t* __restrict__ hit_idx,
-                    const int32_t* __restrict__ link, int dir, int n_slabs, int32_t* __restrict__ out) {
+                    const int32_t* __restrict__ link, const int32_t* __restrict__ mutual, int dir, int n_slabs,
+                    int32_t* __restrict__ out) {
     const int slab = blockIdx.x;
     const int base = row_offsets[slab], n_all = row_offsets[slab + 1] - base;
     const int n = min(n_all, 65535);
@@ -163,18 +169,12 @@ export_links_kernel(const int32_t* __restrict__ row_offsets, const uint16_t* __r
     const int t1 = min(max(slab + dir, 0), n_slabs - 1), t2 = min(max(slab + 2 * dir, 0), n_slabs - 1);
     const int b1 = row_offsets[t1], b2 = row_offsets[t2], e1 = row_offsets[t1 + 1];
     for (int i = threadIdx.x; i < n; i += kChainThreads) {
-        const int32_t v = link[base + i];
+        int32_t v = link[base + i];
+        if (mutual && v >= 0 && mutual[v] != base + i) v = -1;
         const int tbase = (v >= b1 && v < e1) ? b1 : b2;
         out[base + hit_idx[base + i]] = v < 0 ? -1 : tbase + (int32_t)hit_idx[v];
     }
     for (int i = n + threadIdx.x; i < n_all; i += kChainThreads) out[base + i] = -1;
-}
-
-int launch_clean(const DevGeom&, const Workspace& w, const Problem& p, cudaStream_t s) {
-    if (p.n_clusters == 0) return 0;
-    clean_links_kernel<<<div_up(p.n_clusters, kCleanThreads), kCleanThreads, 0, s>>>(p.n_clusters, w.up_raw, w.dn_raw,
-                                                                                    w.up, w.dn, w.claim);
-    return 1;
 }
 
 // Two-level scan for long inputs (the per-slab counts: ~570 k entries at 100 windows, where one CTA takes 0.43 ms):
@@ -257,18 +257,19 @@ int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const 
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
     const int grid = div_up(slabs, kChainThreads / 32);
-    chain_flags_kernel<<<grid, kChainThreads, 0, s>>>(g, p.row_offsets, w.up, w.dn, w.flags, w.slab_part, slabs);
+    clean_flags_kernel<<<grid, kChainThreads, 0, s>>>(g, p.row_offsets, w.up_raw, w.dn_raw, w.up, w.claim, w.flags,
+                                                      w.slab_part, slabs);
     const int scans = launch_scan_int2_long(w.slab_part, slabs, w.scan_tmp, w.counts, 0, 1, s);
     chain_write_kernel<<<grid, kChainThreads, 0, s>>>(p.row_offsets, w.hit_pos, w.flags, w.slab_part, u.start_hits,
                                                       u.start_cap, w.cand_start, w.cand_slab, w.Cmax, slabs);
     return 2 + scans;
 }
 
-int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link, int dir,
-                        int32_t* out, cudaStream_t s) {
+int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link,
+                        const int32_t* mutual, int dir, int32_t* out, cudaStream_t s) {
     const int slabs = p.n_inst * g.R;
     if (slabs == 0 || !out) return 0;
-    export_links_kernel<<<slabs, kChainThreads, 0, s>>>(p.row_offsets, w.hit_idx, link, dir, slabs, out);
+    export_links_kernel<<<slabs, kChainThreads, 0, s>>>(p.row_offsets, w.hit_idx, link, mutual, dir, slabs, out);
     return 1;
 }
 

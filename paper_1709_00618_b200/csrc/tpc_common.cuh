@@ -60,8 +60,7 @@ struct Workspace {
     // (row start + position in the sorted row); the user-facing outputs are translated back through hit_idx.
     int32_t* up_raw;      // [N] S2 links
     int32_t* dn_raw;
-    int32_t* up;          // cleaned
-    int32_t* dn;
+    int32_t* up;          // [N] cleaned up-links (S3; the cleaned down-links are never materialised)
     uint32_t* claim;      // [N] S6 best claiming weight
     uint8_t* flags;       // [N] bit0 start hit, bit1 candidate
     int2* scan_tmp;       // [S*R / 4096 + 2] tile totals of the two-level scan over slab_part
@@ -126,7 +125,6 @@ __device__ __forceinline__ float grid_z0(const DevGeom& g, int inst) {
 // ---- launchers (one per stage; each returns the number of kernels it enqueued) ----
 int launch_bin_rows(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s);
 int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s);
-int launch_clean(const DevGeom& g, const Workspace& w, const Problem& p, cudaStream_t s);
 struct ChainOut {  // optional user-facing S4 outputs (NULL = skip)
     int32_t* start_hits;
     int64_t start_cap;
@@ -138,8 +136,9 @@ int launch_chains(const DevGeom& g, const Workspace& w, const Problem& p, const 
 void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m_cap, int64_t m_host, int64_t* counts,
                       int c0, int c1, cudaStream_t s);
 // parity/debug: a link array of the workspace (sorted space) as input-order indices; dir = row offset of the targets
-int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link, int dir,
-                        int32_t* out, cudaStream_t s);
+// `mutual`: NULL, or the opposite raw link array -- the link is exported only if it is mutual (cleaned on the fly)
+int launch_export_links(const DevGeom& g, const Workspace& w, const Problem& p, const int32_t* link,
+                        const int32_t* mutual, int dir, int32_t* out, cudaStream_t s);
 int launch_fit(const DevGeom& g, const Workspace& w, const Problem& p, const ChainOut& u, bool count_work, cudaStream_t s);
 int launch_follow(const DevGeom& g, const Workspace& w, const Problem& p, int n_sm, bool count_work, cudaStream_t s);
 

@@ -184,7 +184,6 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.up_raw = c.take<int32_t>(n);
     v.dn_raw = c.take<int32_t>(n);
     v.up = c.take<int32_t>(n);
-    v.dn = c.take<int32_t>(n);
     v.claim = c.take<uint32_t>(n);
     v.flags = c.take<uint8_t>(n);
     v.slab_part = c.take<int2>(slabs + 1);
@@ -312,27 +311,25 @@ int tpc_track_on(tpc_tracker* t, void* ws, size_t ws_bytes, cudaStream_t s, bool
     if (tm) cudaEventRecord(ev[1], s);
     launches += launch_neighbours(g, w, p, s);
     if (tm) cudaEventRecord(ev[2], s);
-    launches += launch_clean(g, w, p, s);
-    if (tm) cudaEventRecord(ev[3], s);
     ChainOut co{out->start_hits, out->start_hits ? out->start_capacity : 0, out->cand_hits, out->cand_n,
                 (out->cand_hits || out->cand_n) ? out->cand_capacity : 0};
     launches += launch_chains(g, w, p, co, s);
-    if (tm) cudaEventRecord(ev[4], s);
+    if (tm) cudaEventRecord(ev[3], s);
     launches += launch_fit(g, w, p, co, t->count_work, s);
-    if (tm) cudaEventRecord(ev[5], s);
+    if (tm) cudaEventRecord(ev[4], s);
     launches += launch_follow(g, w, p, t->n_sm, t->count_work, s);
-    if (tm) cudaEventRecord(ev[6], s);
+    if (tm) cudaEventRecord(ev[5], s);
     SelectOut so{out->trk_params, out->trk_cov, out->trk_chi2, out->trk_xref, out->trk_cand_id, out->trk_nhits,
                  out->trk_sector, out->trk_hit_offset, out->trk_hits, out->trk_capacity, out->trk_hits_capacity,
                  out->cluster_owner, out->counts};
     launches += launch_select(g, w, p, so, s);
-    if (tm) cudaEventRecord(ev[7], s);
+    if (tm) cudaEventRecord(ev[6], s);
     // optional parity/debug copies (device to device, same stream)
     if (n_clusters > 0) {
-        launches += launch_export_links(g, w, p, w.up_raw, +1, out->link_up_raw, s);
-        launches += launch_export_links(g, w, p, w.dn_raw, -1, out->link_dn_raw, s);
-        launches += launch_export_links(g, w, p, w.up, +1, out->link_up, s);
-        launches += launch_export_links(g, w, p, w.dn, -1, out->link_dn, s);
+        launches += launch_export_links(g, w, p, w.up_raw, nullptr, +1, out->link_up_raw, s);
+        launches += launch_export_links(g, w, p, w.dn_raw, nullptr, -1, out->link_dn_raw, s);
+        launches += launch_export_links(g, w, p, w.up, nullptr, +1, out->link_up, s);
+        launches += launch_export_links(g, w, p, w.dn_raw, w.up_raw, -1, out->link_dn, s);  // cleaned on the fly
         const int64_t tc = out->tl_capacity < w.Cmax ? out->tl_capacity : w.Cmax;
         if (tc > 0) {
             if (out->tl_params) cudaMemcpyAsync(out->tl_params, w.tl_par, sizeof(float) * 5 * tc, cudaMemcpyDeviceToDevice, s);

@@ -16,8 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libtpctrk.so")
 
 CAND_MAX_HITS = 10
 N_COUNTS = 16
-N_STAGES = 7
-STAGE_NAMES = ("bin", "neighbours", "clean", "chains", "fit", "follow", "select")
+N_STAGES = 6
+STAGE_NAMES = ("bin", "neighbours", "chains", "fit", "follow", "select")
 ERRORS = {-1: "TPC_ERR_ARG", -2: "TPC_ERR_GEOMETRY", -3: "TPC_ERR_WORKSPACE", -4: "TPC_ERR_CUDA",
           -5: "TPC_ERR_CAPACITY", -6: "TPC_ERR_INPUT"}
 
