@@ -417,16 +417,25 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
                 nd += in ? 1 : 0;
             }
             if (nd <= kNbList) {
+                bool tie = false;
                 for (int k = 0; k < (nd > 0 ? cu.nt : 0); k++) {
                     const int ja = k < cu.na ? cu.a0 + k : k + ushift;
                     const float2 u = up.yz[ja];
                     const bool uin = in_window(u, U.ylo, U.yhi, U.zlo, U.zhi);
                     const float t1 = wmul<kUniform>(wu, __fsub_rn(u.x, y)), t3 = wmul<kUniform>(wu, __fsub_rn(u.y, z));
+// strict minimum in visiting order; an exact tie of D with the best so far is only flagged (duplicated clusters, or
+// perfectly straight synthetic tracks): such a hit is searched again by the exact out-of-line path below, so the
+// common case pays no index comparison
 #define TPC_NB_PAIR(T2, T4, Q)                                                                                   \
     {                                                                                                            \
         const float ey = __fsub_rn(t1, T2), ez = __fsub_rn(t3, T4);                                              \
         const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));                                         \
-        consider(best, uin && nd > Q && D <= D2MAX, D, ja, (int)((ld >> (16 * Q)) & 0xffffull), up.idx, dn.idx); \
+        const bool adm = uin && nd > Q && D <= D2MAX;                                                            \
+        const bool lt = adm && D < best.D;                                                                       \
+        tie = tie || (adm && D == best.D);                                                                       \
+        best.D = lt ? D : best.D;                                                                                \
+        best.ju = lt ? ja : best.ju;                                                                             \
+        best.jd = lt ? (int)((ld >> (16 * Q)) & 0xffffull) : best.jd;                                            \
     }
                     TPC_NB_PAIR(t2a, t4a, 0)
                     TPC_NB_PAIR(t2b, t4b, 1)
@@ -435,6 +444,10 @@ __device__ __forceinline__ void search_row(const DevGeom& g, const RowView up, c
                         TPC_NB_PAIR(t2d, t4d, 3)
                     }
 #undef TPC_NB_PAIR
+                }
+                if (tie) {  // resolve by (D, local index of u, local index of d) exactly
+                    best = Best{kInf, -1, -1};
+                    search_dense(g, up, dn, y, z, U, W, wu, wd, best);
                 }
             } else {
                 // more than kNbList window hits in row r-1 (dense spots): pair every window hit of row r+1 with a
