@@ -16,7 +16,10 @@
 
 namespace tpc {
 
-constexpr int kNbThreads = 128;
+#ifndef TPC_NB_THREADS
+#define TPC_NB_THREADS 96  // measured: 64 -> 4.65, 96 -> 4.17, 128 -> 4.31, 192 -> 5.23, 256 -> 5.79 ms on the bench workload
+#endif
+constexpr int kNbThreads = TPC_NB_THREADS;
 constexpr int kNbStageHits = 1024;  // max hits of row r-1 plus row r+1 staged in shared memory (8 B each)
 constexpr int kNbStageTbl = 4096;   // max table entries per row staged in shared memory (2 B each, two rows)
 constexpr int kNbList = 4;          // window hits per neighbour row kept in registers; more -> exact slow path

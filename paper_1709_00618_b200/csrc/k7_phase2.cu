@@ -44,6 +44,7 @@ struct P2Args {
     int32_t* p2_next;
     int32_t* p2_prev;
     int2* p2_part;
+    int2* p2_chain;  // [Tmax / 2 + 1] (innermost segment, merged-track index) of every chain
     int64_t* p2_counts;
     int32_t n_inst;
 };
@@ -185,31 +186,33 @@ inst_first_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2A
     a.p2_first[i] = (int32_t)lo;
 }
 
+// One WARP per track A: the lanes scan the tracks of a neighbouring sector instance 32 at a time (coalesced reads of
+// their rows), and only the few that pass the integer pre-filter pay for the extrapolation.
 __global__ void __launch_bounds__(kP2Threads)
 match_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Args a) {
     const int64_t n_trk = min(a.counts[3], a.Tmax);
-    const int64_t ta = (int64_t)blockIdx.x * kP2Threads + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const int64_t ta = (int64_t)blockIdx.x * (kP2Threads / 32) + (threadIdx.x >> 5);
     if (ta >= n_trk) return;
     const int4 ia = a.p2_info[ta];
     const int la = ia.z;
-    if (ia.w < 1 || la >= g.R - 1) return;  // reaches the last pad row: nothing can continue it
+    if (ia.w < 1 || la >= g.R - 1) return;  // reaches the last pad row: nothing can continue it (warp-uniform)
     const int inst = track_inst(g, a, ta);
     const int window = (inst + g.inst_phase) / g.spe, sec = (inst + g.inst_phase) % g.spe;
     const int side = sec >= g.spe_half ? 1 : 0, phi = sec % g.spe_half;
     const float2 ha = a.p2_last[ta];
     const float xa = g.row_x[la];
     float best_d2 = __int_as_float(0x7f800000);
-    int best_b = -1;
+    int best_b = 0x7fffffff;
     // the two neighbouring sectors of the same side and window.  Rotation from B's frame into A's: by -2h when B is
-    // the next sector in azimuth (dir = +1), by +2h when it is the previous one.  dir = +1 first: its instance (and
-    // with it its track indices) is lower or higher than the other's depending on the wrap, so the lower index on an
-    // exact tie of d2 is kept explicitly.
+    // the next sector in azimuth (dir = +1), by +2h when it is the previous one.
     for (int dir = -1; dir <= 1; dir += 2) {
         const int phi_b = (phi + dir + g.spe_half) % g.spe_half;
         const int inst_b = window * g.spe + side * g.spe_half + phi_b - g.inst_phase;
         if (inst_b < 0 || inst_b >= a.n_inst) continue;  // the neighbour is not part of this call (chunked jobs)
         const float sa = dir > 0 ? -g.sin_2h : g.sin_2h;
-        for (int tb = a.p2_first[inst_b]; tb < a.p2_first[inst_b + 1]; tb++) {
+        const int t_end = a.p2_first[inst_b + 1];
+        for (int tb = a.p2_first[inst_b] + lane; tb < t_end; tb += 32) {
             const int4 ib = a.p2_info[tb];
             if (!(ib.x && ib.y > la && ib.y - la <= kMergeGap)) continue;
             KfState st;
@@ -229,7 +232,14 @@ match_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Args a
             atomicMin(&a.p2_best_prev[tb], ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned long long)ta);
         }
     }
-    a.p2_best_next[ta] = best_b;
+    // nearest over the lanes; an exact tie of d2 goes to the lower track index
+    unsigned long long key = ((unsigned long long)__float_as_uint(best_d2) << 32) | (unsigned)best_b;
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
+        key = other < key ? other : key;
+    }
+    if (lane == 0) a.p2_best_next[ta] = (unsigned)(key & 0xffffffffull) == 0x7fffffffu ? -1 : (int)(key & 0xffffffffull);
 }
 
 __global__ void __launch_bounds__(kP2Threads)
@@ -245,37 +255,46 @@ link_kernel(const __grid_constant__ P2Args a) {
     }
 }
 
-// heads (tracks without a predecessor) per block of 256 tracks
+// heads (tracks without a predecessor) and chain heads (heads with a successor) per block of 256 tracks
 __global__ void __launch_bounds__(256)
 heads_kernel(const __grid_constant__ P2Args a) {
-    __shared__ int s_cnt;
+    __shared__ int s_cnt[2];
     const int64_t n_trk = min(a.counts[3], a.Tmax);
     for (int64_t blk = blockIdx.x; blk * 256 < n_trk; blk += gridDim.x) {
-        if (threadIdx.x == 0) s_cnt = 0;
+        if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0;
         __syncthreads();
         const int64_t t = blk * 256 + threadIdx.x;
         const int head = (t < n_trk && a.p2_prev[t] < 0) ? 1 : 0;
-        const int n = __reduce_add_sync(0xffffffffu, head);
-        if ((threadIdx.x & 31) == 0 && n) atomicAdd(&s_cnt, n);
+        const int chain = (head && a.p2_next[t] >= 0) ? 1 : 0;
+        const int n = __reduce_add_sync(0xffffffffu, head), nc = __reduce_add_sync(0xffffffffu, chain);
+        if ((threadIdx.x & 31) == 0) {
+            if (n) atomicAdd(&s_cnt[0], n);
+            if (nc) atomicAdd(&s_cnt[1], nc);
+        }
         __syncthreads();
-        if (threadIdx.x == 0) a.p2_part[blk] = make_int2(s_cnt, 0);
+        if (threadIdx.x == 0) a.p2_part[blk] = make_int2(s_cnt[0], s_cnt[1]);
         __syncthreads();
     }
 }
 
+// Per-track outputs, the merged-track records of single segments, and the list of chains (merged tracks of two or
+// more segments) for chain_fit_kernel; merged tracks are numbered in ascending innermost segment.
 __global__ void __launch_bounds__(256)
-chain_fit_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Args a, const Phase2Out o) {
-    __shared__ int s_warp[8];
+merged_out_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Args a, const Phase2Out o) {
+    __shared__ int2 s_warp[8];
     const int64_t n_trk = min(a.counts[3], a.Tmax);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     for (int64_t blk = blockIdx.x; blk * 256 < n_trk; blk += gridDim.x) {
         const int64_t t = blk * 256 + threadIdx.x;
         const bool head = t < n_trk && a.p2_prev[t] < 0;
-        const unsigned hm = __ballot_sync(0xffffffffu, head);
-        if (lane == 0) s_warp[wid] = __popc(hm);
+        const bool chain = head && a.p2_next[t] >= 0;
+        const unsigned hm = __ballot_sync(0xffffffffu, head), cm = __ballot_sync(0xffffffffu, chain);
+        if (lane == 0) s_warp[wid] = make_int2(__popc(hm), __popc(cm));
         __syncthreads();
-        int64_t m = a.p2_part[blk].x + __popc(hm & ((1u << lane) - 1u));
-        for (int k = 0; k < wid; k++) m += s_warp[k];
+        const int2 part = a.p2_part[blk];
+        int64_t m = part.x + __popc(hm & ((1u << lane) - 1u));
+        int64_t e = part.y + __popc(cm & ((1u << lane) - 1u));
+        for (int k = 0; k < wid; k++) { m += s_warp[k].x; e += s_warp[k].y; }
         __syncthreads();
         if (t < n_trk) {  // per-track outputs
             if (o.seg_next) o.seg_next[t] = a.p2_next[t];
@@ -290,26 +309,39 @@ chain_fit_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Ar
                 for (int q = 0; q < 15; q++) o.seg_cov[t * 15 + q] = a.p2_cov[t * 15 + q];
         }
         if (!head || m >= o.mtrk_capacity) continue;
+        if (o.mtrk_first) o.mtrk_first[m] = (int32_t)t;
+        if (chain) {  // fitted by chain_fit_kernel, one dense thread per chain
+            a.p2_chain[e] = make_int2((int)t, (int)m);
+            continue;
+        }
+        // not merged: the refit of the track alone
+        const int4 info = a.p2_info[t];
+        if (o.mtrk_nseg) o.mtrk_nseg[m] = 1;
+        if (o.mtrk_nhits) o.mtrk_nhits[m] = info.x ? info.w : 0;
+        if (o.mtrk_ok) o.mtrk_ok[m] = info.x;
+        if (o.mtrk_chi2) o.mtrk_chi2[m] = a.p2_chi2[t];
+        if (o.mtrk_params)
+#pragma unroll
+            for (int q = 0; q < 5; q++) o.mtrk_params[m * 5 + q] = a.p2_par[t * 5 + q];
+        if (o.mtrk_cov)
+#pragma unroll
+            for (int q = 0; q < 15; q++) o.mtrk_cov[m * 15 + q] = a.p2_cov[t * 15 + q];
+        if (!info.x) atomicAdd((unsigned long long*)&a.p2_counts[3], 1ull);
+    }
+}
+
+// Reading M4: one thread per chain; seed on the outermost segment, filter inward through the chain, rotating the
+// state and covariance at every sector boundary.
+__global__ void __launch_bounds__(kP2Threads)
+chain_fit_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Args a, const Phase2Out o) {
+    const int64_t n_chain = a.p2_counts[4];
+    for (int64_t e = (int64_t)blockIdx.x * kP2Threads + threadIdx.x; e < n_chain; e += (int64_t)gridDim.x * kP2Threads) {
+        const int2 ent = a.p2_chain[e];
+        const int64_t t = ent.x, m = ent.y;
+        if (m >= o.mtrk_capacity) continue;
         int nseg = 1;
         int64_t tail = t;
         while (a.p2_next[tail] >= 0 && nseg < 64) { tail = a.p2_next[tail]; nseg++; }
-        if (o.mtrk_first) o.mtrk_first[m] = (int32_t)t;
-        if (o.mtrk_nseg) o.mtrk_nseg[m] = nseg;
-        if (nseg == 1) {  // not merged: the refit of the track alone
-            const int4 info = a.p2_info[t];
-            if (o.mtrk_nhits) o.mtrk_nhits[m] = info.x ? info.w : 0;
-            if (o.mtrk_ok) o.mtrk_ok[m] = info.x;
-            if (o.mtrk_chi2) o.mtrk_chi2[m] = a.p2_chi2[t];
-            if (o.mtrk_params)
-#pragma unroll
-                for (int q = 0; q < 5; q++) o.mtrk_params[m * 5 + q] = a.p2_par[t * 5 + q];
-            if (o.mtrk_cov)
-#pragma unroll
-                for (int q = 0; q < 15; q++) o.mtrk_cov[m * 15 + q] = a.p2_cov[t * 15 + q];
-            if (!info.x) atomicAdd((unsigned long long*)&a.p2_counts[3], 1ull);
-            continue;
-        }
-        // reading M4: seed on the outermost segment, filter inward through the chain
         KfState st = {};
         float x = 0.0f, yref = 0.0f, zref = 0.0f, chi2 = 0.0f;
         int r_first = 0, r_last = 0, n = 0, nhits = 0;
@@ -334,6 +366,7 @@ chain_fit_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Ar
                 ok = filter_inward(g, a, h, st, x, yref, zref, chi2, nhits);
             }
         }
+        if (o.mtrk_nseg) o.mtrk_nseg[m] = nseg;
         if (o.mtrk_nhits) o.mtrk_nhits[m] = ok ? nhits : 0;
         if (o.mtrk_ok) o.mtrk_ok[m] = ok ? 1 : 0;
         if (o.mtrk_chi2) o.mtrk_chi2[m] = ok ? chi2 : 0.0f;
@@ -358,25 +391,27 @@ void launch_scan_int2(int2* part, const int64_t* m_dev, int64_t m_div, int64_t m
                       int c0, int c1, cudaStream_t s);
 
 int launch_phase2(const DevGeom& g, const Workspace& w, const Problem& p, const Phase2Out& o, cudaStream_t s) {
-    cudaMemsetAsync(w.p2_counts, 0, sizeof(int64_t) * 4, s);
+    cudaMemsetAsync(w.p2_counts, 0, sizeof(int64_t) * 8, s);
     int launches = 0;
     if (p.n_clusters > 0) {
         const P2Args a{p.row_offsets, w.hit_yz,     w.cand_slab,    w.tl_rowhit,    w.tl_sel,  w.trk_cand, w.counts,
                        w.Tmax,        w.p2_par,     w.p2_cov,       w.p2_chi2,      w.p2_info, w.p2_last,  w.p2_first,
-                       w.p2_best_prev, w.p2_best_next, w.p2_next,   w.p2_prev,      w.p2_part, w.p2_counts, p.n_inst};
+                       w.p2_best_prev, w.p2_best_next, w.p2_next,   w.p2_prev,      w.p2_part, w.p2_chain, w.p2_counts, p.n_inst};
         // the track count lives on the device: grids are sized by its bound and bounded by it inside
         const int64_t tb = div_up(w.Tmax, kP2Threads);
         const int grid_t = (int)(tb < 148 * 64 ? tb : 148 * 64);
         refit_tracks_kernel<<<grid_t, kP2Threads, 0, s>>>(g, a);
         inst_first_kernel<<<div_up((int64_t)p.n_inst + 1, kP2Threads), kP2Threads, 0, s>>>(g, a);
-        match_kernel<<<(unsigned)tb, kP2Threads, 0, s>>>(g, a);
+        match_kernel<<<(unsigned)div_up(w.Tmax, kP2Threads / 32), kP2Threads, 0, s>>>(g, a);
         link_kernel<<<(unsigned)tb, kP2Threads, 0, s>>>(a);
         const int64_t hb = div_up(w.Tmax, 256);
         const int grid_h = (int)(hb < 148 * 16 ? hb : 148 * 16);
         heads_kernel<<<grid_h, 256, 0, s>>>(a);
-        launch_scan_int2(w.p2_part, w.counts + 3, 256, w.Tmax, 0, w.p2_counts, 0, 3 /* .y sums are 0 */, s);
-        chain_fit_kernel<<<grid_h, 256, 0, s>>>(g, a, o);
-        launches += 7;
+        launch_scan_int2(w.p2_part, w.counts + 3, 256, w.Tmax, 0, w.p2_counts, 0, 4, s);  // [0] heads, [4] chains
+        merged_out_kernel<<<grid_h, 256, 0, s>>>(g, a, o);
+        const int64_t cb = div_up(w.Tmax / 2 + 1, kP2Threads);
+        chain_fit_kernel<<<(int)(cb < 148 * 64 ? cb : 148 * 64), kP2Threads, 0, s>>>(g, a, o);
+        launches += 8;
     }
     p2_counts_kernel<<<1, 32, 0, s>>>(w.p2_counts, o.counts2);
     return launches + 1;

@@ -91,8 +91,9 @@ struct Workspace {
     int32_t* p2_best_next;             // [Tmax]
     int32_t* p2_next;     // [Tmax] links (reading M3)
     int32_t* p2_prev;
-    int2* p2_part;        // [Tmax/256 + 2] heads per block of 256 tracks, then exclusive scan (.x)
-    int64_t* p2_counts;   // [4] merged tracks, links, failed segment refits, failed chain fits
+    int2* p2_part;        // [Tmax/256 + 2] (heads, chain heads) per block of 256 tracks, then exclusive scan
+    int2* p2_chain;       // [Tmax/2 + 1] (innermost segment, merged-track index) of every chain
+    int64_t* p2_counts;   // [8] merged tracks, links, failed segment refits, failed chain fits, chains
 };
 
 struct Problem {

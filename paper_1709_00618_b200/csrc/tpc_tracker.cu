@@ -214,7 +214,8 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.p2_next = c.take<int32_t>(tmax);
     v.p2_prev = c.take<int32_t>(tmax);
     v.p2_part = c.take<int2>(tmax / 256 + 2);
-    v.p2_counts = c.take<int64_t>(4);
+    v.p2_chain = c.take<int2>(tmax / 2 + 1);
+    v.p2_counts = c.take<int64_t>(8);
     if (w) *w = v;
     return (c.off + 255) & ~(size_t)255;
 }
