@@ -1014,3 +1014,119 @@ int64_t orc_phase2(const orc_config *c, const float *clusters, const int32_t *ro
 
 int32_t orc_sizeof_fit(void) { return (int32_t)sizeof(orc_fit); }
 int32_t orc_sizeof_segment(void) { return (int32_t)sizeof(orc_segment); }
+
+/* ================================================================== TIME-COORDINATE TRACKING: vertex estimate
+ *
+ * PAPER.md:102 (Run 3, continuous read-out): "the tracking will run in time coordinate first to estimate the vertex
+ * and only then convert to spacial coordinates".  In continuous read-out the z of a cluster is
+ * its drift time, i.e. the true z plus an unknown offset common to all clusters of one collision (CFG:4 generates
+ * exactly that).  Phases 1 and 2 are translation invariant in z, so they run on the time-like coordinate unchanged;
+ * what is added here (readings T1-T3) is the step the paper names:
+ *  T1 every merged track is extrapolated along its helix to the point of closest approach to the beam line (the z
+ *     axis; a rotation between sector frames does not move it): with u = x c + y s, v = -x s + y c the position along
+ *     and across the direction (c = cos phi, s = sin phi) and kappa = cB q/pt,
+ *         ds = atan2(-kappa u, 1 + kappa v) / kappa   (-> -u / (1 + kappa v) for kappa -> 0),
+ *         z_v = z + (dz/ds) ds,   dca = (sqrt((kappa u)^2 + (1 + kappa v)^2) - 1) / kappa   (-> v).
+ *  T2 per event window (sectors_per_event instances) the z_v of the vertex-like tracks (ok, >= 30 hits, |dca| <= 3 cm)
+ *     are histogrammed in 0.5 cm bins over [z_lo - 50, z_hi + 50) of the geometry; a bin is a vertex seed iff the sum
+ *     of it and its two neighbours is >= 10 and is the maximum over the bins within +-4 (ties: the lowest bin wins);
+ *     the vertex position is the mean z_v of the vertex-like tracks within 1.5 cm of the seed bin's centre.
+ *  T3 every merged track (vertex-like or not) with a successful fit is assigned to the nearest vertex of its window
+ *     within 3 cm in z_v, else to none; z_v(vertex) is the offset that converts the z of the track and of its
+ *     clusters from the time-like to the spatial coordinate.
+ */
+void orc_track_vertex_z(const double p[5], double x, double cB, double *z_v, double *dca) {
+    const double s = p[2], c = sqrt(1.0 - s * s), kap = cB * p[4];
+    const double u = x * c + p[0] * s, v = -x * s + p[0] * c;
+    const double a = -kap * u, b = 1.0 + kap * v;
+    double ds, d;
+    if (fabs(kap) * (fabs(u) + fabs(v)) < 1e-9) {
+        ds = -u / b;
+        d = v;
+    } else {
+        ds = atan2(a, b) / kap;
+        d = (sqrt(a * a + b * b) - 1.0) / kap;
+    }
+    *z_v = p[1] + p[3] * ds;
+    *dca = d;
+}
+
+#define ORC_VTX_BIN 0.5
+#define ORC_VTX_MARGIN 50.0
+#define ORC_VTX_MAX_PER_WINDOW 64
+
+/* T1-T3 on the merged tracks of orc_phase2.  m_inst[m] = sector instance of the innermost segment.  Outputs per
+ * merged track: trk_zv, trk_dca, trk_vtx (global vertex index or -1); vertices (ascending window, then bin): vtx_z,
+ * vtx_window, vtx_ntracks (assigned tracks).  Returns the number of vertices (nothing is written beyond vtx_cap). */
+int64_t orc_vertices(const orc_config *c, int64_t n_merged, const orc_fit *m_fit, const int32_t *m_inst, double *trk_zv,
+                     double *trk_dca, int32_t *trk_vtx, double *vtx_z, int32_t *vtx_window, int32_t *vtx_ntracks,
+                     int64_t vtx_cap) {
+    const double cB = curv_const(c);
+    const int spe = c->sectors_per_event;
+    const double h_lo = (double)c->z_lo - ORC_VTX_MARGIN, h_hi = (double)c->z_hi + ORC_VTX_MARGIN;
+    /* the z < 0 side mirrors the range: use the union [-h, h] with h = max(|h_lo|, |h_hi|) */
+    const double h = fabs(h_lo) > fabs(h_hi) ? fabs(h_lo) : fabs(h_hi);
+    const int nb = (int)ceil(2.0 * h / ORC_VTX_BIN);
+    int32_t *hist = (int32_t *)malloc(sizeof(int32_t) * (size_t)nb);
+    char *like = (char *)malloc((size_t)(n_merged > 0 ? n_merged : 1));
+    for (int64_t m = 0; m < n_merged; m++) {
+        trk_zv[m] = trk_dca[m] = 0.0;
+        trk_vtx[m] = -1;
+        like[m] = 0;
+        if (!m_fit[m].ok) continue;
+        orc_track_vertex_z(m_fit[m].p, (double)c->row_x[m_fit[m].first_row], cB, &trk_zv[m], &trk_dca[m]);
+        like[m] = m_fit[m].nhits >= 30 && fabs(trk_dca[m]) <= 3.0;
+    }
+    int64_t nv = 0, w0 = 0;
+    while (w0 < n_merged) { /* merged tracks are in ascending innermost segment, hence in ascending window */
+        int64_t w1 = w0;
+        const int win = m_inst[w0] / spe;
+        while (w1 < n_merged && m_inst[w1] / spe == win) w1++;
+        memset(hist, 0, sizeof(int32_t) * (size_t)nb);
+        for (int64_t m = w0; m < w1; m++)
+            if (like[m]) {
+                const int b = (int)floor((trk_zv[m] + h) / ORC_VTX_BIN);
+                if (b >= 0 && b < nb) hist[b]++;
+            }
+        const int64_t nv0 = nv;
+        int n_here = 0;
+        for (int b = 0; b < nb && n_here < ORC_VTX_MAX_PER_WINDOW; b++) {
+#define SUM3(q) ((q) < 0 || (q) >= nb ? 0 : hist[q] + ((q) > 0 ? hist[(q) - 1] : 0) + ((q) + 1 < nb ? hist[(q) + 1] : 0))
+            const int s3 = SUM3(b);
+            if (s3 < 10) continue;
+            int is_max = 1;
+            for (int q = b - 4; q <= b + 4 && is_max; q++) {
+                if (q == b) continue;
+                const int o = SUM3(q);
+                if (o > s3 || (o == s3 && q < b)) is_max = 0;
+            }
+#undef SUM3
+            if (!is_max) continue;
+            const double zc = -h + (b + 0.5) * ORC_VTX_BIN;
+            double sum = 0.0;
+            int n = 0;
+            for (int64_t m = w0; m < w1; m++)
+                if (like[m] && fabs(trk_zv[m] - zc) <= 1.5) { sum += trk_zv[m]; n++; }
+            if (nv < vtx_cap) {
+                vtx_z[nv] = sum / n;
+                vtx_window[nv] = win;
+                vtx_ntracks[nv] = 0;
+            }
+            nv++;
+            n_here++;
+        }
+        for (int64_t m = w0; m < w1; m++) { /* T3 */
+            if (!m_fit[m].ok) continue;
+            double best = 0.0;
+            for (int64_t k = nv0; k < nv && k < vtx_cap; k++) {
+                const double d = fabs(trk_zv[m] - vtx_z[k]);
+                if (d <= 3.0 && (trk_vtx[m] < 0 || d < best)) { trk_vtx[m] = (int32_t)k; best = d; }
+            }
+            if (trk_vtx[m] >= 0) vtx_ntracks[trk_vtx[m]]++;
+        }
+        w0 = w1;
+    }
+    free(hist);
+    free(like);
+    return nv;
+}

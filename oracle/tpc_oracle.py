@@ -79,6 +79,7 @@ def lib():
         assert _lib.orc_sizeof_config() == C.sizeof(Config)
         _lib.orc_update.restype = C.c_double
         _lib.orc_phase2.restype = C.c_int64
+        _lib.orc_vertices.restype = C.c_int64
         assert _lib.orc_sizeof_fit() == FIT_DTYPE.itemsize and _lib.orc_sizeof_segment() == C.sizeof(Segment)
     return _lib
 
@@ -307,6 +308,33 @@ class Oracle:
                               C.c_void_p(seg_fit.ctypes.data), _p(nxt, C.c_int32), _p(prv, C.c_int32),
                               _p(mf, C.c_int32), C.c_void_p(m_fit.ctypes.data)) if nt else 0
         return Phase2Result(seg_fit[:nt], nxt[:nt], prv[:nt], mf[:nm], m_fit[:nm])
+
+
+    # ---- time-coordinate tracking: vertex estimate (readings T1-T3) -----------------------
+    def track_vertex_z(self, p, x):
+        """(z_v, dca) of a state p on the plane x: closest approach to the beam line (reading T1)."""
+        p = np.ascontiguousarray(p, np.float64)
+        zv, dca = C.c_double(), C.c_double()
+        lib().orc_track_vertex_z(_p(p, C.c_double), C.c_double(x), C.c_double(self.c_b), C.byref(zv), C.byref(dca))
+        return zv.value, dca.value
+
+    def vertices(self, p2: "Phase2Result", m_inst, vtx_cap=4096):
+        """Readings T1-T3 on the merged tracks of phase2().  m_inst: sector instance of every merged track's innermost
+        segment.  Returns dict(trk_zv, trk_dca, trk_vtx, vtx_z, vtx_window, vtx_ntracks)."""
+        nm = len(p2.m_first)
+        fit = np.ascontiguousarray(p2.m_fit)
+        inst = np.ascontiguousarray(m_inst, np.int32)
+        zv, dca = np.zeros(max(nm, 1)), np.zeros(max(nm, 1))
+        tv = np.full(max(nm, 1), -1, np.int32)
+        vz = np.zeros(vtx_cap)
+        vw = np.zeros(vtx_cap, np.int32)
+        vn = np.zeros(vtx_cap, np.int32)
+        nv = lib().orc_vertices(C.byref(self.cfg), C.c_int64(nm), C.c_void_p(fit.ctypes.data), _p(inst, C.c_int32),
+                                _p(zv, C.c_double), _p(dca, C.c_double), _p(tv, C.c_int32), _p(vz, C.c_double),
+                                _p(vw, C.c_int32), _p(vn, C.c_int32), C.c_int64(vtx_cap)) if nm else 0
+        assert nv <= vtx_cap
+        return dict(trk_zv=zv[:nm], trk_dca=dca[:nm], trk_vtx=tv[:nm], vtx_z=vz[:nv], vtx_window=vw[:nv],
+                    vtx_ntracks=vn[:nv])
 
 
 def unpack_cov(c15):
