@@ -284,6 +284,35 @@ typedef struct {
 
 int tpc_merge_refit(tpc_tracker_t* t, const tpc_phase2_output_t* out);
 
+/*
+ * Time-coordinate tracking: vertex estimate (continuous read-out: "the tracking will run in time
+ * coordinate first to estimate the vertex and only then convert to spacial coordinates").
+ * In continuous read-out the z of a cluster is a drift time: the true z plus an offset common to all clusters of one
+ * collision.  tpc_track_sectors and tpc_merge_refit are translation invariant in z and run on that time-like
+ * coordinate unchanged; this call adds the step the paper names (readings T1-T3):
+ *   T1  z_v, dca of every merged track: its closest approach to the beam line along the fitted helix
+ *   T2  per event window, vertices = local maxima (3-bin sums >= 10, +-4 bins, ties to the lower bin) of the 0.5 cm
+ *       histogram of z_v of the vertex-like tracks (fit ok, >= 30 hits, |dca| <= 3 cm); position = mean z_v of the
+ *       vertex-like tracks within 1.5 cm of the seed bin centre; at most TPC_VTX_MAX_PER_WINDOW per window
+ *   T3  every fitted track goes to the nearest vertex of its window within 3 cm, else to none; z_v of the vertex is
+ *       the offset that converts the track's (and its clusters') z from the time-like to the spatial coordinate.
+ * `merged` is the output struct of the preceding tpc_merge_refit call on this tracker (mtrk_first, mtrk_nhits,
+ * mtrk_ok, mtrk_params and counts2 required); the call reads its arrays and the workspace, same stream, asynchronous.
+ */
+#define TPC_VTX_MAX_PER_WINDOW 64
+typedef struct {
+    float* trk_zv;        /* [n_merged] z of the merged track at its closest approach to the beam line (time-like); required */
+    float* trk_dca;       /* [n_merged] signed distance of closest approach in the transverse plane [cm] */
+    int32_t* trk_vtx;     /* [n_merged] vertex index or -1 */
+    float* vtx_z;         /* [vtx_capacity] vertices in ascending window, then ascending z */
+    int32_t* vtx_window;  /* [vtx_capacity] event window (sector instance / sectors_per_event) */
+    int32_t* vtx_ntracks; /* [vtx_capacity] tracks assigned to the vertex */
+    int64_t vtx_capacity;
+    int64_t* counts3;     /* device [2]: vertices (required count), tracks assigned to a vertex */
+} tpc_vertex_output_t;
+
+int tpc_estimate_vertices(tpc_tracker_t* t, const tpc_phase2_output_t* merged, const tpc_vertex_output_t* out);
+
 const char* tpc_last_error(const tpc_tracker_t* t);
 
 #ifdef __cplusplus

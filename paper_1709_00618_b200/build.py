@@ -29,6 +29,7 @@ SOURCES = {
     "k5_follow.cu": [],
     "k6_select.cu": [],
     "k7_phase2.cu": [],
+    "k8_vertex.cu": [],
     "host_pipeline.cu": [],
 }
 

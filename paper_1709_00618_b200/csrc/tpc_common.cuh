@@ -36,6 +36,8 @@ struct DevGeom {
     float max_s, edge_margin, tan_half;
     int sel_min;
     float cos_2h, sin_2h;  // rotation between neighbouring sector frames: angle 2 * half_angle
+    int vtx_nb;            // bins of the per-window z_v histogram (0.5 cm over [-vtx_h, vtx_h))
+    float vtx_h;
     float sy2, sz2;
     float cB;       // curvature per (q/pt): kappa = cB * q/pt
     const float* row_x;  // device [R]
@@ -94,6 +96,15 @@ struct Workspace {
     int2* p2_part;        // [Tmax/256 + 2] (heads, chain heads) per block of 256 tracks, then exclusive scan
     int2* p2_chain;       // [Tmax/2 + 1] (innermost segment, merged-track index) of every chain
     int64_t* p2_counts;   // [8] merged tracks, links, failed segment refits, failed chain fits, chains
+    // vertex estimate (k8_vertex.cu); n_win = windows of the call, vtx_nb = histogram bins per window
+    int32_t* vz_hist;     // [n_win][vtx_nb] z_v histogram of the vertex-like tracks
+    int32_t* vz_seed;     // [n_win][64] seed bins, ascending
+    int32_t* vz_nseed;    // [n_win + 1] seeds per window, then exclusive scan (vertex index base)
+    long long* vz_sum;    // [n_win][64] fixed-point sums of z_v around the seed (deterministic integer atomics)
+    int32_t* vz_cnt;      // [n_win][64]
+    uint8_t* vz_like;     // [Tmax] 1 = vertex-like, 2 = fitted
+    int64_t* vz_counts;   // [2]
+    int32_t n_win;
 };
 
 struct Problem {
@@ -163,6 +174,16 @@ struct Phase2Out {  // mirrors tpc_phase2_output_t
     int64_t* counts2;
 };
 int launch_phase2(const DevGeom& g, const Workspace& w, const Problem& p, const Phase2Out& o, cudaStream_t s);
+struct VertexOut {  // mirrors tpc_vertex_output_t
+    float *trk_zv, *trk_dca;
+    int32_t* trk_vtx;
+    float* vtx_z;
+    int32_t *vtx_window, *vtx_ntracks;
+    int64_t vtx_capacity;
+    int64_t* counts3;
+};
+int launch_vertices(const DevGeom& g, const Workspace& w, const Problem& p, const Phase2Out& m, const VertexOut& o,
+                    cudaStream_t s);
 int launch_export_tracklets(const DevGeom& g, const Workspace& w, const Problem& p, int32_t* tl_hits, int32_t* tl_rows,
                             int64_t cap, cudaStream_t s);
 

@@ -96,6 +96,12 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     g.sel_min = dflt(p.sel_min_hits, 10);
     g.cos_2h = (float)std::cos(2.0 * (double)geom->half_angle_rad);
     g.sin_2h = (float)std::sin(2.0 * (double)geom->half_angle_rad);
+    {  // z_v histogram of the vertex estimate: 0.5 cm bins over [-h, h), h = the geometry's |z| range + 50 cm
+        const double lo = std::fabs((double)geom->z_lo - 50.0), hi = std::fabs((double)geom->z_hi + 50.0);
+        const double h = lo > hi ? lo : hi;
+        g.vtx_h = (float)h;
+        g.vtx_nb = (int)std::ceil(2.0 * h / 0.5);
+    }
     g.sy2 = (float)((double)geom->sigma_y * (double)geom->sigma_y);
     g.sz2 = (float)((double)geom->sigma_z * (double)geom->sigma_z);
     g.cB = (float)(-0.00299792458 * (double)bz);
@@ -216,6 +222,15 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.p2_part = c.take<int2>(tmax / 256 + 2);
     v.p2_chain = c.take<int2>(tmax / 2 + 1);
     v.p2_counts = c.take<int64_t>(8);
+    const size_t nwin = (size_t)(S > 0 ? S : 1) / (size_t)g.spe + 2;
+    v.n_win = (int32_t)nwin;
+    v.vz_hist = c.take<int32_t>(nwin * (size_t)g.vtx_nb);
+    v.vz_seed = c.take<int32_t>(nwin * TPC_VTX_MAX_PER_WINDOW);
+    v.vz_nseed = c.take<int32_t>(nwin + 1);
+    v.vz_sum = c.take<long long>(nwin * TPC_VTX_MAX_PER_WINDOW);
+    v.vz_cnt = c.take<int32_t>(nwin * TPC_VTX_MAX_PER_WINDOW);
+    v.vz_like = c.take<uint8_t>(tmax);
+    v.vz_counts = c.take<int64_t>(2);
     if (w) *w = v;
     return (c.off + 255) & ~(size_t)255;
 }
@@ -366,6 +381,28 @@ extern "C" int tpc_merge_refit(tpc_tracker_t* t, const tpc_phase2_output_t* out)
                       out->mtrk_first, out->mtrk_nseg, out->mtrk_nhits, out->mtrk_ok, out->mtrk_params, out->mtrk_cov,
                       out->mtrk_chi2, out->mtrk_capacity, out->counts2};
     t->last_launches = launch_phase2(g, w, p, o, t->last_stream);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, std::string("CUDA: ") + cudaGetErrorString(e));
+    return TPC_OK;
+}
+
+extern "C" int tpc_estimate_vertices(tpc_tracker_t* t, const tpc_phase2_output_t* m, const tpc_vertex_output_t* out) {
+    if (!t) return TPC_ERR_ARG;
+    if (!out || !out->counts3 || !out->trk_zv) return fail(t, TPC_ERR_ARG, "out, out->counts3 and out->trk_zv are required");
+    if (!m || !m->mtrk_first || !m->mtrk_nhits || !m->mtrk_ok || !m->mtrk_params || !m->counts2)
+        return fail(t, TPC_ERR_ARG, "merged: mtrk_first, mtrk_nhits, mtrk_ok, mtrk_params and counts2 are required");
+    if (!t->last_ws) return fail(t, TPC_ERR_ARG, "tpc_estimate_vertices needs preceding tpc_track_sectors + tpc_merge_refit calls");
+    Workspace w;
+    carve(t->g, t->last_ws, t->last_n_clusters, t->last_n_inst, &w);
+    DevGeom g = t->g;
+    g.inst_phase = t->last_first_inst % g.spe;
+    Problem p{nullptr, t->input_layout, t->last_row_offsets, t->last_n_inst, t->last_n_clusters};
+    const Phase2Out mo{m->seg_next, m->seg_prev, m->seg_ok, m->seg_params, m->seg_cov, m->seg_chi2, m->mtrk_first,
+                       m->mtrk_nseg, m->mtrk_nhits, m->mtrk_ok, m->mtrk_params, m->mtrk_cov, m->mtrk_chi2,
+                       m->mtrk_capacity, m->counts2};
+    const VertexOut vo{out->trk_zv, out->trk_dca, out->trk_vtx, out->vtx_z, out->vtx_window, out->vtx_ntracks,
+                       out->vtx_capacity, out->counts3};
+    t->last_launches = launch_vertices(g, w, p, mo, vo, t->last_stream);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, std::string("CUDA: ") + cudaGetErrorString(e));
     return TPC_OK;

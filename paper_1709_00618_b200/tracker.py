@@ -25,7 +25,8 @@ EXPORTS = ("tpc_tracker_create", "tpc_tracker_destroy", "tpc_workspace_bytes", "
            "tpc_track_sectors", "tpc_check_counts", "tpc_last_launch_count", "tpc_set_stage_timing",
            "tpc_stage_times_ms", "tpc_last_error", "tpc_track_sectors_host", "tpc_set_work_counters",
            "tpc_set_input_layout", "tpc_pipeline_create", "tpc_pipeline_destroy", "tpc_pipeline_run",
-           "tpc_merge_refit")
+           "tpc_merge_refit", "tpc_estimate_vertices")
+VTX_MAX_PER_WINDOW = 64
 INPUT_LAYOUTS = {"xyzw": 0, "yz": 1, "i16": 2}       # TPC_INPUT_*
 LAYOUT_BYTES = {"xyzw": 16, "yz": 8, "i16": 4}
 I16_Y_STEP, I16_Z_STEP = 1.0 / 256.0, 1.0 / 64.0     # TPC_I16_*_STEP
@@ -71,6 +72,12 @@ class Phase2Output(C.Structure):
                 ("mtrk_nhits", C.c_void_p), ("mtrk_ok", C.c_void_p), ("mtrk_params", C.c_void_p),
                 ("mtrk_cov", C.c_void_p), ("mtrk_chi2", C.c_void_p), ("mtrk_capacity", C.c_int64),
                 ("counts2", C.c_void_p)]
+
+
+class VertexOutput(C.Structure):
+    _fields_ = [("trk_zv", C.c_void_p), ("trk_dca", C.c_void_p), ("trk_vtx", C.c_void_p), ("vtx_z", C.c_void_p),
+                ("vtx_window", C.c_void_p), ("vtx_ntracks", C.c_void_p), ("vtx_capacity", C.c_int64),
+                ("counts3", C.c_void_p)]
 
 
 class Slot(C.Structure):
@@ -122,6 +129,7 @@ def load_library():
                                            C.POINTER(Slot), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.POINTER(HostOutput)]
     lib.tpc_merge_refit.argtypes = [C.c_void_p, C.POINTER(Phase2Output)]
+    lib.tpc_estimate_vertices.argtypes = [C.c_void_p, C.POINTER(Phase2Output), C.POINTER(VertexOutput)]
     lib.tpc_pipeline_create.argtypes = [C.c_void_p, C.POINTER(Slot), C.c_int32, C.POINTER(C.c_void_p)]
     lib.tpc_pipeline_destroy.argtypes = [C.c_void_p]
     lib.tpc_pipeline_destroy.restype = None
@@ -339,17 +347,48 @@ class Tracker:
         """tpc_merge_refit on the tracks of the last track call of this tracker; asynchronous."""
         self._check(self.lib.tpc_merge_refit(self._h, C.byref(out_struct)), "tpc_merge_refit")
 
-    def merge_refit(self, n_tracks):
-        """numpy results of phase 2 for the last track_sectors() call (its workspace is still attached)."""
+    def alloc_vertices(self, n_merged, n_windows):
+        """Device buffers for tpc_estimate_vertices (+ the ctypes struct)."""
+        t = self._torch
+        dev = self.device
+        n, nv = max(int(n_merged), 1), max(int(n_windows), 1) * VTX_MAX_PER_WINDOW
+        bufs = dict(trk_zv=t.empty(n, dtype=t.float32, device=dev), trk_dca=t.empty(n, dtype=t.float32, device=dev),
+                    trk_vtx=t.empty(n, dtype=t.int32, device=dev), vtx_z=t.empty(nv, dtype=t.float32, device=dev),
+                    vtx_window=t.empty(nv, dtype=t.int32, device=dev), vtx_ntracks=t.empty(nv, dtype=t.int32, device=dev),
+                    counts3=t.zeros(2, dtype=t.int64, device=dev))
+        o = VertexOutput()
+        for k, v in bufs.items():
+            setattr(o, k, v.data_ptr())
+        o.vtx_capacity = nv
+        return bufs, o
+
+    def estimate_vertices_device(self, phase2_struct, out_struct):
+        """tpc_estimate_vertices on the merged tracks of the last merge_refit call; asynchronous."""
+        self._check(self.lib.tpc_estimate_vertices(self._h, C.byref(phase2_struct), C.byref(out_struct)),
+                    "tpc_estimate_vertices")
+
+    def merge_refit(self, n_tracks, vertices_for_windows=0):
+        """numpy results of phase 2 for the last track_sectors() call (its workspace is still attached); with
+        vertices_for_windows = n also the vertex estimate (tpc_estimate_vertices) under the key "vertices"."""
         t = self._torch
         with t.cuda.device(self.device):
             bufs, o = self.alloc_phase2(n_tracks)
             self.merge_refit_device(o)
+            vb = None
+            if vertices_for_windows:
+                vb, vo = self.alloc_vertices(n_tracks, vertices_for_windows)
+                self.estimate_vertices_device(o, vo)
             t.cuda.synchronize(self.device)
         c2 = bufs["counts2"].cpu().numpy()
         nm = int(c2[0])
         res = {k: v.cpu().numpy()[:(nm if k.startswith("mtrk") else n_tracks)] for k, v in bufs.items() if k != "counts2"}
         res["counts2"] = c2
+        if vb is not None:
+            c3 = vb["counts3"].cpu().numpy()
+            nv = int(c3[0])
+            res["vertices"] = {k: v.cpu().numpy()[:(nv if k.startswith("vtx") else nm)] for k, v in vb.items()
+                               if k != "counts3"}
+            res["vertices"]["counts3"] = c3
         return res
 
     # ---- convenience: numpy in, numpy out (used by the parity tests) ----------------------------------------------

@@ -44,6 +44,7 @@ def test_binding_structs_match_header_sizes():
     assert C.sizeof(tracker.Slot) == 8 * 4 + C.sizeof(tracker.Output) + 16
     # tpc_phase2_output_t: 13 ptr + int64 + ptr
     assert C.sizeof(tracker.Phase2Output) == 8 * 15
+    assert C.sizeof(tracker.VertexOutput) == 8 * 8
     # tpc_host_output_t: 7 ptr + 2 int64 + 16 int64 + 4 int64 + 4 float
     assert C.sizeof(tracker.HostOutput) == 8 * (7 + 2 + 16 + 4) + 16
 

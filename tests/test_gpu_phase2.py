@@ -114,3 +114,43 @@ def test_phase2_requires_a_preceding_track_call():
     with pytest.raises(TpcError, match="ARG"):
         trk.merge_refit(10)
     trk.close()
+
+
+def test_vertex_estimate_against_oracle():
+    """tpc_estimate_vertices (readings T1-T3) on two CFG:4-like drift windows in one call: the same vertices as the
+    oracle (positions to 1e-3 cm: fp32 z_v and an integer fixed-point mean against fp64), z_v and dca of every merged
+    track within tolerance, >= 99.5 % identical track -> vertex assignments, and the vertices are the generated drift
+    offsets."""
+    from oracle.tpc_oracle import Oracle
+    from paper_1709_00618_b200 import Tracker
+    evs = [dg.drift_window(seed=4005 + i, mean_tracks=300.0, cap_tracks=800) for i in range(2)]
+    ev = dg.concat_events(evs)
+    orc = Oracle.for_event(ev)
+    o = orc.track(ev.clusters, ev.row_offsets, ev.n_inst)
+    trk = Tracker.for_event(ev)
+    g = trk.track_sectors(ev.clusters, ev.row_offsets, ev.n_inst, debug=True)
+    assert np.array_equal(g.trk_cand_id, o.trk_cand) and np.array_equal(g.trk_hits, o.trk_hits)
+    p = trk.merge_refit(g.n_tracks, vertices_for_windows=2)
+    trk.close()
+    q = orc.phase2(ev.clusters, ev.row_offsets, ev.n_inst, o)
+    assert np.array_equal(p["mtrk_first"], q.m_first) and np.array_equal(p["seg_next"], q.seg_next)
+    R = ev.n_rows
+    inst = np.searchsorted(ev.row_offsets[::R], o.cand_hits[o.trk_cand, 0], side="right") - 1
+    vo = orc.vertices(q, inst[q.m_first])
+    vg = p["vertices"]
+    both = p["mtrk_ok"].astype(bool) & q.m_fit["ok"].astype(bool)
+    # z_v and dca are the fitted state extrapolated over the 85..250 cm lever arm to the beam line: a deviation of the
+    # fp32 state inside the north_star parameter tolerance (1e-4 on sinPhi, dz/ds) moves them by up to ~0.02 cm
+    dz = np.abs(vg["trk_zv"][both] - vo["trk_zv"][both])
+    dd = np.abs(vg["trk_dca"][both] - vo["trk_dca"][both])
+    assert dz.max() <= 2e-2 and dd.max() <= 2e-2, (dz.max(), dd.max())
+    assert np.quantile(dz, 0.99) <= 2e-3 and np.quantile(dd, 0.99) <= 2e-3
+    assert len(vg["vtx_z"]) == len(vo["vtx_z"]) == int(vg["counts3"][0]) and len(vo["vtx_z"]) >= 8
+    assert np.array_equal(vg["vtx_window"], vo["vtx_window"])
+    assert np.all(np.abs(vg["vtx_z"] - vo["vtx_z"]) < 1e-3)
+    assert (vg["trk_vtx"] == vo["trk_vtx"]).mean() >= 0.995
+    assert np.abs(vg["vtx_ntracks"] - vo["vtx_ntracks"]).max() <= 2
+    assert int(vg["counts3"][1]) == int((vg["trk_vtx"] >= 0).sum()) == int(vg["vtx_ntracks"].sum())
+    shifts = np.concatenate([np.unique(e.truth["z_shift"]) for e in evs])
+    for z in vg["vtx_z"]:
+        assert np.abs(shifts - z).min() < 0.1
