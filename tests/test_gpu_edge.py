@@ -218,6 +218,24 @@ def test_many_nearly_empty_instances():
     assert g.n_tracks > 500
 
 
+def test_cell_table_index_beyond_32_bits():
+    """1,728 sector instances with the finest row grid (16,384 cells per row): instances x rows x cells = 4.5e9 > 2^32
+    table entries (9 GB), so the follower's table index must be 64 bit (it wrapped silently)."""
+    from paper_1709_00618_b200 import Tracker
+    evs = [dg.full_event(seed=2300 + i, n_prim=12, noise=0.0) for i in range(48)]
+    batch = dg.concat_events(evs)
+    assert batch.n_inst == 1728
+    o = run_oracle(batch)
+    trk = Tracker.for_event(batch, grid_cells_y=64, grid_cell_z=0.98)
+    assert trk.workspace_bytes(batch.n_clusters, batch.n_inst) > 8.5e9  # the table alone: 1728 * 159 * 16400 * 2 B
+    g = trk.track_sectors(batch.clusters, batch.row_offsets, batch.n_inst, debug=True)
+    trk.close()
+    assert_ca_bit_exact(g, o)
+    tr = tracklet_report(g, o)
+    assert tr["ok_mismatch"] == 0 and tr["shared_frac"] >= MIN_SHARED and tr["worst_param_excess"] <= 1.0, tr
+    assert np.array_equal(g.trk_cand_id, o.trk_cand) and g.n_tracks > 200
+
+
 def test_row_longer_than_16_bit_limit_is_flagged():
     """A pad row with more than 65,535 clusters cannot be indexed by the 16-bit local positions: the call flags it
     (counts[5] bit 0 -> TPC_ERR_INPUT from tpc_check_counts), stays inside its buffers and leaves the tracker usable."""
