@@ -284,3 +284,97 @@ def test_twenty_drift_windows_against_oracle():
     # A12/A13 threshold flips: observed 1 per ~130 k candidates -> ~8 expected in ~1 M; allowance 12
     g, o = _check(batch, max_ok_mismatch=12)
     assert abs(g.n_tracks - len(o.trk_cand)) <= 8
+
+
+def test_full_bench_batch_sampled_instances_against_oracle():
+    """BASELINE.json configs[4] at FULL size, in the launch configuration bench.py times: 100 drift windows (3,600
+    sector instances, 116 M clusters) in ONE tpc_track_sectors call.  Sector instances are independent, so the oracle
+    can compute any one of them alone: twelve sampled instances (first, last, both z sides, the largest) are compared
+    output by output -- links, start hits and candidates bit-exact; tracklet hit lists, parameters, covariance, chi2;
+    final assignment -- plus the properties that hold at any size for the whole batch."""
+    import sys
+    import torch
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    from oracle.tpc_oracle import Oracle
+    from paper_1709_00618_b200 import Tracker
+    from parity_util import COV_TOL, PAR_ATOL, PAR_RTOL
+    evs, batch = bench.make_batch(100, 5001, 0)
+    N, S, R = batch.n_clusters, batch.n_inst, batch.n_rows
+    assert S == 3600 and N > 100_000_000
+    trk = Tracker.for_event(batch)
+    dev = trk.device
+    d_cl = torch.from_numpy(batch.clusters).to(dev)
+    d_ro = torch.from_numpy(batch.row_offsets).to(dev)
+    trk.reserve(N, S)
+    trk.set_stream()
+    bufs, out = trk.alloc_outputs(N, debug=True, trk_capacity=N // 20 + 64)
+    trk.track_sectors_device(d_cl, d_ro, S, out)
+    torch.cuda.synchronize(dev)
+    counts = bufs["counts"].cpu().numpy()
+    n_start, n_cand, n_tl, n_trk, n_thits = (int(x) for x in counts[:5])
+    assert counts[5] == 0 and n_cand > 5_000_000 and n_trk > 1_300_000
+    # whole-batch properties (any size)
+    off = bufs["trk_hit_offset"][:n_trk + 1].cpu().numpy()
+    nh = bufs["trk_nhits"][:n_trk].cpu().numpy()
+    assert off[0] == 0 and off[n_trk] == n_thits and np.array_equal(np.diff(off), nh) and nh.min() >= 10
+    cid = bufs["trk_cand_id"][:n_trk].cpu().numpy()
+    assert np.all(np.diff(cid) > 0)
+    assert int((bufs["cluster_owner"] >= 0).sum()) == n_thits
+    cand_first = bufs["cand_hits"][:n_cand, 0].cpu().numpy()
+    assert np.all(np.diff(cand_first) > 0)
+    start_hits = bufs["start_hits"][:n_start].cpu().numpy()
+    inst_sizes = np.diff(batch.row_offsets[::R])
+    sample = sorted({0, 1, 17, 18, 35, 36, 1799, 1800, 3564, 3599, int(np.argmax(inst_sizes)), int(np.argmin(inst_sizes))})
+    worst = 0.0
+    for inst in sample:
+        lo, hi = int(batch.row_offsets[inst * R]), int(batch.row_offsets[(inst + 1) * R])
+        ro1 = (batch.row_offsets[inst * R:(inst + 1) * R + 1] - lo).astype(np.int32)
+        # the instance alone, as instance `inst % 36` of a one-window problem (its z side must survive): pad with
+        # empty instances in front
+        k = inst % 36
+        ro_pad = np.concatenate([np.zeros(k * R, np.int32), ro1, np.full((35 - k) * R, ro1[-1], np.int32)])
+        orc = Oracle.for_event(batch)
+        o = orc.track(batch.clusters[lo:hi], ro_pad, 36)
+
+        def reb(a):  # device slice of a per-cluster index array, re-based to the instance
+            v = a[lo:hi].cpu().numpy()
+            return np.where(v >= 0, v - lo, -1)
+        assert np.array_equal(reb(bufs["link_up_raw"]), o.link_up_raw) and np.array_equal(reb(bufs["link_dn_raw"]), o.link_dn_raw)
+        assert np.array_equal(reb(bufs["link_up"]), o.link_up) and np.array_equal(reb(bufs["link_dn"]), o.link_dn)
+        s0, s1 = np.searchsorted(start_hits, [lo, hi])
+        assert np.array_equal(start_hits[s0:s1] - lo, o.start_hits)
+        c0, c1 = np.searchsorted(cand_first, [lo, hi])
+        assert c1 - c0 == len(o.cand_n)
+        ch = bufs["cand_hits"][c0:c1].cpu().numpy()
+        assert np.array_equal(np.where(ch >= 0, ch - lo, -1), o.cand_hits)
+        assert np.array_equal(bufs["cand_n"][c0:c1].cpu().numpy(), o.cand_n)
+        th = bufs["tl_hits"][c0:c1].cpu().numpy()
+        th = np.where(th >= 0, th - lo, -1)
+        nhg = bufs["tl_nhits"][c0:c1].cpu().numpy()
+        ok_o = o.tracklets["ok"].astype(bool)
+        assert np.array_equal(nhg > 0, ok_o)
+        same = np.all(th == o.tracklet_hits, axis=1) & ok_o
+        assert same.sum() >= MIN_SHARED * ok_o.sum()
+        pg = bufs["tl_params"][c0:c1].cpu().numpy().astype(np.float64)[same]
+        po = o.tracklets["p"][same]
+        ex = np.abs(pg - po) / (PAR_ATOL + PAR_RTOL * np.abs(po))
+        worst = max(worst, float(ex.max()))
+        assert ex.max() <= 1.0
+        cg = bufs["tl_cov"][c0:c1].cpu().numpy().astype(np.float64)[same]
+        co = o.tracklets["cov"][same]
+        ii = np.array([i for i in range(5) for j in range(i + 1)])
+        jj = np.array([j for i in range(5) for j in range(i + 1)])
+        diag = np.array([0, 2, 5, 9, 14])
+        assert (np.abs(cg - co) / (COV_TOL * np.sqrt(co[:, diag[ii]] * co[:, diag[jj]]))).max() <= 1.0
+        # final assignment of this instance's clusters, tracks matched by candidate id
+        own = bufs["cluster_owner"][lo:hi].cpu().numpy()
+        own_g = np.where(own >= 0, cid[np.maximum(own, 0)] - c0, -1)
+        own_o = np.where(o.cluster_owner >= 0, o.trk_cand[np.maximum(o.cluster_owner, 0)], -1)
+        assigned = (own_g >= 0) | (own_o >= 0)
+        assert ((own_g == own_o) & assigned).sum() >= MIN_SHARED * assigned.sum()
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/parity_report.jsonl", "a") as f:
+        f.write(json.dumps(dict(case="cfg5_full_100_windows_sampled", n_clusters=N, instances=sample,
+                                worst_param_excess=worst, n_cand=n_cand, n_tracks=n_trk)) + "\n")
+    trk.close()
