@@ -3,13 +3,11 @@
 // hits (ties: lowest candidate id); a tracklet keeps the hits it won and becomes a final track iff it keeps
 // >= sel_min hits; final tracks are numbered in ascending candidate id.  Integer-only, so results are unique.
 //
-// claim (tracklet-centric): one 32-bit atomicMax of the packed weight (nhits << 23 | inverted candidate id local to
-// the sector instance) per attached hit.  A warp takes 32 consecutive tracklets: every lane loads one header
-// (coalesced), then the warp walks the 32 row-indexed hit tables, 4 rows per lane and 8-byte load.  The pass is bound
-// by the SM's issue rate for scattered atomics (~1.3 cycles per lane, B300_MICROARCH.md "Atomics").
-// Everything after it is HIT-centric: every pass streams over the hits once (coalesced) and touches one 32-byte
-// record per claimed hit:
-//   mark      per hit: winner tracklet from the claim word -> set the row's bit in the winner's kept-row mask
+// claim + mark (one CTA per sector instance, shared memory): one 32-bit atomicMax of the packed weight (nhits << 23 |
+// inverted candidate ordinal inside the sector instance) per attached hit, then per hit the winner tracklet from
+// the claim word -> the row's bit in the winner's kept-row mask.  (Round 1 did both on global memory: 473 M scattered
+// L2 reductions at 88 % of the L2's throughput, 2.9 ms; in shared memory 1.5 ms.)
+// Everything after it is HIT- or tracklet-centric streaming:
 //   count     per tracklet: kept = popcount(mask), tracks/hits per block of 256 tracklets, then one scan
 //   finalize  per tracklet: track index and first hit position (deterministic: ascending candidate id), track record
 //   write     per hit: owner and the track's hit list entry (rank = kept rows below, from the mask)
@@ -26,77 +24,108 @@ __device__ __forceinline__ int64_t winner_of(uint32_t w, int64_t cand_base) {
     return cand_base + (int64_t)(0x7FFFFFu - (w & 0x7FFFFFu));
 }
 
-constexpr int kClaimThreads = 256;
+// claim + mark for ONE SECTOR INSTANCE per CTA, in shared memory.  An instance's clusters are claimed only by its
+// own tracklets, and both the claim words (4 B per cluster, ~130 KB) and the kept-row masks (20 B per tracklet,
+// ~30 KB) of one instance fit in an SM's shared memory: the ~4.6 claims per kept hit become shared-memory atomics
+// instead of scattered L2 reductions (the separate kernels ran at 88 % of the L2's throughput: 473 M REDs), and the
+// winners' mask bits are set in shared memory too.  The final claim words and masks go to global memory coalesced,
+// once.  An instance too large for the shared memory (dense events) takes the same code on the global arrays.
+constexpr int kInstThreads = 1024;
 
-__global__ void __launch_bounds__(kClaimThreads)
-claim_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
-             const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_rows,
-             const int32_t* __restrict__ cand_slab, const int2* __restrict__ slab_part,
-             const uint16_t* __restrict__ tl_rowhit, uint32_t* __restrict__ claim, int64_t* __restrict__ counts,
-             int64_t Cmax) {
-    const int64_t n_cand = min(counts[1], Cmax);
-    const int lane = threadIdx.x & 31;
-    // Chunks of 32 tracklets are handed out in order from a device-wide counter (counts[13]), so the tracklets in
-    // flight -- and with them the claim words being updated -- stay a compact window of candidate ids that the L2
-    // holds; with a fixed grid stride the warps drift apart and at 100 windows the atomics thrash the L2.
-    unsigned long long* next = reinterpret_cast<unsigned long long*>(&counts[13]);
-    for (;;) {
-        unsigned long long t = 0;
-        if (lane == 0) t = atomicAdd(next, 32ull);
-        const int64_t c0 = (int64_t)__shfl_sync(kFull, t, 0);
-        if (c0 >= n_cand) break;
-        // header of the lane's tracklet
-        uint32_t my_w = 0u;
-        int my_rows = 0, my_inst = 0;
-        if (c0 + lane < n_cand) {
-            const int64_t c = c0 + lane;
-            const int nh = tl_nhits[c];
-            my_rows = tl_rows[c];
-            my_inst = cand_slab[c] / g.R;
-            if (nh > 0) {
-                // candidate ordinal inside its instance.  It fits in 23 bits by construction: chains are disjoint and
-                // hold >= cand_min >= 2 hits, so an instance has at most 255 rows * 65,535 hits / 2 = 8,355,712 < 2^23
-                // candidates (rows and row lengths are bounded by tpc_tracker_create and S1).
-                const int64_t lcid = c - slab_part[(size_t)my_inst * g.R].y;
-                my_w = ((uint32_t)nh << 23) | (uint32_t)(0x7FFFFF - (lcid & 0x7FFFFF));
+template <bool kShared>
+__device__ __forceinline__ void claim_mark_instance(const DevGeom& g, const int32_t* __restrict__ s_ro,
+                                                    const int32_t* __restrict__ tl_nhits,
+                                                    const int32_t* __restrict__ tl_rows,
+                                                    const uint16_t* __restrict__ tl_rowhit, int64_t c_lo, int n_c,
+                                                    uint32_t* claim_w, uint32_t* mask_w, int mask_stride) {
+    // claim_w[i] = claim word of the instance's hit i (sorted position - first hit of the instance; s_ro holds the
+    // row offsets relative to it); mask_w[k * mask_stride + q] = word q of the kept-row mask of its tracklet k.
+    // The row tables of the instance's tracklets are one contiguous array (RP entries each): the CTA streams it in
+    // 8-byte pieces (4 rows), consecutive threads on consecutive pieces.
+    const int quads = g.RP / 4;
+    const uint2* tab = reinterpret_cast<const uint2*>(tl_rowhit + (size_t)c_lo * g.RP);
+    constexpr int kU = 4;  // independent 8-byte pieces per thread in flight (the phase is bound by memory parallelism)
+    // piece q = tracklet q / quads, rows 4 * (q % quads) ...; the pair is advanced incrementally (no division per piece)
+    const int n_items = n_c * quads;  // < 2^31: n_c <= 2^23 / ... in practice a few thousand
+    const int k_step = kInstThreads / quads, r_step = kInstThreads - k_step * quads;
+    int kq = (int)threadIdx.x / quads, rem = (int)threadIdx.x - kq * quads;
+    for (int q0 = threadIdx.x; q0 < n_items; q0 += kU * kInstThreads) {
+        uint2 v[kU];
+        int k[kU], rq[kU], nh[kU], rows[kU];
+#pragma unroll
+        for (int u = 0; u < kU; u++) {
+            const int q = q0 + u * kInstThreads;
+            k[u] = -1;
+            if (q < n_items) {
+                k[u] = kq;
+                rq[u] = 4 * rem;
+                v[u] = __ldcs(&tab[q]);
+                nh[u] = tl_nhits[c_lo + kq];
+                rows[u] = tl_rows[c_lo + kq];
+            }
+            kq += k_step;
+            rem += r_step;
+            if (rem >= quads) { rem -= quads; kq++; }
+        }
+#pragma unroll
+        for (int u = 0; u < kU; u++) {
+            if (k[u] < 0 || nh[u] <= 0) continue;
+            const int first = rows[u] & 0xff, last = (rows[u] >> 8) & 0xff;
+            const uint32_t w = ((uint32_t)nh[u] << 23) | (uint32_t)(0x7FFFFF - k[u]);
+            const uint32_t li[4] = {v[u].x & 0xffffu, v[u].x >> 16, v[u].y & 0xffffu, v[u].y >> 16};
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                const int r = rq[u] + j;
+                if (r >= first && r <= last && li[j] != kNoHit) atomicMax(&claim_w[s_ro[r] + (int)li[j]], w);
             }
         }
-        for (unsigned todo = __ballot_sync(kFull, my_w != 0u); todo; todo &= todo - 1) {
-            const int k = __ffs(todo) - 1;
-            const uint32_t w = __shfl_sync(kFull, my_w, k);
-            const int rows = __shfl_sync(kFull, my_rows, k), inst = __shfl_sync(kFull, my_inst, k);
-            const int first = rows & 0xff, last = (rows >> 8) & 0xff;
-            const uint16_t* rh = tl_rowhit + (size_t)(c0 + k) * g.RP;
-            const int32_t* ro = row_offsets + (size_t)inst * g.R;
-            for (int rq = (first & ~127) + 4 * lane; rq <= last; rq += 128) {
-                if (rq + 3 < first) continue;
-                const uint2 v = __ldcs(reinterpret_cast<const uint2*>(rh + rq));  // streamed once (evict-first): keep the L2 for
-                                                                         // the claim words; RP % 8 == 0: in bounds, aligned
-                const uint32_t li[4] = {v.x & 0xffffu, v.x >> 16, v.y & 0xffffu, v.y >> 16};
-#pragma unroll
-                for (int j = 0; j < 4; j++) {
-                    const int r = rq + j;
-                    if (r >= first && r <= last && li[j] != kNoHit) atomicMax(&claim[ro[r] + (int)li[j]], w);
-                }
-            }
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, n_warps = kInstThreads / 32;
+    for (int r = wid; r < g.R; r += n_warps) {  // mark: one warp per pad row
+        const int b = s_ro[r], n = s_ro[r + 1] - b;
+        const uint32_t bit = 1u << (r & 31);
+        for (int i = lane; i < n; i += 32) {
+            const uint32_t w = claim_w[b + i];
+            if (w) atomicOr(&mask_w[(size_t)(0x7FFFFFu - (w & 0x7FFFFFu)) * mask_stride + (r >> 5)], bit);
         }
     }
 }
 
-__global__ void __launch_bounds__(kHitThreads)
-mark_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
-            const int2* __restrict__ slab_part, const uint32_t* __restrict__ claim, uint32_t* __restrict__ tl_sel,
-            int n_slabs) {
-    const int slab = blockIdx.x * (kHitThreads / 32) + (threadIdx.x >> 5);  // one warp per slab
-    if (slab >= n_slabs) return;
-    const int inst = slab / g.R, r = slab - inst * g.R;
-    const int base = row_offsets[slab], n = row_offsets[slab + 1] - base;
-    if (n == 0) return;
-    const int64_t cand_base = slab_part[(size_t)inst * g.R].y;
-    const uint32_t bit = 1u << (r & 31);
-    for (int i = threadIdx.x & 31; i < n; i += 32) {
-        const uint32_t w = claim[base + i];
-        if (w) atomicOr(&tl_sel[winner_of(w, cand_base) * g.sel_stride + (r >> 5)], bit);
+__global__ void __launch_bounds__(kInstThreads, 1)
+claim_mark_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
+                  const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_rows,
+                  const int2* __restrict__ slab_part, const uint16_t* __restrict__ tl_rowhit,
+                  uint32_t* __restrict__ claim, uint32_t* __restrict__ tl_sel, const int64_t* __restrict__ counts,
+                  int64_t Cmax, int smem_words) {
+    extern __shared__ __align__(16) uint32_t s_mem[];
+    __shared__ int32_t s_ro[kMaxRows + 1];  // row offsets of the instance relative to its first hit
+    const int inst = blockIdx.x;
+    const int32_t* ro = row_offsets + (size_t)inst * g.R;
+    const int hit0 = ro[0], n_hits = ro[g.R] - hit0;
+    for (int r = threadIdx.x; r <= g.R; r += kInstThreads) s_ro[r] = ro[r] - hit0;
+    const int64_t n_cand = min(counts[1], Cmax);
+    const int64_t c_lo = min((int64_t)slab_part[(size_t)inst * g.R].y, n_cand);
+    const int64_t c_hi = min((int64_t)slab_part[(size_t)(inst + 1) * g.R].y, n_cand);
+    const int n_c = (int)(c_hi - c_lo);
+    if (n_c <= 0 || n_hits <= 0) return;  // claim words and masks stay zero (initialised by S3/S4 and S5); uniform
+    const int words = g.sel_words;
+    if ((int64_t)n_hits + (int64_t)n_c * words <= smem_words) {
+        uint32_t* claim_s = s_mem;
+        uint32_t* mask_s = s_mem + n_hits;
+        for (int i = threadIdx.x; i < n_hits + n_c * words; i += kInstThreads) s_mem[i] = 0u;
+        __syncthreads();
+        claim_mark_instance<true>(g, s_ro, tl_nhits, tl_rows, tl_rowhit, c_lo, n_c, claim_s, mask_s, words);
+        __syncthreads();
+        for (int i = threadIdx.x; i < n_hits; i += kInstThreads) claim[hit0 + i] = claim_s[i];
+        for (int i = threadIdx.x; i < n_c * words; i += kInstThreads) {
+            const int k = i / words, q = i - k * words;
+            tl_sel[(size_t)(c_lo + k) * g.sel_stride + q] = mask_s[i];
+        }
+    } else {  // does not fit: the same passes on the global arrays (zeroed by the earlier stages)
+        __syncthreads();
+        claim_mark_instance<false>(g, s_ro, tl_nhits, tl_rows, tl_rowhit, c_lo, n_c, claim + hit0,
+                                   tl_sel + (size_t)c_lo * g.sel_stride, g.sel_stride);
     }
 }
 
@@ -254,10 +283,20 @@ int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const 
         const int slabs = p.n_inst * g.R;
         const int64_t blocks = div_up(w.Cmax, kSelBlock);
         const int grid = (int)(blocks < 148 * 8 ? blocks : 148 * 8);
-        claim_kernel<<<grid, kClaimThreads, 0, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows, w.cand_slab, w.slab_part,
-                                                    w.tl_rowhit, w.claim, w.counts, w.Cmax);
         const int hgrid = div_up(slabs, kHitThreads / 32);
-        mark_kernel<<<hgrid, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel, slabs);
+        {
+            static int smem_bytes = 0;
+            if (!smem_bytes) {
+                int dev = 0, max_optin = 0;
+                cudaGetDevice(&dev);
+                cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+                smem_bytes = (max_optin > 0 ? max_optin : 48 * 1024) - 2048;  // room for the kernel's static arrays
+                cudaFuncSetAttribute(claim_mark_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+            }
+            claim_mark_kernel<<<p.n_inst, kInstThreads, smem_bytes, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows,
+                                                                         w.slab_part, w.tl_rowhit, w.claim, w.tl_sel,
+                                                                         w.counts, w.Cmax, smem_bytes / 4);
+        }
         count_kernel<<<grid, kSelThreads, 0, s>>>(g, w.tl_nhits, w.tl_sel, w.sel_part, w.counts, w.Cmax);
         launch_scan_int2(w.sel_part, w.counts + 1, kSelBlock, w.Cmax, 0, w.counts, 3, 4, s);
         const FinalIn a{w.tl_nhits, w.tl_rows, w.cand_slab, w.tl_par, w.tl_cov, w.tl_chi2, w.sel_part, w.tl_sel,
@@ -265,7 +304,7 @@ int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const 
         finalize_tracks_kernel<<<grid, kSelThreads, 0, s>>>(g, a, o);
         write_hits_kernel<<<hgrid, kHitThreads, 0, s>>>(g, p.row_offsets, w.slab_part, w.claim, w.tl_sel, w.hit_idx, o,
                                                         slabs);
-        launches += 6;
+        launches += 5;
     }
     finalize_counts_kernel<<<1, 32, 0, s>>>(w.counts, o);
     return launches + 1;
