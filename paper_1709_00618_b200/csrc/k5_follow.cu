@@ -205,30 +205,56 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
 
 // ---- row-by-row following ------------------------------------------------------------------------------------------
 
-// The best hit of the pick-up search so far.
+// The best hit of the pick-up search so far, and whether an exact tie for the best distance was seen on the way.
 struct PickBest {
-    int j;       // sorted position of the best hit, -1 = none
+    int j;       // sorted position (in its row) of the best hit, -1 = none
     float d2, y, z;
+    bool tie;
 };
 
-// Exact tie between two hits of the search (only duplicated clusters produce one): the lowest local index wins.
-__device__ __noinline__ bool tie_lower_index(const uint16_t* __restrict__ idx, unsigned ja, unsigned jb) {
-    return idx[ja] < idx[jb];
-}
-
-// One hit of the pick-up search: inside the gate and nearer than the best so far?  Ties -> lowest local index.
-// The decision arithmetic is individually rounded fp32 (both sides decide in fp32).
-__device__ __forceinline__ void pick_consider(PickBest& b, const uint16_t* __restrict__ idx, unsigned rb, int j,
-                                              bool valid, float2 h, float yp, float zp, float wy, float wz) {
+// One hit of the pick-up search: inside the gate and nearer than the best so far?  The decision arithmetic is
+// individually rounded fp32 (both sides decide in fp32).  Strictly-nearer wins here; an exact tie for
+// the best distance (only duplicated clusters produce one) is only RECORDED, and the search is then redone out of
+// line by pick_exact with the full rule (lowest local index).  A tie for the minimum is always seen: the second of
+// two equal-best hits meets either the first or something nearer still.
+__device__ __forceinline__ void pick_consider(PickBest& b, int j, bool valid, float2 h, float yp, float zp, float wy,
+                                              float wz) {
     const float dy = __fsub_rn(h.x, yp), dz = __fsub_rn(h.y, zp);
     const float d2 = __fadd_rn(__fmul_rn(dy, dy), __fmul_rn(dz, dz));
     const bool in = valid && fabsf(dy) <= wy && fabsf(dz) <= wz;
-    bool better = in && d2 < b.d2;
-    if (in && d2 == b.d2) better = tie_lower_index(idx, rb + (unsigned)j, rb + (unsigned)b.j);  // b.d2 finite: b.j >= 0
+    const bool better = in && d2 < b.d2;
+    b.tie = b.tie || (in && d2 == b.d2);
     b.j = better ? j : b.j;
     b.d2 = better ? d2 : b.d2;
     b.y = better ? h.x : b.y;
     b.z = better ? h.y : b.z;
+}
+
+// The whole pick-up search of one row with the complete rule: nearest hit inside the gate by (dy^2 + dz^2), ties ->
+// lowest local index.  tb = the row's cell table, rowh / rowi = the row's sorted hits and their local indices.
+__device__ __noinline__ int pick_exact(const uint16_t* __restrict__ tb, const float2* __restrict__ rowh,
+                                       const uint16_t* __restrict__ rowi, int ny, int zb0, int zb1, int ys0, int ys1,
+                                       float yp, float zp, float wy, float wz) {
+    int bj = -1;
+    float bd2 = __int_as_float(0x7f800000);
+    unsigned bi = 0u;
+    for (int zb = zb0; zb <= zb1; zb++) {
+        const uint16_t* t = tb + zb * ny;
+        const int j1 = t[ys1];
+        for (int j = t[ys0]; j < j1; j++) {
+            const float2 h = rowh[j];
+            const float dy = __fsub_rn(h.x, yp), dz = __fsub_rn(h.y, zp);
+            if (!(fabsf(dy) <= wy && fabsf(dz) <= wz)) continue;
+            const float d2 = __fadd_rn(__fmul_rn(dy, dy), __fmul_rn(dz, dz));
+            const unsigned li = rowi[j];
+            if (d2 < bd2 || (d2 == bd2 && li < bi)) {
+                bd2 = d2;
+                bi = li;
+                bj = j;
+            }
+        }
+    }
+    return bj;
 }
 
 __device__ __forceinline__ float sqrt_fast(float x) {  // x > 0, normal range
@@ -245,33 +271,17 @@ __device__ __forceinline__ void store_report(float4 (*s_rep)[kFollowThreads], co
     s_rep[4][threadIdx.x] = make_float4(st.c41, st.c42, st.c43, st.c44);
 }
 
-// The cells of a search window in one row: z bins zb0..zb1, strips ys0 .. ys1 - 1.
-struct Window {
-    int zb0, zb1, ys0, ys1;  // ys1 exclusive
-};
-
-__device__ __forceinline__ Window window_cells(const DevGeom& g, float2 gy, float z0, float yp, float zp, float wy,
-                                               float wz) {
-    Window w;
-    w.zb0 = zbin(zp - wz, z0, g.inv_cz, g.nz);
-    w.zb1 = zbin(zp + wz, z0, g.inv_cz, g.nz);
-    w.ys0 = ybin(yp - wy, gy.x, gy.y, g.ny);
-    w.ys1 = ybin(yp + wy, gy.x, gy.y, g.ny) + 1;
-    return w;
-}
-
-// The window's hits as one sequence of nt sorted positions: the first na start at ja0, element k >= na sits at k + d.
+// The window's hits as one sequence of nt sorted positions: element k < na sits at k + ja0, element k >= na at k + d.
 struct HitSeq {
     int ja0, na, nt, d;
 };
 
-__device__ __forceinline__ HitSeq hit_seq(unsigned tab0, unsigned tab1, bool two) {
+__device__ __forceinline__ HitSeq hit_seq(unsigned t00, unsigned t01, unsigned t10, unsigned t11, bool two) {
     HitSeq s;
-    s.ja0 = (int)(tab0 & 0xffffu);
-    s.na = (int)(tab0 >> 16) - s.ja0;
-    const int jb0 = (int)(tab1 & 0xffffu);
-    s.nt = s.na + (two ? (int)(tab1 >> 16) - jb0 : 0);
-    s.d = jb0 - s.na;
+    s.ja0 = (int)t00;
+    s.na = (int)t01 - (int)t00;
+    s.nt = s.na + (two ? (int)t11 - (int)t10 : 0);
+    s.d = (int)t10 - s.na;
     return s;
 }
 
@@ -280,37 +290,41 @@ __device__ __forceinline__ HitSeq hit_seq(unsigned tab0, unsigned tab1, bool two
 template <bool kCount>
 __global__ void __launch_bounds__(kFollowThreads, kFollowCtasPerSm)
 follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowArgs a) {
-    __shared__ float s_rowx[kMaxRows + 1];
-    __shared__ float2 s_rowy[kMaxRows + 1];      // (y0, strips per cm) of the row's grid
+    // per row: x, lower edge of the y grid, strips per cm, |y| limit of the sector (x tan(half angle) + margin)
+    __shared__ float4 s_row[kMaxRows + 1];
     __shared__ float4 s_rep[5][kFollowThreads];  // reported state of the lane's tracklet (see kDown below)
+    // values touched only in the write-out / refill phase live in shared memory, not in registers of the row loop
+    __shared__ int s_cand[kFollowThreads];        // the lane's candidate id
+    __shared__ int2 s_chunk[kFollowThreads / 32];  // the warp's chunk [x, y) of candidate ids
+    if (threadIdx.x < kFollowThreads / 32) s_chunk[threadIdx.x] = make_int2(0, 0);
     for (int q = threadIdx.x; q < g.R; q += kFollowThreads) {
-        s_rowx[q] = g.row_x[q];
-        s_rowy[q] = make_float2(g.row_y0[q], g.row_inv_sy[q]);
+        const float x = g.row_x[q];
+        s_row[q] = make_float4(x, g.row_y0[q], g.row_inv_sy[q], fmaf(x, g.tan_half, g.edge_margin));
     }
     __syncthreads();
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    const int n_cand = (int)min(a.counts[1], a.Cmax);
-    const size_t cs = (size_t)a.Cmax;
-    unsigned long long* queue = reinterpret_cast<unsigned long long*>(&a.counts[10]);
-    int wn = 0, we = 0;  // the warp's chunk [wn, we) of candidate ids (warp-uniform)
+    const unsigned tab_stride = (unsigned)g.nzp >> 4;  // cell-table row in units of 16 entries (nzp is a multiple)
     bool exhausted = false;
     unsigned n_tr = 0, n_up = 0, n_ex = 0, n_se = 0;  // work counters (kCount only)
 
     // lane state
     int mode = kIdle;
-    int c = 0, slab_base = 0;
+    int slab_base = 0;
     int r = 0, rn = 0, r0 = 0;  // row of the state, row of the coming step, start row
     int nhits = 0, gap = 0, first_row = 0, last_row = 0;
     float yref = 0.0f, zref = 0.0f, z0 = 0.0f, chi2 = 0.0f;
+    float xr = 0.0f;  // x of row r
     KfState st = {};
     int rb_next = 0;  // offset of row rn (loaded one step ahead)
+    uint16_t* rh = a.tl_rowhit;  // the candidate's row-indexed hit table
 
     for (;;) {
         unsigned act = __ballot_sync(full, mode < kDone);
         if (act == 0u || (!exhausted && 32 - __popc(act) >= kFollowReload)) {
             // ---- write-out of ended candidates ----
             if (mode == kDone) {
+                const int c = s_cand[threadIdx.x];
                 const float4 q0 = s_rep[0][threadIdx.x], q1 = s_rep[1][threadIdx.x], q2 = s_rep[2][threadIdx.x],
                              q3 = s_rep[3][threadIdx.x], q4 = s_rep[4][threadIdx.x];
                 float* p = a.tl_par + (size_t)c * 5;
@@ -329,12 +343,16 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             // ---- refill ----
             if (!exhausted) {
                 const unsigned idle = __ballot_sync(full, mode == kIdle);
+                const int n_cand = (int)min(a.counts[1], a.Cmax);
+                const size_t cs = (size_t)a.Cmax;
+                int wn = s_chunk[threadIdx.x >> 5].x, we = s_chunk[threadIdx.x >> 5].y;
                 if (wn == we) {
                     // kFollowChunk = 0: take exactly as many ids as there are idle lanes (best balance at the end of
                     // the queue: no warp sits on ids it cannot start yet)
                     const int take = kFollowChunk > 0 ? kFollowChunk : __popc(idle);
                     unsigned long long v = 0;
-                    if (lane == 0) v = atomicAdd(queue, (unsigned long long)take);
+                    if (lane == 0)
+                        v = atomicAdd(reinterpret_cast<unsigned long long*>(&a.counts[10]), (unsigned long long)take);
                     v = __shfl_sync(full, v, 0);
                     if (v >= (unsigned long long)n_cand) {
                         exhausted = true;
@@ -345,7 +363,8 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 }
                 const int mine = wn + __popc(idle & ((1u << lane) - 1u));
                 if (mode == kIdle && mine < we) {
-                    c = mine;
+                    const int c = mine;
+                    s_cand[threadIdx.x] = c;
                     const float4* ts = a.tl_state + c;
                     const float4 t5 = ts[5 * cs];
                     const int nbits = __float_as_int(t5.w);  // own hits | (last own row - start row) << 8
@@ -369,12 +388,16 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         gap = 0;
                         first_row = r0;
                         r = last_row = r0 + (nbits >> 8);
+                        xr = s_row[r].x;
                         mode = r + 1 < g.R ? kUp : kBack;
                         rn = mode == kUp ? r + 1 : r0;
                         rb_next = a.row_offsets[slab_base + rn];
+                        rh = a.tl_rowhit + (size_t)c * (size_t)g.RP;
                     }
                 }
-                wn = min(we, wn + __popc(idle));
+                __syncwarp();
+                if (lane == 0) s_chunk[threadIdx.x >> 5] = make_int2(min(we, wn + __popc(idle)), we);
+                __syncwarp();
             }
             act = __ballot_sync(full, mode < kDone);
             if (act == 0u && exhausted) break;
@@ -384,68 +407,78 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             // straight path with flags: the lanes of a warp differ in phase, and every branch taken by a few
             // lanes costs the whole warp its instructions.
             const bool is_back = mode == kBack;
-            const bool t_ok = kf_transport(st, s_rowx[rn] - s_rowx[r], g.cB, g.max_s);
+            const bool down = mode == kDown;
+            const float4 rd = s_row[rn];
+            const bool t_ok = kf_transport(st, rd.x - xr, g.cB, g.max_s);
             if (kCount && t_ok) n_tr++;
             r = t_ok ? rn : r;
+            xr = t_ok ? rd.x : xr;
             const float yp = st.y + yref, zp = st.z + zref;
-            const bool inside = fabsf(yp) <= fmaf(s_rowx[r], g.tan_half, g.edge_margin);
+            const bool inside = fabsf(yp) <= rd.w;
             const bool search = t_ok && !is_back && inside;
-            int li = -1;
+            bool hit = false;
             if (search) {
                 // gate: 4 sigma of the predicted residual, capped (sigma > 0: tpc_tracker_create)
                 const float wy = fminf(g.wmax, g.gate * sqrt_fast(st.c00 + g.sy2));
                 const float wz = fminf(g.wmax, g.gate * sqrt_fast(st.c11 + g.sz2));
-                const Window w = window_cells(g, s_rowy[r], z0, yp, zp, wy + kCellMargin, wz + kCellMargin);
-                const unsigned urb = (unsigned)rb_next;
-                // cell-table entries of the exact window (64-bit index: n_inst * R * nzp may exceed 2^32)
-                const uint16_t* tb = a.bin_start + (size_t)(slab_base + r) * (size_t)g.nzp;
-                const uint16_t* ta = tb + w.zb0 * g.ny;
-                const bool two = w.zb1 > w.zb0;
-                const unsigned t00 = ta[w.ys0], t01 = ta[w.ys1];
+                // the cells of the gate window, widened by a margin so that they cover the rounded fp32 gate test
+                const float my = wy + kCellMargin, mz = wz + kCellMargin;
+                const int zb0 = zbin(zp - mz, z0, g.inv_cz, g.nz), zb1 = zbin(zp + mz, z0, g.inv_cz, g.nz);
+                const int ys0 = ybin(yp - my, rd.y, rd.z, g.ny), ys1 = ybin(yp + my, rd.y, rd.z, g.ny) + 1;
+                // cell-table entries of the window (row index in 32-byte units: n_inst * R * nzp may exceed 2^32)
+                const uint16_t* tb = a.bin_start + (size_t)((unsigned)(slab_base + r) * tab_stride) * 16u;
+                const unsigned o0 = (unsigned)(zb0 * g.ny), o1 = (unsigned)(zb1 * g.ny);
+                const bool two = zb1 > zb0;
+                const unsigned t00 = tb[o0 + (unsigned)ys0], t01 = tb[o0 + (unsigned)ys1];
                 unsigned t10 = 0u, t11 = 0u;
                 if (two) {
-                    const uint16_t* tz = tb + w.zb1 * g.ny;
-                    t10 = tz[w.ys0];
-                    t11 = tz[w.ys1];
+                    t10 = tb[o1 + (unsigned)ys0];
+                    t11 = tb[o1 + (unsigned)ys1];
                 }
-                const HitSeq q = hit_seq(t00 | (t01 << 16), t10 | (t11 << 16), two);
+                const HitSeq q = hit_seq(t00, t01, t10, t11, two);
                 if (kCount) {
                     n_se++;
                     n_ex += q.nt;
                 }
-                // The window's hits form one sequence k = 0..nt-1, element k at sorted position seq_pos(k).  The
-                // first kDirectHits are loaded together (one memory round trip), the rest (rare) one by one.
-                PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f};
+                const unsigned urb = (unsigned)rb_next;  // hits of the row: a.hit_yz[urb + position], 32-bit index
+                const float2* rowh = a.hit_yz + urb;
+                // The window's hits form one sequence k = 0..nt-1.  The first kDirectHits are loaded together (one
+                // memory round trip) and compared without a branch, the rest (few lanes) one by one.
+                PickBest b{-1, __int_as_float(0x7f800000), 0.0f, 0.0f, false};
                 {
                     float2 h[kDirectHits];
                     int j[kDirectHits];
 #pragma unroll
                     for (int k = 0; k < kDirectHits; k++) {
-                        j[k] = k < q.na ? q.ja0 + k : k + q.d;
+                        j[k] = k + (k < q.na ? q.ja0 : q.d);
                         h[k] = make_float2(0.0f, 0.0f);
                         if (k < q.nt) h[k] = a.hit_yz[urb + (unsigned)j[k]];
                     }
 #pragma unroll
-                    for (int k = 0; k < kDirectHits; k++)
-                        pick_consider(b, a.hit_idx, urb, j[k], k < q.nt, h[k], yp, zp, wy, wz);
+                    for (int k = 0; k < kDirectHits; k++) pick_consider(b, j[k], k < q.nt, h[k], yp, zp, wy, wz);
                 }
-                for (int k = kDirectHits; k < q.nt; k++) {  // few lanes get here: test the gate first, most hits fail it
-                    const int j = k < q.na ? q.ja0 + k : k + q.d;
+                for (int k = kDirectHits; k < q.nt; k++) {  // test the gate first, most of these hits fail it
+                    const int j = k + (k < q.na ? q.ja0 : q.d);
                     const float2 h = a.hit_yz[urb + (unsigned)j];
                     if (fabsf(__fsub_rn(h.x, yp)) <= wy && fabsf(__fsub_rn(h.y, zp)) <= wz)
-                        pick_consider(b, a.hit_idx, urb, j, true, h, yp, zp, wy, wz);
+                        pick_consider(b, j, true, h, yp, zp, wy, wz);
                 }
                 // z bins in between exist only when the cells are narrower than the gate (non-default grid_cell_z)
-                for (int zb = w.zb0 + 1; zb < w.zb1; zb++) {
-                    const uint16_t* tm = tb + zb * g.ny;
-                    const int jm0 = tm[w.ys0], jm1 = tm[w.ys1];
+                for (int zb = zb0 + 1; zb < zb1; zb++) {
+                    const unsigned om = (unsigned)(zb * g.ny);
+                    const int jm0 = tb[om + (unsigned)ys0], jm1 = tb[om + (unsigned)ys1];
                     if (kCount) n_ex += jm1 - jm0;
-                    for (int j = jm0; j < jm1; j++)
-                        pick_consider(b, a.hit_idx, urb, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
+                    for (int j = jm0; j < jm1; j++) pick_consider(b, j, true, a.hit_yz[urb + (unsigned)j], yp, zp, wy, wz);
                 }
-                li = b.j;
-                __stcs(&a.tl_rowhit[(size_t)c * (size_t)g.RP + (size_t)r], (uint16_t)li);  // -1 = kNoHit
-                if (li >= 0) {
+                if (b.tie) {  // duplicated clusters: redo the search with the complete tie rule
+                    b.j = pick_exact(tb, rowh, a.hit_idx + urb, g.ny, zb0, zb1, ys0, ys1, yp, zp, wy, wz);
+                    const float2 h = a.hit_yz[urb + (unsigned)b.j];  // a tie was between hits inside the gate: b.j >= 0
+                    b.y = h.x;
+                    b.z = h.y;
+                }
+                __stcs(&rh[r], (uint16_t)b.j);  // -1 = kNoHit
+                hit = b.j >= 0;
+                if (hit) {
                     chi2 += kf_update(st, b.y - yref, b.z - zref, g.sy2, g.sz2);
                     yref = b.y;  // the state's (y, z) frame follows the attached hit (kf_update)
                     zref = b.z;
@@ -453,18 +486,17 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 }
             }
             // bookkeeping of the step, as selects
-            const bool hit = li >= 0;
-            const bool down = mode == kDown;
             nhits += hit ? 1 : 0;
-            gap = hit ? 0 : gap + (search ? 1 : 0);
+            gap = (hit || is_back) ? 0 : gap + (search ? 1 : 0);
             first_row = (hit && down) ? r : first_row;
             last_row = (hit && !down) ? r : last_row;
             if ((hit && down) || (is_back && t_ok)) store_report(s_rep, st);  // reported state: see kDown / kBack
-            const bool stop = !t_ok || !inside || gap > g.max_gap;
-            int next;
+            // where to go next: up until the track stops or the detector ends, one step back to the start row, down
+            const bool go_on = t_ok && inside && gap <= g.max_gap && (down ? r > 0 : r + 1 < g.R);
+            const int after = down ? kDone : kBack;
+            int next = go_on ? mode : after;
             if (is_back) {
                 next = (t_ok && r0 > 0) ? kDown : kDone;
-                gap = 0;
                 if (!t_ok) {  // the back transport failed: no tracklet, an all-zero record
                     nhits = 0;
                     chi2 = yref = zref = 0.0f;
@@ -472,15 +504,11 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
 #pragma unroll
                     for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
                 }
-            } else if (down) {
-                next = (stop || r == 0) ? kDone : kDown;
-            } else {
-                next = (stop || r + 1 >= g.R) ? kBack : kUp;
             }
             mode = next;
             rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : r + 1);
+            if (mode < kDone) rb_next = a.row_offsets[slab_base + rn];  // offset of the coming row, one step ahead
         }
-        if (mode < kDone) rb_next = a.row_offsets[slab_base + rn];  // offset of the coming row, one step ahead
     }
     if (kCount) {  // work counters: warp reduction, one atomic per warp and counter
         unsigned v[4] = {n_tr, n_up, n_ex, n_se};

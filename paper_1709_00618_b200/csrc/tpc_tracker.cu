@@ -306,6 +306,10 @@ int tpc_track_on(tpc_tracker* t, void* ws, size_t ws_bytes, cudaStream_t s, bool
     if (!out || !out->counts) return fail(t, TPC_ERR_ARG, "out and out->counts are required");
     if (n_inst < 0 || n_clusters < 0 || n_clusters >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "bad sizes");
     if ((int64_t)n_inst * t->g.R + 1 >= ((int64_t)1 << 31)) return fail(t, TPC_ERR_ARG, "too many sector instances");
+    // the follower addresses the cell table by its 32-byte row units in 32 bits (a table beyond 2^32 units = 137 GB
+    // does not fit the workspace anyway)
+    if ((int64_t)n_inst * t->g.R * (t->g.nzp >> 4) >= ((int64_t)1 << 32))
+        return fail(t, TPC_ERR_ARG, "too many sector instances for this grid");
     if (n_clusters > 0 && (!clusters || n_inst == 0)) return fail(t, TPC_ERR_ARG, "NULL input");
     if (n_inst > 0 && !row_offsets) return fail(t, TPC_ERR_ARG, "row_offsets is required when n_sector_instances > 0");
     if ((uintptr_t)clusters & (uintptr_t)(layout_bytes(t->input_layout) - 1))
