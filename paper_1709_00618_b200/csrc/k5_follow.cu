@@ -32,8 +32,9 @@ constexpr int kFollowChunk = TPC_FOLLOW_CHUNK;  // candidates a warp takes from 
 constexpr int kFollowReload = TPC_FOLLOW_RELOAD;  // parked lanes that trigger a write-out / refill phase
 constexpr int kFitThreads = 128;
 #ifndef TPC_DIRECT_HITS
-#define TPC_DIRECT_HITS 3
+#define TPC_DIRECT_HITS 4
 #endif
+
 constexpr int kDirectHits = TPC_DIRECT_HITS;      // hits of a window examined in line (the rest in a loop)
 constexpr float kCellMargin = 1e-3f;  // [cm] the visited cells are a superset of the rounded fp32 gate test
 
@@ -366,12 +367,13 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     const int c = mine;
                     s_cand[threadIdx.x] = c;
                     const float4* ts = a.tl_state + c;
+                    // all loads of the hand-over in flight together (one memory round trip, then row_offsets)
                     const float4 t5 = ts[5 * cs];
+                    const float4 t0 = ts[0], t1 = ts[cs], t2 = ts[2 * cs], t3 = ts[3 * cs], t4 = ts[4 * cs];
+                    const int slab0 = a.cand_slab[c];
                     const int nbits = __float_as_int(t5.w);  // own hits | (last own row - start row) << 8
                     const int n = nbits & 0xff;
                     if (n > 0) {  // n == 0: the fit of the candidate's own hits failed, nothing to follow
-                        const float4 t0 = ts[0], t1 = ts[cs], t2 = ts[2 * cs], t3 = ts[3 * cs], t4 = ts[4 * cs];
-                        const int slab0 = a.cand_slab[c];
                         const int inst = slab0 / g.R;
                         r0 = slab0 - inst * g.R;
                         slab_base = inst * g.R;
@@ -507,7 +509,9 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             }
             mode = next;
             rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : r + 1);
-            if (mode < kDone) rb_next = a.row_offsets[slab_base + rn];  // offset of the coming row, one step ahead
+            // offset of the coming row, one step ahead.  (Prefetching the next row's cell-table entries as well --
+            // the same cell of row rn -- was measured twice and lost, +0.5 ms: the L1 data pipe is already half busy.)
+            if (mode < kDone) rb_next = a.row_offsets[slab_base + rn];
         }
     }
     if (kCount) {  // work counters: warp reduction, one atomic per warp and counter
