@@ -19,7 +19,7 @@
 #define TPC_FOLLOW_CTAS 7
 #endif
 #ifndef TPC_FOLLOW_RELOAD
-#define TPC_FOLLOW_RELOAD 4
+#define TPC_FOLLOW_RELOAD 6
 #endif
 namespace tpc {
 
