@@ -78,93 +78,81 @@ __device__ __forceinline__ void zero_tracklet(const DevGeom& g, const FollowArgs
 }
 
 // ---- fit of the candidate's own hits -----------------------------------------------------------------------------
+// The candidate's hits are staged per thread in shared memory ([hit][thread]: conflict-free) instead of register
+// arrays: the kernel is bound by the latency of the chain walk (9 dependent loads per thread), and at ~60 registers
+// twice as many warps are resident to hide it as with the hits in registers (104).
 #ifndef TPC_FIT_CTAS
-#define TPC_FIT_CTAS 4
+#define TPC_FIT_CTAS 8
 #endif
 template <bool kCount>
 __global__ void __launch_bounds__(kFitThreads, TPC_FIT_CTAS)
 fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowArgs a) {
+    __shared__ float2 s_h[kCandMax][kFitThreads];      // (y, z) of the candidate's q-th hit
+    __shared__ unsigned s_loc[kCandMax][kFitThreads];  // its position in the sorted row | pad row << 16
     const int n_cand = (int)min(a.counts[1], a.Cmax);
     const int c = blockIdx.x * kFitThreads + threadIdx.x;
+    const int t = threadIdx.x;
     unsigned n_tr = 0, n_up = 0;
     if (c < n_cand) {
         const int slab0 = a.cand_slab[c];
         const int inst = slab0 / g.R;
         const int r0 = slab0 - inst * g.R;
-        // S4 concatenation: the candidate's hits are the first <= cand_max hits of the chain of up-links that
-        // starts at its start hit (sorted global positions); the walk is 9 dependent 4-byte loads per thread
-        int pos[kCandMax];
-        pos[0] = a.cand_start[c];
-        int n = 1;
-#pragma unroll
-        for (int q = 1; q < kCandMax; q++) {
-            pos[q] = (pos[q - 1] >= 0 && q < g.cand_max) ? a.up[pos[q - 1]] : -1;
-            n += pos[q] >= 0 ? 1 : 0;
-        }
-        float2 h[kCandMax];
-        int rb[kCandMax];   // offset of the hit's row
-        int row[kCandMax];  // its pad row: consecutive, or one row skipped where S2 bridged a missing row (A2')
-        float x[kCandMax];
         const int slab_base0 = slab0 - r0;
-#pragma unroll
-        for (int q = 0; q < kCandMax; q++) {
-            h[q] = make_float2(0.0f, 0.0f);
-            rb[q] = 0;
-            row[q] = r0;
-            x[q] = 0.0f;
-            if (q < n) {
-                h[q] = a.hit_yz[pos[q]];
-                if (q == 0) {
-                    rb[q] = a.row_offsets[slab0];
-                } else {
-                    row[q] = row[q - 1] + 1;
-                    rb[q] = a.row_offsets[slab_base0 + row[q]];
-                    if (g.bridge) {
-                        const int nb2 = a.row_offsets[slab_base0 + row[q] + 1];  // row[q] + 1 <= R: a valid entry
-                        if (pos[q] >= nb2) {
-                            row[q]++;
-                            rb[q] = nb2;
-                        }
+        const bool usr = a.usr_cand_hits && c < a.usr_cand_cap;  // parity/user copy: input-order global indices
+        // S4 concatenation: the candidate's hits are the first <= cand_max hits of the chain of up-links that
+        // starts at its start hit (sorted global positions); the walk is 9 dependent 4-byte loads per thread.
+        // Consecutive pad rows, or one row skipped where S2 bridged a missing row (A2').
+        int n = 0, row = r0, rbq = a.row_offsets[slab0];
+        int pos = a.cand_start[c];
+#pragma unroll 1
+        for (int q = 0; q < kCandMax && q < g.cand_max && pos >= 0; q++) {
+            if (q > 0) {
+                row++;
+                rbq = a.row_offsets[slab_base0 + row];
+                if (g.bridge) {
+                    const int nb2 = a.row_offsets[slab_base0 + row + 1];  // row + 1 <= R: a valid entry
+                    if (pos >= nb2) {
+                        row++;
+                        rbq = nb2;
                     }
                 }
-                x[q] = g.row_x[row[q]];
             }
+            const int nxt = a.up[pos];  // next link first: the only dependent load of the walk
+            s_h[q][t] = a.hit_yz[pos];
+            s_loc[q][t] = (unsigned)(pos - rbq) | ((unsigned)row << 16);
+            if (usr) a.usr_cand_hits[(size_t)c * kCandMax + q] = rbq + (int)a.hit_idx[pos];
+            pos = nxt;
+            n = q + 1;
         }
+        if (usr)
+            for (int q = n; q < kCandMax; q++) a.usr_cand_hits[(size_t)c * kCandMax + q] = -1;
+        if (a.usr_cand_n && c < a.usr_cand_cap) a.usr_cand_n[c] = n;
         // seed from hits 0, n/2, n-1.  The state carries y and z relative to the last attached hit: the model is
         // translation invariant in y and z, so this is exact, and it keeps the fp32 rounding of the two
         // coordinates (ulp(20 cm), ulp(250 cm)) out of the state.
         const int i1 = n >> 1, i2 = n - 1;
-        float2 h1 = h[0], h2 = h[0];
-        float x1 = x[0], x2 = x[0];
-#pragma unroll
-        for (int q = 1; q < kCandMax; q++) {
-            if (q == i1) { h1 = h[q]; x1 = x[q]; }
-            if (q == i2) { h2 = h[q]; x2 = x[q]; }
-        }
-        if (a.usr_cand_hits && c < a.usr_cand_cap) {  // parity/user copy: input-order global indices
-#pragma unroll
-            for (int q = 0; q < kCandMax; q++)
-                a.usr_cand_hits[(size_t)c * kCandMax + q] = q < n ? rb[q] + (int)a.hit_idx[pos[q]] : -1;
-        }
-        if (a.usr_cand_n && c < a.usr_cand_cap) a.usr_cand_n[c] = n;
-        float yref = h[0].x, zref = h[0].y;
+        const float2 h0 = s_h[0][t], h1 = s_h[i1][t], h2 = s_h[i2][t];
+        const float x0 = g.row_x[r0], x1 = g.row_x[s_loc[i1][t] >> 16], x2 = g.row_x[s_loc[i2][t] >> 16];
+        float yref = h0.x, zref = h0.y;
         KfState st;
-        bool ok = kf_seed(st, x[0], 0.0f, 0.0f, x1, h1.x - yref, x2, h2.x - yref, h2.y - zref, g.cB, g.max_s, g.p0);
+        bool ok = kf_seed(st, x0, 0.0f, 0.0f, x1, h1.x - yref, x2, h2.x - yref, h2.y - zref, g.cB, g.max_s, g.p0);
         float chi2 = 0.0f;
         if (ok) {
-#pragma unroll
-            for (int q = 0; q < kCandMax; q++) {
-                if (q < n && ok) {
-                    if (q > 0) {
-                        ok = kf_transport(st, x[q] - x[q - 1], g.cB, g.max_s);
-                        if (kCount && ok) n_tr++;
-                    }
-                    if (ok) {
-                        chi2 += kf_update(st, h[q].x - yref, h[q].y - zref, g.sy2, g.sz2);
-                        yref = h[q].x;  // the state's (y, z) frame follows the attached hit (kf_update)
-                        zref = h[q].y;
-                        if (kCount) n_up++;
-                    }
+            float xp = x0;
+#pragma unroll 1
+            for (int q = 0; q < n && ok; q++) {
+                const float2 h = s_h[q][t];
+                if (q > 0) {
+                    const float x = g.row_x[s_loc[q][t] >> 16];
+                    ok = kf_transport(st, x - xp, g.cB, g.max_s);
+                    xp = x;
+                    if (kCount && ok) n_tr++;
+                }
+                if (ok) {
+                    chi2 += kf_update(st, h.x - yref, h.y - zref, g.sy2, g.sz2);
+                    yref = h.x;  // the state's (y, z) frame follows the attached hit (kf_update)
+                    zref = h.y;
+                    if (kCount) n_up++;
                 }
             }
         }
@@ -176,16 +164,17 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
             ts[2 * cs] = make_float4(st.c20, st.c21, st.c22, st.c30);
             ts[3 * cs] = make_float4(st.c31, st.c32, st.c33, st.c40);
             ts[4 * cs] = make_float4(st.c41, st.c42, st.c43, st.c44);
-            int span = 0;  // last own row - start row
             uint16_t* rh = a.tl_rowhit + (size_t)c * g.RP;
-#pragma unroll
-            for (int q = 0; q < kCandMax; q++)
-                if (q < n) {
-                    __stcs(&rh[row[q]], (uint16_t)(pos[q] - rb[q]));
-                    if (q > 0 && row[q] - row[q - 1] == 2) __stcs(&rh[row[q] - 1], kNoHit);  // the bridged row
-                    span = row[q] - r0;
-                }
-            ts[5 * cs] = make_float4(yref, zref, chi2, __int_as_float(n | (span << 8)));
+            int prev = r0;
+            for (int q = 0; q < n; q++) {
+                const unsigned loc = s_loc[q][t];
+                const int rq = (int)(loc >> 16);
+                __stcs(&rh[rq], (uint16_t)(loc & 0xffffu));
+                if (rq - prev == 2) __stcs(&rh[rq - 1], kNoHit);  // the bridged row
+                prev = rq;
+            }
+            // own hits | (last own row - start row) << 8
+            ts[5 * cs] = make_float4(yref, zref, chi2, __int_as_float(n | ((prev - r0) << 8)));
         } else {  // no tracklet: an all-zero record, and the follower skips the candidate
             ts[5 * cs] = make_float4(0.0f, 0.0f, 0.0f, __int_as_float(0));
             zero_tracklet(g, a, c);
