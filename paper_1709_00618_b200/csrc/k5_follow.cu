@@ -16,7 +16,7 @@
 #include "kf_math.cuh"
 
 #ifndef TPC_FOLLOW_CTAS
-#define TPC_FOLLOW_CTAS 7
+#define TPC_FOLLOW_CTAS 8
 #endif
 #ifndef TPC_FOLLOW_RELOAD
 #define TPC_FOLLOW_RELOAD 6
@@ -286,6 +286,11 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
     // values touched only in the write-out / refill phase live in shared memory, not in registers of the row loop
     __shared__ int s_cand[kFollowThreads];        // the lane's candidate id
     __shared__ int2 s_chunk[kFollowThreads / 32];  // the warp's chunk [x, y) of candidate ids
+    // lane state that is read or written once per row at most: kept out of the register file so that
+    // kFollowCtasPerSm CTAs fit (the step is bound by load latency: resident warps count)
+    __shared__ float s_z0[kFollowThreads], s_chi2[kFollowThreads];
+    __shared__ int s_r0[kFollowThreads], s_first[kFollowThreads], s_last[kFollowThreads];
+    __shared__ uint16_t* s_rh[kFollowThreads];  // the candidate's row-indexed hit table
     if (threadIdx.x < kFollowThreads / 32) s_chunk[threadIdx.x] = make_int2(0, 0);
     for (int q = threadIdx.x; q < g.R; q += kFollowThreads) {
         const float x = g.row_x[q];
@@ -301,13 +306,12 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
     // lane state
     int mode = kIdle;
     int slab_base = 0;
-    int r = 0, rn = 0, r0 = 0;  // row of the state, row of the coming step, start row
-    int nhits = 0, gap = 0, first_row = 0, last_row = 0;
-    float yref = 0.0f, zref = 0.0f, z0 = 0.0f, chi2 = 0.0f;
+    int r = 0, rn = 0;  // row of the state, row of the coming step
+    int nhits = 0, gap = 0;
+    float yref = 0.0f, zref = 0.0f;
     float xr = 0.0f;  // x of row r
     KfState st = {};
     int rb_next = 0;  // offset of row rn (loaded one step ahead)
-    uint16_t* rh = a.tl_rowhit;  // the candidate's row-indexed hit table
 
     for (;;) {
         unsigned act = __ballot_sync(full, mode < kDone);
@@ -323,8 +327,9 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 q[0] = q1.y; q[1] = q1.z; q[2] = q1.w; q[3] = q2.x; q[4] = q2.y; q[5] = q2.z; q[6] = q2.w;
                 q[7] = q3.x; q[8] = q3.y; q[9] = q3.z; q[10] = q3.w; q[11] = q4.x; q[12] = q4.y; q[13] = q4.z;
                 q[14] = q4.w;
-                a.tl_chi2[c] = chi2;
-                a.tl_rows[c] = first_row | (last_row << 8) | (first_row << 16);
+                a.tl_chi2[c] = s_chi2[threadIdx.x];
+                const int first_row = s_first[threadIdx.x];
+                a.tl_rows[c] = first_row | (s_last[threadIdx.x] << 8) | (first_row << 16);
                 a.tl_nhits[c] = nhits;
                 uint4* rec = reinterpret_cast<uint4*>(a.tl_sel + (size_t)c * g.sel_stride);
                 for (int q4i = 0; q4i < g.sel_stride / 4; q4i++) rec[q4i] = make_uint4(0u, 0u, 0u, 0u);
@@ -364,9 +369,10 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     const int n = nbits & 0xff;
                     if (n > 0) {  // n == 0: the fit of the candidate's own hits failed, nothing to follow
                         const int inst = slab0 / g.R;
-                        r0 = slab0 - inst * g.R;
+                        const int r0 = slab0 - inst * g.R;
                         slab_base = inst * g.R;
-                        z0 = grid_z0(g, inst);
+                        s_r0[threadIdx.x] = r0;
+                        s_z0[threadIdx.x] = grid_z0(g, inst);
                         st.y = t0.x; st.z = t0.y; st.s = t0.z; st.t = t0.w;
                         st.k = t1.x; st.c00 = t1.y; st.c10 = t1.z; st.c11 = t1.w;
                         st.c20 = t2.x; st.c21 = t2.y; st.c22 = t2.z; st.c30 = t2.w;
@@ -374,16 +380,17 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                         st.c41 = t4.x; st.c42 = t4.y; st.c43 = t4.z; st.c44 = t4.w;
                         yref = t5.x;
                         zref = t5.y;
-                        chi2 = t5.z;
+                        s_chi2[threadIdx.x] = t5.z;
                         nhits = n;
                         gap = 0;
-                        first_row = r0;
-                        r = last_row = r0 + (nbits >> 8);
+                        s_first[threadIdx.x] = r0;
+                        r = r0 + (nbits >> 8);
+                        s_last[threadIdx.x] = r;
                         xr = s_row[r].x;
                         mode = r + 1 < g.R ? kUp : kBack;
                         rn = mode == kUp ? r + 1 : r0;
                         rb_next = a.row_offsets[slab_base + rn];
-                        rh = a.tl_rowhit + (size_t)c * (size_t)g.RP;
+                        s_rh[threadIdx.x] = a.tl_rowhit + (size_t)c * (size_t)g.RP;
                     }
                 }
                 __syncwarp();
@@ -414,6 +421,7 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                 const float wz = fminf(g.wmax, g.gate * sqrt_fast(st.c11 + g.sz2));
                 // the cells of the gate window, widened by a margin so that they cover the rounded fp32 gate test
                 const float my = wy + kCellMargin, mz = wz + kCellMargin;
+                const float z0 = s_z0[threadIdx.x];
                 const int zb0 = zbin(zp - mz, z0, g.inv_cz, g.nz), zb1 = zbin(zp + mz, z0, g.inv_cz, g.nz);
                 const int ys0 = ybin(yp - my, rd.y, rd.z, g.ny), ys1 = ybin(yp + my, rd.y, rd.z, g.ny) + 1;
                 // cell-table entries of the window (row index in 32-byte units: n_inst * R * nzp may exceed 2^32)
@@ -467,10 +475,13 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
                     b.y = h.x;
                     b.z = h.y;
                 }
-                __stcs(&rh[r], (uint16_t)b.j);  // -1 = kNoHit
+                // (Collecting 8 rows of the table in shared memory and storing them with one 16-byte request was
+                // measured: 12.1 ms against 11.3 ms -- the 2-byte stores are not what limits the step.)
+                __stcs(&s_rh[threadIdx.x][r], (uint16_t)b.j);  // -1 = kNoHit
                 hit = b.j >= 0;
                 if (hit) {
-                    chi2 += kf_update(st, b.y - yref, b.z - zref, g.sy2, g.sz2);
+                    s_chi2[threadIdx.x] += kf_update(st, b.y - yref, b.z - zref, g.sy2, g.sz2);
+                    (down ? s_first : s_last)[threadIdx.x] = r;
                     yref = b.y;  // the state's (y, z) frame follows the attached hit (kf_update)
                     zref = b.z;
                     if (kCount) n_up++;
@@ -479,25 +490,25 @@ follow_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ FollowA
             // bookkeeping of the step, as selects
             nhits += hit ? 1 : 0;
             gap = (hit || is_back) ? 0 : gap + (search ? 1 : 0);
-            first_row = (hit && down) ? r : first_row;
-            last_row = (hit && !down) ? r : last_row;
             if ((hit && down) || (is_back && t_ok)) store_report(s_rep, st);  // reported state: see kDown / kBack
             // where to go next: up until the track stops or the detector ends, one step back to the start row, down
             const bool go_on = t_ok && inside && gap <= g.max_gap && (down ? r > 0 : r + 1 < g.R);
             const int after = down ? kDone : kBack;
             int next = go_on ? mode : after;
             if (is_back) {
-                next = (t_ok && r0 > 0) ? kDown : kDone;
+                next = (t_ok && s_r0[threadIdx.x] > 0) ? kDown : kDone;
                 if (!t_ok) {  // the back transport failed: no tracklet, an all-zero record
                     nhits = 0;
-                    chi2 = yref = zref = 0.0f;
-                    first_row = last_row = 0;
+                    yref = zref = 0.0f;
+                    s_chi2[threadIdx.x] = 0.0f;
+                    s_first[threadIdx.x] = s_last[threadIdx.x] = 0;
 #pragma unroll
                     for (int q = 0; q < 5; q++) s_rep[q][threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
                 }
             }
             mode = next;
-            rn = mode == kBack ? r0 : (mode == kDown ? r - 1 : r + 1);
+            rn = mode == kDown ? r - 1 : r + 1;
+            if (mode == kBack) rn = s_r0[threadIdx.x];
             // offset of the coming row, one step ahead.  (Prefetching the next row's cell-table entries as well --
             // the same cell of row rn -- was measured twice and lost, +0.5 ms: the L1 data pipe is already half busy.)
             if (mode < kDone) rb_next = a.row_offsets[slab_base + rn];
