@@ -8,10 +8,9 @@
 // pre-rounded bounds, and the minimum is taken over (D, u, d) lexicographically, so the result does not depend on
 // the order in which the grid presents the hits.  This file is additionally compiled with -fmad=false.
 //
-// One CTA per (sector instance, segment of TPC_NB_SEG_ROWS pad rows; default one row).  The sorted (y,z) and the cell
-// tables of the rows it touches are brought into shared memory by 1-D bulk copies (TMA) completing on mbarriers -- one
-// elected thread issues them, nobody spends instructions on staging; rows or tables too long for the buffers are read
-// in place.  Per hit the search is two flat loops: the window hits of row r-1 (a handful, through the 2-D grid) are
+// One CTA per (sector instance, pad row).  The sorted (y,z) and the cell tables of the rows it touches are brought
+// into shared memory by 1-D bulk copies (TMA) completing on an mbarrier -- one elected thread issues them, nobody
+// spends instructions on staging; rows or tables too long for the buffers are read in place.  Per hit the search is two flat loops: the window hits of row r-1 (a handful, through the 2-D grid) are
 // collected in registers, then every window hit of row r+1 is paired with them.
 #include "tpc_common.cuh"
 
@@ -21,9 +20,6 @@ namespace tpc {
 #define TPC_NB_THREADS 96  // measured: 64 -> 4.65, 96 -> 4.17, 128 -> 4.31, 192 -> 5.23, 256 -> 5.79 ms on the bench workload
 #endif
 constexpr int kNbThreads = TPC_NB_THREADS;
-#ifndef TPC_NB_SEG_ROWS
-#define TPC_NB_SEG_ROWS 1  // measured on the bench workload: 1 -> 4.09, 2 -> 4.16, 4 -> 4.11, 8 -> 4.18, 16 -> 4.51 ms
-#endif
 #ifndef TPC_NB_STAGE_HITS
 #define TPC_NB_STAGE_HITS 382
 #endif
@@ -520,21 +516,20 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
                  : "memory");
 }
 
-// One CTA walks kNbSegRows consecutive pad rows of one sector instance.  The cell table and the sorted hits of every
-// row it touches (its rows plus one halo row on either side) pass through a ring of four shared-memory buffers,
-// filled by 1-D bulk copies (TMA) that one thread issues two rows ahead: a row is fetched once per segment instead of
-// three times (as the row above, the row itself and the row below), and the fetch overlaps the search of the rows
-// before it.  Rows longer than the buffer (cap_hits) and tables beyond kNbStageTbl entries are read in place.
+// One CTA per (sector instance, pad row) slab.  The cell tables and the sorted hits of the rows r-1, r and r+1 come
+// into shared memory by 1-D bulk copies (TMA) that one thread issues, all completing on one mbarrier: nobody spends
+// instructions on staging (15 % of the kernel's instructions when every thread copied its share), and the copies of
+// one CTA overlap the search of the others on the SM.  Rows longer than the buffer (cap_hits) and tables beyond
+// kNbStageTbl entries are read in place.  (A CTA walking a segment of 2..16 consecutive rows through a ring of
+// buffers, each row fetched once instead of three times, was measured too: 4.11-4.51 ms against 4.09 ms -- the
+// per-row barrier costs more than the L2 reads it saves.)
 #ifndef TPC_NB_CTAS
 #define TPC_NB_CTAS 10  // resident CTAs per SM the register allocation aims at (64 registers; 13 -> 4.12 ms, 10 -> 4.09 ms)
 #endif
-constexpr int kNbSegRows = TPC_NB_SEG_ROWS;
-constexpr int kNbRing = kNbSegRows == 1 ? 3 : 4;
-
 struct NbSmem {
     int tbl_bytes;  // bytes of one staged cell table (0 = tables are read in place)
     int cap_hits;   // hits of a row that fit its buffer
-    int buf_bytes;  // one ring buffer: table, then (cap_hits + 2) hits (a copy may start 8 bytes before the row)
+    int buf_bytes;  // one row buffer: table, then (cap_hits + 2) hits (a copy may start 8 bytes before the row)
 };
 
 template <bool kUniform>
@@ -542,81 +537,64 @@ __global__ void __launch_bounds__(kNbThreads, TPC_NB_CTAS)
 neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__ row_offsets,
                   const float2* __restrict__ hit_yz, const uint16_t* __restrict__ hit_idx,
                   const uint16_t* __restrict__ bin_start, int32_t* __restrict__ link_up,
-                  int32_t* __restrict__ link_dn, const int segs_per_inst, const NbSmem sm) {
+                  int32_t* __restrict__ link_dn, const NbSmem sm) {
     extern __shared__ __align__(128) unsigned char sm_raw[];
-    __shared__ __align__(8) unsigned long long s_bar[kNbRing];
-    __shared__ int s_off[kNbSegRows + 4];  // row_offsets of rows ra-1 .. rb+1
-    const int inst = blockIdx.x / segs_per_inst, seg = blockIdx.x - inst * segs_per_inst;
-    const int slab0 = inst * g.R;
-    const int ra = 1 + seg * kNbSegRows, rb = min(ra + kNbSegRows, g.R - 1);  // this CTA's rows: ra .. rb-1
-    // rows 0 and R-1 never own links (reading A6): written by the first / last segment of the instance
-    if (seg == 0) {
-        const int b0 = row_offsets[slab0], b1 = row_offsets[slab0 + 1];
-        for (int i = b0 + threadIdx.x; i < b1; i += kNbThreads) link_up[i] = link_dn[i] = -1;
+    __shared__ __align__(8) unsigned long long s_bar;
+    const int slab = blockIdx.x;
+    const int inst = slab / g.R, r = slab - inst * g.R;
+    const int base = row_offsets[slab];
+    const int n_all = row_offsets[slab + 1] - base;
+    const int n = min(n_all, 65535);
+    // hits beyond the 16-bit limit were not binned (error flag set by S1): they own no links
+    for (int i = n + threadIdx.x; i < n_all; i += kNbThreads) link_up[base + i] = link_dn[base + i] = -1;
+    if (r == 0 || r == g.R - 1) {  // first and last row never own links (reading A6)
+        for (int i = threadIdx.x; i < n; i += kNbThreads) link_up[base + i] = link_dn[base + i] = -1;
+        return;
     }
-    if (seg == segs_per_inst - 1 && g.R > 1) {
-        const int b0 = row_offsets[slab0 + g.R - 1], b1 = row_offsets[slab0 + g.R];
-        for (int i = b0 + threadIdx.x; i < b1; i += kNbThreads) link_up[i] = link_dn[i] = -1;
-    }
-    if (ra >= rb) return;
-    for (int q = threadIdx.x; q <= rb - ra + 2; q += kNbThreads) s_off[q] = row_offsets[slab0 + ra - 1 + q];
+    if (n == 0) return;
+    const int base_dn = row_offsets[slab - 1], base_up = row_offsets[slab + 1];
+    const int n_dn = min(base - base_dn, 65535), n_up = min(row_offsets[slab + 2] - base_up, 65535);
+    // row q = r - 1 + k (k = 0, 1, 2) lives in buffer k
+    const int off3[3] = {base_dn, base, base_up};
+    const int cnt3[3] = {n_dn, n, n_up};
     if (threadIdx.x == 0) {
-        for (int q = 0; q < kNbRing; q++) mbar_init(&s_bar[q], 1);
+        mbar_init(&s_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    const float z0 = grid_z0(g, inst);
-    // row q (ra-1 <= q <= rb) lives in ring buffer (q - ra + 1) % kNbRing
-    auto off_of = [&](int q) { return s_off[q - ra + 1]; };
-    auto hits_of = [&](int q) { return min(s_off[q - ra + 2] - s_off[q - ra + 1], 65535); };
-    auto buf_of = [&](int q) { return sm_raw + (size_t)((q - ra + 1) % kNbRing) * sm.buf_bytes; };
-    auto stage = [&](int q) {  // one thread: start the copies of row q
-        unsigned long long* bar = &s_bar[(q - ra + 1) % kNbRing];
-        unsigned char* buf = buf_of(q);
-        const int n = hits_of(q);
-        const float2* src = hit_yz + off_of(q);
-        const unsigned lead = (unsigned)((uintptr_t)src & 15u);  // 0 or 8: the copy starts at the 16-byte line
-        const unsigned hbytes = (n > 0 && n <= sm.cap_hits) ? (((unsigned)n * 8u + lead + 15u) & ~15u) : 0u;
-        mbar_expect_tx(bar, (unsigned)sm.tbl_bytes + hbytes);
-        if (sm.tbl_bytes) bulk_g2s(buf, bin_start + (size_t)(slab0 + q) * g.nzp, (unsigned)sm.tbl_bytes, bar);
-        if (hbytes) bulk_g2s(buf + sm.tbl_bytes, reinterpret_cast<const unsigned char*>(src) - lead, hbytes, bar);
-    };
-    auto view = [&](int q) {
-        unsigned char* buf = buf_of(q);
-        const int n = hits_of(q);
-        const float2* src = hit_yz + off_of(q);
-        const unsigned lead = (unsigned)((uintptr_t)src & 15u);
-        RowView v;
-        v.yz = (n <= sm.cap_hits) ? reinterpret_cast<const float2*>(buf + sm.tbl_bytes + lead) : src;
-        v.idx = hit_idx + off_of(q);
-        v.tbl = sm.tbl_bytes ? reinterpret_cast<const uint16_t*>(buf) : bin_start + (size_t)(slab0 + q) * g.nzp;
-        v.y0 = g.row_y0[q];
-        v.inv_sy = g.row_inv_sy[q];
-        return v;
-    };
-    if (threadIdx.x == 0) {
-        stage(ra - 1);
-        stage(ra);
-        stage(ra + 1);  // ra + 1 <= rb
-    }
-    for (int r = ra; r < rb; r++) {
-        // rows r-1, r, r+1 are needed; r+1 is the newest copy (the first iteration waits for all three)
-        if (r == ra) {
-            mbar_wait(&s_bar[0], 0u);
-            mbar_wait(&s_bar[1], 0u);
+        unsigned bytes = 0;
+        unsigned hb[3], lead[3];
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            lead[k] = (unsigned)((uintptr_t)(hit_yz + off3[k]) & 15u);  // 0 or 8: the copy starts at the 16-byte line
+            hb[k] = (cnt3[k] > 0 && cnt3[k] <= sm.cap_hits) ? (((unsigned)cnt3[k] * 8u + lead[k] + 15u) & ~15u) : 0u;
+            bytes += hb[k] + (k != 1 ? (unsigned)sm.tbl_bytes : 0u);  // the own row's table is not needed
         }
-        mbar_wait(&s_bar[(r - ra + 2) % kNbRing], (unsigned)(((r - ra + 2) / kNbRing) & 1));
-        __syncthreads();  // every thread is done with row r-1, so the buffer of row r-2 may be overwritten
-        if (threadIdx.x == 0 && r + 2 <= rb) stage(r + 2);
-        const int base = off_of(r);
-        const int n_all = s_off[r - ra + 2] - base;
-        const int n = min(n_all, 65535);
-        // hits beyond the 16-bit limit were not binned (error flag set by S1): they own no links
-        for (int i = n + threadIdx.x; i < n_all; i += kNbThreads) link_up[base + i] = link_dn[base + i] = -1;
-        if (n == 0) continue;
-        const RowView up = view(r + 1), dn = view(r - 1), me = view(r);
-        search_row<kUniform>(g, up, dn, me.yz, n, r, z0, base, off_of(r + 1), off_of(r - 1), link_up, link_dn);
+        mbar_expect_tx(&s_bar, bytes);
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            unsigned char* buf = sm_raw + (size_t)k * sm.buf_bytes;
+            if (k != 1 && sm.tbl_bytes)
+                bulk_g2s(buf, bin_start + (size_t)(slab - 1 + k) * g.nzp, (unsigned)sm.tbl_bytes, &s_bar);
+            if (hb[k])
+                bulk_g2s(buf + sm.tbl_bytes, reinterpret_cast<const unsigned char*>(hit_yz + off3[k]) - lead[k], hb[k],
+                         &s_bar);
+        }
     }
+    __syncthreads();  // the barrier is initialised before anybody waits on it
+    const float z0 = grid_z0(g, inst);
+    RowView v[3];
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        unsigned char* buf = sm_raw + (size_t)k * sm.buf_bytes;
+        const float2* src = hit_yz + off3[k];
+        const unsigned lead = (unsigned)((uintptr_t)src & 15u);
+        v[k].yz = (cnt3[k] <= sm.cap_hits) ? reinterpret_cast<const float2*>(buf + sm.tbl_bytes + lead) : src;
+        v[k].idx = hit_idx + off3[k];
+        v[k].tbl = sm.tbl_bytes ? reinterpret_cast<const uint16_t*>(buf) : bin_start + (size_t)(slab - 1 + k) * g.nzp;
+        v[k].y0 = g.row_y0[r - 1 + k];
+        v[k].inv_sy = g.row_inv_sy[r - 1 + k];
+    }
+    mbar_wait(&s_bar, 0u);
+    search_row<kUniform>(g, v[2], v[0], v[1].yz, n, r, z0, base, base_up, base_dn, link_up, link_dn);
 }
 
 // Class 1 (reading A2', nf_bridge_rows = 1) as its own pass: one WARP per (instance,row) slab reads the row's raw
@@ -696,14 +674,13 @@ int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cu
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
     const NbSmem m = nb_smem(g);
-    const int segs = g.R > 2 ? div_up(g.R - 2, kNbSegRows) : 1;
-    const size_t smem = (size_t)m.buf_bytes * kNbRing;
+    const size_t smem = (size_t)m.buf_bytes * 3;
     if (g.uniform_pitch)
-        neighbours_kernel<true><<<p.n_inst * segs, kNbThreads, smem, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
-                                                                          w.bin_start, w.up_raw, w.dn_raw, segs, m);
+        neighbours_kernel<true><<<slabs, kNbThreads, smem, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
+                                                                w.up_raw, w.dn_raw, m);
     else
-        neighbours_kernel<false><<<p.n_inst * segs, kNbThreads, smem, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
-                                                                           w.bin_start, w.up_raw, w.dn_raw, segs, m);
+        neighbours_kernel<false><<<slabs, kNbThreads, smem, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
+                                                                 w.up_raw, w.dn_raw, m);
     if (g.bridge) {  // class 1 (reading A2'): a second, light pass over the hits that found no adjacent pair
         bridge_links_kernel<<<div_up(slabs, kBrThreads / 32), kBrThreads, 0, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx,
                                                                                   w.bin_start, w.up_raw, w.dn_raw, slabs);
