@@ -524,13 +524,18 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
 // buffers, each row fetched once instead of three times, was measured too: 4.11-4.51 ms against 4.09 ms -- the
 // per-row barrier costs more than the L2 reads it saves.)
 #ifndef TPC_NB_CTAS
-#define TPC_NB_CTAS 10  // resident CTAs per SM the register allocation aims at (64 registers; 13 -> 4.12 ms, 10 -> 4.09 ms)
+#define TPC_NB_CTAS 12  // resident CTAs per SM the register allocation aims at; measured 8 -> 4.09, 10 -> 3.90, 12 -> 3.87, 13 -> 3.97 ms
 #endif
 struct NbSmem {
     int tbl_bytes;  // bytes of one staged cell table (0 = tables are read in place)
     int cap_hits;   // hits of a row that fit its buffer
-    int buf_bytes;  // one row buffer: table, then (cap_hits + 2) hits (a copy may start 8 bytes before the row)
+    int buf_bytes;  // buffer of a neighbour row: table, then (cap_hits + 2) hits (a copy may start 8 bytes before the row)
+    int own_bytes;  // buffer of the own row: hits only
 };
+// buffers in shared memory: row r-1 | row r (hits only) | row r+1
+__device__ __forceinline__ unsigned char* nb_buf(unsigned char* base, const NbSmem& sm, int k) {
+    return base + (k == 0 ? 0 : (k == 1 ? sm.buf_bytes : sm.buf_bytes + sm.own_bytes));
+}
 
 template <bool kUniform>
 __global__ void __launch_bounds__(kNbThreads, TPC_NB_CTAS)
@@ -571,11 +576,11 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
         mbar_expect_tx(&s_bar, bytes);
 #pragma unroll
         for (int k = 0; k < 3; k++) {
-            unsigned char* buf = sm_raw + (size_t)k * sm.buf_bytes;
+            unsigned char* buf = nb_buf(sm_raw, sm, k);
             if (k != 1 && sm.tbl_bytes)
                 bulk_g2s(buf, bin_start + (size_t)(slab - 1 + k) * g.nzp, (unsigned)sm.tbl_bytes, &s_bar);
             if (hb[k])
-                bulk_g2s(buf + sm.tbl_bytes, reinterpret_cast<const unsigned char*>(hit_yz + off3[k]) - lead[k], hb[k],
+                bulk_g2s(buf + (k != 1 ? sm.tbl_bytes : 0), reinterpret_cast<const unsigned char*>(hit_yz + off3[k]) - lead[k], hb[k],
                          &s_bar);
         }
     }
@@ -584,10 +589,10 @@ neighbours_kernel(const __grid_constant__ DevGeom g, const int32_t* __restrict__
     RowView v[3];
 #pragma unroll
     for (int k = 0; k < 3; k++) {
-        unsigned char* buf = sm_raw + (size_t)k * sm.buf_bytes;
+        unsigned char* buf = nb_buf(sm_raw, sm, k);
         const float2* src = hit_yz + off3[k];
         const unsigned lead = (unsigned)((uintptr_t)src & 15u);
-        v[k].yz = (cnt3[k] <= sm.cap_hits) ? reinterpret_cast<const float2*>(buf + sm.tbl_bytes + lead) : src;
+        v[k].yz = (cnt3[k] <= sm.cap_hits) ? reinterpret_cast<const float2*>(buf + (k != 1 ? sm.tbl_bytes : 0) + lead) : src;
         v[k].idx = hit_idx + off3[k];
         v[k].tbl = sm.tbl_bytes ? reinterpret_cast<const uint16_t*>(buf) : bin_start + (size_t)(slab - 1 + k) * g.nzp;
         v[k].y0 = g.row_y0[r - 1 + k];
@@ -667,6 +672,7 @@ static NbSmem nb_smem(const DevGeom& g) {
     m.tbl_bytes = g.nzp <= kNbStageTbl ? g.nzp * 2 : 0;  // nzp is a multiple of 16 entries
     m.cap_hits = kNbStageHits;
     m.buf_bytes = (m.tbl_bytes + (m.cap_hits + 2) * 8 + 127) & ~127;
+    m.own_bytes = ((m.cap_hits + 2) * 8 + 127) & ~127;
     return m;
 }
 
@@ -674,7 +680,7 @@ int launch_neighbours(const DevGeom& g, const Workspace& w, const Problem& p, cu
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
     const NbSmem m = nb_smem(g);
-    const size_t smem = (size_t)m.buf_bytes * 3;
+    const size_t smem = (size_t)m.buf_bytes * 2 + m.own_bytes;
     if (g.uniform_pitch)
         neighbours_kernel<true><<<slabs, kNbThreads, smem, s>>>(g, p.row_offsets, w.hit_yz, w.hit_idx, w.bin_start,
                                                                 w.up_raw, w.dn_raw, m);
