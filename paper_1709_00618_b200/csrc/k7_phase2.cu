@@ -39,6 +39,8 @@ struct P2Args {
     int4* p2_info;
     float2* p2_last;
     int32_t* p2_first;
+    int32_t* p2_rowstart;
+    int32_t* p2_sorted;
     unsigned long long* p2_best_prev;
     int32_t* p2_best_next;
     int32_t* p2_next;
@@ -186,60 +188,106 @@ inst_first_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2A
     a.p2_first[i] = (int32_t)lo;
 }
 
-// One WARP per track A: the lanes scan the tracks of a neighbouring sector instance 32 at a time (coalesced reads of
-// their rows), and only the few that pass the integer pre-filter pay for the extrapolation.
+// Index for the matching: per sector instance the fitted tracks ordered by their first row (counting sort in shared
+// memory, one CTA per instance).  A track can only be continued by tracks that begin in the kMergeGap rows after its
+// last row, so the matching reads that slice instead of all tracks of the neighbouring sectors.  The order inside a
+// row's bucket is not defined; the matching does not depend on it (minimum over (distance, track index)).
+__global__ void __launch_bounds__(kP2Threads)
+index_tracks_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Args a) {
+    __shared__ int s_cnt[kMaxRows + 2];
+    const int inst = blockIdx.x;
+    const int t0 = a.p2_first[inst], t1 = a.p2_first[inst + 1];
+    for (int r = threadIdx.x; r <= g.R; r += kP2Threads) s_cnt[r] = 0;
+    __syncthreads();
+    for (int t = t0 + threadIdx.x; t < t1; t += kP2Threads) {
+        const int4 it = a.p2_info[t];
+        if (it.x) atomicAdd(&s_cnt[it.y], 1);
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {  // exclusive scan of the R counts by one warp; s_cnt[r] becomes the bucket's start
+        int carry = 0;
+        for (int r0 = 0; r0 <= g.R; r0 += 32) {
+            const int r = r0 + threadIdx.x;
+            const int v = r < g.R ? s_cnt[r] : 0;
+            int x = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, x, d);
+                if ((int)threadIdx.x >= d) x += y;
+            }
+            if (r <= g.R) {
+                s_cnt[r] = carry + x - v;
+                a.p2_rowstart[(size_t)inst * (g.R + 1) + r] = t0 + carry + x - v;
+            }
+            carry += __shfl_sync(0xffffffffu, x, 31);
+        }
+    }
+    __syncthreads();
+    for (int t = t0 + threadIdx.x; t < t1; t += kP2Threads) {
+        const int4 it = a.p2_info[t];
+        if (it.x) a.p2_sorted[t0 + atomicAdd(&s_cnt[it.y], 1)] = t;
+    }
+}
+
+// One WARP per track A (grid-stride): the lanes read the tracks of a neighbouring sector instance that begin in the
+// kMergeGap rows after A's last row (index_tracks_kernel), 32 at a time, and those pay for the extrapolation.
 __global__ void __launch_bounds__(kP2Threads)
 match_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Args a) {
     const int64_t n_trk = min(a.counts[3], a.Tmax);
     const int lane = threadIdx.x & 31;
-    const int64_t ta = (int64_t)blockIdx.x * (kP2Threads / 32) + (threadIdx.x >> 5);
-    if (ta >= n_trk) return;
-    const int4 ia = a.p2_info[ta];
-    const int la = ia.z;
-    if (ia.w < 1 || la >= g.R - 1) return;  // reaches the last pad row: nothing can continue it (warp-uniform)
-    const int inst = track_inst(g, a, ta);
-    const int window = (inst + g.inst_phase) / g.spe, sec = (inst + g.inst_phase) % g.spe;
-    const int side = sec >= g.spe_half ? 1 : 0, phi = sec % g.spe_half;
-    const float2 ha = a.p2_last[ta];
-    const float xa = g.row_x[la];
-    float best_d2 = __int_as_float(0x7f800000);
-    int best_b = 0x7fffffff;
-    // the two neighbouring sectors of the same side and window.  Rotation from B's frame into A's: by -2h when B is
-    // the next sector in azimuth (dir = +1), by +2h when it is the previous one.
-    for (int dir = -1; dir <= 1; dir += 2) {
-        const int phi_b = (phi + dir + g.spe_half) % g.spe_half;
-        const int inst_b = window * g.spe + side * g.spe_half + phi_b - g.inst_phase;
-        if (inst_b < 0 || inst_b >= a.n_inst) continue;  // the neighbour is not part of this call (chunked jobs)
-        const float sa = dir > 0 ? -g.sin_2h : g.sin_2h;
-        const int t_end = a.p2_first[inst_b + 1];
-        for (int tb = a.p2_first[inst_b] + lane; tb < t_end; tb += 32) {
-            const int4 ib = a.p2_info[tb];
-            if (!(ib.x && ib.y > la && ib.y - la <= kMergeGap)) continue;
-            KfState st;
-            const float* p = a.p2_par + (size_t)tb * 5;
-            const float* q = a.p2_cov + (size_t)tb * 15;
-            st.y = p[0]; st.z = p[1]; st.s = p[2]; st.t = p[3]; st.k = p[4];
-            st.c00 = q[0]; st.c10 = q[1]; st.c11 = q[2]; st.c20 = q[3]; st.c21 = q[4]; st.c22 = q[5]; st.c30 = q[6];
-            st.c31 = q[7]; st.c32 = q[8]; st.c33 = q[9]; st.c40 = q[10]; st.c41 = q[11]; st.c42 = q[12]; st.c43 = q[13];
-            st.c44 = q[14];
-            float xr;
-            if (!kf_rotate(st, st.y, g.row_x[ib.y], g.cos_2h, sa, g.cB, g.max_s, xr)) continue;
-            if (!kf_transport(st, xa - xr, g.cB, g.max_s)) continue;
-            const float dy = st.y - ha.x, dz = st.z - ha.y;
-            if (!(fabsf(dy) <= kMergeCut && fabsf(dz) <= kMergeCut)) continue;
-            const float d2 = dy * dy + dz * dz;
-            if (d2 < best_d2 || (d2 == best_d2 && tb < best_b)) { best_d2 = d2; best_b = tb; }
-            atomicMin(&a.p2_best_prev[tb], ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned long long)ta);
+    const int64_t n_warps = (int64_t)gridDim.x * (kP2Threads / 32);
+    for (int64_t ta = (int64_t)blockIdx.x * (kP2Threads / 32) + (threadIdx.x >> 5); ta < n_trk; ta += n_warps) {
+        const int4 ia = a.p2_info[ta];
+        const int la = ia.z;
+        if (ia.w < 1 || la >= g.R - 1) continue;  // reaches the last pad row: nothing can continue it (warp-uniform)
+        const int inst = track_inst(g, a, ta);
+        const int window = (inst + g.inst_phase) / g.spe, sec = (inst + g.inst_phase) % g.spe;
+        const int side = sec >= g.spe_half ? 1 : 0, phi = sec % g.spe_half;
+        const float2 ha = a.p2_last[ta];
+        const float xa = g.row_x[la];
+        const int row_hi = min(la + kMergeGap, g.R - 1);  // last row a continuation may begin in
+        float best_d2 = __int_as_float(0x7f800000);
+        int best_b = 0x7fffffff;
+        // the two neighbouring sectors of the same side and window.  Rotation from B's frame into A's: by -2h when B
+        // is the next sector in azimuth (dir = +1), by +2h when it is the previous one.
+        for (int dir = -1; dir <= 1; dir += 2) {
+            const int phi_b = (phi + dir + g.spe_half) % g.spe_half;
+            const int inst_b = window * g.spe + side * g.spe_half + phi_b - g.inst_phase;
+            if (inst_b < 0 || inst_b >= a.n_inst) continue;  // the neighbour is not part of this call (chunked jobs)
+            const float sa = dir > 0 ? -g.sin_2h : g.sin_2h;
+            const int32_t* rs = a.p2_rowstart + (size_t)inst_b * (g.R + 1);
+            const int k_end = rs[row_hi + 1];
+            for (int k = rs[la + 1] + lane; k < k_end; k += 32) {
+                const int tb = a.p2_sorted[k];
+                const int4 ib = a.p2_info[tb];
+                if (!(ib.x && ib.y > la && ib.y - la <= kMergeGap)) continue;  // holds by construction of the slice
+                KfState st;
+                const float* p = a.p2_par + (size_t)tb * 5;
+                const float* q = a.p2_cov + (size_t)tb * 15;
+                st.y = p[0]; st.z = p[1]; st.s = p[2]; st.t = p[3]; st.k = p[4];
+                st.c00 = q[0]; st.c10 = q[1]; st.c11 = q[2]; st.c20 = q[3]; st.c21 = q[4]; st.c22 = q[5];
+                st.c30 = q[6]; st.c31 = q[7]; st.c32 = q[8]; st.c33 = q[9]; st.c40 = q[10]; st.c41 = q[11];
+                st.c42 = q[12]; st.c43 = q[13]; st.c44 = q[14];
+                float xr;
+                if (!kf_rotate(st, st.y, g.row_x[ib.y], g.cos_2h, sa, g.cB, g.max_s, xr)) continue;
+                if (!kf_transport(st, xa - xr, g.cB, g.max_s)) continue;
+                const float dy = st.y - ha.x, dz = st.z - ha.y;
+                if (!(fabsf(dy) <= kMergeCut && fabsf(dz) <= kMergeCut)) continue;
+                const float d2 = dy * dy + dz * dz;
+                if (d2 < best_d2 || (d2 == best_d2 && tb < best_b)) { best_d2 = d2; best_b = tb; }
+                atomicMin(&a.p2_best_prev[tb], ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned long long)ta);
+            }
         }
-    }
-    // nearest over the lanes; an exact tie of d2 goes to the lower track index
-    unsigned long long key = ((unsigned long long)__float_as_uint(best_d2) << 32) | (unsigned)best_b;
+        // nearest over the lanes; an exact tie of d2 goes to the lower track index
+        unsigned long long key = ((unsigned long long)__float_as_uint(best_d2) << 32) | (unsigned)best_b;
 #pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) {
-        const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
-        key = other < key ? other : key;
+        for (int o = 16; o >= 1; o >>= 1) {
+            const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
+            key = other < key ? other : key;
+        }
+        if (lane == 0)
+            a.p2_best_next[ta] = (unsigned)(key & 0xffffffffull) == 0x7fffffffu ? -1 : (int)(key & 0xffffffffull);
     }
-    if (lane == 0) a.p2_best_next[ta] = (unsigned)(key & 0xffffffffull) == 0x7fffffffu ? -1 : (int)(key & 0xffffffffull);
 }
 
 __global__ void __launch_bounds__(kP2Threads)
@@ -396,13 +444,15 @@ int launch_phase2(const DevGeom& g, const Workspace& w, const Problem& p, const 
     if (p.n_clusters > 0) {
         const P2Args a{p.row_offsets, w.hit_yz,     w.cand_slab,    w.tl_rowhit,    w.tl_sel,  w.trk_cand, w.counts,
                        w.Tmax,        w.p2_par,     w.p2_cov,       w.p2_chi2,      w.p2_info, w.p2_last,  w.p2_first,
-                       w.p2_best_prev, w.p2_best_next, w.p2_next,   w.p2_prev,      w.p2_part, w.p2_chain, w.p2_counts, p.n_inst};
+                       w.p2_rowstart, w.p2_sorted, w.p2_best_prev, w.p2_best_next, w.p2_next,   w.p2_prev,      w.p2_part, w.p2_chain, w.p2_counts, p.n_inst};
         // the track count lives on the device: grids are sized by its bound and bounded by it inside
         const int64_t tb = div_up(w.Tmax, kP2Threads);
         const int grid_t = (int)(tb < 148 * 64 ? tb : 148 * 64);
         refit_tracks_kernel<<<grid_t, kP2Threads, 0, s>>>(g, a);
         inst_first_kernel<<<div_up((int64_t)p.n_inst + 1, kP2Threads), kP2Threads, 0, s>>>(g, a);
-        match_kernel<<<(unsigned)div_up(w.Tmax, kP2Threads / 32), kP2Threads, 0, s>>>(g, a);
+        index_tracks_kernel<<<p.n_inst, kP2Threads, 0, s>>>(g, a);
+        const int64_t mb = div_up(w.Tmax, kP2Threads / 32);
+        match_kernel<<<(int)(mb < 148 * 16 ? mb : 148 * 16), kP2Threads, 0, s>>>(g, a);
         link_kernel<<<(unsigned)tb, kP2Threads, 0, s>>>(a);
         const int64_t hb = div_up(w.Tmax, 256);
         const int grid_h = (int)(hb < 148 * 16 ? hb : 148 * 16);
@@ -411,7 +461,7 @@ int launch_phase2(const DevGeom& g, const Workspace& w, const Problem& p, const 
         merged_out_kernel<<<grid_h, 256, 0, s>>>(g, a, o);
         const int64_t cb = div_up(w.Tmax / 2 + 1, kP2Threads);
         chain_fit_kernel<<<(int)(cb < 148 * 64 ? cb : 148 * 64), kP2Threads, 0, s>>>(g, a, o);
-        launches += 8;
+        launches += 9;
     }
     p2_counts_kernel<<<1, 32, 0, s>>>(w.p2_counts, o.counts2);
     return launches + 1;

@@ -89,6 +89,8 @@ struct Workspace {
     int4* p2_info;        // [Tmax] ok, first row, last row, kept hits
     float2* p2_last;      // [Tmax] (y, z) of the outermost kept hit
     int32_t* p2_first;    // [S + 1] first track of every sector instance
+    int32_t* p2_rowstart; // [S][R + 1] per sector instance: start in p2_sorted of the fitted tracks that begin in row r
+    int32_t* p2_sorted;   // [Tmax] fitted tracks of every sector instance, ordered by their first row
     unsigned long long* p2_best_prev;  // [Tmax] (d2 bits << 32 | predecessor) minimum, ~0 = none
     int32_t* p2_best_next;             // [Tmax]
     int32_t* p2_next;     // [Tmax] links (reading M3)

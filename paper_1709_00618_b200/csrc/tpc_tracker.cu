@@ -215,6 +215,8 @@ size_t carve(const DevGeom& g, void* base, int64_t N, int64_t S, Workspace* w) {
     v.p2_info = c.take<int4>(tmax);
     v.p2_last = c.take<float2>(tmax);
     v.p2_first = c.take<int32_t>((size_t)(S > 0 ? S : 1) + 1);
+    v.p2_rowstart = c.take<int32_t>((size_t)(S > 0 ? S : 1) * ((size_t)g.R + 1));
+    v.p2_sorted = c.take<int32_t>(tmax);
     v.p2_best_prev = c.take<unsigned long long>(tmax);
     v.p2_best_next = c.take<int32_t>(tmax);
     v.p2_next = c.take<int32_t>(tmax);

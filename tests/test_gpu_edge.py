@@ -200,11 +200,22 @@ def test_full_size_central_event_against_oracle():
 
 
 def test_dense_rows_unstaged_neighbour_search():
-    """Rows of 700-1000 hits (2,000 tracks in one sector): rows r-1 and r+1 together exceed the 1,024 hits S2 stages
-    in shared memory, so the neighbour rows are read in place; more than two hits per thread in S1."""
+    """Rows of 700-1000 hits (2,000 tracks in one sector): every row exceeds the 382 hits of S2's shared-memory row
+    buffers, so all three rows of a slab are read in place; more than two hits per thread in S1."""
     ev = dg.single_sector(seed=1031, n_tracks=2000)
     n_row = np.diff(ev.row_offsets)
     assert (n_row[:-2] + n_row[2:]).max() > 1024 and n_row.max() > 600
+    _check(ev)
+
+
+def test_rows_around_the_staging_buffer_size():
+    """1,000 tracks in one sector: 44 rows above and 115 rows below the 382 hits of S2's row buffers, so slabs mix rows
+    that arrive by bulk copy with rows read in place (own row, row above, row below in every combination)."""
+    ev = dg.single_sector(seed=1032, n_tracks=1000)
+    n_row = np.diff(ev.row_offsets)
+    big = n_row > 382
+    assert big.sum() > 20 and (~big).sum() > 20
+    assert (big[1:] != big[:-1]).any()  # at least one staged row next to an unstaged one
     _check(ev)
 
 
