@@ -90,10 +90,11 @@ fit_candidates_kernel(const __grid_constant__ DevGeom g, const __grid_constant__
     __shared__ float2 s_h[kCandMax][kFitThreads];      // (y, z) of the candidate's q-th hit
     __shared__ unsigned s_loc[kCandMax][kFitThreads];  // its position in the sorted row | pad row << 16
     const int n_cand = (int)min(a.counts[1], a.Cmax);
-    const int c = blockIdx.x * kFitThreads + threadIdx.x;
     const int t = threadIdx.x;
     unsigned n_tr = 0, n_up = 0;
-    if (c < n_cand) {
+    // grid-stride: the candidate count is only known on the device, and a grid sized by its bound (N / 4) would be
+    // four fifths empty CTAs
+    for (int c = blockIdx.x * kFitThreads + t; c < n_cand; c += gridDim.x * kFitThreads) {
         const int slab0 = a.cand_slab[c];
         const int inst = slab0 / g.R;
         const int r0 = slab0 - inst * g.R;
@@ -534,7 +535,8 @@ int launch_fit(const DevGeom& g, const Workspace& w, const Problem& p, const Cha
     if (p.n_clusters == 0) return 0;
     const FollowArgs a = follow_args(w, p, u);
     // the candidate count lives on the device: the grid is sized by its bound and bounded by it inside
-    const int grid = div_up(w.Cmax, kFitThreads);
+    const int64_t want = div_up(w.Cmax, kFitThreads);
+    const int grid = (int)(want < 148 * TPC_FIT_CTAS * 8 ? want : 148 * TPC_FIT_CTAS * 8);
     if (count_work)
         fit_candidates_kernel<true><<<grid, kFitThreads, 0, s>>>(g, a);
     else
