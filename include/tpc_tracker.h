@@ -139,7 +139,9 @@ int tpc_set_stream(tpc_tracker_t* t, void* cuda_stream);
  * (x, y, z, w); x and w are carried but never read (the row gives x) -- or one of the compact layouts below after
  * tpc_set_input_layout.  row_offsets: DEVICE int32
  * [n_sector_instances * n_rows + 1], CSR, instance-major row-minor, row_offsets[0] = 0 and
- * row_offsets[last] = n_clusters.  Clusters inside a row may be in any order.  n_clusters < 2^31.
+ * row_offsets[last] = n_clusters.  Clusters inside a row may be in any order.  n_clusters < 2^31,
+ * n_sector_instances * n_rows < 2^31 - 1, and the cell tables of all rows together stay below 2^32 units of 32 bytes
+ * (137 GB; n_sector_instances * n_rows * ceil((cells per row + 1) / 16) < 2^32) -- else TPC_ERR_ARG, nothing is done.
  * Asynchronous; one call in flight per tracker.
  */
 int tpc_track_sectors(tpc_tracker_t* t, const void* clusters, const int32_t* row_offsets,
