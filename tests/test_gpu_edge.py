@@ -231,7 +231,8 @@ def test_many_nearly_empty_instances():
 
 def test_cell_table_index_beyond_32_bits():
     """1,728 sector instances with the finest row grid (16,384 cells per row): instances x rows x cells = 4.5e9 > 2^32
-    table entries (9 GB), so the follower's table index must be 64 bit (it wrapped silently)."""
+    table entries (9 GB), beyond a 32-bit ENTRY index (it wrapped silently; the follower now indexes the
+    table by its 32-byte row units, 16 entries each, and the call rejects jobs beyond 2^32 units -- next test)."""
     from paper_1709_00618_b200 import Tracker
     evs = [dg.full_event(seed=2300 + i, n_prim=12, noise=0.0) for i in range(48)]
     batch = dg.concat_events(evs)
@@ -282,6 +283,26 @@ def test_null_row_offsets_is_rejected():
     bufs, out = trk.alloc_outputs(16)
     rc = trk.lib.tpc_track_sectors(trk._h, None, None, 1, 0, C.byref(out))
     assert rc == -1
+    torch.cuda.synchronize()
+    trk.close()
+
+
+def test_cell_table_beyond_the_follower_index_is_rejected():
+    """30,000 sector instances with the finest row grid: 30,000 x 159 rows x 1,025 units of 32 bytes = 4.9e9 >= 2^32,
+    more than the follower's 32-bit unit index covers (a 156 GB table): TPC_ERR_ARG before anything is touched."""
+    import ctypes as C
+    import torch
+    from paper_1709_00618_b200 import Tracker
+    ev = dg.single_sector(seed=1001)
+    trk = Tracker.for_event(ev, grid_cells_y=64, grid_cell_z=0.98)
+    trk.reserve(16, 1)
+    trk.set_stream()
+    bufs, out = trk.alloc_outputs(16)
+    dummy = torch.zeros(64, dtype=torch.int32, device="cuda")
+    rc = trk.lib.tpc_track_sectors(trk._h, dummy.data_ptr(), dummy.data_ptr(), 30_000, 16, C.byref(out))
+    assert rc == -1
+    ok = trk.lib.tpc_track_sectors(trk._h, dummy.data_ptr(), dummy.data_ptr(), 20_000, 16, C.byref(out))
+    assert ok != -1  # 20,000 instances pass the argument checks (and fail later: the workspace is far too small)
     torch.cuda.synchronize()
     trk.close()
 
