@@ -17,7 +17,8 @@ pytestmark = pytest.mark.gpu
 
 def _gpu(ev, **kw):
     from paper_1709_00618_b200 import Tracker
-    trk = Tracker.for_event(ev)
+    create_kw = {k: kw.pop(k) for k in list(kw) if k.startswith("grid_")}  # tracker parameters; the rest per call
+    trk = Tracker.for_event(ev, **create_kw)
     res = trk.track_sectors(ev.clusters, ev.row_offsets, ev.n_inst, debug=True, **kw)
     trk.close()
     return res
@@ -39,9 +40,9 @@ def _rows_of(ev):
     return np.repeat(np.arange(ev.n_inst * ev.n_rows), np.diff(ev.row_offsets)) % ev.n_rows
 
 
-def _check(ev, max_ok_mismatch=0):
+def _check(ev, max_ok_mismatch=0, **gpu_kw):
     o = run_oracle(ev)
-    g = _gpu(ev)
+    g = _gpu(ev, **gpu_kw)
     assert_ca_bit_exact(g, o)
     tr = tracklet_report(g, o)
     fr = final_track_report(g, o, ev.n_clusters)
@@ -109,6 +110,24 @@ def test_dense_spot_slow_paths():
                      np.full(len(x), -1.0)], axis=1).astype(np.float32)
     dense = _rebuild(ev, np.concatenate([ev.clusters, blob]), np.concatenate([rows, extra_rows]))
     _check(dense)
+
+
+@pytest.mark.parametrize("grid", [{}, {"grid_cell_z": 0.7}, {"grid_cell_z": 0.7, "grid_cells_y": 3}])
+def test_duplicated_dense_spot_ties_in_the_slow_paths(grid):
+    """The dense spot with EVERY cluster duplicated: exact ties among more hits than the in-line paths hold (S2: more
+    than four window hits per neighbour row; S5: ties beyond the fourth hit of the gate and, with z bins narrower than
+    the gate, in the loop over the bins in between), all resolved by the lowest local index as in the oracle."""
+    ev = dg.single_sector(seed=1014, n_tracks=40)
+    rows = _rows_of(ev)
+    rng = np.random.default_rng(78)
+    extra_rows = np.repeat(np.arange(60, 75), 8)
+    x = dg.row_x(ev.n_rows)[extra_rows]
+    blob = np.stack([x, rng.uniform(-1.0, 1.0, len(x)), rng.uniform(99.0, 101.5, len(x)),
+                     np.full(len(x), -1.0)], axis=1).astype(np.float32)
+    cl = np.concatenate([ev.clusters, blob])
+    rw = np.concatenate([rows, extra_rows])
+    dup = _rebuild(ev, np.concatenate([cl, cl]), np.concatenate([rw, rw]))
+    _check(dup, **grid)
 
 
 def test_capacity_overflow_is_reported_not_written():
