@@ -4,15 +4,17 @@
 // one-step back transport, phase B downward).  One thread per candidate, all arithmetic fp32 in registers.
 //
 // Two kernels:
-//  * fit_candidates_kernel: seed + Kalman fit of the candidate's own 4..10 hits.  Every address is known up front, so
-//    all loads of a candidate are in flight together; the state after the last own hit goes to tl_state.
+//  * fit_candidates_kernel: the S4 chain walk (<= 9 dependent link loads), then seed + Kalman fit of the candidate's
+//    own 4..10 hits, which wait in a per-thread column of shared memory; the state after the last own hit goes to
+//    tl_state.
 //  * follow_kernel: the row-by-row extrapolation.  Persistent warps, every lane a small state machine that advances
 //    its candidate by ONE pad row per loop iteration (upward / back transport / downward), with the lanes refilled
 //    from a device-wide queue as candidates end.  A pick-up search reads the cell-table entries of the exact gate
 //    window and then the window's first hits, all loads of a kind in flight together; examining a superset of cells
 //    is harmless because every hit still passes the exact gate test (the grid is an acceleration structure only).
-//    (A variant with a two-stage speculative load pipeline was measured in round 1 and lost to this one -- DESIGN.md
-//    section 5 -- and is no longer in the source.)
+//    The 20 filter values and what every step touches live in registers (64: eight CTAs per SM), what a step touches
+//    at most once in shared memory.  (Variants measured and rejected -- speculative loads, prefetches, buffered
+//    stores, an asynchronous candidate supply -- are listed in DESIGN.md section 5.)
 #include "kf_math.cuh"
 
 #ifndef TPC_FOLLOW_CTAS
