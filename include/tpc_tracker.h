@@ -37,6 +37,7 @@ extern "C" {
 #define TPC_ERR_CUDA (-4)      /* a CUDA runtime call failed (text in tpc_last_error) */
 #define TPC_ERR_CAPACITY (-5)  /* tpc_check_counts: an output buffer was too small (results were saturated) */
 #define TPC_ERR_INPUT (-6)     /* tpc_check_counts: device-side input validation failed (row too long, ...) */
+#define TPC_ERR_LIMIT (-7)     /* tpc_start_hits_static: input larger than the library's built-in scratch array */
 
 #define TPC_CAND_MAX_HITS 10   /* stride of cand_hits (reading A7: "usually 4 to 10 hits") */
 #define TPC_N_COUNTS 16
@@ -315,6 +316,41 @@ typedef struct {
 
 int tpc_estimate_vertices(tpc_tracker_t* t, const tpc_phase2_output_t* merged, const tpc_vertex_output_t* out);
 
+/*
+ * Start hits without any allocation (no workspace, no tracker handle).
+ *
+ * For callers that cannot obtain device memory: a component inside a framework that reserved the whole GPU at
+ * start-up and passes each component fixed buffers only, a plug-in of an online loop where cudaMalloc is forbidden
+ * because it synchronises the device under everybody else, code that was lent a stream and nothing more.  Everything
+ * else in this library takes its scratch memory from the caller's workspace; this one call carries its own, a
+ * file-scope __device__ array of 8 * (32 + TPC_STATIC_MAX_CLUSTERS / 2048) bytes = 512.25 KB that every GPU which
+ * loads the library holds until the process exits.  The call itself runs no cudaMalloc, cudaFree or other allocating
+ * routine: one cudaMemsetAsync on that array and one kernel, both on `cuda_stream` (cudaStream_t as void*, NULL = the
+ * legacy default stream); asynchronous.
+ *
+ * The operation is the first half of S4 (link chains begin at start hits): h is a start hit iff
+ * link_up[h] >= 0 and link_dn[h] < 0, where link_up / link_dn are the CLEANED links of S3 as tpc_output_t returns
+ * them (index of the partner in the same arrays, -1 = none).
+ *   link_up, link_dn  DEVICE int32 [n_clusters], read only (16-byte aligned arrays are read a little faster)
+ *   start_hits        DEVICE int32 [start_capacity]: the start hits in ascending index; only what fits is written;
+ *                     NULL allowed when start_capacity = 0 (count only)
+ *   n_start           DEVICE int64 [1]: the REQUIRED count, also when it exceeds start_capacity
+ * The result equals start_hits / counts[0] of tpc_track_sectors for the same links.
+ *
+ * Limit: n_clusters <= TPC_STATIC_MAX_CLUSTERS, else TPC_ERR_LIMIT and nothing is enqueued.  Other returns:
+ * TPC_ERR_ARG (NULL / negative argument), TPC_ERR_CUDA; text from tpc_last_error(NULL) on the calling thread.
+ *
+ * First call on a device: it looks up the device address of the array (cudaGetSymbolAddress, once per device, with
+ * the caller's current device); make that first call before starting any stream capture on that device.
+ * Sharing: all calls on one device use the same array.  The call clears the part it needs, so stale contents of an
+ * earlier call do no harm, but two calls that overlap on the GPU (two streams, two host threads) corrupt each other:
+ * keep them on one stream or order them with events.
+ */
+#define TPC_STATIC_MAX_CLUSTERS (1 << 27) /* 134,217,728 */
+int tpc_start_hits_static(const int32_t* link_up, const int32_t* link_dn, int64_t n_clusters, int32_t* start_hits,
+                          int64_t start_capacity, int64_t* n_start, void* cuda_stream);
+
+/* t = NULL: the text of the last failed tpc_tracker_create / tpc_start_hits_static call of the calling thread. */
 const char* tpc_last_error(const tpc_tracker_t* t);
 
 #ifdef __cplusplus

@@ -30,6 +30,7 @@ SOURCES = {
     "k6_select.cu": [],
     "k7_phase2.cu": [],
     "k8_vertex.cu": [],
+    "k9_start_hits_static.cu": [],
     "host_pipeline.cu": [],
 }
 

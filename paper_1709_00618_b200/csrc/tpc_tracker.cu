@@ -15,6 +15,8 @@ using namespace tpc;
 
 static thread_local std::string g_create_err;
 
+void tpc_set_handleless_error(const std::string& msg) { g_create_err = msg; }
+
 template <typename T>
 static T dflt(T v, T d) { return v == (T)0 ? d : v; }
 

@@ -35,6 +35,10 @@ static inline int fail(tpc_tracker* t, int code, const std::string& msg) {
     return code;
 }
 
+// Error text of entry points that have no tracker handle (tpc_start_hits_static): what tpc_last_error(NULL) returns
+// on this thread.
+void tpc_set_handleless_error(const std::string& msg);
+
 
 // bytes per cluster of an input layout, and the alignment mask of its base pointer
 static inline int64_t layout_bytes(int layout) { return layout == TPC_INPUT_XYZW ? 16 : layout == TPC_INPUT_YZ ? 8 : 4; }

@@ -19,13 +19,14 @@ N_COUNTS = 16
 N_STAGES = 6
 STAGE_NAMES = ("bin", "neighbours", "chains", "fit", "follow", "select")
 ERRORS = {-1: "TPC_ERR_ARG", -2: "TPC_ERR_GEOMETRY", -3: "TPC_ERR_WORKSPACE", -4: "TPC_ERR_CUDA",
-          -5: "TPC_ERR_CAPACITY", -6: "TPC_ERR_INPUT"}
+          -5: "TPC_ERR_CAPACITY", -6: "TPC_ERR_INPUT", -7: "TPC_ERR_LIMIT"}
 
 EXPORTS = ("tpc_tracker_create", "tpc_tracker_destroy", "tpc_workspace_bytes", "tpc_set_workspace", "tpc_set_stream",
            "tpc_track_sectors", "tpc_check_counts", "tpc_last_launch_count", "tpc_set_stage_timing",
            "tpc_stage_times_ms", "tpc_last_error", "tpc_track_sectors_host", "tpc_set_work_counters",
            "tpc_set_input_layout", "tpc_pipeline_create", "tpc_pipeline_destroy", "tpc_pipeline_run",
-           "tpc_merge_refit", "tpc_estimate_vertices")
+           "tpc_merge_refit", "tpc_estimate_vertices", "tpc_start_hits_static")
+STATIC_MAX_CLUSTERS = 1 << 27                        # TPC_STATIC_MAX_CLUSTERS
 VTX_MAX_PER_WINDOW = 64
 INPUT_LAYOUTS = {"xyzw": 0, "yz": 1, "i16": 2}       # TPC_INPUT_*
 LAYOUT_BYTES = {"xyzw": 16, "yz": 8, "i16": 4}
@@ -135,8 +136,34 @@ def load_library():
     lib.tpc_pipeline_destroy.restype = None
     lib.tpc_pipeline_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_int32,
                                      C.POINTER(HostOutput)]
+    lib.tpc_start_hits_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p,
+                                          C.c_void_p]
     _lib = lib
     return lib
+
+
+def start_hits_static(link_up, link_dn, start_hits, n_start, *, n_clusters=None, stream=None):
+    """tpc_start_hits_static on torch CUDA tensors; asynchronous on `stream` (default: torch's current stream).
+
+    The one call of the library that needs neither a workspace nor a Tracker: it is meant for callers that have no
+    way to allocate device memory (a component of a framework that handed out all GPU memory at start-up, a real-time
+    loop where cudaMalloc's device-wide synchronisation is not acceptable).  Its scratch memory is an array built into
+    the library, shared by every call on that GPU: calls must not overlap on the device, and at most
+    STATIC_MAX_CLUSTERS links are accepted (TPC_ERR_LIMIT beyond that).  link_up / link_dn: int32 [n] cleaned links;
+    start_hits: int32 [capacity] or None (count only); n_start: int64 [1] receives the required count.
+    Make the first call on a device before starting any stream capture there (one-time address look-up).
+    """
+    import torch
+    lib = load_library()
+    n = int(link_up.numel() if n_clusters is None else n_clusters)
+    s = stream if stream is not None else torch.cuda.current_stream(link_up.device)
+    with torch.cuda.device(link_up.device):
+        rc = lib.tpc_start_hits_static(C.c_void_p(link_up.data_ptr()), C.c_void_p(link_dn.data_ptr()), n,
+                                       C.c_void_p(start_hits.data_ptr() if start_hits is not None else None),
+                                       int(start_hits.numel()) if start_hits is not None else 0,
+                                       C.c_void_p(n_start.data_ptr()), C.c_void_p(s.cuda_stream))
+    if rc != 0:
+        raise TpcError(f"tpc_start_hits_static: {ERRORS.get(rc, rc)}: {lib.tpc_last_error(None).decode()}")
 
 
 def make_geometry(row_x: np.ndarray, *, z_lo=0.0, z_hi=250.0, sigma_y=0.1, sigma_z=0.1, sectors_per_event=36,
