@@ -32,7 +32,7 @@ extern "C" {
 
 #define TPC_OK 0
 #define TPC_ERR_ARG (-1)       /* NULL / negative / misaligned argument */
-#define TPC_ERR_GEOMETRY (-2)  /* n_rows out of [3,255], rows not strictly increasing or not uniformly spaced */
+#define TPC_ERR_GEOMETRY (-2)  /* n_rows out of [3,255], rows not strictly increasing, or nf_bridge_rows with unequal row steps */
 #define TPC_ERR_WORKSPACE (-3) /* workspace missing or smaller than tpc_workspace_bytes() */
 #define TPC_ERR_CUDA (-4)      /* a CUDA runtime call failed (text in tpc_last_error) */
 #define TPC_ERR_CAPACITY (-5)  /* tpc_check_counts: an output buffer was too small (results were saturated) */
@@ -66,7 +66,9 @@ typedef struct {
 
 typedef struct {
     int32_t n_rows;            /* pad rows per sector, 3..255 (159) */
-    const float* row_x;        /* HOST pointer [n_rows], strictly increasing, uniform pitch (1e-4 rel); copied */
+    const float* row_x;        /* HOST pointer [n_rows], strictly increasing; copied.  The steps need not be equal
+                                  (reading A5': S2 weights its differences by the row steps); a step within
+                                  1e-4 of the mean pitch counts as regular and keeps the default arithmetic bit for bit */
     int32_t sectors_per_event; /* 36 (even) */
     float half_angle_rad;      /* sector half opening angle (10 deg): row half-width = row_x * tan(half_angle) */
     float z_lo, z_hi;          /* z range of the z >= 0 side used for the grid (mirrored for z < 0): 0..250, or
@@ -161,7 +163,9 @@ int tpc_track_sectors(tpc_tracker_t* t, const void* clusters, const int32_t* row
  *                   with z_origin = z_lo on the z >= 0 side and -z_hi on the z < 0 side (the grid origin of that
  *                   side).  Decoding is one exact multiplication and one fp32 addition per coordinate; the tracker
  *                   then runs on the decoded fp32 (y, z) exactly as for TPC_INPUT_YZ.  Clusters outside the
- *                   representable range cannot be given in this layout.
+ *                   representable range cannot be given in this layout: tpc_set_input_layout returns TPC_ERR_ARG
+ *                   when the geometry's z range exceeds 1024 cm or the outermost row's half-width
+ *                   (row_x * tan(half angle) + 0.5 cm) reaches 128 cm.
  */
 #define TPC_INPUT_XYZW 0
 #define TPC_INPUT_YZ 1
@@ -264,8 +268,10 @@ int tpc_track_sectors_host(tpc_tracker_t* t, const void* h_clusters, const int32
  *             innermost segment, in that segment's frame.
  * tpc_merge_refit works on the final tracks of the LAST tpc_track_sectors call of this tracker: it reads that call's
  * workspace and its row_offsets array, so it must follow it (same stream; asynchronous) before the workspace is
- * reused, and row_offsets must still be valid and unchanged.  Track indices are
- * those of that call (positions in trk_*).  All pointers: caller-owned DEVICE memory, NULL = skipped, counts2 required.
+ * reused, and row_offsets must still be valid and unchanged.  A tpc_pipeline_run / tpc_track_sectors_host on this
+ * tracker, or tpc_set_workspace with another buffer, ends that state: tpc_merge_refit then returns TPC_ERR_ARG until
+ * the next tpc_track_sectors call (the pipeline's chunks live in the slots and leave nothing to merge).  Track indices
+ * are those of that call (positions in trk_*).  All pointers: caller-owned DEVICE memory, NULL = skipped, counts2 required.
  */
 typedef struct {
     int32_t* seg_next;   /* [n_tracks] track that continues this one outward in the neighbouring sector, or -1 */
@@ -301,6 +307,8 @@ int tpc_merge_refit(tpc_tracker_t* t, const tpc_phase2_output_t* out);
  *       the offset that converts the track's (and its clusters') z from the time-like to the spatial coordinate.
  * `merged` is the output struct of the preceding tpc_merge_refit call on this tracker (mtrk_first, mtrk_nhits,
  * mtrk_ok, mtrk_params and counts2 required); the call reads its arrays and the workspace, same stream, asynchronous.
+ * mtrk_capacity = 0 gives an empty result (counts3 = 0, 0).  The histogram of one window sits in shared memory:
+ * a geometry whose |z| range exceeds 12.7 km (200 KB of 0.5 cm bins) gets TPC_ERR_ARG here.
  */
 #define TPC_VTX_MAX_PER_WINDOW 64
 typedef struct {

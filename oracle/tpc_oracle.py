@@ -135,7 +135,6 @@ class Oracle:
 
     @classmethod
     def for_event(cls, ev, **kw):
-        from paper_1709_00618_b200 import datagen
         return cls(ev.row_x, ev.bz, z_lo=ev.z_lo, z_hi=ev.z_hi, sigma_y=ev.sigma_y,
                    sigma_z=ev.sigma_z, **kw)
 

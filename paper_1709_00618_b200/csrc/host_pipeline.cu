@@ -156,6 +156,9 @@ extern "C" int tpc_pipeline_run(tpc_pipeline_t* p, const void* h_cl_v, const int
     tpc_tracker* t = p->t;
     if (!h_ro || !hout || inst_per_chunk < 1 || n_inst < 0 || n_clusters < 0) return fail(t, TPC_ERR_ARG, "bad argument");
     if (n_clusters > 0 && !h_cl_v) return fail(t, TPC_ERR_ARG, "NULL clusters");
+    // the chunks run on the slots' workspaces and streams: whatever an earlier tpc_track_sectors call left for
+    // tpc_merge_refit is stale from here on (phase 2 needs a tpc_track_sectors call of its own)
+    t->last_ws = nullptr;
     const auto wall0 = std::chrono::steady_clock::now();
     const int R = t->g.R;
     const int n_slots = (int)p->slots.size();
@@ -203,10 +206,14 @@ extern "C" int tpc_pipeline_run(tpc_pipeline_t* p, const void* h_cl_v, const int
         int ret = TPC_OK;
         if (cnt[3] > o.trk_capacity || (o.trk_hits && cnt[4] > o.trk_hits_capacity))
             ret = fail(t, TPC_ERR_CAPACITY, "slot track capacity too small");
-        if (track_base + nt > hout->trk_capacity || (hout->trk_hits && hit_base + nh > hout->trk_hits_capacity))
-            return fail(t, TPC_ERR_CAPACITY, "host track capacity too small");
+        // The job-wide host arrays are full: this chunk (and every later one) is not downloaded, but its slot still
+        // gets an (empty) download interval and the bases advance, so that the run goes on to the end and
+        // hout->totals report the sizes the caller needs.
+        const bool host_full =
+            track_base + nt > hout->trk_capacity || (hout->trk_hits && hit_base + nh > hout->trk_hits_capacity);
+        if (host_full) ret = fail(t, TPC_ERR_CAPACITY, "host track capacity too small");
         e = cudaEventRecord(p->out0[s], s_out);
-        if (c.n_cl > 0 && e == cudaSuccess) {
+        if (c.n_cl > 0 && e == cudaSuccess && !host_full) {
             int32_t* d_owner = (hout->cluster_owner && o.cluster_owner) ? o.cluster_owner : nullptr;
             int32_t* d_hits = (hout->trk_hits && o.trk_hits) ? o.trk_hits : nullptr;
             int64_t* d_off = (hout->trk_hit_offset && o.trk_hit_offset) ? o.trk_hit_offset : nullptr;
@@ -254,7 +261,7 @@ extern "C" int tpc_pipeline_run(tpc_pipeline_t* p, const void* h_cl_v, const int
         if (i >= 2 * n_slots) CK(read_out_ms(s));
         if (i >= n_slots) {
             const int r = finish(i - n_slots);
-            if (r == TPC_ERR_CAPACITY && rc == TPC_OK) rc = r;  // keep going: the totals tell the required sizes
+            if (r == TPC_ERR_CAPACITY) rc = r;  // keep going (also after the first one): the totals tell the required sizes
             else if (r != TPC_OK) { rc = r; goto done; }
         }
         // upload: the slot's inputs are free once the chunk that used them last has been tracked
@@ -293,7 +300,7 @@ extern "C" int tpc_pipeline_run(tpc_pipeline_t* p, const void* h_cl_v, const int
     for (int j = (nc > n_slots ? nc - n_slots : 0); j < nc; j++) {
         if (j >= n_slots) CK(read_out_ms(j % n_slots));
         const int r = finish(j);
-        if (r == TPC_ERR_CAPACITY && rc == TPC_OK) rc = r;
+        if (r == TPC_ERR_CAPACITY) rc = r;
         else if (r != TPC_OK) { rc = r; goto done; }
     }
     for (int j = (nc > n_slots ? nc - n_slots : 0); j < nc; j++) CK(read_out_ms(j % n_slots));

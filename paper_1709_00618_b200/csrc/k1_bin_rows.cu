@@ -2,6 +2,8 @@
 // One CTA per (sector instance, pad row): counting sort of the row's clusters by grid cell (z bin major, y strip
 // minor), done entirely in shared memory, writing the sorted (y,z) pairs, their original local indices and the
 // cell-start table.  The grid is an acceleration structure only; no result of S2..S6 depends on it.
+#include <mutex>
+
 #include "tpc_common.cuh"
 
 namespace tpc {
@@ -136,12 +138,19 @@ int launch_bin_rows(const DevGeom& g, const Workspace& w, const Problem& p, cuda
     const int slabs = p.n_inst * g.R;
     if (slabs == 0) return 0;
     const size_t smem = (size_t)g.nzp * sizeof(uint16_t);
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(bin_rows_kernel<kInXYZW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaFuncSetAttribute(bin_rows_kernel<kInYZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaFuncSetAttribute(bin_rows_kernel<kInI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = smem;
+    if (smem > 48 * 1024) {  // opt-in size, a property of (kernel, device): cached per device ordinal
+        static std::mutex mu;
+        static size_t configured[kMaxDeviceOrdinals] = {};
+        int dev = 0;
+        cudaGetDevice(&dev);
+        dev = dev >= 0 && dev < kMaxDeviceOrdinals ? dev : 0;
+        std::lock_guard<std::mutex> lock(mu);
+        if (smem > configured[dev]) {
+            cudaFuncSetAttribute(bin_rows_kernel<kInXYZW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(bin_rows_kernel<kInYZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(bin_rows_kernel<kInI16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            configured[dev] = smem;
+        }
     }
     if (p.layout == kInYZ)
         bin_rows_kernel<kInYZ><<<slabs, kBinThreads, smem, s>>>(g, p.clusters, p.row_offsets, w.hit_yz, w.hit_idx,

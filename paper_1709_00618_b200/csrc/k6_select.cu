@@ -11,6 +11,8 @@
 //   count     per tracklet: kept = popcount(mask), tracks/hits per block of 256 tracklets, then one scan
 //   finalize  per tracklet: track index and first hit position (deterministic: ascending candidate id), track record
 //   write     per hit: owner and the track's hit list entry (rank = kept rows below, from the mask)
+#include <mutex>
+
 #include "tpc_common.cuh"
 
 namespace tpc {
@@ -285,13 +287,24 @@ int launch_select(const DevGeom& g, const Workspace& w, const Problem& p, const 
         const int grid = (int)(blocks < 148 * 8 ? blocks : 148 * 8);
         const int hgrid = div_up(slabs, kHitThreads / 32);
         {
-            static int smem_bytes = 0;
-            if (!smem_bytes) {
-                int dev = 0, max_optin = 0;
-                cudaGetDevice(&dev);
-                cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-                smem_bytes = (max_optin > 0 ? max_optin : 48 * 1024) - 2048;  // room for the kernel's static arrays
-                cudaFuncSetAttribute(claim_mark_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+            // the opt-in shared-memory size is a property of (kernel, device): cached per device ordinal, set up by
+            // whichever host thread launches on that device first
+            static std::mutex mu;
+            static int smem_by_dev[kMaxDeviceOrdinals] = {};
+            int dev = 0;
+            cudaGetDevice(&dev);
+            dev = dev >= 0 && dev < kMaxDeviceOrdinals ? dev : 0;
+            int smem_bytes;
+            {
+                std::lock_guard<std::mutex> lock(mu);
+                if (!smem_by_dev[dev]) {
+                    int max_optin = 0;
+                    cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+                    smem_by_dev[dev] = (max_optin > 0 ? max_optin : 48 * 1024) - 2048;  // room for the static arrays
+                    cudaFuncSetAttribute(claim_mark_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         smem_by_dev[dev]);
+                }
+                smem_bytes = smem_by_dev[dev];
             }
             claim_mark_kernel<<<p.n_inst, kInstThreads, smem_bytes, s>>>(g, p.row_offsets, w.tl_nhits, w.tl_rows,
                                                                          w.slab_part, w.tl_rowhit, w.claim, w.tl_sel,

@@ -356,12 +356,13 @@ merged_out_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2A
 #pragma unroll
                 for (int q = 0; q < 15; q++) o.seg_cov[t * 15 + q] = a.p2_cov[t * 15 + q];
         }
-        if (!head || m >= o.mtrk_capacity) continue;
+        if (!head) continue;
+        // every chain goes on the list, also one whose merged index lies beyond the caller's capacity: chain_fit_kernel
+        // walks all p2_counts[4] entries and skips those itself (an unwritten entry would be stale workspace memory)
+        if (chain) a.p2_chain[e] = make_int2((int)t, (int)m);
+        if (m >= o.mtrk_capacity) continue;
         if (o.mtrk_first) o.mtrk_first[m] = (int32_t)t;
-        if (chain) {  // fitted by chain_fit_kernel, one dense thread per chain
-            a.p2_chain[e] = make_int2((int)t, (int)m);
-            continue;
-        }
+        if (chain) continue;  // fitted by chain_fit_kernel, one dense thread per chain
         // not merged: the refit of the track alone
         const int4 info = a.p2_info[t];
         if (o.mtrk_nseg) o.mtrk_nseg[m] = 1;

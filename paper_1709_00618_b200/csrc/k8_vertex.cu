@@ -228,17 +228,20 @@ int launch_vertices(const DevGeom& g, const Workspace& w, const Problem& p, cons
     cudaMemsetAsync(w.vz_cnt, 0, sizeof(int32_t) * (size_t)n_win * kVtxMax, s);
     if (o.vtx_ntracks && o.vtx_capacity > 0) cudaMemsetAsync(o.vtx_ntracks, 0, sizeof(int32_t) * o.vtx_capacity, s);
     int launches = 0;
-    if (p.n_clusters > 0 && o.trk_zv) {
+    const int64_t n_m_max = m.mtrk_capacity < w.Tmax ? m.mtrk_capacity : w.Tmax;
+    if (p.n_clusters > 0 && o.trk_zv && n_m_max > 0) {  // no merged-track slot: no launch (counts3 = 0, 0)
         const VtxArgs a{w.cand_slab, w.trk_cand, w.p2_info, w.vz_hist, w.vz_seed, w.vz_nseed, w.vz_sum, w.vz_cnt,
                         w.vz_like,   w.vz_counts, n_win,    g.inst_phase / g.spe};
-        const int grid_m = div_up(m.mtrk_capacity < w.Tmax ? m.mtrk_capacity : w.Tmax, kVtxThreads);
+        const int grid_m = div_up(n_m_max, kVtxThreads);
         track_vertex_kernel<<<grid_m, kVtxThreads, 0, s>>>(g, a, m, o);
-        vertex_seeds_kernel<<<n_win, kVtxThreads, sizeof(int32_t) * g.vtx_nb, s>>>(g, a);
+        const size_t seed_smem = sizeof(int32_t) * (size_t)g.vtx_nb;  // <= kVtxMaxSmemBytes (checked by the caller)
+        if (seed_smem > 48 * 1024)  // |z| range beyond ~3 km: opt in (cheap, per call: the size depends on the geometry)
+            cudaFuncSetAttribute(vertex_seeds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)seed_smem);
+        vertex_seeds_kernel<<<n_win, kVtxThreads, seed_smem, s>>>(g, a);
         vertex_scan_kernel<<<1, kVtxThreads, 0, s>>>(a);
         vertex_sums_kernel<<<grid_m, kVtxThreads, 0, s>>>(g, a, m, o);
         const int64_t nv_max = (int64_t)n_win * kVtxMax;
-        const int64_t need = (m.mtrk_capacity < w.Tmax ? m.mtrk_capacity : w.Tmax) > nv_max
-                                 ? (m.mtrk_capacity < w.Tmax ? m.mtrk_capacity : w.Tmax) : nv_max;
+        const int64_t need = n_m_max > nv_max ? n_m_max : nv_max;
         vertex_assign_kernel<<<div_up(need, kVtxThreads), kVtxThreads, 0, s>>>(g, a, m, o);
         launches += 5;
     }

@@ -8,6 +8,8 @@ namespace tpc {
 
 constexpr int kCandMax = 10;      // TPC_CAND_MAX_HITS
 constexpr int kMaxRows = 255;
+constexpr size_t kVtxMaxSmemBytes = 200 * 1024;  // vertex_seeds_kernel keeps one window's z_v histogram in shared memory
+constexpr int kMaxDeviceOrdinals = 64;  // per-device caches of kernel attributes (launch helpers)
 constexpr int kMaxCells = 16384;  // cells of one row's grid (positions and the table are 16 bit; S1 keeps 4 B/cell in smem)
 constexpr uint16_t kNoHit = 0xFFFFu;
 constexpr float kKappaPerTesla = 0.00299792458f;

@@ -117,6 +117,7 @@ extern "C" int tpc_tracker_create(const tpc_geometry_t* geom, float bz, tpc_trac
     for (int r = 0; r < R; r++) {
         const float hw = geom->row_x[r] * g.tan_half + 0.5f;  // half-width of the row's y grid
         rows[r] = geom->row_x[r];
+        if (hw > t->y_half_max) t->y_half_max = hw;
         rows[R + r] = -hw;
         rows[2 * R + r] = (float)ny / (2.0f * hw);
         if (r >= 1 && r <= R - 2) {  // step factors of reading A5' (rows 0 and R-1 own no links)
@@ -248,6 +249,7 @@ extern "C" size_t tpc_workspace_bytes(const tpc_tracker_t* t, int64_t max_cluste
 extern "C" int tpc_set_workspace(tpc_tracker_t* t, void* dev_ptr, size_t bytes) {
     if (!t) return TPC_ERR_ARG;
     if (!dev_ptr || ((uintptr_t)dev_ptr & 255)) return fail(t, TPC_ERR_ARG, "workspace must be non-NULL and 256-byte aligned");
+    if (dev_ptr != t->ws || bytes != t->ws_bytes) t->last_ws = nullptr;  // the old workspace may be gone: phase 2 needs a new track call
     t->ws = dev_ptr;
     t->ws_bytes = bytes;
     return TPC_OK;
@@ -265,6 +267,8 @@ extern "C" int tpc_set_input_layout(tpc_tracker_t* t, int32_t layout) {
         return fail(t, TPC_ERR_ARG, "unknown input layout");
     if (layout == TPC_INPUT_I16 && ((double)t->z_hi - (double)t->z_lo) > 65535.0 * (double)TPC_I16_Z_STEP)
         return fail(t, TPC_ERR_ARG, "TPC_INPUT_I16 covers 1024 cm of z; the geometry's z range is wider");
+    if (layout == TPC_INPUT_I16 && !(t->y_half_max < 32768.0f * TPC_I16_Y_STEP))
+        return fail(t, TPC_ERR_ARG, "TPC_INPUT_I16 covers |y| < 128 cm; the outermost pad row is wider");
     t->input_layout = layout;
     return TPC_OK;
 }
@@ -364,13 +368,15 @@ int tpc_track_on(tpc_tracker* t, void* ws, size_t ws_bytes, cudaStream_t s, bool
         }
     }
     t->last_launches = launches;
-    t->last_ws = ws;
-    t->last_ws_bytes = ws_bytes;
-    t->last_stream = s;
-    t->last_first_inst = first_inst;
-    t->last_row_offsets = row_offsets;
-    t->last_n_inst = n_inst;
-    t->last_n_clusters = n_clusters;
+    if (timed) {  // a user call: phase 2 may follow.  The pipeline's chunks (timed == false) leave no such state.
+        t->last_ws = ws;
+        t->last_ws_bytes = ws_bytes;
+        t->last_stream = s;
+        t->last_first_inst = first_inst;
+        t->last_row_offsets = row_offsets;
+        t->last_n_inst = n_inst;
+        t->last_n_clusters = n_clusters;
+    }
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, std::string("CUDA: ") + cudaGetErrorString(e));
     return TPC_OK;
@@ -400,6 +406,8 @@ extern "C" int tpc_estimate_vertices(tpc_tracker_t* t, const tpc_phase2_output_t
     if (!m || !m->mtrk_first || !m->mtrk_nhits || !m->mtrk_ok || !m->mtrk_params || !m->counts2)
         return fail(t, TPC_ERR_ARG, "merged: mtrk_first, mtrk_nhits, mtrk_ok, mtrk_params and counts2 are required");
     if (!t->last_ws) return fail(t, TPC_ERR_ARG, "tpc_estimate_vertices needs preceding tpc_track_sectors + tpc_merge_refit calls");
+    if ((size_t)t->g.vtx_nb * sizeof(int32_t) > kVtxMaxSmemBytes)
+        return fail(t, TPC_ERR_ARG, "the geometry's z range is too wide for the vertex histogram (0.5 cm bins in shared memory)");
     Workspace w;
     carve(t->g, t->last_ws, t->last_n_clusters, t->last_n_inst, &w);
     DevGeom g = t->g;

@@ -13,6 +13,7 @@ struct tpc_tracker {
     cudaStream_t stream = nullptr;
     int n_sm = 148;
     float z_lo = 0.0f, z_hi = 0.0f;  // geometry z range of the z >= 0 side
+    float y_half_max = 0.0f;         // half-width of the outermost row's y grid (limit of TPC_INPUT_I16)
     int last_launches = 0;
     // the problem of the last tpc_track_sectors call: tpc_merge_refit (phase 2) reads its workspace
     void* last_ws = nullptr;

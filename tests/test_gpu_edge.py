@@ -211,6 +211,80 @@ def test_compact_inputs_and_host_pipeline_against_oracle_full_window():
         trk.close()
 
 
+def test_host_pipeline_capacity_overflow_reports_totals():
+    """Host result arrays too small for the job: the run still visits every chunk, returns
+    TPC_ERR_CAPACITY (not a CUDA error from unrecorded events) and hout.totals hold the required sizes; the chunks
+    downloaded before the arrays filled up are intact; a second run on the same pipeline behaves the same, and a
+    pipeline with enough room gives the full result afterwards.  Slot (device) capacity overflow likewise."""
+    import ctypes as C
+    import torch
+    from paper_1709_00618_b200 import Tracker
+    from paper_1709_00618_b200.tracker import HostPipeline
+    ev = dg.full_event(seed=2001)
+    R = ev.n_rows
+    trk = Tracker.for_event(ev)
+    g = trk.track_sectors(ev.clusters, ev.row_offsets, ev.n_inst)
+    h_in = torch.from_numpy(ev.clusters).pin_memory()
+    h_ro = torch.from_numpy(ev.row_offsets).pin_memory()
+    ipc = 4  # 9 chunks on 2 slots: the overflow falls both inside and after the first n_slots chunks
+    mx = max(int(ev.row_offsets[min(i + ipc, ev.n_inst) * R] - ev.row_offsets[i * R]) for i in range(0, ev.n_inst, ipc))
+    per_chunk = [int(((g.trk_sector >= i) & (g.trk_sector < i + ipc)).sum()) for i in range(0, ev.n_inst, ipc)]
+    assert min(per_chunk) > 0
+    for fit_chunks in (0, 3):
+        pipe = HostPipeline(trk, mx, ipc, ev.n_clusters, n_slots=2)
+        cap = sum(per_chunk[:fit_chunks]) + per_chunk[fit_chunks] // 2  # chunk `fit_chunks` no longer fits
+        pipe.hout.trk_capacity = cap
+        for _ in range(2):
+            pipe.host["trk_nhits"].fill_(-5)
+            with torch.cuda.device(trk.device):
+                rc = trk.lib.tpc_pipeline_run(pipe._p, C.c_void_p(h_in.data_ptr()), C.c_void_p(h_ro.data_ptr()),
+                                              ev.n_inst, ev.n_clusters, ipc, C.byref(pipe.hout))
+            assert rc == -5, (rc, trk.lib.tpc_last_error(trk._h))
+            assert int(pipe.hout.totals[3]) == g.n_tracks and int(pipe.hout.totals[4]) == g.n_track_hits
+            assert int(pipe.hout.n_chunks) == len(per_chunk)
+            done = sum(per_chunk[:fit_chunks])
+            got = pipe.host["trk_nhits"].numpy()
+            assert np.array_equal(got[:done], g.trk_nhits[:done]) and np.all(got[done:cap] == -5)
+        pipe.close()
+    # device-side (slot) track capacity too small: same contract
+    pipe = HostPipeline(trk, mx, ipc, ev.n_clusters, n_slots=2)
+    for s in range(2):
+        pipe.slots[s].out.trk_capacity = max(per_chunk) // 2
+    with torch.cuda.device(trk.device):
+        h = C.c_void_p()
+        assert trk.lib.tpc_pipeline_create(trk._h, pipe.slots, 2, C.byref(h)) == 0  # slots are copied at creation
+        rc = trk.lib.tpc_pipeline_run(h, C.c_void_p(h_in.data_ptr()), C.c_void_p(h_ro.data_ptr()), ev.n_inst,
+                                      ev.n_clusters, ipc, C.byref(pipe.hout))
+        trk.lib.tpc_pipeline_destroy(h)
+    assert rc == -5 and int(pipe.hout.totals[3]) == g.n_tracks
+    pipe.close()
+    # enough room: the whole job
+    pipe = HostPipeline(trk, mx, ipc, ev.n_clusters, n_slots=2)
+    ho = pipe.run(h_in, h_ro, ev.n_inst)
+    assert ho["totals"][3] == g.n_tracks
+    assert np.array_equal(pipe.host["trk_nhits"].numpy()[:g.n_tracks], g.trk_nhits)
+    pipe.close()
+    # the pipeline's chunks leave nothing for phase 2: the state of the tpc_track_sectors call above is stale now
+    from paper_1709_00618_b200.tracker import TpcError
+    with pytest.raises(TpcError, match="ARG"):
+        trk.merge_refit(g.n_tracks)
+    trk.close()
+
+
+def test_i16_layout_is_refused_for_rows_wider_than_its_y_range():
+    """TPC_INPUT_I16 holds |y| < 128 cm: a geometry whose outermost row is wider cannot use it."""
+    from paper_1709_00618_b200 import Tracker
+    from paper_1709_00618_b200.tracker import TpcError
+    ok = Tracker(np.linspace(85.0, 247.0, 159).astype(np.float32), 0.5)
+    ok.set_input_layout("i16")
+    ok.close()
+    wide = Tracker(np.linspace(85.0, 730.0, 159).astype(np.float32), 0.5)  # 730 tan(10 deg) + 0.5 = 129.2 cm
+    with pytest.raises(TpcError, match="128 cm"):
+        wide.set_input_layout("i16")
+    wide.set_input_layout("yz")
+    wide.close()
+
+
 def test_full_size_central_event_against_oracle():
     """CFG:3 at full size: 8,000 primaries + 20 % secondaries, 10 % noise, ~1.5 M clusters, ~260 hits per row."""
     ev = dg.central_event(seed=3001)

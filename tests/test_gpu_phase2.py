@@ -106,6 +106,52 @@ def test_phase2_batch_of_drift_windows():
     # (track -> instance through the oracle's candidate list)
 
 
+def test_phase2_merged_track_capacity_too_small():
+    """mtrk_capacity below the number of merged tracks: counts2[0] is the required count, the records that fit equal
+    those of a full-size call, nothing is written beyond the capacity, and chains whose merged index lies beyond it are
+    skipped cleanly (every chain is on chain_fit's list, also the ones that do not fit)."""
+    import torch
+    from paper_1709_00618_b200 import Tracker
+    ev = dg.full_event(seed=2001)
+    trk = Tracker.for_event(ev)
+    g = trk.track_sectors(ev.clusters, ev.row_offsets, ev.n_inst)
+    nt = g.n_tracks
+    full = trk.merge_refit(nt)
+    nm = int(full["counts2"][0])
+    assert int((full["mtrk_nseg"] >= 2).sum()) >= 100
+    keys = ("mtrk_first", "mtrk_nseg", "mtrk_nhits", "mtrk_ok", "mtrk_params", "mtrk_cov", "mtrk_chi2")
+    for cap in (nm // 3, 1):
+        # sentinel-filled outputs: what lies beyond the capacity must stay untouched
+        bufs, o = trk.alloc_phase2(nt)
+        for k in keys:
+            bufs[k].fill_(-77)
+        o.mtrk_capacity = cap
+        trk.merge_refit_device(o)
+        torch.cuda.synchronize()
+        c2 = bufs["counts2"].cpu().numpy()
+        assert int(c2[0]) == nm and int(c2[1]) == int(full["counts2"][1])
+        for k in keys:
+            got = bufs[k].cpu().numpy()
+            assert np.array_equal(got[:cap], full[k][:cap]), k
+            assert np.all(got[cap:] == -77), k
+        for k in ("seg_next", "seg_prev", "seg_ok"):
+            assert np.array_equal(bufs[k].cpu().numpy()[:nt], full[k])
+    # no merged-track slot at all: phase 2 and the vertex step return empty results instead of a launch error
+    bufs, o = trk.alloc_phase2(nt)
+    o.mtrk_capacity = 0
+    trk.merge_refit_device(o)
+    vb, vo = trk.alloc_vertices(nt, 1)
+    vb["counts3"].fill_(-3)
+    trk.estimate_vertices_device(o, vo)
+    torch.cuda.synchronize()
+    assert int(bufs["counts2"].cpu()[0]) == nm and vb["counts3"].cpu().tolist() == [0, 0]
+    # and a full-size call afterwards still gives the same answer
+    again = trk.merge_refit(nt)
+    for k in keys:
+        assert np.array_equal(again[k], full[k]), k
+    trk.close()
+
+
 def test_phase2_requires_a_preceding_track_call():
     from paper_1709_00618_b200 import Tracker
     from paper_1709_00618_b200.tracker import TpcError
