@@ -169,6 +169,23 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def measure_fp32_peak(torch, dev):
+    """fp32 FMA rate of this GPU from the bench-only library (csrc_bench/fp32_peak.cu: 8 independent FMA chains per
+    thread, 64 warps per SM), TFLOP/s; None if the library is missing."""
+    import ctypes as C
+    path = os.path.join(ROOT, "paper_1709_00618_b200", "libtpcbench.so")
+    if not os.path.exists(path):
+        return None
+    lib = C.CDLL(path)
+    lib.tpc_bench_fp32_peak.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_double)]
+    out = torch.zeros(1, dtype=torch.float32, device=dev)
+    tf = C.c_double(0.0)
+    with torch.cuda.device(dev):
+        rc = lib.tpc_bench_fp32_peak(C.c_void_p(out.data_ptr()), 4096, 5,
+                                     C.c_void_p(torch.cuda.current_stream(dev).cuda_stream), C.byref(tf))
+    return float(tf.value) if rc == 0 and tf.value > 0 else None
+
+
 def measured_traffic(workload, windows, n_clusters):
     """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, or None if no capture of this
     workload is committed."""
@@ -180,6 +197,19 @@ def measured_traffic(workload, windows, n_clusters):
     if d.get("workload") != workload or int(d.get("windows", -1)) != int(windows) or int(d.get("n_clusters", -1)) != int(n_clusters):
         return None, f"committed capture is for {d.get('workload')} x {d.get('windows')} windows; not this workload"
     return float(d["dram_bytes_per_launch"]), f"{d['source']} (commit {d.get('commit', '?')})"
+
+
+def committed_capture(workload, windows, n_clusters):
+    """The other figures of the committed ncu capture (profiles/roofline_traffic.json) for this exact workload: DRAM
+    bytes of the whole step and the issue statistics of the dominant kernel.  {} when the capture is of another size."""
+    try:
+        with open(TRAFFIC_JSON) as f:
+            d = json.load(f)
+    except Exception:
+        return {}
+    if d.get("workload") != workload or int(d.get("windows", -1)) != int(windows) or int(d.get("n_clusters", -1)) != int(n_clusters):
+        return {}
+    return d
 
 
 def run_e2e(torch, trk, dev, layout, host_in, h_ro, batch, args, combine):
@@ -253,6 +283,7 @@ def run_ours(args):
     trk.set_stream()
     trk.set_stage_timing(True)
     bufs, out = trk.alloc_outputs(N, trk_capacity=N // 20 + 64)
+    fp32_measured = measure_fp32_peak(torch, dev)  # a few ms, before anything is timed
 
     def barrier():
         if world > 1:
@@ -298,6 +329,32 @@ def run_ours(args):
     st = [trk.stage_times_ms(a) for a in range(k)]  # the untimed counting call above recorded no events
     stage_ms = {nme: float(np.mean([s[nme] for s in st])) for nme in st[0]}
     own = bufs["cluster_owner"][:evs[0].n_clusters].cpu().numpy()  # window 0 of the default reading (physics report)
+
+    # ---- the same step with the candidate lists requested (north_star: "-> candidates and fitted tracks") ------------
+    with_cand = None
+    if "cand" not in skip:
+        cc = int(counts[1]) + 64
+        d_ch = torch.empty((cc, 10), dtype=torch.int32, device=dev)
+        d_cn = torch.empty(cc, dtype=torch.int32, device=dev)
+        out_c = type(out).from_buffer_copy(out)  # same outputs + cand_hits / cand_n
+        out_c.cand_hits, out_c.cand_n, out_c.cand_capacity = d_ch.data_ptr(), d_cn.data_ptr(), cc
+        trk.set_stream()
+        trk.track_sectors_device(d_cl, d_ro, S, out_c)
+        evc = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)]
+        for a, b in evc:
+            a.record()
+            trk.track_sectors_device(d_cl, d_ro, S, out_c)
+            b.record()
+        torch.cuda.synchronize(dev)
+        c_ms = float(np.mean([a.elapsed_time(b) for a, b in evc]))
+        with_cand = {"what": "the timed step with cand_hits / cand_n also written (the headline call passes "
+                             "cand_capacity = 0: final tracks and cluster owners only)",
+                     "ms_per_step": c_ms, "delta_ms": c_ms - ms_step, "value": N / (c_ms * 1e-3), "unit": UNIT,
+                     "candidates": int(counts[1]), "bytes_written": int(counts[1]) * 44,
+                     "cand_n_checksum": int(d_cn[:int(counts[1])].sum().item())}
+        del d_ch, d_cn
+        trk.track_sectors_device(d_cl, d_ro, S, out)  # phase 2 below works on the headline call's outputs
+        torch.cuda.synchronize(dev)
 
     # ---- phase 2 on the same batch: sector merger + refit of the final tracks -----------------
     phase2 = None
@@ -411,6 +468,45 @@ def run_ours(args):
     roof_path = {"bound": "hbm", "achieved": path_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": path_gbs / hbm_peak,
                  "bytes_per_cluster_model": BYTES_PER_CLUSTER_PATH, "peak_source": peak_src,
                  "frac_of_nominal_8TBs": path_gbs / 8000.0}
+    if fp32_measured:
+        roof["peak_measured"] = {"value": fp32_measured, "unit": "TFLOP/s", "frac": ach / fp32_measured,
+                                 "frac_of_nominal": fp32_measured / fp32_peak,
+                                 "how": "FMA chains (8 per thread, 64 warps per SM), best of 5 launches, CUDA events; "
+                                        "paper_1709_00618_b200/csrc_bench/fp32_peak.cu, run at the start of this bench"}
+    # SURVEY 8(d)'s headline fraction and the issue view of the dominant kernel go INSIDE `roofline` (the key the
+    # driver's record keeps); `roofline_path_hbm` stays as before for readers of earlier rounds' lines.
+    cap = committed_capture(WORKLOAD, args.windows, N)
+    roof["path_hbm"] = dict(roof_path)
+    if cap.get("step_dram_bytes"):
+        nb = float(cap["step_dram_bytes"])
+        roof["path_hbm"].update({
+            "ncu_dram_bytes_per_step": nb, "ncu_bytes_per_cluster": nb / N,
+            "ncu_over_model": nb / (BYTES_PER_CLUSTER_PATH * N),
+            "dram_gbs_at_ncu_bytes": nb / (ms_step * 1e-3) / 1e9,
+            "ncu_source": f"{cap.get('step_dram_source', '')} (commit {cap.get('commit', '?')})",
+            "rule": "SURVEY 8(d): achieved = min(ncu bytes, model bytes per cluster x N) / step time"})
+    if cap.get("warp_instructions_per_launch"):
+        wi = float(cap["warp_instructions_per_launch"])
+        slots = N_SM * 4 * sm_max * 1e6 * t_follow  # 4 schedulers per SM, one warp instruction per cycle each
+        roof["issue"] = {"warp_instructions_per_launch": wi, "issue_slots_per_launch": slots,
+                         "frac_of_issue_slots": wi / slots, "ncu_issue_active": cap.get("issue_active"),
+                         "lanes_per_instruction": cap.get("lanes_per_instruction"),
+                         "lane_instructions_per_row_step": wi * float(cap.get("lanes_per_instruction", 32.0)) / max(tr_f, 1),
+                         "source": f"{cap.get('issue_source', '')} (commit {cap.get('commit', '?')}); the slot count "
+                                   "uses this run's measured launch time"}
+    if e2e is not None:
+        def _sub(x):
+            return None if x is None else {k: x[k] for k in ("value", "unit", "ms_per_step", "h2d_bytes_per_step",
+                                                             "d2h_bytes_per_step", "h2d_ms", "compute_ms", "d2h_ms",
+                                                             "input")}
+        e2e["fp32_yz"] = _sub(e2e_yz)
+        e2e["fp32_xyzw"] = _sub(e2e_xyzw)
+        e2e["series_note"] = ("the headline e2e streams the 16-bit fixed-point layout (SURVEY 8(f) NEXT-4, "
+                              "parity-tested against the oracle on the decoded coordinates) and downloads "
+                              "cluster_owner + trk_params/trk_nhits/trk_sector; BASELINE.json configs[4] names fp32 "
+                              "clusters: that figure is fp32_yz (same tracker results as float4, bit for bit) and "
+                              "fp32_xyzw (the round-1 layout).  Round 1's e2e uploaded float4 and downloaded all seven "
+                              "result arrays incl. trk_cov and trk_hits, so the series breaks between rounds 1 and 2")
     cpu = None
     if world == 1 and "cpu" not in skip:
         cpu, _ = cpu_baseline(evs, 1)
@@ -430,7 +526,7 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": launches,
             "e2e": e2e, "e2e_xyzw_f32": e2e_xyzw, "e2e_yz_f32": e2e_yz,
             "roofline": roof, "roofline_path_hbm": roof_path, "cpu_baseline": cpu,
-            "stage_ms": stage_ms, "phase2_merge_refit": phase2, "single_window": single,
+            "stage_ms": stage_ms, "with_candidates": with_cand, "phase2_merge_refit": phase2, "single_window": single,
             "results": {"candidates": int(counts[1]), "tracklets": int(counts[2]), "tracks": int(counts[3]),
                         "track_hits": int(counts[4]), "error_flags": int(counts[5])},
             "physics_window0": phys,
@@ -454,7 +550,7 @@ def main():
                          "linear-scaling check of PAPER.md:33")
     ap.add_argument("--seed0", type=int, default=5001)
     ap.add_argument("--tune", default="", help='JSON dict of performance-only tracker parameters, e.g. {"grid_cells_y": 8}')
-    ap.add_argument("--skip", default="", help="comma list of optional sections to leave out: e2e,phase2,single,bridge,cpu")
+    ap.add_argument("--skip", default="", help="comma list of optional sections to leave out: e2e,phase2,single,bridge,cpu,cand")
     args = ap.parse_args()
     global WORKLOAD
     WORKLOAD = args.workload

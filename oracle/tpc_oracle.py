@@ -289,14 +289,22 @@ class Oracle:
 
     def phase2(self, clusters, row_offsets, n_inst, res: "OracleResult") -> Phase2Result:
         """Merger + refit on the final tracks of `res` (an OracleResult of the same input)."""
-        cl = np.ascontiguousarray(clusters, np.float32)
         ro = np.ascontiguousarray(row_offsets, np.int32)
         nt = len(res.trk_cand)
         inst = (np.searchsorted(ro[::self.n_rows], res.cand_hits[res.trk_cand, 0], side="right") - 1).astype(np.int32) \
             if nt else np.zeros(0, np.int32)
-        inst = np.ascontiguousarray(inst)
-        off = np.ascontiguousarray(res.trk_hit_offset, np.int64)
-        hits = np.ascontiguousarray(res.trk_hits, np.int32)
+        return self.phase2_on_tracks(clusters, row_offsets, n_inst, inst, res.trk_hit_offset, res.trk_hits)
+
+    def phase2_on_tracks(self, clusters, row_offsets, n_inst, trk_inst, trk_hit_offset, trk_hits) -> Phase2Result:
+        """Merger + refit (orc_phase2) on ANY list of final tracks of this input: sector instance per track, CSR
+        offsets and kept hits (global cluster indices, rows increasing).  The GPU parity tests pass the GPU's own
+        S6 output here, so that phase 2 is compared on identical tracks at sizes where S5 near-ties flip."""
+        cl = np.ascontiguousarray(clusters, np.float32)
+        ro = np.ascontiguousarray(row_offsets, np.int32)
+        nt = len(trk_inst)
+        inst = np.ascontiguousarray(trk_inst, np.int32)
+        off = np.ascontiguousarray(trk_hit_offset, np.int64)
+        hits = np.ascontiguousarray(trk_hits, np.int32)
         seg_fit = np.zeros(max(nt, 1), FIT_DTYPE)
         m_fit = np.zeros(max(nt, 1), FIT_DTYPE)
         nxt = np.full(max(nt, 1), -1, np.int32)

@@ -35,15 +35,22 @@ SOURCES = {
 }
 
 
+# bench-only helpers (not part of the C ABI of include/tpc_tracker.h): libtpcbench.so, loaded by bench.py
+BENCH_SRC = os.path.join(HERE, "csrc_bench")
+BENCH_LIB = os.path.join(HERE, "libtpcbench.so")
+
+
 def _deps_mtime() -> float:
     paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+    paths += [os.path.join(BENCH_SRC, f) for f in os.listdir(BENCH_SRC)]
     paths.append(os.path.join(os.path.dirname(HERE), "include", "tpc_tracker.h"))
     paths.append(os.path.abspath(__file__))
     return max(os.path.getmtime(p) for p in paths)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _deps_mtime():
+    if (not force and os.path.exists(LIB) and os.path.exists(BENCH_LIB)
+            and min(os.path.getmtime(LIB), os.path.getmtime(BENCH_LIB)) >= _deps_mtime()):
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     objs = []
@@ -63,6 +70,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if r.returncode != 0:
         sys.stderr.write(log[-1])
         raise RuntimeError("link failed")
+    cmd = [NVCC, *ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-Wall", "-shared", "-o", BENCH_LIB,
+           *[os.path.join(BENCH_SRC, f) for f in sorted(os.listdir(BENCH_SRC)) if f.endswith(".cu")]]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    log.append("$ " + " ".join(cmd) + "\n" + r.stdout + r.stderr)
+    if r.returncode != 0:
+        sys.stderr.write(log[-1])
+        raise RuntimeError("nvcc failed on the bench-only library")
     with open(os.path.join(OBJ, "build.log"), "w") as f:
         f.write("\n".join(log))
     if verbose:

@@ -502,4 +502,36 @@ def test_full_bench_batch_sampled_instances_against_oracle():
     with open("gpurun_out/parity_report.jsonl", "a") as f:
         f.write(json.dumps(dict(case="cfg5_full_100_windows_sampled", n_clusters=N, instances=sample,
                                 worst_param_excess=worst, n_cand=n_cand, n_tracks=n_trk)) + "\n")
+    # ---- phase 2 at the size bench.py times it: tpc_merge_refit on all 1.39 M final tracks of this call, compared
+    # with the oracle on three sampled WINDOWS (36 instances each: links never leave a window).  The oracle's phase 2
+    # gets the GPU's own final tracks of the window, so S5 near-tie flips do not stand in the way.
+    from test_gpu_phase2 import _phase2_compare
+    p2bufs, p2o = trk.alloc_phase2(n_trk)
+    trk.merge_refit_device(p2o)
+    torch.cuda.synchronize(dev)
+    c2 = p2bufs["counts2"].cpu().numpy()
+    assert c2[0] == n_trk - c2[1] and c2[1] > 500_000
+    sec = bufs["trk_sector"][:n_trk].cpu().numpy()
+    hits = bufs["trk_hits"]
+    mfirst = p2bufs["mtrk_first"][:int(c2[0])].cpu().numpy()
+    for w in (0, 57, 99):
+        t0, t1 = (int(x) for x in np.searchsorted(sec, [36 * w, 36 * (w + 1)]))
+        lo, hi = int(batch.row_offsets[36 * w * R]), int(batch.row_offsets[36 * (w + 1) * R])
+        ro_w = (batch.row_offsets[36 * w * R:36 * (w + 1) * R + 1] - lo).astype(np.int32)
+        off_w = off[t0:t1 + 1] - off[t0]
+        hits_w = hits[int(off[t0]):int(off[t1])].cpu().numpy() - lo
+        q = Oracle.for_event(batch).phase2_on_tracks(batch.clusters[lo:hi], ro_w, 36, sec[t0:t1] - 36 * w, off_w, hits_w)
+        m0, m1 = (int(x) for x in np.searchsorted(mfirst, [t0, t1]))
+
+        def loc(name, a, b, shift=None):
+            v = p2bufs[name][a:b].cpu().numpy()
+            return np.where(v >= 0, v - shift, -1) if shift is not None else v
+        pw = {k: loc(k, t0, t1) for k in ("seg_ok", "seg_params", "seg_cov", "seg_chi2")}
+        pw.update(seg_next=loc("seg_next", t0, t1, t0), seg_prev=loc("seg_prev", t0, t1, t0))
+        pw.update({k: loc(k, m0, m1) for k in ("mtrk_nseg", "mtrk_nhits", "mtrk_ok", "mtrk_params", "mtrk_cov")})
+        pw["mtrk_first"] = loc("mtrk_first", m0, m1, t0)
+        assert pw["seg_next"].max() < t1 - t0  # a link never leaves its window
+        pw["counts2"] = np.array([m1 - m0, int((pw["seg_next"] >= 0).sum())])
+        rep = _phase2_compare(pw, q, t1 - t0, min_links=3000)
+        assert rep["chains_3plus_compared"] >= 1, rep
     trk.close()
