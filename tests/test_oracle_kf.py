@@ -250,11 +250,47 @@ def test_pulls_and_chi2_smeared_noise_free():
     assert len(pulls) >= 800
     # Means: y, sinPhi, q/pt are unbiased.  dz/ds carries a small second-order (extended-Kalman linearisation)
     # bias of ~ +0.1 sigma * sign(dz/ds), which the one-step back transport turns into ~ -0.13 sigma on z at the
-    # innermost hit (measured: it flips sign with eta and shrinks with a more diffuse prior; DESIGN.md "Readings",
-    # note on A8).  This sample has dz/ds > 0 throughout, so those two are allowed 0.2.
+    # innermost hit (it flips sign with eta: test_pulls_of_a_sample_symmetric_in_eta_are_unbiased below; DESIGN.md
+    # "Readings", note on A8).  This sample has dz/ds > 0 throughout, so those two are allowed 0.2.
     assert np.all(np.abs(pulls.mean(0)) < np.array([0.1, 0.2, 0.1, 0.2, 0.1])), pulls.mean(0)
     assert np.all(np.abs(pulls.std(0) - 1.0) < 0.1), pulls.std(0)
     assert abs(np.mean(chi2ndf) - 1.0) < 0.05
+
+
+def test_pulls_of_a_sample_symmetric_in_eta_are_unbiased():
+    """The companion of the one-sided sample above: with both signs of eta -- the z >= 0 sector instance
+    and its z < 0 partner -- the small bias on z and dz/ds changes sign with the side, so that the whole sample has all
+    five pull means within 0.1 (S8(c): 0 +- 0.1), while each side alone shows it."""
+    pulls, side = [], []
+    for seed in range(16):
+        rng = np.random.default_rng(100 + seed)
+        n = 80
+        trk = dict(pt=0.5 + rng.exponential(0.7, n), eta=rng.uniform(-0.9, 0.9, n),
+                   q=np.where(rng.uniform(size=n) < 0.5, -1.0, 1.0), phi0=rng.uniform(0.10, 0.25, n),
+                   x0=np.zeros(n), y0=np.zeros(n), z0=np.zeros(n))
+        ev = dg.from_tracks(trk, bz=BZ, sigma_y=0.1, sigma_z=0.1, seed=seed, single=False)
+        o = Oracle.for_event(ev)
+        r = o.track(ev.clusters, ev.row_offsets, ev.n_inst)
+        t64 = {k: np.asarray(v, float) for k, v in trk.items()}
+        for t in range(len(r.trk_cand)):
+            hits = r.trk_hits[r.trk_hit_offset[t]:r.trk_hit_offset[t + 1]]
+            tl = r.tracklets[r.trk_cand[t]]
+            lab = ev.labels[hits]
+            inst = int(np.searchsorted(ev.row_offsets[::ev.n_rows], hits[0], side="right")) - 1
+            if tl["nhits"] <= 100 or len(hits) != tl["nhits"] or not np.all(lab == lab[0]) or inst % 18 != 0:
+                continue
+            truth = dg.local_truth_state(t64, int(lab[0]), float(RX[tl["ref_row"]]), BZ, sector=0)
+            pulls.append((tl["p"] - truth) / np.sqrt(np.diag(unpack_cov(tl["cov"]))))
+            side.append(inst // 18)
+    pulls, side = np.array(pulls), np.array(side)
+    a, c = pulls[side == 0], pulls[side == 1]
+    assert len(a) >= 300 and len(c) >= 300
+    assert np.all(np.abs(pulls.mean(0)) < 0.1), pulls.mean(0)
+    assert np.all(np.abs(pulls.std(0) - 1.0) < 0.1), pulls.std(0)
+    # the bias itself: z and dz/ds, opposite on the two sides (dz/ds > 0 on the z >= 0 side, < 0 on the other)
+    assert a[:, 1].mean() < -0.05 and c[:, 1].mean() > 0.05, (a.mean(0), c.mean(0))
+    assert a[:, 3].mean() > 0.05 and c[:, 3].mean() < -0.05, (a.mean(0), c.mean(0))
+    assert np.all(np.abs(a.mean(0)) < 0.2) and np.all(np.abs(c.mean(0)) < 0.2)
 
 
 # ---------------------------------------------------------------- S6 selector on hand-made tracklets
