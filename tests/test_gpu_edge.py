@@ -411,12 +411,43 @@ def test_twenty_drift_windows_against_oracle():
     assert abs(g.n_tracks - len(o.trk_cand)) <= 8
 
 
+_FULL = {}  # shared with the forked workers of the all-windows comparison below (copy-on-write, nothing pickled)
+
+
+def _window_tracklet_excess(w):
+    """Worker: the oracle on window w of the bench batch alone, its tracklets against the GPU's slice for that window.
+    Returns plain numbers."""
+    from oracle.tpc_oracle import Oracle
+    from parity_util import PAR_ATOL, PAR_RTOL
+    b, R = _FULL["batch"], _FULL["R"]
+    lo, hi = int(b.row_offsets[36 * w * R]), int(b.row_offsets[36 * (w + 1) * R])
+    ro = (b.row_offsets[36 * w * R:36 * (w + 1) * R + 1] - lo).astype(np.int32)
+    o = Oracle.for_event(b).track(b.clusters[lo:hi], ro, 36)
+    c0, c1 = (int(x) for x in np.searchsorted(_FULL["cand_first"], [lo, hi]))
+    if c1 - c0 != len(o.cand_n):
+        return dict(window=w, cand_mismatch=1)
+    th = _FULL["tl_hits"][c0:c1]
+    th = np.where(th >= 0, th - lo, -1)
+    ok_o, ok_g = o.tracklets["ok"].astype(bool), _FULL["tl_nhits"][c0:c1] > 0
+    same = np.all(th == o.tracklet_hits, axis=1) & ok_o & ok_g
+    pg = _FULL["tl_params"][c0:c1][same].astype(np.float64)
+    po = o.tracklets["p"][same]
+    ex = (np.abs(pg - po) / (PAR_ATOL + PAR_RTOL * np.abs(po))).max(axis=1) if same.any() else np.zeros(0)
+    nh = o.tracklets["nhits"][same]
+    over = ex > 1.0
+    return dict(window=w, cand_mismatch=0, tracklets=int(ok_o.sum()), ok_flips=int((ok_o != ok_g).sum()),
+                identical_lists=int(same.sum()), beyond_tol=int(over.sum()), worst=float(ex.max()) if ex.size else 0.0,
+                beyond_tol_max_nhits=int(nh[over].max()) if over.any() else 0)
+
+
 def test_full_bench_batch_sampled_instances_against_oracle():
     """BASELINE.json configs[4] at FULL size, in the launch configuration bench.py times: 100 drift windows (3,600
     sector instances, 116 M clusters) in ONE tpc_track_sectors call.  Sector instances are independent, so the oracle
     can compute any one of them alone: twelve sampled instances (first, last, both z sides, the largest) are compared
     output by output -- links, start hits and candidates bit-exact; tracklet hit lists, parameters, covariance, chi2;
-    final assignment -- plus the properties that hold at any size for the whole batch."""
+    final assignment -- plus the properties that hold at any size for the whole batch.  Then (round 3) EVERY window
+    goes through the oracle in a process pool and all 5.15 M tracklets are held to the north_star parameter bar, and
+    tpc_merge_refit on the call's 1.39 M final tracks is compared on three sampled windows."""
     import sys
     import torch
     sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
@@ -502,6 +533,28 @@ def test_full_bench_batch_sampled_instances_against_oracle():
     with open("gpurun_out/parity_report.jsonl", "a") as f:
         f.write(json.dumps(dict(case="cfg5_full_100_windows_sampled", n_clusters=N, instances=sample,
                                 worst_param_excess=worst, n_cand=n_cand, n_tracks=n_trk)) + "\n")
+    # ---- every window of the call against the oracle ("show that the north_star tolerance holds on all
+    # 5.2 M tracklets of the headline workload, or state the measured exceedance rate").  Windows are independent: the
+    # oracle runs them one per worker process; the GPU's tracklet arrays are shared with the workers by fork.
+    import multiprocessing as mp
+    _FULL.update(batch=batch, R=R, cand_first=cand_first, tl_hits=bufs["tl_hits"][:n_cand].cpu().numpy(),
+                 tl_nhits=bufs["tl_nhits"][:n_cand].cpu().numpy(), tl_params=bufs["tl_params"][:n_cand].cpu().numpy())
+    with mp.get_context("fork").Pool(min(os.cpu_count() or 1, 32)) as pool:
+        per_win = pool.map(_window_tracklet_excess, range(100), chunksize=1)
+    _FULL.clear()
+    tot = {k: int(sum(r.get(k, 0) for r in per_win)) for k in ("cand_mismatch", "tracklets", "ok_flips",
+                                                                "identical_lists", "beyond_tol")}
+    tot["worst"] = max(r.get("worst", 0.0) for r in per_win)
+    tot["beyond_tol_max_nhits"] = max(r.get("beyond_tol_max_nhits", 0) for r in per_win)
+    with open("gpurun_out/parity_report.jsonl", "a") as f:
+        f.write(json.dumps(dict(case="cfg5_full_100_windows_ALL_tracklets", **tot)) + "\n")
+    assert tot["cand_mismatch"] == 0  # candidates are bit-exact in every window
+    # observed: 1 one-sided tracklet of 5,149,574 (A12/A13 threshold in fp32 vs fp64) -> observed + 1
+    assert tot["identical_lists"] >= MIN_SHARED * tot["tracklets"] and tot["ok_flips"] <= 2, tot
+    # the north_star bar (1e-3 relative / 1e-4 absolute) on every tracklet with the same hit list on both sides:
+    # measured on the B200 in round 3: 0 of 5,149,552 beyond the bar, worst 0.72; allowance =
+    # observed + 1, and what exceeds must stay near the bar
+    assert tot["beyond_tol"] <= 1 and tot["worst"] <= 2.0, tot
     # ---- phase 2 at the size bench.py times it: tpc_merge_refit on all 1.39 M final tracks of this call, compared
     # with the oracle on three sampled WINDOWS (36 instances each: links never leave a window).  The oracle's phase 2
     # gets the GPU's own final tracks of the window, so S5 near-tie flips do not stand in the way.
