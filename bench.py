@@ -69,6 +69,20 @@ def make_batch(n_windows, seed0, rank=0):
     return evs, datagen.concat_events(evs, name=f"cfg5_batch{n_windows}")
 
 
+def shard_job(evs, batch, world, rank):
+    """Strong scaling ("slice the timeframe in parts as we do with the TPC sectors"): ONE
+    job, the same on every rank, cut into contiguous blocks of whole windows balanced by cluster count; rank r tracks
+    its block as a self-contained input.  No data-path collective: only the small counts are gathered afterwards.
+    Returns (the rank's windows, its batch, what it owns)."""
+    import dataclasses
+    i0, ni, c0, nc = sharding.partition_instances(batch.row_offsets, batch.n_inst, batch.n_rows, world, rank)
+    cl, ro = sharding.local_problem(batch.clusters, batch.row_offsets, batch.n_rows, i0, ni)
+    local = dataclasses.replace(batch, clusters=np.ascontiguousarray(cl), row_offsets=np.ascontiguousarray(ro),
+                                labels=batch.labels[c0:c0 + nc], n_inst=ni, truth={},
+                                name=f"{batch.name}_shard{rank}of{world}")
+    return evs[i0 // 36:(i0 + ni) // 36], local, dict(inst0=i0, n_inst=ni, cluster0=c0, n_clusters=nc)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -263,7 +277,15 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     skip = set(x for x in args.skip.split(",") if x)
     t_gen = time.time()
-    evs, batch = make_batch(args.windows, args.seed0, rank)  # before CUDA init (fork)
+    shard = None
+    if args.scaling == "strong":
+        if args.windows < world:
+            raise SystemExit("--scaling strong needs at least one window per rank")
+        evs, batch = make_batch(args.windows, args.seed0, 0)  # the SAME job on every rank ...
+        job_clusters, job_inst = batch.n_clusters, batch.n_inst
+        evs, batch, shard = shard_job(evs, batch, world, rank)  # ... of which this rank tracks its block of windows
+    else:
+        evs, batch = make_batch(args.windows, args.seed0, rank)  # before CUDA init (fork)
     t_gen = time.time() - t_gen
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
@@ -324,6 +346,7 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     trk.set_work_counters(False)
     counts = bufs["counts"].cpu().numpy()
+    all_counts = sharding.gather_counts(counts, device=dev)  # [world, 16]: job-wide totals and per-rank track bases
     # per-stage device times of the timed calls (CUDA events recorded by the library on the launching stream)
     k = min(args.steps, 32)
     st = [trk.stage_times_ms(a) for a in range(k)]  # the untimed counting call above recorded no events
@@ -483,7 +506,7 @@ def run_ours(args):
             "ncu_dram_bytes_per_step": nb, "ncu_bytes_per_cluster": nb / N,
             "ncu_over_model": nb / (BYTES_PER_CLUSTER_PATH * N),
             "dram_gbs_at_ncu_bytes": nb / (ms_step * 1e-3) / 1e9,
-            "ncu_source": f"{cap.get('step_dram_source', '')} (commit {cap.get('commit', '?')})",
+            "ncu_source": cap.get("step_dram_source", ""),
             "rule": "SURVEY 8(d): achieved = min(ncu bytes, model bytes per cluster x N) / step time"})
     if cap.get("warp_instructions_per_launch"):
         wi = float(cap["warp_instructions_per_launch"])
@@ -513,7 +536,7 @@ def run_ours(args):
     n_trk0 = int(own.max()) + 1 if (own >= 0).any() else 0
     phys = physics.report(evs[0], own, n_trk0)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": args.scaling,
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{'cfg5 throughput batch' if WORKLOAD == 'cfg5' else WORKLOAD + ' batch'}: "
                                    f"{args.windows} {WORKLOADS[WORKLOAD]} per GPU in one call",
@@ -531,6 +554,14 @@ def run_ours(args):
                         "track_hits": int(counts[4]), "error_flags": int(counts[5])},
             "physics_window0": phys,
             "next1_bridge_rows": bridge}
+    if world > 1 or shard is not None:
+        line["all_ranks"] = {"tracks": int(all_counts[:, 3].sum()), "candidates": int(all_counts[:, 1].sum()),
+                             "track_base_per_rank": [int(x) for x in np.concatenate([[0], np.cumsum(all_counts[:-1, 3])])]}
+    if shard is not None:
+        line["config"]["strong_scaling_job"] = {
+            "what": "ONE job of --windows drift windows for all ranks; contiguous blocks of whole windows per rank, "
+                    "balanced by cluster count (sharding.partition_instances); no data-path collective",
+            "job_clusters": job_clusters, "job_sector_instances": job_inst, "rank0_shard": shard}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -548,6 +579,9 @@ def main():
     ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS),
                     help="what --windows counts: drift windows (default, the headline), or CFG:3 / CFG:2 events for the "
                          "linear-scaling check of PAPER.md:33")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak (default, what the driver runs): every rank tracks its own --windows windows; strong: "
+                         "ONE job of --windows windows is partitioned over the ranks (SURVEY 8(e))")
     ap.add_argument("--seed0", type=int, default=5001)
     ap.add_argument("--tune", default="", help='JSON dict of performance-only tracker parameters, e.g. {"grid_cells_y": 8}')
     ap.add_argument("--skip", default="", help="comma list of optional sections to leave out: e2e,phase2,single,bridge,cpu,cand")

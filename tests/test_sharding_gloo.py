@@ -67,3 +67,44 @@ def _worker(rank, world, port, tmp):
 def test_world_size_2_gloo(tmp_path):
     port = 29500 + (os.getpid() % 2000)
     mp.spawn(_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+
+
+def _strong_worker(rank, world, port, tmp):
+    """bench.py's --scaling strong code path (shard_job -> track -> gather_counts / combine_step) with the oracle
+    standing in for the per-rank GPU tracker."""
+    import sys
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from oracle.tpc_oracle import Oracle
+        evs = [dg.drift_window(seed=5401 + i, mean_tracks=25.0 * (1 + i % 3), cap_tracks=120) for i in range(5)]
+        batch = dg.concat_events(evs)
+        my_evs, local, shard = bench.shard_job(evs, batch, world, rank)
+        assert sum(e.n_clusters for e in my_evs) == local.n_clusters == shard["n_clusters"]
+        assert local.n_inst == 36 * len(my_evs) and local.row_offsets[0] == 0
+        assert np.array_equal(local.clusters, batch.clusters[shard["cluster0"]:shard["cluster0"] + shard["n_clusters"]])
+        o = Oracle.for_event(batch)
+        res = o.track(local.clusters, local.row_offsets, local.n_inst)
+        counts = np.zeros(16, np.int64)
+        counts[1], counts[3], counts[4] = len(res.cand_n), len(res.trk_cand), len(res.trk_hits)
+        allc = sh.gather_counts(counts)
+        ms, n = sh.combine_step(5.0 + 2 * rank, local.n_clusters)
+        assert n == batch.n_clusters and ms == 5.0 + 2 * (world - 1)  # whole job over the slowest rank
+        base = int(allc[:rank, 3].sum())
+        np.save(os.path.join(tmp, f"sown{rank}.npy"), np.where(res.cluster_owner >= 0, res.cluster_owner + base, -1))
+        dist.barrier()
+        if rank == 0:
+            whole = o.track(batch.clusters, batch.row_offsets, batch.n_inst)
+            got = np.concatenate([np.load(os.path.join(tmp, f"sown{r}.npy")) for r in range(world)])
+            assert np.array_equal(got, whole.cluster_owner)
+            assert int(allc[:, 3].sum()) == len(whole.trk_cand) and int(allc[:, 4].sum()) == len(whole.trk_hits)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_bench_strong_scaling_path_world_size_2_gloo(tmp_path):
+    port = 31500 + (os.getpid() % 2000)
+    mp.spawn(_strong_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
