@@ -393,11 +393,29 @@ chain_fit_kernel(const __grid_constant__ DevGeom g, const __grid_constant__ P2Ar
         while (a.p2_next[tail] >= 0 && nseg < 64) { tail = a.p2_next[tail]; nseg++; }
         KfState st = {};
         float x = 0.0f, yref = 0.0f, zref = 0.0f, chi2 = 0.0f;
-        int r_first = 0, r_last = 0, n = 0, nhits = 0;
+        int nhits = 0;
         int64_t cur = tail;
         HitWalk h = hit_walk(g, a, a.trk_cand[cur]);
-        bool ok = seed_outer(g, a, h, st, x, yref, zref, r_first, r_last, n);
-        if (ok) ok = filter_inward(g, a, h, st, x, yref, zref, chi2, nhits);
+        // The outermost segment is not fitted again: refit_tracks_kernel has just run exactly this seed + inward pass
+        // over its kept hits (reading M1 = the first leg of M4) and left the state at its innermost kept hit in
+        // p2_par / p2_cov / p2_chi2.  The state is taken back into the frame relative to that hit; what is lost is
+        // the rounding of y and z to fp32 when they were stored (<= 4e-6 cm at y ~ 100 cm).
+        const int4 tinfo = a.p2_info[tail];
+        bool ok = tinfo.x != 0;
+        if (ok) {
+            const float2 h0 = hit_at(a, h, tinfo.y);
+            const float* sp = a.p2_par + tail * 5;
+            const float* sc = a.p2_cov + tail * 15;
+            yref = h0.x;
+            zref = h0.y;
+            st.y = sp[0] - yref; st.z = sp[1] - zref; st.s = sp[2]; st.t = sp[3]; st.k = sp[4];
+            st.c00 = sc[0]; st.c10 = sc[1]; st.c11 = sc[2]; st.c20 = sc[3]; st.c21 = sc[4]; st.c22 = sc[5];
+            st.c30 = sc[6]; st.c31 = sc[7]; st.c32 = sc[8]; st.c33 = sc[9]; st.c40 = sc[10]; st.c41 = sc[11];
+            st.c42 = sc[12]; st.c43 = sc[13]; st.c44 = sc[14];
+            x = g.row_x[tinfo.y];
+            chi2 = a.p2_chi2[tail];
+            nhits = tinfo.w;
+        }
         while (ok && cur != t) {
             const int64_t inner = a.p2_prev[cur];
             const int sec_o = (track_inst(g, a, cur) + g.inst_phase) % g.spe_half;  // azimuth index (same side)
